@@ -1,0 +1,304 @@
+#!/usr/bin/env python
+"""Benchmark of the TCR-NET hot path on B200 (contract: see DESIGN.md section 8).
+
+A "step" is one pass of the whole hot path over one batch of synthetic input:
+A1 pack -> A2 schedule -> A3/A4 distances with early exit -> A5 emission -> A6 sort/CSR/degrees.
+Workload at N=1 GPU: BASELINE.json configs[3] ("cfg4": N = 800,000 CDR3-beta-shaped sequences,
+l_max = 1), the configuration the metric is quoted on.
+
+  value : N(N-1)/2 pairs decided per second, raw inputs already resident in HBM, device-timed.
+  e2e   : the same through the C ABI with HOST buffers (tcrnet_load H2D + build + tcrnet_copy_csr
+          D2H inside the timed region, wall clock between synchronisations).
+  roofline : the distance kernel against the INT32 ALU-pipe peak.
+  cpu_baseline : the oracle, as it stands, on this box's host cores, on a bounded sample.
+
+`--impl reference` times the oracle alone (rank 0 only).  N > 1: one process per GPU, each rank
+builds an independent repertoire of the same shape (replicas, no data-path collective): weak.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+WORKLOAD = "cfg4"
+ALU_LANES_PER_SM = 64          # INT32 ALU-pipe lanes per SM per clock on sm_100
+ALU_OPS_PER_COLUMN = 7         # LOP3 per pair and text column (distance.cu)
+ALU_OPS_PER_TEST = 4           # 2 LOP3 + IADD3 + ISETP per pair and early-exit test
+ORACLE_SAMPLE_ROWS = 64
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return json.load(open(p)), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows = []
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, reasons = [], [], set()
+        for t, line in self.rows:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                clk, mx = float(f[0]), float(f[1])
+            except ValueError:
+                continue
+            smax.append(mx)
+            if t0 <= t <= t1:
+                sm.append(clk)
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(d, l_max: int, rows: int, seed: int = 0):
+    """The oracle (tier 0: full Wagner-Fischer table, no pruning) on `rows` random rows against
+    every other row.  Returns (pairs/s, cells/s, threads, seconds, pairs)."""
+    import oracle
+    rng = np.random.default_rng(seed)
+    sample = np.sort(rng.choice(d.n, size=min(rows, d.n), replace=False))
+    t0 = time.perf_counter()
+    _, threads = oracle.edges(d.residues, d.lengths, l_max, rows=sample, all_partners=True, tier=0)
+    dt = time.perf_counter() - t0
+    pairs = int(sample.size) * (d.n - 1)
+    cells = float((d.lengths[sample].astype(np.int64) * (int(d.lengths.astype(np.int64).sum()))).sum()
+                  - (d.lengths[sample].astype(np.int64) ** 2).sum())
+    return pairs / dt, cells / dt, threads, dt, pairs
+
+
+def run_reference(args, rank: int) -> None:
+    if rank != 0:
+        return
+    from cdr3_synth import CONFIGS, generate
+    cfg = CONFIGS[WORKLOAD]
+    d = generate(cfg)
+    l_max = cfg.l_max[0]
+    for _ in range(args.warmup):
+        oracle_sample(d, l_max, 4)
+    times, pairs, threads = [], 0, 0
+    for k in range(args.steps):
+        pps, cps, threads, dt, pairs = oracle_sample(d, l_max, ORACLE_SAMPLE_ROWS, seed=k)
+        times.append(dt)
+    ms = 1e3 * float(np.mean(times))
+    value = pairs / (ms * 1e-3)
+    sample = f"{ORACLE_SAMPLE_ROWS} random rows x all {d.n - 1} partners per step ({pairs} pairs), tier-0 full table"
+    print(json.dumps({
+        "impl": "reference", "metric": "levenshtein_pairs_per_s", "value": value, "unit": "pairs/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+        "config": {"workload": f"{WORKLOAD}: N={cfg.n} synthetic CDR3b, l_max={l_max} (bounded sample per step)"},
+        "cpu_baseline": {"value": value, "unit": "pairs/s", "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "pairs/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default=WORKLOAD, help="cdr3_synth config name (bench line: cfg4)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--first-check", type=int, default=0)
+    ap.add_argument("--text-chunk", type=int, default=0)
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_2112_06613_b200 as pkg
+    from cdr3_synth import CONFIGS, generate
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = CONFIGS[args.workload]
+    l_max = cfg.l_max[0]
+    d = generate(cfg, seed=cfg.seed + 1000 * rank)  # replicas: an independent repertoire per rank
+    n = d.n
+    pairs_all = n * (n - 1) // 2
+
+    # raw inputs: pinned host copies (e2e) and device copies (value)
+    h_res = torch.from_numpy(d.residues).pin_memory()
+    h_len = torch.from_numpy(d.lengths).pin_memory()
+    d_res, d_len = h_res.cuda(non_blocking=True), h_len.cuda(non_blocking=True)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
+
+    net = pkg.TcrNet(local_rank)
+    if args.first_check:
+        net.set_option(pkg.OPT_FIRST_CHECK, args.first_check)
+    if args.text_chunk:
+        net.set_option(pkg.OPT_TEXT_CHUNK, args.text_chunk)
+
+    def step_device():
+        net.load(d_res, d_len)
+        return net.build(l_max)
+
+    def step_host():
+        net.load(h_res.numpy(), h_len.numpy())
+        net.build(l_max)
+        return net.copy_csr()
+
+    # work accounting pass (instrumented kernel, outside every timed region)
+    net.set_option(pkg.OPT_COUNT_WORK, 1)
+    step_device()
+    work = net.get_stats()
+    net.set_option(pkg.OPT_COUNT_WORK, 0)
+
+    for _ in range(max(args.warmup, 3) if args.warmup else 0):
+        step_device()
+
+    # ---- timed: K steps, device-resident inputs, CUDA events on the library's stream ----
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    stats = []
+    barrier()
+    t_wall0 = time.perf_counter()
+    for k in range(args.steps):
+        flush.fill_(k)  # L2 flush between timed iterations (not timed)
+        ev[k][0].record()
+        n_edges = step_device()
+        ev[k][1].record()
+        stats.append(net.get_stats())
+    barrier()
+    t_wall1 = time.perf_counter()
+    ms_steps = [a.elapsed_time(b) for a, b in ev]
+    ms_step = float(np.mean(ms_steps))
+    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
+
+    # ---- timed: end to end from host buffers through the C ABI ----
+    for _ in range(2):
+        step_host()
+    barrier()
+    e2e_times = []
+    for k in range(args.steps):
+        flush.fill_(k)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        rp, cl, dg = step_host()
+        torch.cuda.synchronize()
+        e2e_times.append(time.perf_counter() - t0)
+    barrier()
+    ms_e2e = 1e3 * float(np.mean(e2e_times))
+    h2d = int(d.residues.nbytes + d.lengths.nbytes)
+    d2h = int(rp.nbytes + cl.nbytes + dg.nbytes)
+
+    if world > 1:
+        t = torch.tensor([ms_step, ms_e2e], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_step, ms_e2e = float(t[0]), float(t[1])
+
+    if rank == 0:
+        peaks, peak_kind = _peaks()
+        n_sm = torch.cuda.get_device_properties(local_rank).multi_processor_count
+        ms_dist = float(np.mean([s["ms_distance"] for s in stats]))
+        ms_sort = float(np.mean([s["ms_sort"] for s in stats]))
+        ms_csr = float(np.mean([s["ms_csr"] for s in stats]))
+        ms_load = float(np.mean([s["ms_load"] for s in stats]))
+        alu_ops = ALU_OPS_PER_COLUMN * work["lane_columns_exec"] + ALU_OPS_PER_TEST * work["lane_tests_exec"]
+        achieved = alu_ops / (ms_dist * 1e-3) / 1e12
+        peak = n_sm * ALU_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12
+        probes = {}
+        for kind, name in ((0, "lop3"), (2, "imad"), (3, "lop3_imad_mix"), (5, "myers_step")):
+            ops, mhz = net.probe_int32(kind)
+            probes[name] = {"tera_per_s": ops / 1e12, "sm_mhz": mhz}
+        out = {
+            "metric": "levenshtein_pairs_per_s", "value": world * pairs_all / (ms_step * 1e-3), "unit": "pairs/s",
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "config": {
+                "workload": f"{args.workload}: N={n} synthetic CDR3b (BASELINE.json configs[{cfg.index - 1}]), l_max={l_max}",
+                "n": n, "l_max": l_max, "edges": int(n_edges), "l2": "flushed between timed steps (256 MiB write)",
+                "parallelism": "replicas" if world > 1 else "single GPU", "first_check": work["first_check"],
+            },
+            "clocks": clocks,
+            "e2e": {"value": world * pairs_all / (ms_e2e * 1e-3), "unit": "pairs/s", "ms_per_step": ms_e2e,
+                    "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+            "gpu_launches": int(sum(s["launches_load"] + s["launches_build"] for s in stats)),
+            "roofline": {
+                "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TIOP/s (INT32 ALU-pipe lane-ops)",
+                "frac": achieved / peak, "traffic": None, "kernel": "k_distance", "kernel_ms": ms_dist,
+                "peak_source": f"{n_sm} SMs x {ALU_LANES_PER_SM} lanes x {peaks['sm_max_mhz']} MHz ({peak_kind} sm_max_mhz)",
+                "alu_ops_per_launch": alu_ops, "measured_pipe_peaks": probes,
+            },
+            "detail": {
+                "pairs_kept": work["pairs_kept"], "cells_kept": work["cells_kept"], "cells_all": work["cells_all"],
+                "pairs_per_s_evaluated": work["pairs_kept"] / (ms_dist * 1e-3),
+                "gcups_evaluated": work["cells_kept"] / (ms_dist * 1e-3) / 1e9,
+                "gcups_effective": work["cells_all"] / (ms_step * 1e-3) / 1e9,
+                "columns_executed_fraction": work["lane_columns_exec"] / max(1, work["columns_kept"]),
+                "ms_pack": ms_load, "ms_distance": ms_dist, "ms_sort": ms_sort, "ms_csr": ms_csr,
+                "work_items": work["work_items"], "ms_steps": ms_steps,
+            },
+        }
+        if not args.no_cpu_baseline and world == 1:
+            pps, cps, threads, dt, pairs = oracle_sample(d, l_max, ORACLE_SAMPLE_ROWS)
+            out["cpu_baseline"] = {
+                "value": pps, "unit": "pairs/s", "cores": threads, "kind": "oracle", "gcups": cps / 1e9,
+                "sample": f"{ORACLE_SAMPLE_ROWS} random rows x all {n - 1} partners ({pairs} pairs, {dt:.1f} s), tier-0 full table",
+            }
+        print(json.dumps(out))
+    net.destroy()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

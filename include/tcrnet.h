@@ -1,0 +1,219 @@
+/*
+ * tcrnet.h - C ABI of the B200-native TCR-NET hot path.
+ *
+ * What the library computes (PAPER.md = /root/reference/PAPER.md, arXiv 2112.06613):
+ *
+ *   Input   N sequences s_0..s_{N-1} over the amino-acid alphabet (PAPER.md:209-213,
+ *           section II.F) and a threshold l_max in N_0.
+ *   Output  the TCR network of PAPER.md:297 (section II.M): one node per input row,
+ *           an undirected edge {i,j} "if and only if the Levenshtein distance l between
+ *           two CDR3b sequences does not exceed a threshold value l_max (thus l <= l_max)";
+ *           the Levenshtein distance is the unit-cost edit distance of PAPER.md:277-293
+ *           (section II.L, Eq. 15-16).  The edge set is returned as the strict upper
+ *           triangle of the adjacency matrix of PAPER.md:301-318 (section II.N, Eq. 17) in
+ *           CSR form - rows i ascending, inside a row the neighbours j > i ascending,
+ *           0-based - plus the node degrees d(u) = sum_v A_uv of PAPER.md:224 (section II.G).
+ *           The paper names this step "the computationally most expensive task"
+ *           (GPU design of the original: section II.O).
+ *
+ * The result is unique (no ties, no tolerance): it must equal, bit for bit, what the plain
+ * double loop over a Wagner-Fischer table yields.  Readings of the paper where it is silent or
+ * garbled (threshold is "<=", duplicates stay distinct nodes, no self loops, length limit 64)
+ * are listed in DESIGN.md section 3.
+ *
+ * Conventions for every call
+ *   - Return value: TCRNET_OK (0) or a negative tcrnet_status.  Nothing throws, aborts or
+ *     prints.  A failed call leaves the context usable (the previous load / build, if any,
+ *     may have been dropped: tcrnet_csr then returns TCRNET_ERR_STATE).
+ *   - A context is bound to one CUDA device and one stream; all device work is issued on that
+ *     stream.  A context is not thread-safe; different contexts are independent.
+ *   - "host" / "device" in a parameter comment says which address space the pointer is in.
+ *   - There is no CPU fallback: without a CUDA device tcrnet_create fails with TCRNET_ERR_CUDA.
+ */
+#ifndef TCRNET_H_
+#define TCRNET_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define TCRNET_API __attribute__((visibility("default")))
+#else
+#define TCRNET_API
+#endif
+
+#define TCRNET_VERSION 100 /* 1.0.0 */
+#define TCRNET_MAX_LEN 64  /* one machine word per sequence (BASELINE.json north_star) */
+
+typedef enum tcrnet_status {
+    TCRNET_OK = 0,
+    TCRNET_ERR_ARG = -1,           /* NULL pointer, n < 1, unknown option, ...                 */
+    TCRNET_ERR_LENGTH = -2,        /* a sequence length is 0 or > TCRNET_MAX_LEN               */
+    TCRNET_ERR_RESIDUE = -3,       /* a residue byte is outside 'A'..'Z'                       */
+    TCRNET_ERR_LMAX = -4,          /* l_max outside 0..TCRNET_MAX_LEN                          */
+    TCRNET_ERR_STATE = -5,         /* build before load, csr/degrees before build              */
+    TCRNET_ERR_NOMEM = -6,         /* the allocator returned NULL / cudaMalloc failed          */
+    TCRNET_ERR_EDGE_OVERFLOW = -7, /* more edges than the configured hard limit                */
+    TCRNET_ERR_CUDA = -8           /* any other CUDA runtime error (see tcrnet_last_cuda_error)*/
+} tcrnet_status;
+
+typedef struct tcrnet_ctx tcrnet_ctx; /* opaque */
+
+/*
+ * Device-memory allocator supplied by the caller (the Python binding backs it with
+ * torch.empty(..., device="cuda"), so PyTorch's caching allocator owns every byte).
+ * alloc returns a device pointer aligned to >= 256 bytes, or NULL; free releases it.
+ * Both are called from the thread that calls into the library, never from a kernel.
+ * Pass NULL to tcrnet_create to let the library use cudaMalloc / cudaFree.
+ */
+typedef struct tcrnet_allocator {
+    void* (*alloc)(void* user, size_t bytes);
+    void (*free)(void* user, void* ptr);
+    void* user;
+} tcrnet_allocator;
+
+/* Options for tcrnet_set_option (all optional; defaults in parentheses). */
+typedef enum tcrnet_option {
+    TCRNET_OPT_EARLY_EXIT = 1,    /* 1: exact banded early exit on (default), 0: every column of
+                                     every kept pair is computed.  Never changes the result
+                                     (PAPER.md:326 describes the abort as a time saver only). */
+    TCRNET_OPT_FIRST_CHECK = 2,   /* text columns processed before the first early-exit test;
+                                     0 = automatic (l_max + 4, clamped to 3..8)               */
+    TCRNET_OPT_EDGE_CAPACITY = 3, /* initial capacity of the edge buffer in edges; 0 = automatic
+                                     (max(1 Mi, 16 N)).  The buffer grows to the exact count
+                                     and the distance pass is re-run if it was too small.      */
+    TCRNET_OPT_EDGE_LIMIT = 4,    /* hard limit in edges (default and maximum 2^31): beyond it
+                                     tcrnet_build fails with TCRNET_ERR_EDGE_OVERFLOW          */
+    TCRNET_OPT_COUNT_WORK = 5,    /* 1: the distance kernel also counts executed columns and
+                                     tests (slower, for roofline accounting); default 0        */
+    TCRNET_OPT_TEXT_CHUNK = 6     /* texts per work item (multiple of 256; default 2048)       */
+} tcrnet_option;
+
+/* Work and timing of the last tcrnet_load / tcrnet_build (tcrnet_get_stats). */
+typedef struct tcrnet_stats {
+    int64_t n;                 /* sequences loaded                                            */
+    int64_t total_len;         /* residues loaded                                             */
+    int32_t min_len, max_len;  /* shortest / longest sequence                                 */
+    int32_t l_max;             /* threshold of the last build                                 */
+    int32_t first_check;       /* columns before the first early-exit test (0: early exit off)*/
+    int64_t n_edges;           /* |E|                                                         */
+    int64_t pairs_all;         /* N(N-1)/2                                                    */
+    int64_t pairs_kept;        /* pairs with |len_i - len_j| <= l_max (the ones evaluated)    */
+    int64_t cells_all;         /* sum over all pairs of len_i * len_j (DP cells, nominal)     */
+    int64_t cells_kept;        /* same over the kept pairs                                    */
+    int64_t columns_kept;      /* sum over kept pairs of the text length (nominal columns)    */
+    int64_t lane_columns_exec; /* 32 x warp-level column steps executed  (COUNT_WORK only)    */
+    int64_t lane_tests_exec;   /* 32 x warp-level early-exit tests executed (COUNT_WORK only) */
+    int64_t lane_pairs_exec;   /* 32 x warp-level (pattern-warp, text) visits (COUNT_WORK only)*/
+    int64_t work_items;        /* CTAs of the distance kernel                                 */
+    int32_t distance_passes;   /* 1, or 2 if the edge buffer had to grow                      */
+    int32_t launches_load;     /* kernels launched by the last tcrnet_load[_device]           */
+    int32_t launches_build;    /* kernels launched by the last tcrnet_build                   */
+    float ms_load;             /* device time of the last load (H2D copy + pack), CUDA events */
+    float ms_distance;         /* distance kernel(s) incl. emission                           */
+    float ms_sort;             /* radix sort of the edge keys                                 */
+    float ms_csr;              /* row_ptr / col / degrees                                     */
+    float ms_build;            /* whole tcrnet_build on the device                            */
+} tcrnet_stats;
+
+/*
+ * Create a context on CUDA device `device` that issues all work on `cuda_stream`
+ * (a cudaStream_t passed as void*; NULL = the legacy default stream).
+ * `allocator` may be NULL (see above); the struct is copied.
+ * Errors: TCRNET_ERR_ARG (out == NULL), TCRNET_ERR_CUDA (no such device / no driver),
+ * TCRNET_ERR_NOMEM.
+ */
+TCRNET_API int tcrnet_create(tcrnet_ctx** out, int device, void* cuda_stream, const tcrnet_allocator* allocator);
+
+/* Release every buffer the context owns and the context itself.  NULL is allowed. */
+TCRNET_API void tcrnet_destroy(tcrnet_ctx* ctx);
+
+/*
+ * Step A1 (pack): take N sequences, validate them, copy them to the device and lay them out
+ * for the distance kernel (5-bit residue codes, stable sort by (length, row), length buckets,
+ * permutation).  PAPER.md:326 ("each a.a. is saved as a number ... BYTE"), north_star (1).
+ *
+ *   residues  host, uint8[sum(lengths)]: the rows concatenated, ASCII 'A'..'Z' (any of the 26
+ *             letters is a legal residue; only equality matters - DESIGN.md reading Q8)
+ *   lengths   host, int32[n], each in 1..TCRNET_MAX_LEN
+ *   n         1 .. 2^31-2
+ *
+ * Both arrays are borrowed for the duration of the call only.  Node ids of the output are the
+ * caller's row indices 0..n-1; the internal sort is invisible.  Replaces any previous load and
+ * drops any previous build.  Synchronises the stream.
+ * Errors: ARG, LENGTH, RESIDUE, NOMEM, CUDA.
+ */
+TCRNET_API int tcrnet_load(tcrnet_ctx* ctx, const uint8_t* residues, const int32_t* lengths, int64_t n);
+
+/*
+ * Same as tcrnet_load with both arrays already in device memory (ordered on the context's
+ * stream).  total_len must equal sum(lengths); it sizes the residue array.
+ * The arrays are borrowed for the duration of the call only (they are re-laid out into
+ * buffers the context owns).
+ */
+TCRNET_API int tcrnet_load_device(tcrnet_ctx* ctx, const uint8_t* residues_dev, const int32_t* lengths_dev, int64_t n,
+                       int64_t total_len);
+
+/*
+ * Steps A2-A6: enumerate the length-compatible pairs (|len_i - len_j| <= l_max, each unordered
+ * pair once), compute every such pair's Levenshtein distance (bit-parallel, exact), keep the
+ * pairs with distance <= l_max, and assemble CSR + degrees on the device
+ * (PAPER.md:301-318, 224).  l_max in 0..TCRNET_MAX_LEN.  May be called repeatedly on one load.
+ * *n_edges_out (host, may be NULL) receives |E|.  Synchronises the stream.
+ * Errors: STATE (no load), LMAX, NOMEM, EDGE_OVERFLOW, CUDA.
+ */
+TCRNET_API int tcrnet_build(tcrnet_ctx* ctx, int l_max, int64_t* n_edges_out);
+
+/*
+ * Borrow the CSR of the last build: *row_ptr_dev -> device int64[n+1], *col_dev -> device
+ * int32[|E|] (NULL when |E| = 0).  Row i lists the neighbours j > i in ascending order;
+ * row_ptr[n] = |E|.  Owned by the context, valid until the next tcrnet_build / tcrnet_load /
+ * tcrnet_destroy.  Either out pointer may be NULL.  Errors: ARG, STATE.
+ */
+TCRNET_API int tcrnet_csr(tcrnet_ctx* ctx, const int64_t** row_ptr_dev, const int32_t** col_dev);
+
+/*
+ * Borrow the degrees of the last build: *deg_dev -> device int32[n]; deg[u] counts both
+ * directions (sum(deg) = 2|E|).  Same lifetime as tcrnet_csr.
+ */
+TCRNET_API int tcrnet_degrees(tcrnet_ctx* ctx, const int32_t** deg_dev);
+
+/*
+ * Copy the last build to host buffers (any may be NULL to skip it): row_ptr_host int64[n+1],
+ * col_host int32[|E|], deg_host int32[n].  Synchronises the stream.  Errors: STATE, CUDA.
+ */
+TCRNET_API int tcrnet_copy_csr(tcrnet_ctx* ctx, int64_t* row_ptr_host, int32_t* col_host, int32_t* deg_host);
+
+/* Set a tcrnet_option.  Takes effect at the next tcrnet_build.  Errors: ARG. */
+TCRNET_API int tcrnet_set_option(tcrnet_ctx* ctx, int option, int64_t value);
+
+/* Fill *out (host) with the work / timing record described above.  Errors: ARG. */
+TCRNET_API int tcrnet_get_stats(tcrnet_ctx* ctx, tcrnet_stats* out);
+
+/*
+ * Measurement aid for the roofline denominator: run a dependent-chain-
+ * free microkernel of one instruction class on every SM and report thread-level operations
+ * per second.  kind: 0 = LOP3 (ALU pipe), 1 = IADD3 (ALU pipe), 2 = IMAD (FMA pipe),
+ * 3 = LOP3 and IMAD interleaved 1:1, 4 = POPC, 5 = the Myers column step itself on registers
+ * (reports column steps per second).  *ops_per_s and *sm_clock_mhz (observed, from
+ * clock64 / event time) are host pointers.  Errors: ARG, CUDA.
+ */
+TCRNET_API int tcrnet_probe_int32(tcrnet_ctx* ctx, int kind, double* ops_per_s, double* sm_clock_mhz);
+
+/* Last cudaError_t seen by this context (0 if none), for diagnostics. */
+TCRNET_API int tcrnet_last_cuda_error(tcrnet_ctx* ctx);
+
+/* Static string for a tcrnet_status. */
+TCRNET_API const char* tcrnet_strerror(int status);
+
+/* TCRNET_VERSION the library was built with. */
+TCRNET_API int tcrnet_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TCRNET_H_ */

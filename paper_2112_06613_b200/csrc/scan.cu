@@ -1,0 +1,144 @@
+// Device-wide exclusive prefix sums (used for row offsets, split histograms).
+// Three launches: per-tile sums -> scan of the tile sums by one CTA -> per-tile scan + offset.
+// HBM-bound streaming passes: 2 reads + 1 write of the array.
+#include "tcrnet_internal.h"
+
+namespace tcrnet {
+namespace {
+
+constexpr int kScanThreads = 256;
+constexpr int kScanItems = 16;
+constexpr int kScanTile = kScanThreads * kScanItems;  // 4096
+
+template <typename T>
+__device__ __forceinline__ T warp_inclusive(T v) {
+    const int lane = threadIdx.x & 31;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        T o = __shfl_up_sync(0xffffffffu, v, d);
+        if (lane >= d) v += o;
+    }
+    return v;
+}
+
+// Exclusive scan of one value per thread across the CTA; *total gets the CTA sum.
+template <typename T>
+__device__ __forceinline__ T block_exclusive(T v, T* warp_sums /*[32]*/, T* total) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    T inc = warp_inclusive(v);
+    if (lane == 31) warp_sums[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        T w = lane < nwarp ? warp_sums[lane] : T(0);
+        T wi = warp_inclusive(w);
+        warp_sums[lane] = wi - w;  // exclusive
+        if (lane == 31) *total = wi;
+    }
+    __syncthreads();
+    T r = warp_sums[warp] + inc - v;
+    __syncthreads();
+    return r;
+}
+
+template <typename TIn, typename TOut>
+__global__ void __launch_bounds__(kScanThreads) k_tile_sums(const TIn* __restrict__ in, int64_t n,
+                                                           TOut* __restrict__ tile_sums) {
+    __shared__ TOut ws[32];
+    __shared__ TOut tot;
+    const int64_t base = (int64_t)blockIdx.x * kScanTile;
+    TOut acc = 0;
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        int64_t i = base + (int64_t)k * kScanThreads + threadIdx.x;  // coalesced
+        if (i < n) acc += (TOut)in[i];
+    }
+    block_exclusive(acc, ws, &tot);
+    if (threadIdx.x == 0) tile_sums[blockIdx.x] = tot;
+}
+
+// One CTA scans the tile sums in place (exclusive), chunk by chunk with a carry.
+template <typename TOut>
+__global__ void __launch_bounds__(1024) k_scan_tile_sums(TOut* __restrict__ tile_sums, int64_t n_tiles) {
+    __shared__ TOut ws[32];
+    __shared__ TOut tot;
+    TOut carry = 0;
+    for (int64_t c = 0; c < n_tiles; c += 1024) {
+        int64_t i = c + threadIdx.x;
+        TOut v = i < n_tiles ? tile_sums[i] : TOut(0);
+        TOut ex = block_exclusive(v, ws, &tot);
+        if (i < n_tiles) tile_sums[i] = carry + ex;
+        carry += tot;
+        __syncthreads();
+    }
+}
+
+template <typename TIn, typename TOut>
+__global__ void __launch_bounds__(kScanThreads) k_tile_scan(const TIn* __restrict__ in, TOut* __restrict__ out,
+                                                           int64_t n, const TOut* __restrict__ tile_sums,
+                                                           int write_total) {
+    __shared__ TOut ws[32];
+    __shared__ TOut tot;
+    __shared__ TOut stage[kScanTile];
+    const int64_t base = (int64_t)blockIdx.x * kScanTile;
+    // coalesced load into shared memory, then each thread owns kScanItems consecutive items
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        int idx = k * kScanThreads + threadIdx.x;
+        int64_t i = base + idx;
+        stage[idx] = i < n ? (TOut)in[i] : TOut(0);
+    }
+    __syncthreads();
+    TOut local[kScanItems];
+    TOut acc = 0;
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        local[k] = acc;
+        acc += stage[threadIdx.x * kScanItems + k];
+    }
+    TOut ex = block_exclusive(acc, ws, &tot) + tile_sums[blockIdx.x];
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) stage[threadIdx.x * kScanItems + k] = local[k] + ex;
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        int idx = k * kScanThreads + threadIdx.x;
+        int64_t i = base + idx;
+        if (i < n) out[i] = stage[idx];
+    }
+    if (write_total && blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) out[n] = tile_sums[blockIdx.x] + tot;
+}
+
+template <typename TIn, typename TOut>
+cudaError_t scan_impl(const TIn* in, TOut* out, int64_t n, bool write_total, void* scratch, cudaStream_t s,
+                      int* launches) {
+    if (n <= 0) {
+        if (write_total) return cudaMemsetAsync(out, 0, sizeof(TOut), s);
+        return cudaSuccess;
+    }
+    const int64_t tiles = (n + kScanTile - 1) / kScanTile;
+    TOut* sums = static_cast<TOut*>(scratch);
+    k_tile_sums<TIn, TOut><<<(unsigned)tiles, kScanThreads, 0, s>>>(in, n, sums);
+    k_scan_tile_sums<TOut><<<1, 1024, 0, s>>>(sums, tiles);
+    k_tile_scan<TIn, TOut><<<(unsigned)tiles, kScanThreads, 0, s>>>(in, out, n, sums, write_total ? 1 : 0);
+    *launches += 3;
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+size_t scan_scratch_bytes(int64_t n) {
+    int64_t tiles = (n + kScanTile - 1) / kScanTile;
+    return (size_t)(tiles > 0 ? tiles : 1) * sizeof(int64_t);
+}
+
+cudaError_t exclusive_scan_i32_to_i64(const int32_t* in, int64_t* out, int64_t n, bool write_total, void* scratch,
+                                      cudaStream_t s, int* launches) {
+    return scan_impl<int32_t, int64_t>(in, out, n, write_total, scratch, s, launches);
+}
+
+cudaError_t exclusive_scan_u32(const uint32_t* in, uint32_t* out, int64_t n, void* scratch, cudaStream_t s,
+                               int* launches) {
+    return scan_impl<uint32_t, uint32_t>(in, out, n, false, scratch, s, launches);
+}
+
+}  // namespace tcrnet

@@ -1,0 +1,100 @@
+// Internal declarations shared by the translation units of libtcrnet_b200.so.
+// Nothing here is part of the C ABI (include/tcrnet.h) and nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "tcrnet.h"
+
+namespace tcrnet {
+
+constexpr int kMaxLen = TCRNET_MAX_LEN;  // one machine word per sequence
+constexpr int kNumLen = kMaxLen + 1;     // length buckets, indexed by length 0..64
+constexpr int kNumCodes = 26;            // residue code = byte - 'A'
+constexpr int kPadCode = 26;             // text padding: selects an all-zero Peq row
+constexpr int kPeqRows = 27;             // 26 residue rows + the zero row
+constexpr int kTQ = 256;                 // patterns per CTA of the distance kernel (8 warps)
+constexpr int kTT = 64;                  // texts staged into shared memory per pipeline stage
+
+// Per-length layout of the packed sequence tables (filled on the host after the histogram).
+struct LengthTable {
+    int32_t start[kNumLen + 1];    // first sorted position of each length bucket (+ end sentinel)
+    int64_t txt_base[kNumLen + 1]; // first 32-bit word of the bucket's text rows in `txt`
+    int32_t row_words[kNumLen];    // words per text row = round_up(len, 4)
+};
+
+// One (pattern bucket, text bucket) pair of the tile scheduler (step A2).
+struct WorkRow {
+    int64_t item_begin;  // first work item (CTA) of this row
+    int64_t txt_base;    // first word of the text bucket's rows
+    int32_t p_start;     // sorted position of the first pattern (the shorter-or-equal length)
+    int32_t p_count;
+    int32_t t_start;     // sorted position of the first text
+    int32_t t_count;
+    int32_t m;           // pattern length
+    int32_t n;           // text length, m <= n <= m + l_max
+    int32_t row_words;   // words per text row
+    int32_t n_tchunks;   // text chunks per pattern tile
+    int32_t diag;        // 1: same bucket, only sorted p < t counts
+    int32_t pad_;
+};
+
+struct DistanceParams {
+    const WorkRow* rows;
+    int32_t n_rows;
+    int32_t l_max;
+    int32_t tchunk;      // texts per work item
+    int32_t pat_stride;  // bytes per pattern row
+    const uint32_t* txt; // text rows: one 32-bit residue code per column, padded with kPadCode
+    const uint8_t* pat;  // pattern rows: one residue code per byte, row = sorted position
+    const int32_t* perm; // sorted position -> caller's row index
+    unsigned long long* edges;       // keys (min(i,j) << 32) | max(i,j)
+    unsigned long long* edge_count;  // device counter (keeps counting beyond capacity)
+    unsigned long long edge_cap;
+    unsigned long long* work;        // [3]: lane-columns, lane-tests, lane-visits (COUNT only)
+};
+
+// ---- launch wrappers (each returns cudaGetLastError(); *launches is incremented per kernel) ----
+
+// scan.cu: out[i] = sum_{k<i} in[k] for i in 0..n (n+1 outputs when write_total).
+// scratch must hold scan_scratch_bytes(n).
+size_t scan_scratch_bytes(int64_t n);
+cudaError_t exclusive_scan_i32_to_i64(const int32_t* in, int64_t* out, int64_t n, bool write_total,
+                                      void* scratch, cudaStream_t s, int* launches);
+cudaError_t exclusive_scan_u32(const uint32_t* in, uint32_t* out, int64_t n, void* scratch,
+                               cudaStream_t s, int* launches);
+
+// split.cu: one stable counting-sort pass over 8-bit digits.
+int64_t split_num_blocks(int64_t n);
+// lengths -> perm (sorted by (clamped length, row)); hist_scratch uint32[256*blocks] x2.
+cudaError_t split_by_length(const int32_t* lengths, int64_t n, int32_t* perm_out, uint32_t* hist,
+                            uint32_t* hist_scanned, void* scan_scratch, cudaStream_t s, int* launches);
+// one radix pass on 64-bit keys, digit = (key >> shift) & 255.
+cudaError_t split_keys_u64(const unsigned long long* in, unsigned long long* out, int64_t n, int shift,
+                           uint32_t* hist, uint32_t* hist_scanned, void* scan_scratch, cudaStream_t s,
+                           int* launches);
+
+// pack.cu
+cudaError_t launch_length_hist(const int32_t* lengths, int64_t n, unsigned long long* hist /*[kNumLen]*/,
+                               uint32_t* flags, cudaStream_t s, int* launches);
+cudaError_t launch_pack(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths,
+                        const int32_t* perm, int64_t n, const LengthTable& lt, int pat_stride,
+                        uint8_t* pat, uint32_t* txt, uint32_t* flags, cudaStream_t s, int* launches);
+
+// distance.cu
+size_t distance_smem_bytes(bool wide, int max_row_words);
+cudaError_t launch_distance(const DistanceParams& p, int64_t n_items, bool wide, int first_check,
+                            bool count_work, int max_row_words, cudaStream_t s, int* launches);
+
+// csr.cu
+cudaError_t launch_csr(const unsigned long long* sorted_keys, int64_t n_edges, int64_t n, int64_t* row_ptr,
+                       int32_t* col, int32_t* deg, cudaStream_t s, int* launches);
+
+// probe.cu
+cudaError_t launch_probe(int kind, int n_sm, unsigned long long* out /*[2]: ops, cycles*/, float* ms,
+                         cudaStream_t s);
+
+enum : uint32_t { kFlagBadLength = 1u, kFlagBadResidue = 2u };
+
+}  // namespace tcrnet

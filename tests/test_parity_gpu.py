@@ -1,0 +1,294 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Bar: bit-exact (integer / index work; the result is unique).  Small configs are compared in
+full; BASELINE.json's large configs are compared on sampled nodes' full neighbourhoods that
+the oracle computes one by one, plus properties that hold at any size.
+"""
+import itertools
+
+import numpy as np
+import pytest
+
+from cdr3_synth import generate
+from cdr3_synth.generator import from_strings
+from helpers import (assert_same_network, check_csr_invariants, neighbours_from_csr, neighbours_from_pairs)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    import paper_2112_06613_b200 as p
+    return p
+
+
+@pytest.fixture(scope="module")
+def oracle():
+    import oracle as o
+    return o
+
+
+def gpu_network(pkg, residues, lengths, l_max, **opts):
+    with pkg.TcrNet(0) as net:
+        for k, v in opts.items():
+            net.set_option(k, v)
+        net.load(residues, lengths)
+        net.build(l_max)
+        out = net.copy_csr()
+        out_stats = net.get_stats()
+    return out, out_stats
+
+
+# ------------------------------------------------------------------ full comparisons
+@pytest.mark.parametrize("l_max", [0, 1, 2, 3, 5])
+def test_cfg1_full(pkg, oracle, l_max):
+    d = generate("cfg1")
+    got, st = gpu_network(pkg, d.residues, d.lengths, l_max)
+    want = oracle.network(d.residues, d.lengths, l_max, tier=0)[:3]
+    assert_same_network(got, want)
+    check_csr_invariants(*got, d.n)
+    assert st["pairs_all"] == d.n * (d.n - 1) // 2 and st["launches_build"] > 0
+
+
+@pytest.mark.parametrize("l_max,tier", [(1, 1), (2, 0)])
+def test_cfg2_full(pkg, oracle, l_max, tier):
+    """N = 50,000: several hundred tiles, ragged tails in every bucket."""
+    d = generate("cfg2")
+    got, st = gpu_network(pkg, d.residues, d.lengths, l_max)
+    want = oracle.network(d.residues, d.lengths, l_max, tier=tier)[:3]
+    assert_same_network(got, want)
+    check_csr_invariants(*got, d.n)
+
+
+def test_early_exit_and_schedule_do_not_change_the_result(pkg):
+    """the abort only saves time.  Every test position, early exit off, small
+    text chunks and a tiny edge buffer (forces the second distance pass) give the same bytes."""
+    d = generate("cfg2", n=20000)
+    for l_max in (1, 3):
+        ref, st0 = gpu_network(pkg, d.residues, d.lengths, l_max, **{pkg.OPT_EARLY_EXIT: 0})
+        assert st0["first_check"] == 0
+        for fc in range(3, 9):
+            got, st = gpu_network(pkg, d.residues, d.lengths, l_max, **{pkg.OPT_FIRST_CHECK: fc})
+            assert st["first_check"] == fc
+            assert_same_network(got, ref)
+        got, st = gpu_network(pkg, d.residues, d.lengths, l_max, **{pkg.OPT_TEXT_CHUNK: 256, pkg.OPT_EDGE_CAPACITY: 100})
+        assert st["distance_passes"] == 2
+        assert_same_network(got, ref)
+        got, st = gpu_network(pkg, d.residues, d.lengths, l_max, **{pkg.OPT_COUNT_WORK: 1})
+        assert_same_network(got, ref)
+        assert 0 < st["lane_columns_exec"] and st["lane_pairs_exec"] >= st["pairs_kept"]
+
+
+def test_device_load_equals_host_load(pkg):
+    import torch
+    d = generate("cfg1")
+    ref, _ = gpu_network(pkg, d.residues, d.lengths, 2)
+    with pkg.TcrNet(0) as net:
+        net.load(torch.from_numpy(d.residues).cuda(), torch.from_numpy(d.lengths).cuda())
+        net.build(2)
+        rp, cl = net.csr()
+        dg = net.degrees()
+        got = (rp.cpu().numpy(), cl.cpu().numpy(), dg.cpu().numpy())
+        assert_same_network(got, ref)
+        # repeated builds on one load, different thresholds
+        e1 = net.build(1)
+        e3 = net.build(3)
+        assert e1 <= int(ref[0][-1]) <= e3
+
+
+# ------------------------------------------------------------------ edge cases
+def test_single_and_pair(pkg):
+    got, _ = gpu_network(pkg, *from_strings(["CASSF"]), 3)
+    assert got[0].tolist() == [0, 0] and got[1].size == 0 and got[2].tolist() == [0]
+    got, _ = gpu_network(pkg, *from_strings(["CASSF", "CASSF"]), 0)
+    assert got[0].tolist() == [0, 1, 1] and got[1].tolist() == [1] and got[2].tolist() == [1, 1]
+    got, _ = gpu_network(pkg, *from_strings(["CASSF", "CASTF"]), 0)
+    assert got[1].size == 0
+    got, _ = gpu_network(pkg, *from_strings(["CASSF", "CASTF"]), 1)
+    assert got[1].tolist() == [1]
+
+
+def test_paper_five_node_example(pkg):
+    """PAPER.md:305-318 realised by strings at l_max = 1 (see tests/golden/paper_adjacency_example.txt)."""
+    got, _ = gpu_network(pkg, *from_strings(["AAAA", "AAAB", "AACA", "AEDB", "AADB"]), 1)
+    assert got[0].tolist() == [0, 2, 3, 3, 4, 4] and got[1].tolist() == [1, 2, 4, 4] and got[2].tolist() == [2, 2, 1, 1, 2]
+
+
+def test_all_duplicates_complete_graph(pkg, oracle):
+    """Reading Q3: r copies -> K_r for every l_max; r chosen to leave ragged warps and tiles."""
+    r = 777
+    res, ln = from_strings(["CASSLGQGNTEAFF"] * r)
+    for l_max in (0, 2):
+        got, _ = gpu_network(pkg, res, ln, l_max)
+        assert int(got[0][-1]) == r * (r - 1) // 2
+        assert (got[2] == r - 1).all()
+        check_csr_invariants(*got, r)
+
+
+def test_lmax_at_least_max_length_gives_complete_graph(pkg, oracle):
+    d = generate("cfg1", n=300)
+    got, _ = gpu_network(pkg, d.residues, d.lengths, 25)
+    assert int(got[0][-1]) == 300 * 299 // 2
+    got, _ = gpu_network(pkg, d.residues, d.lengths, 64)
+    assert int(got[0][-1]) == 300 * 299 // 2
+
+
+def test_all_lengths_1_to_64_incl_wide_words(pkg, oracle):
+    """Lengths 1..64 (patterns > 32 take the 64-bit kernel), tiny alphabet so that edges exist,
+    several thresholds incl. ones larger than the first-test column."""
+    rng = np.random.default_rng(11)
+    strings = []
+    for length in range(1, 65):
+        base = "".join("ACD"[i] for i in rng.integers(0, 3, length))
+        strings.append(base)
+        for _ in range(6):
+            s = list(base)
+            for _ in range(int(rng.integers(0, 4))):
+                k = int(rng.integers(0, 3))
+                p = int(rng.integers(0, len(s)))
+                if k == 0:
+                    s[p] = "ACD"[int(rng.integers(0, 3))]
+                elif k == 1 and len(s) < 64:
+                    s.insert(p, "ACD"[int(rng.integers(0, 3))])
+                elif k == 2 and len(s) > 1:
+                    del s[p]
+            strings.append("".join(s))
+    order = rng.permutation(len(strings))
+    strings = [strings[i] for i in order]
+    res, ln = from_strings(strings)
+    for l_max in (0, 1, 2, 4, 9, 20):
+        got, _ = gpu_network(pkg, res, ln, l_max)
+        want = oracle.network(res, ln, l_max, tier=0)[:3]
+        assert_same_network(got, want)
+        got, _ = gpu_network(pkg, res, ln, l_max, **{pkg.OPT_EARLY_EXIT: 0})
+        assert_same_network(got, want)
+
+
+def test_length_64_and_all_26_letters(pkg, oracle):
+    rng = np.random.default_rng(5)
+    letters = "ABCDEFGHIJKLMNOPQRSTUVWXYZ"
+    strings = []
+    for _ in range(40):
+        base = [letters[i] for i in rng.integers(0, 26, 64)]
+        strings.append("".join(base))
+        for k in range(1, 4):
+            s = base[:]
+            for p in rng.choice(64, k, replace=False):
+                s[p] = letters[int(rng.integers(0, 26))]
+            strings.append("".join(s))
+            strings.append("".join(s[1:]))  # one deletion at the front: length 63
+    res, ln = from_strings(strings)
+    for l_max in (1, 3):
+        got, _ = gpu_network(pkg, res, ln, l_max)
+        assert_same_network(got, oracle.network(res, ln, l_max, tier=0)[:3])
+
+
+def test_equal_length_is_not_hamming(pkg):
+    """Reading Q6: a cyclic shift has Hamming distance 4 but Levenshtein distance 2."""
+    got, _ = gpu_network(pkg, *from_strings(["ABCD", "BCDA"]), 2)
+    assert got[1].tolist() == [1]
+    got, _ = gpu_network(pkg, *from_strings(["ABCD", "BCDA"]), 1)
+    assert got[1].size == 0
+
+
+def test_errors(pkg):
+    with pkg.TcrNet(0) as net:
+        with pytest.raises(pkg.TcrNetError) as e:
+            net.build(1)
+        assert e.value.status == pkg.ERR_STATE
+        for bad in (0, 65):
+            with pytest.raises(pkg.TcrNetError) as e:
+                net.load(np.full(70, ord("A"), np.uint8), np.array([5, bad], np.int32))
+            assert e.value.status == pkg.ERR_LENGTH
+        with pytest.raises(pkg.TcrNetError) as e:
+            net.load(np.frombuffer(b"CASSaF", np.uint8), np.array([6], np.int32))
+        assert e.value.status == pkg.ERR_RESIDUE
+        with pytest.raises(pkg.TcrNetError) as e:
+            net.csr()
+        assert e.value.status == pkg.ERR_STATE
+        res, ln = from_strings(["CASSF"] * 50)
+        net.load(res, ln)
+        for bad in (-1, 65):
+            with pytest.raises(pkg.TcrNetError) as e:
+                net.build(bad)
+            assert e.value.status == pkg.ERR_LMAX
+        net.set_option(pkg.OPT_EDGE_LIMIT, 100)
+        with pytest.raises(pkg.TcrNetError) as e:
+            net.build(0)  # 1225 edges > limit
+        assert e.value.status == pkg.ERR_EDGE_OVERFLOW
+        net.set_option(pkg.OPT_EDGE_LIMIT, 1 << 31)
+        assert net.build(0) == 1225  # the context stays usable
+        with pytest.raises(pkg.TcrNetError):
+            net.set_option(99, 1)
+
+
+def test_device_side_validation(pkg):
+    import torch
+    with pkg.TcrNet(0) as net:
+        res = torch.full((20,), ord("A"), dtype=torch.uint8, device="cuda")
+        with pytest.raises(pkg.TcrNetError) as e:
+            net.load(res, torch.tensor([20, 0], dtype=torch.int32, device="cuda"))
+        assert e.value.status == pkg.ERR_LENGTH
+        res[7] = ord("~")
+        with pytest.raises(pkg.TcrNetError) as e:
+            net.load(res, torch.tensor([10, 10], dtype=torch.int32, device="cuda"))
+        assert e.value.status == pkg.ERR_RESIDUE
+
+
+# ------------------------------------------------------------------ BASELINE.json's large configs
+def _sampled_parity(pkg, oracle, name, l_max, n_sample, seed):
+    d = generate(name)
+    (rp, cl, dg), st = gpu_network(pkg, d.residues, d.lengths, l_max)
+    check_csr_invariants(rp, cl, dg, d.n)
+    rng = np.random.default_rng(seed)
+    # half uniformly random nodes, half nodes the GPU says have neighbours (so the test sees edges)
+    nodes = np.unique(np.concatenate([rng.choice(d.n, n_sample // 2, replace=False),
+                                      rng.choice(np.nonzero(dg > 0)[0], n_sample // 2, replace=False)]))
+    pairs, _ = oracle.edges(d.residues, d.lengths, l_max, rows=nodes, all_partners=True, tier=0)
+    want = neighbours_from_pairs(pairs, nodes)
+    got = neighbours_from_csr(rp, cl, nodes)
+    n_edges_seen = 0
+    for u in nodes:
+        assert np.array_equal(got[int(u)], want[int(u)]), f"node {u}"
+        assert dg[u] == want[int(u)].size
+        n_edges_seen += want[int(u)].size
+    assert n_edges_seen > 0
+    # generator-linked lower bound over ALL family pairs: edits sum <= l_max  =>  edge
+    order = np.argsort(d.family, kind="stable")
+    fam = d.family[order]
+    starts = np.nonzero(np.diff(fam, prepend=-2))[0]
+    keys = set()
+    rows_of = np.repeat(np.arange(d.n, dtype=np.int64), np.diff(rp))
+    edge_keys = rows_of * d.n + cl
+    must = []
+    for a, b in zip(starts, list(starts[1:]) + [fam.size]):
+        if fam[a] < 0:
+            continue
+        members = order[a:b]
+        low = members[d.n_edits[members] <= l_max]
+        for x, y in itertools.combinations(low.tolist(), 2):
+            if d.n_edits[x] + d.n_edits[y] <= l_max:
+                must.append(min(x, y) * d.n + max(x, y))
+        if len(must) > 400000:
+            break
+    must = np.array(must, dtype=np.int64)
+    assert must.size > 0 and np.isin(must, edge_keys).all()
+    return st
+
+
+def test_cfg3_sampled(pkg, oracle):
+    _sampled_parity(pkg, oracle, "cfg3", 2, 64, 3)
+
+
+def test_cfg4_sampled_headline_config(pkg, oracle):
+    """N = 800,000, l_max = 1: the configuration bench.py times, default launch configuration."""
+    st = _sampled_parity(pkg, oracle, "cfg4", 1, 48, 4)
+    assert st["pairs_all"] == 800000 * 799999 // 2
+    assert st["distance_passes"] == 1
+
+
+def test_cfg5_sampled(pkg, oracle):
+    """N = 2,000,000, l_max = 3, lengths 5..40 (patterns > 32 use 64-bit words)."""
+    _sampled_parity(pkg, oracle, "cfg5", 3, 24, 5)
