@@ -35,7 +35,7 @@ WORKLOAD = "cfg4"
 ALU_LANES_PER_SM = 64          # INT32 ALU-pipe lanes per SM per clock on sm_100
 ALU_OPS_PER_COLUMN = 7         # LOP3 per pair and text column (distance.cu)
 ALU_OPS_PER_TEST = 4           # 2 LOP3 + IADD3 + ISETP per pair and early-exit test
-ORACLE_SAMPLE_ROWS = 64
+ORACLE_SAMPLE_ROWS = 1024
 
 
 def _peaks():

@@ -30,9 +30,9 @@ def oracle():
     return o
 
 
-def gpu_network(pkg, residues, lengths, l_max, **opts):
+def gpu_network(pkg, residues, lengths, l_max, opts=None):
     with pkg.TcrNet(0) as net:
-        for k, v in opts.items():
+        for k, v in (opts or {}).items():
             net.set_option(k, v)
         net.load(residues, lengths)
         net.build(l_max)
@@ -67,16 +67,16 @@ def test_early_exit_and_schedule_do_not_change_the_result(pkg):
     text chunks and a tiny edge buffer (forces the second distance pass) give the same bytes."""
     d = generate("cfg2", n=20000)
     for l_max in (1, 3):
-        ref, st0 = gpu_network(pkg, d.residues, d.lengths, l_max, **{pkg.OPT_EARLY_EXIT: 0})
+        ref, st0 = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_EARLY_EXIT: 0})
         assert st0["first_check"] == 0
         for fc in range(3, 9):
-            got, st = gpu_network(pkg, d.residues, d.lengths, l_max, **{pkg.OPT_FIRST_CHECK: fc})
+            got, st = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_FIRST_CHECK: fc})
             assert st["first_check"] == fc
             assert_same_network(got, ref)
-        got, st = gpu_network(pkg, d.residues, d.lengths, l_max, **{pkg.OPT_TEXT_CHUNK: 256, pkg.OPT_EDGE_CAPACITY: 100})
+        got, st = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_TEXT_CHUNK: 256, pkg.OPT_EDGE_CAPACITY: 100})
         assert st["distance_passes"] == 2
         assert_same_network(got, ref)
-        got, st = gpu_network(pkg, d.residues, d.lengths, l_max, **{pkg.OPT_COUNT_WORK: 1})
+        got, st = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_COUNT_WORK: 1})
         assert_same_network(got, ref)
         assert 0 < st["lane_columns_exec"] and st["lane_pairs_exec"] >= st["pairs_kept"]
 
@@ -162,7 +162,7 @@ def test_all_lengths_1_to_64_incl_wide_words(pkg, oracle):
         got, _ = gpu_network(pkg, res, ln, l_max)
         want = oracle.network(res, ln, l_max, tier=0)[:3]
         assert_same_network(got, want)
-        got, _ = gpu_network(pkg, res, ln, l_max, **{pkg.OPT_EARLY_EXIT: 0})
+        got, _ = gpu_network(pkg, res, ln, l_max, {pkg.OPT_EARLY_EXIT: 0})
         assert_same_network(got, want)
 
 
