@@ -36,6 +36,9 @@ ALU_LANES_PER_SM = 64          # INT32 ALU-pipe lanes per SM per clock on sm_100
 ALU_OPS_PER_COLUMN = 7         # LOP3 per pair and text column (distance.cu)
 ALU_OPS_PER_TEST = 4           # 2 LOP3 + IADD3 + ISETP per pair and early-exit test
 ORACLE_SAMPLE_ROWS = 1024
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_distance launch at cfg4, from the ncu --set full
+# capture summarised in profiles/r1_distance_ncu.txt (84.32 MB + 21.21 MB)
+NCU_DRAM_BYTES_PER_LAUNCH = {"cfg4": 105_532_672}
 
 
 def _peaks():
@@ -274,7 +277,7 @@ def main() -> None:
             "gpu_launches": int(sum(s["launches_load"] + s["launches_build"] for s in stats)),
             "roofline": {
                 "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TIOP/s (INT32 ALU-pipe lane-ops)",
-                "frac": achieved / peak, "traffic": None, "kernel": "k_distance", "kernel_ms": ms_dist,
+                "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.workload), "kernel": "k_distance", "kernel_ms": ms_dist,
                 "peak_source": f"{n_sm} SMs x {ALU_LANES_PER_SM} lanes x {peaks['sm_max_mhz']} MHz ({peak_kind} sm_max_mhz)",
                 "alu_ops_per_launch": alu_ops, "measured_pipe_peaks": probes,
             },
