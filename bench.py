@@ -34,6 +34,7 @@ if ROOT not in sys.path:
 WORKLOAD = "cfg4"
 ALU_LANES_PER_SM = 64          # INT32 ALU-pipe lanes per SM per clock on sm_100
 ALU_OPS_PER_COLUMN = 7         # LOP3 per pair and text column (distance.cu)
+ALU_OPS_FIRST_COLUMN = 3       # the first column of a text needs only 3 (constant Pv, Mv = 0)
 ALU_OPS_PER_TEST = 4           # 2 LOP3 + IADD3 + ISETP per pair and early-exit test
 ORACLE_SAMPLE_ROWS = 1024
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_distance launch at cfg4, from the ncu --set full
@@ -255,7 +256,8 @@ def main() -> None:
         ms_sort = float(np.mean([s["ms_sort"] for s in stats]))
         ms_csr = float(np.mean([s["ms_csr"] for s in stats]))
         ms_load = float(np.mean([s["ms_load"] for s in stats]))
-        alu_ops = ALU_OPS_PER_COLUMN * work["lane_columns_exec"] + ALU_OPS_PER_TEST * work["lane_tests_exec"]
+        alu_ops = (ALU_OPS_PER_COLUMN * work["lane_columns_exec"] + ALU_OPS_PER_TEST * work["lane_tests_exec"]
+                   - (ALU_OPS_PER_COLUMN - ALU_OPS_FIRST_COLUMN) * work["lane_pairs_exec"] * (work["first_check"] > 0))
         achieved = alu_ops / (ms_dist * 1e-3) / 1e12
         peak = n_sm * ALU_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12
         probes = {}

@@ -82,7 +82,7 @@ typedef enum tcrnet_option {
                                      every kept pair is computed.  Never changes the result
                                      (PAPER.md:326 describes the abort as a time saver only). */
     TCRNET_OPT_FIRST_CHECK = 2,   /* text columns processed before the first early-exit test;
-                                     0 = automatic (l_max + 4, clamped to 3..8)               */
+                                     0 = automatic (l_max + 2, clamped to 3..8)               */
     TCRNET_OPT_EDGE_CAPACITY = 3, /* initial capacity of the edge buffer in edges; 0 = automatic
                                      (max(1 Mi, 16 N)).  The buffer grows to the exact count
                                      and the distance pass is re-run if it was too small.      */

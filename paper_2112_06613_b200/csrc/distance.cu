@@ -62,6 +62,15 @@ __host__ __device__ constexpr int peq_row_bytes() {
     return (kTQ + WordOps<W>::kRowPad) * (int)sizeof(W);
 }
 
+// lop3.b32 with an immediate truth table (a = 0xF0, b = 0xCC, c = 0xAA): written as PTX so that
+// the front end cannot re-associate the recurrence into more LOP3s than the seven it needs.
+template <int LUT>
+__device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t r;
+    asm("lop3.b32 %0, %1, %2, %3, %4;" : "=r"(r) : "r"(a), "r"(b), "r"(c), "n"(LUT));
+    return r;
+}
+
 template <typename W>
 __device__ __forceinline__ void column_step(W Eq, W& Pv, W& Mv) {
     const W s = (Eq & Pv) + Pv;
@@ -74,15 +83,76 @@ __device__ __forceinline__ void column_step(W Eq, W& Pv, W& Mv) {
     Mv = D0 & ~X;
 }
 
-// K consecutive columns whose residue codes are c[0..K): all Peq loads first, then the chain.
+template <>
+__device__ __forceinline__ void column_step<uint32_t>(uint32_t Eq, uint32_t& Pv, uint32_t& Mv) {
+    const uint32_t t = lop3<0xC0>(Eq, Pv, 0u);        // Eq & Pv
+    const uint32_t s = t + Pv;
+    const uint32_t D0a = lop3<0xBE>(s, Pv, Mv);       // (s ^ Pv) | Mv
+    const uint32_t D0 = lop3<0xFC>(D0a, Eq, 0u);      // | Eq
+    const uint32_t nHp = lop3<0x0E>(Mv, D0, Pv);      // ~Mv & (D0 | Pv) = ~Hp
+    const uint32_t Hn = lop3<0xC0>(Pv, D0, 0u);       // Pv & D0
+    const uint32_t X = nHp + nHp;                     // ~((Hp << 1) | 1)
+    const uint32_t Hn2 = Hn + Hn;                     // Hn << 1
+    Pv = lop3<0xF2>(Hn2, D0, X);                      // Hn2 | (~D0 & X)
+    Mv = lop3<0x30>(D0, X, 0u);                       // D0 & ~X
+}
+
+// Column 0 starts from Pv = low(m), Mv = 0.  Bits at and above m are don't-cares (they never flow
+// down and are masked at every popcount), so ~Hp = D0 | Pv may be replaced by the constant Pv, and
+// Hn = Pv & D0 by D0:  X = Pv0 + Pv0 is a constant and the step needs 3 LOP3 + 2 adds.
+template <typename W>
+__device__ __forceinline__ void first_column_step(W Eq, W Pv0, W X0, W& Pv, W& Mv) {
+    const W s = Eq + Pv0;            // Eq & Pv0 = Eq: Peq has no bits at or above m
+    const W D0 = ((s ^ Pv0) | Eq);
+    const W Hn2 = D0 + D0;
+    Pv = Hn2 | (~D0 & X0);
+    Mv = D0 & ~X0;
+}
+template <>
+__device__ __forceinline__ void first_column_step<uint32_t>(uint32_t Eq, uint32_t Pv0, uint32_t X0, uint32_t& Pv,
+                                                             uint32_t& Mv) {
+    const uint32_t s = Eq + Pv0;
+    const uint32_t D0 = lop3<0xBE>(s, Pv0, Eq);       // (s ^ Pv0) | Eq
+    const uint32_t Hn2 = D0 + D0;
+    Pv = lop3<0xF2>(Hn2, D0, X0);                     // Hn2 | (~D0 & X0)
+    Mv = lop3<0x30>(D0, X0, 0u);                      // D0 & ~X0
+}
+
+// Shared-memory accesses by 32-bit shared address (no generic-pointer arithmetic in the hot loop).
+// The text loads are volatile so that they stay behind the barrier that publishes the stage; the Peq
+// loads depend on their results.
+template <typename W>
+__device__ __forceinline__ W peq_load(uint32_t lane_addr, uint32_t code);
+template <>
+__device__ __forceinline__ uint32_t peq_load<uint32_t>(uint32_t lane_addr, uint32_t code) {
+    uint32_t v;
+    asm("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(lane_addr + code * (uint32_t)peq_row_bytes<uint32_t>()));
+    return v;
+}
+template <>
+__device__ __forceinline__ uint64_t peq_load<uint64_t>(uint32_t lane_addr, uint32_t code) {
+    unsigned long long v;
+    asm("ld.shared.u64 %0, [%1];" : "=l"(v) : "r"(lane_addr + code * (uint32_t)peq_row_bytes<uint64_t>()));
+    return v;
+}
+__device__ __forceinline__ void text_load4(uint32_t addr, uint32_t* c) {
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(c[0]), "=r"(c[1]), "=r"(c[2]), "=r"(c[3]) : "r"(addr));
+}
+__device__ __forceinline__ uint32_t text_load1(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+
+// The first K columns of a text (codes c[0..K)): all Peq loads first, then the chain.
 template <typename W, int K>
-__device__ __forceinline__ void columns(const unsigned char* lane_col, const uint32_t* c, W& Pv, W& Mv) {
+__device__ __forceinline__ void first_columns(uint32_t lane_addr, const uint32_t* c, W Pv0, W X0, W& Pv, W& Mv) {
     W Eq[K > 0 ? K : 1];
 #pragma unroll
-    for (int q = 0; q < K; ++q)
-        Eq[q] = *reinterpret_cast<const W*>(lane_col + c[q] * (uint32_t)peq_row_bytes<W>());
+    for (int q = 0; q < K; ++q) Eq[q] = peq_load<W>(lane_addr, c[q]);
+    if (K > 0) first_column_step<W>(Eq[0], Pv0, X0, Pv, Mv);
 #pragma unroll
-    for (int q = 0; q < K; ++q) column_step<W>(Eq[q], Pv, Mv);
+    for (int q = 1; q < K; ++q) column_step<W>(Eq[q], Pv, Mv);
 }
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
@@ -95,10 +165,15 @@ __device__ __forceinline__ void cp_async_wait() {
     asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory");
 }
 
+// FIRST = text columns processed before the first early-exit test (0: early exit off).
+// Hot path per (warp, text): one or two broadcast LDS.128 (the first 4 / 8 residue codes), FIRST unrolled
+// columns, one test; ~95 % of the visits end there.  Everything else (remaining columns with a test every
+// second column, the final distance, emission) is the cold path.
 template <typename W, int FIRST, bool COUNT>
 __global__ void __launch_bounds__(kTQ) k_distance(const __grid_constant__ DistanceParams P) {
     extern __shared__ __align__(16) unsigned char smem[];
     constexpr int kRowBytes = peq_row_bytes<W>();
+    constexpr int kRowWords = kRowBytes / (int)sizeof(W);
     constexpr uint32_t kFull = 0xffffffffu;
     W* peq = reinterpret_cast<W*>(smem);
     uint32_t* tbuf = reinterpret_cast<uint32_t*>(smem + kPeqRows * kRowBytes);
@@ -128,7 +203,7 @@ __global__ void __launch_bounds__(kTQ) k_distance(const __grid_constant__ Distan
     const int p_rel = p_tile0 + tid;
     const bool p_valid = p_rel < R.p_count;
 #pragma unroll
-    for (int r = 0; r < kPeqRows; ++r) peq[r * (kRowBytes / (int)sizeof(W)) + tid] = W(0);
+    for (int r = 0; r < kPeqRows; ++r) peq[r * kRowWords + tid] = W(0);
     if (p_valid) {
         const uint4* prow = reinterpret_cast<const uint4*>(P.pat + (size_t)(R.p_start + p_rel) * P.pat_stride);
         for (int i0 = 0; i0 < m; i0 += 16) {
@@ -139,14 +214,29 @@ __global__ void __launch_bounds__(kTQ) k_distance(const __grid_constant__ Distan
                 const int i = i0 + k;
                 if (i < m) {
                     const uint32_t c = (w4[k >> 2] >> ((k & 3) * 8)) & 0xffu;
-                    peq[c * (kRowBytes / (int)sizeof(W)) + tid] |= W(1) << i;
+                    peq[c * kRowWords + tid] |= W(1) << i;
                 }
             }
         }
     }
-    const unsigned char* lane_col = smem + tid * (int)sizeof(W);
+    const uint32_t smem_addr = (uint32_t)__cvta_generic_to_shared(smem);
+    const uint32_t lane_addr = smem_addr + tid * (uint32_t)sizeof(W);
+    const uint32_t tbuf_addr = smem_addr + kPeqRows * kRowBytes;
     const W pv_init = low_mask<W>(m);
+    W x_init = pv_init + pv_init;
     const W m_mask = pv_init;
+
+    // the hot test: after FIRST columns, rows 1..FIRST-delta of the column (only if FIRST > delta, FIRST <= n)
+    const bool hot = FIRST > 0 && FIRST <= n && FIRST > delta;
+    const W first_mask = low_mask<W>(hot ? FIRST - delta : 0);
+    int first_thr = l_max - FIRST;            // dead  <=>  popc(Pv & mask) - popc(Mv & mask) > first_thr
+    // keep the loop invariants of the hot loop in registers (ptxas otherwise re-derives them per text)
+    asm volatile("" : "+r"(first_thr));
+    if (sizeof(W) == 4) {
+        uint32_t x32 = (uint32_t)x_init;
+        asm volatile("" : "+r"(x32));
+        x_init = (W)x32;
+    }
 
     // ---- text pipeline: kTT rows per stage, two stages, 16-byte cp.async ----
     const uint32_t* txt_chunk = P.txt + R.txt_base + (int64_t)chunk_t0 * rw;
@@ -171,81 +261,61 @@ __global__ void __launch_bounds__(kTQ) k_distance(const __grid_constant__ Distan
         cp_async_wait<1>();
         __syncthreads();
 
-        const uint32_t* tb = tbuf + (sub & 1) * stage_words;
+        const int sub_t0 = chunk_t0 + sub * kTT;
         const int cnt = min(kTT, chunk_cnt - sub * kTT);
-        for (int tt = 0; tt < cnt; ++tt) {
-            const int t_rel = chunk_t0 + sub * kTT + tt;
-            if (R.diag && t_rel <= warp_p0) continue;  // every lane has p >= t
-            const uint4* trow = reinterpret_cast<const uint4*>(tb + tt * rw);
-            W Pv = pv_init, Mv = W(0);
-            bool alive = true;
-            int g = 0;
-            if (COUNT) ++n_visits;
-
-            // lower bound on the final diagonal after column j; only called with j > delta
-            auto all_dead = [&](int j) -> bool {
-                const W msk = low_mask<W>(j - delta);
-                const int lb = j + WordOps<W>::popc(Pv & msk) - WordOps<W>::popc(Mv & msk);
-                if (COUNT) ++n_tests;
-                return !__any_sync(kFull, lb <= l_max);
-            };
-
-            if (FIRST > 0 && n >= 8) {
-                const uint4 o0 = trow[0], o1 = trow[1];
-                const uint32_t c[8] = {o0.x, o0.y, o0.z, o0.w, o1.x, o1.y, o1.z, o1.w};
-                columns<W, FIRST>(lane_col, c, Pv, Mv);
-                if (COUNT) n_cols += FIRST;
-                if (FIRST > delta && all_dead(FIRST)) alive = false;
-                if (alive) {
-                    columns<W, 8 - FIRST>(lane_col, c + FIRST, Pv, Mv);
-                    if (COUNT) n_cols += 8 - FIRST;
-                    if (FIRST < 8 && 8 > delta && all_dead(8)) alive = false;
+        // same bucket: texts at or before this warp's first pattern pair with nobody (sorted p < t only)
+        const int tt_begin = R.diag ? max(0, warp_p0 + 1 - sub_t0) : 0;
+        const uint32_t row_bytes = (uint32_t)rw * 4u;
+        uint32_t row_addr = tbuf_addr + (uint32_t)((sub & 1) * stage_words + tt_begin * rw) * 4u;
+        // ---- cold path: the remaining columns (a test after every second one), distance, emission ----
+        auto finish = [&](int tt, uint32_t row_addr, W Pv, W Mv, int j) {
+            for (; j < n; ++j) {
+                const W Eq = peq_load<W>(lane_addr, text_load1(row_addr + 4u * (uint32_t)j));
+                column_step<W>(Eq, Pv, Mv);
+                if (COUNT) ++n_cols;
+                const int jj = j + 1;
+                if (FIRST > 0 && (jj & 1) == 0 && jj > delta && jj < n) {
+                    const W msk = low_mask<W>(jj - delta);
+                    const int lb = jj + WordOps<W>::popc(Pv & msk) - WordOps<W>::popc(Mv & msk);
+                    if (COUNT) ++n_tests;
+                    if (!__any_sync(kFull, lb <= l_max)) return;
                 }
-                g = 2;
             }
-            if (alive) {
-                const int n_groups = n >> 2;
-                for (; g < n_groups; ++g) {
-                    const uint4 o = trow[g];
-                    const uint32_t c[4] = {o.x, o.y, o.z, o.w};
-                    columns<W, 4>(lane_col, c, Pv, Mv);
-                    if (COUNT) n_cols += 4;
-                    if (FIRST > 0) {
-                        const int j = 4 * (g + 1);
-                        if (j > delta && all_dead(j)) {
-                            alive = false;
-                            break;
-                        }
+            const int d = n + WordOps<W>::popc(Pv & m_mask) - WordOps<W>::popc(Mv & m_mask);
+            const int t_rel = sub_t0 + tt;
+            const bool edge = d <= l_max && p_valid && (!R.diag || p_rel < t_rel);
+            const uint32_t bal = __ballot_sync(kFull, edge);
+            if (bal) {
+                unsigned long long base = 0;
+                if (lane == 0) base = atomicAdd(P.edge_count, (unsigned long long)__popc(bal));
+                base = __shfl_sync(kFull, base, 0);
+                if (edge) {
+                    const unsigned long long pos = base + __popc(bal & ((1u << lane) - 1u));
+                    if (pos < P.edge_cap) {
+                        const uint32_t oi = (uint32_t)P.perm[R.p_start + p_rel];
+                        const uint32_t oj = (uint32_t)P.perm[R.t_start + t_rel];
+                        const uint32_t a = min(oi, oj), b = max(oi, oj);
+                        P.edges[pos] = ((unsigned long long)a << 32) | b;
                     }
                 }
             }
-            if (alive) {
-                const int rem = n & 3;
-                if (rem) {
-                    const uint4 o = trow[n >> 2];
-                    const uint32_t c[3] = {o.x, o.y, o.z};
-                    if (rem == 1) columns<W, 1>(lane_col, c, Pv, Mv);
-                    else if (rem == 2) columns<W, 2>(lane_col, c, Pv, Mv);
-                    else columns<W, 3>(lane_col, c, Pv, Mv);
-                    if (COUNT) n_cols += rem;
-                }
-                const int d = n + WordOps<W>::popc(Pv & m_mask) - WordOps<W>::popc(Mv & m_mask);
-                const bool edge = d <= l_max && p_valid && (!R.diag || p_rel < t_rel);
-                const uint32_t bal = __ballot_sync(kFull, edge);
-                if (bal) {
-                    unsigned long long base = 0;
-                    if (lane == 0) base = atomicAdd(P.edge_count, (unsigned long long)__popc(bal));
-                    base = __shfl_sync(kFull, base, 0);
-                    if (edge) {
-                        const unsigned long long pos = base + __popc(bal & ((1u << lane) - 1u));
-                        if (pos < P.edge_cap) {
-                            const uint32_t oi = (uint32_t)P.perm[R.p_start + p_rel];
-                            const uint32_t oj = (uint32_t)P.perm[R.t_start + t_rel];
-                            const uint32_t a = min(oi, oj), b = max(oi, oj);
-                            P.edges[pos] = ((unsigned long long)a << 32) | b;
-                        }
-                    }
-                }
+        };
+        if (hot) {
+            // ---- hot loop: 1-2 broadcast LDS.128, FIRST unrolled columns, one warp-wide test ----
+            for (int tt = tt_begin; tt < cnt; ++tt, row_addr += row_bytes) {
+                uint32_t c[8];
+                W Pv, Mv;
+                text_load4(row_addr, c);
+                if (FIRST > 4) text_load4(row_addr + 16u, c + 4);
+                first_columns<W, FIRST>(lane_addr, c, pv_init, x_init, Pv, Mv);
+                const int score = WordOps<W>::popc(Pv & first_mask) - WordOps<W>::popc(Mv & first_mask);
+                if (COUNT) { ++n_visits; n_cols += FIRST; ++n_tests; }
+                if (__any_sync(kFull, score <= first_thr)) finish(tt, row_addr, Pv, Mv, FIRST);
+            }
+        } else {
+            for (int tt = tt_begin; tt < cnt; ++tt, row_addr += row_bytes) {
+                if (COUNT) ++n_visits;
+                finish(tt, row_addr, pv_init, W(0), 0);
             }
         }
         __syncthreads();  // stage (sub & 1) is free for the load issued two iterations later

@@ -17,11 +17,28 @@ constexpr int kWarps = kThreads / 32;
 constexpr int kRounds = 16;
 constexpr int kItemsPerBlock = kThreads * kRounds;  // 4096
 
+// Digits of the sequence sort (step A1).  `perm_in` is the current order (NULL = identity).
 struct LengthDigit {
     const int32_t* lengths;
+    const int32_t* perm_in;
     __device__ __forceinline__ uint32_t digit(int64_t i) const {
-        int32_t l = lengths[i];
+        const int32_t l = lengths[perm_in ? perm_in[i] : i];
         return (l < 0 || l > kMaxLen) ? 0u : (uint32_t)l;  // invalid lengths are reported elsewhere
+    }
+};
+
+struct ResidueDigit {  // residue at position k (0 = past the end), for the lexicographic sub-order
+    const uint8_t* residues;
+    const int64_t* offsets;
+    const int32_t* lengths;
+    const int32_t* perm_in;
+    int k;
+    __device__ __forceinline__ uint32_t digit(int64_t i) const {
+        const int64_t o = perm_in ? perm_in[i] : i;
+        const int32_t l = lengths[o];
+        if (l < 1 || l > kMaxLen || k >= l) return 0u;
+        const uint32_t c = (uint32_t)residues[offsets[o] + k] - (uint32_t)'A';
+        return (c < 26u ? c : 26u) + 1u;  // invalid residues are reported by the pack kernel
     }
 };
 
@@ -48,8 +65,11 @@ __global__ void __launch_bounds__(kThreads) k_split_hist(D src, int64_t n, uint3
 }
 
 struct PermSink {
-    int32_t* perm;
-    __device__ __forceinline__ void put(int64_t pos, int64_t i) const { perm[pos] = (int32_t)i; }
+    const int32_t* perm_in;
+    int32_t* perm_out;
+    __device__ __forceinline__ void put(int64_t pos, int64_t i) const {
+        perm_out[pos] = perm_in ? perm_in[i] : (int32_t)i;
+    }
 };
 
 struct KeySink {
@@ -114,9 +134,18 @@ cudaError_t split_impl(D src, S sink, int64_t n, uint32_t* hist, uint32_t* hist_
 
 int64_t split_num_blocks(int64_t n) { return n > 0 ? (n + kItemsPerBlock - 1) / kItemsPerBlock : 1; }
 
-cudaError_t split_by_length(const int32_t* lengths, int64_t n, int32_t* perm_out, uint32_t* hist,
-                            uint32_t* hist_scanned, void* scan_scratch, cudaStream_t s, int* launches) {
-    return split_impl(LengthDigit{lengths}, PermSink{perm_out}, n, hist, hist_scanned, scan_scratch, s, launches);
+cudaError_t split_by_length(const int32_t* lengths, const int32_t* perm_in, int64_t n, int32_t* perm_out,
+                            uint32_t* hist, uint32_t* hist_scanned, void* scan_scratch, cudaStream_t s,
+                            int* launches) {
+    return split_impl(LengthDigit{lengths, perm_in}, PermSink{perm_in, perm_out}, n, hist, hist_scanned,
+                      scan_scratch, s, launches);
+}
+
+cudaError_t split_by_residue(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths,
+                             const int32_t* perm_in, int k, int64_t n, int32_t* perm_out, uint32_t* hist,
+                             uint32_t* hist_scanned, void* scan_scratch, cudaStream_t s, int* launches) {
+    return split_impl(ResidueDigit{residues, offsets, lengths, perm_in, k}, PermSink{perm_in, perm_out}, n, hist,
+                      hist_scanned, scan_scratch, s, launches);
 }
 
 cudaError_t split_keys_u64(const unsigned long long* in, unsigned long long* out, int64_t n, int shift,

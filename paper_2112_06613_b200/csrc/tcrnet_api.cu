@@ -179,16 +179,42 @@ int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len
         dev_free(ctx, offsets);
         return rc;
     }
+    // Sort key: (length, first kSortPrefix residues, row).  LSD: least significant digit first, every
+    // pass stable.  The sub-order inside a length bucket is free (results are mapped back through
+    // perm); the lexicographic one makes the 32 patterns of a warp share their first residues, so the
+    // early-exit test of the distance kernel fails or holds for the whole warp at once.
+    DevBuf perm_tmp;
+    rc = dev_reserve(ctx, perm_tmp, sizeof(int32_t) * (size_t)n);
+    if (rc != TCRNET_OK) {
+        dev_free(ctx, offsets);
+        return rc;
+    }
     cudaError_t e = exclusive_scan_i32_to_i64(d_len, (int64_t*)offsets.p, n, true, ctx->scan_scratch.p, s, launches);
-    if (e == cudaSuccess)
-        e = split_by_length(d_len, n, (int32_t*)ctx->perm.p, (uint32_t*)ctx->split_hist.p,
-                            (uint32_t*)ctx->split_hist_scanned.p, ctx->scan_scratch.p, s, launches);
+    {
+        // kSortPrefix + 1 passes ping-pong between the two buffers; arrange for the last to land in ctx->perm
+        int32_t* bufs[2] = {(int32_t*)ctx->perm.p, (int32_t*)perm_tmp.p};
+        int cur = kSortPrefix & 1;  // buffer written by the first pass
+        const int32_t* in = nullptr;
+        for (int k = kSortPrefix - 1; k >= 0 && e == cudaSuccess; --k) {
+            e = split_by_residue(d_res, (const int64_t*)offsets.p, d_len, in, k, n, bufs[cur],
+                                 (uint32_t*)ctx->split_hist.p, (uint32_t*)ctx->split_hist_scanned.p,
+                                 ctx->scan_scratch.p, s, launches);
+            in = bufs[cur];
+            cur ^= 1;
+        }
+        if (e == cudaSuccess)
+            e = split_by_length(d_len, in, n, bufs[cur], (uint32_t*)ctx->split_hist.p,
+                                (uint32_t*)ctx->split_hist_scanned.p, ctx->scan_scratch.p, s, launches);
+        // cur is now the index of the buffer holding the final order
+        if (bufs[cur] != (int32_t*)ctx->perm.p) e = e == cudaSuccess ? cudaErrorUnknown : e;
+    }
     if (e == cudaSuccess)
         e = launch_pack(d_res, (const int64_t*)offsets.p, d_len, (const int32_t*)ctx->perm.p, n, lt, ctx->pat_stride,
                         (uint8_t*)ctx->pat.p, (uint32_t*)ctx->txt.p, &dc->flags, s, launches);
     if (e == cudaSuccess) e = cudaMemcpyAsync(&ctx->h_ctrl->flags, &dc->flags, sizeof(uint32_t), cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     dev_free(ctx, offsets);
+    dev_free(ctx, perm_tmp);
     TRY_CUDA(e);
     if (ctx->h_ctrl->flags & kFlagBadResidue) return TCRNET_ERR_RESIDUE;
 
@@ -445,7 +471,7 @@ int tcrnet_build(tcrnet_ctx* ctx, int l_max, int64_t* n_edges_out) {
     st.work_items = sch.items_narrow + sch.items_wide;
     int first_check = 0;
     if (ctx->early_exit) {
-        first_check = ctx->first_check_opt ? ctx->first_check_opt : l_max + 4;
+        first_check = ctx->first_check_opt ? ctx->first_check_opt : l_max + 2;
         first_check = std::max(3, std::min(8, first_check));
     }
     st.first_check = first_check;

@@ -16,6 +16,7 @@ constexpr int kPadCode = 26;             // text padding: selects an all-zero Pe
 constexpr int kPeqRows = 27;             // 26 residue rows + the zero row
 constexpr int kTQ = 256;                 // patterns per CTA of the distance kernel (8 warps)
 constexpr int kTT = 64;                  // texts staged into shared memory per pipeline stage
+constexpr int kSortPrefix = 6;           // residues of the lexicographic sub-order inside a length bucket
 
 // Per-length layout of the packed sequence tables (filled on the host after the histogram).
 struct LengthTable {
@@ -67,9 +68,14 @@ cudaError_t exclusive_scan_u32(const uint32_t* in, uint32_t* out, int64_t n, voi
 
 // split.cu: one stable counting-sort pass over 8-bit digits.
 int64_t split_num_blocks(int64_t n);
-// lengths -> perm (sorted by (clamped length, row)); hist_scratch uint32[256*blocks] x2.
-cudaError_t split_by_length(const int32_t* lengths, int64_t n, int32_t* perm_out, uint32_t* hist,
-                            uint32_t* hist_scanned, void* scan_scratch, cudaStream_t s, int* launches);
+// Stable passes of the sequence sort: perm_out = perm_in (NULL = identity) re-ordered by the clamped
+// length / by the residue at position k.  hist, hist_scanned: uint32[256 * split_num_blocks(n)].
+cudaError_t split_by_length(const int32_t* lengths, const int32_t* perm_in, int64_t n, int32_t* perm_out,
+                            uint32_t* hist, uint32_t* hist_scanned, void* scan_scratch, cudaStream_t s,
+                            int* launches);
+cudaError_t split_by_residue(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths,
+                             const int32_t* perm_in, int k, int64_t n, int32_t* perm_out, uint32_t* hist,
+                             uint32_t* hist_scanned, void* scan_scratch, cudaStream_t s, int* launches);
 // one radix pass on 64-bit keys, digit = (key >> shift) & 255.
 cudaError_t split_keys_u64(const unsigned long long* in, unsigned long long* out, int64_t n, int shift,
                            uint32_t* hist, uint32_t* hist_scanned, void* scan_scratch, cudaStream_t s,
