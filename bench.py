@@ -36,6 +36,7 @@ ALU_LANES_PER_SM = 64          # INT32 ALU-pipe lanes per SM per clock on sm_100
 ALU_OPS_PER_COLUMN = 7         # LOP3 per pair and text column (distance.cu)
 ALU_OPS_FIRST_COLUMN = 3       # the first column of a text needs only 3 (constant Pv, Mv = 0)
 ALU_OPS_PER_TEST = 4           # 2 LOP3 + IADD3 + ISETP per pair and early-exit test
+ALU_OPS_PER_PREFIX_TEST = 3    # PRMT + LOP3 + ISETP per pair and trie-node exit test (distance_trie.cu)
 ORACLE_SAMPLE_ROWS = 1024
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_distance launch at cfg4, from the ncu --set full
 # capture summarised in profiles/r1_distance_ncu.txt (84.32 MB + 21.21 MB)
@@ -148,6 +149,8 @@ def main() -> None:
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--first-check", type=int, default=0)
     ap.add_argument("--text-chunk", type=int, default=0)
+    ap.add_argument("--trie-chunk", type=int, default=0)
+    ap.add_argument("--no-trie", action="store_true", help="text-chunk kernel only (every kept pair visited)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -190,6 +193,10 @@ def main() -> None:
         net.set_option(pkg.OPT_FIRST_CHECK, args.first_check)
     if args.text_chunk:
         net.set_option(pkg.OPT_TEXT_CHUNK, args.text_chunk)
+    if args.trie_chunk:
+        net.set_option(pkg.OPT_TRIE_CHUNK, args.trie_chunk)
+    if args.no_trie:
+        net.set_option(pkg.OPT_PREFIX_TRIE, 0)
 
     def step_device():
         net.load(d_res, d_len)
@@ -257,6 +264,7 @@ def main() -> None:
         ms_csr = float(np.mean([s["ms_csr"] for s in stats]))
         ms_load = float(np.mean([s["ms_load"] for s in stats]))
         alu_ops = (ALU_OPS_PER_COLUMN * work["lane_columns_exec"] + ALU_OPS_PER_TEST * work["lane_tests_exec"]
+                   + ALU_OPS_PER_PREFIX_TEST * work["lane_prefix_tests_exec"]
                    - (ALU_OPS_PER_COLUMN - ALU_OPS_FIRST_COLUMN) * work["lane_pairs_exec"] * (work["first_check"] > 0))
         achieved = alu_ops / (ms_dist * 1e-3) / 1e12
         peak = n_sm * ALU_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12
@@ -279,7 +287,7 @@ def main() -> None:
             "gpu_launches": int(sum(s["launches_load"] + s["launches_build"] for s in stats)),
             "roofline": {
                 "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TIOP/s (INT32 ALU-pipe lane-ops)",
-                "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.workload), "kernel": "k_distance", "kernel_ms": ms_dist,
+                "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.workload), "kernel": "k_distance_trie" if work["work_items_trie"] else "k_distance", "kernel_ms": ms_dist,
                 "peak_source": f"{n_sm} SMs x {ALU_LANES_PER_SM} lanes x {peaks['sm_max_mhz']} MHz ({peak_kind} sm_max_mhz)",
                 "alu_ops_per_launch": alu_ops, "measured_pipe_peaks": probes,
             },
@@ -290,7 +298,10 @@ def main() -> None:
                 "gcups_effective": work["cells_all"] / (ms_step * 1e-3) / 1e9,
                 "columns_executed_fraction": work["lane_columns_exec"] / max(1, work["columns_kept"]),
                 "ms_pack": ms_load, "ms_distance": ms_dist, "ms_sort": ms_sort, "ms_csr": ms_csr,
-                "work_items": work["work_items"], "ms_steps": ms_steps,
+                "work_items": work["work_items"], "work_items_trie": work["work_items_trie"],
+                "trie_nodes": work["trie_nodes"], "lane_columns_exec": work["lane_columns_exec"],
+                "lane_prefix_tests_exec": work["lane_prefix_tests_exec"], "lane_tests_exec": work["lane_tests_exec"],
+                "ms_steps": ms_steps,
             },
         }
         if not args.no_cpu_baseline and world == 1:

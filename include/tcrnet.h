@@ -90,7 +90,16 @@ typedef enum tcrnet_option {
                                      tcrnet_build fails with TCRNET_ERR_EDGE_OVERFLOW          */
     TCRNET_OPT_COUNT_WORK = 5,    /* 1: the distance kernel also counts executed columns and
                                      tests (slower, for roofline accounting); default 0        */
-    TCRNET_OPT_TEXT_CHUNK = 6     /* texts per work item (multiple of 256; default 2048)       */
+    TCRNET_OPT_TEXT_CHUNK = 6,    /* texts per work item of the text-chunk kernel (multiple of
+                                     256; default 2048)                                        */
+    TCRNET_OPT_PREFIX_TRIE = 7,   /* 1 (default): bucket pairs whose early exit can act within the
+                                     first 6 text columns are evaluated through the prefix trie
+                                     over the sorted texts (shared prefix columns computed once,
+                                     whole runs of texts skipped by one exit test); 0: every kept
+                                     pair is visited by the text-chunk kernel.  Never changes the
+                                     result.                                                   */
+    TCRNET_OPT_TRIE_CHUNK = 8     /* texts per work item of the prefix-trie kernel (multiple of
+                                     256; default 32768)                                       */
 } tcrnet_option;
 
 /* Work and timing of the last tcrnet_load / tcrnet_build (tcrnet_get_stats). */
@@ -108,8 +117,11 @@ typedef struct tcrnet_stats {
     int64_t columns_kept;      /* sum over kept pairs of the text length (nominal columns)    */
     int64_t lane_columns_exec; /* 32 x warp-level column steps executed  (COUNT_WORK only)    */
     int64_t lane_tests_exec;   /* 32 x warp-level early-exit tests executed (COUNT_WORK only) */
-    int64_t lane_pairs_exec;   /* 32 x warp-level (pattern-warp, text) visits (COUNT_WORK only)*/
-    int64_t work_items;        /* CTAs of the distance kernel                                 */
+    int64_t lane_pairs_exec;   /* 32 x warp-level first-column steps (3-LOP3 form; COUNT_WORK) */
+    int64_t lane_prefix_tests_exec; /* 32 x warp-level trie-node exit tests (COUNT_WORK only)  */
+    int64_t work_items;        /* CTAs of the distance kernels                                */
+    int64_t work_items_trie;   /* ... of which prefix-trie kernel                             */
+    int64_t trie_nodes;        /* nodes of the prefix trie built by the last load             */
     int32_t distance_passes;   /* 1, or 2 if the edge buffer had to grow                      */
     int32_t launches_load;     /* kernels launched by the last tcrnet_load[_device]           */
     int32_t launches_build;    /* kernels launched by the last tcrnet_build                   */

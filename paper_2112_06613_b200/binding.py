@@ -21,6 +21,7 @@ LIB_PATH = os.path.join(_HERE, "libtcrnet_b200.so")
 OK, ERR_ARG, ERR_LENGTH, ERR_RESIDUE, ERR_LMAX, ERR_STATE, ERR_NOMEM, ERR_EDGE_OVERFLOW, ERR_CUDA = (
     0, -1, -2, -3, -4, -5, -6, -7, -8)
 OPT_EARLY_EXIT, OPT_FIRST_CHECK, OPT_EDGE_CAPACITY, OPT_EDGE_LIMIT, OPT_COUNT_WORK, OPT_TEXT_CHUNK = 1, 2, 3, 4, 5, 6
+OPT_PREFIX_TRIE, OPT_TRIE_CHUNK = 7, 8
 
 EXPORTS = (
     "tcrnet_create", "tcrnet_destroy", "tcrnet_load", "tcrnet_load_device", "tcrnet_build", "tcrnet_csr",
@@ -41,7 +42,8 @@ class tcrnet_stats(C.Structure):
         ("l_max", C.c_int32), ("first_check", C.c_int32), ("n_edges", C.c_int64), ("pairs_all", C.c_int64),
         ("pairs_kept", C.c_int64), ("cells_all", C.c_int64), ("cells_kept", C.c_int64),
         ("columns_kept", C.c_int64), ("lane_columns_exec", C.c_int64), ("lane_tests_exec", C.c_int64),
-        ("lane_pairs_exec", C.c_int64), ("work_items", C.c_int64), ("distance_passes", C.c_int32),
+        ("lane_pairs_exec", C.c_int64), ("lane_prefix_tests_exec", C.c_int64), ("work_items", C.c_int64),
+        ("work_items_trie", C.c_int64), ("trie_nodes", C.c_int64), ("distance_passes", C.c_int32),
         ("launches_load", C.c_int32), ("launches_build", C.c_int32), ("ms_load", C.c_float),
         ("ms_distance", C.c_float), ("ms_sort", C.c_float), ("ms_csr", C.c_float), ("ms_build", C.c_float),
     ]

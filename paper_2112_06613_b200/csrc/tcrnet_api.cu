@@ -1,6 +1,7 @@
 // C ABI of libtcrnet_b200.so (include/tcrnet.h): context, memory, the host half of the tile
 // scheduler (step A2) and the orchestration of steps A1-A6 on one CUDA stream.
 #include <algorithm>
+#include <cstddef>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -19,10 +20,12 @@ struct DevBuf {
 struct HostCtrl {  // pinned mirror of the small device control block
     unsigned long long hist[kNumLen];
     unsigned long long edge_count;
-    unsigned long long work[3];
+    unsigned long long work[4];
     unsigned long long probe[3];
     uint32_t flags;
     uint32_t pad_;
+    uint32_t trie_counts[8];          // [k] = nodes of trie level k
+    uint32_t trie_root[kNumLen + 1];  // [L] = first level-1 node of length bucket L (non-empty buckets)
 };
 
 }  // namespace
@@ -42,6 +45,8 @@ struct tcrnet_ctx {
     int64_t edge_limit = (int64_t)1 << 31;
     int count_work = 0;
     int tchunk = 2048;
+    int prefix_trie = 1;
+    int trie_chunk = 32768;
 
     // load state
     bool loaded = false;
@@ -49,7 +54,9 @@ struct tcrnet_ctx {
     int64_t hist[kNumLen] = {};
     LengthTable lt{};
     int pat_stride = 0;
-    DevBuf perm, pat, txt;
+    DevBuf perm, pat, txt, trie;
+    TrieLevels trie_levels{};
+    uint32_t trie_root[kNumLen + 1] = {};  // level-1 node range of bucket L: [trie_root[L], trie_root[L+1])
 
     // build state
     bool built = false;
@@ -211,12 +218,41 @@ int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len
     if (e == cudaSuccess)
         e = launch_pack(d_res, (const int64_t*)offsets.p, d_len, (const int32_t*)ctx->perm.p, n, lt, ctx->pat_stride,
                         (uint8_t*)ctx->pat.p, (uint32_t*)ctx->txt.p, &dc->flags, s, launches);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(&ctx->h_ctrl->flags, &dc->flags, sizeof(uint32_t), cudaMemcpyDeviceToHost, s);
+    // prefix trie over the sorted texts (trie.cu); scratch: lcp8 + per-tile counts
+    DevBuf trie_scratch;
+    if (e == cudaSuccess) {
+        size_t node_total = 0, level_off[kTrieDepth + 1] = {};
+        for (int k = 1; k <= kTrieDepth; ++k) {
+            level_off[k] = node_total;
+            node_total += (size_t)trie_level_capacity(n, k);
+        }
+        const size_t lcp_bytes = (((size_t)n + 15) & ~(size_t)15) + 256;  // keeps the tile counts aligned
+        rc = dev_reserve(ctx, ctx->trie, node_total * sizeof(TrieNode));
+        if (rc == TCRNET_OK) rc = dev_reserve(ctx, trie_scratch, lcp_bytes + (size_t)trie_tiles(n) * 8 * sizeof(uint32_t));
+        if (rc == TCRNET_OK) {
+            for (int k = 1; k <= kTrieDepth; ++k) ctx->trie_levels.p[k] = (TrieNode*)ctx->trie.p + level_off[k];
+            ctx->trie_levels.p[0] = nullptr;
+            e = launch_trie_build((const uint32_t*)ctx->txt.p, lt, n, (uint8_t*)trie_scratch.p,
+                                  (uint32_t*)((uint8_t*)trie_scratch.p + (lcp_bytes & ~(size_t)255)), ctx->trie_levels,
+                                  dc->trie_counts, dc->trie_root, s, launches);
+        }
+    }
+    if (rc == TCRNET_OK && e == cudaSuccess)
+        e = cudaMemcpyAsync(&ctx->h_ctrl->flags, &dc->flags,
+                            sizeof(HostCtrl) - offsetof(HostCtrl, flags), cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     dev_free(ctx, offsets);
     dev_free(ctx, perm_tmp);
+    dev_free(ctx, trie_scratch);
+    if (rc != TCRNET_OK) return rc;
     TRY_CUDA(e);
     if (ctx->h_ctrl->flags & kFlagBadResidue) return TCRNET_ERR_RESIDUE;
+    // level-1 node range of every bucket (empty buckets get an empty range)
+    ctx->trie_root[kNumLen] = ctx->h_ctrl->trie_counts[1];
+    for (int l = kNumLen - 1; l >= 0; --l)
+        ctx->trie_root[l] = ctx->hist[l] ? ctx->h_ctrl->trie_root[l] : ctx->trie_root[l + 1];
+    ctx->stats.trie_nodes = 0;
+    for (int k = 1; k <= kTrieDepth; ++k) ctx->stats.trie_nodes += ctx->h_ctrl->trie_counts[k];
 
     ctx->n = n;
     ctx->total_len = total_len;
@@ -228,14 +264,19 @@ int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len
     return TCRNET_OK;
 }
 
+// The four launches of the distance step: {chunk kernel, trie kernel} x {32-bit, 64-bit words}.
 struct Schedule {
-    std::vector<WorkRow> narrow, wide;  // pattern length <= 32 / > 32
-    int64_t items_narrow = 0, items_wide = 0;
-    int max_rw_narrow = 4, max_rw_wide = 4;
+    struct Part {
+        std::vector<WorkRow> rows;
+        int64_t items = 0;
+        int max_rw = 4;
+    };
+    Part part[2][2];  // [trie][wide]
+    int first_test = 0;  // trie kernel: first level with an early-exit test (0: trie not used)
 };
 
 // Step A2, host side: the (pattern bucket, text bucket) pairs with len_t - len_p in 0..l_max.
-void make_schedule(const tcrnet_ctx* ctx, int l_max, Schedule& sch, tcrnet_stats& st) {
+void make_schedule(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule& sch, tcrnet_stats& st) {
     const LengthTable& lt = ctx->lt;
     st.pairs_kept = st.cells_kept = st.columns_kept = st.cells_all = 0;
     long double cells_all = 0;
@@ -249,6 +290,10 @@ void make_schedule(const tcrnet_ctx* ctx, int l_max, Schedule& sch, tcrnet_stats
     }
     st.cells_all = (int64_t)cells_all;
     st.pairs_all = ctx->n * (ctx->n - 1) / 2;
+    // The trie kernel serves the rows whose early exit can act inside the trie: first test level
+    // <= kTrieDepth and at least one text column beyond the trie.
+    const bool use_trie = ctx->prefix_trie && first_check >= 3 && first_check <= kTrieDepth;
+    sch.first_test = use_trie ? first_check : 0;
     for (int m = 1; m < kNumLen; ++m) {
         if (!ctx->hist[m]) continue;
         for (int n = m; n <= std::min(kMaxLen, m + l_max); ++n) {
@@ -259,6 +304,7 @@ void make_schedule(const tcrnet_ctx* ctx, int l_max, Schedule& sch, tcrnet_stats
             st.cells_kept += pairs * m * n;
             st.columns_kept += pairs * n;
             if (pairs == 0) continue;
+            const bool trie = use_trie && n > kTrieDepth;
             WorkRow r{};
             r.txt_base = lt.txt_base[n];
             r.p_start = lt.start[m];
@@ -268,35 +314,36 @@ void make_schedule(const tcrnet_ctx* ctx, int l_max, Schedule& sch, tcrnet_stats
             r.m = m;
             r.n = n;
             r.row_words = lt.row_words[n];
-            r.n_tchunks = (int32_t)((tc + ctx->tchunk - 1) / ctx->tchunk);
+            r.tchunk = trie ? ctx->trie_chunk : ctx->tchunk;
+            r.n_tchunks = (int32_t)((tc + r.tchunk - 1) / r.tchunk);
             r.diag = (m == n) ? 1 : 0;
-            (m <= 32 ? sch.narrow : sch.wide).push_back(r);
+            r.root_begin = ctx->trie_root[n];
+            r.root_end = ctx->trie_root[n + 1];
+            sch.part[trie ? 1 : 0][m <= 32 ? 0 : 1].rows.push_back(r);
         }
     }
-    auto finish = [&](std::vector<WorkRow>& rows, int64_t& items, int& max_rw) {
-        auto n_items = [](const WorkRow& r) { return (int64_t)((r.p_count + kTQ - 1) / kTQ) * r.n_tchunks; };
-        // big rows first: the small buckets fill the tail of the launch
-        std::stable_sort(rows.begin(), rows.end(), [&](const WorkRow& a, const WorkRow& b) {
-            return (long double)a.p_count * a.t_count * a.n > (long double)b.p_count * b.t_count * b.n;
-        });
-        items = 0;
-        for (WorkRow& r : rows) {
-            r.item_begin = items;
-            items += n_items(r);
-            max_rw = std::max(max_rw, (int)r.row_words);
+    for (auto& by_kernel : sch.part)
+        for (Schedule::Part& part : by_kernel) {
+            auto n_items = [](const WorkRow& r) { return (int64_t)((r.p_count + kTQ - 1) / kTQ) * r.n_tchunks; };
+            // big rows first: the small buckets fill the tail of the launch
+            std::stable_sort(part.rows.begin(), part.rows.end(), [&](const WorkRow& a, const WorkRow& b) {
+                return (long double)a.p_count * a.t_count * a.n > (long double)b.p_count * b.t_count * b.n;
+            });
+            part.items = 0;
+            for (WorkRow& r : part.rows) {
+                r.item_begin = part.items;
+                part.items += n_items(r);
+                part.max_rw = std::max(part.max_rw, (int)r.row_words);
+            }
         }
-    };
-    finish(sch.narrow, sch.items_narrow, sch.max_rw_narrow);
-    finish(sch.wide, sch.items_wide, sch.max_rw_wide);
 }
 
 int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_check, uint64_t cap, int* launches) {
     cudaStream_t s = ctx->stream;
     HostCtrl* dc = d_ctrl(ctx);
-    TRY_CUDA(cudaMemsetAsync(&dc->edge_count, 0, sizeof(unsigned long long) * 4, s));  // edge_count + work[3]
+    TRY_CUDA(cudaMemsetAsync(&dc->edge_count, 0, sizeof(unsigned long long) * 5, s));  // edge_count + work[4]
     DistanceParams p{};
     p.l_max = l_max;
-    p.tchunk = ctx->tchunk;
     p.pat_stride = ctx->pat_stride;
     p.txt = (const uint32_t*)ctx->txt.p;
     p.pat = (const uint8_t*)ctx->pat.p;
@@ -305,18 +352,22 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
     p.edge_count = &dc->edge_count;
     p.edge_cap = cap;
     p.work = dc->work;
+    for (int k = 0; k <= kTrieDepth; ++k) p.trie[k] = ctx->trie_levels.p[k];
     const WorkRow* d_rows = (const WorkRow*)ctx->rows.p;
-    if (!sch.narrow.empty()) {
-        p.rows = d_rows;
-        p.n_rows = (int32_t)sch.narrow.size();
-        TRY_CUDA(launch_distance(p, sch.items_narrow, false, first_check, ctx->count_work != 0, sch.max_rw_narrow, s, launches));
-    }
-    if (!sch.wide.empty()) {
-        p.rows = d_rows + sch.narrow.size();
-        p.n_rows = (int32_t)sch.wide.size();
-        TRY_CUDA(launch_distance(p, sch.items_wide, true, first_check, ctx->count_work != 0, sch.max_rw_wide, s, launches));
-    }
-    TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->edge_count, &dc->edge_count, sizeof(unsigned long long) * 4,
+    for (int trie = 1; trie >= 0; --trie)
+        for (int wide = 0; wide < 2; ++wide) {
+            const Schedule::Part& part = sch.part[trie][wide];
+            if (!part.rows.empty()) {
+                p.rows = d_rows;
+                p.n_rows = (int32_t)part.rows.size();
+                if (trie)
+                    TRY_CUDA(launch_distance_trie(p, part.items, wide != 0, sch.first_test, ctx->count_work != 0, s, launches));
+                else
+                    TRY_CUDA(launch_distance(p, part.items, wide != 0, first_check, ctx->count_work != 0, part.max_rw, s, launches));
+            }
+            d_rows += part.rows.size();
+        }
+    TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->edge_count, &dc->edge_count, sizeof(unsigned long long) * 5,
                              cudaMemcpyDeviceToHost, s));
     TRY_CUDA(cudaStreamSynchronize(s));
     return TCRNET_OK;
@@ -382,7 +433,7 @@ void tcrnet_destroy(tcrnet_ctx* ctx) {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
-    DevBuf* bufs[] = {&ctx->perm, &ctx->pat, &ctx->txt, &ctx->keys_a, &ctx->keys_b, &ctx->split_hist,
+    DevBuf* bufs[] = {&ctx->perm, &ctx->pat, &ctx->txt, &ctx->trie, &ctx->keys_a, &ctx->keys_b, &ctx->split_hist,
                       &ctx->split_hist_scanned, &ctx->scan_scratch, &ctx->rows, &ctx->row_ptr, &ctx->col,
                       &ctx->deg, &ctx->ctrl};
     for (DevBuf* b : bufs) dev_free(ctx, *b);
@@ -465,24 +516,36 @@ int tcrnet_build(tcrnet_ctx* ctx, int l_max, int64_t* n_edges_out) {
     const int64_t n = ctx->n;
 
     // ---- A2: schedule ----
-    Schedule sch;
-    make_schedule(ctx, l_max, sch, st);
-    st.l_max = l_max;
-    st.work_items = sch.items_narrow + sch.items_wide;
     int first_check = 0;
     if (ctx->early_exit) {
         first_check = ctx->first_check_opt ? ctx->first_check_opt : l_max + 2;
         first_check = std::max(3, std::min(8, first_check));
     }
     st.first_check = first_check;
-    const size_t n_rows = sch.narrow.size() + sch.wide.size();
+    Schedule sch;
+    make_schedule(ctx, l_max, first_check, sch, st);
+    st.l_max = l_max;
+    st.work_items = st.work_items_trie = 0;
+    size_t n_rows = 0;
+    for (int trie = 0; trie < 2; ++trie)
+        for (int wide = 0; wide < 2; ++wide) {
+            st.work_items += sch.part[trie][wide].items;
+            if (trie) st.work_items_trie += sch.part[trie][wide].items;
+            n_rows += sch.part[trie][wide].rows.size();
+        }
     TRY(dev_reserve(ctx, ctx->rows, sizeof(WorkRow) * std::max<size_t>(n_rows, 1)));
     TRY_CUDA(cudaEventRecord(ctx->ev[0], s));
-    if (!sch.narrow.empty())
-        TRY_CUDA(cudaMemcpyAsync(ctx->rows.p, sch.narrow.data(), sizeof(WorkRow) * sch.narrow.size(), cudaMemcpyHostToDevice, s));
-    if (!sch.wide.empty())
-        TRY_CUDA(cudaMemcpyAsync((WorkRow*)ctx->rows.p + sch.narrow.size(), sch.wide.data(),
-                                 sizeof(WorkRow) * sch.wide.size(), cudaMemcpyHostToDevice, s));
+    {
+        // same order as run_distance walks them: trie parts first
+        WorkRow* dst = (WorkRow*)ctx->rows.p;
+        for (int trie = 1; trie >= 0; --trie)
+            for (int wide = 0; wide < 2; ++wide) {
+                const std::vector<WorkRow>& rows = sch.part[trie][wide].rows;
+                if (!rows.empty())
+                    TRY_CUDA(cudaMemcpyAsync(dst, rows.data(), sizeof(WorkRow) * rows.size(), cudaMemcpyHostToDevice, s));
+                dst += rows.size();
+            }
+    }
 
     // ---- A3-A5: distances + emission (second pass only if the edge buffer was too small) ----
     int64_t cap = ctx->edge_capacity_opt > 0 ? ctx->edge_capacity_opt : std::max<int64_t>((int64_t)1 << 20, 16 * n);
@@ -504,6 +567,7 @@ int tcrnet_build(tcrnet_ctx* ctx, int l_max, int64_t* n_edges_out) {
     st.lane_columns_exec = (int64_t)ctx->h_ctrl->work[0];
     st.lane_tests_exec = (int64_t)ctx->h_ctrl->work[1];
     st.lane_pairs_exec = (int64_t)ctx->h_ctrl->work[2];
+    st.lane_prefix_tests_exec = (int64_t)ctx->h_ctrl->work[3];
     TRY_CUDA(cudaEventRecord(ctx->ev[1], s));
 
     // ---- A6a: LSD radix sort of the keys (u << 32) | v over the significant bits only ----
@@ -603,6 +667,14 @@ int tcrnet_set_option(tcrnet_ctx* ctx, int option, int64_t value) {
         case TCRNET_OPT_TEXT_CHUNK:
             if (value < kTQ || value % kTQ != 0 || value > (1 << 20)) return TCRNET_ERR_ARG;
             ctx->tchunk = (int)value;
+            return TCRNET_OK;
+        case TCRNET_OPT_PREFIX_TRIE:
+            if (value != 0 && value != 1) return TCRNET_ERR_ARG;
+            ctx->prefix_trie = (int)value;
+            return TCRNET_OK;
+        case TCRNET_OPT_TRIE_CHUNK:
+            if (value < kTQ || value % kTQ != 0 || value > (1 << 24)) return TCRNET_ERR_ARG;
+            ctx->trie_chunk = (int)value;
             return TCRNET_OK;
         default: return TCRNET_ERR_ARG;
     }

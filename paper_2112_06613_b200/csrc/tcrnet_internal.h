@@ -17,6 +17,8 @@ constexpr int kPeqRows = 27;             // 26 residue rows + the zero row
 constexpr int kTQ = 256;                 // patterns per CTA of the distance kernel (8 warps)
 constexpr int kTT = 64;                  // texts staged into shared memory per pipeline stage
 constexpr int kSortPrefix = 6;           // residues of the lexicographic sub-order inside a length bucket
+constexpr int kTrieDepth = kSortPrefix;  // levels 1..kTrieDepth of the prefix trie over each text bucket
+constexpr int kTrieFan = 32;             // staging slots per trie level (a node has <= 27 children + sentinel)
 
 // Per-length layout of the packed sequence tables (filled on the host after the histogram).
 struct LengthTable {
@@ -38,14 +40,30 @@ struct WorkRow {
     int32_t row_words;   // words per text row
     int32_t n_tchunks;   // text chunks per pattern tile
     int32_t diag;        // 1: same bucket, only sorted p < t counts
-    int32_t pad_;
+    int32_t tchunk;      // texts per work item
+    uint32_t root_begin; // trie kernel: the text bucket's level-1 nodes are [root_begin, root_end)
+    uint32_t root_end;
+};
+static_assert(sizeof(WorkRow) == 64, "WorkRow is copied to the device as an array");
+
+// One node of the prefix trie (trie.cu).  Level k holds one node per maximal run of consecutive
+// texts of one length bucket that share their first k residues; the nodes of a level are stored in
+// sorted-text order followed by one sentinel, so node i's ranges end where node i+1's begin.
+struct TrieNode {
+    uint32_t text_begin;   // sorted position of the run's first text
+    uint32_t child_begin;  // first child in level k+1 (level kTrieDepth: = text_begin)
+    uint32_t code;         // residue code at position k-1 of the run's texts (kPadCode past the end)
+    uint32_t pad_;
+};
+static_assert(sizeof(TrieNode) == 16, "TrieNode is read with 128-bit loads");
+struct TrieLevels {
+    TrieNode* p[kTrieDepth + 1];  // [k] = nodes of level k, k = 1..kTrieDepth ([0] unused)
 };
 
 struct DistanceParams {
     const WorkRow* rows;
     int32_t n_rows;
     int32_t l_max;
-    int32_t tchunk;      // texts per work item
     int32_t pat_stride;  // bytes per pattern row
     const uint32_t* txt; // text rows: one 32-bit residue code per column, padded with kPadCode
     const uint8_t* pat;  // pattern rows: one residue code per byte, row = sorted position
@@ -53,7 +71,9 @@ struct DistanceParams {
     unsigned long long* edges;       // keys (min(i,j) << 32) | max(i,j)
     unsigned long long* edge_count;  // device counter (keeps counting beyond capacity)
     unsigned long long edge_cap;
-    unsigned long long* work;        // [3]: lane-columns, lane-tests, lane-visits (COUNT only)
+    unsigned long long* work;        // [4]: lane-columns, lane-tests (4 ALU ops), lane-first-columns,
+                                     //      lane-prefix-tests (3 ALU ops); COUNT only
+    const TrieNode* trie[kTrieDepth + 1];  // trie kernel: nodes of level 1..kTrieDepth ([0] unused)
 };
 
 // ---- launch wrappers (each returns cudaGetLastError(); *launches is incremented per kernel) ----
@@ -65,6 +85,8 @@ cudaError_t exclusive_scan_i32_to_i64(const int32_t* in, int64_t* out, int64_t n
                                       void* scratch, cudaStream_t s, int* launches);
 cudaError_t exclusive_scan_u32(const uint32_t* in, uint32_t* out, int64_t n, void* scratch,
                                cudaStream_t s, int* launches);
+cudaError_t exclusive_scan_u32_total(const uint32_t* in, uint32_t* out /*[n+1]*/, int64_t n, void* scratch,
+                                     cudaStream_t s, int* launches);
 
 // split.cu: one stable counting-sort pass over 8-bit digits.
 int64_t split_num_blocks(int64_t n);
@@ -88,10 +110,27 @@ cudaError_t launch_pack(const uint8_t* residues, const int64_t* offsets, const i
                         const int32_t* perm, int64_t n, const LengthTable& lt, int pat_stride,
                         uint8_t* pat, uint32_t* txt, uint32_t* flags, cudaStream_t s, int* launches);
 
+// trie.cu: prefix trie over the sorted texts (levels 1..kTrieDepth, all length buckets).
+//   lcp8        : scratch, uint8[round_up(n,16) + 16]
+//   tile_counts : scratch, uint32[trie_tiles(n) * 8]
+//   levels.p[k] : level k, capacity trie_level_capacity(n, k) nodes (sentinel included)
+//   counts      : device uint32[8]: [k] = number of nodes of level k (k = 1..kTrieDepth)
+//   root        : device uint32[kNumLen + 1]: [L] = first level-1 node of length bucket L (only the
+//                 entries of non-empty buckets are written)
+int64_t trie_tiles(int64_t n);
+int64_t trie_level_capacity(int64_t n, int level);
+cudaError_t launch_trie_build(const uint32_t* txt, const LengthTable& lt, int64_t n, uint8_t* lcp8,
+                              uint32_t* tile_counts, const TrieLevels& levels, uint32_t* counts, uint32_t* root,
+                              cudaStream_t s, int* launches);
+
 // distance.cu
 size_t distance_smem_bytes(bool wide, int max_row_words);
 cudaError_t launch_distance(const DistanceParams& p, int64_t n_items, bool wide, int first_check,
                             bool count_work, int max_row_words, cudaStream_t s, int* launches);
+// distance_trie.cu: the prefix-trie kernel; first_test (first level with an early-exit test) in 3..kTrieDepth
+size_t distance_trie_smem_bytes(bool wide);
+cudaError_t launch_distance_trie(const DistanceParams& p, int64_t n_items, bool wide, int first_test,
+                                 bool count_work, cudaStream_t s, int* launches);
 
 // csr.cu
 cudaError_t launch_csr(const unsigned long long* sorted_keys, int64_t n_edges, int64_t n, int64_t* row_ptr,

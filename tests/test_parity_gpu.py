@@ -76,9 +76,64 @@ def test_early_exit_and_schedule_do_not_change_the_result(pkg):
         got, st = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_TEXT_CHUNK: 256, pkg.OPT_EDGE_CAPACITY: 100})
         assert st["distance_passes"] == 2
         assert_same_network(got, ref)
-        got, st = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_COUNT_WORK: 1})
+        got, st = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_COUNT_WORK: 1, pkg.OPT_PREFIX_TRIE: 0})
         assert_same_network(got, ref)
         assert 0 < st["lane_columns_exec"] and st["lane_pairs_exec"] >= st["pairs_kept"]
+        assert st["work_items_trie"] == 0
+
+
+def test_prefix_trie_does_not_change_the_result(pkg, oracle):
+    """The prefix-trie kernel (default) against the text-chunk kernel and the oracle: every first
+    test level, tiny trie chunks (chunk borders inside trie nodes), work counters on."""
+    d = generate("cfg2", n=20000)
+    for l_max in (0, 1, 2, 3, 4):
+        ref, st0 = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_PREFIX_TRIE: 0})
+        assert st0["work_items_trie"] == 0
+        got, st = gpu_network(pkg, d.residues, d.lengths, l_max)
+        assert st["work_items_trie"] > 0 and st["trie_nodes"] > d.n
+        assert_same_network(got, ref)
+        for ft in range(3, 7):
+            got, st = gpu_network(pkg, d.residues, d.lengths, l_max,
+                                  {pkg.OPT_FIRST_CHECK: ft, pkg.OPT_TRIE_CHUNK: 256 * ft, pkg.OPT_COUNT_WORK: ft & 1})
+            assert st["first_check"] == ft and st["work_items_trie"] > 0
+            assert_same_network(got, ref)
+            if ft & 1:
+                assert st["lane_prefix_tests_exec"] > 0 and st["lane_columns_exec"] > 0
+    want = oracle.network(d.residues, d.lengths, 2, tier=1)[:3]
+    got, _ = gpu_network(pkg, d.residues, d.lengths, 2)
+    assert_same_network(got, want)
+
+
+def test_prefix_trie_shared_prefixes_and_short_buckets(pkg, oracle):
+    """Real CDR3-beta rows mostly start CASS...: few distinct prefixes, deep shared runs, many
+    duplicates; plus buckets shorter than the trie depth (they take the text-chunk kernel) and a
+    forced first test level with l_max larger than the trie can prune."""
+    rng = np.random.default_rng(23)
+    letters = "ACDEFGHIKLMNPQRSTVWY"
+    strings = []
+    for _ in range(3000):
+        length = int(rng.integers(3, 19))
+        body = "".join(letters[i] for i in rng.integers(0, 20, max(0, length - 4)))
+        s = ("CASS" + body)[:length]
+        strings.append(s)
+        for _ in range(int(rng.integers(0, 3))):
+            t = list(s)
+            k = int(rng.integers(0, 3))
+            q = int(rng.integers(0, len(t)))
+            if k == 0:
+                t[q] = letters[int(rng.integers(0, 20))]
+            elif k == 1:
+                t.insert(q, letters[int(rng.integers(0, 20))])
+            elif len(t) > 1:
+                del t[q]
+            strings.append("".join(t))
+    order = rng.permutation(len(strings))
+    res, ln = from_strings([strings[i] for i in order])
+    for l_max, opts in ((0, {}), (1, {}), (2, {}), (3, {pkg.OPT_TRIE_CHUNK: 256}), (6, {pkg.OPT_FIRST_CHECK: 3})):
+        want = oracle.network(res, ln, l_max, tier=0)[:3]
+        got, st = gpu_network(pkg, res, ln, l_max, opts)
+        assert st["work_items_trie"] > 0
+        assert_same_network(got, want)
 
 
 def test_device_load_equals_host_load(pkg):
