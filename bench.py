@@ -38,9 +38,9 @@ ALU_OPS_FIRST_COLUMN = 3       # the first column of a text needs only 3 (consta
 ALU_OPS_PER_TEST = 4           # 2 LOP3 + IADD3 + ISETP per pair and early-exit test
 ALU_OPS_PER_PREFIX_TEST = 3    # PRMT + LOP3 + ISETP per pair and trie-node exit test (distance_trie.cu)
 ORACLE_SAMPLE_ROWS = 1024
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_distance launch at cfg4, from the ncu --set full
-# capture summarised in profiles/r1_distance_ncu.txt (84.32 MB + 21.21 MB)
-NCU_DRAM_BYTES_PER_LAUNCH = {"cfg4": 105_532_672}
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_distance_trie launch at cfg4, from the ncu --set full
+# capture summarised in profiles/r1b_trie_ncu.txt (95.23 MB + 21.60 MB)
+NCU_DRAM_BYTES_PER_LAUNCH = {"cfg4": 116_831_744}
 
 
 def _peaks():
