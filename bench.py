@@ -36,7 +36,7 @@ ALU_LANES_PER_SM = 64          # INT32 ALU-pipe lanes per SM per clock on sm_100
 ALU_OPS_PER_COLUMN = 7         # LOP3 per pair and text column (distance.cu)
 ALU_OPS_FIRST_COLUMN = 3       # the first column of a text needs only 3 (constant Pv, Mv = 0)
 ALU_OPS_PER_TEST = 4           # 2 LOP3 + IADD3 + ISETP per pair and early-exit test
-ALU_OPS_PER_PREFIX_TEST = 3    # PRMT + LOP3 + ISETP per pair and trie-node exit test (distance_trie.cu)
+ALU_OPS_PER_PREFIX_TEST = 2    # LOP3 + ISETP per pair and DP cell read in a guided expansion (distance_trie.cu)
 ORACLE_SAMPLE_ROWS = 1024
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_distance_trie launch at cfg4, from the ncu --set full
 # capture summarised in profiles/r1b_trie_ncu.txt (95.23 MB + 21.60 MB)

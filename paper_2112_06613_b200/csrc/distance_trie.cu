@@ -10,11 +10,21 @@
 //     neighbours in lexicographic order) walks the trie depth-first.  Entering a level-k node
 //     costs ONE column step (its residue code at position k-1) on top of the parent's (Pv, Mv):
 //     the columns of a shared prefix are computed once per node, not once per text.
-//   * From level FT on (FT = first test level, default l_max + 2) every node is followed by the
-//     early-exit test: the cell D[k - delta][k] of the final diagonal is a lower bound of
-//     lev(pattern, text) for EVERY text below the node, so if it exceeds l_max in all 32 lanes
-//     the whole subtree is skipped.  PAPER.md:326 ("abort, as soon as the smallest intermediate
-//     result exceeds" l_max) - here one abort disposes of a whole run of texts.
+//   * Early exit: the cell D[k - delta][k] of the final diagonal is a lower bound of
+//     lev(pattern, text) for EVERY text below a level-k node, so a node where it exceeds l_max in
+//     all 32 lanes is dead with its whole subtree.  PAPER.md:326 ("abort, as soon as the smallest
+//     intermediate result exceeds" l_max) - here one abort disposes of a whole run of texts.
+//   * Dead children are not even visited ("guided expansion"; levels k <= l_max have no dead
+//     children and are walked in full): before a node's children are walked, every lane derives from
+//     its parent column (Pv, Mv) the exact set V of residue codes c whose child would be alive,
+//         D_c[i][k] = min( D_0[i][k],  min over rows r <= i with a_r = c of D[r-1][k-1] + (i - r) ),
+//     (i = k - delta; D_0 = the column of a code that matches nowhere), i.e.
+//         V = (all codes, if D_0[i][k] <= l_max)  |  { a_(i-t) : D[i-1-t][k-1] + 2t <= l_max, t = 0..l_max }
+//     with D_0[i][k] <= l_max  <=>  D[i][k-1] <= l_max - 1  or  D[i-1-u][k-1] <= l_max - 1 - 2u for
+//     some u in 0..l_max-1.  Each cell costs one LOP3 + POPC + compare.  The warp visits the
+//     children whose code is in the OR of the 32 lanes' V (one REDUX) and in the node's child-code
+//     bitmap; the child's slot is popc(bitmap & low(code)).  V is exact, so no per-child test is
+//     needed.
 //   * Texts below a surviving level-kTrieDepth node are finished column by column from the node's
 //     state (a test after every second column), then the distance is read off Pv / Mv and
 //     surviving pairs are emitted as in distance.cu.
@@ -25,15 +35,16 @@
 // staged in a per-warp, per-level shared-memory buffer; the walk then reads them with broadcast
 // LDS.128.
 //
-// The prefix test needs one POPC: with v = (Pv & 0xffff) | (Mv << 16) (one PRMT) and
-// x = (v ^ 0xffff0000) & (mask | mask << 16), popc(x) = popc(Pv & mask) + (k - delta) - popc(Mv & mask),
-// hence  k + popc(Pv & mask) - popc(Mv & mask) > l_max  <=>  popc(x) > l_max - delta  for every level.
+// A cell needs one POPC: with v = ((Pv & 0xffff) | (Mv << 16)) ^ 0xffff0000 (PRMT + LOP3, once per
+// node) and mask2(r) = low(r) in both halves, popc(v & mask2(r)) = popc(Pv & low(r)) + r - popc(Mv & low(r))
+// = D[r][k-1] - (k-1) + r, so for r = i-1-u:  D[r][k-1] = popc(v & mask2(r)) + delta + u.
 #include "myers.cuh"
 
 namespace tcrnet {
 namespace {
 
 constexpr uint32_t kFull = 0xffffffffu;
+constexpr int kClipLevels = 3;  // levels whose nodes are clipped to the work item's text chunk
 
 template <typename W, bool COUNT>
 struct Walk {
@@ -42,10 +53,12 @@ struct Walk {
     uint32_t lane_addr;       // shared address of this lane's Peq column
     uint32_t t_start;         // sorted position of the bucket's first text
     uint32_t lo, hi;          // texts [lo, hi) (sorted positions) are this warp's share of the bucket
-    uint32_t mask2[kTrieDepth + 1];  // per level: low(k - delta) in both halves (0: no test possible)
+    uint32_t mask2[kTrieDepth + 1];  // [q] = low(q - delta) in both 16-bit halves (0 when q <= delta)
+    uint32_t ohs[kTrieDepth + 1];    // [q] = 1 << code of pattern row q - delta (0: no such row / no pattern)
     W pv_init, x_init, m_mask;
     int rw, n, delta;
     int thr;                  // l_max - delta; -1 in lanes without a pattern
+    int l_max;                // warp-uniform
     int l_max_lane;           // l_max; -1 in lanes without a pattern
     int lane, p_sorted, diag;
     unsigned long long n_cols = 0, n_tests = 0, n_first = 0, n_ptests = 0;
@@ -85,22 +98,47 @@ __device__ __forceinline__ void finish_texts(Walk<W, COUNT>& w, const DistancePa
 }
 
 // Expand the level-LEVEL nodes [cb, ce) (the children of one level-(LEVEL-1) node, or the roots of
-// the text bucket); (Pv, Mv) is the DP column after LEVEL-1 text residues.
-template <typename W, int FT, bool COUNT, int LEVEL>
+// the text bucket) whose residue codes are the set bits of cm; (Pv, Mv) is the DP column after
+// LEVEL-1 text residues.
+template <typename W, bool COUNT, int LEVEL>
 __device__ __forceinline__ void visit(Walk<W, COUNT>& w, const DistanceParams& P, uint32_t cb, uint32_t ce,
-                                      const W Pv, const W Mv) {
+                                      uint32_t cm, const W Pv, const W Mv) {
+    uint32_t U = cm;
+    // Guided expansion: the codes whose child is alive in at least one lane.  Every child is alive
+    // while LEVEL <= l_max (D[i][k] <= k), and there is no final-diagonal cell while LEVEL <= delta.
+    if (LEVEL > w.l_max && LEVEL > w.delta) {  // warp-uniform
+        const uint32_t v = __byte_perm((uint32_t)Pv, (uint32_t)Mv, 0x5410) ^ 0xffff0000u;
+        bool alive0 = __popc(v & w.mask2[LEVEL]) <= w.thr;  // D[i][k-1] <= l_max - 1
+        uint32_t V = 0u;
+#pragma unroll
+        for (int t = 0; t < LEVEL; ++t) {
+            if (t <= w.l_max) {  // warp-uniform
+                const int pt = __popc(v & w.mask2[LEVEL - 1 - t]);  // D[i-1-t][k-1] - delta - t
+                alive0 = alive0 || (pt <= w.thr - 1 - 2 * t);
+                if (pt <= w.thr - 2 * t) V |= w.ohs[LEVEL - t];
+                if (COUNT) ++w.n_ptests;
+            }
+        }
+        if (COUNT) ++w.n_ptests;
+        if (alive0) V = kFull;
+        U = __reduce_or_sync(kFull, V) & cm;
+        if (U == 0u) return;
+    }
     uint4* sb = w.stage + (LEVEL - 1) * kTrieFan;
     const int cnt = (int)(ce - cb);  // <= 27 by construction
     __syncwarp();
     if (w.lane <= cnt) sb[w.lane] = __ldg(reinterpret_cast<const uint4*>(P.trie[LEVEL]) + cb + w.lane);
     __syncwarp();
-    for (int i = 0; i < cnt; ++i) {
-        const uint4 nd = sb[i];  // text_begin, child_begin, code
-        if (LEVEL < FT) {        // clip the cheap upper levels to this warp's texts
-            const uint32_t text_end = sb[i + 1].x;
-            if (text_end <= w.lo || nd.x >= w.hi) continue;
+    do {
+        const uint32_t c = (uint32_t)__ffs((int)U) - 1u;
+        U &= U - 1u;
+        const int i = __popc(cm & ((1u << c) - 1u));
+        const uint4 nd = sb[i];      // text_begin, child_begin, code (= c), child codes
+        const uint4 nx = sb[i + 1];
+        if (LEVEL <= kClipLevels) {  // clip the upper levels to this warp's texts
+            if (nx.x <= w.lo || nd.x >= w.hi) continue;
         }
-        const W Eq = peq_load<W>(w.lane_addr, nd.z);
+        const W Eq = peq_load<W>(w.lane_addr, c);
         W P2 = Pv, M2 = Mv;
         if (LEVEL == 1) {
             first_column_step<W>(Eq, w.pv_init, w.x_init, P2, M2);
@@ -109,23 +147,16 @@ __device__ __forceinline__ void visit(Walk<W, COUNT>& w, const DistanceParams& P
             column_step<W>(Eq, P2, M2);
         }
         if (COUNT) ++w.n_cols;
-        if (LEVEL >= FT) {
-            const uint32_t v = __byte_perm((uint32_t)P2, (uint32_t)M2, 0x5410);
-            const uint32_t x = (v ^ 0xffff0000u) & w.mask2[LEVEL];
-            if (COUNT) ++w.n_ptests;
-            if (!__any_sync(kFull, __popc(x) <= w.thr)) continue;
-        }
-        const uint4 nx = sb[i + 1];
         if constexpr (LEVEL < kTrieDepth) {
-            visit<W, FT, COUNT, LEVEL + 1>(w, P, nd.y, nx.y, P2, M2);
+            visit<W, COUNT, LEVEL + 1>(w, P, nd.y, nx.y, nd.w, P2, M2);
         } else {
             const uint32_t t0 = max(nd.x, w.lo), t1 = min(nx.x, w.hi);
             if (t0 < t1) finish_texts<W, COUNT>(w, P, t0, t1, P2, M2);
         }
-    }
+    } while (U);
 }
 
-template <typename W, int FT, bool COUNT>
+template <typename W, bool COUNT>
 __global__ void __launch_bounds__(kTQ) k_distance_trie(const __grid_constant__ DistanceParams P) {
     extern __shared__ __align__(16) unsigned char smem[];
     constexpr int kRowBytes = peq_row_bytes<W>();
@@ -166,6 +197,18 @@ __global__ void __launch_bounds__(kTQ) k_distance_trie(const __grid_constant__ D
     w.hi = (uint32_t)(R.t_start + hi_rel);
 #pragma unroll
     for (int k = 0; k <= kTrieDepth; ++k) w.mask2[k] = k > delta ? ((1u << (k - delta)) - 1u) * 0x10001u : 0u;
+    {
+        // one-hot codes of the pattern's first rows, shifted by delta: ohs[q] belongs to row q - delta
+        const uint8_t* prow = P.pat + (size_t)(R.p_start + p_rel) * P.pat_stride;
+        const uint2 head = p_valid ? __ldg(reinterpret_cast<const uint2*>(prow)) : make_uint2(0xffffffffu, 0xffffffffu);
+#pragma unroll
+        for (int q = 0; q <= kTrieDepth; ++q) {
+            const int r = q - delta;  // 1-based pattern row
+            uint32_t code = 0xffu;
+            if (r >= 1 && r <= m) code = ((r <= 4 ? head.x : head.y) >> (8 * ((r - 1) & 3))) & 0xffu;
+            w.ohs[q] = code < 32u ? 1u << code : 0u;
+        }
+    }
     w.pv_init = low_mask<W>(m);
     w.x_init = w.pv_init + w.pv_init;
     w.m_mask = w.pv_init;
@@ -174,11 +217,19 @@ __global__ void __launch_bounds__(kTQ) k_distance_trie(const __grid_constant__ D
     w.delta = delta;
     w.thr = p_valid ? P.l_max - delta : -1;
     w.l_max_lane = p_valid ? P.l_max : -1;
+    w.l_max = P.l_max;
     w.lane = lane;
     w.p_sorted = R.p_start + p_rel;
     w.diag = R.diag;
 
-    visit<W, FT, COUNT, 1>(w, P, R.root_begin, R.root_end, w.pv_init, W(0));
+    // codes of the bucket's level-1 nodes
+    uint32_t root_codes = 0u;
+    {
+        const int cnt = (int)(R.root_end - R.root_begin);
+        if (lane < cnt) root_codes = 1u << (P.trie[1][R.root_begin + lane].code & 31u);
+        root_codes = __reduce_or_sync(kFull, root_codes);
+    }
+    visit<W, COUNT, 1>(w, P, R.root_begin, R.root_end, root_codes, w.pv_init, W(0));
 
     if (COUNT) {
         // warp-level counters (identical in all lanes): lane 0 reports 32 lanes' worth
@@ -191,24 +242,13 @@ __global__ void __launch_bounds__(kTQ) k_distance_trie(const __grid_constant__ D
     }
 }
 
-template <typename W, int FT, bool COUNT>
+template <typename W, bool COUNT>
 cudaError_t launch_one(const DistanceParams& p, int64_t n_items, size_t smem, cudaStream_t s) {
-    auto kern = k_distance_trie<W, FT, COUNT>;
+    auto kern = k_distance_trie<W, COUNT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kern<<<(unsigned)n_items, kTQ, smem, s>>>(p);
     return cudaGetLastError();
-}
-
-template <typename W, bool COUNT>
-cudaError_t launch_ft(const DistanceParams& p, int64_t n_items, int ft, size_t smem, cudaStream_t s) {
-    switch (ft) {
-        case 3: return launch_one<W, 3, COUNT>(p, n_items, smem, s);
-        case 4: return launch_one<W, 4, COUNT>(p, n_items, smem, s);
-        case 5: return launch_one<W, 5, COUNT>(p, n_items, smem, s);
-        case 6: return launch_one<W, 6, COUNT>(p, n_items, smem, s);
-        default: return cudaErrorInvalidValue;
-    }
 }
 
 }  // namespace
@@ -218,17 +258,17 @@ size_t distance_trie_smem_bytes(bool wide) {
     return peq + (size_t)(kTQ / 32) * kTrieDepth * kTrieFan * sizeof(uint4);
 }
 
-cudaError_t launch_distance_trie(const DistanceParams& p, int64_t n_items, bool wide, int first_test,
-                                 bool count_work, cudaStream_t s, int* launches) {
+cudaError_t launch_distance_trie(const DistanceParams& p, int64_t n_items, bool wide, bool count_work,
+                                 cudaStream_t s, int* launches) {
     if (n_items <= 0) return cudaSuccess;
     if (n_items > 0x7fffffffLL) return cudaErrorInvalidValue;
     const size_t smem = distance_trie_smem_bytes(wide);
     *launches += 1;
     if (wide)
-        return count_work ? launch_ft<uint64_t, true>(p, n_items, first_test, smem, s)
-                          : launch_ft<uint64_t, false>(p, n_items, first_test, smem, s);
-    return count_work ? launch_ft<uint32_t, true>(p, n_items, first_test, smem, s)
-                      : launch_ft<uint32_t, false>(p, n_items, first_test, smem, s);
+        return count_work ? launch_one<uint64_t, true>(p, n_items, smem, s)
+                          : launch_one<uint64_t, false>(p, n_items, smem, s);
+    return count_work ? launch_one<uint32_t, true>(p, n_items, smem, s)
+                      : launch_one<uint32_t, false>(p, n_items, smem, s);
 }
 
 }  // namespace tcrnet

@@ -361,7 +361,7 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
                 p.rows = d_rows;
                 p.n_rows = (int32_t)part.rows.size();
                 if (trie)
-                    TRY_CUDA(launch_distance_trie(p, part.items, wide != 0, sch.first_test, ctx->count_work != 0, s, launches));
+                    TRY_CUDA(launch_distance_trie(p, part.items, wide != 0, ctx->count_work != 0, s, launches));
                 else
                     TRY_CUDA(launch_distance(p, part.items, wide != 0, first_check, ctx->count_work != 0, part.max_rw, s, launches));
             }

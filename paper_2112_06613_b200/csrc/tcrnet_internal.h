@@ -53,7 +53,7 @@ struct TrieNode {
     uint32_t text_begin;   // sorted position of the run's first text
     uint32_t child_begin;  // first child in level k+1 (level kTrieDepth: = text_begin)
     uint32_t code;         // residue code at position k-1 of the run's texts (kPadCode past the end)
-    uint32_t pad_;
+    uint32_t child_codes;  // bit c set iff a child with residue code c exists (levels < kTrieDepth)
 };
 static_assert(sizeof(TrieNode) == 16, "TrieNode is read with 128-bit loads");
 struct TrieLevels {
@@ -127,10 +127,10 @@ cudaError_t launch_trie_build(const uint32_t* txt, const LengthTable& lt, int64_
 size_t distance_smem_bytes(bool wide, int max_row_words);
 cudaError_t launch_distance(const DistanceParams& p, int64_t n_items, bool wide, int first_check,
                             bool count_work, int max_row_words, cudaStream_t s, int* launches);
-// distance_trie.cu: the prefix-trie kernel; first_test (first level with an early-exit test) in 3..kTrieDepth
+// distance_trie.cu: the prefix-trie kernel
 size_t distance_trie_smem_bytes(bool wide);
-cudaError_t launch_distance_trie(const DistanceParams& p, int64_t n_items, bool wide, int first_test,
-                                 bool count_work, cudaStream_t s, int* launches);
+cudaError_t launch_distance_trie(const DistanceParams& p, int64_t n_items, bool wide, bool count_work,
+                                 cudaStream_t s, int* launches);
 
 // csr.cu
 cudaError_t launch_csr(const unsigned long long* sorted_keys, int64_t n_edges, int64_t n, int64_t* row_ptr,

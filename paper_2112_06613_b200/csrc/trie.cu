@@ -16,6 +16,8 @@
 //   k_trie_count  per tile of 4096 positions, the number of run starts of every level.
 //   k_trie_scan   exclusive scan of the tile counts (one CTA), totals, sentinels.
 //   k_trie_emit   node ids by ranking inside the tile; writes the nodes.
+//   k_trie_child_codes  per node of levels 1..kTrieDepth-1, the bitmap of its children's residue codes
+//                 (the guided expansion of distance_trie.cu addresses a child by popc(bitmap & low(code))).
 #include "tcrnet_internal.h"
 
 namespace tcrnet {
@@ -182,7 +184,7 @@ __global__ void __launch_bounds__(1024) k_trie_scan(uint32_t* __restrict__ tile_
         sentinel.text_begin = (uint32_t)n;
         sentinel.child_begin = k < kTrieDepth ? carry[k + 1] : (uint32_t)n;
         sentinel.code = (uint32_t)kPadCode;
-        sentinel.pad_ = 0u;
+        sentinel.child_codes = 0u;
         lv.p[k][carry[k]] = sentinel;
     }
 }
@@ -235,7 +237,7 @@ __global__ void __launch_bounds__(kThreads) k_trie_emit(const uint32_t* __restri
                 nd.text_begin = (uint32_t)s;
                 nd.child_begin = id[k + 1];
                 nd.code = k - 1 < len ? row[k - 1] : (uint32_t)kPadCode;
-                nd.pad_ = 0u;
+                nd.child_codes = 0u;
                 level_nodes[k][id[k]] = nd;
             }
         }
@@ -243,6 +245,20 @@ __global__ void __launch_bounds__(kThreads) k_trie_emit(const uint32_t* __restri
         for (int k = 1; k <= kTrieDepth; ++k)
             if (lcp < (uint32_t)k) ++id[k];
     }
+}
+
+// blockIdx.y + 1 = level k; thread = node of level k; OR of the codes of its children in level k+1.
+__global__ void __launch_bounds__(kThreads) k_trie_child_codes(const __grid_constant__ TrieLevels lv,
+                                                              const uint32_t* __restrict__ counts) {
+    const int k = blockIdx.y + 1;
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= counts[k]) return;
+    TrieNode* nodes = lv.p[k];
+    const TrieNode* kids = lv.p[k + 1];
+    const uint32_t b = nodes[i].child_begin, e = nodes[i + 1].child_begin;  // i + 1 may be the sentinel
+    uint32_t codes = 0u;
+    for (uint32_t c = b; c < e; ++c) codes |= 1u << (kids[c].code & 31u);
+    nodes[i].child_codes = codes;
 }
 
 }  // namespace
@@ -264,7 +280,8 @@ cudaError_t launch_trie_build(const uint32_t* txt, const LengthTable& lt, int64_
     k_trie_count<<<(unsigned)tiles, kThreads, 0, s>>>(lcp8, n, tile_counts);
     k_trie_scan<<<1, 1024, 0, s>>>(tile_counts, tiles, n, lv, counts);
     k_trie_emit<<<(unsigned)tiles, kThreads, 0, s>>>(txt, lt, n, lcp8, tile_counts, lv, root);
-    *launches += 4;
+    k_trie_child_codes<<<dim3((unsigned)((n + kThreads - 1) / kThreads), kTrieDepth - 1), kThreads, 0, s>>>(lv, counts);
+    *launches += 5;
     return cudaGetLastError();
 }
 
