@@ -202,10 +202,19 @@ def main() -> None:
         net.load(d_res, d_len)
         return net.build(l_max)
 
+    e2e_split = [0.0, 0.0, 0.0]
+
     def step_host():
+        t0 = time.perf_counter()
         net.load(h_res.numpy(), h_len.numpy())
+        t1 = time.perf_counter()
         net.build(l_max)
-        return net.copy_csr()
+        t2 = time.perf_counter()
+        out = net.copy_csr(staged=True)  # page-locked result buffers owned by the binding
+        t3 = time.perf_counter()
+        for i, dt in enumerate((t1 - t0, t2 - t1, t3 - t2)):
+            e2e_split[i] += dt
+        return out
 
     # work accounting pass (instrumented kernel, outside every timed region)
     net.set_option(pkg.OPT_COUNT_WORK, 1)
@@ -238,6 +247,7 @@ def main() -> None:
     for _ in range(2):
         step_host()
     barrier()
+    e2e_split[:] = [0.0, 0.0, 0.0]
     e2e_times = []
     for k in range(args.steps):
         flush.fill_(k)
@@ -283,7 +293,8 @@ def main() -> None:
             },
             "clocks": clocks,
             "e2e": {"value": world * pairs_all / (ms_e2e * 1e-3), "unit": "pairs/s", "ms_per_step": ms_e2e,
-                    "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+                    "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "ms_load_build_copy": [1e3 * x / args.steps for x in e2e_split]},
             "gpu_launches": int(sum(s["launches_load"] + s["launches_build"] for s in stats)),
             "roofline": {
                 "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TIOP/s (INT32 ALU-pipe lane-ops)",

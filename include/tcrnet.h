@@ -98,8 +98,16 @@ typedef enum tcrnet_option {
                                      whole runs of texts skipped by one exit test); 0: every kept
                                      pair is visited by the text-chunk kernel.  Never changes the
                                      result.                                                   */
-    TCRNET_OPT_TRIE_CHUNK = 8     /* texts per work item of the prefix-trie kernel (multiple of
+    TCRNET_OPT_TRIE_CHUNK = 8,    /* texts per work item of the prefix-trie kernel (multiple of
                                      256; default 32768)                                       */
+    TCRNET_OPT_N_QUERY = 9        /* rectangular (query x repertoire) mode: the
+                                     antigen-specific network "replaces the first N_a rows" by
+                                     antigen-cognate sequences and analyses only those nodes.
+                                     n_q > 0: rows 0..n_q-1 of the next tcrnet_load are the query
+                                     rows and builds keep only the edges with at least one query
+                                     endpoint (query-query and query-repertoire); pairs of two
+                                     non-query rows are never evaluated.  0 (default): all pairs.
+                                     Takes effect at the next tcrnet_load.                      */
 } tcrnet_option;
 
 /* Work and timing of the last tcrnet_load / tcrnet_build (tcrnet_get_stats). */
@@ -179,6 +187,46 @@ TCRNET_API int tcrnet_load_device(tcrnet_ctx* ctx, const uint8_t* residues_dev, 
  * Errors: STATE (no load), LMAX, NOMEM, EDGE_OVERFLOW, CUDA.
  */
 TCRNET_API int tcrnet_build(tcrnet_ctx* ctx, int l_max, int64_t* n_edges_out);
+
+/*
+ * Step 8(e), multi-GPU sharding: steps A2-A5 for the work items  shard + k * n_shards  only
+ * (interleaved, so that every shard gets the same mix of large and small length buckets).
+ * Every rank loads the same sequences and calls this with its own `shard`; the union over
+ * shard = 0..n_shards-1 of the emitted keys is exactly the edge set, each edge in exactly one
+ * shard.  *keys_dev (may be NULL) -> device uint64[*n_keys_out], unsorted, key = (i << 32) | j
+ * with i < j the caller's row indices; owned by the context, valid until the next build /
+ * assemble / restrict / load.  No CSR is produced: exchange the keys (all-gather over NCCL) and
+ * call tcrnet_assemble.  Errors: ARG (shard outside 0..n_shards-1), STATE, LMAX, NOMEM,
+ * EDGE_OVERFLOW, CUDA.
+ */
+TCRNET_API int tcrnet_build_shard(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, const uint64_t** keys_dev,
+                                  int64_t* n_keys_out);
+
+/*
+ * Step A6 on an edge list supplied by the caller: sort the n_keys keys (i << 32) | j (device
+ * uint64, any order, each edge once, i < j < n) and build CSR + degrees as tcrnet_build does
+ * (PAPER.md:301-318, 224).  keys_dev is copied unless it is the pointer tcrnet_build_shard
+ * returned (then the sort runs in place).  Errors: ARG (a key with i >= j or j >= n), STATE
+ * (no load), NOMEM, EDGE_OVERFLOW, CUDA.
+ */
+TCRNET_API int tcrnet_assemble(tcrnet_ctx* ctx, const uint64_t* keys_dev, int64_t n_keys, int64_t* n_edges_out);
+
+/*
+ * Distance labels: *dist_dev -> device uint8[|E|], dist[e] = Levenshtein
+ * distance of the two endpoints of edge e of the current CSR (aligned with
+ * col).  Computed on first use after a build.  NULL when |E| = 0.  Same lifetime as tcrnet_csr.
+ * Errors: ARG, STATE, NOMEM, CUDA.
+ */
+TCRNET_API int tcrnet_edge_distances(tcrnet_ctx* ctx, const uint8_t** dist_dev);
+
+/*
+ * Threshold sweep without re-evaluating pairs (Fig. 2(i): the largest component
+ * as a function of l_max): replace the current network, built at threshold L, by the network at
+ * l_max <= L, i.e. keep the edges with distance label <= l_max and rebuild row_ptr / col /
+ * degrees (and the labels).  The result equals tcrnet_build(l_max) bit for bit.  May be chained
+ * with decreasing l_max.  Errors: STATE (no build), LMAX (l_max < 0 or > L), NOMEM, CUDA.
+ */
+TCRNET_API int tcrnet_restrict(tcrnet_ctx* ctx, int l_max, int64_t* n_edges_out);
 
 /*
  * Borrow the CSR of the last build: *row_ptr_dev -> device int64[n+1], *col_dev -> device

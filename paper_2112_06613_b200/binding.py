@@ -21,12 +21,13 @@ LIB_PATH = os.path.join(_HERE, "libtcrnet_b200.so")
 OK, ERR_ARG, ERR_LENGTH, ERR_RESIDUE, ERR_LMAX, ERR_STATE, ERR_NOMEM, ERR_EDGE_OVERFLOW, ERR_CUDA = (
     0, -1, -2, -3, -4, -5, -6, -7, -8)
 OPT_EARLY_EXIT, OPT_FIRST_CHECK, OPT_EDGE_CAPACITY, OPT_EDGE_LIMIT, OPT_COUNT_WORK, OPT_TEXT_CHUNK = 1, 2, 3, 4, 5, 6
-OPT_PREFIX_TRIE, OPT_TRIE_CHUNK = 7, 8
+OPT_PREFIX_TRIE, OPT_TRIE_CHUNK, OPT_N_QUERY = 7, 8, 9
 
 EXPORTS = (
     "tcrnet_create", "tcrnet_destroy", "tcrnet_load", "tcrnet_load_device", "tcrnet_build", "tcrnet_csr",
     "tcrnet_degrees", "tcrnet_copy_csr", "tcrnet_set_option", "tcrnet_get_stats", "tcrnet_probe_int32",
-    "tcrnet_last_cuda_error", "tcrnet_strerror", "tcrnet_version",
+    "tcrnet_last_cuda_error", "tcrnet_strerror", "tcrnet_version", "tcrnet_build_shard", "tcrnet_assemble",
+    "tcrnet_edge_distances", "tcrnet_restrict",
 )
 
 
@@ -79,6 +80,14 @@ def load_library() -> C.CDLL:
     lib.tcrnet_load_device.argtypes = [vp, vp, vp, C.c_int64, C.c_int64]
     lib.tcrnet_build.restype = C.c_int
     lib.tcrnet_build.argtypes = [vp, C.c_int, i64p]
+    lib.tcrnet_build_shard.restype = C.c_int
+    lib.tcrnet_build_shard.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.POINTER(vp), i64p]
+    lib.tcrnet_assemble.restype = C.c_int
+    lib.tcrnet_assemble.argtypes = [vp, vp, C.c_int64, i64p]
+    lib.tcrnet_edge_distances.restype = C.c_int
+    lib.tcrnet_edge_distances.argtypes = [vp, C.POINTER(vp)]
+    lib.tcrnet_restrict.restype = C.c_int
+    lib.tcrnet_restrict.argtypes = [vp, C.c_int, i64p]
     lib.tcrnet_csr.restype = C.c_int
     lib.tcrnet_csr.argtypes = [vp, C.POINTER(vp), C.POINTER(vp)]
     lib.tcrnet_degrees.restype = C.c_int
@@ -127,6 +136,7 @@ class TcrNet:
         self.device = torch.device("cuda", device)
         self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self._blocks: Dict[int, "torch.Tensor"] = {}
+        self._staging: Dict[str, "torch.Tensor"] = {}  # page-locked host buffers of copy_csr(staged=True)
 
         def _alloc(_user, nbytes):
             try:
@@ -186,7 +196,7 @@ class TcrNet:
             residues = np.ascontiguousarray(residues, dtype=np.uint8)
             lengths = np.ascontiguousarray(lengths, dtype=np.int32)
             n = int(lengths.size)
-            if n >= 1 and int(lengths.astype(np.int64).clip(min=0).sum()) > residues.size:
+            if n >= 1 and int(np.maximum(lengths, 0).sum(dtype=np.int64)) > residues.size:
                 raise TcrNetError(ERR_ARG, "tcrnet_load (residues shorter than sum(lengths))")
             _check(self._lib.tcrnet_load(self._ctx, residues.ctypes.data_as(C.POINTER(C.c_uint8)),
                                          lengths.ctypes.data_as(C.POINTER(C.c_int32)), n), "tcrnet_load")
@@ -196,6 +206,44 @@ class TcrNet:
     def build(self, l_max: int) -> int:
         e = C.c_int64(0)
         _check(self._lib.tcrnet_build(self._ctx, int(l_max), C.byref(e)), "tcrnet_build")
+        self.n_edges = int(e.value)
+        return self.n_edges
+
+    def build_shard(self, l_max: int, shard: int, n_shards: int) -> "torch.Tensor":
+        """tcrnet_build_shard: this shard's edge keys (i << 32) | j as an int64 CUDA tensor (a view of
+        library memory, valid until the next build / assemble / restrict / load)."""
+        torch = self._torch
+        keys, e = C.c_void_p(), C.c_int64(0)
+        _check(self._lib.tcrnet_build_shard(self._ctx, int(l_max), int(shard), int(n_shards), C.byref(keys),
+                                            C.byref(e)), "tcrnet_build_shard")
+        self.n_edges = 0
+        if not e.value:
+            return torch.empty(0, dtype=torch.int64, device=self.device)
+        return self._view(keys.value, torch.int64, int(e.value))
+
+    def assemble(self, keys: "torch.Tensor") -> int:
+        """tcrnet_assemble: CSR + degrees from an int64 CUDA tensor of keys (i << 32) | j."""
+        torch = self._torch
+        assert keys.is_cuda and keys.dtype == torch.int64
+        keys = keys.contiguous()
+        e = C.c_int64(0)
+        _check(self._lib.tcrnet_assemble(self._ctx, C.c_void_p(keys.data_ptr() if keys.numel() else 0),
+                                         int(keys.numel()), C.byref(e)), "tcrnet_assemble")
+        self.n_edges = int(e.value)
+        return self.n_edges
+
+    def edge_distances(self) -> "torch.Tensor":
+        """tcrnet_edge_distances: uint8[E] aligned with col (a view of library memory)."""
+        torch = self._torch
+        d = C.c_void_p()
+        _check(self._lib.tcrnet_edge_distances(self._ctx, C.byref(d)), "tcrnet_edge_distances")
+        if not d.value:
+            return torch.empty(0, dtype=torch.uint8, device=self.device)
+        return self._view(d.value, torch.uint8, self.n_edges)
+
+    def restrict(self, l_max: int) -> int:
+        e = C.c_int64(0)
+        _check(self._lib.tcrnet_restrict(self._ctx, int(l_max), C.byref(e)), "tcrnet_restrict")
         self.n_edges = int(e.value)
         return self.n_edges
 
@@ -219,11 +267,25 @@ class TcrNet:
         _check(self._lib.tcrnet_degrees(self._ctx, C.byref(dg)), "tcrnet_degrees")
         return self._view(dg.value, self._torch.int32, self.n)
 
-    def copy_csr(self, row_ptr: bool = True, col: bool = True, deg: bool = True):
-        """tcrnet_copy_csr into fresh numpy arrays: (row_ptr, col, deg) (None where skipped)."""
-        rp = np.empty(self.n + 1, dtype=np.int64) if row_ptr else None
-        cl = np.empty(self.n_edges, dtype=np.int32) if col else None
-        dg = np.empty(self.n, dtype=np.int32) if deg else None
+    def _host(self, name: str, count: int, dtype, staged: bool):
+        if not staged:
+            return np.empty(count, dtype=dtype)
+        nbytes = max(count, 1) * np.dtype(dtype).itemsize
+        t = self._staging.get(name)
+        if t is None or t.numel() < nbytes:
+            t = self._torch.empty(nbytes + nbytes // 4, dtype=self._torch.uint8, pin_memory=True)
+            self._staging[name] = t
+        return t.numpy()[:count * np.dtype(dtype).itemsize].view(dtype)
+
+    def copy_csr(self, row_ptr: bool = True, col: bool = True, deg: bool = True, staged: bool = False):
+        """tcrnet_copy_csr into numpy arrays: (row_ptr, col, deg) (None where skipped).
+
+        staged=False: fresh pageable arrays.  staged=True: views of page-locked staging buffers
+        owned by this object and reused by the next staged call (the device-to-host copy then runs
+        at full PCIe rate; the caller must be done with them before calling again)."""
+        rp = self._host("row_ptr", self.n + 1, np.int64, staged) if row_ptr else None
+        cl = self._host("col", self.n_edges, np.int32, staged) if col else None
+        dg = self._host("deg", self.n, np.int32, staged) if deg else None
         _check(self._lib.tcrnet_copy_csr(
             self._ctx,
             rp.ctypes.data_as(C.POINTER(C.c_int64)) if rp is not None else None,

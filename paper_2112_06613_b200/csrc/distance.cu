@@ -37,7 +37,7 @@ __global__ void __launch_bounds__(kTQ) k_distance(const __grid_constant__ Distan
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
     // ---- step A2, device side: which (bucket pair, pattern tile, text chunk) is this CTA? ----
-    const int64_t item = blockIdx.x;
+    const int64_t item = work_item(P);
     const WorkRow R = find_row(P, item);
     const int64_t local = item - R.item_begin;
     const int pi = (int)(local / R.n_tchunks), qi = (int)(local % R.n_tchunks);
@@ -119,7 +119,7 @@ __global__ void __launch_bounds__(kTQ) k_distance(const __grid_constant__ Distan
             const int d = n + WordOps<W>::popc(Pv & m_mask) - WordOps<W>::popc(Mv & m_mask);
             const int t_rel = sub_t0 + tt;
             const bool edge = d <= l_max && p_valid && (!R.diag || p_rel < t_rel);
-            emit_edges(P, edge, lane, R.p_start + p_rel, R.t_start + t_rel);
+            emit_edges(P, edge, lane, R.p_start + p_rel, R.t_start + t_rel, m, n);
         };
         if (hot) {
             // ---- hot loop: 1-2 broadcast LDS.128, FIRST unrolled columns, one warp-wide test ----
@@ -150,7 +150,7 @@ cudaError_t launch_one(const DistanceParams& p, int64_t n_items, size_t smem, cu
     auto kern = k_distance<W, FIRST, COUNT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    kern<<<(unsigned)n_items, kTQ, smem, s>>>(p);
+    kern<<<(unsigned)((n_items - p.shard + p.n_shards - 1) / p.n_shards), kTQ, smem, s>>>(p);
     return cudaGetLastError();
 }
 
@@ -177,7 +177,7 @@ size_t distance_smem_bytes(bool wide, int max_row_words) {
 
 cudaError_t launch_distance(const DistanceParams& p, int64_t n_items, bool wide, int first_check, bool count_work,
                             int max_row_words, cudaStream_t s, int* launches) {
-    if (n_items <= 0) return cudaSuccess;
+    if (n_items <= p.shard) return cudaSuccess;
     if (n_items > 0x7fffffffLL) return cudaErrorInvalidValue;
     const size_t smem = distance_smem_bytes(wide, max_row_words);
     *launches += 1;

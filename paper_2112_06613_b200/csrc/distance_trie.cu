@@ -93,7 +93,7 @@ __device__ __forceinline__ void finish_texts(Walk<W, COUNT>& w, const DistancePa
         if (dead) continue;
         const int d = w.n + WordOps<W>::popc(Pv & w.m_mask) - WordOps<W>::popc(Mv & w.m_mask);
         const bool edge = d <= w.l_max_lane && (!w.diag || (uint32_t)w.p_sorted < t);
-        emit_edges(P, edge, w.lane, w.p_sorted, (int)t);
+        emit_edges(P, edge, w.lane, w.p_sorted, (int)t, w.n - w.delta, w.n);
     }
 }
 
@@ -167,7 +167,7 @@ __global__ void __launch_bounds__(kTQ) k_distance_trie(const __grid_constant__ D
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
     // ---- step A2, device side: which (bucket pair, pattern tile, text chunk) is this CTA? ----
-    const int64_t item = blockIdx.x;
+    const int64_t item = work_item(P);
     const WorkRow R = find_row(P, item);
     const int64_t local = item - R.item_begin;
     const int pi = (int)(local / R.n_tchunks), qi = (int)(local % R.n_tchunks);
@@ -247,7 +247,7 @@ cudaError_t launch_one(const DistanceParams& p, int64_t n_items, size_t smem, cu
     auto kern = k_distance_trie<W, COUNT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    kern<<<(unsigned)n_items, kTQ, smem, s>>>(p);
+    kern<<<(unsigned)((n_items - p.shard + p.n_shards - 1) / p.n_shards), kTQ, smem, s>>>(p);
     return cudaGetLastError();
 }
 
@@ -260,7 +260,7 @@ size_t distance_trie_smem_bytes(bool wide) {
 
 cudaError_t launch_distance_trie(const DistanceParams& p, int64_t n_items, bool wide, bool count_work,
                                  cudaStream_t s, int* launches) {
-    if (n_items <= 0) return cudaSuccess;
+    if (n_items <= p.shard) return cudaSuccess;
     if (n_items > 0x7fffffffLL) return cudaErrorInvalidValue;
     const size_t smem = distance_trie_smem_bytes(wide);
     *launches += 1;

@@ -177,7 +177,15 @@ __device__ __forceinline__ void build_peq(W* peq, int tid, bool p_valid, const u
 }
 
 // Step A5: warp-aggregated emission of the pairs (pattern p_sorted, text t_sorted) with `edge` set.
-__device__ __forceinline__ void emit_edges(const DistanceParams& P, bool edge, int lane, int p_sorted, int t_sorted) {
+__device__ __forceinline__ void emit_edges(const DistanceParams& P, bool edge, int lane, int p_sorted, int t_sorted,
+                                           int m, int n) {
+    uint32_t oi = 0, oj = 0;
+    if (edge) {
+        oi = (uint32_t)P.perm_p[p_sorted];
+        oj = (uint32_t)P.perm_t[t_sorted];
+        if (P.mode == kPairsQueryAll) edge = oj >= (uint32_t)P.n_query || n > m || oi < oj;
+        else if (P.mode == kPairsAllQuery) edge = oi >= (uint32_t)P.n_query;
+    }
     const uint32_t bal = __ballot_sync(0xffffffffu, edge);
     if (bal) {
         unsigned long long base = 0;
@@ -186,8 +194,6 @@ __device__ __forceinline__ void emit_edges(const DistanceParams& P, bool edge, i
         if (edge) {
             const unsigned long long pos = base + __popc(bal & ((1u << lane) - 1u));
             if (pos < P.edge_cap) {
-                const uint32_t oi = (uint32_t)P.perm[p_sorted];
-                const uint32_t oj = (uint32_t)P.perm[t_sorted];
                 const uint32_t a = min(oi, oj), b = max(oi, oj);
                 P.edges[pos] = ((unsigned long long)a << 32) | b;
             }
@@ -196,6 +202,9 @@ __device__ __forceinline__ void emit_edges(const DistanceParams& P, bool edge, i
 }
 
 // Step A2, device side: the WorkRow that contains work item `item`.
+__device__ __forceinline__ int64_t work_item(const DistanceParams& P) {  // step 8(e): interleaved shards
+    return (int64_t)blockIdx.x * P.n_shards + P.shard;
+}
 __device__ __forceinline__ const WorkRow& find_row(const DistanceParams& P, int64_t item) {
     int lo = 0, hi = P.n_rows;
     while (hi - lo > 1) {

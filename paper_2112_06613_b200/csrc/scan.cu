@@ -141,4 +141,9 @@ cudaError_t exclusive_scan_u32(const uint32_t* in, uint32_t* out, int64_t n, voi
     return scan_impl<uint32_t, uint32_t>(in, out, n, false, scratch, s, launches);
 }
 
+cudaError_t exclusive_scan_u32_total(const uint32_t* in, uint32_t* out, int64_t n, void* scratch, cudaStream_t s,
+                                     int* launches) {
+    return scan_impl<uint32_t, uint32_t>(in, out, n, true, scratch, s, launches);
+}
+
 }  // namespace tcrnet

@@ -30,6 +30,20 @@ struct HostCtrl {  // pinned mirror of the small device control block
 
 }  // namespace
 
+// One packed set of sequences: all rows, or the query rows of the rectangular mode.
+struct SeqSet {
+    bool loaded = false;
+    int64_t n = 0, total_len = 0;
+    int64_t hist[kNumLen] = {};
+    int min_len = 0, max_len = 0;
+    LengthTable lt{};
+    int pat_stride = 0;
+    DevBuf perm, pat, txt, trie;
+    TrieLevels trie_levels{};
+    uint32_t trie_root[kNumLen + 1] = {};  // level-1 node range of bucket L: [trie_root[L], trie_root[L+1])
+    int64_t trie_nodes = 0;
+};
+
 struct tcrnet_ctx {
     int device = 0;
     cudaStream_t stream = nullptr;
@@ -48,20 +62,22 @@ struct tcrnet_ctx {
     int prefix_trie = 1;
     int trie_chunk = 32768;
 
+    int64_t n_query = 0;  // > 0: rectangular mode (TCRNET_OPT_N_QUERY)
+
     // load state
     bool loaded = false;
-    int64_t n = 0, total_len = 0;
-    int64_t hist[kNumLen] = {};
-    LengthTable lt{};
-    int pat_stride = 0;
-    DevBuf perm, pat, txt, trie;
-    TrieLevels trie_levels{};
-    uint32_t trie_root[kNumLen + 1] = {};  // level-1 node range of bucket L: [trie_root[L], trie_root[L+1])
+    int64_t n = 0;
+    SeqSet all, query;
+    DevBuf in_res, in_len, offsets, perm_tmp, trie_scratch;  // load scratch, kept between loads (grow-only)
 
     // build state
-    bool built = false;
-    int64_t n_edges = 0;
+    bool built = false;      // CSR + degrees valid
+    bool have_keys = false;  // tcrnet_build_shard left unsorted keys in keys_a
+    bool have_dist = false;  // edge_dist valid for the current CSR
+    int built_l_max = 0;
+    int64_t n_edges = 0, n_keys = 0;
     DevBuf keys_a, keys_b, split_hist, split_hist_scanned, scan_scratch, rows, row_ptr, col, deg;
+    DevBuf inv_perm, edge_dist, edge_dist_b, flags, flag_pos;
 
     DevBuf ctrl;               // device HostCtrl
     HostCtrl* h_ctrl = nullptr;  // pinned
@@ -126,18 +142,24 @@ int bits_for(int64_t max_value) {  // number of bits needed to represent max_val
 
 void drop_build(tcrnet_ctx* ctx) {
     ctx->built = false;
+    ctx->have_keys = false;
+    ctx->have_dist = false;
     ctx->n_edges = 0;
+    ctx->n_keys = 0;
 }
 
 void drop_load(tcrnet_ctx* ctx) {
     drop_build(ctx);
     ctx->loaded = false;
+    ctx->all.loaded = ctx->query.loaded = false;
     ctx->n = 0;
 }
 
-// Steps A1: everything after the raw arrays are in device memory.
-int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len, int64_t n, int64_t total_len,
-                     int* launches) {
+// Step A1: everything after the raw arrays are in device memory.  Packs rows 0..n-1 into `set`.
+// total_len < 0: not known (the query prefix of the rows); it is then taken from the histogram.
+int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* d_len, int64_t n, int64_t total_len,
+             int* launches) {
+    set.loaded = false;
     cudaStream_t s = ctx->stream;
     HostCtrl* dc = d_ctrl(ctx);
     TRY_CUDA(cudaMemsetAsync(dc, 0, sizeof(HostCtrl), s));
@@ -148,58 +170,53 @@ int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len
     int64_t sum = 0, cnt = 0;
     int min_len = kMaxLen, max_len = 0;
     for (int l = 0; l < kNumLen; ++l) {
-        ctx->hist[l] = (int64_t)ctx->h_ctrl->hist[l];
-        if (ctx->hist[l]) {
+        set.hist[l] = (int64_t)ctx->h_ctrl->hist[l];
+        if (set.hist[l]) {
             min_len = std::min(min_len, l);
             max_len = std::max(max_len, l);
         }
-        sum += ctx->hist[l] * l;
-        cnt += ctx->hist[l];
+        sum += set.hist[l] * l;
+        cnt += set.hist[l];
     }
-    if (cnt != n || sum != total_len) return TCRNET_ERR_ARG;
+    if (cnt != n || (total_len >= 0 && sum != total_len)) return TCRNET_ERR_ARG;
+    total_len = sum;
 
     // per-length layout
-    LengthTable& lt = ctx->lt;
+    LengthTable& lt = set.lt;
     int64_t pos = 0, words = 0;
     for (int l = 0; l < kNumLen; ++l) {
         lt.start[l] = (int32_t)pos;
         lt.txt_base[l] = words;
         lt.row_words[l] = (l + 3) & ~3;
-        pos += ctx->hist[l];
-        words += ctx->hist[l] * lt.row_words[l];
+        pos += set.hist[l];
+        words += set.hist[l] * lt.row_words[l];
     }
     lt.start[kNumLen] = (int32_t)pos;
     lt.txt_base[kNumLen] = words;
-    ctx->pat_stride = (max_len + 15) & ~15;
+    set.pat_stride = (max_len + 15) & ~15;
 
     // offsets, stable sort by (length, row), re-layout
-    DevBuf offsets;
+    DevBuf& offsets = ctx->offsets;
     const int64_t blocks = split_num_blocks(n);
     int rc = dev_reserve(ctx, offsets, sizeof(int64_t) * (size_t)(n + 1));
     if (rc == TCRNET_OK) rc = dev_reserve(ctx, ctx->scan_scratch, std::max(scan_scratch_bytes(n), scan_scratch_bytes(256 * blocks)));
     if (rc == TCRNET_OK) rc = dev_reserve(ctx, ctx->split_hist, sizeof(uint32_t) * 256 * (size_t)blocks);
     if (rc == TCRNET_OK) rc = dev_reserve(ctx, ctx->split_hist_scanned, sizeof(uint32_t) * 256 * (size_t)blocks);
-    if (rc == TCRNET_OK) rc = dev_reserve(ctx, ctx->perm, sizeof(int32_t) * (size_t)n);
-    if (rc == TCRNET_OK) rc = dev_reserve(ctx, ctx->pat, (size_t)n * ctx->pat_stride);
-    if (rc == TCRNET_OK) rc = dev_reserve(ctx, ctx->txt, sizeof(uint32_t) * (size_t)(words + 4));
-    if (rc != TCRNET_OK) {
-        dev_free(ctx, offsets);
-        return rc;
-    }
+    if (rc == TCRNET_OK) rc = dev_reserve(ctx, set.perm, sizeof(int32_t) * (size_t)n);
+    if (rc == TCRNET_OK) rc = dev_reserve(ctx, set.pat, (size_t)n * set.pat_stride);
+    if (rc == TCRNET_OK) rc = dev_reserve(ctx, set.txt, sizeof(uint32_t) * (size_t)(words + 4));
+    if (rc != TCRNET_OK) return rc;
     // Sort key: (length, first kSortPrefix residues, row).  LSD: least significant digit first, every
     // pass stable.  The sub-order inside a length bucket is free (results are mapped back through
     // perm); the lexicographic one makes the 32 patterns of a warp share their first residues, so the
     // early-exit test of the distance kernel fails or holds for the whole warp at once.
-    DevBuf perm_tmp;
+    DevBuf& perm_tmp = ctx->perm_tmp;
     rc = dev_reserve(ctx, perm_tmp, sizeof(int32_t) * (size_t)n);
-    if (rc != TCRNET_OK) {
-        dev_free(ctx, offsets);
-        return rc;
-    }
+    if (rc != TCRNET_OK) return rc;
     cudaError_t e = exclusive_scan_i32_to_i64(d_len, (int64_t*)offsets.p, n, true, ctx->scan_scratch.p, s, launches);
     {
         // kSortPrefix + 1 passes ping-pong between the two buffers; arrange for the last to land in ctx->perm
-        int32_t* bufs[2] = {(int32_t*)ctx->perm.p, (int32_t*)perm_tmp.p};
+        int32_t* bufs[2] = {(int32_t*)set.perm.p, (int32_t*)perm_tmp.p};
         int cur = kSortPrefix & 1;  // buffer written by the first pass
         const int32_t* in = nullptr;
         for (int k = kSortPrefix - 1; k >= 0 && e == cudaSuccess; --k) {
@@ -213,13 +230,13 @@ int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len
             e = split_by_length(d_len, in, n, bufs[cur], (uint32_t*)ctx->split_hist.p,
                                 (uint32_t*)ctx->split_hist_scanned.p, ctx->scan_scratch.p, s, launches);
         // cur is now the index of the buffer holding the final order
-        if (bufs[cur] != (int32_t*)ctx->perm.p) e = e == cudaSuccess ? cudaErrorUnknown : e;
+        if (bufs[cur] != (int32_t*)set.perm.p) e = e == cudaSuccess ? cudaErrorUnknown : e;
     }
     if (e == cudaSuccess)
-        e = launch_pack(d_res, (const int64_t*)offsets.p, d_len, (const int32_t*)ctx->perm.p, n, lt, ctx->pat_stride,
-                        (uint8_t*)ctx->pat.p, (uint32_t*)ctx->txt.p, &dc->flags, s, launches);
+        e = launch_pack(d_res, (const int64_t*)offsets.p, d_len, (const int32_t*)set.perm.p, n, lt, set.pat_stride,
+                        (uint8_t*)set.pat.p, (uint32_t*)set.txt.p, &dc->flags, s, launches);
     // prefix trie over the sorted texts (trie.cu); scratch: lcp8 + per-tile counts
-    DevBuf trie_scratch;
+    DevBuf& trie_scratch = ctx->trie_scratch;
     if (e == cudaSuccess) {
         size_t node_total = 0, level_off[kTrieDepth + 1] = {};
         for (int k = 1; k <= kTrieDepth; ++k) {
@@ -227,13 +244,13 @@ int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len
             node_total += (size_t)trie_level_capacity(n, k);
         }
         const size_t lcp_bytes = (((size_t)n + 15) & ~(size_t)15) + 256;  // keeps the tile counts aligned
-        rc = dev_reserve(ctx, ctx->trie, node_total * sizeof(TrieNode));
+        rc = dev_reserve(ctx, set.trie, node_total * sizeof(TrieNode));
         if (rc == TCRNET_OK) rc = dev_reserve(ctx, trie_scratch, lcp_bytes + (size_t)trie_tiles(n) * 8 * sizeof(uint32_t));
         if (rc == TCRNET_OK) {
-            for (int k = 1; k <= kTrieDepth; ++k) ctx->trie_levels.p[k] = (TrieNode*)ctx->trie.p + level_off[k];
-            ctx->trie_levels.p[0] = nullptr;
-            e = launch_trie_build((const uint32_t*)ctx->txt.p, lt, n, (uint8_t*)trie_scratch.p,
-                                  (uint32_t*)((uint8_t*)trie_scratch.p + (lcp_bytes & ~(size_t)255)), ctx->trie_levels,
+            for (int k = 1; k <= kTrieDepth; ++k) set.trie_levels.p[k] = (TrieNode*)set.trie.p + level_off[k];
+            set.trie_levels.p[0] = nullptr;
+            e = launch_trie_build((const uint32_t*)set.txt.p, lt, n, (uint8_t*)trie_scratch.p,
+                                  (uint32_t*)((uint8_t*)trie_scratch.p + (lcp_bytes & ~(size_t)255)), set.trie_levels,
                                   dc->trie_counts, dc->trie_root, s, launches);
         }
     }
@@ -241,88 +258,95 @@ int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len
         e = cudaMemcpyAsync(&ctx->h_ctrl->flags, &dc->flags,
                             sizeof(HostCtrl) - offsetof(HostCtrl, flags), cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-    dev_free(ctx, offsets);
-    dev_free(ctx, perm_tmp);
-    dev_free(ctx, trie_scratch);
     if (rc != TCRNET_OK) return rc;
     TRY_CUDA(e);
     if (ctx->h_ctrl->flags & kFlagBadResidue) return TCRNET_ERR_RESIDUE;
     // level-1 node range of every bucket (empty buckets get an empty range)
-    ctx->trie_root[kNumLen] = ctx->h_ctrl->trie_counts[1];
+    set.trie_root[kNumLen] = ctx->h_ctrl->trie_counts[1];
     for (int l = kNumLen - 1; l >= 0; --l)
-        ctx->trie_root[l] = ctx->hist[l] ? ctx->h_ctrl->trie_root[l] : ctx->trie_root[l + 1];
-    ctx->stats.trie_nodes = 0;
-    for (int k = 1; k <= kTrieDepth; ++k) ctx->stats.trie_nodes += ctx->h_ctrl->trie_counts[k];
+        set.trie_root[l] = set.hist[l] ? ctx->h_ctrl->trie_root[l] : set.trie_root[l + 1];
+    set.trie_nodes = 0;
+    for (int k = 1; k <= kTrieDepth; ++k) set.trie_nodes += ctx->h_ctrl->trie_counts[k];
+    set.n = n;
+    set.total_len = total_len;
+    set.min_len = min_len;
+    set.max_len = max_len;
+    set.loaded = true;
+    return TCRNET_OK;
+}
 
+int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len, int64_t n, int64_t total_len,
+                     int* launches) {
+    TRY(pack_set(ctx, ctx->all, d_res, d_len, n, total_len, launches));
+    if (ctx->n_query > 0 && ctx->n_query < n) TRY(pack_set(ctx, ctx->query, d_res, d_len, ctx->n_query, -1, launches));
     ctx->n = n;
-    ctx->total_len = total_len;
     ctx->stats.n = n;
     ctx->stats.total_len = total_len;
-    ctx->stats.min_len = min_len;
-    ctx->stats.max_len = max_len;
+    ctx->stats.min_len = ctx->all.min_len;
+    ctx->stats.max_len = ctx->all.max_len;
+    ctx->stats.trie_nodes = ctx->all.trie_nodes;
     ctx->loaded = true;
     return TCRNET_OK;
 }
 
-// The four launches of the distance step: {chunk kernel, trie kernel} x {32-bit, 64-bit words}.
+
+// One pass of the distance step = (pattern set, text set, which pairs to keep); each pass has up to
+// four launches: {chunk kernel, trie kernel} x {32-bit, 64-bit words}.
 struct Schedule {
     struct Part {
         std::vector<WorkRow> rows;
         int64_t items = 0;
         int max_rw = 4;
     };
-    Part part[2][2];  // [trie][wide]
-    int first_test = 0;  // trie kernel: first level with an early-exit test (0: trie not used)
+    struct Pass {
+        const SeqSet* pset = nullptr;
+        const SeqSet* tset = nullptr;
+        int mode = kPairsSelf;
+        Part part[2][2];  // [trie][wide]
+    };
+    std::vector<Pass> passes;
+    size_t n_rows = 0;
 };
 
-// Step A2, host side: the (pattern bucket, text bucket) pairs with len_t - len_p in 0..l_max.
-void make_schedule(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule& sch, tcrnet_stats& st) {
-    const LengthTable& lt = ctx->lt;
-    st.pairs_kept = st.cells_kept = st.columns_kept = st.cells_all = 0;
-    long double cells_all = 0;
-    {
-        long double sum_len = 0, sum_sq = 0;  // sum over unordered pairs of la*lb = ((sum l)^2 - sum l^2) / 2
-        for (int l = 1; l < kNumLen; ++l) {
-            sum_len += (long double)ctx->hist[l] * l;
-            sum_sq += (long double)ctx->hist[l] * l * l;
-        }
-        cells_all = (sum_len * sum_len - sum_sq) / 2;
-    }
-    st.cells_all = (int64_t)cells_all;
-    st.pairs_all = ctx->n * (ctx->n - 1) / 2;
+// Step A2, host side: the (pattern bucket, text bucket) pairs with len_t - len_p in 0..l_max
+// (kPairsAllQuery: 1..l_max; the equal-length pairs belong to the kPairsQueryAll pass).
+void schedule_pass(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule::Pass& pass, tcrnet_stats& st) {
+    const SeqSet& ps = *pass.pset;
+    const SeqSet& ts = *pass.tset;
     // The trie kernel serves the rows whose early exit can act inside the trie: first test level
     // <= kTrieDepth and at least one text column beyond the trie.
     const bool use_trie = ctx->prefix_trie && first_check >= 3 && first_check <= kTrieDepth;
-    sch.first_test = use_trie ? first_check : 0;
     for (int m = 1; m < kNumLen; ++m) {
-        if (!ctx->hist[m]) continue;
-        for (int n = m; n <= std::min(kMaxLen, m + l_max); ++n) {
-            if (!ctx->hist[n]) continue;
-            const int64_t pc = ctx->hist[m], tc = ctx->hist[n];
-            const int64_t pairs = (m == n) ? pc * (pc - 1) / 2 : pc * tc;
+        if (!ps.hist[m]) continue;
+        const int n0 = pass.mode == kPairsAllQuery ? m + 1 : m;
+        for (int n = n0; n <= std::min(kMaxLen, m + l_max); ++n) {
+            if (!ts.hist[n]) continue;
+            const int64_t pc = ps.hist[m], tc = ts.hist[n];
+            const bool diag = pass.mode == kPairsSelf && m == n;
+            const int64_t pairs = diag ? pc * (pc - 1) / 2 : pc * tc;
             st.pairs_kept += pairs;
             st.cells_kept += pairs * m * n;
             st.columns_kept += pairs * n;
             if (pairs == 0) continue;
             const bool trie = use_trie && n > kTrieDepth;
             WorkRow r{};
-            r.txt_base = lt.txt_base[n];
-            r.p_start = lt.start[m];
+            r.txt_base = ts.lt.txt_base[n];
+            r.p_start = ps.lt.start[m];
             r.p_count = (int32_t)pc;
-            r.t_start = lt.start[n];
+            r.t_start = ts.lt.start[n];
             r.t_count = (int32_t)tc;
             r.m = m;
             r.n = n;
-            r.row_words = lt.row_words[n];
+            r.row_words = ts.lt.row_words[n];
             r.tchunk = trie ? ctx->trie_chunk : ctx->tchunk;
             r.n_tchunks = (int32_t)((tc + r.tchunk - 1) / r.tchunk);
-            r.diag = (m == n) ? 1 : 0;
-            r.root_begin = ctx->trie_root[n];
-            r.root_end = ctx->trie_root[n + 1];
-            sch.part[trie ? 1 : 0][m <= 32 ? 0 : 1].rows.push_back(r);
+            r.diag = diag ? 1 : 0;
+            r.root_begin = ts.trie_root[n];
+            r.root_end = ts.trie_root[n + 1];
+            pass.part[trie ? 1 : 0][m <= 32 ? 0 : 1].rows.push_back(r);
         }
     }
-    for (auto& by_kernel : sch.part)
+    for (auto& by_kernel : pass.part)
         for (Schedule::Part& part : by_kernel) {
             auto n_items = [](const WorkRow& r) { return (int64_t)((r.p_count + kTQ - 1) / kTQ) * r.n_tchunks; };
             // big rows first: the small buckets fill the tail of the launch
@@ -338,38 +362,198 @@ void make_schedule(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule& 
         }
 }
 
-int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_check, uint64_t cap, int* launches) {
+void make_schedule(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule& sch, tcrnet_stats& st) {
+    st.pairs_kept = st.cells_kept = st.columns_kept = st.cells_all = 0;
+    {
+        long double sum_len = 0, sum_sq = 0;  // sum over unordered pairs of la*lb = ((sum l)^2 - sum l^2) / 2
+        for (int l = 1; l < kNumLen; ++l) {
+            sum_len += (long double)ctx->all.hist[l] * l;
+            sum_sq += (long double)ctx->all.hist[l] * l * l;
+        }
+        st.cells_all = (int64_t)((sum_len * sum_len - sum_sq) / 2);
+    }
+    st.pairs_all = ctx->n * (ctx->n - 1) / 2;
+    if (ctx->query.loaded) {  // rectangular mode: the pairs with at least one endpoint among the query rows
+        const int64_t rest = ctx->n - ctx->query.n;
+        st.pairs_all = ctx->query.n * (ctx->query.n - 1) / 2 + ctx->query.n * rest;
+        sch.passes.resize(2);
+        sch.passes[0].pset = &ctx->query;
+        sch.passes[0].tset = &ctx->all;
+        sch.passes[0].mode = kPairsQueryAll;
+        sch.passes[1].pset = &ctx->all;
+        sch.passes[1].tset = &ctx->query;
+        sch.passes[1].mode = kPairsAllQuery;
+    } else {
+        sch.passes.resize(1);
+        sch.passes[0].pset = sch.passes[0].tset = &ctx->all;
+        sch.passes[0].mode = kPairsSelf;
+    }
+    st.work_items = st.work_items_trie = 0;
+    sch.n_rows = 0;
+    for (Schedule::Pass& pass : sch.passes) {
+        schedule_pass(ctx, l_max, first_check, pass, st);
+        for (int trie = 0; trie < 2; ++trie)
+            for (int wide = 0; wide < 2; ++wide) {
+                st.work_items += pass.part[trie][wide].items;
+                if (trie) st.work_items_trie += pass.part[trie][wide].items;
+                sch.n_rows += pass.part[trie][wide].rows.size();
+            }
+    }
+}
+
+int upload_schedule(tcrnet_ctx* ctx, const Schedule& sch) {
+    TRY(dev_reserve(ctx, ctx->rows, sizeof(WorkRow) * std::max<size_t>(sch.n_rows, 1)));
+    WorkRow* dst = (WorkRow*)ctx->rows.p;
+    for (const Schedule::Pass& pass : sch.passes)  // same order as run_distance walks them: trie parts first
+        for (int trie = 1; trie >= 0; --trie)
+            for (int wide = 0; wide < 2; ++wide) {
+                const std::vector<WorkRow>& rows = pass.part[trie][wide].rows;
+                if (!rows.empty())
+                    TRY_CUDA(cudaMemcpyAsync(dst, rows.data(), sizeof(WorkRow) * rows.size(), cudaMemcpyHostToDevice,
+                                             ctx->stream));
+                dst += rows.size();
+            }
+    return TCRNET_OK;
+}
+
+int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_check, uint64_t cap, int shard,
+                 int n_shards, int* launches) {
     cudaStream_t s = ctx->stream;
     HostCtrl* dc = d_ctrl(ctx);
     TRY_CUDA(cudaMemsetAsync(&dc->edge_count, 0, sizeof(unsigned long long) * 5, s));  // edge_count + work[4]
-    DistanceParams p{};
-    p.l_max = l_max;
-    p.pat_stride = ctx->pat_stride;
-    p.txt = (const uint32_t*)ctx->txt.p;
-    p.pat = (const uint8_t*)ctx->pat.p;
-    p.perm = (const int32_t*)ctx->perm.p;
-    p.edges = (unsigned long long*)ctx->keys_a.p;
-    p.edge_count = &dc->edge_count;
-    p.edge_cap = cap;
-    p.work = dc->work;
-    for (int k = 0; k <= kTrieDepth; ++k) p.trie[k] = ctx->trie_levels.p[k];
     const WorkRow* d_rows = (const WorkRow*)ctx->rows.p;
-    for (int trie = 1; trie >= 0; --trie)
-        for (int wide = 0; wide < 2; ++wide) {
-            const Schedule::Part& part = sch.part[trie][wide];
-            if (!part.rows.empty()) {
-                p.rows = d_rows;
-                p.n_rows = (int32_t)part.rows.size();
-                if (trie)
-                    TRY_CUDA(launch_distance_trie(p, part.items, wide != 0, ctx->count_work != 0, s, launches));
-                else
-                    TRY_CUDA(launch_distance(p, part.items, wide != 0, first_check, ctx->count_work != 0, part.max_rw, s, launches));
+    for (const Schedule::Pass& pass : sch.passes) {
+        DistanceParams p{};
+        p.l_max = l_max;
+        p.mode = pass.mode;
+        p.n_query = (int32_t)ctx->query.n;
+        p.shard = shard;
+        p.n_shards = n_shards;
+        p.pat_stride = pass.pset->pat_stride;
+        p.pat = (const uint8_t*)pass.pset->pat.p;
+        p.perm_p = (const int32_t*)pass.pset->perm.p;
+        p.txt = (const uint32_t*)pass.tset->txt.p;
+        p.perm_t = (const int32_t*)pass.tset->perm.p;
+        for (int k = 0; k <= kTrieDepth; ++k) p.trie[k] = pass.tset->trie_levels.p[k];
+        p.edges = (unsigned long long*)ctx->keys_a.p;
+        p.edge_count = &dc->edge_count;
+        p.edge_cap = cap;
+        p.work = dc->work;
+        for (int trie = 1; trie >= 0; --trie)
+            for (int wide = 0; wide < 2; ++wide) {
+                const Schedule::Part& part = pass.part[trie][wide];
+                if (!part.rows.empty()) {
+                    p.rows = d_rows;
+                    p.n_rows = (int32_t)part.rows.size();
+                    if (trie)
+                        TRY_CUDA(launch_distance_trie(p, part.items, wide != 0, ctx->count_work != 0, s, launches));
+                    else
+                        TRY_CUDA(launch_distance(p, part.items, wide != 0, first_check, ctx->count_work != 0,
+                                                 part.max_rw, s, launches));
+                }
+                d_rows += part.rows.size();
             }
-            d_rows += part.rows.size();
-        }
+    }
     TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->edge_count, &dc->edge_count, sizeof(unsigned long long) * 5,
                              cudaMemcpyDeviceToHost, s));
     TRY_CUDA(cudaStreamSynchronize(s));
+    return TCRNET_OK;
+}
+
+// Steps A2-A5 for the work items of one shard: unsorted keys in keys_a, ctx->n_keys of them.
+int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* launches) {
+    tcrnet_stats& st = ctx->stats;
+    cudaStream_t s = ctx->stream;
+    const int64_t n = ctx->n;
+    int first_check = 0;
+    if (ctx->early_exit) {
+        first_check = ctx->first_check_opt ? ctx->first_check_opt : l_max + 2;
+        first_check = std::max(3, std::min(8, first_check));
+    }
+    st.first_check = first_check;
+    st.l_max = l_max;
+    Schedule sch;
+    make_schedule(ctx, l_max, first_check, sch, st);
+    TRY_CUDA(cudaEventRecord(ctx->ev[0], s));
+    TRY(upload_schedule(ctx, sch));
+
+    // distances + emission (second pass only if the edge buffer was too small)
+    int64_t cap = ctx->edge_capacity_opt > 0 ? ctx->edge_capacity_opt : std::max<int64_t>((int64_t)1 << 20, 16 * n);
+    cap = std::min(cap, ctx->edge_limit);
+    cap = std::max<int64_t>(cap, 1);
+    if (ctx->keys_a.p && (int64_t)(ctx->keys_a.bytes / 8) > cap) cap = std::min<int64_t>(ctx->keys_a.bytes / 8, ctx->edge_limit);
+    TRY(dev_reserve(ctx, ctx->keys_a, sizeof(unsigned long long) * (size_t)cap));
+    st.distance_passes = 1;
+    TRY(run_distance(ctx, sch, l_max, first_check, (uint64_t)cap, shard, n_shards, launches));
+    int64_t n_keys = (int64_t)ctx->h_ctrl->edge_count;
+    if (n_keys > ctx->edge_limit) return TCRNET_ERR_EDGE_OVERFLOW;
+    if (n_keys > cap) {
+        cap = n_keys;
+        TRY(dev_reserve(ctx, ctx->keys_a, sizeof(unsigned long long) * (size_t)cap));
+        st.distance_passes = 2;
+        TRY(run_distance(ctx, sch, l_max, first_check, (uint64_t)cap, shard, n_shards, launches));
+        if ((int64_t)ctx->h_ctrl->edge_count != n_keys) return TCRNET_ERR_CUDA;  // cannot happen: same input
+    }
+    st.lane_columns_exec = (int64_t)ctx->h_ctrl->work[0];
+    st.lane_tests_exec = (int64_t)ctx->h_ctrl->work[1];
+    st.lane_pairs_exec = (int64_t)ctx->h_ctrl->work[2];
+    st.lane_prefix_tests_exec = (int64_t)ctx->h_ctrl->work[3];
+    TRY_CUDA(cudaEventRecord(ctx->ev[1], s));
+    ctx->n_keys = n_keys;
+    return TCRNET_OK;
+}
+
+// Step A6 on the n_keys keys (u << 32) | v in keys_a: LSD radix sort over the significant bits, CSR, degrees.
+int assemble_phase(tcrnet_ctx* ctx, int64_t n_keys, int* launches) {
+    tcrnet_stats& st = ctx->stats;
+    cudaStream_t s = ctx->stream;
+    const int64_t n = ctx->n;
+    const unsigned long long* sorted = (const unsigned long long*)ctx->keys_a.p;
+    if (n_keys > 1) {
+        const int64_t blocks = split_num_blocks(n_keys);
+        TRY(dev_reserve(ctx, ctx->keys_b, sizeof(unsigned long long) * (size_t)n_keys));
+        TRY(dev_reserve(ctx, ctx->split_hist, sizeof(uint32_t) * 256 * (size_t)blocks));
+        TRY(dev_reserve(ctx, ctx->split_hist_scanned, sizeof(uint32_t) * 256 * (size_t)blocks));
+        TRY(dev_reserve(ctx, ctx->scan_scratch, scan_scratch_bytes(256 * blocks)));
+        const int id_bits = bits_for(n - 1 > 0 ? n - 1 : 1);
+        unsigned long long* a = (unsigned long long*)ctx->keys_a.p;
+        unsigned long long* b = (unsigned long long*)ctx->keys_b.p;
+        for (int half = 0; half < 2; ++half)
+            for (int sh = 0; sh < id_bits; sh += 8) {
+                TRY_CUDA(split_keys_u64(a, b, n_keys, 32 * half + sh, (uint32_t*)ctx->split_hist.p,
+                                        (uint32_t*)ctx->split_hist_scanned.p, ctx->scan_scratch.p, s, launches));
+                std::swap(a, b);
+            }
+        sorted = a;
+    }
+    TRY_CUDA(cudaEventRecord(ctx->ev[2], s));
+    TRY(dev_reserve(ctx, ctx->row_ptr, sizeof(int64_t) * (size_t)(n + 1)));
+    TRY(dev_reserve(ctx, ctx->col, sizeof(int32_t) * (size_t)std::max<int64_t>(n_keys, 1)));
+    TRY(dev_reserve(ctx, ctx->deg, sizeof(int32_t) * (size_t)n));
+    TRY_CUDA(launch_csr(sorted, n_keys, n, (int64_t*)ctx->row_ptr.p, (int32_t*)ctx->col.p, (int32_t*)ctx->deg.p, s, launches));
+    TRY_CUDA(cudaEventRecord(ctx->ev[3], s));
+    TRY_CUDA(cudaEventSynchronize(ctx->ev[3]));
+    TRY_CUDA(cudaEventElapsedTime(&st.ms_sort, ctx->ev[1], ctx->ev[2]));
+    TRY_CUDA(cudaEventElapsedTime(&st.ms_csr, ctx->ev[2], ctx->ev[3]));
+    st.n_edges = n_keys;
+    ctx->n_edges = n_keys;
+    ctx->have_keys = false;  // the sort used keys_a
+    ctx->have_dist = false;
+    ctx->built = true;
+    return TCRNET_OK;
+}
+
+// Distance labels of the current CSR's edges (labels.cu), computed on first use.
+int ensure_edge_distances(tcrnet_ctx* ctx, int* launches) {
+    if (ctx->have_dist) return TCRNET_OK;
+    cudaStream_t s = ctx->stream;
+    TRY(dev_reserve(ctx, ctx->inv_perm, sizeof(int32_t) * (size_t)ctx->n));
+    TRY(dev_reserve(ctx, ctx->edge_dist, (size_t)std::max<int64_t>(ctx->n_edges, 1)));
+    TRY_CUDA(launch_inverse_perm((const int32_t*)ctx->all.perm.p, ctx->n, (int32_t*)ctx->inv_perm.p, s, launches));
+    TRY_CUDA(launch_edge_distances((const int64_t*)ctx->row_ptr.p, (const int32_t*)ctx->col.p, ctx->n, ctx->n_edges,
+                                   (const int32_t*)ctx->inv_perm.p, (const uint8_t*)ctx->all.pat.p,
+                                   ctx->all.pat_stride, (uint8_t*)ctx->edge_dist.p, s, launches));
+    ctx->have_dist = true;
     return TCRNET_OK;
 }
 
@@ -433,7 +617,10 @@ void tcrnet_destroy(tcrnet_ctx* ctx) {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
-    DevBuf* bufs[] = {&ctx->perm, &ctx->pat, &ctx->txt, &ctx->trie, &ctx->keys_a, &ctx->keys_b, &ctx->split_hist,
+    DevBuf* bufs[] = {&ctx->all.perm, &ctx->all.pat, &ctx->all.txt, &ctx->all.trie, &ctx->query.perm, &ctx->query.pat,
+                      &ctx->query.txt, &ctx->query.trie, &ctx->inv_perm, &ctx->edge_dist, &ctx->edge_dist_b, &ctx->flags,
+                      &ctx->flag_pos, &ctx->in_res, &ctx->in_len, &ctx->offsets,
+                      &ctx->perm_tmp, &ctx->trie_scratch, &ctx->keys_a, &ctx->keys_b, &ctx->split_hist,
                       &ctx->split_hist_scanned, &ctx->scan_scratch, &ctx->rows, &ctx->row_ptr, &ctx->col,
                       &ctx->deg, &ctx->ctrl};
     for (DevBuf* b : bufs) dev_free(ctx, *b);
@@ -469,7 +656,8 @@ int tcrnet_load(tcrnet_ctx* ctx, const uint8_t* residues, const int32_t* lengths
         if (lengths[i] < 1 || lengths[i] > kMaxLen) return TCRNET_ERR_LENGTH;
         total_len += lengths[i];
     }
-    DevBuf d_res, d_len;
+    DevBuf& d_res = ctx->in_res;
+    DevBuf& d_len = ctx->in_len;
     int rc = dev_reserve(ctx, d_res, (size_t)total_len);
     if (rc == TCRNET_OK) rc = dev_reserve(ctx, d_len, sizeof(int32_t) * (size_t)n);
     int launches = 0;
@@ -497,9 +685,7 @@ int tcrnet_load(tcrnet_ctx* ctx, const uint8_t* residues, const int32_t* lengths
             drop_load(ctx);
         }
     }
-    cudaStreamSynchronize(ctx->stream);
-    dev_free(ctx, d_res);
-    dev_free(ctx, d_len);
+    if (rc != TCRNET_OK) cudaStreamSynchronize(ctx->stream);  // the host arrays are borrowed for this call only
     ctx->stats.launches_load = launches;
     return rc;
 }
@@ -510,103 +696,135 @@ int tcrnet_build(tcrnet_ctx* ctx, int l_max, int64_t* n_edges_out) {
     if (l_max < 0 || l_max > kMaxLen) return TCRNET_ERR_LMAX;
     TRY_CUDA(cudaSetDevice(ctx->device));
     drop_build(ctx);
-    cudaStream_t s = ctx->stream;
-    tcrnet_stats& st = ctx->stats;
     int launches = 0;
-    const int64_t n = ctx->n;
-
-    // ---- A2: schedule ----
-    int first_check = 0;
-    if (ctx->early_exit) {
-        first_check = ctx->first_check_opt ? ctx->first_check_opt : l_max + 2;
-        first_check = std::max(3, std::min(8, first_check));
-    }
-    st.first_check = first_check;
-    Schedule sch;
-    make_schedule(ctx, l_max, first_check, sch, st);
-    st.l_max = l_max;
-    st.work_items = st.work_items_trie = 0;
-    size_t n_rows = 0;
-    for (int trie = 0; trie < 2; ++trie)
-        for (int wide = 0; wide < 2; ++wide) {
-            st.work_items += sch.part[trie][wide].items;
-            if (trie) st.work_items_trie += sch.part[trie][wide].items;
-            n_rows += sch.part[trie][wide].rows.size();
-        }
-    TRY(dev_reserve(ctx, ctx->rows, sizeof(WorkRow) * std::max<size_t>(n_rows, 1)));
-    TRY_CUDA(cudaEventRecord(ctx->ev[0], s));
-    {
-        // same order as run_distance walks them: trie parts first
-        WorkRow* dst = (WorkRow*)ctx->rows.p;
-        for (int trie = 1; trie >= 0; --trie)
-            for (int wide = 0; wide < 2; ++wide) {
-                const std::vector<WorkRow>& rows = sch.part[trie][wide].rows;
-                if (!rows.empty())
-                    TRY_CUDA(cudaMemcpyAsync(dst, rows.data(), sizeof(WorkRow) * rows.size(), cudaMemcpyHostToDevice, s));
-                dst += rows.size();
-            }
-    }
-
-    // ---- A3-A5: distances + emission (second pass only if the edge buffer was too small) ----
-    int64_t cap = ctx->edge_capacity_opt > 0 ? ctx->edge_capacity_opt : std::max<int64_t>((int64_t)1 << 20, 16 * n);
-    cap = std::min(cap, ctx->edge_limit);
-    cap = std::max<int64_t>(cap, 1);
-    if (ctx->keys_a.p && (int64_t)(ctx->keys_a.bytes / 8) > cap) cap = std::min<int64_t>(ctx->keys_a.bytes / 8, ctx->edge_limit);
-    TRY(dev_reserve(ctx, ctx->keys_a, sizeof(unsigned long long) * (size_t)cap));
-    st.distance_passes = 1;
-    TRY(run_distance(ctx, sch, l_max, first_check, (uint64_t)cap, &launches));
-    int64_t n_edges = (int64_t)ctx->h_ctrl->edge_count;
-    if (n_edges > ctx->edge_limit) return TCRNET_ERR_EDGE_OVERFLOW;
-    if (n_edges > cap) {
-        cap = n_edges;
-        TRY(dev_reserve(ctx, ctx->keys_a, sizeof(unsigned long long) * (size_t)cap));
-        st.distance_passes = 2;
-        TRY(run_distance(ctx, sch, l_max, first_check, (uint64_t)cap, &launches));
-        if ((int64_t)ctx->h_ctrl->edge_count != n_edges) return TCRNET_ERR_CUDA;  // cannot happen: same input
-    }
-    st.lane_columns_exec = (int64_t)ctx->h_ctrl->work[0];
-    st.lane_tests_exec = (int64_t)ctx->h_ctrl->work[1];
-    st.lane_pairs_exec = (int64_t)ctx->h_ctrl->work[2];
-    st.lane_prefix_tests_exec = (int64_t)ctx->h_ctrl->work[3];
-    TRY_CUDA(cudaEventRecord(ctx->ev[1], s));
-
-    // ---- A6a: LSD radix sort of the keys (u << 32) | v over the significant bits only ----
-    const unsigned long long* sorted = (const unsigned long long*)ctx->keys_a.p;
-    if (n_edges > 1) {
-        const int64_t blocks = split_num_blocks(n_edges);
-        TRY(dev_reserve(ctx, ctx->keys_b, sizeof(unsigned long long) * (size_t)n_edges));
-        TRY(dev_reserve(ctx, ctx->split_hist, sizeof(uint32_t) * 256 * (size_t)blocks));
-        TRY(dev_reserve(ctx, ctx->split_hist_scanned, sizeof(uint32_t) * 256 * (size_t)blocks));
-        TRY(dev_reserve(ctx, ctx->scan_scratch, scan_scratch_bytes(256 * blocks)));
-        const int id_bits = bits_for(n - 1 > 0 ? n - 1 : 1);
-        unsigned long long* a = (unsigned long long*)ctx->keys_a.p;
-        unsigned long long* b = (unsigned long long*)ctx->keys_b.p;
-        for (int half = 0; half < 2; ++half)
-            for (int sh = 0; sh < id_bits; sh += 8) {
-                TRY_CUDA(split_keys_u64(a, b, n_edges, 32 * half + sh, (uint32_t*)ctx->split_hist.p,
-                                        (uint32_t*)ctx->split_hist_scanned.p, ctx->scan_scratch.p, s, &launches));
-                std::swap(a, b);
-            }
-        sorted = a;
-    }
-    TRY_CUDA(cudaEventRecord(ctx->ev[2], s));
-
-    // ---- A6b: CSR + degrees ----
-    TRY(dev_reserve(ctx, ctx->row_ptr, sizeof(int64_t) * (size_t)(n + 1)));
-    TRY(dev_reserve(ctx, ctx->col, sizeof(int32_t) * (size_t)std::max<int64_t>(n_edges, 1)));
-    TRY(dev_reserve(ctx, ctx->deg, sizeof(int32_t) * (size_t)n));
-    TRY_CUDA(launch_csr(sorted, n_edges, n, (int64_t*)ctx->row_ptr.p, (int32_t*)ctx->col.p, (int32_t*)ctx->deg.p, s, &launches));
-    TRY_CUDA(cudaEventRecord(ctx->ev[3], s));
-    TRY_CUDA(cudaEventSynchronize(ctx->ev[3]));
+    TRY(distance_phase(ctx, l_max, 0, 1, &launches));
+    TRY(assemble_phase(ctx, ctx->n_keys, &launches));
+    tcrnet_stats& st = ctx->stats;
     TRY_CUDA(cudaEventElapsedTime(&st.ms_distance, ctx->ev[0], ctx->ev[1]));
-    TRY_CUDA(cudaEventElapsedTime(&st.ms_sort, ctx->ev[1], ctx->ev[2]));
-    TRY_CUDA(cudaEventElapsedTime(&st.ms_csr, ctx->ev[2], ctx->ev[3]));
     TRY_CUDA(cudaEventElapsedTime(&st.ms_build, ctx->ev[0], ctx->ev[3]));
     st.launches_build = launches;
-    st.n_edges = n_edges;
-    ctx->n_edges = n_edges;
-    ctx->built = true;
-    if (n_edges_out) *n_edges_out = n_edges;
+    ctx->built_l_max = l_max;
+    if (n_edges_out) *n_edges_out = ctx->n_edges;
+    return TCRNET_OK;
+}
+
+int tcrnet_build_shard(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, const uint64_t** keys_dev,
+                       int64_t* n_keys_out) {
+    if (!ctx || n_shards < 1 || shard < 0 || shard >= n_shards) return TCRNET_ERR_ARG;
+    if (!ctx->loaded) return TCRNET_ERR_STATE;
+    if (l_max < 0 || l_max > kMaxLen) return TCRNET_ERR_LMAX;
+    TRY_CUDA(cudaSetDevice(ctx->device));
+    drop_build(ctx);
+    int launches = 0;
+    TRY(distance_phase(ctx, l_max, shard, n_shards, &launches));
+    tcrnet_stats& st = ctx->stats;
+    TRY_CUDA(cudaEventSynchronize(ctx->ev[1]));
+    TRY_CUDA(cudaEventElapsedTime(&st.ms_distance, ctx->ev[0], ctx->ev[1]));
+    st.ms_sort = st.ms_csr = 0.f;
+    st.ms_build = st.ms_distance;
+    st.launches_build = launches;
+    st.n_edges = ctx->n_keys;
+    ctx->have_keys = true;
+    ctx->built_l_max = l_max;
+    if (keys_dev) *keys_dev = ctx->n_keys ? (const uint64_t*)ctx->keys_a.p : nullptr;
+    if (n_keys_out) *n_keys_out = ctx->n_keys;
+    return TCRNET_OK;
+}
+
+int tcrnet_assemble(tcrnet_ctx* ctx, const uint64_t* keys_dev, int64_t n_keys, int64_t* n_edges_out) {
+    if (!ctx || n_keys < 0 || (n_keys > 0 && !keys_dev)) return TCRNET_ERR_ARG;
+    if (!ctx->loaded) return TCRNET_ERR_STATE;
+    if (n_keys > ctx->edge_limit) return TCRNET_ERR_EDGE_OVERFLOW;
+    TRY_CUDA(cudaSetDevice(ctx->device));
+    cudaStream_t s = ctx->stream;
+    const bool in_place = n_keys > 0 && keys_dev == (const uint64_t*)ctx->keys_a.p;
+    if (in_place && !(ctx->have_keys && n_keys <= ctx->n_keys)) return TCRNET_ERR_ARG;
+    ctx->built = false;
+    ctx->have_dist = false;
+    int launches = 0;
+    if (!in_place) {
+        // keys_dev may not alias the context's buffers: reserve first (contents are not preserved), then copy
+        ctx->have_keys = false;
+        TRY(dev_reserve(ctx, ctx->keys_a, sizeof(unsigned long long) * (size_t)std::max<int64_t>(n_keys, 1)));
+        if (n_keys)
+            TRY_CUDA(cudaMemcpyAsync(ctx->keys_a.p, keys_dev, sizeof(unsigned long long) * (size_t)n_keys,
+                                     cudaMemcpyDeviceToDevice, s));
+    }
+    HostCtrl* dc = d_ctrl(ctx);
+    TRY_CUDA(cudaMemsetAsync(&dc->flags, 0, sizeof(uint32_t), s));
+    TRY_CUDA(launch_validate_keys((const unsigned long long*)ctx->keys_a.p, n_keys, ctx->n, &dc->flags, s, &launches));
+    TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->flags, &dc->flags, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+    TRY_CUDA(cudaEventRecord(ctx->ev[1], s));
+    TRY_CUDA(cudaStreamSynchronize(s));
+    if (ctx->h_ctrl->flags) return TCRNET_ERR_ARG;
+    TRY(assemble_phase(ctx, n_keys, &launches));
+    ctx->stats.launches_build = launches;
+    TRY_CUDA(cudaEventElapsedTime(&ctx->stats.ms_build, ctx->ev[1], ctx->ev[3]));
+    if (n_edges_out) *n_edges_out = ctx->n_edges;
+    return TCRNET_OK;
+}
+
+int tcrnet_edge_distances(tcrnet_ctx* ctx, const uint8_t** dist_dev) {
+    if (!ctx || !dist_dev) return TCRNET_ERR_ARG;
+    if (!ctx->built) return TCRNET_ERR_STATE;
+    TRY_CUDA(cudaSetDevice(ctx->device));
+    int launches = 0;
+    TRY(ensure_edge_distances(ctx, &launches));
+    TRY_CUDA(cudaStreamSynchronize(ctx->stream));
+    *dist_dev = ctx->n_edges ? (const uint8_t*)ctx->edge_dist.p : nullptr;
+    return TCRNET_OK;
+}
+
+int tcrnet_restrict(tcrnet_ctx* ctx, int l_max, int64_t* n_edges_out) {
+    if (!ctx) return TCRNET_ERR_ARG;
+    if (!ctx->built) return TCRNET_ERR_STATE;
+    if (l_max < 0 || l_max > ctx->built_l_max) return TCRNET_ERR_LMAX;
+    TRY_CUDA(cudaSetDevice(ctx->device));
+    cudaStream_t s = ctx->stream;
+    int launches = 0;
+    TRY(ensure_edge_distances(ctx, &launches));
+    const int64_t e_old = ctx->n_edges;
+    int64_t e_new = 0;
+    TRY_CUDA(cudaEventRecord(ctx->ev[1], s));
+    if (e_old > 0) {
+        TRY(dev_reserve(ctx, ctx->flags, sizeof(uint32_t) * (size_t)e_old));
+        TRY(dev_reserve(ctx, ctx->flag_pos, sizeof(uint32_t) * (size_t)(e_old + 1)));
+        TRY(dev_reserve(ctx, ctx->scan_scratch, scan_scratch_bytes(e_old)));
+        TRY(dev_reserve(ctx, ctx->keys_a, sizeof(unsigned long long) * (size_t)e_old));
+        TRY(dev_reserve(ctx, ctx->edge_dist_b, (size_t)e_old));
+        TRY_CUDA(launch_restrict_flags((const uint8_t*)ctx->edge_dist.p, e_old, l_max, (uint32_t*)ctx->flags.p, s, &launches));
+        TRY_CUDA(exclusive_scan_u32_total((const uint32_t*)ctx->flags.p, (uint32_t*)ctx->flag_pos.p, e_old,
+                                          ctx->scan_scratch.p, s, &launches));
+        TRY_CUDA(launch_restrict_compact((const int64_t*)ctx->row_ptr.p, (const int32_t*)ctx->col.p,
+                                         (const uint8_t*)ctx->edge_dist.p, ctx->n, e_old, (const uint32_t*)ctx->flags.p,
+                                         (const uint32_t*)ctx->flag_pos.p, (unsigned long long*)ctx->keys_a.p,
+                                         (uint8_t*)ctx->edge_dist_b.p, s, &launches));
+        uint32_t total = 0;
+        TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->flags, (const uint32_t*)ctx->flag_pos.p + e_old, sizeof(uint32_t),
+                                 cudaMemcpyDeviceToHost, s));
+        TRY_CUDA(cudaStreamSynchronize(s));
+        total = ctx->h_ctrl->flags;
+        e_new = (int64_t)total;
+        std::swap(ctx->edge_dist, ctx->edge_dist_b);
+    }
+    // the compaction is stable, so the keys are already sorted: CSR + degrees directly
+    TRY_CUDA(cudaEventRecord(ctx->ev[2], s));
+    TRY_CUDA(launch_csr((const unsigned long long*)ctx->keys_a.p, e_new, ctx->n, (int64_t*)ctx->row_ptr.p,
+                        (int32_t*)ctx->col.p, (int32_t*)ctx->deg.p, s, &launches));
+    TRY_CUDA(cudaEventRecord(ctx->ev[3], s));
+    TRY_CUDA(cudaEventSynchronize(ctx->ev[3]));
+    tcrnet_stats& st = ctx->stats;
+    st.ms_distance = 0.f;
+    TRY_CUDA(cudaEventElapsedTime(&st.ms_sort, ctx->ev[1], ctx->ev[2]));
+    TRY_CUDA(cudaEventElapsedTime(&st.ms_csr, ctx->ev[2], ctx->ev[3]));
+    TRY_CUDA(cudaEventElapsedTime(&st.ms_build, ctx->ev[1], ctx->ev[3]));
+    st.launches_build = launches;
+    st.l_max = l_max;
+    st.n_edges = e_new;
+    ctx->n_edges = e_new;
+    ctx->built_l_max = l_max;
+    ctx->have_keys = false;
+    if (n_edges_out) *n_edges_out = e_new;
     return TCRNET_OK;
 }
 
@@ -671,6 +889,10 @@ int tcrnet_set_option(tcrnet_ctx* ctx, int option, int64_t value) {
         case TCRNET_OPT_PREFIX_TRIE:
             if (value != 0 && value != 1) return TCRNET_ERR_ARG;
             ctx->prefix_trie = (int)value;
+            return TCRNET_OK;
+        case TCRNET_OPT_N_QUERY:
+            if (value < 0 || value > 0x7ffffffeLL) return TCRNET_ERR_ARG;
+            ctx->n_query = value;
             return TCRNET_OK;
         case TCRNET_OPT_TRIE_CHUNK:
             if (value < kTQ || value % kTQ != 0 || value > (1 << 24)) return TCRNET_ERR_ARG;

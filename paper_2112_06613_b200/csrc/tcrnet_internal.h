@@ -60,14 +60,29 @@ struct TrieLevels {
     TrieNode* p[kTrieDepth + 1];  // [k] = nodes of level k, k = 1..kTrieDepth ([0] unused)
 };
 
+// Which pairs a distance launch keeps (step A5).  kPairsSelf: patterns and texts are the same
+// set, every unordered pair once (same-bucket rows keep sorted p < t).  The other two are the
+// passes of the rectangular (query x repertoire) mode, where at least one endpoint is a query
+// row (caller's rows 0..n_query-1):
+//   kPairsQueryAll  patterns = query set, texts = all rows, len_t >= len_p; a text that is itself
+//                   a query is kept only if it is longer, or of equal length with the larger row id
+//   kPairsAllQuery  patterns = all rows, texts = query set, len_t > len_p; patterns that are
+//                   queries themselves are dropped (the pair was found by the first pass)
+enum PairMode : int32_t { kPairsSelf = 0, kPairsQueryAll = 1, kPairsAllQuery = 2 };
+
 struct DistanceParams {
     const WorkRow* rows;
     int32_t n_rows;
     int32_t l_max;
     int32_t pat_stride;  // bytes per pattern row
+    int32_t mode;        // PairMode
+    int32_t n_query;     // rectangular mode: rows 0..n_query-1 of the caller are the queries
+    int32_t shard;       // this launch handles the work items  shard + k * n_shards  (step 8(e))
+    int32_t n_shards;
     const uint32_t* txt; // text rows: one 32-bit residue code per column, padded with kPadCode
     const uint8_t* pat;  // pattern rows: one residue code per byte, row = sorted position
-    const int32_t* perm; // sorted position -> caller's row index
+    const int32_t* perm_p; // sorted position -> caller's row index, pattern set
+    const int32_t* perm_t; // ... text set
     unsigned long long* edges;       // keys (min(i,j) << 32) | max(i,j)
     unsigned long long* edge_count;  // device counter (keeps counting beyond capacity)
     unsigned long long edge_cap;
@@ -130,6 +145,22 @@ cudaError_t launch_distance(const DistanceParams& p, int64_t n_items, bool wide,
 // distance_trie.cu: the prefix-trie kernel
 size_t distance_trie_smem_bytes(bool wide);
 cudaError_t launch_distance_trie(const DistanceParams& p, int64_t n_items, bool wide, bool count_work,
+                                 cudaStream_t s, int* launches);
+
+// labels.cu: distance labels of the final edges, threshold restriction, key validation
+cudaError_t launch_inverse_perm(const int32_t* perm, int64_t n, int32_t* inv, cudaStream_t s, int* launches);
+cudaError_t launch_edge_distances(const int64_t* row_ptr, const int32_t* col, int64_t n, int64_t n_edges,
+                                  const int32_t* inv_perm, const uint8_t* pat, int pat_stride, uint8_t* dist,
+                                  cudaStream_t s, int* launches);
+// flags[e] = dist[e] <= l_max (uint32 0/1)
+cudaError_t launch_restrict_flags(const uint8_t* dist, int64_t n_edges, int l_max, uint32_t* flags, cudaStream_t s,
+                                  int* launches);
+// stable compaction of the kept edges into keys (row << 32 | col) and their labels
+cudaError_t launch_restrict_compact(const int64_t* row_ptr, const int32_t* col, const uint8_t* dist, int64_t n,
+                                    int64_t n_edges, const uint32_t* flags, const uint32_t* pos /*exclusive scan*/,
+                                    unsigned long long* keys_out, uint8_t* dist_out, cudaStream_t s, int* launches);
+// *flag |= 1 if any key has u >= v or v >= n
+cudaError_t launch_validate_keys(const unsigned long long* keys, int64_t n_keys, int64_t n, uint32_t* flag,
                                  cudaStream_t s, int* launches);
 
 // csr.cu

@@ -347,3 +347,102 @@ def test_cfg4_sampled_headline_config(pkg, oracle):
 def test_cfg5_sampled(pkg, oracle):
     """N = 2,000,000, l_max = 3, lengths 5..40 (patterns > 32 use 64-bit words)."""
     _sampled_parity(pkg, oracle, "cfg5", 3, 24, 5)
+
+
+# ------------------------------------------------------------------ 8(e): shards; 8(f): labels, sweep, query mode
+def test_shards_partition_the_edge_set(pkg, oracle):
+    """tcrnet_build_shard: the work items are dealt out to the shards interleaved; the shards' key
+    lists are disjoint, their union assembled by tcrnet_assemble is the oracle's network."""
+    import torch
+    d = generate("cfg2", n=20000)
+    for l_max, n_shards in ((1, 2), (3, 3), (2, 7)):
+        want = oracle.network(d.residues, d.lengths, l_max, tier=1)[:3]
+        with pkg.TcrNet(0) as net:
+            net.load(d.residues, d.lengths)
+            parts = [net.build_shard(l_max, r, n_shards).clone() for r in range(n_shards)]
+            allk = torch.cat(parts)
+            assert allk.numel() == int(want[0][-1]) and torch.unique(allk).numel() == allk.numel()
+            assert sum(p.numel() > 0 for p in parts) == n_shards          # every shard got real work
+            assert net.assemble(allk) == int(want[0][-1])
+            assert_same_network(net.copy_csr(), want)
+            # in-place assemble of one shard's own keys, then a plain build on the same context
+            k0 = net.build_shard(l_max, 0, n_shards)
+            assert net.assemble(k0) == parts[0].numel()
+            rp, cl, dg = net.copy_csr()
+            check_csr_invariants(rp, cl, dg, d.n)
+            net.build(l_max)
+            assert_same_network(net.copy_csr(), want)
+            # a key outside the strict upper triangle / the node range is rejected
+            bad = allk.clone()
+            bad[0] = (5 << 32) | 5
+            with pytest.raises(pkg.TcrNetError) as ei:
+                net.assemble(bad)
+            assert ei.value.status == pkg.ERR_ARG
+            bad[0] = (5 << 32) | d.n
+            with pytest.raises(pkg.TcrNetError):
+                net.assemble(bad)
+
+
+def test_edge_distances_and_threshold_sweep(pkg, oracle):
+    """NEXT-3: labels of a build at l_max = 4 equal the oracle's distances edge by edge, and the
+    chain restrict(3), restrict(2), ... reproduces the oracle's network at every threshold
+    (Fig. 2(i) sweeps l_max on one repertoire)."""
+    d = generate("cfg1")
+    off = np.concatenate([[0], np.cumsum(d.lengths)])
+    seq = lambda i: d.residues[off[i]:off[i + 1]]
+    with pkg.TcrNet(0) as net:
+        net.load(d.residues, d.lengths)
+        net.build(4)
+        rp, cl, dg = net.copy_csr()
+        dist = net.edge_distances().cpu().numpy()
+        assert dist.shape == cl.shape
+        rows = np.repeat(np.arange(d.n), np.diff(rp))
+        want_d = np.array([oracle.lev(seq(u), seq(v)) for u, v in zip(rows, cl)], dtype=np.uint8)
+        assert np.array_equal(dist, want_d)
+        for l in (4, 3, 2, 1, 0):
+            e = net.restrict(l)
+            want = oracle.network(d.residues, d.lengths, l, tier=0)[:3]
+            assert e == int(want[0][-1])
+            assert_same_network(net.copy_csr(), want)
+            lab = net.edge_distances().cpu().numpy()
+            assert lab.size == e and (lab <= l).all()
+        with pytest.raises(pkg.TcrNetError) as ei:
+            net.restrict(1)      # the network is now the one at l_max = 0
+        assert ei.value.status == pkg.ERR_LMAX
+
+
+def _query_network(oracle, d, n_query, l_max):
+    """Oracle side of the rectangular mode: rows 0..n_query-1 against every other row."""
+    pairs, _ = oracle.edges(d.residues, d.lengths, l_max, rows=np.arange(n_query), all_partners=True, tier=0)
+    lo, hi = pairs.min(axis=1), pairs.max(axis=1)
+    keys = np.unique((lo << 32) | hi)
+    canon = np.stack([keys >> 32, keys & 0xffffffff], axis=1)
+    return oracle.csr(canon, d.n)
+
+
+@pytest.mark.parametrize("n_query", [1, 37, 700])
+def test_query_mode(pkg, oracle, n_query):
+    """NEXT-2 (PAPER.md:109-115, antigen-specific networks): the first N_a rows are the queries;
+    the build keeps exactly the edges with at least one query endpoint."""
+    d = generate("cfg2", n=12000)
+    for l_max, opts in ((0, {}), (1, {}), (2, {}), (3, {pkg.OPT_PREFIX_TRIE: 0}), (4, {pkg.OPT_TRIE_CHUNK: 512})):
+        want = _query_network(oracle, d, n_query, l_max)
+        with pkg.TcrNet(0) as net:
+            for k, v in opts.items():
+                net.set_option(k, v)
+            net.set_option(pkg.OPT_N_QUERY, n_query)
+            net.load(d.residues, d.lengths)
+            net.build(l_max)
+            got = net.copy_csr()
+            st = net.get_stats()
+            assert_same_network(got, want)
+            assert (np.diff(got[0])[n_query:] == 0).all()                 # no row without a query endpoint
+            assert st["pairs_all"] == n_query * (n_query - 1) // 2 + n_query * (d.n - n_query)
+            # query mode off again on the same context -> the full network
+            net.set_option(pkg.OPT_N_QUERY, 0)
+            net.load(d.residues, d.lengths)
+            net.build(l_max)
+            full = net.copy_csr()
+        assert int(full[0][-1]) >= int(want[0][-1])
+        if l_max == 1:
+            assert_same_network(full, oracle.network(d.residues, d.lengths, 1, tier=1)[:3])
