@@ -39,8 +39,8 @@ ALU_OPS_PER_TEST = 4           # 2 LOP3 + IADD3 + ISETP per pair and early-exit 
 ALU_OPS_PER_PREFIX_TEST = 2    # LOP3 + ISETP per pair and DP cell read in a guided expansion (distance_trie.cu)
 ORACLE_SAMPLE_ROWS = 1024
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_distance_trie launch at cfg4, from the ncu --set full
-# capture summarised in profiles/r1b_trie_ncu.txt (95.23 MB + 21.60 MB)
-NCU_DRAM_BYTES_PER_LAUNCH = {"cfg4": 116_831_744}
+# capture summarised in profiles/r1c_trie_ncu.txt (94.63 MB + 22.30 MB)
+NCU_DRAM_BYTES_PER_LAUNCH = {"cfg4": 116_930_816}
 
 
 def _peaks():
@@ -51,35 +51,61 @@ def _peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    """SM clock / throttle reasons during the timed region (B200_PROFILING.md recipe).  The timed region
+    of this path is tens of milliseconds, far below nvidia-smi's shortest loop, so the sampler polls NVML
+    in-process (the same counters nvidia-smi prints) every ~1 ms; nvidia-smi -lms is the fallback."""
 
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index: int):
-        self.rows = []
+        self.rows = []      # (t, sm_mhz, set of reasons)
+        self.sm_max = None
+        self.stop_flag = False
         self.proc = None
+        self.source = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[index]) if vis and all(x.strip().isdigit() for x in vis.split(",")) else index
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.nv = pynvml
+            self.sm_max = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.source = "nvml"
+            self.thread = threading.Thread(target=self._poll_nvml, daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            self.nv = None
         try:
             self.proc = subprocess.Popen(
-                ["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                ["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "20"],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.source = "nvidia-smi"
+            self.thread = threading.Thread(target=self._pump_smi, daemon=True)
             self.thread.start()
         except Exception:
             self.proc = None
 
-    def _pump(self):
-        for line in self.proc.stdout:
-            self.rows.append((time.perf_counter(), line.strip()))
+    def _poll_nvml(self):
+        nv = self.nv
+        names = (("hw_slowdown", nv.nvmlClocksThrottleReasonHwSlowdown),
+                 ("hw_thermal_slowdown", nv.nvmlClocksThrottleReasonHwThermalSlowdown),
+                 ("sw_thermal_slowdown", nv.nvmlClocksThrottleReasonSwThermalSlowdown),
+                 ("sw_power_cap", nv.nvmlClocksThrottleReasonSwPowerCap))
+        while not self.stop_flag:
+            try:
+                clk = float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                self.rows.append((time.perf_counter(), clk, {n for n, bit in names if mask & bit}))
+            except Exception:
+                pass
+            time.sleep(0.001)
 
-    def stop(self, t0: float, t1: float) -> dict:
-        if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
-        self.proc.terminate()
-        sm, smax, reasons = [], [], set()
-        for t, line in self.rows:
+    def _pump_smi(self):
+        for line in self.proc.stdout:
             f = [x.strip() for x in line.split(",")]
             if len(f) < 7:
                 continue
@@ -87,14 +113,25 @@ class ClockSampler:
                 clk, mx = float(f[0]), float(f[1])
             except ValueError:
                 continue
-            smax.append(mx)
+            self.sm_max = mx
+            reasons = {n for n, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"),
+                                         f[3:7]) if v.lower().startswith("active")}
+            self.rows.append((time.perf_counter(), clk, reasons))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.source is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "samples": 0, "reasons": ["no clock source"]}
+        time.sleep(0.05)
+        self.stop_flag = True
+        if self.proc is not None:
+            self.proc.terminate()
+        sm, reasons = [], set()
+        for t, clk, rs in list(self.rows):
             if t0 <= t <= t1:
                 sm.append(clk)
-                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
-                    if v.lower().startswith("active"):
-                        reasons.add(name)
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
-                "samples": len(sm), "reasons": sorted(reasons)}
+                reasons |= rs
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": self.sm_max,
+                "samples": len(sm), "source": self.source, "reasons": sorted(reasons)}
 
 
 def oracle_sample(d, l_max: int, rows: int, seed: int = 0):

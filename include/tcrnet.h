@@ -99,7 +99,7 @@ typedef enum tcrnet_option {
                                      pair is visited by the text-chunk kernel.  Never changes the
                                      result.                                                   */
     TCRNET_OPT_TRIE_CHUNK = 8,    /* texts per work item of the prefix-trie kernel (multiple of
-                                     256; default 32768)                                       */
+                                     256; default 1048576)                                    */
     TCRNET_OPT_N_QUERY = 9        /* rectangular (query x repertoire) mode: the
                                      antigen-specific network "replaces the first N_a rows" by
                                      antigen-cognate sequences and analyses only those nodes.

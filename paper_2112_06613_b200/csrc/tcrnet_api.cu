@@ -60,7 +60,7 @@ struct tcrnet_ctx {
     int count_work = 0;
     int tchunk = 2048;
     int prefix_trie = 1;
-    int trie_chunk = 32768;
+    int trie_chunk = 1 << 20;  // in practice the whole text bucket: the top of the trie is walked once per pattern tile
 
     int64_t n_query = 0;  // > 0: rectangular mode (TCRNET_OPT_N_QUERY)
 
