@@ -229,6 +229,65 @@ TCRNET_API int tcrnet_edge_distances(tcrnet_ctx* ctx, const uint8_t** dist_dev);
 TCRNET_API int tcrnet_restrict(tcrnet_ctx* ctx, int l_max, int64_t* n_edges_out);
 
 /*
+ * ---- Network observables on the current CSR (what the paper does with the
+ * ---- 8e5-node network, Fig. 2(f)-(h); definitions in PAPER.md section II.G-II.J) ----------------
+ * All four need a built network (tcrnet_build / assemble / restrict), run on the context's stream,
+ * synchronise it, and return pointers owned by the context that stay valid until the CSR changes
+ * (next build / assemble / restrict / load) or the context is destroyed.  Errors: ARG, STATE,
+ * NOMEM, CUDA.
+ */
+
+/*
+ * Degree distribution ("the relative frequency of nodes with degree d"):
+ * *hist_dev -> device int64[*max_degree_out + 1], hist[d] = number of nodes with d(u) = d, so
+ * p_d = hist[d] / N and <d> = sum_d d p_d.  Either out pointer may be NULL.
+ */
+TCRNET_API int tcrnet_degree_histogram(tcrnet_ctx* ctx, const int64_t** hist_dev, int32_t* max_degree_out);
+
+/*
+ * Average neighbour degree (Eq. 9; Fig. 2(f)): with H = max degree + 1,
+ *   *nn_sum_dev    -> device int64[n]:  sum over the neighbours v of u of d(v)  (the average neighbour
+ *                     degree of node u is nn_sum[u] / d(u))
+ *   *class_sum_dev -> device int64[H]:  sum of nn_sum[u] over the nodes of degree d
+ *   *knn_dev       -> device double[H]: <d_nn>(d) = sum_d' d' P(d'|d) = class_sum[d] / (d * hist[d]),
+ *                     one IEEE-754 division of two exactly converted integers; 0 for d = 0 and for
+ *                     empty degree classes (reading Q15)
+ * Any out pointer may be NULL.
+ */
+TCRNET_API int tcrnet_neighbor_degree(tcrnet_ctx* ctx, const int64_t** nn_sum_dev, const int64_t** class_sum_dev,
+                                      const double** knn_dev);
+
+/*
+ * Connected components ("The largest connected component (LCC) is the largest
+ * connected subgraph"): *label_dev -> device int32[n], label[u] = smallest node id of u's component
+ * (unique); *comp_size_dev -> device int32[n], number of nodes of u's component (the cluster-size
+ * distribution of PAPER.md:224 is its histogram over the nodes with label[u] == u);
+ * *n_components_out, *lcc_out (host): number of components, size of the largest.  Any may be NULL.
+ */
+TCRNET_API int tcrnet_components(tcrnet_ctx* ctx, const int32_t** label_dev, const int32_t** comp_size_dev,
+                                 int64_t* n_components_out, int64_t* lcc_out);
+
+/*
+ * Site percolation / robustness (Fig. 2(g),(h)): nodes are removed along ONE
+ * removal order supplied by the caller (the method's random draw is an input: removal_rank[u] =
+ * position of node u in the order, a permutation of 0..n-1; reading Q14).  Step k looks at the
+ * subgraph induced by the nodes with removal_rank[u] >= n_removed[k] (p = n_removed[k] / N) and
+ * reports
+ *   lcc_out[k]        size of its largest connected component, LCC(p)
+ *   lcc_norm1_out[k]  Eq. 12: LCC(p) / ((1 - p) N) = LCC / (N - n_removed[k]); 0 when
+ *                     nothing is left (reading Q16)
+ *   lcc_norm2_out[k]  Eq. 13: Eq. 12 divided by its value at p = 0
+ *   deg_hist_out      int64[n_steps][max_degree + 1] (max_degree of the full network, see
+ *                     tcrnet_degree_histogram): degree histogram of the remaining subgraph, Fig. 2(h)
+ * removal_rank: host int32[n]; n_removed: host int64[n_steps], each in 0..n, any order; the four outputs
+ * are host arrays, each may be NULL.  n_steps >= 0.  The CSR itself is not modified.
+ * Errors: ARG (not a permutation, a step outside 0..n), STATE, NOMEM, CUDA.
+ */
+TCRNET_API int tcrnet_percolation(tcrnet_ctx* ctx, const int32_t* removal_rank, const int64_t* n_removed,
+                                  int32_t n_steps, int64_t* lcc_out, double* lcc_norm1_out, double* lcc_norm2_out,
+                                  int64_t* deg_hist_out);
+
+/*
  * Borrow the CSR of the last build: *row_ptr_dev -> device int64[n+1], *col_dev -> device
  * int32[|E|] (NULL when |E| = 0).  Row i lists the neighbours j > i in ascending order;
  * row_ptr[n] = |E|.  Owned by the context, valid until the next tcrnet_build / tcrnet_load /

@@ -27,7 +27,8 @@ EXPORTS = (
     "tcrnet_create", "tcrnet_destroy", "tcrnet_load", "tcrnet_load_device", "tcrnet_build", "tcrnet_csr",
     "tcrnet_degrees", "tcrnet_copy_csr", "tcrnet_set_option", "tcrnet_get_stats", "tcrnet_probe_int32",
     "tcrnet_last_cuda_error", "tcrnet_strerror", "tcrnet_version", "tcrnet_build_shard", "tcrnet_assemble",
-    "tcrnet_edge_distances", "tcrnet_restrict",
+    "tcrnet_edge_distances", "tcrnet_restrict", "tcrnet_degree_histogram", "tcrnet_neighbor_degree",
+    "tcrnet_components", "tcrnet_percolation",
 )
 
 
@@ -88,6 +89,15 @@ def load_library() -> C.CDLL:
     lib.tcrnet_edge_distances.argtypes = [vp, C.POINTER(vp)]
     lib.tcrnet_restrict.restype = C.c_int
     lib.tcrnet_restrict.argtypes = [vp, C.c_int, i64p]
+    lib.tcrnet_degree_histogram.restype = C.c_int
+    lib.tcrnet_degree_histogram.argtypes = [vp, C.POINTER(vp), i32p]
+    lib.tcrnet_neighbor_degree.restype = C.c_int
+    lib.tcrnet_neighbor_degree.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
+    lib.tcrnet_components.restype = C.c_int
+    lib.tcrnet_components.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), i64p, i64p]
+    lib.tcrnet_percolation.restype = C.c_int
+    lib.tcrnet_percolation.argtypes = [vp, i32p, i64p, C.c_int32, i64p, C.POINTER(C.c_double),
+                                       C.POINTER(C.c_double), i64p]
     lib.tcrnet_csr.restype = C.c_int
     lib.tcrnet_csr.argtypes = [vp, C.POINTER(vp), C.POINTER(vp)]
     lib.tcrnet_degrees.restype = C.c_int
@@ -246,6 +256,50 @@ class TcrNet:
         _check(self._lib.tcrnet_restrict(self._ctx, int(l_max), C.byref(e)), "tcrnet_restrict")
         self.n_edges = int(e.value)
         return self.n_edges
+
+    # -- network observables on the current CSR -------------------------
+    def degree_histogram(self) -> "torch.Tensor":
+        """tcrnet_degree_histogram: int64[max_degree + 1] (a view of library memory)."""
+        h, m = C.c_void_p(), C.c_int32(0)
+        _check(self._lib.tcrnet_degree_histogram(self._ctx, C.byref(h), C.byref(m)), "tcrnet_degree_histogram")
+        return self._view(h.value, self._torch.int64, int(m.value) + 1)
+
+    def neighbor_degree(self):
+        """tcrnet_neighbor_degree: (nn_sum int64[n], class_sum int64[H], knn float64[H]) views, H = max degree + 1."""
+        torch = self._torch
+        hist_len = int(self.degree_histogram().numel())
+        a, b, c = C.c_void_p(), C.c_void_p(), C.c_void_p()
+        _check(self._lib.tcrnet_neighbor_degree(self._ctx, C.byref(a), C.byref(b), C.byref(c)), "tcrnet_neighbor_degree")
+        return (self._view(a.value, torch.int64, self.n), self._view(b.value, torch.int64, hist_len),
+                self._view(c.value, torch.float64, hist_len))
+
+    def components(self):
+        """tcrnet_components: (label int32[n], comp_size int32[n], n_components, lcc)."""
+        torch = self._torch
+        a, b, nc, lcc = C.c_void_p(), C.c_void_p(), C.c_int64(0), C.c_int64(0)
+        _check(self._lib.tcrnet_components(self._ctx, C.byref(a), C.byref(b), C.byref(nc), C.byref(lcc)),
+               "tcrnet_components")
+        return (self._view(a.value, torch.int32, self.n), self._view(b.value, torch.int32, self.n), int(nc.value),
+                int(lcc.value))
+
+    def percolation(self, removal_rank, n_removed, deg_hist: bool = False):
+        """tcrnet_percolation: (lcc int64[K], lcc_norm1 float64[K], lcc_norm2 float64[K], deg_hist int64[K, H] or
+        None) as numpy arrays; removal_rank is a host permutation of 0..n-1, n_removed the steps."""
+        rank = np.ascontiguousarray(removal_rank, dtype=np.int32)
+        steps = np.ascontiguousarray(n_removed, dtype=np.int64)
+        if rank.size != self.n:
+            raise TcrNetError(ERR_ARG, "tcrnet_percolation (removal_rank must have n entries)")
+        k = int(steps.size)
+        lcc = np.zeros(k, dtype=np.int64)
+        n1 = np.zeros(k, dtype=np.float64)
+        n2 = np.zeros(k, dtype=np.float64)
+        hist = np.zeros((k, int(self.degree_histogram().numel())), dtype=np.int64) if deg_hist else None
+        f64p = C.POINTER(C.c_double)
+        _check(self._lib.tcrnet_percolation(
+            self._ctx, rank.ctypes.data_as(C.POINTER(C.c_int32)), steps.ctypes.data_as(C.POINTER(C.c_int64)), k,
+            lcc.ctypes.data_as(C.POINTER(C.c_int64)), n1.ctypes.data_as(f64p), n2.ctypes.data_as(f64p),
+            hist.ctypes.data_as(C.POINTER(C.c_int64)) if hist is not None else None), "tcrnet_percolation")
+        return lcc, n1, n2, hist
 
     def _view(self, ptr: int, dtype, count: int):
         """Zero-copy torch view of library-owned device memory (it was allocated by torch)."""

@@ -6,102 +6,7 @@
 #include <new>
 #include <vector>
 
-#include "tcrnet_internal.h"
-
-using namespace tcrnet;
-
-namespace {
-
-struct DevBuf {
-    void* p = nullptr;
-    size_t bytes = 0;
-};
-
-struct HostCtrl {  // pinned mirror of the small device control block
-    unsigned long long hist[kNumLen];
-    unsigned long long edge_count;
-    unsigned long long work[4];
-    unsigned long long probe[3];
-    uint32_t flags;
-    uint32_t pad_;
-    uint32_t trie_counts[8];          // [k] = nodes of trie level k
-    uint32_t trie_root[kNumLen + 1];  // [L] = first level-1 node of length bucket L (non-empty buckets)
-};
-
-}  // namespace
-
-// One packed set of sequences: all rows, or the query rows of the rectangular mode.
-struct SeqSet {
-    bool loaded = false;
-    int64_t n = 0, total_len = 0;
-    int64_t hist[kNumLen] = {};
-    int min_len = 0, max_len = 0;
-    LengthTable lt{};
-    int pat_stride = 0;
-    DevBuf perm, pat, txt, trie;
-    TrieLevels trie_levels{};
-    uint32_t trie_root[kNumLen + 1] = {};  // level-1 node range of bucket L: [trie_root[L], trie_root[L+1])
-    int64_t trie_nodes = 0;
-};
-
-struct tcrnet_ctx {
-    int device = 0;
-    cudaStream_t stream = nullptr;
-    tcrnet_allocator alloc{};
-    bool has_alloc = false;
-    int last_cuda = 0;
-    int n_sm = 0;
-
-    // options
-    int early_exit = 1;
-    int first_check_opt = 0;
-    int64_t edge_capacity_opt = 0;
-    int64_t edge_limit = (int64_t)1 << 31;
-    int count_work = 0;
-    int tchunk = 2048;
-    int prefix_trie = 1;
-    int trie_chunk = 1 << 20;  // in practice the whole text bucket: the top of the trie is walked once per pattern tile
-
-    int64_t n_query = 0;  // > 0: rectangular mode (TCRNET_OPT_N_QUERY)
-
-    // load state
-    bool loaded = false;
-    int64_t n = 0;
-    SeqSet all, query;
-    DevBuf in_res, in_len, offsets, perm_tmp, trie_scratch;  // load scratch, kept between loads (grow-only)
-
-    // build state
-    bool built = false;      // CSR + degrees valid
-    bool have_keys = false;  // tcrnet_build_shard left unsorted keys in keys_a
-    bool have_dist = false;  // edge_dist valid for the current CSR
-    int built_l_max = 0;
-    int64_t n_edges = 0, n_keys = 0;
-    DevBuf keys_a, keys_b, split_hist, split_hist_scanned, scan_scratch, rows, row_ptr, col, deg;
-    DevBuf inv_perm, edge_dist, edge_dist_b, flags, flag_pos;
-
-    DevBuf ctrl;               // device HostCtrl
-    HostCtrl* h_ctrl = nullptr;  // pinned
-    cudaEvent_t ev[6] = {};
-    tcrnet_stats stats{};
-};
-
-namespace {
-
-#define TRY_CUDA(expr)                         \
-    do {                                       \
-        cudaError_t e__ = (expr);              \
-        if (e__ != cudaSuccess) {              \
-            ctx->last_cuda = (int)e__;         \
-            (void)cudaGetLastError();          \
-            return TCRNET_ERR_CUDA;            \
-        }                                      \
-    } while (0)
-
-#define TRY(expr)                     \
-    do {                              \
-        int rc__ = (expr);            \
-        if (rc__ != TCRNET_OK) return rc__; \
-    } while (0)
+#include "tcrnet_ctx.h"
 
 void dev_free(tcrnet_ctx* ctx, DevBuf& b) {
     if (b.p) {
@@ -132,6 +37,10 @@ int dev_reserve(tcrnet_ctx* ctx, DevBuf& b, size_t bytes) {
     return TCRNET_OK;
 }
 
+void drop_observables(tcrnet_ctx* ctx) { ctx->have_hist = ctx->have_nn = ctx->have_cc = false; }
+
+namespace {
+
 HostCtrl* d_ctrl(tcrnet_ctx* ctx) { return static_cast<HostCtrl*>(ctx->ctrl.p); }
 
 int bits_for(int64_t max_value) {  // number of bits needed to represent max_value (>= 1)
@@ -141,6 +50,7 @@ int bits_for(int64_t max_value) {  // number of bits needed to represent max_val
 }
 
 void drop_build(tcrnet_ctx* ctx) {
+    drop_observables(ctx);
     ctx->built = false;
     ctx->have_keys = false;
     ctx->have_dist = false;
@@ -539,6 +449,7 @@ int assemble_phase(tcrnet_ctx* ctx, int64_t n_keys, int* launches) {
     ctx->n_edges = n_keys;
     ctx->have_keys = false;  // the sort used keys_a
     ctx->have_dist = false;
+    drop_observables(ctx);
     ctx->built = true;
     return TCRNET_OK;
 }
@@ -622,7 +533,9 @@ void tcrnet_destroy(tcrnet_ctx* ctx) {
                       &ctx->flag_pos, &ctx->in_res, &ctx->in_len, &ctx->offsets,
                       &ctx->perm_tmp, &ctx->trie_scratch, &ctx->keys_a, &ctx->keys_b, &ctx->split_hist,
                       &ctx->split_hist_scanned, &ctx->scan_scratch, &ctx->rows, &ctx->row_ptr, &ctx->col,
-                      &ctx->deg, &ctx->ctrl};
+                      &ctx->deg, &ctx->ctrl, &ctx->obs_ctrl, &ctx->deg_hist, &ctx->nn_sum, &ctx->class_sum, &ctx->knn,
+                      &ctx->cc_parent, &ctx->cc_count, &ctx->cc_label, &ctx->cc_size, &ctx->perc_rank,
+                      &ctx->perc_seen, &ctx->perc_deg, &ctx->perc_hist, &ctx->perc_lcc};
     for (DevBuf* b : bufs) dev_free(ctx, *b);
     if (ctx->h_ctrl) cudaFreeHost(ctx->h_ctrl);
     for (cudaEvent_t ev : ctx->ev)
@@ -741,6 +654,7 @@ int tcrnet_assemble(tcrnet_ctx* ctx, const uint64_t* keys_dev, int64_t n_keys, i
     if (in_place && !(ctx->have_keys && n_keys <= ctx->n_keys)) return TCRNET_ERR_ARG;
     ctx->built = false;
     ctx->have_dist = false;
+    drop_observables(ctx);
     int launches = 0;
     if (!in_place) {
         // keys_dev may not alias the context's buffers: reserve first (contents are not preserved), then copy
@@ -785,6 +699,7 @@ int tcrnet_restrict(tcrnet_ctx* ctx, int l_max, int64_t* n_edges_out) {
     TRY(ensure_edge_distances(ctx, &launches));
     const int64_t e_old = ctx->n_edges;
     int64_t e_new = 0;
+    drop_observables(ctx);
     TRY_CUDA(cudaEventRecord(ctx->ev[1], s));
     if (e_old > 0) {
         TRY(dev_reserve(ctx, ctx->flags, sizeof(uint32_t) * (size_t)e_old));

@@ -1,0 +1,108 @@
+// The context behind the opaque tcrnet_ctx of include/tcrnet.h, shared by the translation units that
+// implement the C ABI (tcrnet_api.cu: load / build / CSR; observables_api.cu: network observables).
+// Internal to libtcrnet_b200.so.
+#pragma once
+
+#include "tcrnet_internal.h"
+
+using namespace tcrnet;
+
+struct DevBuf {
+    void* p = nullptr;
+    size_t bytes = 0;
+};
+
+struct HostCtrl {  // pinned mirror of the small device control block
+    unsigned long long hist[kNumLen];
+    unsigned long long edge_count;
+    unsigned long long work[4];
+    unsigned long long probe[3];
+    uint32_t flags;
+    uint32_t pad_;
+    uint32_t trie_counts[8];          // [k] = nodes of trie level k
+    uint32_t trie_root[kNumLen + 1];  // [L] = first level-1 node of length bucket L (non-empty buckets)
+};
+
+// One packed set of sequences: all rows, or the query rows of the rectangular mode.
+struct SeqSet {
+    bool loaded = false;
+    int64_t n = 0, total_len = 0;
+    int64_t hist[kNumLen] = {};
+    int min_len = 0, max_len = 0;
+    LengthTable lt{};
+    int pat_stride = 0;
+    DevBuf perm, pat, txt, trie;
+    TrieLevels trie_levels{};
+    uint32_t trie_root[kNumLen + 1] = {};  // level-1 node range of bucket L: [trie_root[L], trie_root[L+1])
+    int64_t trie_nodes = 0;
+};
+
+struct tcrnet_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    tcrnet_allocator alloc{};
+    bool has_alloc = false;
+    int last_cuda = 0;
+    int n_sm = 0;
+
+    // options
+    int early_exit = 1;
+    int first_check_opt = 0;
+    int64_t edge_capacity_opt = 0;
+    int64_t edge_limit = (int64_t)1 << 31;
+    int count_work = 0;
+    int tchunk = 2048;
+    int prefix_trie = 1;
+    int trie_chunk = 1 << 20;  // in practice the whole text bucket: the top of the trie is walked once per pattern tile
+
+    int64_t n_query = 0;  // > 0: rectangular mode (TCRNET_OPT_N_QUERY)
+
+    // load state
+    bool loaded = false;
+    int64_t n = 0;
+    SeqSet all, query;
+    DevBuf in_res, in_len, offsets, perm_tmp, trie_scratch;  // load scratch, kept between loads (grow-only)
+
+    // build state
+    bool built = false;      // CSR + degrees valid
+    bool have_keys = false;  // tcrnet_build_shard left unsorted keys in keys_a
+    bool have_dist = false;  // edge_dist valid for the current CSR
+    int built_l_max = 0;
+    int64_t n_edges = 0, n_keys = 0;
+    DevBuf keys_a, keys_b, split_hist, split_hist_scanned, scan_scratch, rows, row_ptr, col, deg;
+    DevBuf inv_perm, edge_dist, edge_dist_b, flags, flag_pos;
+
+    // observables state (observables_api.cu); valid for the current CSR only
+    bool have_hist = false, have_nn = false, have_cc = false;
+    int32_t max_degree = 0;
+    int64_t n_components = 0, lcc = 0;
+    DevBuf obs_ctrl, deg_hist, nn_sum, class_sum, knn, cc_parent, cc_count, cc_label, cc_size;
+    DevBuf perc_rank, perc_seen, perc_deg, perc_hist, perc_lcc;
+
+    DevBuf ctrl;               // device HostCtrl
+    HostCtrl* h_ctrl = nullptr;  // pinned
+    cudaEvent_t ev[6] = {};
+    tcrnet_stats stats{};
+};
+
+#define TRY_CUDA(expr)                         \
+    do {                                       \
+        cudaError_t e__ = (expr);              \
+        if (e__ != cudaSuccess) {              \
+            ctx->last_cuda = (int)e__;         \
+            (void)cudaGetLastError();          \
+            return TCRNET_ERR_CUDA;            \
+        }                                      \
+    } while (0)
+
+#define TRY(expr)                     \
+    do {                              \
+        int rc__ = (expr);            \
+        if (rc__ != TCRNET_OK) return rc__; \
+    } while (0)
+
+
+// tcrnet_api.cu
+void dev_free(tcrnet_ctx* ctx, DevBuf& b);
+int dev_reserve(tcrnet_ctx* ctx, DevBuf& b, size_t bytes);  // at least `bytes` (contents not preserved)
+void drop_observables(tcrnet_ctx* ctx);                     // the CSR changed: cached observables are stale

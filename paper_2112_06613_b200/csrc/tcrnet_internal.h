@@ -167,6 +167,27 @@ cudaError_t launch_validate_keys(const unsigned long long* keys, int64_t n_keys,
 cudaError_t launch_csr(const unsigned long long* sorted_keys, int64_t n_edges, int64_t n, int64_t* row_ptr,
                        int32_t* col, int32_t* deg, cudaStream_t s, int* launches);
 
+// observables.cu: network observables on the CSR (degree distribution, Eq. 9, components, percolation steps)
+cudaError_t launch_max_degree(const int32_t* deg, int64_t n, int32_t* out /*zeroed*/, cudaStream_t s, int* launches);
+// hist[d] += number of alive nodes with deg[u] = d (rank == NULL: all nodes; else alive <=> rank[u] >= threshold)
+cudaError_t launch_degree_hist(const int32_t* deg, int64_t n, const int32_t* rank, int32_t threshold,
+                               unsigned long long* hist /*zeroed*/, cudaStream_t s, int* launches);
+// nn_sum, class_sum zeroed by the caller; knn[d] = class_sum[d] / (d * hist[d])
+cudaError_t launch_neighbor_degree(const int64_t* row_ptr, const int32_t* col, const int32_t* deg, int64_t n,
+                                   const unsigned long long* hist, int32_t hist_len, unsigned long long* nn_sum,
+                                   unsigned long long* class_sum, double* knn, cudaStream_t s, int* launches);
+// union-find over the edges with two alive ends: label[u] (may be NULL) = smallest id of u's component (-1: dead),
+// count[root] = component size, *lcc = max size, *n_comp = number of components (both zeroed by the caller);
+// sub_deg (may be NULL) = degrees inside the induced subgraph.
+cudaError_t launch_components(const int64_t* row_ptr, const int32_t* col, int64_t n, const int32_t* rank,
+                              int32_t threshold, int32_t* parent, int32_t* count, int32_t* label, int32_t* sub_deg,
+                              unsigned long long* lcc, unsigned long long* n_comp, cudaStream_t s, int* launches);
+cudaError_t launch_component_sizes(int64_t n, const int32_t* label, const int32_t* count, int32_t* comp_size,
+                                   cudaStream_t s, int* launches);
+// *flag |= 1 unless rank is a permutation of 0..n-1; seen: zeroed uint32[(n + 31) / 32]
+cudaError_t launch_check_permutation(const int32_t* rank, int64_t n, uint32_t* seen, uint32_t* flag, cudaStream_t s,
+                                     int* launches);
+
 // probe.cu
 cudaError_t launch_probe(int kind, int n_sm, unsigned long long* out /*[2]: ops, cycles*/, float* ms,
                          cudaStream_t s);
