@@ -1,5 +1,5 @@
-// Steps A3-A5, prefix-trie kernel (the default whenever the early exit is on and can act within
-// the first kTrieDepth text columns).
+// Steps A3-A5, prefix-trie kernel (the default whenever the early exit is on, l_max <= kTrieMaxL and
+// the texts are longer than the trie is deep).
 //
 // Same arithmetic as distance.cu - the Myers/Hyyro column recurrence of myers.cuh, the exact
 // final-diagonal early exit, warp-aggregated emission - but the texts of a
@@ -10,153 +10,201 @@
 //     neighbours in lexicographic order) walks the trie depth-first.  Entering a level-k node
 //     costs ONE column step (its residue code at position k-1) on top of the parent's (Pv, Mv):
 //     the columns of a shared prefix are computed once per node, not once per text.
-//   * Early exit: the cell D[k - delta][k] of the final diagonal is a lower bound of
-//     lev(pattern, text) for EVERY text below a level-k node, so a node where it exceeds l_max in
-//     all 32 lanes is dead with its whole subtree.  PAPER.md:326 ("abort, as soon as the smallest
-//     intermediate result exceeds" l_max) - here one abort disposes of a whole run of texts.
+//   * The final-diagonal cell is TRACKED, not recomputed: with i = k - delta (delta = n - m),
+//     dg = D[i][k] is carried along the walk and a column step updates it from its own D0 word,
+//         D[i][k] = D[i-1][k-1] + 1 - D0[bit i-1]        (D0 bit = "the diagonal did not increase"),
+//     starting from D[0][delta] = delta.  DP values never decrease along a diagonal and
+//     lev(pattern, text) = D[m][n] is the last cell of this one, so dg > l_max in all 32 lanes kills
+//     the node with its whole subtree ("abort, as soon as the smallest intermediate
+//     result exceeds" l_max - here one abort disposes of a whole run of texts), and after the last
+//     column dg IS the distance: no popcount anywhere.
 //   * Dead children are not even visited ("guided expansion"; levels k <= l_max have no dead
-//     children and are walked in full): before a node's children are walked, every lane derives from
-//     its parent column (Pv, Mv) the exact set V of residue codes c whose child would be alive,
-//         D_c[i][k] = min( D_0[i][k],  min over rows r <= i with a_r = c of D[r-1][k-1] + (i - r) ),
-//     (i = k - delta; D_0 = the column of a code that matches nowhere), i.e.
-//         V = (all codes, if D_0[i][k] <= l_max)  |  { a_(i-t) : D[i-1-t][k-1] + 2t <= l_max, t = 0..l_max }
-//     with D_0[i][k] <= l_max  <=>  D[i][k-1] <= l_max - 1  or  D[i-1-u][k-1] <= l_max - 1 - 2u for
-//     some u in 0..l_max-1.  Each cell costs one LOP3 + POPC + compare.  The warp visits the
-//     children whose code is in the OR of the 32 lanes' V (one REDUX) and in the node's child-code
-//     bitmap; the child's slot is popc(bitmap & low(code)).  V is exact, so no per-child test is
-//     needed.
+//     children and are walked in full).  Before a node's children are walked, every lane derives
+//     from its parent column (Pv, Mv, dg = D[i-1][k-1]) the exact set V of residue codes c whose
+//     child would be alive, i.e. D_c[i][k] = dg + 1 - D0_c[bit i-1] <= l_max:
+//         dg <  l_max                       V = all codes
+//         dg == l_max, Mv[bit i-1] set      V = all codes      (D0_c >= Mv for every c)
+//         dg == l_max                       V = { a_i } + { a_(i-t) : Pv[bits i-1-t .. i-2] all set, t >= 1 }
+//         dg >  l_max                       V = {}             (the lane is dead for good)
+//     (the three terms of D0 = carry | Eq | Mv; a carry reaches bit i-1 from a match at bit i-1-t
+//     through t set bits of Pv).  D[i-1-t][k-1] = dg - t >= delta + t bounds t by (l_max - delta) / 2,
+//     so the t-loop has 0 iterations for l_max <= 1, one for l_max <= 3, two for l_max = 4.
+//     The warp visits the children whose code is in the OR of the 32 lanes' V (one REDUX) and in the
+//     node's child-code bitmap.  V is exact, so no per-child test is needed.
 //   * Texts below a surviving level-kTrieDepth node are finished column by column from the node's
-//     state (a test after every second column), then the distance is read off Pv / Mv and
-//     surviving pairs are emitted as in distance.cu.
+//     state (a vote after every second column); surviving pairs (dg <= l_max after column n) are
+//     emitted as in distance.cu.
 //
 // Everything a warp does is warp-uniform (all lanes visit the same node / text), so there is no
 // divergence; lanes differ only in their pattern.  The children of the node being expanded
 // (<= 27, plus the next node as sentinel) are fetched with one coalesced 128-bit load per lane and
-// staged in a per-warp, per-level shared-memory buffer; the walk then reads them with broadcast
-// LDS.128.
+// staged in a per-warp, per-level shared-memory buffer INDEXED BY RESIDUE CODE as
+// (text_begin, text_end, child_begin, child_codes); the walk reads a child with one broadcast LDS.128.
 //
-// A cell needs one POPC: with v = ((Pv & 0xffff) | (Mv << 16)) ^ 0xffff0000 (PRMT + LOP3, once per
-// node) and mask2(r) = low(r) in both halves, popc(v & mask2(r)) = popc(Pv & low(r)) + r - popc(Mv & low(r))
-// = D[r][k-1] - (k-1) + r, so for r = i-1-u:  D[r][k-1] = popc(v & mask2(r)) + delta + u.
+// The kernel is specialised on l_max (template LMAX = 0..kTrieMaxL): thresholds are immediates and
+// the t-loop is unrolled to its exact trip count.  delta is run-time but warp-uniform; it enters only
+// through six precomputed bit masks.
 #include "myers.cuh"
 
 namespace tcrnet {
 namespace {
 
 constexpr uint32_t kFull = 0xffffffffu;
-constexpr int kClipLevels = 3;  // levels whose nodes are clipped to the work item's text chunk
+constexpr int kClipLevels = 3;      // levels whose nodes are clipped to the work item's text chunk
+constexpr int kDeadLane = 1 << 20;  // dg of a lane without a pattern: never alive, never emitted
+#ifndef TCRNET_SMALL_SUBTREE
+#define TCRNET_SMALL_SUBTREE 0
+#endif
+// subtrees of <= this many texts leave the trie and are finished text by text (0: never)
+constexpr uint32_t kSmallSubtree = TCRNET_SMALL_SUBTREE;
 
 template <typename W, bool COUNT>
 struct Walk {
-    uint4* stage;             // this warp's staging buffers: [kTrieDepth][kTrieFan] nodes
-    const uint32_t* rows;     // first text row of the text bucket
+    uint32_t stage_addr;      // shared address of this warp's staging buffers: [kTrieDepth][kTrieFan] children by code
     uint32_t lane_addr;       // shared address of this lane's Peq column
-    uint32_t t_start;         // sorted position of the bucket's first text
+    const uint32_t* rows;     // text row of sorted position 0 of this bucket's numbering (bucket base - t_start rows)
     uint32_t lo, hi;          // texts [lo, hi) (sorted positions) are this warp's share of the bucket
-    uint32_t mask2[kTrieDepth + 1];  // [q] = low(q - delta) in both 16-bit halves (0 when q <= delta)
-    uint32_t ohs[kTrieDepth + 1];    // [q] = 1 << code of pattern row q - delta (0: no such row / no pattern)
-    W pv_init, x_init, m_mask;
-    int rw, n, delta;
-    int thr;                  // l_max - delta; -1 in lanes without a pattern
-    int l_max;                // warp-uniform
-    int l_max_lane;           // l_max; -1 in lanes without a pattern
-    int lane, p_sorted, diag;
-    unsigned long long n_cols = 0, n_tests = 0, n_first = 0, n_ptests = 0;
+    uint32_t ohs[kTrieDepth + 1];   // [q] = 1 << code of pattern row q - delta (0: no such row / no pattern)
+    uint32_t dsh;             // delta + 1: the bit of pattern row q - delta is (1 << q) >> dsh (0 when q <= delta)
+    W pv_init;
+    int rw, n;
+    int lane, p_sorted;
+    int p_lim;                // same bucket: p_sorted (only sorted p < t counts); else -1
+    unsigned long long n_cols = 0, n_tests = 0, n_first = 0, n_vsets = 0;
+
+    __device__ __forceinline__ uint32_t dbit(int q) const { return (1u << q) >> dsh; }
 };
 
-// The texts [t0, t1) below a surviving deepest-level node: remaining columns, distance, emission.
-template <typename W, bool COUNT>
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void sts128(uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
+__device__ __forceinline__ uint32_t top_bit(uint32_t x) {  // index of the highest set bit (x != 0)
+    uint32_t r;
+    asm("bfind.u32 %0, %1;" : "=r"(r) : "r"(x));
+    return r;
+}
+
+// The texts [t0, t1) of a surviving subtree, one by one: the text columns START .. n-1 (0-based) on top
+// of the state (Pv0, Mv0, dg0) after START columns, with the tracked final-diagonal cell; emission.
+// START = kTrieDepth below a deepest-level node; START = LEVEL - 1 for the small subtrees that leave the
+// trie early (visit()).  START >= l_max >= delta, so every column has its final-diagonal row.
+template <typename W, int LMAX, bool COUNT, int START>
 __device__ __forceinline__ void finish_texts(Walk<W, COUNT>& w, const DistanceParams& P, uint32_t t0, uint32_t t1,
-                                             const W Pv0, const W Mv0) {
+                                             const W Pv0, const W Mv0, const int dg0) {
+    static_assert(START >= 1 && START >= LMAX, "column 0 has its own step; final-diagonal rows exist from column delta on");
+    constexpr int kJ0 = START & ~3;  // the 128-bit load that holds column START
+    // exit vote after every column, or after every second one for l_max <= 1 (measured: cfg4 / cfg5)
+    constexpr int kVoteEvery = LMAX >= 2 ? 1 : 2;
     for (uint32_t t = t0; t < t1; ++t) {
-        const uint32_t* row = w.rows + (size_t)(t - w.t_start) * w.rw;
+        const uint4* row = reinterpret_cast<const uint4*>(w.rows + (size_t)t * w.rw);
         W Pv = Pv0, Mv = Mv0;
+        W bm = (W)w.dbit(START + 1);  // bit of row j + 1 - delta for column j = START
+        int dg = dg0;
         bool dead = false;
-        for (int j0 = kTrieDepth & ~3; j0 < w.n && !dead; j0 += 4) {
-            const uint4 c4 = __ldg(reinterpret_cast<const uint4*>(row + j0));  // same address in all lanes
+        // four columns per 128-bit load (the same address in all lanes)
+        for (int j0 = kJ0; j0 < w.n; j0 += 4) {
+            const uint4 c4 = __ldg(row + (j0 >> 2));
             const uint32_t c[4] = {c4.x, c4.y, c4.z, c4.w};
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
+                if (j0 == kJ0 && q < (START & 3)) continue;  // columns already in (Pv0, Mv0)
                 const int j = j0 + q;
-                if (j < kTrieDepth || j >= w.n || dead) continue;
-                column_step<W>(peq_load<W>(w.lane_addr, c[q]), Pv, Mv);
+                if (j >= w.n) break;  // warp-uniform
+                const W D0 = column_step<W>(peq_load<W>(w.lane_addr, c[q]), Pv, Mv);
+                if ((D0 & bm) == W(0)) ++dg;
+                bm += bm;
                 if (COUNT) ++w.n_cols;
-                const int jj = j + 1;
-                if ((jj & 1) == 0 && jj < w.n && jj > w.delta) {
-                    const W msk = low_mask<W>(jj - w.delta);
-                    const int lb = jj + WordOps<W>::popc(Pv & msk) - WordOps<W>::popc(Mv & msk);
+                if (kVoteEvery == 1 || (q & 1)) {
                     if (COUNT) ++w.n_tests;
-                    if (!__any_sync(kFull, lb <= w.l_max_lane)) dead = true;
+                    if (!__any_sync(kFull, dg <= LMAX)) {
+                        dead = true;
+                        break;
+                    }
                 }
             }
+            if (dead) break;
         }
         if (dead) continue;
-        const int d = w.n + WordOps<W>::popc(Pv & w.m_mask) - WordOps<W>::popc(Mv & w.m_mask);
-        const bool edge = d <= w.l_max_lane && (!w.diag || (uint32_t)w.p_sorted < t);
-        emit_edges(P, edge, w.lane, w.p_sorted, (int)t, w.n - w.delta, w.n);
+        const bool edge = dg <= LMAX && w.p_lim < (int)t;
+        emit_edges(P, edge, w.lane, w.p_sorted, (int)t, w.n - (int)w.dsh + 1, w.n);
     }
 }
 
-// Expand the level-LEVEL nodes [cb, ce) (the children of one level-(LEVEL-1) node, or the roots of
-// the text bucket) whose residue codes are the set bits of cm; (Pv, Mv) is the DP column after
-// LEVEL-1 text residues.
-template <typename W, bool COUNT, int LEVEL>
-__device__ __forceinline__ void visit(Walk<W, COUNT>& w, const DistanceParams& P, uint32_t cb, uint32_t ce,
-                                      uint32_t cm, const W Pv, const W Mv) {
+// Expand the children (level LEVEL, nodes [cb, cb + popc(cm)), residue codes = the set bits of cm) of
+// one level-(LEVEL-1) node, or the roots of the text bucket.  (Pv, Mv) is the DP column after LEVEL-1
+// text residues and dg = D[LEVEL-1-delta][LEVEL-1] its final-diagonal cell (delta while there is none).
+template <typename W, int LMAX, bool COUNT, int LEVEL>
+__device__ __forceinline__ void visit(Walk<W, COUNT>& w, const DistanceParams& P, uint32_t cb, uint32_t cm,
+                                      const W Pv, const W Mv, const int dg) {
     uint32_t U = cm;
     // Guided expansion: the codes whose child is alive in at least one lane.  Every child is alive
-    // while LEVEL <= l_max (D[i][k] <= k), and there is no final-diagonal cell while LEVEL <= delta.
-    if (LEVEL > w.l_max && LEVEL > w.delta) {  // warp-uniform
-        const uint32_t v = __byte_perm((uint32_t)Pv, (uint32_t)Mv, 0x5410) ^ 0xffff0000u;
-        bool alive0 = __popc(v & w.mask2[LEVEL]) <= w.thr;  // D[i][k-1] <= l_max - 1
-        uint32_t V = 0u;
+    // while LEVEL <= l_max (D[i][k] <= k); LEVEL > l_max >= delta, so row i = LEVEL - delta exists.
+    if constexpr (LEVEL > LMAX) {
+        const uint32_t b = w.dbit(LEVEL);
+        uint32_t V = w.ohs[LEVEL];
 #pragma unroll
-        for (int t = 0; t < LEVEL; ++t) {
-            if (t <= w.l_max) {  // warp-uniform
-                const int pt = __popc(v & w.mask2[LEVEL - 1 - t]);  // D[i-1-t][k-1] - delta - t
-                alive0 = alive0 || (pt <= w.thr - 1 - 2 * t);
-                if (pt <= w.thr - 2 * t) V |= w.ohs[LEVEL - t];
-                if (COUNT) ++w.n_ptests;
-            }
+        for (int t = 1; t <= LMAX / 2; ++t) {
+            const uint32_t run = b - (b >> t);  // bits i-1-t .. i-2 (b itself when there is no row i-t: ohs = 0)
+            if (((uint32_t)Pv & run) == run) V |= w.ohs[LEVEL - t];
         }
-        if (COUNT) ++w.n_ptests;
-        if (alive0) V = kFull;
+        if (dg != LMAX) V = 0u;
+        if (dg < LMAX || (dg == LMAX && ((uint32_t)Mv & b) != 0u)) V = kFull;
+        if (COUNT) ++w.n_vsets;
         U = __reduce_or_sync(kFull, V) & cm;
         if (U == 0u) return;
     }
-    uint4* sb = w.stage + (LEVEL - 1) * kTrieFan;
-    const int cnt = (int)(ce - cb);  // <= 27 by construction
-    __syncwarp();
-    if (w.lane <= cnt) sb[w.lane] = __ldg(reinterpret_cast<const uint4*>(P.trie[LEVEL]) + cb + w.lane);
-    __syncwarp();
+    const uint32_t sb = w.stage_addr + (LEVEL - 1) * kTrieFan * 16;
+    {
+        const uint32_t cnt = (uint32_t)__popc(cm);  // <= 27 by construction; node cb + cnt is the next node or the sentinel
+        __syncwarp();
+        const uint4 nd = __ldg(reinterpret_cast<const uint4*>(P.trie[LEVEL]) + (cb + min((uint32_t)w.lane, cnt)));
+        const uint32_t text_end = __shfl_down_sync(kFull, nd.x, 1);
+        if ((uint32_t)w.lane < cnt) sts128(sb + nd.z * 16, nd.x, text_end, nd.y, nd.w);  // code < kTrieFan
+        __syncwarp();
+    }
     do {
-        const uint32_t c = (uint32_t)__ffs((int)U) - 1u;
-        U &= U - 1u;
-        const int i = __popc(cm & ((1u << c) - 1u));
-        const uint4 nd = sb[i];      // text_begin, child_begin, code (= c), child codes
-        const uint4 nx = sb[i + 1];
+        const uint32_t c = top_bit(U);
+        U ^= 1u << c;
+        const uint4 nd = lds128(sb + c * 16);  // text_begin, text_end, child_begin, child_codes
         if (LEVEL <= kClipLevels) {  // clip the upper levels to this warp's texts
-            if (nx.x <= w.lo || nd.x >= w.hi) continue;
+            if (nd.y <= w.lo || nd.x >= w.hi) continue;
+        }
+        if constexpr (LEVEL >= 2 && LEVEL > LMAX) {
+            if (nd.y - nd.x <= kSmallSubtree) {  // a few texts: finish them from this column on
+                const uint32_t t0 = max(nd.x, w.lo), t1 = min(nd.y, w.hi);
+                if (t0 < t1) finish_texts<W, LMAX, COUNT, LEVEL - 1>(w, P, t0, t1, Pv, Mv, dg);
+                continue;
+            }
         }
         const W Eq = peq_load<W>(w.lane_addr, c);
         W P2 = Pv, M2 = Mv;
+        W D0;
         if (LEVEL == 1) {
-            first_column_step<W>(Eq, w.pv_init, w.x_init, P2, M2);
+            D0 = first_column_step<W>(Eq, w.pv_init, w.pv_init + w.pv_init, P2, M2);
             if (COUNT) ++w.n_first;
         } else {
-            column_step<W>(Eq, P2, M2);
+            D0 = column_step<W>(Eq, P2, M2);
         }
         if (COUNT) ++w.n_cols;
+        int dg2 = dg;
+        if (LEVEL > LMAX || LEVEL >= (int)w.dsh) {  // row LEVEL - delta >= 1 exists (warp-uniform)
+            if (((uint32_t)D0 & w.dbit(LEVEL)) == 0u) ++dg2;
+        }
         if constexpr (LEVEL < kTrieDepth) {
-            visit<W, COUNT, LEVEL + 1>(w, P, nd.y, nx.y, nd.w, P2, M2);
+            visit<W, LMAX, COUNT, LEVEL + 1>(w, P, nd.z, nd.w, P2, M2, dg2);
         } else {
-            const uint32_t t0 = max(nd.x, w.lo), t1 = min(nx.x, w.hi);
-            if (t0 < t1) finish_texts<W, COUNT>(w, P, t0, t1, P2, M2);
+            const uint32_t t0 = max(nd.x, w.lo), t1 = min(nd.y, w.hi);
+            if (t0 < t1) finish_texts<W, LMAX, COUNT, kTrieDepth>(w, P, t0, t1, P2, M2, dg2);
         }
     } while (U);
 }
 
-template <typename W, bool COUNT>
+template <typename W, int LMAX, bool COUNT>
 __global__ void __launch_bounds__(kTQ) k_distance_trie(const __grid_constant__ DistanceParams P) {
     extern __shared__ __align__(16) unsigned char smem[];
     constexpr int kRowBytes = peq_row_bytes<W>();
@@ -177,7 +225,7 @@ __global__ void __launch_bounds__(kTQ) k_distance_trie(const __grid_constant__ D
     if (R.diag && chunk_t0 + chunk_cnt <= p_tile0 + 1) return;  // wholly on/below the diagonal
 
     const int m = R.m, n = R.n;
-    const int delta = n - m;                  // 0 <= delta <= l_max
+    const int delta = n - m;                  // 0 <= delta <= l_max = LMAX
     const int p_rel = p_tile0 + tid;
     const bool p_valid = p_rel < R.p_count;
     build_peq<W>(peq, tid, p_valid, P.pat + (size_t)(R.p_start + p_rel) * P.pat_stride, m);
@@ -189,14 +237,12 @@ __global__ void __launch_bounds__(kTQ) k_distance_trie(const __grid_constant__ D
     if (lo_rel >= hi_rel || warp_p0 >= R.p_count) return;  // warp-uniform; no CTA barrier follows
 
     Walk<W, COUNT> w;
-    w.stage = stage_all + warp * (kTrieDepth * kTrieFan);
-    w.rows = P.txt + R.txt_base;
+    w.stage_addr = (uint32_t)__cvta_generic_to_shared(stage_all) + warp * (kTrieDepth * kTrieFan * 16);
+    w.rows = P.txt + R.txt_base - (size_t)R.t_start * R.row_words;
     w.lane_addr = (uint32_t)__cvta_generic_to_shared(smem) + tid * (uint32_t)sizeof(W);
-    w.t_start = (uint32_t)R.t_start;
     w.lo = (uint32_t)(R.t_start + lo_rel);
     w.hi = (uint32_t)(R.t_start + hi_rel);
-#pragma unroll
-    for (int k = 0; k <= kTrieDepth; ++k) w.mask2[k] = k > delta ? ((1u << (k - delta)) - 1u) * 0x10001u : 0u;
+    w.dsh = (uint32_t)delta + 1u;
     {
         // one-hot codes of the pattern's first rows, shifted by delta: ohs[q] belongs to row q - delta
         const uint8_t* prow = P.pat + (size_t)(R.p_start + p_rel) * P.pat_stride;
@@ -210,17 +256,11 @@ __global__ void __launch_bounds__(kTQ) k_distance_trie(const __grid_constant__ D
         }
     }
     w.pv_init = low_mask<W>(m);
-    w.x_init = w.pv_init + w.pv_init;
-    w.m_mask = w.pv_init;
     w.rw = R.row_words;
     w.n = n;
-    w.delta = delta;
-    w.thr = p_valid ? P.l_max - delta : -1;
-    w.l_max_lane = p_valid ? P.l_max : -1;
-    w.l_max = P.l_max;
     w.lane = lane;
     w.p_sorted = R.p_start + p_rel;
-    w.diag = R.diag;
+    w.p_lim = R.diag ? w.p_sorted : -1;
 
     // codes of the bucket's level-1 nodes
     uint32_t root_codes = 0u;
@@ -229,7 +269,8 @@ __global__ void __launch_bounds__(kTQ) k_distance_trie(const __grid_constant__ D
         if (lane < cnt) root_codes = 1u << (P.trie[1][R.root_begin + lane].code & 31u);
         root_codes = __reduce_or_sync(kFull, root_codes);
     }
-    visit<W, COUNT, 1>(w, P, R.root_begin, R.root_end, root_codes, w.pv_init, W(0));
+    // D[0][delta] = delta is the first cell of the final diagonal
+    visit<W, LMAX, COUNT, 1>(w, P, R.root_begin, root_codes, w.pv_init, W(0), p_valid ? delta : kDeadLane);
 
     if (COUNT) {
         // warp-level counters (identical in all lanes): lane 0 reports 32 lanes' worth
@@ -237,18 +278,36 @@ __global__ void __launch_bounds__(kTQ) k_distance_trie(const __grid_constant__ D
             atomicAdd(P.work + 0, w.n_cols * 32ull);
             atomicAdd(P.work + 1, w.n_tests * 32ull);
             atomicAdd(P.work + 2, w.n_first * 32ull);
-            atomicAdd(P.work + 3, w.n_ptests * 32ull);
+            atomicAdd(P.work + 3, w.n_vsets * 32ull);
         }
     }
 }
 
-template <typename W, bool COUNT>
+template <typename W, int LMAX, bool COUNT>
 cudaError_t launch_one(const DistanceParams& p, int64_t n_items, size_t smem, cudaStream_t s) {
-    auto kern = k_distance_trie<W, COUNT>;
+    auto kern = k_distance_trie<W, LMAX, COUNT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kern<<<(unsigned)((n_items - p.shard + p.n_shards - 1) / p.n_shards), kTQ, smem, s>>>(p);
     return cudaGetLastError();
+}
+
+template <typename W, int LMAX>
+cudaError_t launch_lmax(const DistanceParams& p, int64_t n_items, bool count_work, size_t smem, cudaStream_t s) {
+    return count_work ? launch_one<W, LMAX, true>(p, n_items, smem, s) : launch_one<W, LMAX, false>(p, n_items, smem, s);
+}
+
+template <typename W>
+cudaError_t launch_word(const DistanceParams& p, int64_t n_items, bool count_work, size_t smem, cudaStream_t s) {
+    static_assert(kTrieMaxL == 4, "one case per specialised l_max");
+    switch (p.l_max) {
+        case 0: return launch_lmax<W, 0>(p, n_items, count_work, smem, s);
+        case 1: return launch_lmax<W, 1>(p, n_items, count_work, smem, s);
+        case 2: return launch_lmax<W, 2>(p, n_items, count_work, smem, s);
+        case 3: return launch_lmax<W, 3>(p, n_items, count_work, smem, s);
+        case 4: return launch_lmax<W, 4>(p, n_items, count_work, smem, s);
+        default: return cudaErrorInvalidValue;
+    }
 }
 
 }  // namespace
@@ -264,11 +323,8 @@ cudaError_t launch_distance_trie(const DistanceParams& p, int64_t n_items, bool 
     if (n_items > 0x7fffffffLL) return cudaErrorInvalidValue;
     const size_t smem = distance_trie_smem_bytes(wide);
     *launches += 1;
-    if (wide)
-        return count_work ? launch_one<uint64_t, true>(p, n_items, smem, s)
-                          : launch_one<uint64_t, false>(p, n_items, smem, s);
-    return count_work ? launch_one<uint32_t, true>(p, n_items, smem, s)
-                      : launch_one<uint32_t, false>(p, n_items, smem, s);
+    return wide ? launch_word<uint64_t>(p, n_items, count_work, smem, s)
+                : launch_word<uint32_t>(p, n_items, count_work, smem, s);
 }
 
 }  // namespace tcrnet

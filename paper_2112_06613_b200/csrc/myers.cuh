@@ -59,8 +59,10 @@ __device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c) {
     return r;
 }
 
+// Every step returns D0 (bit i set iff D[i+1][j] = D[i][j-1]: the diagonal did not increase), which the
+// trie kernel uses to track the final-diagonal cell without popcounts.
 template <typename W>
-__device__ __forceinline__ void column_step(W Eq, W& Pv, W& Mv) {
+__device__ __forceinline__ W column_step(W Eq, W& Pv, W& Mv) {
     const W s = (Eq & Pv) + Pv;
     const W D0 = ((s ^ Pv) | Mv) | Eq;
     const W nHp = ~Mv & (D0 | Pv);  // ~Hp
@@ -69,10 +71,11 @@ __device__ __forceinline__ void column_step(W Eq, W& Pv, W& Mv) {
     const W Hn2 = Hn + Hn;          // Hn << 1
     Pv = Hn2 | (~D0 & X);
     Mv = D0 & ~X;
+    return D0;
 }
 
 template <>
-__device__ __forceinline__ void column_step<uint32_t>(uint32_t Eq, uint32_t& Pv, uint32_t& Mv) {
+__device__ __forceinline__ uint32_t column_step<uint32_t>(uint32_t Eq, uint32_t& Pv, uint32_t& Mv) {
     const uint32_t t = lop3<0xC0>(Eq, Pv, 0u);        // Eq & Pv
     const uint32_t s = t + Pv;
     const uint32_t D0a = lop3<0xBE>(s, Pv, Mv);       // (s ^ Pv) | Mv
@@ -83,27 +86,30 @@ __device__ __forceinline__ void column_step<uint32_t>(uint32_t Eq, uint32_t& Pv,
     const uint32_t Hn2 = Hn + Hn;                     // Hn << 1
     Pv = lop3<0xF2>(Hn2, D0, X);                      // Hn2 | (~D0 & X)
     Mv = lop3<0x30>(D0, X, 0u);                       // D0 & ~X
+    return D0;
 }
 
 // Column 0 starts from Pv = low(m), Mv = 0.  Bits at and above m are don't-cares (they never flow
 // down and are masked at every popcount), so ~Hp = D0 | Pv may be replaced by the constant Pv, and
 // Hn = Pv & D0 by D0:  X = Pv0 + Pv0 is a constant and the step needs 3 LOP3 + 2 adds.
 template <typename W>
-__device__ __forceinline__ void first_column_step(W Eq, W Pv0, W X0, W& Pv, W& Mv) {
+__device__ __forceinline__ W first_column_step(W Eq, W Pv0, W X0, W& Pv, W& Mv) {
     const W s = Eq + Pv0;            // Eq & Pv0 = Eq: Peq has no bits at or above m
     const W D0 = ((s ^ Pv0) | Eq);
     const W Hn2 = D0 + D0;
     Pv = Hn2 | (~D0 & X0);
     Mv = D0 & ~X0;
+    return D0;
 }
 template <>
-__device__ __forceinline__ void first_column_step<uint32_t>(uint32_t Eq, uint32_t Pv0, uint32_t X0, uint32_t& Pv,
-                                                             uint32_t& Mv) {
+__device__ __forceinline__ uint32_t first_column_step<uint32_t>(uint32_t Eq, uint32_t Pv0, uint32_t X0, uint32_t& Pv,
+                                                                 uint32_t& Mv) {
     const uint32_t s = Eq + Pv0;
     const uint32_t D0 = lop3<0xBE>(s, Pv0, Eq);       // (s ^ Pv0) | Eq
     const uint32_t Hn2 = D0 + D0;
     Pv = lop3<0xF2>(Hn2, D0, X0);                     // Hn2 | (~D0 & X0)
     Mv = lop3<0x30>(D0, X0, 0u);                      // D0 & ~X0
+    return D0;
 }
 
 // Shared-memory accesses by 32-bit shared address (no generic-pointer arithmetic in the hot loop).

@@ -223,9 +223,9 @@ struct Schedule {
 void schedule_pass(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule::Pass& pass, tcrnet_stats& st) {
     const SeqSet& ps = *pass.pset;
     const SeqSet& ts = *pass.tset;
-    // The trie kernel serves the rows whose early exit can act inside the trie: first test level
-    // <= kTrieDepth and at least one text column beyond the trie.
-    const bool use_trie = ctx->prefix_trie && first_check >= 3 && first_check <= kTrieDepth;
+    // The trie kernel serves the rows whose early exit can act inside the trie (l_max <= kTrieMaxL, the
+    // values it is specialised on) and that have at least one text column beyond the trie.
+    const bool use_trie = ctx->prefix_trie && first_check > 0 && l_max <= kTrieMaxL;
     for (int m = 1; m < kNumLen; ++m) {
         if (!ps.hist[m]) continue;
         const int n0 = pass.mode == kPairsAllQuery ? m + 1 : m;

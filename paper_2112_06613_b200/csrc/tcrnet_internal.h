@@ -18,7 +18,8 @@ constexpr int kTQ = 256;                 // patterns per CTA of the distance ker
 constexpr int kTT = 64;                  // texts staged into shared memory per pipeline stage
 constexpr int kSortPrefix = 6;           // residues of the lexicographic sub-order inside a length bucket
 constexpr int kTrieDepth = kSortPrefix;  // levels 1..kTrieDepth of the prefix trie over each text bucket
-constexpr int kTrieFan = 32;             // staging slots per trie level (a node has <= 27 children + sentinel)
+constexpr int kTrieFan = 32;             // staging slots per trie level, indexed by residue code (0..26)
+constexpr int kTrieMaxL = 4;             // the trie kernel is specialised on l_max = 0..kTrieMaxL
 
 // Per-length layout of the packed sequence tables (filled on the host after the histogram).
 struct LengthTable {
@@ -86,8 +87,8 @@ struct DistanceParams {
     unsigned long long* edges;       // keys (min(i,j) << 32) | max(i,j)
     unsigned long long* edge_count;  // device counter (keeps counting beyond capacity)
     unsigned long long edge_cap;
-    unsigned long long* work;        // [4]: lane-columns, lane-tests (4 ALU ops), lane-first-columns,
-                                     //      lane-prefix-tests (3 ALU ops); COUNT only
+    unsigned long long* work;        // [4]: lane-columns, lane-tests (exit votes), lane-first-columns,
+                                     //      lane-V-sets (guided expansions); COUNT only
     const TrieNode* trie[kTrieDepth + 1];  // trie kernel: nodes of level 1..kTrieDepth ([0] unused)
 };
 

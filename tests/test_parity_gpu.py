@@ -106,8 +106,8 @@ def test_prefix_trie_does_not_change_the_result(pkg, oracle):
 
 def test_prefix_trie_shared_prefixes_and_short_buckets(pkg, oracle):
     """Real CDR3-beta rows mostly start CASS...: few distinct prefixes, deep shared runs, many
-    duplicates; plus buckets shorter than the trie depth (they take the text-chunk kernel) and a
-    forced first test level with l_max larger than the trie can prune."""
+    duplicates; plus buckets shorter than the trie depth (they take the text-chunk kernel), every
+    l_max the trie kernel is specialised on (0..4), and an l_max beyond them (text-chunk kernel only)."""
     rng = np.random.default_rng(23)
     letters = "ACDEFGHIKLMNPQRSTVWY"
     strings = []
@@ -129,10 +129,11 @@ def test_prefix_trie_shared_prefixes_and_short_buckets(pkg, oracle):
             strings.append("".join(t))
     order = rng.permutation(len(strings))
     res, ln = from_strings([strings[i] for i in order])
-    for l_max, opts in ((0, {}), (1, {}), (2, {}), (3, {pkg.OPT_TRIE_CHUNK: 256}), (6, {pkg.OPT_FIRST_CHECK: 3})):
+    for l_max, opts in ((0, {}), (1, {}), (2, {}), (3, {pkg.OPT_TRIE_CHUNK: 256}), (4, {}), (4, {pkg.OPT_TRIE_CHUNK: 512}),
+                        (6, {pkg.OPT_FIRST_CHECK: 3})):
         want = oracle.network(res, ln, l_max, tier=0)[:3]
         got, st = gpu_network(pkg, res, ln, l_max, opts)
-        assert st["work_items_trie"] > 0
+        assert (st["work_items_trie"] > 0) == (l_max <= 4)
         assert_same_network(got, want)
 
 
