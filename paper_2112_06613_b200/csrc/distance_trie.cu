@@ -52,11 +52,6 @@ namespace {
 constexpr uint32_t kFull = 0xffffffffu;
 constexpr int kClipLevels = 3;      // levels whose nodes are clipped to the work item's text chunk
 constexpr int kDeadLane = 1 << 20;  // dg of a lane without a pattern: never alive, never emitted
-#ifndef TCRNET_SMALL_SUBTREE
-#define TCRNET_SMALL_SUBTREE 0
-#endif
-// subtrees of <= this many texts leave the trie and are finished text by text (0: never)
-constexpr uint32_t kSmallSubtree = TCRNET_SMALL_SUBTREE;
 
 template <typename W, bool COUNT>
 struct Walk {
@@ -89,14 +84,15 @@ __device__ __forceinline__ uint32_t top_bit(uint32_t x) {  // index of the highe
     return r;
 }
 
-// The texts [t0, t1) of a surviving subtree, one by one: the text columns START .. n-1 (0-based) on top
-// of the state (Pv0, Mv0, dg0) after START columns, with the tracked final-diagonal cell; emission.
-// START = kTrieDepth below a deepest-level node; START = LEVEL - 1 for the small subtrees that leave the
-// trie early (visit()).  START >= l_max >= delta, so every column has its final-diagonal row.
-template <typename W, int LMAX, bool COUNT, int START>
+// The texts [t0, t1) below a surviving deepest-level node, one by one: the text columns kTrieDepth .. n-1
+// (0-based) on top of the node's state (Pv0, Mv0, dg0) with the tracked final-diagonal cell; emission.
+// (Leaving the trie earlier for subtrees of one or two texts was measured and is slower: the walk's exact
+// V sets prune more than the votes of this loop.)
+template <typename W, int LMAX, bool COUNT>
 __device__ __forceinline__ void finish_texts(Walk<W, COUNT>& w, const DistanceParams& P, uint32_t t0, uint32_t t1,
                                              const W Pv0, const W Mv0, const int dg0) {
-    static_assert(START >= 1 && START >= LMAX, "column 0 has its own step; final-diagonal rows exist from column delta on");
+    constexpr int START = kTrieDepth;
+    static_assert(START >= 1 && START >= kTrieMaxL, "column 0 has its own step; final-diagonal rows exist from column delta on");
     constexpr int kJ0 = START & ~3;  // the 128-bit load that holds column START
     // exit vote after every column, or after every second one for l_max <= 1 (measured: cfg4 / cfg5)
     constexpr int kVoteEvery = LMAX >= 2 ? 1 : 2;
@@ -164,7 +160,9 @@ __device__ __forceinline__ void visit(Walk<W, COUNT>& w, const DistanceParams& P
         __syncwarp();
         const uint4 nd = __ldg(reinterpret_cast<const uint4*>(P.trie[LEVEL]) + (cb + min((uint32_t)w.lane, cnt)));
         const uint32_t text_end = __shfl_down_sync(kFull, nd.x, 1);
-        if ((uint32_t)w.lane < cnt) sts128(sb + nd.z * 16, nd.x, text_end, nd.y, nd.w);  // code < kTrieFan
+        if ((uint32_t)w.lane < cnt) {
+            sts128(sb + nd.z * 16, nd.x, text_end, nd.y, nd.w);  // code < kTrieFan
+        }
         __syncwarp();
     }
     do {
@@ -173,13 +171,6 @@ __device__ __forceinline__ void visit(Walk<W, COUNT>& w, const DistanceParams& P
         const uint4 nd = lds128(sb + c * 16);  // text_begin, text_end, child_begin, child_codes
         if (LEVEL <= kClipLevels) {  // clip the upper levels to this warp's texts
             if (nd.y <= w.lo || nd.x >= w.hi) continue;
-        }
-        if constexpr (LEVEL >= 2 && LEVEL > LMAX) {
-            if (nd.y - nd.x <= kSmallSubtree) {  // a few texts: finish them from this column on
-                const uint32_t t0 = max(nd.x, w.lo), t1 = min(nd.y, w.hi);
-                if (t0 < t1) finish_texts<W, LMAX, COUNT, LEVEL - 1>(w, P, t0, t1, Pv, Mv, dg);
-                continue;
-            }
         }
         const W Eq = peq_load<W>(w.lane_addr, c);
         W P2 = Pv, M2 = Mv;
@@ -199,13 +190,13 @@ __device__ __forceinline__ void visit(Walk<W, COUNT>& w, const DistanceParams& P
             visit<W, LMAX, COUNT, LEVEL + 1>(w, P, nd.z, nd.w, P2, M2, dg2);
         } else {
             const uint32_t t0 = max(nd.x, w.lo), t1 = min(nd.y, w.hi);
-            if (t0 < t1) finish_texts<W, LMAX, COUNT, kTrieDepth>(w, P, t0, t1, P2, M2, dg2);
+            if (t0 < t1) finish_texts<W, LMAX, COUNT>(w, P, t0, t1, P2, M2, dg2);
         }
     } while (U);
 }
 
 template <typename W, int LMAX, bool COUNT>
-__global__ void __launch_bounds__(kTQ) k_distance_trie(const __grid_constant__ DistanceParams P) {
+__global__ void __launch_bounds__(kTQ, sizeof(W) == 4 ? 4 : 2) k_distance_trie(const __grid_constant__ DistanceParams P) {
     extern __shared__ __align__(16) unsigned char smem[];
     constexpr int kRowBytes = peq_row_bytes<W>();
     static_assert((kPeqRows * kRowBytes) % 16 == 0, "the staging buffers follow the Peq table");

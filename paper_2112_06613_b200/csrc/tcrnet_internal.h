@@ -18,7 +18,7 @@ constexpr int kTQ = 256;                 // patterns per CTA of the distance ker
 constexpr int kTT = 64;                  // texts staged into shared memory per pipeline stage
 constexpr int kSortPrefix = 6;           // residues of the lexicographic sub-order inside a length bucket
 constexpr int kTrieDepth = kSortPrefix;  // levels 1..kTrieDepth of the prefix trie over each text bucket
-constexpr int kTrieFan = 32;             // staging slots per trie level, indexed by residue code (0..26)
+constexpr int kTrieFan = 27;             // staging slots per trie level, indexed by residue code (0..26)
 constexpr int kTrieMaxL = 4;             // the trie kernel is specialised on l_max = 0..kTrieMaxL
 
 // Per-length layout of the packed sequence tables (filled on the host after the histogram).
