@@ -35,6 +35,34 @@ __global__ void __launch_bounds__(256) k_length_hist(const int32_t* __restrict__
         if (h[i]) atomicAdd(&hist[i], (unsigned long long)h[i]);
 }
 
+// Sort key of the sequence sort: (clamped length, first kSortPrefix residues as 5-bit digits, 0 = past the
+// end, 27 = not a letter); the payload of row i is i.  Invalid lengths / residues are reported by
+// k_length_hist / k_pack, here they only have to land somewhere.
+__global__ void __launch_bounds__(256) k_seq_keys(const uint8_t* __restrict__ residues,
+                                                 const int64_t* __restrict__ offsets,
+                                                 const int32_t* __restrict__ lengths, int64_t n,
+                                                 unsigned long long* __restrict__ keys, int32_t* __restrict__ vals) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int32_t l = lengths[i];
+    if (l < 1 || l > kMaxLen) l = 0;
+    const uint8_t* src = residues + offsets[i];
+    unsigned long long key = (unsigned long long)(uint32_t)l;
+#pragma unroll
+    for (int k = 0; k < kSortPrefix; ++k) {
+        uint32_t d = 0u;
+        if (k < l) {
+            const uint32_t c = (uint32_t)src[k] - (uint32_t)'A';
+            d = (c < 26u ? c : 26u) + 1u;
+        }
+        key = (key << 5) | d;
+    }
+    keys[i] = key;
+    vals[i] = (int32_t)i;
+}
+
+// One thread per sorted position: the pattern row is written with 128-bit stores (pat_stride is a
+// multiple of 16), the text row with one 128-bit store per four columns.
 __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residues,
                                              const int64_t* __restrict__ offsets,
                                              const int32_t* __restrict__ lengths,
@@ -48,20 +76,37 @@ __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residu
         const int32_t o = perm[s];
         const int32_t len = lengths[o];
         const uint8_t* src = residues + offsets[o];
-        uint8_t* prow = pat + (size_t)s * pat_stride;
-        uint32_t* trow = txt + lt.txt_base[len] + (int64_t)(s - lt.start[len]) * lt.row_words[len];
+        uint4* prow = reinterpret_cast<uint4*>(pat + (size_t)s * pat_stride);
         const int rw = lt.row_words[len];
-        for (int i = 0; i < pat_stride; ++i) {
-            uint32_t c = 0xffu;
-            if (i < len) {
-                c = (uint32_t)src[i] - (uint32_t)'A';
-                if (c >= (uint32_t)kNumCodes) {
-                    bad = true;
-                    c = 0;
+        uint4* trow = reinterpret_cast<uint4*>(txt + lt.txt_base[len] + (int64_t)(s - lt.start[len]) * rw);
+        for (int i0 = 0; i0 < pat_stride; i0 += 16) {
+            uint32_t c[16];
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+                const int i = i0 + k;
+                c[k] = 0xffu;
+                if (i < len) {
+                    c[k] = (uint32_t)src[i] - (uint32_t)'A';
+                    if (c[k] >= (uint32_t)kNumCodes) {
+                        bad = true;
+                        c[k] = 0;
+                    }
                 }
             }
-            prow[i] = (uint8_t)c;
-            if (i < rw) trow[i] = i < len ? c : (uint32_t)kPadCode;
+            uint32_t w4[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) w4[k] = c[4 * k] | (c[4 * k + 1] << 8) | (c[4 * k + 2] << 16) | (c[4 * k + 3] << 24);
+            prow[i0 >> 4] = make_uint4(w4[0], w4[1], w4[2], w4[3]);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int i = i0 + 4 * k;  // text columns i .. i+3
+                if (i < rw) {
+                    uint32_t t[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) t[q] = i + q < len ? c[4 * k + q] : (uint32_t)kPadCode;
+                    trow[i >> 2] = make_uint4(t[0], t[1], t[2], t[3]);
+                }
+            }
         }
     }
     if (__syncthreads_or(bad) && threadIdx.x == 0) atomicOr(flags, kFlagBadResidue);
@@ -74,6 +119,14 @@ cudaError_t launch_length_hist(const int32_t* lengths, int64_t n, unsigned long 
     int64_t blocks = (n + 255) / 256;
     if (blocks > 148 * 8) blocks = 148 * 8;
     k_length_hist<<<(unsigned)blocks, 256, 0, s>>>(lengths, n, hist, flags);
+    *launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_seq_keys(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths, int64_t n,
+                            unsigned long long* keys, int32_t* vals, cudaStream_t s, int* launches) {
+    if (n <= 0) return cudaSuccess;
+    k_seq_keys<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(residues, offsets, lengths, n, keys, vals);
     *launches += 1;
     return cudaGetLastError();
 }

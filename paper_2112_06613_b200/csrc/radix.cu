@@ -1,0 +1,173 @@
+// Stable LSD radix sort over 8-bit digits of 64-bit keys, with an optional 32-bit payload: the sequence
+// sort of step A1 (composite (length, first residues) keys, payload = caller's row) and the edge-key sort
+// of step A6.  HBM/L2-bound streaming; three launches per pass, no spinning on other CTAs:
+//
+//   k_radix_hist     per tile of 4096 keys, the 256 digit counts (shared-memory atomics), stored digit-major
+//                    (hist[d * tiles + tile]) and added to the pass's global digit totals;
+//   k_radix_scan     CTA d turns row d of `hist` into global output positions: the total of all smaller
+//                    digits (from the global totals) + the exclusive prefix over the tiles;
+//   k_radix_scatter  each warp owns 512 consecutive keys of its tile and ranks equal digits in order
+//                    (__match_any_sync + a warp-private running count in shared memory, no CTA barrier
+//                    inside the loop), the 8 warp counts are chained once, keys go straight to their
+//                    final slot.  Order inside a digit = input order, so every pass is stable.
+#include <utility>
+
+#include "tcrnet_internal.h"
+
+namespace tcrnet {
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kWarps = kThreads / 32;
+constexpr int kRounds = 16;                      // keys per thread
+constexpr int kTile = kThreads * kRounds;        // 4096 keys per CTA
+constexpr int kWarpItems = 32 * kRounds;         // 512 consecutive keys per warp
+constexpr uint32_t kFull = 0xffffffffu;
+
+__global__ void __launch_bounds__(kThreads) k_radix_hist(const unsigned long long* __restrict__ keys, int64_t n,
+                                                        int shift, uint32_t* __restrict__ hist,
+                                                        uint32_t* __restrict__ totals, uint32_t tiles) {
+    __shared__ uint32_t h[256];
+    h[threadIdx.x] = 0;
+    __syncthreads();
+    const int64_t base = (int64_t)blockIdx.x * kTile;
+#pragma unroll 4
+    for (int r = 0; r < kRounds; ++r) {
+        const int64_t i = base + (int64_t)r * kThreads + threadIdx.x;
+        if (i < n) atomicAdd(&h[(uint32_t)(keys[i] >> shift) & 255u], 1u);
+    }
+    __syncthreads();
+    const uint32_t c = h[threadIdx.x];
+    hist[(size_t)threadIdx.x * tiles + blockIdx.x] = c;
+    if (c) atomicAdd(&totals[threadIdx.x], c);
+}
+
+// Row d of hist (tiles entries) -> first output slot of (digit d, tile t), in place.
+__global__ void __launch_bounds__(kThreads) k_radix_scan(uint32_t* __restrict__ hist,
+                                                        const uint32_t* __restrict__ totals, uint32_t tiles) {
+    __shared__ uint32_t wsum[kWarps];
+    const uint32_t d = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // total of the smaller digits
+    uint32_t below = tid < d ? totals[tid] : 0u;
+    below = __reduce_add_sync(kFull, below);
+    if (lane == 0) wsum[warp] = below;
+    __syncthreads();
+    uint32_t digit_base = 0;
+#pragma unroll
+    for (int w = 0; w < kWarps; ++w) digit_base += wsum[w];
+    __syncthreads();
+    // each thread owns a contiguous chunk of the row
+    uint32_t* row = hist + (size_t)d * tiles;
+    const uint32_t per = (tiles + kThreads - 1) / kThreads;
+    const uint32_t b = min(tid * per, tiles), e = min(b + per, tiles);
+    uint32_t sum = 0;
+    for (uint32_t t = b; t < e; ++t) sum += row[t];
+    // exclusive scan of the 256 partial sums (warp scan + warp totals)
+    uint32_t incl = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(kFull, incl, o);
+        if ((int)lane >= o) incl += v;
+    }
+    if (lane == 31) wsum[warp] = incl;
+    __syncthreads();
+    uint32_t run = digit_base + incl - sum;
+    for (uint32_t w = 0; w < warp; ++w) run += wsum[w];
+    for (uint32_t t = b; t < e; ++t) {
+        const uint32_t c = row[t];
+        row[t] = run;
+        run += c;
+    }
+}
+
+template <bool HAS_VAL>
+__global__ void __launch_bounds__(kThreads) k_radix_scatter(const unsigned long long* __restrict__ keys_in,
+                                                           unsigned long long* __restrict__ keys_out,
+                                                           const int32_t* __restrict__ vals_in,
+                                                           int32_t* __restrict__ vals_out, int64_t n, int shift,
+                                                           const uint32_t* __restrict__ scanned, uint32_t tiles) {
+    __shared__ uint32_t wh[kWarps][256];  // per warp: running digit counts, then first output slots
+    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+#pragma unroll
+    for (int w = 0; w < kWarps; ++w) wh[w][tid] = 0;
+    __syncthreads();
+    const int64_t first = (int64_t)blockIdx.x * kTile + (int64_t)warp * kWarpItems + lane;
+    const uint32_t lt = (1u << lane) - 1u;
+    unsigned long long key[kRounds];
+    uint32_t rank[kRounds];  // rank among the warp's keys of the same digit | digit << 16 (0xffffffff: no key)
+#pragma unroll
+    for (int r = 0; r < kRounds; ++r) {
+        const int64_t i = first + r * 32;
+        const bool valid = i < n;
+        key[r] = valid ? keys_in[i] : 0ull;
+        const uint32_t d = valid ? (uint32_t)(key[r] >> shift) & 255u : 256u + lane;  // invalid lanes match nobody
+        const uint32_t peers = __match_any_sync(kFull, d);
+        const int leader = __ffs((int)peers) - 1;
+        uint32_t old = 0;
+        if (valid && (int)lane == leader) {
+            old = wh[warp][d];
+            wh[warp][d] = old + __popc(peers);
+        }
+        old = __shfl_sync(kFull, old, leader);
+        rank[r] = valid ? (old + __popc(peers & lt)) | (d << 16) : 0xffffffffu;
+        __syncwarp();
+    }
+    __syncthreads();
+    {
+        uint32_t run = scanned[(size_t)tid * tiles + blockIdx.x];
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) {
+            const uint32_t c = wh[w][tid];
+            wh[w][tid] = run;
+            run += c;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < kRounds; ++r) {
+        if (rank[r] != 0xffffffffu) {
+            const uint32_t pos = wh[warp][rank[r] >> 16] + (rank[r] & 0xffffu);
+            keys_out[pos] = key[r];
+            if (HAS_VAL) vals_out[pos] = vals_in[first + r * 32];
+        }
+    }
+}
+
+}  // namespace
+
+int64_t radix_tiles(int64_t n) { return n > 0 ? (n + kTile - 1) / kTile : 1; }
+
+size_t radix_scratch_bytes(int64_t n) {
+    return ((size_t)radix_tiles(n) * 256 + (size_t)kRadixMaxPasses * 256) * sizeof(uint32_t);
+}
+
+cudaError_t radix_sort_u64(unsigned long long* keys_a, unsigned long long* keys_b, int32_t* vals_a, int32_t* vals_b,
+                           int64_t n, const int* shifts, int n_passes, void* scratch, cudaStream_t s, int* launches,
+                           bool* result_in_b) {
+    *result_in_b = false;
+    if (n <= 1 || n_passes <= 0) return cudaSuccess;
+    if (n_passes > kRadixMaxPasses || n > 0x7fffffffLL) return cudaErrorInvalidValue;
+    const uint32_t tiles = (uint32_t)radix_tiles(n);
+    uint32_t* totals = (uint32_t*)scratch;                 // [kRadixMaxPasses][256]
+    uint32_t* hist = totals + kRadixMaxPasses * 256;       // [256][tiles]
+    cudaError_t e = cudaMemsetAsync(totals, 0, sizeof(uint32_t) * kRadixMaxPasses * 256, s);
+    if (e != cudaSuccess) return e;
+    const bool has_val = vals_a != nullptr;
+    for (int p = 0; p < n_passes; ++p) {
+        k_radix_hist<<<tiles, kThreads, 0, s>>>(keys_a, n, shifts[p], hist, totals + p * 256, tiles);
+        k_radix_scan<<<256, kThreads, 0, s>>>(hist, totals + p * 256, tiles);
+        if (has_val)
+            k_radix_scatter<true><<<tiles, kThreads, 0, s>>>(keys_a, keys_b, vals_a, vals_b, n, shifts[p], hist, tiles);
+        else
+            k_radix_scatter<false><<<tiles, kThreads, 0, s>>>(keys_a, keys_b, nullptr, nullptr, n, shifts[p], hist, tiles);
+        *launches += 3;
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        std::swap(keys_a, keys_b);
+        std::swap(vals_a, vals_b);
+        *result_in_b = !*result_in_b;
+    }
+    return cudaSuccess;
+}
+
+}  // namespace tcrnet

@@ -105,42 +105,40 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
     lt.txt_base[kNumLen] = words;
     set.pat_stride = (max_len + 15) & ~15;
 
-    // offsets, stable sort by (length, row), re-layout
+    // offsets, stable sort by (length, first residues, row), re-layout
     DevBuf& offsets = ctx->offsets;
-    const int64_t blocks = split_num_blocks(n);
     int rc = dev_reserve(ctx, offsets, sizeof(int64_t) * (size_t)(n + 1));
-    if (rc == TCRNET_OK) rc = dev_reserve(ctx, ctx->scan_scratch, std::max(scan_scratch_bytes(n), scan_scratch_bytes(256 * blocks)));
-    if (rc == TCRNET_OK) rc = dev_reserve(ctx, ctx->split_hist, sizeof(uint32_t) * 256 * (size_t)blocks);
-    if (rc == TCRNET_OK) rc = dev_reserve(ctx, ctx->split_hist_scanned, sizeof(uint32_t) * 256 * (size_t)blocks);
+    if (rc == TCRNET_OK) rc = dev_reserve(ctx, ctx->scan_scratch, scan_scratch_bytes(n));
+    if (rc == TCRNET_OK) rc = dev_reserve(ctx, ctx->radix_scratch, radix_scratch_bytes(n));
+    if (rc == TCRNET_OK) rc = dev_reserve(ctx, ctx->keys_a, sizeof(unsigned long long) * (size_t)n);
+    if (rc == TCRNET_OK) rc = dev_reserve(ctx, ctx->keys_b, sizeof(unsigned long long) * (size_t)n);
+    if (rc == TCRNET_OK) rc = dev_reserve(ctx, ctx->perm_tmp, sizeof(int32_t) * (size_t)n);
     if (rc == TCRNET_OK) rc = dev_reserve(ctx, set.perm, sizeof(int32_t) * (size_t)n);
     if (rc == TCRNET_OK) rc = dev_reserve(ctx, set.pat, (size_t)n * set.pat_stride);
     if (rc == TCRNET_OK) rc = dev_reserve(ctx, set.txt, sizeof(uint32_t) * (size_t)(words + 4));
     if (rc != TCRNET_OK) return rc;
-    // Sort key: (length, first kSortPrefix residues, row).  LSD: least significant digit first, every
-    // pass stable.  The sub-order inside a length bucket is free (results are mapped back through
-    // perm); the lexicographic one makes the 32 patterns of a warp share their first residues, so the
-    // early-exit test of the distance kernel fails or holds for the whole warp at once.
-    DevBuf& perm_tmp = ctx->perm_tmp;
-    rc = dev_reserve(ctx, perm_tmp, sizeof(int32_t) * (size_t)n);
-    if (rc != TCRNET_OK) return rc;
+    // Sort key: (length, first kSortPrefix residues, row): one composite 64-bit key per row, stable LSD
+    // radix sort with the row as payload.  The sub-order inside a length bucket is free (results are mapped
+    // back through perm); the lexicographic one makes the 32 patterns of a warp share their first residues
+    // and puts the texts of a bucket in trie order.
     cudaError_t e = exclusive_scan_i32_to_i64(d_len, (int64_t*)offsets.p, n, true, ctx->scan_scratch.p, s, launches);
     {
-        // kSortPrefix + 1 passes ping-pong between the two buffers; arrange for the last to land in ctx->perm
-        int32_t* bufs[2] = {(int32_t*)set.perm.p, (int32_t*)perm_tmp.p};
-        int cur = kSortPrefix & 1;  // buffer written by the first pass
-        const int32_t* in = nullptr;
-        for (int k = kSortPrefix - 1; k >= 0 && e == cudaSuccess; --k) {
-            e = split_by_residue(d_res, (const int64_t*)offsets.p, d_len, in, k, n, bufs[cur],
-                                 (uint32_t*)ctx->split_hist.p, (uint32_t*)ctx->split_hist_scanned.p,
-                                 ctx->scan_scratch.p, s, launches);
-            in = bufs[cur];
-            cur ^= 1;
-        }
+        constexpr int kPasses = (kSeqKeyBits + 7) / 8;
+        int shifts[kPasses];
+        for (int p = 0; p < kPasses; ++p) shifts[p] = 8 * p;
+        // an odd number of passes ends in the b buffers: make those set.perm
+        int32_t* va = (int32_t*)(kPasses & 1 ? ctx->perm_tmp.p : set.perm.p);
+        int32_t* vb = (int32_t*)(kPasses & 1 ? set.perm.p : ctx->perm_tmp.p);
         if (e == cudaSuccess)
-            e = split_by_length(d_len, in, n, bufs[cur], (uint32_t*)ctx->split_hist.p,
-                                (uint32_t*)ctx->split_hist_scanned.p, ctx->scan_scratch.p, s, launches);
-        // cur is now the index of the buffer holding the final order
-        if (bufs[cur] != (int32_t*)set.perm.p) e = e == cudaSuccess ? cudaErrorUnknown : e;
+            e = launch_seq_keys(d_res, (const int64_t*)offsets.p, d_len, n, (unsigned long long*)ctx->keys_a.p, va, s,
+                                launches);
+        bool in_b = false;
+        if (e == cudaSuccess)
+            e = radix_sort_u64((unsigned long long*)ctx->keys_a.p, (unsigned long long*)ctx->keys_b.p, va, vb, n, shifts,
+                               kPasses, ctx->radix_scratch.p, s, launches, &in_b);
+        if (e == cudaSuccess && n > 1 && (in_b ? vb : va) != (int32_t*)set.perm.p) e = cudaErrorUnknown;
+        if (e == cudaSuccess && n == 1)  // nothing was sorted: the payload sits in va
+            e = cudaMemcpyAsync(set.perm.p, va, sizeof(int32_t), cudaMemcpyDeviceToDevice, s);
     }
     if (e == cudaSuccess)
         e = launch_pack(d_res, (const int64_t*)offsets.p, d_len, (const int32_t*)set.perm.p, n, lt, set.pat_stride,
@@ -420,21 +418,16 @@ int assemble_phase(tcrnet_ctx* ctx, int64_t n_keys, int* launches) {
     const int64_t n = ctx->n;
     const unsigned long long* sorted = (const unsigned long long*)ctx->keys_a.p;
     if (n_keys > 1) {
-        const int64_t blocks = split_num_blocks(n_keys);
         TRY(dev_reserve(ctx, ctx->keys_b, sizeof(unsigned long long) * (size_t)n_keys));
-        TRY(dev_reserve(ctx, ctx->split_hist, sizeof(uint32_t) * 256 * (size_t)blocks));
-        TRY(dev_reserve(ctx, ctx->split_hist_scanned, sizeof(uint32_t) * 256 * (size_t)blocks));
-        TRY(dev_reserve(ctx, ctx->scan_scratch, scan_scratch_bytes(256 * blocks)));
+        TRY(dev_reserve(ctx, ctx->radix_scratch, radix_scratch_bytes(n_keys)));
         const int id_bits = bits_for(n - 1 > 0 ? n - 1 : 1);
-        unsigned long long* a = (unsigned long long*)ctx->keys_a.p;
-        unsigned long long* b = (unsigned long long*)ctx->keys_b.p;
+        int shifts[kRadixMaxPasses], n_passes = 0;
         for (int half = 0; half < 2; ++half)
-            for (int sh = 0; sh < id_bits; sh += 8) {
-                TRY_CUDA(split_keys_u64(a, b, n_keys, 32 * half + sh, (uint32_t*)ctx->split_hist.p,
-                                        (uint32_t*)ctx->split_hist_scanned.p, ctx->scan_scratch.p, s, launches));
-                std::swap(a, b);
-            }
-        sorted = a;
+            for (int sh = 0; sh < id_bits; sh += 8) shifts[n_passes++] = 32 * half + sh;
+        bool in_b = false;
+        TRY_CUDA(radix_sort_u64((unsigned long long*)ctx->keys_a.p, (unsigned long long*)ctx->keys_b.p, nullptr, nullptr,
+                                n_keys, shifts, n_passes, ctx->radix_scratch.p, s, launches, &in_b));
+        if (in_b) sorted = (const unsigned long long*)ctx->keys_b.p;
     }
     TRY_CUDA(cudaEventRecord(ctx->ev[2], s));
     TRY(dev_reserve(ctx, ctx->row_ptr, sizeof(int64_t) * (size_t)(n + 1)));
@@ -531,8 +524,8 @@ void tcrnet_destroy(tcrnet_ctx* ctx) {
     DevBuf* bufs[] = {&ctx->all.perm, &ctx->all.pat, &ctx->all.txt, &ctx->all.trie, &ctx->query.perm, &ctx->query.pat,
                       &ctx->query.txt, &ctx->query.trie, &ctx->inv_perm, &ctx->edge_dist, &ctx->edge_dist_b, &ctx->flags,
                       &ctx->flag_pos, &ctx->in_res, &ctx->in_len, &ctx->offsets,
-                      &ctx->perm_tmp, &ctx->trie_scratch, &ctx->keys_a, &ctx->keys_b, &ctx->split_hist,
-                      &ctx->split_hist_scanned, &ctx->scan_scratch, &ctx->rows, &ctx->row_ptr, &ctx->col,
+                      &ctx->perm_tmp, &ctx->trie_scratch, &ctx->keys_a, &ctx->keys_b, &ctx->radix_scratch,
+                      &ctx->scan_scratch, &ctx->rows, &ctx->row_ptr, &ctx->col,
                       &ctx->deg, &ctx->ctrl, &ctx->obs_ctrl, &ctx->deg_hist, &ctx->nn_sum, &ctx->class_sum, &ctx->knn,
                       &ctx->cc_parent, &ctx->cc_count, &ctx->cc_label, &ctx->cc_size, &ctx->perc_rank,
                       &ctx->perc_seen, &ctx->perc_deg, &ctx->perc_hist, &ctx->perc_lcc};

@@ -69,7 +69,7 @@ struct tcrnet_ctx {
     bool have_dist = false;  // edge_dist valid for the current CSR
     int built_l_max = 0;
     int64_t n_edges = 0, n_keys = 0;
-    DevBuf keys_a, keys_b, split_hist, split_hist_scanned, scan_scratch, rows, row_ptr, col, deg;
+    DevBuf keys_a, keys_b, radix_scratch, scan_scratch, rows, row_ptr, col, deg;
     DevBuf inv_perm, edge_dist, edge_dist_b, flags, flag_pos;
 
     // observables state (observables_api.cu); valid for the current CSR only

@@ -104,24 +104,22 @@ cudaError_t exclusive_scan_u32(const uint32_t* in, uint32_t* out, int64_t n, voi
 cudaError_t exclusive_scan_u32_total(const uint32_t* in, uint32_t* out /*[n+1]*/, int64_t n, void* scratch,
                                      cudaStream_t s, int* launches);
 
-// split.cu: one stable counting-sort pass over 8-bit digits.
-int64_t split_num_blocks(int64_t n);
-// Stable passes of the sequence sort: perm_out = perm_in (NULL = identity) re-ordered by the clamped
-// length / by the residue at position k.  hist, hist_scanned: uint32[256 * split_num_blocks(n)].
-cudaError_t split_by_length(const int32_t* lengths, const int32_t* perm_in, int64_t n, int32_t* perm_out,
-                            uint32_t* hist, uint32_t* hist_scanned, void* scan_scratch, cudaStream_t s,
-                            int* launches);
-cudaError_t split_by_residue(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths,
-                             const int32_t* perm_in, int k, int64_t n, int32_t* perm_out, uint32_t* hist,
-                             uint32_t* hist_scanned, void* scan_scratch, cudaStream_t s, int* launches);
-// one radix pass on 64-bit keys, digit = (key >> shift) & 255.
-cudaError_t split_keys_u64(const unsigned long long* in, unsigned long long* out, int64_t n, int shift,
-                           uint32_t* hist, uint32_t* hist_scanned, void* scan_scratch, cudaStream_t s,
-                           int* launches);
+// radix.cu: stable LSD radix sort of 64-bit keys (optional 32-bit payload) over the 8-bit digits
+// (key >> shifts[p]) & 255, p = 0..n_passes-1 in that order.  Ping-pongs between the a and b buffers;
+// *result_in_b says where the sorted sequence ends up.  scratch: radix_scratch_bytes(n).
+constexpr int kRadixMaxPasses = 8;
+size_t radix_scratch_bytes(int64_t n);
+cudaError_t radix_sort_u64(unsigned long long* keys_a, unsigned long long* keys_b, int32_t* vals_a, int32_t* vals_b,
+                           int64_t n, const int* shifts, int n_passes, void* scratch, cudaStream_t s, int* launches,
+                           bool* result_in_b);
 
 // pack.cu
 cudaError_t launch_length_hist(const int32_t* lengths, int64_t n, unsigned long long* hist /*[kNumLen]*/,
                                uint32_t* flags, cudaStream_t s, int* launches);
+// sort key of row i: (clamped length << 30) | the first kSortPrefix residues, 5 bits each (0 = past the end); vals[i] = i
+constexpr int kSeqKeyBits = 6 + 5 * kSortPrefix;
+cudaError_t launch_seq_keys(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths, int64_t n,
+                            unsigned long long* keys, int32_t* vals, cudaStream_t s, int* launches);
 cudaError_t launch_pack(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths,
                         const int32_t* perm, int64_t n, const LengthTable& lt, int pat_stride,
                         uint8_t* pat, uint32_t* txt, uint32_t* flags, cudaStream_t s, int* launches);
