@@ -39,8 +39,8 @@ ALU_OPS_PER_TEST = 4           # 2 LOP3 + IADD3 + ISETP per pair and early-exit 
 ALU_OPS_PER_PREFIX_TEST = 2    # LOP3 + ISETP per pair and DP cell read in a guided expansion (distance_trie.cu)
 ORACLE_SAMPLE_ROWS = 1024
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_distance_trie launch at cfg4, from the ncu --set full
-# capture summarised in profiles/r1c_trie_ncu.txt (94.63 MB + 22.30 MB)
-NCU_DRAM_BYTES_PER_LAUNCH = {"cfg4": 116_930_816}
+# capture summarised in profiles/r1d_trie_ncu.txt (95.40 MB + 19.77 MB)
+NCU_DRAM_BYTES_PER_LAUNCH = {"cfg4": 115_171_584}
 
 
 def _peaks():
