@@ -5,9 +5,10 @@
 // final-diagonal early exit, warp-aggregated emission - but the texts of a
 // length bucket are visited through the prefix trie of trie.cu instead of one by one:
 //
-//   * One CTA = 256 patterns of one length (one per thread, Peq column private in shared memory)
-//     against a chunk [lo, hi) of the sorted texts of one length.  A warp (32 patterns that are
-//     neighbours in lexicographic order) walks the trie depth-first.  Entering a level-k node
+//   * One work item = one warp = 32 patterns of one length (one per lane, neighbours in lexicographic
+//     order, Peq column private in shared memory) against a chunk [lo, hi) of the sorted texts of one
+//     length.  The kernel is persistent: every warp claims items from a device-wide queue until it is
+//     empty.  The warp walks the trie depth-first.  Entering a level-k node
 //     costs ONE column step (its residue code at position k-1) on top of the parent's (Pv, Mv):
 //     the columns of a shared prefix are computed once per node, not once per text.
 //   * The final-diagonal cell is TRACKED, not recomputed: with i = k - delta (delta = n - m),
@@ -44,12 +45,26 @@
 // The kernel is specialised on l_max (template LMAX = 0..kTrieMaxL): thresholds are immediates and
 // the t-loop is unrolled to its exact trip count.  delta is run-time but warp-uniform; it enters only
 // through six precomputed bit masks.
+#include <algorithm>
+
 #include "myers.cuh"
 
 namespace tcrnet {
 namespace {
 
 constexpr uint32_t kFull = 0xffffffffu;
+constexpr int kTrieWarps = 8;                    // warps per CTA (independent of each other)
+constexpr int kTrieThreads = 32 * kTrieWarps;
+// Per-warp shared memory: Peq[kPeqRows][kTrieTile + 1 words] (the odd row stride keeps the row address a true
+// multiply-add, which ptxas issues on the FMA pipe), then the staging buffers [kTrieDepth][kTrieFan] x 16 B.
+template <typename W>
+__host__ __device__ constexpr int trie_peq_row_bytes() {
+    return (kTrieTile + 1) * (int)sizeof(W);
+}
+template <typename W>
+__host__ __device__ constexpr int trie_warp_smem_bytes() {
+    return ((kPeqRows * trie_peq_row_bytes<W>() + 15) & ~15) + kTrieDepth * kTrieFan * 16;
+}
 constexpr int kClipLevels = 3;      // levels whose nodes are clipped to the work item's text chunk
 constexpr int kDeadLane = 1 << 20;  // dg of a lane without a pattern: never alive, never emitted
 
@@ -111,7 +126,7 @@ __device__ __forceinline__ void finish_texts(Walk<W, COUNT>& w, const DistancePa
                 if (j0 == kJ0 && q < (START & 3)) continue;  // columns already in (Pv0, Mv0)
                 const int j = j0 + q;
                 if (j >= w.n) break;  // warp-uniform
-                const W D0 = column_step<W>(peq_load<W>(w.lane_addr, c[q]), Pv, Mv);
+                const W D0 = column_step<W>(peq_load<W, trie_peq_row_bytes<W>()>(w.lane_addr, c[q]), Pv, Mv);
                 if ((D0 & bm) == W(0)) ++dg;
                 bm += bm;
                 if (COUNT) ++w.n_cols;
@@ -172,7 +187,7 @@ __device__ __forceinline__ void visit(Walk<W, COUNT>& w, const DistanceParams& P
         if (LEVEL <= kClipLevels) {  // clip the upper levels to this warp's texts
             if (nd.y <= w.lo || nd.x >= w.hi) continue;
         }
-        const W Eq = peq_load<W>(w.lane_addr, c);
+        const W Eq = peq_load<W, trie_peq_row_bytes<W>()>(w.lane_addr, c);
         W P2 = Pv, M2 = Mv;
         W D0;
         if (LEVEL == 1) {
@@ -195,73 +210,84 @@ __device__ __forceinline__ void visit(Walk<W, COUNT>& w, const DistanceParams& P
     } while (U);
 }
 
+// One warp = one work item at a time: kTrieTile patterns of one length (neighbours in lexicographic order) against
+// a chunk of one text bucket.  Items are claimed from a device-wide queue (one atomicAdd per item, big rows first),
+// so a warp slot is never idle while work is left; each warp owns a private Peq table and staging buffer in shared
+// memory and there is no CTA-level barrier anywhere.
 template <typename W, int LMAX, bool COUNT>
-__global__ void __launch_bounds__(kTQ, sizeof(W) == 4 ? 4 : 2) k_distance_trie(const __grid_constant__ DistanceParams P) {
+__global__ void __launch_bounds__(kTrieThreads, sizeof(W) == 4 ? 4 : 2) k_distance_trie(const __grid_constant__ DistanceParams P) {
     extern __shared__ __align__(16) unsigned char smem[];
-    constexpr int kRowBytes = peq_row_bytes<W>();
-    static_assert((kPeqRows * kRowBytes) % 16 == 0, "the staging buffers follow the Peq table");
-    W* peq = reinterpret_cast<W*>(smem);
-    uint4* stage_all = reinterpret_cast<uint4*>(smem + kPeqRows * kRowBytes);
+    constexpr int kRowBytes = trie_peq_row_bytes<W>();
+    constexpr int kWarpBytes = trie_warp_smem_bytes<W>();
 
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-
-    // ---- step A2, device side: which (bucket pair, pattern tile, text chunk) is this CTA? ----
-    const int64_t item = work_item(P);
-    const WorkRow R = find_row(P, item);
-    const int64_t local = item - R.item_begin;
-    const int pi = (int)(local / R.n_tchunks), qi = (int)(local % R.n_tchunks);
-    const int p_tile0 = pi * kTQ;             // relative to the pattern bucket
-    const int chunk_t0 = qi * R.tchunk;       // relative to the text bucket
-    const int chunk_cnt = min(R.tchunk, R.t_count - chunk_t0);
-    if (R.diag && chunk_t0 + chunk_cnt <= p_tile0 + 1) return;  // wholly on/below the diagonal
-
-    const int m = R.m, n = R.n;
-    const int delta = n - m;                  // 0 <= delta <= l_max = LMAX
-    const int p_rel = p_tile0 + tid;
-    const bool p_valid = p_rel < R.p_count;
-    build_peq<W>(peq, tid, p_valid, P.pat + (size_t)(R.p_start + p_rel) * P.pat_stride, m);
-
-    // same bucket: a warp pairs only with the texts after its first pattern (sorted p < t)
-    const int warp_p0 = p_tile0 + warp * 32;
-    const int lo_rel = R.diag ? max(chunk_t0, warp_p0 + 1) : chunk_t0;
-    const int hi_rel = chunk_t0 + chunk_cnt;
-    if (lo_rel >= hi_rel || warp_p0 >= R.p_count) return;  // warp-uniform; no CTA barrier follows
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    unsigned char* wsmem = smem + warp * kWarpBytes;
+    W* peq = reinterpret_cast<W*>(wsmem);
+    const uint32_t peq_addr = (uint32_t)__cvta_generic_to_shared(wsmem);
 
     Walk<W, COUNT> w;
-    w.stage_addr = (uint32_t)__cvta_generic_to_shared(stage_all) + warp * (kTrieDepth * kTrieFan * 16);
-    w.rows = P.txt + R.txt_base - (size_t)R.t_start * R.row_words;
-    w.lane_addr = (uint32_t)__cvta_generic_to_shared(smem) + tid * (uint32_t)sizeof(W);
-    w.lo = (uint32_t)(R.t_start + lo_rel);
-    w.hi = (uint32_t)(R.t_start + hi_rel);
-    w.dsh = (uint32_t)delta + 1u;
-    {
-        // one-hot codes of the pattern's first rows, shifted by delta: ohs[q] belongs to row q - delta
-        const uint8_t* prow = P.pat + (size_t)(R.p_start + p_rel) * P.pat_stride;
-        const uint2 head = p_valid ? __ldg(reinterpret_cast<const uint2*>(prow)) : make_uint2(0xffffffffu, 0xffffffffu);
-#pragma unroll
-        for (int q = 0; q <= kTrieDepth; ++q) {
-            const int r = q - delta;  // 1-based pattern row
-            uint32_t code = 0xffu;
-            if (r >= 1 && r <= m) code = ((r <= 4 ? head.x : head.y) >> (8 * ((r - 1) & 3))) & 0xffu;
-            w.ohs[q] = code < 32u ? 1u << code : 0u;
-        }
-    }
-    w.pv_init = low_mask<W>(m);
-    w.rw = R.row_words;
-    w.n = n;
+    w.stage_addr = peq_addr + ((kPeqRows * kRowBytes + 15) & ~15);
+    w.lane_addr = peq_addr + lane * (uint32_t)sizeof(W);
     w.lane = lane;
-    w.p_sorted = R.p_start + p_rel;
-    w.p_lim = R.diag ? w.p_sorted : -1;
 
-    // codes of the bucket's level-1 nodes
-    uint32_t root_codes = 0u;
-    {
-        const int cnt = (int)(R.root_end - R.root_begin);
-        if (lane < cnt) root_codes = 1u << (P.trie[1][R.root_begin + lane].code & 31u);
-        root_codes = __reduce_or_sync(kFull, root_codes);
+    const long long n_local = (P.n_items - P.shard + P.n_shards - 1) / P.n_shards;  // step 8(e): interleaved shards
+    for (;;) {
+        // ---- step A2, device side: claim the next (bucket pair, pattern tile, text chunk) ----
+        unsigned long long q = 0;
+        if (lane == 0) q = atomicAdd(P.queue, 1ull);
+        q = __shfl_sync(kFull, q, 0);
+        if ((long long)q >= n_local) break;
+        const int64_t item = (int64_t)q * P.n_shards + P.shard;
+        const WorkRow R = find_row(P, item);
+        const int64_t local = item - R.item_begin;
+        const int pi = (int)(local / R.n_tchunks), qi = (int)(local % R.n_tchunks);
+        const int p_tile0 = pi * kTrieTile;       // relative to the pattern bucket
+        const int chunk_t0 = qi * R.tchunk;       // relative to the text bucket
+        const int chunk_cnt = min(R.tchunk, R.t_count - chunk_t0);
+        // same bucket: a warp pairs only with the texts after its first pattern (sorted p < t)
+        const int lo_rel = R.diag ? max(chunk_t0, p_tile0 + 1) : chunk_t0;
+        const int hi_rel = chunk_t0 + chunk_cnt;
+        if (lo_rel >= hi_rel) continue;  // wholly on/below the diagonal
+
+        const int m = R.m, n = R.n;
+        const int delta = n - m;                  // 0 <= delta <= l_max = LMAX
+        const int p_rel = p_tile0 + lane;
+        const bool p_valid = p_rel < R.p_count;
+        const uint8_t* prow = P.pat + (size_t)(R.p_start + p_rel) * P.pat_stride;
+        __syncwarp();  // the previous item's Peq reads are done
+        build_peq<W, kRowBytes>(peq, lane, p_valid, prow, m);
+
+        w.rows = P.txt + R.txt_base - (size_t)R.t_start * R.row_words;
+        w.lo = (uint32_t)(R.t_start + lo_rel);
+        w.hi = (uint32_t)(R.t_start + hi_rel);
+        w.dsh = (uint32_t)delta + 1u;
+        {
+            // one-hot codes of the pattern's first rows, shifted by delta: ohs[q] belongs to row q - delta
+            const uint2 head = p_valid ? __ldg(reinterpret_cast<const uint2*>(prow)) : make_uint2(0xffffffffu, 0xffffffffu);
+#pragma unroll
+            for (int k = 0; k <= kTrieDepth; ++k) {
+                const int r = k - delta;  // 1-based pattern row
+                uint32_t code = 0xffu;
+                if (r >= 1 && r <= m) code = ((r <= 4 ? head.x : head.y) >> (8 * ((r - 1) & 3))) & 0xffu;
+                w.ohs[k] = code < 32u ? 1u << code : 0u;
+            }
+        }
+        w.pv_init = low_mask<W>(m);
+        w.rw = R.row_words;
+        w.n = n;
+        w.p_sorted = R.p_start + p_rel;
+        w.p_lim = R.diag ? w.p_sorted : -1;
+
+        // codes of the bucket's level-1 nodes
+        uint32_t root_codes = 0u;
+        {
+            const int cnt = (int)(R.root_end - R.root_begin);
+            if (lane < cnt) root_codes = 1u << (P.trie[1][R.root_begin + lane].code & 31u);
+            root_codes = __reduce_or_sync(kFull, root_codes);
+        }
+        // D[0][delta] = delta is the first cell of the final diagonal
+        visit<W, LMAX, COUNT, 1>(w, P, R.root_begin, root_codes, w.pv_init, W(0), p_valid ? delta : kDeadLane);
     }
-    // D[0][delta] = delta is the first cell of the final diagonal
-    visit<W, LMAX, COUNT, 1>(w, P, R.root_begin, root_codes, w.pv_init, W(0), p_valid ? delta : kDeadLane);
 
     if (COUNT) {
         // warp-level counters (identical in all lanes): lane 0 reports 32 lanes' worth
@@ -275,28 +301,33 @@ __global__ void __launch_bounds__(kTQ, sizeof(W) == 4 ? 4 : 2) k_distance_trie(c
 }
 
 template <typename W, int LMAX, bool COUNT>
-cudaError_t launch_one(const DistanceParams& p, int64_t n_items, size_t smem, cudaStream_t s) {
+cudaError_t launch_one(const DistanceParams& p, int64_t n_items, size_t smem, int n_sm, cudaStream_t s) {
     auto kern = k_distance_trie<W, LMAX, COUNT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    kern<<<(unsigned)((n_items - p.shard + p.n_shards - 1) / p.n_shards), kTQ, smem, s>>>(p);
+    // persistent: every warp slot the kernel can hold, or one warp per item if there are fewer
+    const int64_t n_local = (n_items - p.shard + p.n_shards - 1) / p.n_shards;
+    const int64_t ctas_full = (int64_t)n_sm * (sizeof(W) == 4 ? 4 : 2);
+    const int64_t ctas = std::max<int64_t>(1, std::min(ctas_full, (n_local + kTrieWarps - 1) / kTrieWarps));
+    kern<<<(unsigned)ctas, kTrieThreads, smem, s>>>(p);
     return cudaGetLastError();
 }
 
 template <typename W, int LMAX>
-cudaError_t launch_lmax(const DistanceParams& p, int64_t n_items, bool count_work, size_t smem, cudaStream_t s) {
-    return count_work ? launch_one<W, LMAX, true>(p, n_items, smem, s) : launch_one<W, LMAX, false>(p, n_items, smem, s);
+cudaError_t launch_lmax(const DistanceParams& p, int64_t n_items, bool count_work, size_t smem, int n_sm, cudaStream_t s) {
+    return count_work ? launch_one<W, LMAX, true>(p, n_items, smem, n_sm, s)
+                      : launch_one<W, LMAX, false>(p, n_items, smem, n_sm, s);
 }
 
 template <typename W>
-cudaError_t launch_word(const DistanceParams& p, int64_t n_items, bool count_work, size_t smem, cudaStream_t s) {
+cudaError_t launch_word(const DistanceParams& p, int64_t n_items, bool count_work, size_t smem, int n_sm, cudaStream_t s) {
     static_assert(kTrieMaxL == 4, "one case per specialised l_max");
     switch (p.l_max) {
-        case 0: return launch_lmax<W, 0>(p, n_items, count_work, smem, s);
-        case 1: return launch_lmax<W, 1>(p, n_items, count_work, smem, s);
-        case 2: return launch_lmax<W, 2>(p, n_items, count_work, smem, s);
-        case 3: return launch_lmax<W, 3>(p, n_items, count_work, smem, s);
-        case 4: return launch_lmax<W, 4>(p, n_items, count_work, smem, s);
+        case 0: return launch_lmax<W, 0>(p, n_items, count_work, smem, n_sm, s);
+        case 1: return launch_lmax<W, 1>(p, n_items, count_work, smem, n_sm, s);
+        case 2: return launch_lmax<W, 2>(p, n_items, count_work, smem, n_sm, s);
+        case 3: return launch_lmax<W, 3>(p, n_items, count_work, smem, n_sm, s);
+        case 4: return launch_lmax<W, 4>(p, n_items, count_work, smem, n_sm, s);
         default: return cudaErrorInvalidValue;
     }
 }
@@ -304,18 +335,16 @@ cudaError_t launch_word(const DistanceParams& p, int64_t n_items, bool count_wor
 }  // namespace
 
 size_t distance_trie_smem_bytes(bool wide) {
-    const size_t peq = (size_t)kPeqRows * (wide ? peq_row_bytes<uint64_t>() : peq_row_bytes<uint32_t>());
-    return peq + (size_t)(kTQ / 32) * kTrieDepth * kTrieFan * sizeof(uint4);
+    return (size_t)kTrieWarps * (wide ? trie_warp_smem_bytes<uint64_t>() : trie_warp_smem_bytes<uint32_t>());
 }
 
-cudaError_t launch_distance_trie(const DistanceParams& p, int64_t n_items, bool wide, bool count_work,
+cudaError_t launch_distance_trie(const DistanceParams& p, int64_t n_items, bool wide, bool count_work, int n_sm,
                                  cudaStream_t s, int* launches) {
     if (n_items <= p.shard) return cudaSuccess;
-    if (n_items > 0x7fffffffLL) return cudaErrorInvalidValue;
     const size_t smem = distance_trie_smem_bytes(wide);
     *launches += 1;
-    return wide ? launch_word<uint64_t>(p, n_items, count_work, smem, s)
-                : launch_word<uint32_t>(p, n_items, count_work, smem, s);
+    return wide ? launch_word<uint64_t>(p, n_items, count_work, smem, n_sm, s)
+                : launch_word<uint32_t>(p, n_items, count_work, smem, n_sm, s);
 }
 
 }  // namespace tcrnet

@@ -115,18 +115,17 @@ __device__ __forceinline__ uint32_t first_column_step<uint32_t>(uint32_t Eq, uin
 // Shared-memory accesses by 32-bit shared address (no generic-pointer arithmetic in the hot loop).
 // The text loads are volatile so that they stay behind the barrier that publishes the stage; the Peq
 // loads depend on their results.
-template <typename W>
-__device__ __forceinline__ W peq_load(uint32_t lane_addr, uint32_t code);
-template <>
-__device__ __forceinline__ uint32_t peq_load<uint32_t>(uint32_t lane_addr, uint32_t code) {
-    uint32_t v;
-    asm("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(lane_addr + code * (uint32_t)peq_row_bytes<uint32_t>()));
-    return v;
+__device__ __forceinline__ void lds_word(uint32_t addr, uint32_t& v) { asm("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr)); }
+__device__ __forceinline__ void lds_word(uint32_t addr, uint64_t& v) {
+    unsigned long long t;
+    asm("ld.shared.u64 %0, [%1];" : "=l"(t) : "r"(addr));
+    v = t;
 }
-template <>
-__device__ __forceinline__ uint64_t peq_load<uint64_t>(uint32_t lane_addr, uint32_t code) {
-    unsigned long long v;
-    asm("ld.shared.u64 %0, [%1];" : "=l"(v) : "r"(lane_addr + code * (uint32_t)peq_row_bytes<uint64_t>()));
+// Peq[code] of this thread's pattern; ROW_BYTES = bytes per Peq row (one word per pattern of the tile + padding)
+template <typename W, int ROW_BYTES = peq_row_bytes<W>()>
+__device__ __forceinline__ W peq_load(uint32_t lane_addr, uint32_t code) {
+    W v;
+    lds_word(lane_addr + code * (uint32_t)ROW_BYTES, v);
     return v;
 }
 __device__ __forceinline__ void text_load4(uint32_t addr, uint32_t* c) {
@@ -160,9 +159,9 @@ __device__ __forceinline__ void cp_async_wait() {
 }
 
 // Peq for this thread's pattern: column `tid` of peq[code][*] (private to the thread: no barrier).
-template <typename W>
+template <typename W, int ROW_BYTES = peq_row_bytes<W>()>
 __device__ __forceinline__ void build_peq(W* peq, int tid, bool p_valid, const uint8_t* pat_row, int m) {
-    constexpr int kRowWords = peq_row_bytes<W>() / (int)sizeof(W);
+    constexpr int kRowWords = ROW_BYTES / (int)sizeof(W);
 #pragma unroll
     for (int r = 0; r < kPeqRows; ++r) peq[r * kRowWords + tid] = W(0);
     if (p_valid) {

@@ -254,9 +254,10 @@ void schedule_pass(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule::
             pass.part[trie ? 1 : 0][m <= 32 ? 0 : 1].rows.push_back(r);
         }
     }
-    for (auto& by_kernel : pass.part)
-        for (Schedule::Part& part : by_kernel) {
-            auto n_items = [](const WorkRow& r) { return (int64_t)((r.p_count + kTQ - 1) / kTQ) * r.n_tchunks; };
+    for (int trie = 0; trie < 2; ++trie)
+        for (Schedule::Part& part : pass.part[trie]) {
+            const int tile = trie ? kTrieTile : kTQ;  // patterns per work item
+            auto n_items = [tile](const WorkRow& r) { return (int64_t)((r.p_count + tile - 1) / tile) * r.n_tchunks; };
             // big rows first: the small buckets fill the tail of the launch
             std::stable_sort(part.rows.begin(), part.rows.end(), [&](const WorkRow& a, const WorkRow& b) {
                 return (long double)a.p_count * a.t_count * a.n > (long double)b.p_count * b.t_count * b.n;
@@ -328,7 +329,9 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
                  int n_shards, int* launches) {
     cudaStream_t s = ctx->stream;
     HostCtrl* dc = d_ctrl(ctx);
-    TRY_CUDA(cudaMemsetAsync(&dc->edge_count, 0, sizeof(unsigned long long) * 5, s));  // edge_count + work[4]
+    static_assert(offsetof(HostCtrl, queue) == offsetof(HostCtrl, edge_count) + 5 * sizeof(unsigned long long), "one memset");
+    TRY_CUDA(cudaMemsetAsync(&dc->edge_count, 0, sizeof(unsigned long long) * (5 + kTrieQueues), s));  // edge_count, work[4], queue[]
+    int n_queues = 0;
     const WorkRow* d_rows = (const WorkRow*)ctx->rows.p;
     for (const Schedule::Pass& pass : sch.passes) {
         DistanceParams p{};
@@ -353,9 +356,12 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
                 if (!part.rows.empty()) {
                     p.rows = d_rows;
                     p.n_rows = (int32_t)part.rows.size();
-                    if (trie)
-                        TRY_CUDA(launch_distance_trie(p, part.items, wide != 0, ctx->count_work != 0, s, launches));
-                    else
+                    if (trie) {
+                        if (n_queues >= kTrieQueues) return TCRNET_ERR_STATE;  // at most 2 passes x 2 word sizes
+                        p.queue = dc->queue + n_queues++;
+                        p.n_items = part.items;
+                        TRY_CUDA(launch_distance_trie(p, part.items, wide != 0, ctx->count_work != 0, ctx->n_sm, s, launches));
+                    } else
                         TRY_CUDA(launch_distance(p, part.items, wide != 0, first_check, ctx->count_work != 0,
                                                  part.max_rw, s, launches));
                 }

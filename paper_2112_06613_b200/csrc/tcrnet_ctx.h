@@ -16,6 +16,7 @@ struct HostCtrl {  // pinned mirror of the small device control block
     unsigned long long hist[kNumLen];
     unsigned long long edge_count;
     unsigned long long work[4];
+    unsigned long long queue[kTrieQueues];  // dynamic work queues of the trie launches (zeroed with edge_count)
     unsigned long long probe[3];
     uint32_t flags;
     uint32_t pad_;

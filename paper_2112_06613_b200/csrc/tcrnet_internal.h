@@ -20,6 +20,8 @@ constexpr int kSortPrefix = 6;           // residues of the lexicographic sub-or
 constexpr int kTrieDepth = kSortPrefix;  // levels 1..kTrieDepth of the prefix trie over each text bucket
 constexpr int kTrieFan = 27;             // staging slots per trie level, indexed by residue code (0..26)
 constexpr int kTrieMaxL = 4;             // the trie kernel is specialised on l_max = 0..kTrieMaxL
+constexpr int kTrieTile = 32;            // patterns per work item of the trie kernel: one warp
+constexpr int kTrieQueues = 8;           // dynamic work queues (one per trie launch of a distance pass)
 
 // Per-length layout of the packed sequence tables (filled on the host after the histogram).
 struct LengthTable {
@@ -30,7 +32,7 @@ struct LengthTable {
 
 // One (pattern bucket, text bucket) pair of the tile scheduler (step A2).
 struct WorkRow {
-    int64_t item_begin;  // first work item (CTA) of this row
+    int64_t item_begin;  // first work item of this row (chunk kernel: one CTA, kTQ patterns; trie kernel: one warp, kTrieTile)
     int64_t txt_base;    // first word of the text bucket's rows
     int32_t p_start;     // sorted position of the first pattern (the shorter-or-equal length)
     int32_t p_count;
@@ -90,6 +92,8 @@ struct DistanceParams {
     unsigned long long* work;        // [4]: lane-columns, lane-tests (exit votes), lane-first-columns,
                                      //      lane-V-sets (guided expansions); COUNT only
     const TrieNode* trie[kTrieDepth + 1];  // trie kernel: nodes of level 1..kTrieDepth ([0] unused)
+    unsigned long long* queue;       // trie kernel: next unclaimed work item of this launch (zeroed before the launch)
+    int64_t n_items;                 // trie kernel: work items of all shards of this launch
 };
 
 // ---- launch wrappers (each returns cudaGetLastError(); *launches is incremented per kernel) ----
@@ -143,7 +147,7 @@ cudaError_t launch_distance(const DistanceParams& p, int64_t n_items, bool wide,
                             bool count_work, int max_row_words, cudaStream_t s, int* launches);
 // distance_trie.cu: the prefix-trie kernel
 size_t distance_trie_smem_bytes(bool wide);
-cudaError_t launch_distance_trie(const DistanceParams& p, int64_t n_items, bool wide, bool count_work,
+cudaError_t launch_distance_trie(const DistanceParams& p, int64_t n_items, bool wide, bool count_work, int n_sm,
                                  cudaStream_t s, int* launches);
 
 // labels.cu: distance labels of the final edges, threshold restriction, key validation
