@@ -206,7 +206,7 @@ class TcrNet:
             residues = np.ascontiguousarray(residues, dtype=np.uint8)
             lengths = np.ascontiguousarray(lengths, dtype=np.int32)
             n = int(lengths.size)
-            if n >= 1 and int(np.maximum(lengths, 0).sum(dtype=np.int64)) > residues.size:
+            if n >= 1 and int(lengths.sum(dtype=np.int64)) > residues.size:  # (negative lengths: rejected by the library)
                 raise TcrNetError(ERR_ARG, "tcrnet_load (residues shorter than sum(lengths))")
             _check(self._lib.tcrnet_load(self._ctx, residues.ctypes.data_as(C.POINTER(C.c_uint8)),
                                          lengths.ctypes.data_as(C.POINTER(C.c_int32)), n), "tcrnet_load")

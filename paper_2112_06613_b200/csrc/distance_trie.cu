@@ -93,10 +93,34 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
 __device__ __forceinline__ void sts128(uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
     asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
 }
+// Pin a value in a register: the compiler may not recompute it from its definition (threadIdx, the shared window).
+__device__ __forceinline__ void keep(uint32_t& x) { asm volatile("" : "+r"(x)); }
 __device__ __forceinline__ uint32_t top_bit(uint32_t x) {  // index of the highest set bit (x != 0)
     uint32_t r;
     asm("bfind.u32 %0, %1;" : "=r"(r) : "r"(x));
     return r;
+}
+
+// Columns j0 + Q0 .. j0 + 3 of one text (residue codes c4; FULL: all of them exist, else only those < n).
+// Returns false when the exit vote kills the text (dg > l_max in all 32 lanes).
+template <typename W, int LMAX, bool COUNT, int Q0, bool FULL>
+__device__ __forceinline__ bool columns4(Walk<W, COUNT>& w, const uint4 c4, int j0, W& Pv, W& Mv, W& bm, int& dg) {
+    // exit vote after every column, or after every second one for l_max <= 1 (measured: cfg4 / cfg5)
+    constexpr int kVoteEvery = LMAX >= 2 ? 1 : 2;
+    const uint32_t c[4] = {c4.x, c4.y, c4.z, c4.w};
+#pragma unroll
+    for (int q = Q0; q < 4; ++q) {
+        if (!FULL && j0 + q >= w.n) return true;  // warp-uniform
+        const W D0 = column_step<W>(peq_load<W, trie_peq_row_bytes<W>()>(w.lane_addr, c[q]), Pv, Mv);
+        if ((D0 & bm) == W(0)) ++dg;
+        bm += bm;
+        if (COUNT) ++w.n_cols;
+        if (kVoteEvery == 1 || (q & 1)) {
+            if (COUNT) ++w.n_tests;
+            if (!__any_sync(kFull, dg <= LMAX)) return false;
+        }
+    }
+    return true;
 }
 
 // The texts [t0, t1) below a surviving deepest-level node, one by one: the text columns kTrieDepth .. n-1
@@ -105,52 +129,49 @@ __device__ __forceinline__ uint32_t top_bit(uint32_t x) {  // index of the highe
 // V sets prune more than the votes of this loop.)
 template <typename W, int LMAX, bool COUNT>
 __device__ __forceinline__ void finish_texts(Walk<W, COUNT>& w, const DistanceParams& P, uint32_t t0, uint32_t t1,
-                                             const W Pv0, const W Mv0, const int dg0) {
+                                             uint4 c4, const W Pv0, const W Mv0, const int dg0) {
     constexpr int START = kTrieDepth;
     static_assert(START >= 1 && START >= kTrieMaxL, "column 0 has its own step; final-diagonal rows exist from column delta on");
     constexpr int kJ0 = START & ~3;  // the 128-bit load that holds column START
-    // exit vote after every column, or after every second one for l_max <= 1 (measured: cfg4 / cfg5)
-    constexpr int kVoteEvery = LMAX >= 2 ? 1 : 2;
+    // c4 = the first columns of text t0 (requested by the caller before its own column step); those of text t + 1
+    // are requested before text t is processed, so the L2 latency of a row overlaps the previous text's columns
     for (uint32_t t = t0; t < t1; ++t) {
         const uint4* row = reinterpret_cast<const uint4*>(w.rows + (size_t)t * w.rw);
+        const uint4 c4_here = c4;
+        if (t + 1u < t1) c4 = __ldg(row + ((w.rw + kJ0) >> 2));
         W Pv = Pv0, Mv = Mv0;
         W bm = (W)w.dbit(START + 1);  // bit of row j + 1 - delta for column j = START
         int dg = dg0;
-        bool dead = false;
         // four columns per 128-bit load (the same address in all lanes)
-        for (int j0 = kJ0; j0 < w.n; j0 += 4) {
-            const uint4 c4 = __ldg(row + (j0 >> 2));
-            const uint32_t c[4] = {c4.x, c4.y, c4.z, c4.w};
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                if (j0 == kJ0 && q < (START & 3)) continue;  // columns already in (Pv0, Mv0)
-                const int j = j0 + q;
-                if (j >= w.n) break;  // warp-uniform
-                const W D0 = column_step<W>(peq_load<W, trie_peq_row_bytes<W>()>(w.lane_addr, c[q]), Pv, Mv);
-                if ((D0 & bm) == W(0)) ++dg;
-                bm += bm;
-                if (COUNT) ++w.n_cols;
-                if (kVoteEvery == 1 || (q & 1)) {
-                    if (COUNT) ++w.n_tests;
-                    if (!__any_sync(kFull, dg <= LMAX)) {
-                        dead = true;
-                        break;
-                    }
-                }
-            }
-            if (dead) break;
+        int j0 = kJ0;
+        bool alive;
+        {
+            alive = kJ0 + 4 <= w.n ? columns4<W, LMAX, COUNT, START & 3, true>(w, c4_here, kJ0, Pv, Mv, bm, dg)
+                                   : columns4<W, LMAX, COUNT, START & 3, false>(w, c4_here, kJ0, Pv, Mv, bm, dg);
+            j0 += 4;
         }
-        if (dead) continue;
+        while (alive && j0 + 4 <= w.n) {
+            alive = columns4<W, LMAX, COUNT, 0, true>(w, __ldg(row + (j0 >> 2)), j0, Pv, Mv, bm, dg);
+            j0 += 4;
+        }
+        if (alive && j0 < w.n) alive = columns4<W, LMAX, COUNT, 0, false>(w, __ldg(row + (j0 >> 2)), j0, Pv, Mv, bm, dg);
+        if (!alive) continue;
         const bool edge = dg <= LMAX && w.p_lim < (int)t;
         emit_edges(P, edge, w.lane, w.p_sorted, (int)t, w.n - (int)w.dsh + 1, w.n);
     }
+}
+
+// Lane i's share of the children [cb, cb + popc(cm)] of a node (the last one is the next node or the sentinel).
+template <int LEVEL>
+__device__ __forceinline__ uint4 load_children(const DistanceParams& P, uint32_t cb, uint32_t cm, int lane) {
+    return __ldg(reinterpret_cast<const uint4*>(P.trie[LEVEL]) + (cb + min((uint32_t)lane, (uint32_t)__popc(cm))));
 }
 
 // Expand the children (level LEVEL, nodes [cb, cb + popc(cm)), residue codes = the set bits of cm) of
 // one level-(LEVEL-1) node, or the roots of the text bucket.  (Pv, Mv) is the DP column after LEVEL-1
 // text residues and dg = D[LEVEL-1-delta][LEVEL-1] its final-diagonal cell (delta while there is none).
 template <typename W, int LMAX, bool COUNT, int LEVEL>
-__device__ __forceinline__ void visit(Walk<W, COUNT>& w, const DistanceParams& P, uint32_t cb, uint32_t cm,
+__device__ __forceinline__ void visit(Walk<W, COUNT>& w, const DistanceParams& P, uint32_t cm, const uint4 nd_lane,
                                       const W Pv, const W Mv, const int dg) {
     uint32_t U = cm;
     // Guided expansion: the codes whose child is alive in at least one lane.  Every child is alive
@@ -173,11 +194,9 @@ __device__ __forceinline__ void visit(Walk<W, COUNT>& w, const DistanceParams& P
     {
         const uint32_t cnt = (uint32_t)__popc(cm);  // <= 27 by construction; node cb + cnt is the next node or the sentinel
         __syncwarp();
-        const uint4 nd = __ldg(reinterpret_cast<const uint4*>(P.trie[LEVEL]) + (cb + min((uint32_t)w.lane, cnt)));
+        const uint4 nd = nd_lane;  // child min(lane, cnt), requested by the caller before its own column step
         const uint32_t text_end = __shfl_down_sync(kFull, nd.x, 1);
-        if ((uint32_t)w.lane < cnt) {
-            sts128(sb + nd.z * 16, nd.x, text_end, nd.y, nd.w);  // code < kTrieFan
-        }
+        if ((uint32_t)w.lane < cnt) sts128(sb + nd.z * 16, nd.x, text_end, nd.y, nd.w);  // code < kTrieFan
         __syncwarp();
     }
     do {
@@ -186,6 +205,17 @@ __device__ __forceinline__ void visit(Walk<W, COUNT>& w, const DistanceParams& P
         const uint4 nd = lds128(sb + c * 16);  // text_begin, text_end, child_begin, child_codes
         if (LEVEL <= kClipLevels) {  // clip the upper levels to this warp's texts
             if (nd.y <= w.lo || nd.x >= w.hi) continue;
+        }
+        // what the walk needs below this child - its children (one per lane), or the first columns of its first
+        // text - is requested now: the L2 latency overlaps the column step and the V sets
+        uint4 below = make_uint4(0u, 0u, 0u, 0u);
+        uint32_t t0 = 0u, t1 = 0u;
+        if constexpr (LEVEL < kTrieDepth) {
+            below = load_children<LEVEL + 1>(P, nd.z, nd.w, w.lane);
+        } else {
+            t0 = max(nd.x, w.lo), t1 = min(nd.y, w.hi);
+            if (t0 >= t1) continue;
+            below = __ldg(reinterpret_cast<const uint4*>(w.rows + (size_t)t0 * w.rw) + (kTrieDepth >> 2));
         }
         const W Eq = peq_load<W, trie_peq_row_bytes<W>()>(w.lane_addr, c);
         W P2 = Pv, M2 = Mv;
@@ -202,10 +232,9 @@ __device__ __forceinline__ void visit(Walk<W, COUNT>& w, const DistanceParams& P
             if (((uint32_t)D0 & w.dbit(LEVEL)) == 0u) ++dg2;
         }
         if constexpr (LEVEL < kTrieDepth) {
-            visit<W, LMAX, COUNT, LEVEL + 1>(w, P, nd.z, nd.w, P2, M2, dg2);
+            visit<W, LMAX, COUNT, LEVEL + 1>(w, P, nd.w, below, P2, M2, dg2);
         } else {
-            const uint32_t t0 = max(nd.x, w.lo), t1 = min(nd.y, w.hi);
-            if (t0 < t1) finish_texts<W, LMAX, COUNT>(w, P, t0, t1, P2, M2, dg2);
+            finish_texts<W, LMAX, COUNT>(w, P, t0, t1, below, P2, M2, dg2);
         }
     } while (U);
 }
@@ -228,6 +257,8 @@ __global__ void __launch_bounds__(kTrieThreads, sizeof(W) == 4 ? 4 : 2) k_distan
     Walk<W, COUNT> w;
     w.stage_addr = peq_addr + ((kPeqRows * kRowBytes + 15) & ~15);
     w.lane_addr = peq_addr + lane * (uint32_t)sizeof(W);
+    keep(w.stage_addr);
+    keep(w.lane_addr);
     w.lane = lane;
 
     const long long n_local = (P.n_items - P.shard + P.n_shards - 1) / P.n_shards;  // step 8(e): interleaved shards
@@ -261,6 +292,7 @@ __global__ void __launch_bounds__(kTrieThreads, sizeof(W) == 4 ? 4 : 2) k_distan
         w.lo = (uint32_t)(R.t_start + lo_rel);
         w.hi = (uint32_t)(R.t_start + hi_rel);
         w.dsh = (uint32_t)delta + 1u;
+        keep(w.dsh);
         {
             // one-hot codes of the pattern's first rows, shifted by delta: ohs[q] belongs to row q - delta
             const uint2 head = p_valid ? __ldg(reinterpret_cast<const uint2*>(prow)) : make_uint2(0xffffffffu, 0xffffffffu);
@@ -286,7 +318,8 @@ __global__ void __launch_bounds__(kTrieThreads, sizeof(W) == 4 ? 4 : 2) k_distan
             root_codes = __reduce_or_sync(kFull, root_codes);
         }
         // D[0][delta] = delta is the first cell of the final diagonal
-        visit<W, LMAX, COUNT, 1>(w, P, R.root_begin, root_codes, w.pv_init, W(0), p_valid ? delta : kDeadLane);
+        visit<W, LMAX, COUNT, 1>(w, P, root_codes, load_children<1>(P, R.root_begin, root_codes, lane), w.pv_init, W(0),
+                                 p_valid ? delta : kDeadLane);
     }
 
     if (COUNT) {

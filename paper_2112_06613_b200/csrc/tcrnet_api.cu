@@ -562,22 +562,30 @@ int tcrnet_load(tcrnet_ctx* ctx, const uint8_t* residues, const int32_t* lengths
     if (!ctx || !residues || !lengths || n < 1 || n > 0x7ffffffeLL) return TCRNET_ERR_ARG;
     TRY_CUDA(cudaSetDevice(ctx->device));
     drop_load(ctx);
-    // the host pass only sizes the copy; validation proper happens on the device
-    int64_t total_len = 0;
-    for (int64_t i = 0; i < n; ++i) {
-        if (lengths[i] < 1 || lengths[i] > kMaxLen) return TCRNET_ERR_LENGTH;
-        total_len += lengths[i];
-    }
+    // The lengths go first: their copy runs while the host pass below sizes the residue copy (validation proper
+    // happens on the device; this pass only keeps the sum meaningful).
     DevBuf& d_res = ctx->in_res;
     DevBuf& d_len = ctx->in_len;
-    int rc = dev_reserve(ctx, d_res, (size_t)total_len);
-    if (rc == TCRNET_OK) rc = dev_reserve(ctx, d_len, sizeof(int32_t) * (size_t)n);
+    cudaStream_t s = ctx->stream;
+    int rc = dev_reserve(ctx, d_len, sizeof(int32_t) * (size_t)n);
+    if (rc != TCRNET_OK) return rc;
+    TRY_CUDA(cudaEventRecord(ctx->ev[0], s));
+    TRY_CUDA(cudaMemcpyAsync(d_len.p, lengths, sizeof(int32_t) * (size_t)n, cudaMemcpyHostToDevice, s));
+    int64_t total_len = 0;
+    uint32_t bad = 0;
+    for (int64_t i = 0; i < n; ++i) {
+        const int32_t l = lengths[i];
+        bad |= (uint32_t)(l - 1) >= (uint32_t)kMaxLen;
+        total_len += l;
+    }
+    if (bad) {
+        cudaStreamSynchronize(s);  // the host array is borrowed for this call only
+        return TCRNET_ERR_LENGTH;
+    }
+    rc = dev_reserve(ctx, d_res, (size_t)total_len);
     int launches = 0;
     if (rc == TCRNET_OK) {
-        cudaStream_t s = ctx->stream;
-        cudaError_t e = cudaEventRecord(ctx->ev[0], s);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(d_res.p, residues, (size_t)total_len, cudaMemcpyHostToDevice, s);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(d_len.p, lengths, sizeof(int32_t) * (size_t)n, cudaMemcpyHostToDevice, s);
+        cudaError_t e = cudaMemcpyAsync(d_res.p, residues, (size_t)total_len, cudaMemcpyHostToDevice, s);
         if (e != cudaSuccess) {
             ctx->last_cuda = (int)e;
             (void)cudaGetLastError();
