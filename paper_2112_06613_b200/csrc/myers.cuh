@@ -198,10 +198,9 @@ __device__ __forceinline__ void emit_edges(const DistanceParams& P, bool edge, i
         base = __shfl_sync(0xffffffffu, base, 0);
         if (edge) {
             const unsigned long long pos = base + __popc(bal & ((1u << lane) - 1u));
-            if (pos < P.edge_cap) {
-                const uint32_t a = min(oi, oj), b = max(oi, oj);
-                P.edges[pos] = ((unsigned long long)a << 32) | b;
-            }
+            const uint32_t a = min(oi, oj), b = max(oi, oj);
+            atomicAdd(P.row_count + a, 1);
+            if (pos < P.edge_cap) P.edges[pos] = ((unsigned long long)a << 32) | b;
         }
     }
 }

@@ -331,6 +331,7 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
     HostCtrl* dc = d_ctrl(ctx);
     static_assert(offsetof(HostCtrl, queue) == offsetof(HostCtrl, edge_count) + 5 * sizeof(unsigned long long), "one memset");
     TRY_CUDA(cudaMemsetAsync(&dc->edge_count, 0, sizeof(unsigned long long) * (5 + kTrieQueues), s));  // edge_count, work[4], queue[]
+    TRY_CUDA(cudaMemsetAsync(ctx->row_count.p, 0, sizeof(int32_t) * (size_t)ctx->n, s));
     int n_queues = 0;
     const WorkRow* d_rows = (const WorkRow*)ctx->rows.p;
     for (const Schedule::Pass& pass : sch.passes) {
@@ -347,6 +348,7 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
         p.perm_t = (const int32_t*)pass.tset->perm.p;
         for (int k = 0; k <= kTrieDepth; ++k) p.trie[k] = pass.tset->trie_levels.p[k];
         p.edges = (unsigned long long*)ctx->keys_a.p;
+        p.row_count = (int32_t*)ctx->row_count.p;
         p.edge_count = &dc->edge_count;
         p.edge_cap = cap;
         p.work = dc->work;
@@ -397,6 +399,7 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
     cap = std::max<int64_t>(cap, 1);
     if (ctx->keys_a.p && (int64_t)(ctx->keys_a.bytes / 8) > cap) cap = std::min<int64_t>(ctx->keys_a.bytes / 8, ctx->edge_limit);
     TRY(dev_reserve(ctx, ctx->keys_a, sizeof(unsigned long long) * (size_t)cap));
+    TRY(dev_reserve(ctx, ctx->row_count, sizeof(int32_t) * (size_t)n));
     st.distance_passes = 1;
     TRY(run_distance(ctx, sch, l_max, first_check, (uint64_t)cap, shard, n_shards, launches));
     int64_t n_keys = (int64_t)ctx->h_ctrl->edge_count;
@@ -417,36 +420,34 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
     return TCRNET_OK;
 }
 
-// Step A6 on the n_keys keys (u << 32) | v in keys_a: LSD radix sort over the significant bits, CSR, degrees.
-int assemble_phase(tcrnet_ctx* ctx, int64_t n_keys, int* launches) {
+// Step A6 on the n_keys unsorted keys (u << 32) | v in keys_a: per-row counts (left in row_count by the emission
+// when counts_ready), prefix sum -> row_ptr, every edge into a slot of its row, rows ordered; degrees.
+int assemble_phase(tcrnet_ctx* ctx, int64_t n_keys, bool counts_ready, int* launches) {
     tcrnet_stats& st = ctx->stats;
     cudaStream_t s = ctx->stream;
     const int64_t n = ctx->n;
-    const unsigned long long* sorted = (const unsigned long long*)ctx->keys_a.p;
-    if (n_keys > 1) {
-        TRY(dev_reserve(ctx, ctx->keys_b, sizeof(unsigned long long) * (size_t)n_keys));
-        TRY(dev_reserve(ctx, ctx->radix_scratch, radix_scratch_bytes(n_keys)));
-        const int id_bits = bits_for(n - 1 > 0 ? n - 1 : 1);
-        int shifts[kRadixMaxPasses], n_passes = 0;
-        for (int half = 0; half < 2; ++half)
-            for (int sh = 0; sh < id_bits; sh += 8) shifts[n_passes++] = 32 * half + sh;
-        bool in_b = false;
-        TRY_CUDA(radix_sort_u64((unsigned long long*)ctx->keys_a.p, (unsigned long long*)ctx->keys_b.p, nullptr, nullptr,
-                                n_keys, shifts, n_passes, ctx->radix_scratch.p, s, launches, &in_b));
-        if (in_b) sorted = (const unsigned long long*)ctx->keys_b.p;
-    }
-    TRY_CUDA(cudaEventRecord(ctx->ev[2], s));
+    HostCtrl* dc = d_ctrl(ctx);
+    TRY(dev_reserve(ctx, ctx->row_count, sizeof(int32_t) * (size_t)n));
+    TRY(dev_reserve(ctx, ctx->long_rows, sizeof(int32_t) * (size_t)n));
+    TRY(dev_reserve(ctx, ctx->scan_scratch, scan_scratch_bytes(n)));
     TRY(dev_reserve(ctx, ctx->row_ptr, sizeof(int64_t) * (size_t)(n + 1)));
     TRY(dev_reserve(ctx, ctx->col, sizeof(int32_t) * (size_t)std::max<int64_t>(n_keys, 1)));
     TRY(dev_reserve(ctx, ctx->deg, sizeof(int32_t) * (size_t)n));
-    TRY_CUDA(launch_csr(sorted, n_keys, n, (int64_t*)ctx->row_ptr.p, (int32_t*)ctx->col.p, (int32_t*)ctx->deg.p, s, launches));
+    if (!counts_ready) {
+        TRY_CUDA(cudaMemsetAsync(ctx->row_count.p, 0, sizeof(int32_t) * (size_t)n, s));
+        TRY_CUDA(launch_count_rows((const unsigned long long*)ctx->keys_a.p, n_keys, (int32_t*)ctx->row_count.p, s, launches));
+    }
+    TRY_CUDA(cudaEventRecord(ctx->ev[2], s));
+    TRY_CUDA(launch_csr_unsorted((const unsigned long long*)ctx->keys_a.p, n_keys, n, (int32_t*)ctx->row_count.p,
+                                 (int64_t*)ctx->row_ptr.p, (int32_t*)ctx->col.p, (int32_t*)ctx->deg.p,
+                                 (int32_t*)ctx->long_rows.p, &dc->n_long, ctx->scan_scratch.p, s, launches));
     TRY_CUDA(cudaEventRecord(ctx->ev[3], s));
     TRY_CUDA(cudaEventSynchronize(ctx->ev[3]));
     TRY_CUDA(cudaEventElapsedTime(&st.ms_sort, ctx->ev[1], ctx->ev[2]));
     TRY_CUDA(cudaEventElapsedTime(&st.ms_csr, ctx->ev[2], ctx->ev[3]));
     st.n_edges = n_keys;
     ctx->n_edges = n_keys;
-    ctx->have_keys = false;  // the sort used keys_a
+    ctx->have_keys = false;
     ctx->have_dist = false;
     drop_observables(ctx);
     ctx->built = true;
@@ -531,7 +532,7 @@ void tcrnet_destroy(tcrnet_ctx* ctx) {
                       &ctx->query.txt, &ctx->query.trie, &ctx->inv_perm, &ctx->edge_dist, &ctx->edge_dist_b, &ctx->flags,
                       &ctx->flag_pos, &ctx->in_res, &ctx->in_len, &ctx->offsets,
                       &ctx->perm_tmp, &ctx->trie_scratch, &ctx->keys_a, &ctx->keys_b, &ctx->radix_scratch,
-                      &ctx->scan_scratch, &ctx->rows, &ctx->row_ptr, &ctx->col,
+                      &ctx->scan_scratch, &ctx->rows, &ctx->row_ptr, &ctx->col, &ctx->row_count, &ctx->long_rows,
                       &ctx->deg, &ctx->ctrl, &ctx->obs_ctrl, &ctx->deg_hist, &ctx->nn_sum, &ctx->class_sum, &ctx->knn,
                       &ctx->cc_parent, &ctx->cc_count, &ctx->cc_label, &ctx->cc_size, &ctx->perc_rank,
                       &ctx->perc_seen, &ctx->perc_deg, &ctx->perc_hist, &ctx->perc_lcc};
@@ -618,7 +619,7 @@ int tcrnet_build(tcrnet_ctx* ctx, int l_max, int64_t* n_edges_out) {
     drop_build(ctx);
     int launches = 0;
     TRY(distance_phase(ctx, l_max, 0, 1, &launches));
-    TRY(assemble_phase(ctx, ctx->n_keys, &launches));
+    TRY(assemble_phase(ctx, ctx->n_keys, true, &launches));
     tcrnet_stats& st = ctx->stats;
     TRY_CUDA(cudaEventElapsedTime(&st.ms_distance, ctx->ev[0], ctx->ev[1]));
     TRY_CUDA(cudaEventElapsedTime(&st.ms_build, ctx->ev[0], ctx->ev[3]));
@@ -678,7 +679,7 @@ int tcrnet_assemble(tcrnet_ctx* ctx, const uint64_t* keys_dev, int64_t n_keys, i
     TRY_CUDA(cudaEventRecord(ctx->ev[1], s));
     TRY_CUDA(cudaStreamSynchronize(s));
     if (ctx->h_ctrl->flags) return TCRNET_ERR_ARG;
-    TRY(assemble_phase(ctx, n_keys, &launches));
+    TRY(assemble_phase(ctx, n_keys, false, &launches));
     ctx->stats.launches_build = launches;
     TRY_CUDA(cudaEventElapsedTime(&ctx->stats.ms_build, ctx->ev[1], ctx->ev[3]));
     if (n_edges_out) *n_edges_out = ctx->n_edges;

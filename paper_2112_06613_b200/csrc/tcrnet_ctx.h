@@ -19,7 +19,7 @@ struct HostCtrl {  // pinned mirror of the small device control block
     unsigned long long queue[kTrieQueues];  // dynamic work queues of the trie launches (zeroed with edge_count)
     unsigned long long probe[3];
     uint32_t flags;
-    uint32_t pad_;
+    uint32_t n_long;                  // rows queued for k_sort_long_rows
     uint32_t trie_counts[8];          // [k] = nodes of trie level k
     uint32_t trie_root[kNumLen + 1];  // [L] = first level-1 node of length bucket L (non-empty buckets)
 };
@@ -70,7 +70,7 @@ struct tcrnet_ctx {
     bool have_dist = false;  // edge_dist valid for the current CSR
     int built_l_max = 0;
     int64_t n_edges = 0, n_keys = 0;
-    DevBuf keys_a, keys_b, radix_scratch, scan_scratch, rows, row_ptr, col, deg;
+    DevBuf keys_a, keys_b, radix_scratch, scan_scratch, rows, row_ptr, col, deg, row_count, long_rows;
     DevBuf inv_perm, edge_dist, edge_dist_b, flags, flag_pos;
 
     // observables state (observables_api.cu); valid for the current CSR only

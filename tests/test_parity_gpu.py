@@ -183,6 +183,18 @@ def test_all_duplicates_complete_graph(pkg, oracle):
         check_csr_invariants(*got, r)
 
 
+def test_rows_of_every_sorting_regime(pkg, oracle):
+    """The CSR step orders a row by one thread (<= 32 neighbours), in shared memory (<= 8192) or in place
+    (beyond): a clique of 9,001 copies has rows of every such length; the other strings hang off it."""
+    strings = ["CASSLGQF"] * 5000 + ["CASSLGQW", "CASRLGQF", "CWWWWWWW"] + ["CASSLGQF"] * 4001 + ["CASSLGF"] * 40
+    res, ln = from_strings(strings)
+    got, _ = gpu_network(pkg, res, ln, 1)
+    want = oracle.network(res, ln, 1, tier=1)[:3]
+    assert_same_network(got, want)
+    check_csr_invariants(*got, len(strings))
+    assert int(np.diff(got[0]).max()) > 8192
+
+
 def test_lmax_at_least_max_length_gives_complete_graph(pkg, oracle):
     d = generate("cfg1", n=300)
     got, _ = gpu_network(pkg, d.residues, d.lengths, 25)
