@@ -44,74 +44,82 @@ __global__ void __launch_bounds__(256) k_col_deg_lower(const unsigned long long*
 
 // ---- unsorted keys -> CSR without a global sort (the path of tcrnet_build / tcrnet_assemble) ----
 //
-// The edges of a row are few (a handful at TCR scale), so the CSR is built the way a CSR is defined: count the
-// edges of every row (done by the emission itself, or by k_count_rows for caller-supplied keys), prefix-sum the
-// counts into row_ptr, drop every edge into a free slot of its row, then order each row.  Per edge: 8 B read,
-// 4 B written, two L2 atomics; per node 12 B + the scan.  The result is the same CSR a global sort of the keys
-// yields (rows ascending by construction, neighbours ascending after the row sorts).
-constexpr int kShortRow = 32;    // rows up to this many neighbours: insertion sort by one thread
+// The edges of a row are few (a handful at TCR scale), so the CSR is built the way a CSR is defined.  The
+// emission (or k_count_rows for caller-supplied keys) counts, for every edge (u, v), row_count[u]++ and
+// deg[v]++ (fire-and-forget L2 reductions); then
+//   row_ptr   = exclusive prefix sum of row_count                                   (scan.cu)
+//   k_scatter_keys   every key into a free slot of its row: bucket[row_ptr[u] + --row_count[u]] = key
+//   k_rank_rows      one thread per slot: col[row_ptr[u] + #{w in row u : w < v}] = v for rows of <= kRankRow
+//                    neighbours (equal keys of a caller's list: ties broken by slot); coalesced, the row is
+//                    read from L1.  The thread of slot 0 adds the row length to deg[u] and queues longer rows
+//   k_sort_long_rows one CTA per queued row: bitonic network in shared memory (<= kSmemRow) or in place.
+// Per edge: 8 B read + 8 B written at random (scatter), 8 B read + 4 B written in order (rank), two L2
+// reductions and one L2 atomic; per node 12 B + the scan.  All of it is L2-resident at TCR scale.  The result
+// is the CSR a global sort of the keys yields (rows ascending by construction, neighbours by rank).
+constexpr int kRankRow = 64;     // rows up to this many neighbours are ordered by ranking, one thread per edge
 constexpr int kSmemRow = 8192;   // longer rows up to this many: bitonic network in shared memory; beyond: in place
 
 __global__ void __launch_bounds__(256) k_count_rows(const unsigned long long* __restrict__ keys, int64_t n_keys,
-                                                   int32_t* __restrict__ row_count) {
-    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_keys; e += (int64_t)gridDim.x * blockDim.x)
-        atomicAdd(&row_count[keys[e] >> 32], 1);
-}
-
-// row_count[u] = edges of row u not yet placed: the cursor counts down to 0
-__global__ void __launch_bounds__(256) k_scatter_cols(const unsigned long long* __restrict__ keys, int64_t n_keys,
-                                                     const int64_t* __restrict__ row_ptr, int32_t* __restrict__ row_count,
-                                                     int32_t* __restrict__ col, int32_t* __restrict__ deg) {
+                                                   int32_t* __restrict__ row_count, int32_t* __restrict__ deg) {
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_keys; e += (int64_t)gridDim.x * blockDim.x) {
         const unsigned long long k = keys[e];
-        const uint32_t u = (uint32_t)(k >> 32), v = (uint32_t)k;
-        const int32_t slot = atomicSub(&row_count[u], 1) - 1;
-        col[row_ptr[u] + slot] = (int32_t)v;
-        atomicAdd(&deg[v], 1);
+        atomicAdd(&row_count[k >> 32], 1);
+        atomicAdd(&deg[(uint32_t)k], 1);
     }
 }
 
-// deg[u] += neighbours above u; short rows are ordered here, long ones are queued for k_sort_long_rows
-__global__ void __launch_bounds__(256) k_sort_rows(const int64_t* __restrict__ row_ptr, int64_t n, int32_t* __restrict__ col,
+// row_count[u] = edges of row u not yet placed: counts down to 0
+__global__ void __launch_bounds__(256) k_scatter_keys(const unsigned long long* __restrict__ keys, int64_t n_keys,
+                                                     const int64_t* __restrict__ row_ptr, int32_t* __restrict__ row_count,
+                                                     unsigned long long* __restrict__ bucket) {
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_keys; e += (int64_t)gridDim.x * blockDim.x) {
+        const unsigned long long k = keys[e];
+        const uint32_t u = (uint32_t)(k >> 32);
+        const int32_t slot = atomicSub(&row_count[u], 1) - 1;
+        bucket[row_ptr[u] + slot] = k;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_rank_rows(const unsigned long long* __restrict__ bucket, int64_t n_keys,
+                                                  const int64_t* __restrict__ row_ptr, int32_t* __restrict__ col,
                                                   int32_t* __restrict__ deg, int32_t* __restrict__ long_rows,
                                                   uint32_t* __restrict__ n_long) {
-    const int64_t u = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (u >= n) return;
+    const int64_t pos = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (pos >= n_keys) return;
+    const unsigned long long k = bucket[pos];
+    const uint32_t u = (uint32_t)(k >> 32), v = (uint32_t)k;
     const int64_t b = row_ptr[u];
-    const int64_t len = row_ptr[u + 1] - b;
-    deg[u] += (int32_t)len;
-    if (len <= 1) return;
-    if (len > kShortRow) {
-        long_rows[atomicAdd(n_long, 1u)] = (int32_t)u;
-        return;
+    const int len = (int)(row_ptr[u + 1] - b);
+    const int my = (int)(pos - b);
+    if (my == 0) {
+        deg[u] += len;  // the neighbours above u (those below were counted by the emission)
+        if (len > kRankRow) long_rows[atomicAdd(n_long, 1u)] = (int32_t)u;
     }
-    int32_t* a = col + b;
-    for (int i = 1; i < (int)len; ++i) {
-        const int32_t x = a[i];
-        int j = i;
-        while (j > 0 && a[j - 1] > x) {
-            a[j] = a[j - 1];
-            --j;
-        }
-        a[j] = x;
+    if (len > kRankRow) return;
+    const unsigned long long* a = bucket + b;
+    int rank = 0;
+    for (int i = 0; i < len; ++i) {
+        const uint32_t x = (uint32_t)a[i];
+        rank += (x < v) || (x == v && i < my);
     }
+    col[b + rank] = (int32_t)v;
 }
 
 // One CTA per queued row: ascending bitonic network over the next power of two, the missing tail being virtual
 // +infinity entries (every exchange puts the smaller value at the smaller index, so they never move).
-__global__ void __launch_bounds__(256) k_sort_long_rows(const int64_t* __restrict__ row_ptr, int32_t* __restrict__ col,
-                                                       const int32_t* __restrict__ long_rows,
+__global__ void __launch_bounds__(256) k_sort_long_rows(const int64_t* __restrict__ row_ptr,
+                                                       const unsigned long long* __restrict__ bucket,
+                                                       int32_t* __restrict__ col, const int32_t* __restrict__ long_rows,
                                                        const uint32_t* __restrict__ n_long) {
     __shared__ int32_t buf[kSmemRow];
     const uint32_t rows = *n_long;
     for (uint32_t r = blockIdx.x; r < rows; r += gridDim.x) {
         const int64_t u = long_rows[r];
-        int32_t* g = col + row_ptr[u];
-        const int64_t len = row_ptr[u + 1] - row_ptr[u];
+        const int64_t b = row_ptr[u];
+        const int64_t len = row_ptr[u + 1] - b;
         const bool in_smem = len <= kSmemRow;
-        int32_t* a = in_smem ? buf : g;
-        if (in_smem)
-            for (int64_t i = threadIdx.x; i < len; i += blockDim.x) buf[i] = g[i];
+        int32_t* a = in_smem ? buf : col + b;
+        for (int64_t i = threadIdx.x; i < len; i += blockDim.x) a[i] = (int32_t)(uint32_t)bucket[b + i];
         __syncthreads();
         int64_t p2 = 1;
         while (p2 < len) p2 <<= 1;
@@ -134,37 +142,34 @@ __global__ void __launch_bounds__(256) k_sort_long_rows(const int64_t* __restric
             }
         }
         if (in_smem)
-            for (int64_t i = threadIdx.x; i < len; i += blockDim.x) g[i] = buf[i];
+            for (int64_t i = threadIdx.x; i < len; i += blockDim.x) col[b + i] = buf[i];
         __syncthreads();
     }
 }
 
 }  // namespace
 
-cudaError_t launch_count_rows(const unsigned long long* keys, int64_t n_keys, int32_t* row_count, cudaStream_t s,
-                              int* launches) {
+cudaError_t launch_count_rows(const unsigned long long* keys, int64_t n_keys, int32_t* row_count, int32_t* deg,
+                              cudaStream_t s, int* launches) {
     if (n_keys <= 0) return cudaSuccess;
     const int64_t blocks = std::min<int64_t>((n_keys + 255) / 256, 148 * 16);
-    k_count_rows<<<(unsigned)blocks, 256, 0, s>>>(keys, n_keys, row_count);
+    k_count_rows<<<(unsigned)blocks, 256, 0, s>>>(keys, n_keys, row_count, deg);
     *launches += 1;
     return cudaGetLastError();
 }
 
 cudaError_t launch_csr_unsorted(const unsigned long long* keys, int64_t n_keys, int64_t n, int32_t* row_count,
-                                int64_t* row_ptr, int32_t* col, int32_t* deg, int32_t* long_rows, uint32_t* n_long,
-                                void* scan_scratch, cudaStream_t s, int* launches) {
+                                int64_t* row_ptr, unsigned long long* bucket, int32_t* col, int32_t* deg,
+                                int32_t* long_rows, uint32_t* n_long, void* scan_scratch, cudaStream_t s,
+                                int* launches) {
     cudaError_t e = exclusive_scan_i32_to_i64(row_count, row_ptr, n, true, scan_scratch, s, launches);
-    if (e == cudaSuccess) e = cudaMemsetAsync(deg, 0, sizeof(int32_t) * (size_t)n, s);
     if (e == cudaSuccess) e = cudaMemsetAsync(n_long, 0, sizeof(uint32_t), s);
-    if (e != cudaSuccess) return e;
-    if (n_keys > 0) {
-        const int64_t blocks = std::min<int64_t>((n_keys + 255) / 256, 148 * 16);
-        k_scatter_cols<<<(unsigned)blocks, 256, 0, s>>>(keys, n_keys, row_ptr, row_count, col, deg);
-        *launches += 1;
-    }
-    k_sort_rows<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(row_ptr, n, col, deg, long_rows, n_long);
-    k_sort_long_rows<<<(unsigned)std::min<int64_t>(n, 148 * 4), 256, 0, s>>>(row_ptr, col, long_rows, n_long);
-    *launches += 2;
+    if (e != cudaSuccess || n_keys <= 0) return e;
+    const int64_t blocks = (n_keys + 255) / 256;
+    k_scatter_keys<<<(unsigned)std::min<int64_t>(blocks, 148 * 32), 256, 0, s>>>(keys, n_keys, row_ptr, row_count, bucket);
+    k_rank_rows<<<(unsigned)blocks, 256, 0, s>>>(bucket, n_keys, row_ptr, col, deg, long_rows, n_long);
+    k_sort_long_rows<<<(unsigned)std::min<int64_t>(n, 148 * 4), 256, 0, s>>>(row_ptr, bucket, col, long_rows, n_long);
+    *launches += 3;
     return cudaGetLastError();
 }
 

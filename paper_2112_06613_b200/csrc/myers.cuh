@@ -200,6 +200,7 @@ __device__ __forceinline__ void emit_edges(const DistanceParams& P, bool edge, i
             const unsigned long long pos = base + __popc(bal & ((1u << lane) - 1u));
             const uint32_t a = min(oi, oj), b = max(oi, oj);
             atomicAdd(P.row_count + a, 1);
+            atomicAdd(P.deg + b, 1);
             if (pos < P.edge_cap) P.edges[pos] = ((unsigned long long)a << 32) | b;
         }
     }

@@ -332,6 +332,7 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
     static_assert(offsetof(HostCtrl, queue) == offsetof(HostCtrl, edge_count) + 5 * sizeof(unsigned long long), "one memset");
     TRY_CUDA(cudaMemsetAsync(&dc->edge_count, 0, sizeof(unsigned long long) * (5 + kTrieQueues), s));  // edge_count, work[4], queue[]
     TRY_CUDA(cudaMemsetAsync(ctx->row_count.p, 0, sizeof(int32_t) * (size_t)ctx->n, s));
+    TRY_CUDA(cudaMemsetAsync(ctx->deg.p, 0, sizeof(int32_t) * (size_t)ctx->n, s));
     int n_queues = 0;
     const WorkRow* d_rows = (const WorkRow*)ctx->rows.p;
     for (const Schedule::Pass& pass : sch.passes) {
@@ -349,6 +350,7 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
         for (int k = 0; k <= kTrieDepth; ++k) p.trie[k] = pass.tset->trie_levels.p[k];
         p.edges = (unsigned long long*)ctx->keys_a.p;
         p.row_count = (int32_t*)ctx->row_count.p;
+        p.deg = (int32_t*)ctx->deg.p;
         p.edge_count = &dc->edge_count;
         p.edge_cap = cap;
         p.work = dc->work;
@@ -400,6 +402,7 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
     if (ctx->keys_a.p && (int64_t)(ctx->keys_a.bytes / 8) > cap) cap = std::min<int64_t>(ctx->keys_a.bytes / 8, ctx->edge_limit);
     TRY(dev_reserve(ctx, ctx->keys_a, sizeof(unsigned long long) * (size_t)cap));
     TRY(dev_reserve(ctx, ctx->row_count, sizeof(int32_t) * (size_t)n));
+    TRY(dev_reserve(ctx, ctx->deg, sizeof(int32_t) * (size_t)n));
     st.distance_passes = 1;
     TRY(run_distance(ctx, sch, l_max, first_check, (uint64_t)cap, shard, n_shards, launches));
     int64_t n_keys = (int64_t)ctx->h_ctrl->edge_count;
@@ -433,14 +436,18 @@ int assemble_phase(tcrnet_ctx* ctx, int64_t n_keys, bool counts_ready, int* laun
     TRY(dev_reserve(ctx, ctx->row_ptr, sizeof(int64_t) * (size_t)(n + 1)));
     TRY(dev_reserve(ctx, ctx->col, sizeof(int32_t) * (size_t)std::max<int64_t>(n_keys, 1)));
     TRY(dev_reserve(ctx, ctx->deg, sizeof(int32_t) * (size_t)n));
+    TRY(dev_reserve(ctx, ctx->keys_b, sizeof(unsigned long long) * (size_t)std::max<int64_t>(n_keys, 1)));
     if (!counts_ready) {
         TRY_CUDA(cudaMemsetAsync(ctx->row_count.p, 0, sizeof(int32_t) * (size_t)n, s));
-        TRY_CUDA(launch_count_rows((const unsigned long long*)ctx->keys_a.p, n_keys, (int32_t*)ctx->row_count.p, s, launches));
+        TRY_CUDA(cudaMemsetAsync(ctx->deg.p, 0, sizeof(int32_t) * (size_t)n, s));
+        TRY_CUDA(launch_count_rows((const unsigned long long*)ctx->keys_a.p, n_keys, (int32_t*)ctx->row_count.p,
+                                   (int32_t*)ctx->deg.p, s, launches));
     }
     TRY_CUDA(cudaEventRecord(ctx->ev[2], s));
     TRY_CUDA(launch_csr_unsorted((const unsigned long long*)ctx->keys_a.p, n_keys, n, (int32_t*)ctx->row_count.p,
-                                 (int64_t*)ctx->row_ptr.p, (int32_t*)ctx->col.p, (int32_t*)ctx->deg.p,
-                                 (int32_t*)ctx->long_rows.p, &dc->n_long, ctx->scan_scratch.p, s, launches));
+                                 (int64_t*)ctx->row_ptr.p, (unsigned long long*)ctx->keys_b.p, (int32_t*)ctx->col.p,
+                                 (int32_t*)ctx->deg.p, (int32_t*)ctx->long_rows.p, &dc->n_long, ctx->scan_scratch.p, s,
+                                 launches));
     TRY_CUDA(cudaEventRecord(ctx->ev[3], s));
     TRY_CUDA(cudaEventSynchronize(ctx->ev[3]));
     TRY_CUDA(cudaEventElapsedTime(&st.ms_sort, ctx->ev[1], ctx->ev[2]));

@@ -88,6 +88,7 @@ struct DistanceParams {
     const int32_t* perm_t; // ... text set
     unsigned long long* edges;       // keys (min(i,j) << 32) | max(i,j)
     int32_t* row_count;              // [n]: += 1 at the smaller endpoint of every emitted edge (input of the CSR step)
+    int32_t* deg;                    // [n]: += 1 at the larger endpoint
     unsigned long long* edge_count;  // device counter (keeps counting beyond capacity)
     unsigned long long edge_cap;
     unsigned long long* work;        // [4]: lane-columns, lane-tests (exit votes), lane-first-columns,
@@ -168,14 +169,16 @@ cudaError_t launch_validate_keys(const unsigned long long* keys, int64_t n_keys,
                                  cudaStream_t s, int* launches);
 
 // csr.cu
-// row_count[u] += number of keys whose first index is u
-cudaError_t launch_count_rows(const unsigned long long* keys, int64_t n_keys, int32_t* row_count, cudaStream_t s,
-                              int* launches);
-// CSR + degrees from UNSORTED keys whose per-row counts are in row_count (consumed: all zero afterwards).
+// counts of caller-supplied keys: row_count[u]++, deg[v]++ (both zeroed by the caller)
+cudaError_t launch_count_rows(const unsigned long long* keys, int64_t n_keys, int32_t* row_count, int32_t* deg,
+                              cudaStream_t s, int* launches);
+// CSR + degrees from UNSORTED keys whose counts are in row_count[u] (edges of row u; consumed: all zero
+// afterwards) and deg[v] (edges whose larger endpoint is v).  bucket: uint64[n_keys] scratch,
 // long_rows: int32[n] scratch, n_long: device counter, scan_scratch: scan_scratch_bytes(n).
 cudaError_t launch_csr_unsorted(const unsigned long long* keys, int64_t n_keys, int64_t n, int32_t* row_count,
-                                int64_t* row_ptr, int32_t* col, int32_t* deg, int32_t* long_rows, uint32_t* n_long,
-                                void* scan_scratch, cudaStream_t s, int* launches);
+                                int64_t* row_ptr, unsigned long long* bucket, int32_t* col, int32_t* deg,
+                                int32_t* long_rows, uint32_t* n_long, void* scan_scratch, cudaStream_t s,
+                                int* launches);
 // the same from keys that are already sorted (tcrnet_restrict)
 cudaError_t launch_csr(const unsigned long long* sorted_keys, int64_t n_edges, int64_t n, int64_t* row_ptr,
                        int32_t* col, int32_t* deg, cudaStream_t s, int* launches);
