@@ -100,7 +100,7 @@ typedef enum tcrnet_option {
                                      result.                                                   */
     TCRNET_OPT_TRIE_CHUNK = 8,    /* texts per work item of the prefix-trie kernel (multiple of
                                      256; default 1048576)                                    */
-    TCRNET_OPT_N_QUERY = 9        /* rectangular (query x repertoire) mode: the
+    TCRNET_OPT_N_QUERY = 9,       /* rectangular (query x repertoire) mode: the
                                      antigen-specific network "replaces the first N_a rows" by
                                      antigen-cognate sequences and analyses only those nodes.
                                      n_q > 0: rows 0..n_q-1 of the next tcrnet_load are the query
@@ -108,6 +108,13 @@ typedef enum tcrnet_option {
                                      endpoint (query-query and query-repertoire); pairs of two
                                      non-query rows are never evaluated.  0 (default): all pairs.
                                      Takes effect at the next tcrnet_load.                      */
+    TCRNET_OPT_DEDUP = 10         /* 1 (default): rows with identical sequences are collapsed at
+                                     load; the distance step runs over the distinct sequences and
+                                     the emission multiplies every surviving pair by the rows
+                                     behind it (reading Q3: one node per row, duplicates joined
+                                     for every l_max >= 0).  0: every row is its own pattern /
+                                     text.  Never changes the result.  Ignored (off) in the
+                                     rectangular mode.  Takes effect at the next load.          */
 } tcrnet_option;
 
 /* Work and timing of the last tcrnet_load / tcrnet_build (tcrnet_get_stats). */
@@ -135,9 +142,11 @@ typedef struct tcrnet_stats {
     int32_t launches_build;    /* kernels launched by the last tcrnet_build                   */
     float ms_load;             /* device time of the last load (H2D copy + pack), CUDA events */
     float ms_distance;         /* distance kernel(s) incl. emission                           */
-    float ms_sort;             /* radix sort of the edge keys                                 */
+    float ms_sort;             /* counting of caller-supplied keys (tcrnet_assemble), else ~0  */
     float ms_csr;              /* row_ptr / col / degrees                                     */
     float ms_build;            /* whole tcrnet_build on the device                            */
+    int64_t n_distinct;        /* distinct sequences among the rows (= n when TCRNET_OPT_DEDUP
+                                  is off or in the rectangular mode)                         */
 } tcrnet_stats;
 
 /*

@@ -21,7 +21,7 @@ LIB_PATH = os.path.join(_HERE, "libtcrnet_b200.so")
 OK, ERR_ARG, ERR_LENGTH, ERR_RESIDUE, ERR_LMAX, ERR_STATE, ERR_NOMEM, ERR_EDGE_OVERFLOW, ERR_CUDA = (
     0, -1, -2, -3, -4, -5, -6, -7, -8)
 OPT_EARLY_EXIT, OPT_FIRST_CHECK, OPT_EDGE_CAPACITY, OPT_EDGE_LIMIT, OPT_COUNT_WORK, OPT_TEXT_CHUNK = 1, 2, 3, 4, 5, 6
-OPT_PREFIX_TRIE, OPT_TRIE_CHUNK, OPT_N_QUERY = 7, 8, 9
+OPT_PREFIX_TRIE, OPT_TRIE_CHUNK, OPT_N_QUERY, OPT_DEDUP = 7, 8, 9, 10
 
 EXPORTS = (
     "tcrnet_create", "tcrnet_destroy", "tcrnet_load", "tcrnet_load_device", "tcrnet_build", "tcrnet_csr",
@@ -48,6 +48,7 @@ class tcrnet_stats(C.Structure):
         ("work_items_trie", C.c_int64), ("trie_nodes", C.c_int64), ("distance_passes", C.c_int32),
         ("launches_load", C.c_int32), ("launches_build", C.c_int32), ("ms_load", C.c_float),
         ("ms_distance", C.c_float), ("ms_sort", C.c_float), ("ms_csr", C.c_float), ("ms_build", C.c_float),
+        ("n_distinct", C.c_int64),
     ]
 
 

@@ -1,0 +1,343 @@
+// Step A0 (before the pack): rows with identical sequences are collapsed.
+//
+// Reading Q3 keeps one node per input row, and repertoires are full of repeated CDR3
+// sequences (public clones).  Identical rows have identical distances to everything,
+// so the all-pairs step runs over the DISTINCT sequences only and the emission multiplies a surviving
+// pair of distinct sequences by the rows behind them (myers.cuh emit_edges); the rows of one sequence
+// are joined to each other directly (k_emit_cliques: d = 0 <= l_max for every l_max).  Nothing about
+// the result changes - only the number of pairs the distance kernel has to decide.
+//
+//   k_dedup_insert   open-addressing table, one 64-bit word per slot = (fingerprint << 32) | smallest row
+//                    seen with that fingerprint: atomicCAS on the empty slot, atomicMin afterwards
+//   k_dedup_lookup   every row finds its slot again, compares its bytes with the slot's row and becomes a
+//                    duplicate of it, or (first row of its sequence, fingerprint clash, invalid row) stays
+//   scan             ids of the distinct sequences in input-row order (deterministic)
+//   k_dedup_groups   uid of every row, rows per uid, length / residue offset of every uid
+//   scan + k_dedup_fill   the rows of every uid, contiguous (order inside a group is irrelevant)
+// Rows with an invalid length or out-of-range offset are never read and never merged; the pack step
+// reports them.  HBM/L2-bound: ~100 B per row over all kernels.
+#include "tcrnet_internal.h"
+
+namespace tcrnet {
+namespace {
+
+constexpr unsigned long long kEmptySlot = ~0ull;
+
+__device__ __forceinline__ bool row_ok(int64_t off, int32_t len, int64_t total_len) {
+    return len >= 1 && len <= kMaxLen && off >= 0 && off + len <= total_len;
+}
+
+__device__ __forceinline__ unsigned long long hash_row(const uint8_t* src, int len) {
+    unsigned long long h = 0xcbf29ce484222325ull ^ (unsigned long long)len;
+    for (int i = 0; i < len; ++i) h = (h ^ src[i]) * 0x100000001b3ull;  // FNV-1a
+    h ^= h >> 33;                                                      // + a finaliser for the high bits
+    h *= 0xff51afd7ed558ccdull;
+    h ^= h >> 33;
+    return h;
+}
+
+__global__ void __launch_bounds__(256) k_dedup_insert(const uint8_t* __restrict__ residues,
+                                                     const int64_t* __restrict__ offsets,
+                                                     const int32_t* __restrict__ lengths, int64_t n, int64_t total_len,
+                                                     unsigned long long* __restrict__ table, uint32_t mask,
+                                                     unsigned long long* __restrict__ hash) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int64_t off = offsets[i];
+    const int32_t len = lengths[i];
+    if (!row_ok(off, len, total_len)) {
+        hash[i] = kEmptySlot;  // never merged
+        return;
+    }
+    unsigned long long h = hash_row(residues + off, len);
+    if (h == kEmptySlot) h = 0;
+    hash[i] = h;
+    const unsigned long long fp = h & 0xffffffff00000000ull;
+    const unsigned long long mine = fp | (unsigned long long)i;
+    uint32_t s = (uint32_t)h & mask;
+    for (;;) {
+        unsigned long long cur = table[s];
+        if (cur == kEmptySlot) {
+            cur = atomicCAS(&table[s], kEmptySlot, mine);
+            if (cur == kEmptySlot) return;
+        }
+        if ((cur & 0xffffffff00000000ull) == fp) {
+            atomicMin(&table[s], mine);
+            return;
+        }
+        s = (s + 1u) & mask;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_dedup_lookup(const uint8_t* __restrict__ residues,
+                                                     const int64_t* __restrict__ offsets,
+                                                     const int32_t* __restrict__ lengths, int64_t n,
+                                                     const unsigned long long* __restrict__ table, uint32_t mask,
+                                                     const unsigned long long* __restrict__ hash,
+                                                     int32_t* __restrict__ rep_of, uint32_t* __restrict__ is_first) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const unsigned long long h = hash[i];
+    int64_t rep = i;
+    if (h != kEmptySlot) {
+        const unsigned long long fp = h & 0xffffffff00000000ull;
+        uint32_t s = (uint32_t)h & mask;
+        for (;;) {
+            const unsigned long long cur = table[s];
+            if ((cur & 0xffffffff00000000ull) == fp && cur != kEmptySlot) {
+                rep = (int64_t)(cur & 0xffffffffull);
+                break;
+            }
+            s = (s + 1u) & mask;
+        }
+        if (rep != i) {
+            const int32_t len = lengths[i];
+            bool same = lengths[rep] == len;
+            if (same) {
+                const uint8_t* a = residues + offsets[i];
+                const uint8_t* b = residues + offsets[rep];
+                for (int k = 0; k < len; ++k) same = same && a[k] == b[k];
+            }
+            if (!same) rep = i;  // fingerprint clash: stays a sequence of its own
+        }
+    }
+    rep_of[i] = (int32_t)rep;
+    is_first[i] = rep == i ? 1u : 0u;
+}
+
+__global__ void __launch_bounds__(256) k_dedup_groups(const int32_t* __restrict__ rep_of,
+                                                     const uint32_t* __restrict__ first_rank,
+                                                     const int64_t* __restrict__ offsets,
+                                                     const int32_t* __restrict__ lengths, int64_t n,
+                                                     int32_t* __restrict__ uid_of, uint32_t* __restrict__ group_count,
+                                                     int32_t* __restrict__ len_u, int64_t* __restrict__ off_u) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int32_t rep = rep_of[i];
+    const uint32_t uid = first_rank[rep];
+    uid_of[i] = (int32_t)uid;
+    atomicAdd(&group_count[uid], 1u);
+    if (rep == i) {
+        len_u[uid] = lengths[i];
+        off_u[uid] = offsets[i];
+    }
+}
+
+// group_count[uid] counts down to 0 while the rows take their places
+__global__ void __launch_bounds__(256) k_dedup_fill(const int32_t* __restrict__ uid_of, int64_t n,
+                                                   const uint32_t* __restrict__ group_start,
+                                                   uint32_t* __restrict__ group_count, int32_t* __restrict__ members) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t uid = (uint32_t)uid_of[i];
+    const uint32_t slot = atomicSub(&group_count[uid], 1u) - 1u;
+    members[group_start[uid] + slot] = (int32_t)i;
+}
+
+// perm[sorted position] = uid  ->  the row itself when it is alone, else kGroupFlag | uid
+__global__ void __launch_bounds__(256) k_dedup_codes(int32_t* __restrict__ perm, int64_t n_u,
+                                                    const uint32_t* __restrict__ group_start,
+                                                    const int32_t* __restrict__ members) {
+    const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n_u) return;
+    const uint32_t uid = (uint32_t)perm[s];
+    const uint32_t b = group_start[uid];
+    perm[s] = group_start[uid + 1] - b == 1u ? members[b] : (int32_t)(kGroupFlag | uid);
+}
+
+// Edges between the rows of one sequence: the thread of member slot x joins it to the slots after it.  Output
+// offsets: warp scan + one atomicAdd per warp.
+__global__ void __launch_bounds__(256) k_emit_cliques(const int32_t* __restrict__ members,
+                                                     const int32_t* __restrict__ uid_of,
+                                                     const uint32_t* __restrict__ group_start, int64_t n,
+                                                     unsigned long long* __restrict__ edges,
+                                                     unsigned long long* __restrict__ edge_count,
+                                                     unsigned long long edge_cap, int32_t* __restrict__ row_count,
+                                                     int32_t* __restrict__ deg) {
+    constexpr uint32_t kFullMask = 0xffffffffu;
+    const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    uint32_t r = 0, end = 0, rest = 0;
+    if (s < n) {
+        r = (uint32_t)members[s];
+        end = group_start[(uint32_t)uid_of[r] + 1u];
+        rest = end - 1u - (uint32_t)s;  // slots after this one
+    }
+    if (!__any_sync(kFullMask, rest != 0u)) return;
+    unsigned long long incl = rest;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned long long v = __shfl_up_sync(kFullMask, incl, o);
+        if (lane >= o) incl += v;
+    }
+    unsigned long long base = 0;
+    if (lane == 31) base = atomicAdd(edge_count, incl);
+    unsigned long long pos = __shfl_sync(kFullMask, base, 31) + incl - rest;
+    for (uint32_t y = (uint32_t)s + 1u; y < end; ++y, ++pos) {
+        const uint32_t q = (uint32_t)members[y];
+        const uint32_t a = min(r, q), b = max(r, q);
+        atomicAdd(row_count + a, 1);
+        atomicAdd(deg + b, 1);
+        if (pos < edge_cap) edges[pos] = ((unsigned long long)a << 32) | b;
+    }
+}
+
+// The pairs of distinct sequences the distance kernel recorded (codes: a row, or kGroupFlag | uid) -> the edges
+// between the rows behind them, counted for the CSR step.  One warp handles 32 entries: the output offsets are
+// a warp scan + one atomicAdd; a lane writes up to kOwn edges itself, larger products are shared by the warp.
+__global__ void __launch_bounds__(256) k_expand_entries(const unsigned long long* __restrict__ entries,
+                                                       const unsigned long long* __restrict__ n_entries_dev,
+                                                       unsigned long long entry_cap,
+                                                       const uint32_t* __restrict__ group_start,
+                                                       const int32_t* __restrict__ members,
+                                                       unsigned long long* __restrict__ edges,
+                                                       unsigned long long* __restrict__ edge_total,
+                                                       unsigned long long edge_cap, int32_t* __restrict__ row_count,
+                                                       int32_t* __restrict__ deg) {
+    constexpr uint32_t kFullMask = 0xffffffffu;
+    constexpr unsigned long long kOwn = 8;
+    const unsigned long long n_ent = min(*n_entries_dev, entry_cap);
+    const int lane = threadIdx.x & 31;
+    const unsigned long long warps = ((unsigned long long)gridDim.x * blockDim.x) >> 5;
+    for (unsigned long long e0 = ((unsigned long long)blockIdx.x * blockDim.x + threadIdx.x) & ~31ull; e0 < n_ent;
+         e0 += warps * 32ull) {
+        const bool have = e0 + lane < n_ent;
+        const unsigned long long key = have ? entries[e0 + lane] : 0ull;
+        const uint32_t oi = (uint32_t)(key >> 32), oj = (uint32_t)key;
+        uint32_t bi = 0, ni = 1, bj = 0, nj = 1;  // rows behind each side: members[b .. b + n), or the row itself
+        if (have && (oi & kGroupFlag)) {
+            const uint32_t g = oi & ~kGroupFlag;
+            bi = group_start[g];
+            ni = group_start[g + 1] - bi;
+        }
+        if (have && (oj & kGroupFlag)) {
+            const uint32_t g = oj & ~kGroupFlag;
+            bj = group_start[g];
+            nj = group_start[g + 1] - bj;
+        }
+        const unsigned long long w = have ? (unsigned long long)ni * nj : 0ull;
+        unsigned long long incl = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned long long v = __shfl_up_sync(kFullMask, incl, o);
+            if (lane >= o) incl += v;
+        }
+        unsigned long long base = 0;
+        if (lane == 31) base = atomicAdd(edge_total, incl);
+        base = __shfl_sync(kFullMask, base, 31);
+        const unsigned long long first = base + incl - w;
+        auto put = [&](unsigned long long pos, uint32_t ri, uint32_t rj) {
+            const uint32_t a = min(ri, rj), b = max(ri, rj);
+            atomicAdd(row_count + a, 1);
+            atomicAdd(deg + b, 1);
+            if (pos < edge_cap) edges[pos] = ((unsigned long long)a << 32) | b;
+        };
+        if (have && w <= kOwn) {
+            unsigned long long pos = first;
+            for (uint32_t x = 0; x < ni; ++x) {
+                const uint32_t ri = (oi & kGroupFlag) ? (uint32_t)members[bi + x] : oi;
+                for (uint32_t y = 0; y < nj; ++y, ++pos) put(pos, ri, (oj & kGroupFlag) ? (uint32_t)members[bj + y] : oj);
+            }
+        }
+        uint32_t big = __ballot_sync(kFullMask, have && w > kOwn);
+        while (big) {
+            const int src = __ffs((int)big) - 1;
+            big &= big - 1u;
+            const uint32_t s_oi = __shfl_sync(kFullMask, oi, src), s_oj = __shfl_sync(kFullMask, oj, src);
+            const uint32_t s_bi = __shfl_sync(kFullMask, bi, src), s_bj = __shfl_sync(kFullMask, bj, src);
+            const uint32_t s_nj = __shfl_sync(kFullMask, nj, src);
+            const unsigned long long s_w = __shfl_sync(kFullMask, w, src), s_first = __shfl_sync(kFullMask, first, src);
+            for (unsigned long long k = (unsigned long long)lane; k < s_w; k += 32ull) {
+                const uint32_t x = (uint32_t)(k / s_nj), y = (uint32_t)(k % s_nj);
+                put(s_first + k, (s_oi & kGroupFlag) ? (uint32_t)members[s_bi + x] : s_oi,
+                    (s_oj & kGroupFlag) ? (uint32_t)members[s_bj + y] : s_oj);
+            }
+        }
+    }
+}
+
+// inverse of the coded perm: every row -> the sorted position of its sequence
+__global__ void __launch_bounds__(256) k_inverse_perm_groups(const int32_t* __restrict__ perm, int64_t n_u,
+                                                            const uint32_t* __restrict__ group_start,
+                                                            const int32_t* __restrict__ members,
+                                                            int32_t* __restrict__ inv) {
+    const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n_u) return;
+    const uint32_t code = (uint32_t)perm[s];
+    if (code & kGroupFlag) {
+        const uint32_t uid = code & ~kGroupFlag;
+        for (uint32_t k = group_start[uid]; k < group_start[uid + 1]; ++k) inv[members[k]] = (int32_t)s;
+    } else {
+        inv[code] = (int32_t)s;
+    }
+}
+
+unsigned grid_for(int64_t n) { return (unsigned)((n + 255) / 256); }
+
+}  // namespace
+
+uint32_t dedup_table_slots(int64_t n) {
+    uint32_t m = 1024;
+    while ((int64_t)m < 2 * n && m < (1u << 31)) m <<= 1;
+    return m;
+}
+
+cudaError_t launch_dedup_find(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths, int64_t n,
+                              int64_t total_len, unsigned long long* table, uint32_t slots, unsigned long long* hash,
+                              int32_t* rep_of, uint32_t* is_first, cudaStream_t s, int* launches) {
+    cudaError_t e = cudaMemsetAsync(table, 0xff, sizeof(unsigned long long) * (size_t)slots, s);
+    if (e != cudaSuccess) return e;
+    k_dedup_insert<<<grid_for(n), 256, 0, s>>>(residues, offsets, lengths, n, total_len, table, slots - 1u, hash);
+    k_dedup_lookup<<<grid_for(n), 256, 0, s>>>(residues, offsets, lengths, n, table, slots - 1u, hash, rep_of, is_first);
+    *launches += 2;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_dedup_groups(const int32_t* rep_of, const uint32_t* first_rank, const int64_t* offsets,
+                                const int32_t* lengths, int64_t n, int32_t* uid_of, uint32_t* group_count,
+                                int32_t* len_u, int64_t* off_u, cudaStream_t s, int* launches) {
+    k_dedup_groups<<<grid_for(n), 256, 0, s>>>(rep_of, first_rank, offsets, lengths, n, uid_of, group_count, len_u, off_u);
+    *launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_dedup_fill(const int32_t* uid_of, int64_t n, const uint32_t* group_start, uint32_t* group_count,
+                              int32_t* members, cudaStream_t s, int* launches) {
+    k_dedup_fill<<<grid_for(n), 256, 0, s>>>(uid_of, n, group_start, group_count, members);
+    *launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_dedup_codes(int32_t* perm, int64_t n_u, const uint32_t* group_start, const int32_t* members,
+                               cudaStream_t s, int* launches) {
+    k_dedup_codes<<<grid_for(n_u), 256, 0, s>>>(perm, n_u, group_start, members);
+    *launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_emit_cliques(const int32_t* members, const int32_t* uid_of, const uint32_t* group_start, int64_t n,
+                                unsigned long long* edges, unsigned long long* edge_count, unsigned long long edge_cap,
+                                int32_t* row_count, int32_t* deg, cudaStream_t s, int* launches) {
+    k_emit_cliques<<<grid_for(n), 256, 0, s>>>(members, uid_of, group_start, n, edges, edge_count, edge_cap, row_count, deg);
+    *launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_expand_entries(const unsigned long long* entries, const unsigned long long* n_entries_dev,
+                                  unsigned long long entry_cap, const uint32_t* group_start, const int32_t* members,
+                                  unsigned long long* edges, unsigned long long* edge_total, unsigned long long edge_cap,
+                                  int32_t* row_count, int32_t* deg, int n_sm, cudaStream_t s, int* launches) {
+    k_expand_entries<<<(unsigned)(n_sm * 8), 256, 0, s>>>(entries, n_entries_dev, entry_cap, group_start, members, edges,
+                                                          edge_total, edge_cap, row_count, deg);
+    *launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_inverse_perm_groups(const int32_t* perm, int64_t n_u, const uint32_t* group_start,
+                                       const int32_t* members, int32_t* inv, cudaStream_t s, int* launches) {
+    k_inverse_perm_groups<<<grid_for(n_u), 256, 0, s>>>(perm, n_u, group_start, members, inv);
+    *launches += 1;
+    return cudaGetLastError();
+}
+
+}  // namespace tcrnet

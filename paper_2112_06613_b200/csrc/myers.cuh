@@ -182,6 +182,10 @@ __device__ __forceinline__ void build_peq(W* peq, int tid, bool p_valid, const u
 }
 
 // Step A5: warp-aggregated emission of the pairs (pattern p_sorted, text t_sorted) with `edge` set.
+// perm maps a sorted position to the caller's row.  When the load collapsed identical sequences (dedup.cu,
+// P.group_start != NULL) it maps to the row of a sequence that only one row has, or to kGroupFlag | uid of a
+// shared one; the pair is then only recorded here and k_expand_entries turns it into its (rows) x (rows) edges
+// and does the counting.
 __device__ __forceinline__ void emit_edges(const DistanceParams& P, bool edge, int lane, int p_sorted, int t_sorted,
                                            int m, int n) {
     uint32_t oi = 0, oj = 0;
@@ -199,8 +203,10 @@ __device__ __forceinline__ void emit_edges(const DistanceParams& P, bool edge, i
         if (edge) {
             const unsigned long long pos = base + __popc(bal & ((1u << lane) - 1u));
             const uint32_t a = min(oi, oj), b = max(oi, oj);
-            atomicAdd(P.row_count + a, 1);
-            atomicAdd(P.deg + b, 1);
+            if (P.group_start == nullptr) {  // the keys are final: count them for the CSR step
+                atomicAdd(P.row_count + a, 1);
+                atomicAdd(P.deg + b, 1);
+            }
             if (pos < P.edge_cap) P.edges[pos] = ((unsigned long long)a << 32) | b;
         }
     }

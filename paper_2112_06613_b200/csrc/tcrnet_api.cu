@@ -67,9 +67,13 @@ void drop_load(tcrnet_ctx* ctx) {
 
 // Step A1: everything after the raw arrays are in device memory.  Packs rows 0..n-1 into `set`.
 // total_len < 0: not known (the query prefix of the rows); it is then taken from the histogram.
+// ext_offsets != NULL: residue offset of every row (the rows need not be contiguous in d_res); else the rows are
+// concatenated in order.
 int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* d_len, int64_t n, int64_t total_len,
-             int* launches) {
+             const int64_t* ext_offsets, int* launches) {
     set.loaded = false;
+    set.grouped = false;
+    set.n_rows = n;
     cudaStream_t s = ctx->stream;
     HostCtrl* dc = d_ctrl(ctx);
     TRY_CUDA(cudaMemsetAsync(dc, 0, sizeof(HostCtrl), s));
@@ -121,7 +125,12 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
     // radix sort with the row as payload.  The sub-order inside a length bucket is free (results are mapped
     // back through perm); the lexicographic one makes the 32 patterns of a warp share their first residues
     // and puts the texts of a bucket in trie order.
-    cudaError_t e = exclusive_scan_i32_to_i64(d_len, (int64_t*)offsets.p, n, true, ctx->scan_scratch.p, s, launches);
+    cudaError_t e = cudaSuccess;
+    const int64_t* d_off = ext_offsets;
+    if (!d_off) {
+        e = exclusive_scan_i32_to_i64(d_len, (int64_t*)offsets.p, n, true, ctx->scan_scratch.p, s, launches);
+        d_off = (const int64_t*)offsets.p;
+    }
     {
         constexpr int kPasses = (kSeqKeyBits + 7) / 8;
         int shifts[kPasses];
@@ -130,8 +139,7 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
         int32_t* va = (int32_t*)(kPasses & 1 ? ctx->perm_tmp.p : set.perm.p);
         int32_t* vb = (int32_t*)(kPasses & 1 ? set.perm.p : ctx->perm_tmp.p);
         if (e == cudaSuccess)
-            e = launch_seq_keys(d_res, (const int64_t*)offsets.p, d_len, n, (unsigned long long*)ctx->keys_a.p, va, s,
-                                launches);
+            e = launch_seq_keys(d_res, d_off, d_len, n, (unsigned long long*)ctx->keys_a.p, va, s, launches);
         bool in_b = false;
         if (e == cudaSuccess)
             e = radix_sort_u64((unsigned long long*)ctx->keys_a.p, (unsigned long long*)ctx->keys_b.p, va, vb, n, shifts,
@@ -141,7 +149,7 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
             e = cudaMemcpyAsync(set.perm.p, va, sizeof(int32_t), cudaMemcpyDeviceToDevice, s);
     }
     if (e == cudaSuccess)
-        e = launch_pack(d_res, (const int64_t*)offsets.p, d_len, (const int32_t*)set.perm.p, n, lt, set.pat_stride,
+        e = launch_pack(d_res, d_off, d_len, (const int32_t*)set.perm.p, n, lt, set.pat_stride,
                         (uint8_t*)set.pat.p, (uint32_t*)set.txt.p, &dc->flags, s, launches);
     // prefix trie over the sorted texts (trie.cu); scratch: lcp8 + per-tile counts
     DevBuf& trie_scratch = ctx->trie_scratch;
@@ -183,10 +191,77 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
     return TCRNET_OK;
 }
 
+// Step A0 (dedup.cu): the distinct sequences of the rows.  On success *n_u of them, their lengths / residue
+// offsets in dd_len / dd_off, and in `set` the rows behind every distinct sequence.
+int dedup_rows(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* d_len, int64_t n, int64_t total_len,
+               int64_t* n_u, int* launches) {
+    cudaStream_t s = ctx->stream;
+    HostCtrl* dc = d_ctrl(ctx);
+    const uint32_t slots = dedup_table_slots(n);
+    TRY(dev_reserve(ctx, ctx->scan_scratch, scan_scratch_bytes(n + 1)));
+    TRY(dev_reserve(ctx, ctx->dd_offsets, sizeof(int64_t) * (size_t)(n + 1)));
+    TRY(dev_reserve(ctx, ctx->dd_table, sizeof(unsigned long long) * (size_t)slots));
+    TRY(dev_reserve(ctx, ctx->dd_hash, sizeof(unsigned long long) * (size_t)n));
+    TRY(dev_reserve(ctx, ctx->dd_rep, sizeof(int32_t) * (size_t)n));
+    TRY(dev_reserve(ctx, ctx->dd_first, sizeof(uint32_t) * (size_t)n));
+    TRY(dev_reserve(ctx, ctx->dd_rank, sizeof(uint32_t) * (size_t)(n + 1)));
+    TRY(dev_reserve(ctx, ctx->dd_count, sizeof(uint32_t) * (size_t)(n + 1)));
+    TRY(dev_reserve(ctx, ctx->dd_len, sizeof(int32_t) * (size_t)n));
+    TRY(dev_reserve(ctx, ctx->dd_off, sizeof(int64_t) * (size_t)n));
+    TRY(dev_reserve(ctx, set.uid_of, sizeof(int32_t) * (size_t)n));
+    TRY(dev_reserve(ctx, set.group_start, sizeof(uint32_t) * (size_t)(n + 2)));
+    TRY(dev_reserve(ctx, set.members, sizeof(int32_t) * (size_t)n));
+    const int64_t* off = (const int64_t*)ctx->dd_offsets.p;
+    uint32_t* rank = (uint32_t*)ctx->dd_rank.p;
+    uint32_t* count = (uint32_t*)ctx->dd_count.p;
+    TRY_CUDA(cudaMemsetAsync(dc, 0, sizeof(HostCtrl), s));
+    TRY_CUDA(launch_length_hist(d_len, n, dc->hist, &dc->flags, s, launches));  // of the ROWS (nominal work, validation)
+    TRY_CUDA(cudaMemcpyAsync(ctx->h_ctrl, dc, offsetof(HostCtrl, edge_count), cudaMemcpyDeviceToHost, s));
+    TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->flags, &dc->flags, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+    TRY_CUDA(exclusive_scan_i32_to_i64(d_len, (int64_t*)ctx->dd_offsets.p, n, true, ctx->scan_scratch.p, s, launches));
+    TRY_CUDA(launch_dedup_find(d_res, off, d_len, n, total_len, (unsigned long long*)ctx->dd_table.p, slots,
+                               (unsigned long long*)ctx->dd_hash.p, (int32_t*)ctx->dd_rep.p, (uint32_t*)ctx->dd_first.p, s,
+                               launches));
+    TRY_CUDA(exclusive_scan_u32_total((const uint32_t*)ctx->dd_first.p, rank, n, ctx->scan_scratch.p, s, launches));
+    TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->n_distinct, rank + n, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+    TRY_CUDA(cudaMemsetAsync(count, 0, sizeof(uint32_t) * (size_t)(n + 1), s));
+    TRY_CUDA(launch_dedup_groups((const int32_t*)ctx->dd_rep.p, rank, off, d_len, n, (int32_t*)set.uid_of.p, count,
+                                 (int32_t*)ctx->dd_len.p, (int64_t*)ctx->dd_off.p, s, launches));
+    // group_start over n + 1 counts (the tail is zero): entry n_u is the total = n
+    TRY_CUDA(exclusive_scan_u32_total(count, (uint32_t*)set.group_start.p, n + 1, ctx->scan_scratch.p, s, launches));
+    TRY_CUDA(launch_dedup_fill((const int32_t*)set.uid_of.p, n, (const uint32_t*)set.group_start.p, count,
+                               (int32_t*)set.members.p, s, launches));
+    TRY_CUDA(cudaStreamSynchronize(s));
+    if (ctx->h_ctrl->flags & kFlagBadLength) return TCRNET_ERR_LENGTH;
+    for (int l = 0; l < kNumLen; ++l) ctx->row_hist[l] = (int64_t)ctx->h_ctrl->hist[l];
+    *n_u = (int64_t)ctx->h_ctrl->n_distinct;
+    if (*n_u < 1 || *n_u > n) return TCRNET_ERR_CUDA;
+    return TCRNET_OK;
+}
+
 int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len, int64_t n, int64_t total_len,
                      int* launches) {
-    TRY(pack_set(ctx, ctx->all, d_res, d_len, n, total_len, launches));
-    if (ctx->n_query > 0 && ctx->n_query < n) TRY(pack_set(ctx, ctx->query, d_res, d_len, ctx->n_query, -1, launches));
+    const bool rect = ctx->n_query > 0 && ctx->n_query < n;
+    int64_t n_u = n;
+    if (ctx->dedup && !rect && n >= 2) {
+        TRY(dedup_rows(ctx, ctx->all, d_res, d_len, n, total_len, &n_u, launches));
+        if (n_u < n) {
+            TRY(pack_set(ctx, ctx->all, d_res, (const int32_t*)ctx->dd_len.p, n_u, -1, (const int64_t*)ctx->dd_off.p,
+                         launches));
+            TRY_CUDA(launch_dedup_codes((int32_t*)ctx->all.perm.p, n_u, (const uint32_t*)ctx->all.group_start.p,
+                                        (const int32_t*)ctx->all.members.p, ctx->stream, launches));
+            ctx->all.grouped = true;
+            ctx->all.n_rows = n;
+        }
+    }
+    if (!ctx->all.loaded || !ctx->all.grouped) {
+        n_u = n;
+        TRY(pack_set(ctx, ctx->all, d_res, d_len, n, total_len, nullptr, launches));
+    }
+    if (rect) TRY(pack_set(ctx, ctx->query, d_res, d_len, ctx->n_query, -1, nullptr, launches));
+    if (!ctx->all.grouped)
+        for (int l = 0; l < kNumLen; ++l) ctx->row_hist[l] = ctx->all.hist[l];
+    ctx->stats.n_distinct = n_u;
     ctx->n = n;
     ctx->stats.n = n;
     ctx->stats.total_len = total_len;
@@ -276,8 +351,8 @@ void make_schedule(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule& 
     {
         long double sum_len = 0, sum_sq = 0;  // sum over unordered pairs of la*lb = ((sum l)^2 - sum l^2) / 2
         for (int l = 1; l < kNumLen; ++l) {
-            sum_len += (long double)ctx->all.hist[l] * l;
-            sum_sq += (long double)ctx->all.hist[l] * l * l;
+            sum_len += (long double)ctx->row_hist[l] * l;
+            sum_sq += (long double)ctx->row_hist[l] * l * l;
         }
         st.cells_all = (int64_t)((sum_len * sum_len - sum_sq) / 2);
     }
@@ -325,17 +400,23 @@ int upload_schedule(tcrnet_ctx* ctx, const Schedule& sch) {
     return TCRNET_OK;
 }
 
-int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_check, uint64_t cap, int shard,
-                 int n_shards, int* launches) {
+// cap: capacity of keys_a (the pairs the distance kernels record); cap_b: of keys_b (grouped loads only: the edges
+// between rows after the expansion).
+// expand_only: the recorded pairs in keys_a are complete, only keys_b was too small - redo the expansion alone.
+int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_check, uint64_t cap, uint64_t cap_b, int shard,
+                 int n_shards, bool expand_only, int* launches) {
     cudaStream_t s = ctx->stream;
     HostCtrl* dc = d_ctrl(ctx);
     static_assert(offsetof(HostCtrl, queue) == offsetof(HostCtrl, edge_count) + 5 * sizeof(unsigned long long), "one memset");
-    TRY_CUDA(cudaMemsetAsync(&dc->edge_count, 0, sizeof(unsigned long long) * (5 + kTrieQueues), s));  // edge_count, work[4], queue[]
+    static_assert(offsetof(HostCtrl, edge_total) == offsetof(HostCtrl, queue) + kTrieQueues * sizeof(unsigned long long), "one memset");
+    if (expand_only) TRY_CUDA(cudaMemsetAsync(&dc->edge_total, 0, sizeof(unsigned long long), s));
+    else TRY_CUDA(cudaMemsetAsync(&dc->edge_count, 0, sizeof(unsigned long long) * (6 + kTrieQueues), s));  // edge_count, work[4], queue[], edge_total
     TRY_CUDA(cudaMemsetAsync(ctx->row_count.p, 0, sizeof(int32_t) * (size_t)ctx->n, s));
     TRY_CUDA(cudaMemsetAsync(ctx->deg.p, 0, sizeof(int32_t) * (size_t)ctx->n, s));
     int n_queues = 0;
     const WorkRow* d_rows = (const WorkRow*)ctx->rows.p;
     for (const Schedule::Pass& pass : sch.passes) {
+        if (expand_only) break;
         DistanceParams p{};
         p.l_max = l_max;
         p.mode = pass.mode;
@@ -351,6 +432,8 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
         p.edges = (unsigned long long*)ctx->keys_a.p;
         p.row_count = (int32_t*)ctx->row_count.p;
         p.deg = (int32_t*)ctx->deg.p;
+        p.group_start = ctx->all.grouped ? (const uint32_t*)ctx->all.group_start.p : nullptr;
+        p.members = ctx->all.grouped ? (const int32_t*)ctx->all.members.p : nullptr;
         p.edge_count = &dc->edge_count;
         p.edge_cap = cap;
         p.work = dc->work;
@@ -371,6 +454,19 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
                 }
                 d_rows += part.rows.size();
             }
+    }
+    if (ctx->all.grouped) {
+        // the recorded pairs of distinct sequences -> edges between rows (keys_b), counted for the CSR step; the rows
+        // of every shared sequence are joined to each other (d = 0) by the first shard
+        const uint32_t* gs = (const uint32_t*)ctx->all.group_start.p;
+        const int32_t* mem = (const int32_t*)ctx->all.members.p;
+        if (shard == 0)
+            TRY_CUDA(launch_emit_cliques(mem, (const int32_t*)ctx->all.uid_of.p, gs, ctx->n, (unsigned long long*)ctx->keys_b.p,
+                                         &dc->edge_total, cap_b, (int32_t*)ctx->row_count.p, (int32_t*)ctx->deg.p, s, launches));
+        TRY_CUDA(launch_expand_entries((const unsigned long long*)ctx->keys_a.p, &dc->edge_count, cap, gs, mem,
+                                       (unsigned long long*)ctx->keys_b.p, &dc->edge_total, cap_b, (int32_t*)ctx->row_count.p,
+                                       (int32_t*)ctx->deg.p, ctx->n_sm, s, launches));
+        TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->edge_total, &dc->edge_total, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
     }
     TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->edge_count, &dc->edge_count, sizeof(unsigned long long) * 5,
                              cudaMemcpyDeviceToHost, s));
@@ -403,17 +499,34 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
     TRY(dev_reserve(ctx, ctx->keys_a, sizeof(unsigned long long) * (size_t)cap));
     TRY(dev_reserve(ctx, ctx->row_count, sizeof(int32_t) * (size_t)n));
     TRY(dev_reserve(ctx, ctx->deg, sizeof(int32_t) * (size_t)n));
-    st.distance_passes = 1;
-    TRY(run_distance(ctx, sch, l_max, first_check, (uint64_t)cap, shard, n_shards, launches));
-    int64_t n_keys = (int64_t)ctx->h_ctrl->edge_count;
-    if (n_keys > ctx->edge_limit) return TCRNET_ERR_EDGE_OVERFLOW;
-    if (n_keys > cap) {
-        cap = n_keys;
-        TRY(dev_reserve(ctx, ctx->keys_a, sizeof(unsigned long long) * (size_t)cap));
-        st.distance_passes = 2;
-        TRY(run_distance(ctx, sch, l_max, first_check, (uint64_t)cap, shard, n_shards, launches));
-        if ((int64_t)ctx->h_ctrl->edge_count != n_keys) return TCRNET_ERR_CUDA;  // cannot happen: same input
+    const bool grouped = ctx->all.grouped;
+    int64_t cap_b = 0;
+    if (grouped) {
+        cap_b = std::max<int64_t>(cap, (int64_t)(ctx->keys_b.bytes / 8));
+        cap_b = std::min(cap_b, ctx->edge_limit);
+        TRY(dev_reserve(ctx, ctx->keys_b, sizeof(unsigned long long) * (size_t)cap_b));
     }
+    int64_t n_keys = 0;
+    st.distance_passes = 0;
+    for (bool expand_only = false;;) {
+        if (!expand_only) ++st.distance_passes;
+        TRY(run_distance(ctx, sch, l_max, first_check, (uint64_t)cap, (uint64_t)cap_b, shard, n_shards, expand_only, launches));
+        const int64_t n_rec = (int64_t)ctx->h_ctrl->edge_count;  // pairs recorded by the distance kernels
+        n_keys = grouped ? (int64_t)ctx->h_ctrl->edge_total : n_rec;
+        if (n_rec > ctx->edge_limit || (n_rec <= cap && n_keys > ctx->edge_limit)) return TCRNET_ERR_EDGE_OVERFLOW;
+        if (n_rec > cap) {  // the record buffer was too small: grow it to the exact count and run again
+            if (st.distance_passes >= 2) return TCRNET_ERR_CUDA;  // cannot happen: same input
+            cap = n_rec;
+            TRY(dev_reserve(ctx, ctx->keys_a, sizeof(unsigned long long) * (size_t)cap));
+            continue;
+        }
+        if (!grouped || n_keys <= cap_b) break;
+        if (expand_only) return TCRNET_ERR_CUDA;  // cannot happen: exact size
+        cap_b = n_keys;
+        TRY(dev_reserve(ctx, ctx->keys_b, sizeof(unsigned long long) * (size_t)cap_b));
+        expand_only = true;
+    }
+    if (grouped) std::swap(ctx->keys_a, ctx->keys_b);  // the edges between rows are what the CSR step takes
     st.lane_columns_exec = (int64_t)ctx->h_ctrl->work[0];
     st.lane_tests_exec = (int64_t)ctx->h_ctrl->work[1];
     st.lane_pairs_exec = (int64_t)ctx->h_ctrl->work[2];
@@ -467,7 +580,11 @@ int ensure_edge_distances(tcrnet_ctx* ctx, int* launches) {
     cudaStream_t s = ctx->stream;
     TRY(dev_reserve(ctx, ctx->inv_perm, sizeof(int32_t) * (size_t)ctx->n));
     TRY(dev_reserve(ctx, ctx->edge_dist, (size_t)std::max<int64_t>(ctx->n_edges, 1)));
-    TRY_CUDA(launch_inverse_perm((const int32_t*)ctx->all.perm.p, ctx->n, (int32_t*)ctx->inv_perm.p, s, launches));
+    if (ctx->all.grouped)
+        TRY_CUDA(launch_inverse_perm_groups((const int32_t*)ctx->all.perm.p, ctx->all.n, (const uint32_t*)ctx->all.group_start.p,
+                                            (const int32_t*)ctx->all.members.p, (int32_t*)ctx->inv_perm.p, s, launches));
+    else
+        TRY_CUDA(launch_inverse_perm((const int32_t*)ctx->all.perm.p, ctx->n, (int32_t*)ctx->inv_perm.p, s, launches));
     TRY_CUDA(launch_edge_distances((const int64_t*)ctx->row_ptr.p, (const int32_t*)ctx->col.p, ctx->n, ctx->n_edges,
                                    (const int32_t*)ctx->inv_perm.p, (const uint8_t*)ctx->all.pat.p,
                                    ctx->all.pat_stride, (uint8_t*)ctx->edge_dist.p, s, launches));
@@ -539,7 +656,9 @@ void tcrnet_destroy(tcrnet_ctx* ctx) {
                       &ctx->query.txt, &ctx->query.trie, &ctx->inv_perm, &ctx->edge_dist, &ctx->edge_dist_b, &ctx->flags,
                       &ctx->flag_pos, &ctx->in_res, &ctx->in_len, &ctx->offsets,
                       &ctx->perm_tmp, &ctx->trie_scratch, &ctx->keys_a, &ctx->keys_b, &ctx->radix_scratch,
-                      &ctx->scan_scratch, &ctx->rows, &ctx->row_ptr, &ctx->col, &ctx->row_count, &ctx->long_rows,
+                      &ctx->scan_scratch, &ctx->rows, &ctx->row_ptr, &ctx->col, &ctx->row_count, &ctx->long_rows, &ctx->all.group_start, &ctx->all.members, &ctx->all.uid_of,
+                      &ctx->dd_table, &ctx->dd_hash, &ctx->dd_rep, &ctx->dd_first, &ctx->dd_rank, &ctx->dd_count, &ctx->dd_len,
+                      &ctx->dd_off, &ctx->dd_offsets,
                       &ctx->deg, &ctx->ctrl, &ctx->obs_ctrl, &ctx->deg_hist, &ctx->nn_sum, &ctx->class_sum, &ctx->knn,
                       &ctx->cc_parent, &ctx->cc_count, &ctx->cc_label, &ctx->cc_size, &ctx->perc_rank,
                       &ctx->perc_seen, &ctx->perc_deg, &ctx->perc_hist, &ctx->perc_lcc};
@@ -823,6 +942,10 @@ int tcrnet_set_option(tcrnet_ctx* ctx, int option, int64_t value) {
         case TCRNET_OPT_N_QUERY:
             if (value < 0 || value > 0x7ffffffeLL) return TCRNET_ERR_ARG;
             ctx->n_query = value;
+            return TCRNET_OK;
+        case TCRNET_OPT_DEDUP:
+            if (value != 0 && value != 1) return TCRNET_ERR_ARG;
+            ctx->dedup = (int)value;
             return TCRNET_OK;
         case TCRNET_OPT_TRIE_CHUNK:
             if (value < kTQ || value % kTQ != 0 || value > (1 << 24)) return TCRNET_ERR_ARG;

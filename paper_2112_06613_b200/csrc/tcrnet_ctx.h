@@ -17,9 +17,12 @@ struct HostCtrl {  // pinned mirror of the small device control block
     unsigned long long edge_count;
     unsigned long long work[4];
     unsigned long long queue[kTrieQueues];  // dynamic work queues of the trie launches (zeroed with edge_count)
+    unsigned long long edge_total;    // dedup: edges between rows after the expansion of the recorded pairs
     unsigned long long probe[3];
     uint32_t flags;
     uint32_t n_long;                  // rows queued for k_sort_long_rows
+    uint32_t n_distinct;              // dedup: distinct sequences of the load
+    uint32_t pad_;
     uint32_t trie_counts[8];          // [k] = nodes of trie level k
     uint32_t trie_root[kNumLen + 1];  // [L] = first level-1 node of length bucket L (non-empty buckets)
 };
@@ -36,6 +39,10 @@ struct SeqSet {
     TrieLevels trie_levels{};
     uint32_t trie_root[kNumLen + 1] = {};  // level-1 node range of bucket L: [trie_root[L], trie_root[L+1])
     int64_t trie_nodes = 0;
+    // dedup.cu: the set holds the distinct sequences of n_rows rows; perm is coded (row, or kGroupFlag | uid)
+    bool grouped = false;
+    int64_t n_rows = 0;
+    DevBuf group_start, members, uid_of;
 };
 
 struct tcrnet_ctx {
@@ -56,13 +63,16 @@ struct tcrnet_ctx {
     int prefix_trie = 1;
     int trie_chunk = 1 << 20;  // in practice the whole text bucket: the top of the trie is walked once per pattern tile
 
+    int dedup = 1;        // collapse identical sequences at load (TCRNET_OPT_DEDUP)
     int64_t n_query = 0;  // > 0: rectangular mode (TCRNET_OPT_N_QUERY)
 
     // load state
     bool loaded = false;
     int64_t n = 0;
     SeqSet all, query;
+    int64_t row_hist[kNumLen] = {};  // length histogram of the ROWS (all.hist counts distinct sequences when grouped)
     DevBuf in_res, in_len, offsets, perm_tmp, trie_scratch;  // load scratch, kept between loads (grow-only)
+    DevBuf dd_table, dd_hash, dd_rep, dd_first, dd_rank, dd_count, dd_len, dd_off, dd_offsets;  // dedup scratch
 
     // build state
     bool built = false;      // CSR + degrees valid

@@ -22,6 +22,7 @@ constexpr int kTrieFan = 27;             // staging slots per trie level, indexe
 constexpr int kTrieMaxL = 4;             // the trie kernel is specialised on l_max = 0..kTrieMaxL
 constexpr int kTrieTile = 32;            // patterns per work item of the trie kernel: one warp
 constexpr int kTrieQueues = 8;           // dynamic work queues (one per trie launch of a distance pass)
+constexpr uint32_t kGroupFlag = 0x80000000u;  // perm entry = kGroupFlag | uid: a sequence shared by several rows (dedup.cu)
 
 // Per-length layout of the packed sequence tables (filled on the host after the histogram).
 struct LengthTable {
@@ -89,6 +90,8 @@ struct DistanceParams {
     unsigned long long* edges;       // keys (min(i,j) << 32) | max(i,j)
     int32_t* row_count;              // [n]: += 1 at the smaller endpoint of every emitted edge (input of the CSR step)
     int32_t* deg;                    // [n]: += 1 at the larger endpoint
+    const uint32_t* group_start;     // dedup: the rows of sequence uid are members[group_start[uid] .. group_start[uid+1])
+    const int32_t* members;
     unsigned long long* edge_count;  // device counter (keeps counting beyond capacity)
     unsigned long long edge_cap;
     unsigned long long* work;        // [4]: lane-columns, lane-tests (exit votes), lane-first-columns,
@@ -142,6 +145,34 @@ int64_t trie_level_capacity(int64_t n, int level);
 cudaError_t launch_trie_build(const uint32_t* txt, const LengthTable& lt, int64_t n, uint8_t* lcp8,
                               uint32_t* tile_counts, const TrieLevels& levels, uint32_t* counts, uint32_t* root,
                               cudaStream_t s, int* launches);
+
+// dedup.cu: identical sequences collapse before the pack (see the file header for the steps)
+uint32_t dedup_table_slots(int64_t n);
+cudaError_t launch_dedup_find(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths, int64_t n,
+                              int64_t total_len, unsigned long long* table, uint32_t slots, unsigned long long* hash,
+                              int32_t* rep_of, uint32_t* is_first, cudaStream_t s, int* launches);
+// first_rank = exclusive scan of is_first; group_count zeroed by the caller
+cudaError_t launch_dedup_groups(const int32_t* rep_of, const uint32_t* first_rank, const int64_t* offsets,
+                                const int32_t* lengths, int64_t n, int32_t* uid_of, uint32_t* group_count,
+                                int32_t* len_u, int64_t* off_u, cudaStream_t s, int* launches);
+// group_start = exclusive scan of group_count (n_u + 1 entries); group_count is consumed
+cudaError_t launch_dedup_fill(const int32_t* uid_of, int64_t n, const uint32_t* group_start, uint32_t* group_count,
+                              int32_t* members, cudaStream_t s, int* launches);
+// perm[s] = uid -> the row itself (a sequence of one row) or kGroupFlag | uid
+cudaError_t launch_dedup_codes(int32_t* perm, int64_t n_u, const uint32_t* group_start, const int32_t* members,
+                               cudaStream_t s, int* launches);
+// the edges among the rows of every shared sequence (distance 0)
+cudaError_t launch_emit_cliques(const int32_t* members, const int32_t* uid_of, const uint32_t* group_start, int64_t n,
+                                unsigned long long* edges, unsigned long long* edge_count, unsigned long long edge_cap,
+                                int32_t* row_count, int32_t* deg, cudaStream_t s, int* launches);
+// the recorded pairs of distinct sequences (at most entry_cap of the *n_entries_dev counted) -> edges between rows
+cudaError_t launch_expand_entries(const unsigned long long* entries, const unsigned long long* n_entries_dev,
+                                  unsigned long long entry_cap, const uint32_t* group_start, const int32_t* members,
+                                  unsigned long long* edges, unsigned long long* edge_total, unsigned long long edge_cap,
+                                  int32_t* row_count, int32_t* deg, int n_sm, cudaStream_t s, int* launches);
+// inv[row] = sorted position of the row's sequence, from the coded perm
+cudaError_t launch_inverse_perm_groups(const int32_t* perm, int64_t n_u, const uint32_t* group_start,
+                                       const int32_t* members, int32_t* inv, cudaStream_t s, int* launches);
 
 // distance.cu
 size_t distance_smem_bytes(bool wide, int max_row_words);

@@ -73,8 +73,12 @@ def test_early_exit_and_schedule_do_not_change_the_result(pkg):
             got, st = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_FIRST_CHECK: fc})
             assert st["first_check"] == fc
             assert_same_network(got, ref)
-        got, st = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_TEXT_CHUNK: 256, pkg.OPT_EDGE_CAPACITY: 100})
+        got, st = gpu_network(pkg, d.residues, d.lengths, l_max,
+                              {pkg.OPT_TEXT_CHUNK: 256, pkg.OPT_EDGE_CAPACITY: 100, pkg.OPT_DEDUP: 0})
         assert st["distance_passes"] == 2
+        assert_same_network(got, ref)
+        # collapsed load: the record buffer and / or the expanded edge buffer have to grow
+        got, st = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_EDGE_CAPACITY: 100})
         assert_same_network(got, ref)
         got, st = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_COUNT_WORK: 1, pkg.OPT_PREFIX_TRIE: 0})
         assert_same_network(got, ref)
@@ -181,6 +185,28 @@ def test_all_duplicates_complete_graph(pkg, oracle):
         assert int(got[0][-1]) == r * (r - 1) // 2
         assert (got[2] == r - 1).all()
         check_csr_invariants(*got, r)
+
+
+@pytest.mark.parametrize("l_max", [0, 1, 3])
+def test_collapsing_identical_sequences_does_not_change_the_result(pkg, oracle, l_max):
+    """TCRNET_OPT_DEDUP: the distance step over the distinct sequences + multiplied emission (groups of 1, 2, many
+    rows on either side, cliques inside a group) equals the row-by-row build and the oracle."""
+    d = generate("cfg1")
+    on, st_on = gpu_network(pkg, d.residues, d.lengths, l_max)
+    off, st_off = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_DEDUP: 0})
+    assert st_on["n_distinct"] < d.n == st_off["n_distinct"]
+    assert st_on["n_distinct"] == len({bytes(r) for r in np.split(d.residues, np.cumsum(d.lengths)[:-1])})
+    assert st_on["pairs_kept"] < st_off["pairs_kept"] and st_on["pairs_all"] == st_off["pairs_all"]
+    assert_same_network(on, off)
+    assert_same_network(on, oracle.network(d.residues, d.lengths, l_max, tier=0)[:3])
+    # hubs: two sequences at distance 1 with many rows each, next to singletons and a third shared sequence
+    strings = ["CASSLGQF"] * 70 + ["CASSLGQW"] * 45 + ["CASSLGQ", "CASSLGQFF", "CWWWW"] + ["CASRLGQF"] * 3
+    rng = np.random.default_rng(5)
+    strings = [strings[i] for i in rng.permutation(len(strings))]
+    res, ln = from_strings(strings)
+    got, st = gpu_network(pkg, res, ln, l_max)
+    assert st["n_distinct"] == 6
+    assert_same_network(got, oracle.network(res, ln, l_max, tier=0)[:3])
 
 
 def test_rows_of_every_sorting_regime(pkg, oracle):
