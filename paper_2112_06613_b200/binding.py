@@ -207,7 +207,10 @@ class TcrNet:
             residues = np.ascontiguousarray(residues, dtype=np.uint8)
             lengths = np.ascontiguousarray(lengths, dtype=np.int32)
             n = int(lengths.size)
-            if n >= 1 and int(lengths.sum(dtype=np.int64)) > residues.size:  # (negative lengths: rejected by the library)
+            # Exact for valid lengths (1..64); invalid ones are rejected by the library before it reads a residue,
+            # so the 32-bit accumulator (vectorised: this sum is on the end-to-end path) may wrap for them.
+            total = int(np.add.reduce(lengths, dtype=np.int32)) if n <= (1 << 25) else int(lengths.sum(dtype=np.int64))
+            if n >= 1 and total > residues.size:
                 raise TcrNetError(ERR_ARG, "tcrnet_load (residues shorter than sum(lengths))")
             _check(self._lib.tcrnet_load(self._ctx, residues.ctypes.data_as(C.POINTER(C.c_uint8)),
                                          lengths.ctypes.data_as(C.POINTER(C.c_int32)), n), "tcrnet_load")

@@ -260,6 +260,11 @@ __global__ void __launch_bounds__(kTrieThreads, sizeof(W) == 4 ? 4 : 2) k_distan
     keep(w.stage_addr);
     keep(w.lane_addr);
     w.lane = lane;
+    {
+        uint32_t l = (uint32_t)w.lane;
+        keep(l);
+        w.lane = (int)l;
+    }
 
     const long long n_local = (P.n_items - P.shard + P.n_shards - 1) / P.n_shards;  // step 8(e): interleaved shards
     for (;;) {

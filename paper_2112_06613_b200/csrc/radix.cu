@@ -1,12 +1,12 @@
 // Stable LSD radix sort over 8-bit digits of 64-bit keys, with an optional 32-bit payload: the sequence
-// sort of step A1 (composite (length, first residues) keys, payload = caller's row) and the edge-key sort
-// of step A6.  HBM/L2-bound streaming; three launches per pass, no spinning on other CTAs:
+// sort of step A1 (composite (length, first residues) keys, payload = caller's row).  HBM/L2-bound
+// streaming; three launches per pass, no spinning on other CTAs:
 //
-//   k_radix_hist     per tile of 4096 keys, the 256 digit counts (shared-memory atomics), stored digit-major
+//   k_radix_hist     per tile of 4096 (1024 for short inputs) keys, the 256 digit counts (shared-memory atomics), stored digit-major
 //                    (hist[d * tiles + tile]) and added to the pass's global digit totals;
 //   k_radix_scan     CTA d turns row d of `hist` into global output positions: the total of all smaller
 //                    digits (from the global totals) + the exclusive prefix over the tiles;
-//   k_radix_scatter  each warp owns 512 consecutive keys of its tile and ranks equal digits in order
+//   k_radix_scatter  each warp owns 512 (128) consecutive keys of its tile and ranks equal digits in order
 //                    (__match_any_sync + a warp-private running count in shared memory, no CTA barrier
 //                    inside the loop), the 8 warp counts are chained once, keys go straight to their
 //                    final slot.  Order inside a digit = input order, so every pass is stable.
@@ -19,14 +19,17 @@ namespace {
 
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
-constexpr int kRounds = 16;                      // keys per thread
-constexpr int kTile = kThreads * kRounds;        // 4096 keys per CTA
-constexpr int kWarpItems = 32 * kRounds;         // 512 consecutive keys per warp
 constexpr uint32_t kFull = 0xffffffffu;
+// keys per thread (ROUNDS): 16 for long inputs (4096 keys per CTA, 512 consecutive keys per warp); 4 below
+// kSmallN keys, where 4096-key tiles would leave most SMs without a CTA and every pass is latency-bound
+constexpr int64_t kSmallN = (int64_t)1 << 22;
+__host__ __device__ constexpr int rounds_for(int64_t n) { return n < kSmallN ? 4 : 16; }
 
+template <int kRounds>
 __global__ void __launch_bounds__(kThreads) k_radix_hist(const unsigned long long* __restrict__ keys, int64_t n,
                                                         int shift, uint32_t* __restrict__ hist,
                                                         uint32_t* __restrict__ totals, uint32_t tiles) {
+    constexpr int kTile = kThreads * kRounds;
     __shared__ uint32_t h[256];
     h[threadIdx.x] = 0;
     __syncthreads();
@@ -80,12 +83,13 @@ __global__ void __launch_bounds__(kThreads) k_radix_scan(uint32_t* __restrict__ 
     }
 }
 
-template <bool HAS_VAL>
+template <bool HAS_VAL, int kRounds>
 __global__ void __launch_bounds__(kThreads) k_radix_scatter(const unsigned long long* __restrict__ keys_in,
                                                            unsigned long long* __restrict__ keys_out,
                                                            const int32_t* __restrict__ vals_in,
                                                            int32_t* __restrict__ vals_out, int64_t n, int shift,
                                                            const uint32_t* __restrict__ scanned, uint32_t tiles) {
+    constexpr int kTile = kThreads * kRounds, kWarpItems = 32 * kRounds;
     __shared__ uint32_t wh[kWarps][256];  // per warp: running digit counts, then first output slots
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 #pragma unroll
@@ -135,7 +139,10 @@ __global__ void __launch_bounds__(kThreads) k_radix_scatter(const unsigned long 
 
 }  // namespace
 
-int64_t radix_tiles(int64_t n) { return n > 0 ? (n + kTile - 1) / kTile : 1; }
+int64_t radix_tiles(int64_t n) {
+    const int64_t tile = (int64_t)kThreads * rounds_for(n);
+    return n > 0 ? (n + tile - 1) / tile : 1;
+}
 
 size_t radix_scratch_bytes(int64_t n) {
     return ((size_t)radix_tiles(n) * 256 + (size_t)kRadixMaxPasses * 256) * sizeof(uint32_t);
@@ -153,13 +160,19 @@ cudaError_t radix_sort_u64(unsigned long long* keys_a, unsigned long long* keys_
     cudaError_t e = cudaMemsetAsync(totals, 0, sizeof(uint32_t) * kRadixMaxPasses * 256, s);
     if (e != cudaSuccess) return e;
     const bool has_val = vals_a != nullptr;
+    const bool small = rounds_for(n) == 4;
     for (int p = 0; p < n_passes; ++p) {
-        k_radix_hist<<<tiles, kThreads, 0, s>>>(keys_a, n, shifts[p], hist, totals + p * 256, tiles);
+        if (small) k_radix_hist<4><<<tiles, kThreads, 0, s>>>(keys_a, n, shifts[p], hist, totals + p * 256, tiles);
+        else k_radix_hist<16><<<tiles, kThreads, 0, s>>>(keys_a, n, shifts[p], hist, totals + p * 256, tiles);
         k_radix_scan<<<256, kThreads, 0, s>>>(hist, totals + p * 256, tiles);
-        if (has_val)
-            k_radix_scatter<true><<<tiles, kThreads, 0, s>>>(keys_a, keys_b, vals_a, vals_b, n, shifts[p], hist, tiles);
+        if (has_val && small)
+            k_radix_scatter<true, 4><<<tiles, kThreads, 0, s>>>(keys_a, keys_b, vals_a, vals_b, n, shifts[p], hist, tiles);
+        else if (has_val)
+            k_radix_scatter<true, 16><<<tiles, kThreads, 0, s>>>(keys_a, keys_b, vals_a, vals_b, n, shifts[p], hist, tiles);
+        else if (small)
+            k_radix_scatter<false, 4><<<tiles, kThreads, 0, s>>>(keys_a, keys_b, nullptr, nullptr, n, shifts[p], hist, tiles);
         else
-            k_radix_scatter<false><<<tiles, kThreads, 0, s>>>(keys_a, keys_b, nullptr, nullptr, n, shifts[p], hist, tiles);
+            k_radix_scatter<false, 16><<<tiles, kThreads, 0, s>>>(keys_a, keys_b, nullptr, nullptr, n, shifts[p], hist, tiles);
         *launches += 3;
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
