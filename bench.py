@@ -39,8 +39,8 @@ ALU_OPS_PER_TEST = 4           # 2 LOP3 + IADD3 + ISETP per pair and early-exit 
 ALU_OPS_PER_PREFIX_TEST = 2    # LOP3 + ISETP per pair and DP cell read in a guided expansion (distance_trie.cu)
 ORACLE_SAMPLE_ROWS = 1024
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_distance_trie launch at cfg4, from the ncu --set full
-# capture summarised in profiles/r1d_trie_ncu.txt (95.40 MB + 19.77 MB)
-NCU_DRAM_BYTES_PER_LAUNCH = {"cfg4": 115_171_584}
+# capture summarised in profiles/r1e_trie_ncu.txt (65.39 MB + 3.84 MB)
+NCU_DRAM_BYTES_PER_LAUNCH = {"cfg4": 69_231_360}
 
 
 def _peaks():
@@ -307,13 +307,14 @@ def main() -> None:
         peaks, peak_kind = _peaks()
         n_sm = torch.cuda.get_device_properties(local_rank).multi_processor_count
         ms_dist = float(np.mean([s["ms_distance"] for s in stats]))
+        ms_kernel = float(np.mean([s["ms_kernel"] for s in stats]))  # the distance kernel launch alone
         ms_sort = float(np.mean([s["ms_sort"] for s in stats]))
         ms_csr = float(np.mean([s["ms_csr"] for s in stats]))
         ms_load = float(np.mean([s["ms_load"] for s in stats]))
         alu_ops = (ALU_OPS_PER_COLUMN * work["lane_columns_exec"] + ALU_OPS_PER_TEST * work["lane_tests_exec"]
                    + ALU_OPS_PER_PREFIX_TEST * work["lane_prefix_tests_exec"]
                    - (ALU_OPS_PER_COLUMN - ALU_OPS_FIRST_COLUMN) * work["lane_pairs_exec"] * (work["first_check"] > 0))
-        achieved = alu_ops / (ms_dist * 1e-3) / 1e12
+        achieved = alu_ops / (ms_kernel * 1e-3) / 1e12
         peak = n_sm * ALU_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12
         probes = {}
         for kind, name in ((0, "lop3"), (2, "imad"), (3, "lop3_imad_mix"), (5, "myers_step")):
@@ -335,17 +336,18 @@ def main() -> None:
             "gpu_launches": int(sum(s["launches_load"] + s["launches_build"] for s in stats)),
             "roofline": {
                 "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TIOP/s (INT32 ALU-pipe lane-ops)",
-                "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.workload), "kernel": "k_distance_trie" if work["work_items_trie"] else "k_distance", "kernel_ms": ms_dist,
+                "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.workload), "kernel": "k_distance_trie" if work["work_items_trie"] else "k_distance", "kernel_ms": ms_kernel,
                 "peak_source": f"{n_sm} SMs x {ALU_LANES_PER_SM} lanes x {peaks['sm_max_mhz']} MHz ({peak_kind} sm_max_mhz)",
                 "alu_ops_per_launch": alu_ops, "measured_pipe_peaks": probes,
             },
             "detail": {
                 "pairs_kept": work["pairs_kept"], "cells_kept": work["cells_kept"], "cells_all": work["cells_all"],
-                "pairs_per_s_evaluated": work["pairs_kept"] / (ms_dist * 1e-3),
-                "gcups_evaluated": work["cells_kept"] / (ms_dist * 1e-3) / 1e9,
+                "n_distinct": work["n_distinct"],
+                "pairs_per_s_evaluated": work["pairs_kept"] / (ms_kernel * 1e-3),
+                "gcups_evaluated": work["cells_kept"] / (ms_kernel * 1e-3) / 1e9,
                 "gcups_effective": work["cells_all"] / (ms_step * 1e-3) / 1e9,
                 "columns_executed_fraction": work["lane_columns_exec"] / max(1, work["columns_kept"]),
-                "ms_pack": ms_load, "ms_distance": ms_dist, "ms_sort": ms_sort, "ms_csr": ms_csr,
+                "ms_pack": ms_load, "ms_distance": ms_dist, "ms_distance_kernel": ms_kernel, "ms_sort": ms_sort, "ms_csr": ms_csr,
                 "work_items": work["work_items"], "work_items_trie": work["work_items_trie"],
                 "trie_nodes": work["trie_nodes"], "lane_columns_exec": work["lane_columns_exec"],
                 "lane_prefix_tests_exec": work["lane_prefix_tests_exec"], "lane_tests_exec": work["lane_tests_exec"],

@@ -147,6 +147,10 @@ typedef struct tcrnet_stats {
     float ms_build;            /* whole tcrnet_build on the device                            */
     int64_t n_distinct;        /* distinct sequences among the rows (= n when TCRNET_OPT_DEDUP
                                   is off or in the rectangular mode)                         */
+    float ms_kernel;           /* the distance kernel launches alone (CUDA events right around
+                                  them; ms_distance adds the schedule upload, the counter
+                                  resets and the expansion of collapsed pairs)               */
+    float pad_;
 } tcrnet_stats;
 
 /*

@@ -48,7 +48,7 @@ class tcrnet_stats(C.Structure):
         ("work_items_trie", C.c_int64), ("trie_nodes", C.c_int64), ("distance_passes", C.c_int32),
         ("launches_load", C.c_int32), ("launches_build", C.c_int32), ("ms_load", C.c_float),
         ("ms_distance", C.c_float), ("ms_sort", C.c_float), ("ms_csr", C.c_float), ("ms_build", C.c_float),
-        ("n_distinct", C.c_int64),
+        ("n_distinct", C.c_int64), ("ms_kernel", C.c_float), ("pad_", C.c_float),
     ]
 
 

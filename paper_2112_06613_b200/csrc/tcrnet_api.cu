@@ -415,6 +415,7 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
     TRY_CUDA(cudaMemsetAsync(ctx->deg.p, 0, sizeof(int32_t) * (size_t)ctx->n, s));
     int n_queues = 0;
     const WorkRow* d_rows = (const WorkRow*)ctx->rows.p;
+    if (!expand_only) TRY_CUDA(cudaEventRecord(ctx->ev[4], s));
     for (const Schedule::Pass& pass : sch.passes) {
         if (expand_only) break;
         DistanceParams p{};
@@ -455,6 +456,7 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
                 d_rows += part.rows.size();
             }
     }
+    if (!expand_only) TRY_CUDA(cudaEventRecord(ctx->ev[5], s));
     if (ctx->all.grouped) {
         // the recorded pairs of distinct sequences -> edges between rows (keys_b), counted for the CSR step; the rows
         // of every shared sequence are joined to each other (d = 0) by the first shard
@@ -527,6 +529,7 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
         expand_only = true;
     }
     if (grouped) std::swap(ctx->keys_a, ctx->keys_b);  // the edges between rows are what the CSR step takes
+    TRY_CUDA(cudaEventElapsedTime(&st.ms_kernel, ctx->ev[4], ctx->ev[5]));  // of the last pass (both complete: synced)
     st.lane_columns_exec = (int64_t)ctx->h_ctrl->work[0];
     st.lane_tests_exec = (int64_t)ctx->h_ctrl->work[1];
     st.lane_pairs_exec = (int64_t)ctx->h_ctrl->work[2];
