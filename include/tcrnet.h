@@ -216,10 +216,10 @@ TCRNET_API int tcrnet_build_shard(tcrnet_ctx* ctx, int l_max, int shard, int n_s
                                   int64_t* n_keys_out);
 
 /*
- * Step A6 on an edge list supplied by the caller: sort the n_keys keys (i << 32) | j (device
+ * Step A6 on an edge list supplied by the caller: order the n_keys keys (i << 32) | j (device
  * uint64, any order, each edge once, i < j < n) and build CSR + degrees as tcrnet_build does
  * (PAPER.md:301-318, 224).  keys_dev is copied unless it is the pointer tcrnet_build_shard
- * returned (then the sort runs in place).  Errors: ARG (a key with i >= j or j >= n), STATE
+ * returned (then it runs in place).  Errors: ARG (a key with i >= j or j >= n), STATE
  * (no load), NOMEM, EDGE_OVERFLOW, CUDA.
  */
 TCRNET_API int tcrnet_assemble(tcrnet_ctx* ctx, const uint64_t* keys_dev, int64_t n_keys, int64_t* n_edges_out);
