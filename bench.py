@@ -354,6 +354,17 @@ def main() -> None:
                 "ms_steps": ms_steps,
             },
         }
+        # the emission / CSR passes against the HBM peak (algorithmic bytes of DESIGN.md section 7:
+        # expansion 8 B read per recorded pair + 8 B written per edge; A6 bucket scatter 8 + 8 B, rank 8 + 4 B per edge,
+        # 12 B per node and the scan's 4 + 8 B per node)
+        e_cnt = int(n_edges)
+        csr_bytes = e_cnt * 28 + n * 24
+        out["hbm_passes"] = {
+            "csr_algorithmic_bytes": csr_bytes, "csr_ms": ms_csr,
+            "csr_gb_per_s": csr_bytes / (ms_csr * 1e-3) / 1e9 if ms_csr > 0 else None,
+            "csr_frac_of_hbm_peak": (csr_bytes / (ms_csr * 1e-3) / 1e9) / peaks["hbm_gbs"] if ms_csr > 0 else None,
+            "note": "L2-resident, launch- and latency-bound at this size (6 launches, 20-50 us each)",
+        }
         if not args.no_cpu_baseline and world == 1:
             pps, cps, threads, dt, pairs = oracle_sample(d, l_max, ORACLE_SAMPLE_ROWS)
             out["cpu_baseline"] = {

@@ -15,10 +15,13 @@
 namespace tcrnet {
 namespace {
 
+// n_dev != NULL: the number of rows is read from device memory (it is at most n)
 __global__ void __launch_bounds__(256) k_length_hist(const int32_t* __restrict__ lengths, int64_t n,
+                                                    const uint32_t* __restrict__ n_dev,
                                                     unsigned long long* __restrict__ hist,
                                                     uint32_t* __restrict__ flags) {
     __shared__ uint32_t h[kNumLen];
+    if (n_dev) n = min(n, (int64_t)*n_dev);
     for (int i = threadIdx.x; i < kNumLen; i += blockDim.x) h[i] = 0;
     __syncthreads();
     bool bad = false;
@@ -114,11 +117,11 @@ __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residu
 
 }  // namespace
 
-cudaError_t launch_length_hist(const int32_t* lengths, int64_t n, unsigned long long* hist, uint32_t* flags,
-                               cudaStream_t s, int* launches) {
+cudaError_t launch_length_hist(const int32_t* lengths, int64_t n, const uint32_t* n_dev, unsigned long long* hist,
+                               uint32_t* flags, cudaStream_t s, int* launches) {
     int64_t blocks = (n + 255) / 256;
     if (blocks > 148 * 8) blocks = 148 * 8;
-    k_length_hist<<<(unsigned)blocks, 256, 0, s>>>(lengths, n, hist, flags);
+    k_length_hist<<<(unsigned)blocks, 256, 0, s>>>(lengths, n, n_dev, hist, flags);
     *launches += 1;
     return cudaGetLastError();
 }

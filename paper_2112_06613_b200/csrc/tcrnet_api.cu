@@ -69,22 +69,26 @@ void drop_load(tcrnet_ctx* ctx) {
 // total_len < 0: not known (the query prefix of the rows); it is then taken from the histogram.
 // ext_offsets != NULL: residue offset of every row (the rows need not be contiguous in d_res); else the rows are
 // concatenated in order.
+// pre_hist != NULL: the (validated) length histogram of the rows is already on the host.
 int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* d_len, int64_t n, int64_t total_len,
-             const int64_t* ext_offsets, int* launches) {
+             const int64_t* ext_offsets, const unsigned long long* pre_hist, int* launches) {
     set.loaded = false;
     set.grouped = false;
     set.n_rows = n;
     cudaStream_t s = ctx->stream;
     HostCtrl* dc = d_ctrl(ctx);
     TRY_CUDA(cudaMemsetAsync(dc, 0, sizeof(HostCtrl), s));
-    TRY_CUDA(launch_length_hist(d_len, n, dc->hist, &dc->flags, s, launches));
-    TRY_CUDA(cudaMemcpyAsync(ctx->h_ctrl, dc, sizeof(HostCtrl), cudaMemcpyDeviceToHost, s));
-    TRY_CUDA(cudaStreamSynchronize(s));
-    if (ctx->h_ctrl->flags & kFlagBadLength) return TCRNET_ERR_LENGTH;
+    if (!pre_hist) {
+        TRY_CUDA(launch_length_hist(d_len, n, nullptr, dc->hist, &dc->flags, s, launches));
+        TRY_CUDA(cudaMemcpyAsync(ctx->h_ctrl, dc, sizeof(HostCtrl), cudaMemcpyDeviceToHost, s));
+        TRY_CUDA(cudaStreamSynchronize(s));
+        if (ctx->h_ctrl->flags & kFlagBadLength) return TCRNET_ERR_LENGTH;
+        pre_hist = ctx->h_ctrl->hist;
+    }
     int64_t sum = 0, cnt = 0;
     int min_len = kMaxLen, max_len = 0;
     for (int l = 0; l < kNumLen; ++l) {
-        set.hist[l] = (int64_t)ctx->h_ctrl->hist[l];
+        set.hist[l] = (int64_t)pre_hist[l];
         if (set.hist[l]) {
             min_len = std::min(min_len, l);
             max_len = std::max(max_len, l);
@@ -215,9 +219,7 @@ int dedup_rows(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t
     uint32_t* rank = (uint32_t*)ctx->dd_rank.p;
     uint32_t* count = (uint32_t*)ctx->dd_count.p;
     TRY_CUDA(cudaMemsetAsync(dc, 0, sizeof(HostCtrl), s));
-    TRY_CUDA(launch_length_hist(d_len, n, dc->hist, &dc->flags, s, launches));  // of the ROWS (nominal work, validation)
-    TRY_CUDA(cudaMemcpyAsync(ctx->h_ctrl, dc, offsetof(HostCtrl, edge_count), cudaMemcpyDeviceToHost, s));
-    TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->flags, &dc->flags, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+    TRY_CUDA(launch_length_hist(d_len, n, nullptr, dc->hist, &dc->flags, s, launches));  // of the ROWS (nominal work, validation)
     TRY_CUDA(exclusive_scan_i32_to_i64(d_len, (int64_t*)ctx->dd_offsets.p, n, true, ctx->scan_scratch.p, s, launches));
     TRY_CUDA(launch_dedup_find(d_res, off, d_len, n, total_len, (unsigned long long*)ctx->dd_table.p, slots,
                                (unsigned long long*)ctx->dd_hash.p, (int32_t*)ctx->dd_rep.p, (uint32_t*)ctx->dd_first.p, s,
@@ -227,13 +229,21 @@ int dedup_rows(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t
     TRY_CUDA(cudaMemsetAsync(count, 0, sizeof(uint32_t) * (size_t)(n + 1), s));
     TRY_CUDA(launch_dedup_groups((const int32_t*)ctx->dd_rep.p, rank, off, d_len, n, (int32_t*)set.uid_of.p, count,
                                  (int32_t*)ctx->dd_len.p, (int64_t*)ctx->dd_off.p, s, launches));
+    // the length histogram of the distinct sequences, so that the pack needs no round trip of its own
+    TRY_CUDA(launch_length_hist((const int32_t*)ctx->dd_len.p, n, rank + n, dc->hist_u, &dc->flags, s, launches));
+    TRY_CUDA(cudaMemcpyAsync(ctx->h_ctrl->hist, dc->hist, sizeof(dc->hist), cudaMemcpyDeviceToHost, s));
+    TRY_CUDA(cudaMemcpyAsync(ctx->h_ctrl->hist_u, dc->hist_u, sizeof(dc->hist_u), cudaMemcpyDeviceToHost, s));
+    TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->flags, &dc->flags, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
     // group_start over n + 1 counts (the tail is zero): entry n_u is the total = n
     TRY_CUDA(exclusive_scan_u32_total(count, (uint32_t*)set.group_start.p, n + 1, ctx->scan_scratch.p, s, launches));
     TRY_CUDA(launch_dedup_fill((const int32_t*)set.uid_of.p, n, (const uint32_t*)set.group_start.p, count,
                                (int32_t*)set.members.p, s, launches));
     TRY_CUDA(cudaStreamSynchronize(s));
     if (ctx->h_ctrl->flags & kFlagBadLength) return TCRNET_ERR_LENGTH;
-    for (int l = 0; l < kNumLen; ++l) ctx->row_hist[l] = (int64_t)ctx->h_ctrl->hist[l];
+    for (int l = 0; l < kNumLen; ++l) {
+        ctx->row_hist[l] = (int64_t)ctx->h_ctrl->hist[l];
+        ctx->hist_u_host[l] = ctx->h_ctrl->hist_u[l];  // (the pack clears the control block)
+    }
     *n_u = (int64_t)ctx->h_ctrl->n_distinct;
     if (*n_u < 1 || *n_u > n) return TCRNET_ERR_CUDA;
     return TCRNET_OK;
@@ -247,7 +257,7 @@ int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len
         TRY(dedup_rows(ctx, ctx->all, d_res, d_len, n, total_len, &n_u, launches));
         if (n_u < n) {
             TRY(pack_set(ctx, ctx->all, d_res, (const int32_t*)ctx->dd_len.p, n_u, -1, (const int64_t*)ctx->dd_off.p,
-                         launches));
+                         ctx->hist_u_host, launches));
             TRY_CUDA(launch_dedup_codes((int32_t*)ctx->all.perm.p, n_u, (const uint32_t*)ctx->all.group_start.p,
                                         (const int32_t*)ctx->all.members.p, ctx->stream, launches));
             ctx->all.grouped = true;
@@ -256,9 +266,9 @@ int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len
     }
     if (!ctx->all.loaded || !ctx->all.grouped) {
         n_u = n;
-        TRY(pack_set(ctx, ctx->all, d_res, d_len, n, total_len, nullptr, launches));
+        TRY(pack_set(ctx, ctx->all, d_res, d_len, n, total_len, nullptr, nullptr, launches));
     }
-    if (rect) TRY(pack_set(ctx, ctx->query, d_res, d_len, ctx->n_query, -1, nullptr, launches));
+    if (rect) TRY(pack_set(ctx, ctx->query, d_res, d_len, ctx->n_query, -1, nullptr, nullptr, launches));
     if (!ctx->all.grouped)
         for (int l = 0; l < kNumLen; ++l) ctx->row_hist[l] = ctx->all.hist[l];
     ctx->stats.n_distinct = n_u;

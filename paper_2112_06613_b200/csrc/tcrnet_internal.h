@@ -123,8 +123,9 @@ cudaError_t radix_sort_u64(unsigned long long* keys_a, unsigned long long* keys_
                            bool* result_in_b);
 
 // pack.cu
-cudaError_t launch_length_hist(const int32_t* lengths, int64_t n, unsigned long long* hist /*[kNumLen]*/,
-                               uint32_t* flags, cudaStream_t s, int* launches);
+// n_dev (may be NULL): device count of rows, at most n
+cudaError_t launch_length_hist(const int32_t* lengths, int64_t n, const uint32_t* n_dev,
+                               unsigned long long* hist /*[kNumLen]*/, uint32_t* flags, cudaStream_t s, int* launches);
 // sort key of row i: (clamped length << 30) | the first kSortPrefix residues, 5 bits each (0 = past the end); vals[i] = i
 constexpr int kSeqKeyBits = 6 + 5 * kSortPrefix;
 cudaError_t launch_seq_keys(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths, int64_t n,
