@@ -200,8 +200,8 @@ __device__ __forceinline__ void visit(Walk<W, COUNT>& w, const DistanceParams& P
         __syncwarp();
     }
     do {
-        const uint32_t c = top_bit(U);
-        U ^= 1u << c;
+        const uint32_t c = (uint32_t)__ffs((int)U) - 1u;  // children in ascending code order
+        U &= U - 1u;
         const uint4 nd = lds128(sb + c * 16);  // text_begin, text_end, child_begin, child_codes
         if (LEVEL <= kClipLevels) {  // clip the upper levels to this warp's texts
             if (nd.y <= w.lo || nd.x >= w.hi) continue;
