@@ -209,6 +209,27 @@ def test_collapsing_identical_sequences_does_not_change_the_result(pkg, oracle, 
     assert_same_network(got, oracle.network(res, ln, l_max, tier=0)[:3])
 
 
+@pytest.mark.parametrize("seed", [0, 1, 2, 3])
+def test_heavily_repeated_rows_random(pkg, oracle, seed):
+    """Random multiplicities (1 .. 60 rows per sequence) over a family-structured base set, shuffled; every l_max,
+    also with an edge buffer that has to grow (records and expansion)."""
+    rng = np.random.default_rng(100 + seed)
+    d = generate("cfg1", n=400)
+    rows = np.split(d.residues, np.cumsum(d.lengths)[:-1])
+    mult = rng.choice([1, 1, 1, 2, 3, 7, 25, 60], size=len(rows))
+    strings = [bytes(rows[i]).decode() for i in range(len(rows)) for _ in range(int(mult[i]))]
+    strings = [strings[i] for i in rng.permutation(len(strings))]
+    res, ln = from_strings(strings)
+    for l_max in (0, 1, 2):
+        want = oracle.network(res, ln, l_max, tier=1)[:3]
+        got, st = gpu_network(pkg, res, ln, l_max)
+        assert st["n_distinct"] == len(set(strings))
+        assert_same_network(got, want)
+        got, _ = gpu_network(pkg, res, ln, l_max, {pkg.OPT_EDGE_CAPACITY: 7})
+        assert_same_network(got, want)
+    check_csr_invariants(*got, len(strings))
+
+
 def test_rows_of_every_sorting_regime(pkg, oracle):
     """The CSR step orders a row by one thread (<= 32 neighbours), in shared memory (<= 8192) or in place
     (beyond): a clique of 9,001 copies has rows of every such length; the other strings hang off it."""
