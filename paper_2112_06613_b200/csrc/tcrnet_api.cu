@@ -71,7 +71,7 @@ void drop_load(tcrnet_ctx* ctx) {
 // concatenated in order.
 // pre_hist != NULL: the (validated) length histogram of the rows is already on the host.
 int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* d_len, int64_t n, int64_t total_len,
-             const int64_t* ext_offsets, const unsigned long long* pre_hist, int* launches) {
+             const int64_t* ext_offsets, const unsigned long long* pre_hist, bool code_groups, int* launches) {
     set.loaded = false;
     set.grouped = false;
     set.n_rows = n;
@@ -174,6 +174,11 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
                                   dc->trie_counts, dc->trie_root, s, launches);
         }
     }
+    // collapsed load: the rows were the distinct sequences; perm (position -> uid) has served the pack and now
+    // becomes position -> row, or kGroupFlag | uid of a shared sequence
+    if (rc == TCRNET_OK && e == cudaSuccess && code_groups)
+        e = launch_dedup_codes((int32_t*)set.perm.p, n, (const uint32_t*)set.group_start.p, (const int32_t*)set.members.p, s,
+                               launches);
     if (rc == TCRNET_OK && e == cudaSuccess)
         e = cudaMemcpyAsync(&ctx->h_ctrl->flags, &dc->flags,
                             sizeof(HostCtrl) - offsetof(HostCtrl, flags), cudaMemcpyDeviceToHost, s);
@@ -257,18 +262,16 @@ int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len
         TRY(dedup_rows(ctx, ctx->all, d_res, d_len, n, total_len, &n_u, launches));
         if (n_u < n) {
             TRY(pack_set(ctx, ctx->all, d_res, (const int32_t*)ctx->dd_len.p, n_u, -1, (const int64_t*)ctx->dd_off.p,
-                         ctx->hist_u_host, launches));
-            TRY_CUDA(launch_dedup_codes((int32_t*)ctx->all.perm.p, n_u, (const uint32_t*)ctx->all.group_start.p,
-                                        (const int32_t*)ctx->all.members.p, ctx->stream, launches));
+                         ctx->hist_u_host, true, launches));
             ctx->all.grouped = true;
             ctx->all.n_rows = n;
         }
     }
     if (!ctx->all.loaded || !ctx->all.grouped) {
         n_u = n;
-        TRY(pack_set(ctx, ctx->all, d_res, d_len, n, total_len, nullptr, nullptr, launches));
+        TRY(pack_set(ctx, ctx->all, d_res, d_len, n, total_len, nullptr, nullptr, false, launches));
     }
-    if (rect) TRY(pack_set(ctx, ctx->query, d_res, d_len, ctx->n_query, -1, nullptr, nullptr, launches));
+    if (rect) TRY(pack_set(ctx, ctx->query, d_res, d_len, ctx->n_query, -1, nullptr, nullptr, false, launches));
     if (!ctx->all.grouped)
         for (int l = 0; l < kNumLen; ++l) ctx->row_hist[l] = ctx->all.hist[l];
     ctx->stats.n_distinct = n_u;
