@@ -126,7 +126,9 @@ typedef struct tcrnet_stats {
     int32_t first_check;       /* columns before the first early-exit test (0: early exit off)*/
     int64_t n_edges;           /* |E|                                                         */
     int64_t pairs_all;         /* N(N-1)/2                                                    */
-    int64_t pairs_kept;        /* pairs with |len_i - len_j| <= l_max (the ones evaluated)    */
+    int64_t pairs_kept;        /* pairs with |len_i - len_j| <= l_max that are evaluated: of
+                                  distinct sequences when the load collapsed identical rows;
+                                  cells_kept / columns_kept likewise                           */
     int64_t cells_all;         /* sum over all pairs of len_i * len_j (DP cells, nominal)     */
     int64_t cells_kept;        /* same over the kept pairs                                    */
     int64_t columns_kept;      /* sum over kept pairs of the text length (nominal columns)    */
@@ -134,7 +136,8 @@ typedef struct tcrnet_stats {
     int64_t lane_tests_exec;   /* 32 x warp-level early-exit tests executed (COUNT_WORK only) */
     int64_t lane_pairs_exec;   /* 32 x warp-level first-column steps (3-LOP3 form; COUNT_WORK) */
     int64_t lane_prefix_tests_exec; /* 32 x warp-level trie-node exit tests (COUNT_WORK only)  */
-    int64_t work_items;        /* CTAs of the distance kernels                                */
+    int64_t work_items;        /* work items of the distance kernels (text-chunk kernel: one
+                                  CTA of 256 patterns; prefix-trie kernel: one warp of 32)     */
     int64_t work_items_trie;   /* ... of which prefix-trie kernel                             */
     int64_t trie_nodes;        /* nodes of the prefix trie built by the last load             */
     int32_t distance_passes;   /* 1, or 2 if the edge buffer had to grow                      */
