@@ -339,6 +339,8 @@ def main() -> None:
                 "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.workload), "kernel": "k_distance_trie" if work["work_items_trie"] else "k_distance", "kernel_ms": ms_kernel,
                 "peak_source": f"{n_sm} SMs x {ALU_LANES_PER_SM} lanes x {peaks['sm_max_mhz']} MHz ({peak_kind} sm_max_mhz)",
                 "alu_ops_per_launch": alu_ops, "measured_pipe_peaks": probes,
+                # also against the issue-slot ceiling (4 schedulers x 32 lanes per SM and clock)
+                "issue_ceiling": 2 * peak, "frac_of_issue_ceiling": achieved / (2 * peak),
             },
             "detail": {
                 "pairs_kept": work["pairs_kept"], "cells_kept": work["cells_kept"], "cells_all": work["cells_all"],
