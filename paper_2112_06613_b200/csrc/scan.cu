@@ -1,5 +1,8 @@
-// Device-wide exclusive prefix sums (used for row offsets, split histograms).
-// Three launches: per-tile sums -> scan of the tile sums by one CTA -> per-tile scan + offset.
+// Device-wide exclusive prefix sums (row offsets, ranks of the distinct sequences, group and CSR row starts).
+// Long inputs, three launches: per-tile sums -> scan of the tile sums by one CTA -> per-tile scan + offset.
+// Up to kFusedTiles tiles of 1024 (every scan at TCR scale), two launches: per-tile sums -> per-tile scan, each
+// CTA adding up the sums of the tiles before it itself (<= 8 loads per thread): these scans are latency-bound,
+// so a launch less and four times as many CTAs matter more than the re-read sums.
 // HBM-bound streaming passes: 2 reads + 1 write of the array.
 #include "tcrnet_internal.h"
 
@@ -7,8 +10,8 @@ namespace tcrnet {
 namespace {
 
 constexpr int kScanThreads = 256;
-constexpr int kScanItems = 16;
-constexpr int kScanTile = kScanThreads * kScanItems;  // 4096
+constexpr int64_t kFusedTiles = 2048;  // short path: n <= 2,097,152
+__host__ __device__ constexpr int scan_items(bool fused) { return fused ? 4 : 16; }  // per thread: tiles of 1024 / 4096
 
 template <typename T>
 __device__ __forceinline__ T warp_inclusive(T v) {
@@ -40,9 +43,10 @@ __device__ __forceinline__ T block_exclusive(T v, T* warp_sums /*[32]*/, T* tota
     return r;
 }
 
-template <typename TIn, typename TOut>
+template <typename TIn, typename TOut, bool FUSED>
 __global__ void __launch_bounds__(kScanThreads) k_tile_sums(const TIn* __restrict__ in, int64_t n,
                                                            TOut* __restrict__ tile_sums) {
+    constexpr int kScanItems = scan_items(FUSED), kScanTile = kScanThreads * kScanItems;
     __shared__ TOut ws[32];
     __shared__ TOut tot;
     const int64_t base = (int64_t)blockIdx.x * kScanTile;
@@ -72,14 +76,26 @@ __global__ void __launch_bounds__(1024) k_scan_tile_sums(TOut* __restrict__ tile
     }
 }
 
-template <typename TIn, typename TOut>
+// FUSED: tile_sums holds the plain sums and this CTA adds up those of the tiles before it; else their exclusive scan.
+template <typename TIn, typename TOut, bool FUSED>
 __global__ void __launch_bounds__(kScanThreads) k_tile_scan(const TIn* __restrict__ in, TOut* __restrict__ out,
                                                            int64_t n, const TOut* __restrict__ tile_sums,
                                                            int write_total) {
+    constexpr int kScanItems = scan_items(FUSED), kScanTile = kScanThreads * kScanItems;
     __shared__ TOut ws[32];
     __shared__ TOut tot;
     __shared__ TOut stage[kScanTile];
     const int64_t base = (int64_t)blockIdx.x * kScanTile;
+    TOut tile_base;
+    if (FUSED) {
+        TOut before = 0;
+        for (unsigned t = threadIdx.x; t < blockIdx.x; t += kScanThreads) before += tile_sums[t];
+        block_exclusive(before, ws, &tot);
+        tile_base = tot;
+        __syncthreads();  // tot is reused below
+    } else {
+        tile_base = tile_sums[blockIdx.x];
+    }
     // coalesced load into shared memory, then each thread owns kScanItems consecutive items
 #pragma unroll
     for (int k = 0; k < kScanItems; ++k) {
@@ -95,7 +111,7 @@ __global__ void __launch_bounds__(kScanThreads) k_tile_scan(const TIn* __restric
         local[k] = acc;
         acc += stage[threadIdx.x * kScanItems + k];
     }
-    TOut ex = block_exclusive(acc, ws, &tot) + tile_sums[blockIdx.x];
+    TOut ex = block_exclusive(acc, ws, &tot) + tile_base;
 #pragma unroll
     for (int k = 0; k < kScanItems; ++k) stage[threadIdx.x * kScanItems + k] = local[k] + ex;
     __syncthreads();
@@ -105,7 +121,7 @@ __global__ void __launch_bounds__(kScanThreads) k_tile_scan(const TIn* __restric
         int64_t i = base + idx;
         if (i < n) out[i] = stage[idx];
     }
-    if (write_total && blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) out[n] = tile_sums[blockIdx.x] + tot;
+    if (write_total && blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) out[n] = tile_base + tot;
 }
 
 template <typename TIn, typename TOut>
@@ -115,11 +131,19 @@ cudaError_t scan_impl(const TIn* in, TOut* out, int64_t n, bool write_total, voi
         if (write_total) return cudaMemsetAsync(out, 0, sizeof(TOut), s);
         return cudaSuccess;
     }
-    const int64_t tiles = (n + kScanTile - 1) / kScanTile;
     TOut* sums = static_cast<TOut*>(scratch);
-    k_tile_sums<TIn, TOut><<<(unsigned)tiles, kScanThreads, 0, s>>>(in, n, sums);
+    const int64_t small_tile = kScanThreads * scan_items(true), big_tile = kScanThreads * scan_items(false);
+    if ((n + small_tile - 1) / small_tile <= kFusedTiles) {
+        const int64_t tiles = (n + small_tile - 1) / small_tile;
+        k_tile_sums<TIn, TOut, true><<<(unsigned)tiles, kScanThreads, 0, s>>>(in, n, sums);
+        k_tile_scan<TIn, TOut, true><<<(unsigned)tiles, kScanThreads, 0, s>>>(in, out, n, sums, write_total ? 1 : 0);
+        *launches += 2;
+        return cudaGetLastError();
+    }
+    const int64_t tiles = (n + big_tile - 1) / big_tile;
+    k_tile_sums<TIn, TOut, false><<<(unsigned)tiles, kScanThreads, 0, s>>>(in, n, sums);
     k_scan_tile_sums<TOut><<<1, 1024, 0, s>>>(sums, tiles);
-    k_tile_scan<TIn, TOut><<<(unsigned)tiles, kScanThreads, 0, s>>>(in, out, n, sums, write_total ? 1 : 0);
+    k_tile_scan<TIn, TOut, false><<<(unsigned)tiles, kScanThreads, 0, s>>>(in, out, n, sums, write_total ? 1 : 0);
     *launches += 3;
     return cudaGetLastError();
 }
@@ -127,7 +151,8 @@ cudaError_t scan_impl(const TIn* in, TOut* out, int64_t n, bool write_total, voi
 }  // namespace
 
 size_t scan_scratch_bytes(int64_t n) {
-    int64_t tiles = (n + kScanTile - 1) / kScanTile;
+    const int64_t tile = kScanThreads * scan_items(true);  // the smaller tile: an upper bound for both paths
+    const int64_t tiles = (n + tile - 1) / tile;
     return (size_t)(tiles > 0 ? tiles : 1) * sizeof(int64_t);
 }
 
