@@ -13,7 +13,7 @@
 //   k_trie_lcp    lcp8[s] = number of leading residues sorted position s shares with s-1
 //                 (0 at the first position of a bucket, kTrieDepth when >= kTrieDepth are shared);
 //                 s starts a level-k run iff lcp8[s] < k.
-//   k_trie_count  per tile of 4096 positions, the number of run starts of every level.
+//   k_trie_count  per tile of 1024 positions, the number of run starts of every level.
 //   k_trie_scan   exclusive scan of the tile counts (one CTA), totals, sentinels.
 //   k_trie_emit   node ids by ranking inside the tile; writes the nodes.
 //   k_trie_child_codes  per node of levels 1..kTrieDepth-1, the bitmap of its children's residue codes
@@ -24,8 +24,9 @@ namespace tcrnet {
 namespace {
 
 constexpr int kThreads = 256;
-constexpr int kItems = 16;                     // positions per thread: one 128-bit load of lcp8
-constexpr int kTile = kThreads * kItems;       // 4096
+constexpr int kItems = 4;                      // positions per thread: one 32-bit load of lcp8 (short serial chains:
+                                               // these kernels are latency-bound at TCR scale)
+constexpr int kTile = kThreads * kItems;       // 1024
 constexpr int kCountStride = 8;                // uint32 per tile in tile_counts ([1..kTrieDepth] used)
 static_assert(kTrieDepth <= 6, "level counts are packed as 4 x 16 bit + 2 x 16 bit");
 
@@ -60,7 +61,7 @@ __global__ void __launch_bounds__(kThreads) k_trie_lcp(const uint32_t* __restric
 }
 
 // Run-start flags of one position packed as counters: level k in bits 16(k-1).. of lo (k = 1..4) and
-// bits 16(k-5).. of hi (k = 5, 6).  A tile has 4096 positions, so 16 bits per counter suffice.
+// bits 16(k-5).. of hi (k = 5, 6).  A tile has 1024 positions, so 16 bits per counter suffice.
 struct Packed {
     unsigned long long lo;
     uint32_t hi;
@@ -78,12 +79,12 @@ __device__ __forceinline__ uint32_t level_count(const Packed& p, int k) {
     return k <= 4 ? (uint32_t)(p.lo >> (16 * (k - 1))) & 0xffffu : (p.hi >> (16 * (k - 5))) & 0xffffu;
 }
 
-// 16 lcp values of this thread (255 = beyond n: starts nothing)
+// the kItems lcp values of this thread (255 = beyond n: starts nothing)
 __device__ __forceinline__ void load_lcp16(const uint8_t* lcp8, int64_t first, int64_t n, uint32_t* v) {
-    const uint4 q = *reinterpret_cast<const uint4*>(lcp8 + first);  // the buffer is padded to a multiple of 16
-    const uint32_t w[4] = {q.x, q.y, q.z, q.w};
+    static_assert(kItems == 4, "one 32-bit load");
+    const uint32_t w = *reinterpret_cast<const uint32_t*>(lcp8 + first);  // the buffer is padded to a multiple of 16
 #pragma unroll
-    for (int i = 0; i < kItems; ++i) v[i] = first + i < n ? (w[i >> 2] >> (8 * (i & 3))) & 0xffu : 255u;
+    for (int i = 0; i < kItems; ++i) v[i] = first + i < n ? (w >> (8 * i)) & 0xffu : 255u;
 }
 
 // Exclusive scan of one Packed per thread across the CTA; *total = CTA sum.
