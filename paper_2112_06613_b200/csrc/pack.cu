@@ -120,7 +120,7 @@ __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residu
 cudaError_t launch_length_hist(const int32_t* lengths, int64_t n, const uint32_t* n_dev, unsigned long long* hist,
                                uint32_t* flags, cudaStream_t s, int* launches) {
     int64_t blocks = (n + 255) / 256;
-    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks > kGridSMs * 8) blocks = kGridSMs * 8;
     k_length_hist<<<(unsigned)blocks, 256, 0, s>>>(lengths, n, n_dev, hist, flags);
     *launches += 1;
     return cudaGetLastError();

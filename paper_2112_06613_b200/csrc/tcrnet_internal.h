@@ -20,6 +20,7 @@ constexpr int kSortPrefix = 6;           // residues of the lexicographic sub-or
 constexpr int kTrieDepth = kSortPrefix;  // levels 1..kTrieDepth of the prefix trie over each text bucket
 constexpr int kTrieFan = 27;             // staging slots per trie level, indexed by residue code (0..26)
 constexpr int kTrieMaxL = 4;             // the trie kernel is specialised on l_max = 0..kTrieMaxL
+constexpr int kGridSMs = 148;            // B200: grid-stride kernels are sized in multiples of the SM count
 constexpr int kTrieTile = 32;            // patterns per work item of the trie kernel: one warp
 constexpr int kTrieQueues = 8;           // dynamic work queues (one per trie launch of a distance pass)
 constexpr uint32_t kGroupFlag = 0x80000000u;  // perm entry = kGroupFlag | uid: a sequence shared by several rows (dedup.cu)
