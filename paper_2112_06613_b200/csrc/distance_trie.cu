@@ -95,11 +95,6 @@ __device__ __forceinline__ void sts128(uint32_t addr, uint32_t x, uint32_t y, ui
 }
 // Pin a value in a register: the compiler may not recompute it from its definition (threadIdx, the shared window).
 __device__ __forceinline__ void keep(uint32_t& x) { asm volatile("" : "+r"(x)); }
-__device__ __forceinline__ uint32_t top_bit(uint32_t x) {  // index of the highest set bit (x != 0)
-    uint32_t r;
-    asm("bfind.u32 %0, %1;" : "=r"(r) : "r"(x));
-    return r;
-}
 
 // Columns j0 + Q0 .. j0 + 3 of one text (residue codes c4; FULL: all of them exist, else only those < n).
 // Returns false when the exit vote kills the text (dg > l_max in all 32 lanes).
