@@ -146,7 +146,8 @@ __global__ void __launch_bounds__(256) k_dedup_codes(int32_t* __restrict__ perm,
 }
 
 // Edges between the rows of one sequence: the thread of member slot x joins it to the slots after it.  Output
-// offsets: warp scan + one atomicAdd per warp.
+// offsets: warp scan + one atomicAdd per warp.  Counting for the CSR step is done per ROW, not per edge: row r
+// of a group has one edge to every other row of it, the larger ones count for row_count[r], the smaller for deg[r].
 __global__ void __launch_bounds__(256) k_emit_cliques(const int32_t* __restrict__ members,
                                                      const int32_t* __restrict__ uid_of,
                                                      const uint32_t* __restrict__ group_start, int64_t n,
@@ -157,11 +158,20 @@ __global__ void __launch_bounds__(256) k_emit_cliques(const int32_t* __restrict_
     constexpr uint32_t kFullMask = 0xffffffffu;
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
-    uint32_t r = 0, end = 0, rest = 0;
+    uint32_t r = 0, begin = 0, end = 0, rest = 0;
     if (s < n) {
         r = (uint32_t)members[s];
-        end = group_start[(uint32_t)uid_of[r] + 1u];
+        const uint32_t uid = (uint32_t)uid_of[r];
+        begin = group_start[uid];
+        end = group_start[uid + 1u];
         rest = end - 1u - (uint32_t)s;  // slots after this one
+    }
+    if (end - begin > 1u) {
+        uint32_t larger = 0;
+        for (uint32_t y = begin; y < end; ++y) larger += (uint32_t)members[y] > r;
+        const uint32_t smaller = end - begin - 1u - larger;
+        if (larger) atomicAdd(row_count + r, (int)larger);
+        if (smaller) atomicAdd(deg + r, (int)smaller);
     }
     if (!__any_sync(kFullMask, rest != 0u)) return;
     unsigned long long incl = rest;
@@ -176,8 +186,6 @@ __global__ void __launch_bounds__(256) k_emit_cliques(const int32_t* __restrict_
     for (uint32_t y = (uint32_t)s + 1u; y < end; ++y, ++pos) {
         const uint32_t q = (uint32_t)members[y];
         const uint32_t a = min(r, q), b = max(r, q);
-        atomicAdd(row_count + a, 1);
-        atomicAdd(deg + b, 1);
         if (pos < edge_cap) edges[pos] = ((unsigned long long)a << 32) | b;
     }
 }
