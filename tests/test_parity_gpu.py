@@ -404,6 +404,18 @@ def test_cfg4_sampled_headline_config(pkg, oracle):
     assert st["distance_passes"] == 1
 
 
+def test_cfg4_whole_network_is_the_same_row_by_row(pkg):
+    """At the full headline size the collapsed build (the default, what bench.py times) equals, byte for byte, the
+    build that takes every row as its own pattern / text (two independent paths
+    through the kernels; the oracle covers sampled neighbourhoods of the same network in the test above)."""
+    d = generate("cfg4")
+    on, st_on = gpu_network(pkg, d.residues, d.lengths, 1)
+    off, st_off = gpu_network(pkg, d.residues, d.lengths, 1, {pkg.OPT_DEDUP: 0})
+    assert st_on["n_distinct"] < st_off["n_distinct"] == d.n
+    assert_same_network(on, off)
+    check_csr_invariants(*on, d.n)
+
+
 def test_cfg5_sampled(pkg, oracle):
     """N = 2,000,000, l_max = 3, lengths 5..40 (patterns > 32 use 64-bit words)."""
     _sampled_parity(pkg, oracle, "cfg5", 3, 24, 5)
