@@ -38,7 +38,7 @@ __global__ void __launch_bounds__(256) k_length_hist(const int32_t* __restrict__
         if (h[i]) atomicAdd(&hist[i], (unsigned long long)h[i]);
 }
 
-// Sort key of the sequence sort: (clamped length, first kSortPrefix residues as 5-bit digits, 0 = past the
+// Sort key of the sequence sort: (length - 1 in 6 bits, first kSortPrefix residues as 5-bit digits, 0 = past the
 // end, 27 = not a letter); the payload of row i is i.  Invalid lengths / residues are reported by
 // k_length_hist / k_pack, here they only have to land somewhere.
 __global__ void __launch_bounds__(256) k_seq_keys(const uint8_t* __restrict__ residues,
@@ -48,9 +48,9 @@ __global__ void __launch_bounds__(256) k_seq_keys(const uint8_t* __restrict__ re
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     int32_t l = lengths[i];
-    if (l < 1 || l > kMaxLen) l = 0;
+    if (l < 1 || l > kMaxLen) l = 0;  // (the load fails on such a row; it only has to land somewhere)
     const uint8_t* src = residues + offsets[i];
-    unsigned long long key = (unsigned long long)(uint32_t)l;
+    unsigned long long key = (unsigned long long)(uint32_t)(l > 0 ? l - 1 : 0);
 #pragma unroll
     for (int k = 0; k < kSortPrefix; ++k) {
         uint32_t d = 0u;

@@ -1,8 +1,8 @@
-// Stable LSD radix sort over 8-bit digits of 64-bit keys, with an optional 32-bit payload: the sequence
+// Stable LSD radix sort over kRadixBits-bit (9) digits of 64-bit keys, with an optional 32-bit payload: the sequence
 // sort of step A1 (composite (length, first residues) keys, payload = caller's row).  HBM/L2-bound
 // streaming; three launches per pass, no spinning on other CTAs:
 //
-//   k_radix_hist     per tile of 4096 (1024 for short inputs) keys, the 256 digit counts (shared-memory atomics), stored digit-major
+//   k_radix_hist     per tile of 4096 (1024 for short inputs) keys, the 512 digit counts (shared-memory atomics), stored digit-major
 //                    (hist[d * tiles + tile]) and added to the pass's global digit totals;
 //   k_radix_scan     CTA d turns row d of `hist` into global output positions: the total of all smaller
 //                    digits (from the global totals) + the exclusive prefix over the tiles;
@@ -20,6 +20,8 @@ namespace {
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
 constexpr uint32_t kFull = 0xffffffffu;
+constexpr int kDigits = 1 << kRadixBits;  // 512: the 36-bit sequence key takes 4 passes
+static_assert(kDigits % kThreads == 0 && kDigits <= 0x8000, "digit loops stride by the CTA; rank | digit << 16");
 // keys per thread (ROUNDS): 16 for long inputs (4096 keys per CTA, 512 consecutive keys per warp); 4 below
 // kSmallN keys, where 4096-key tiles would leave most SMs without a CTA and every pass is latency-bound
 constexpr int64_t kSmallN = (int64_t)1 << 22;
@@ -30,19 +32,21 @@ __global__ void __launch_bounds__(kThreads) k_radix_hist(const unsigned long lon
                                                         int shift, uint32_t* __restrict__ hist,
                                                         uint32_t* __restrict__ totals, uint32_t tiles) {
     constexpr int kTile = kThreads * kRounds;
-    __shared__ uint32_t h[256];
-    h[threadIdx.x] = 0;
+    __shared__ uint32_t h[kDigits];
+    for (int d = threadIdx.x; d < kDigits; d += kThreads) h[d] = 0;
     __syncthreads();
     const int64_t base = (int64_t)blockIdx.x * kTile;
 #pragma unroll 4
     for (int r = 0; r < kRounds; ++r) {
         const int64_t i = base + (int64_t)r * kThreads + threadIdx.x;
-        if (i < n) atomicAdd(&h[(uint32_t)(keys[i] >> shift) & 255u], 1u);
+        if (i < n) atomicAdd(&h[(uint32_t)(keys[i] >> shift) & (uint32_t)(kDigits - 1)], 1u);
     }
     __syncthreads();
-    const uint32_t c = h[threadIdx.x];
-    hist[(size_t)threadIdx.x * tiles + blockIdx.x] = c;
-    if (c) atomicAdd(&totals[threadIdx.x], c);
+    for (int d = threadIdx.x; d < kDigits; d += kThreads) {
+        const uint32_t c = h[d];
+        hist[(size_t)d * tiles + blockIdx.x] = c;
+        if (c) atomicAdd(&totals[d], c);
+    }
 }
 
 // Row d of hist (tiles entries) -> first output slot of (digit d, tile t), in place.
@@ -51,7 +55,8 @@ __global__ void __launch_bounds__(kThreads) k_radix_scan(uint32_t* __restrict__ 
     __shared__ uint32_t wsum[kWarps];
     const uint32_t d = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // total of the smaller digits
-    uint32_t below = tid < d ? totals[tid] : 0u;
+    uint32_t below = 0u;
+    for (uint32_t t = tid; t < d; t += kThreads) below += totals[t];
     below = __reduce_add_sync(kFull, below);
     if (lane == 0) wsum[warp] = below;
     __syncthreads();
@@ -90,10 +95,12 @@ __global__ void __launch_bounds__(kThreads) k_radix_scatter(const unsigned long 
                                                            int32_t* __restrict__ vals_out, int64_t n, int shift,
                                                            const uint32_t* __restrict__ scanned, uint32_t tiles) {
     constexpr int kTile = kThreads * kRounds, kWarpItems = 32 * kRounds;
-    __shared__ uint32_t wh[kWarps][256];  // per warp: running digit counts, then first output slots
+    __shared__ uint32_t wh[kWarps][kDigits];  // per warp: running digit counts, then first output slots
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int d = tid; d < kDigits; d += kThreads) {
 #pragma unroll
-    for (int w = 0; w < kWarps; ++w) wh[w][tid] = 0;
+        for (int w = 0; w < kWarps; ++w) wh[w][d] = 0;
+    }
     __syncthreads();
     const int64_t first = (int64_t)blockIdx.x * kTile + (int64_t)warp * kWarpItems + lane;
     const uint32_t lt = (1u << lane) - 1u;
@@ -104,7 +111,7 @@ __global__ void __launch_bounds__(kThreads) k_radix_scatter(const unsigned long 
         const int64_t i = first + r * 32;
         const bool valid = i < n;
         key[r] = valid ? keys_in[i] : 0ull;
-        const uint32_t d = valid ? (uint32_t)(key[r] >> shift) & 255u : 256u + lane;  // invalid lanes match nobody
+        const uint32_t d = valid ? (uint32_t)(key[r] >> shift) & (uint32_t)(kDigits - 1) : kDigits + lane;  // invalid lanes match nobody
         const uint32_t peers = __match_any_sync(kFull, d);
         const int leader = __ffs((int)peers) - 1;
         uint32_t old = 0;
@@ -117,12 +124,12 @@ __global__ void __launch_bounds__(kThreads) k_radix_scatter(const unsigned long 
         __syncwarp();
     }
     __syncthreads();
-    {
-        uint32_t run = scanned[(size_t)tid * tiles + blockIdx.x];
+    for (int d = tid; d < kDigits; d += kThreads) {
+        uint32_t run = scanned[(size_t)d * tiles + blockIdx.x];
 #pragma unroll
         for (int w = 0; w < kWarps; ++w) {
-            const uint32_t c = wh[w][tid];
-            wh[w][tid] = run;
+            const uint32_t c = wh[w][d];
+            wh[w][d] = run;
             run += c;
         }
     }
@@ -145,7 +152,7 @@ int64_t radix_tiles(int64_t n) {
 }
 
 size_t radix_scratch_bytes(int64_t n) {
-    return ((size_t)radix_tiles(n) * 256 + (size_t)kRadixMaxPasses * 256) * sizeof(uint32_t);
+    return ((size_t)radix_tiles(n) * kDigits + (size_t)kRadixMaxPasses * kDigits) * sizeof(uint32_t);
 }
 
 cudaError_t radix_sort_u64(unsigned long long* keys_a, unsigned long long* keys_b, int32_t* vals_a, int32_t* vals_b,
@@ -155,16 +162,16 @@ cudaError_t radix_sort_u64(unsigned long long* keys_a, unsigned long long* keys_
     if (n <= 1 || n_passes <= 0) return cudaSuccess;
     if (n_passes > kRadixMaxPasses || n > 0x7fffffffLL) return cudaErrorInvalidValue;
     const uint32_t tiles = (uint32_t)radix_tiles(n);
-    uint32_t* totals = (uint32_t*)scratch;                 // [kRadixMaxPasses][256]
-    uint32_t* hist = totals + kRadixMaxPasses * 256;       // [256][tiles]
-    cudaError_t e = cudaMemsetAsync(totals, 0, sizeof(uint32_t) * kRadixMaxPasses * 256, s);
+    uint32_t* totals = (uint32_t*)scratch;                     // [kRadixMaxPasses][kDigits]
+    uint32_t* hist = totals + kRadixMaxPasses * kDigits;       // [kDigits][tiles]
+    cudaError_t e = cudaMemsetAsync(totals, 0, sizeof(uint32_t) * kRadixMaxPasses * kDigits, s);
     if (e != cudaSuccess) return e;
     const bool has_val = vals_a != nullptr;
     const bool small = rounds_for(n) == 4;
     for (int p = 0; p < n_passes; ++p) {
-        if (small) k_radix_hist<4><<<tiles, kThreads, 0, s>>>(keys_a, n, shifts[p], hist, totals + p * 256, tiles);
-        else k_radix_hist<16><<<tiles, kThreads, 0, s>>>(keys_a, n, shifts[p], hist, totals + p * 256, tiles);
-        k_radix_scan<<<256, kThreads, 0, s>>>(hist, totals + p * 256, tiles);
+        if (small) k_radix_hist<4><<<tiles, kThreads, 0, s>>>(keys_a, n, shifts[p], hist, totals + p * kDigits, tiles);
+        else k_radix_hist<16><<<tiles, kThreads, 0, s>>>(keys_a, n, shifts[p], hist, totals + p * kDigits, tiles);
+        k_radix_scan<<<kDigits, kThreads, 0, s>>>(hist, totals + p * kDigits, tiles);
         if (has_val && small)
             k_radix_scatter<true, 4><<<tiles, kThreads, 0, s>>>(keys_a, keys_b, vals_a, vals_b, n, shifts[p], hist, tiles);
         else if (has_val)

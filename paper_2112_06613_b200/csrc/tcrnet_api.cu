@@ -136,9 +136,9 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
         d_off = (const int64_t*)offsets.p;
     }
     {
-        constexpr int kPasses = (kSeqKeyBits + 7) / 8;
+        constexpr int kPasses = (kSeqKeyBits + kRadixBits - 1) / kRadixBits;
         int shifts[kPasses];
-        for (int p = 0; p < kPasses; ++p) shifts[p] = 8 * p;
+        for (int p = 0; p < kPasses; ++p) shifts[p] = kRadixBits * p;
         // an odd number of passes ends in the b buffers: make those set.perm
         int32_t* va = (int32_t*)(kPasses & 1 ? ctx->perm_tmp.p : set.perm.p);
         int32_t* vb = (int32_t*)(kPasses & 1 ? set.perm.p : ctx->perm_tmp.p);

@@ -114,10 +114,11 @@ cudaError_t exclusive_scan_u32(const uint32_t* in, uint32_t* out, int64_t n, voi
 cudaError_t exclusive_scan_u32_total(const uint32_t* in, uint32_t* out /*[n+1]*/, int64_t n, void* scratch,
                                      cudaStream_t s, int* launches);
 
-// radix.cu: stable LSD radix sort of 64-bit keys (optional 32-bit payload) over the 8-bit digits
-// (key >> shifts[p]) & 255, p = 0..n_passes-1 in that order.  Ping-pongs between the a and b buffers;
+// radix.cu: stable LSD radix sort of 64-bit keys (optional 32-bit payload) over the kRadixBits-bit digits
+// (key >> shifts[p]) & (2^kRadixBits - 1), p = 0..n_passes-1 in that order.  Ping-pongs between the a and b buffers;
 // *result_in_b says where the sorted sequence ends up.  scratch: radix_scratch_bytes(n).
 constexpr int kRadixMaxPasses = 8;
+constexpr int kRadixBits = 9;
 size_t radix_scratch_bytes(int64_t n);
 cudaError_t radix_sort_u64(unsigned long long* keys_a, unsigned long long* keys_b, int32_t* vals_a, int32_t* vals_b,
                            int64_t n, const int* shifts, int n_passes, void* scratch, cudaStream_t s, int* launches,
@@ -127,8 +128,8 @@ cudaError_t radix_sort_u64(unsigned long long* keys_a, unsigned long long* keys_
 // n_dev (may be NULL): device count of rows, at most n
 cudaError_t launch_length_hist(const int32_t* lengths, int64_t n, const uint32_t* n_dev,
                                unsigned long long* hist /*[kNumLen]*/, uint32_t* flags, cudaStream_t s, int* launches);
-// sort key of row i: (clamped length << 30) | the first kSortPrefix residues, 5 bits each (0 = past the end); vals[i] = i
-constexpr int kSeqKeyBits = 6 + 5 * kSortPrefix;
+// sort key of row i: ((length - 1) << 30, invalid lengths: 0) | the first kSortPrefix residues, 5 bits each (0 = past the end); vals[i] = i
+constexpr int kSeqKeyBits = 6 + 5 * kSortPrefix;  // length - 1 (0..63) takes 6 bits
 cudaError_t launch_seq_keys(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths, int64_t n,
                             unsigned long long* keys, int32_t* vals, cudaStream_t s, int* launches);
 cudaError_t launch_pack(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths,
