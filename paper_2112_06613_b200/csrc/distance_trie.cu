@@ -63,7 +63,7 @@ __host__ __device__ constexpr int trie_peq_row_bytes() {
 }
 template <typename W>
 __host__ __device__ constexpr int trie_warp_smem_bytes() {
-    return ((kPeqRows * trie_peq_row_bytes<W>() + 15) & ~15) + kTrieDepth * kTrieFan * 16;
+    return ((kPeqRows * trie_peq_row_bytes<W>() + 15) & ~15) + kTrieDepth * kTrieFan * 16 + kTrieDepth * 128;
 }
 constexpr int kClipLevels = 3;      // levels whose nodes are clipped to the work item's text chunk
 constexpr int kDeadLane = 1 << 20;  // dg of a lane without a pattern: never alive, never emitted
@@ -74,7 +74,8 @@ struct Walk {
     uint32_t lane_addr;       // shared address of this lane's Peq column
     const uint32_t* rows;     // text row of sorted position 0 of this bucket's numbering (bucket base - t_start rows)
     uint32_t lo, hi;          // texts [lo, hi) (sorted positions) are this warp's share of the bucket
-    uint32_t ohs[kTrieDepth + 1];   // [q] = 1 << code of pattern row q - delta (0: no such row / no pattern)
+    uint32_t ohs_addr;        // shared address of this lane's one-hot codes: [q - 1] = 1 << code of pattern row q - delta
+                              // (0: no such row / no pattern), q = 1..kTrieDepth, stride 128 B
     uint32_t dsh;             // delta + 1: the bit of pattern row q - delta is (1 << q) >> dsh (0 when q <= delta)
     W pv_init;
     int rw, n;
@@ -89,6 +90,14 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
     uint4 v;
     asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
     return v;
+}
+__device__ __forceinline__ uint32_t lds32(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void sts32(uint32_t addr, uint32_t v) {
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
 __device__ __forceinline__ void sts128(uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
     asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
@@ -173,11 +182,11 @@ __device__ __forceinline__ void visit(Walk<W, COUNT>& w, const DistanceParams& P
     // while LEVEL <= l_max (D[i][k] <= k); LEVEL > l_max >= delta, so row i = LEVEL - delta exists.
     if constexpr (LEVEL > LMAX) {
         const uint32_t b = w.dbit(LEVEL);
-        uint32_t V = w.ohs[LEVEL];
+        uint32_t V = lds32(w.ohs_addr + (LEVEL - 1) * 128);
 #pragma unroll
         for (int t = 1; t <= LMAX / 2; ++t) {
             const uint32_t run = b - (b >> t);  // bits i-1-t .. i-2 (b itself when there is no row i-t: ohs = 0)
-            if (((uint32_t)Pv & run) == run) V |= w.ohs[LEVEL - t];
+            if (((uint32_t)Pv & run) == run) V |= lds32(w.ohs_addr + (LEVEL - t - 1) * 128);
         }
         if (dg != LMAX) V = 0u;
         if (dg < LMAX || (dg == LMAX && ((uint32_t)Mv & b) != 0u)) V = kFull;
@@ -252,8 +261,10 @@ __global__ void __launch_bounds__(kTrieThreads, sizeof(W) == 4 ? 4 : 2) k_distan
     Walk<W, COUNT> w;
     w.stage_addr = peq_addr + ((kPeqRows * kRowBytes + 15) & ~15);
     w.lane_addr = peq_addr + lane * (uint32_t)sizeof(W);
+    w.ohs_addr = w.stage_addr + kTrieDepth * kTrieFan * 16 + lane * 4u;
     keep(w.stage_addr);
     keep(w.lane_addr);
+    keep(w.ohs_addr);
     w.lane = lane;
     {
         uint32_t l = (uint32_t)w.lane;
@@ -301,7 +312,7 @@ __global__ void __launch_bounds__(kTrieThreads, sizeof(W) == 4 ? 4 : 2) k_distan
                 const int r = k - delta;  // 1-based pattern row
                 uint32_t code = 0xffu;
                 if (r >= 1 && r <= m) code = ((r <= 4 ? head.x : head.y) >> (8 * ((r - 1) & 3))) & 0xffu;
-                w.ohs[k] = code < 32u ? 1u << code : 0u;
+                if (k >= 1) sts32(w.ohs_addr + (k - 1) * 128, code < 32u ? 1u << code : 0u);
             }
         }
         w.pv_init = low_mask<W>(m);
