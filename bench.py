@@ -39,8 +39,8 @@ ALU_OPS_PER_TEST = 4           # 2 LOP3 + IADD3 + ISETP per pair and early-exit 
 ALU_OPS_PER_PREFIX_TEST = 2    # LOP3 + ISETP per pair and DP cell read in a guided expansion (distance_trie.cu)
 ORACLE_SAMPLE_ROWS = 1024
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_distance_trie launch at cfg4, from the ncu --set full
-# capture summarised in profiles/r1e_trie_ncu.txt (65.39 MB + 3.71 MB)
-NCU_DRAM_BYTES_PER_LAUNCH = {"cfg4": 69_096_704}
+# capture summarised in profiles/r1e_trie_ncu.txt (65.39 MB + 3.55 MB)
+NCU_DRAM_BYTES_PER_LAUNCH = {"cfg4": 68_938_240}
 
 
 def _peaks():
