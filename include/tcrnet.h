@@ -108,13 +108,28 @@ typedef enum tcrnet_option {
                                      endpoint (query-query and query-repertoire); pairs of two
                                      non-query rows are never evaluated.  0 (default): all pairs.
                                      Takes effect at the next tcrnet_load.                      */
-    TCRNET_OPT_DEDUP = 10         /* 1 (default): rows with identical sequences are collapsed at
+    TCRNET_OPT_DEDUP = 10,        /* 1 (default): rows with identical sequences are collapsed at
                                      load; the distance step runs over the distinct sequences and
                                      the emission multiplies every surviving pair by the rows
                                      behind it (reading Q3: one node per row, duplicates joined
                                      for every l_max >= 0).  0: every row is its own pattern /
                                      text.  Never changes the result.  Ignored (off) in the
                                      rectangular mode.  Takes effect at the next load.          */
+    TCRNET_OPT_SEGMENT_JOIN = 11, /* exact candidate filter in front of the distance kernel: a text cut
+                                     into l_max + 1 segments shares at least one of them, unchanged and
+                                     shifted by at most the edits allow, with every sequence within
+                                     l_max of it; only pairs found through a hash index of the segments
+                                     are handed to the column recurrence.  -1 (default): used for
+                                     2 <= l_max <= 4 (all-pairs mode, early exit on); 1: also for
+                                     l_max <= 1; 0: never (every length-compatible pair is visited
+                                     through the prefix trie / text-chunk kernels).  Never changes the
+                                     result.                                                      */
+    TCRNET_OPT_FAST_L1 = 12       /* 1: builds with l_max <= 1 go through the segment
+                                     join and decide each candidate WITHOUT the recurrence - equal
+                                     lengths: XOR of the 5-bit packed codes confined to one residue;
+                                     lengths differing by one: common prefix + common suffix cover the
+                                     shorter sequence.  0 (default).  Never changes the result; its
+                                     time is reported beside, not inside, the cell-update metrics.  */
 } tcrnet_option;
 
 /* Work and timing of the last tcrnet_load / tcrnet_build (tcrnet_get_stats). */
@@ -153,7 +168,16 @@ typedef struct tcrnet_stats {
     float ms_kernel;           /* the distance kernel launches alone (CUDA events right around
                                   them; ms_distance adds the schedule upload, the counter
                                   resets and the expansion of collapsed pairs)               */
-    float pad_;
+    float ms_index;            /* segment join: building the segment index (inside ms_distance)  */
+    int64_t lane_columns_live; /* column steps of lanes whose pair was still undecided (COUNT_WORK;
+                                  join kernel; the trie / chunk kernels report warp-level counts)   */
+    int64_t join_probes;       /* segment join: directory look-ups (COUNT_WORK)                  */
+    int64_t join_entries;      /* ... directory entries read (COUNT_WORK)                        */
+    int64_t join_candidates;   /* ... pairs handed to the recurrence / the l_max <= 1 check        */
+    int64_t work_items_join;   /* work items (32 patterns) of the join kernels                    */
+    int64_t join_index_entries;/* (text, segment) entries of the index                            */
+    int32_t join_mode;         /* 0: not used, 1: join + recurrence, 2: join + l_max <= 1 fast path */
+    int32_t pad2_;
 } tcrnet_stats;
 
 /*
@@ -170,8 +194,10 @@ TCRNET_API void tcrnet_destroy(tcrnet_ctx* ctx);
 
 /*
  * Step A1 (pack): take N sequences, validate them, copy them to the device and lay them out
- * for the distance kernel (5-bit residue codes, stable sort by (length, row), length buckets,
- * permutation).  PAPER.md:326 ("each a.a. is saved as a number ... BYTE"), north_star (1).
+ * for the distance kernels (rows collapsed to distinct sequences, stable sort by (length, first six
+ * residues, row), length buckets, permutation; per sorted position one row of 8-bit residue codes for
+ * the match masks and one row of 5-bit packed codes, 16 bytes up to 25 residues; prefix trie over the
+ * sorted texts).  PAPER.md:326 ("each a.a. is saved as a number ... BYTE"), north_star (1).
  *
  *   residues  host, uint8[sum(lengths)]: the rows concatenated, ASCII 'A'..'Z' (any of the 26
  *             letters is a legal residue; only equality matters - DESIGN.md reading Q8)

@@ -21,7 +21,7 @@ LIB_PATH = os.path.join(_HERE, "libtcrnet_b200.so")
 OK, ERR_ARG, ERR_LENGTH, ERR_RESIDUE, ERR_LMAX, ERR_STATE, ERR_NOMEM, ERR_EDGE_OVERFLOW, ERR_CUDA = (
     0, -1, -2, -3, -4, -5, -6, -7, -8)
 OPT_EARLY_EXIT, OPT_FIRST_CHECK, OPT_EDGE_CAPACITY, OPT_EDGE_LIMIT, OPT_COUNT_WORK, OPT_TEXT_CHUNK = 1, 2, 3, 4, 5, 6
-OPT_PREFIX_TRIE, OPT_TRIE_CHUNK, OPT_N_QUERY, OPT_DEDUP = 7, 8, 9, 10
+OPT_PREFIX_TRIE, OPT_TRIE_CHUNK, OPT_N_QUERY, OPT_DEDUP, OPT_SEGMENT_JOIN, OPT_FAST_L1 = 7, 8, 9, 10, 11, 12
 
 EXPORTS = (
     "tcrnet_create", "tcrnet_destroy", "tcrnet_load", "tcrnet_load_device", "tcrnet_build", "tcrnet_csr",
@@ -48,7 +48,10 @@ class tcrnet_stats(C.Structure):
         ("work_items_trie", C.c_int64), ("trie_nodes", C.c_int64), ("distance_passes", C.c_int32),
         ("launches_load", C.c_int32), ("launches_build", C.c_int32), ("ms_load", C.c_float),
         ("ms_distance", C.c_float), ("ms_sort", C.c_float), ("ms_csr", C.c_float), ("ms_build", C.c_float),
-        ("n_distinct", C.c_int64), ("ms_kernel", C.c_float), ("pad_", C.c_float),
+        ("n_distinct", C.c_int64), ("ms_kernel", C.c_float), ("ms_index", C.c_float),
+        ("lane_columns_live", C.c_int64), ("join_probes", C.c_int64), ("join_entries", C.c_int64),
+        ("join_candidates", C.c_int64), ("work_items_join", C.c_int64), ("join_index_entries", C.c_int64),
+        ("join_mode", C.c_int32), ("pad2_", C.c_int32),
     ]
 
 

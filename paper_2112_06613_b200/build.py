@@ -1,7 +1,9 @@
 """Compile csrc/*.cu into paper_2112_06613_b200/libtcrnet_b200.so for sm_100a (in-tree).
 
 nvcc cross-compiles without a GPU.  The .so is git-ignored but travels to the GPU box with the
-repo snapshot, so tests and bench never JIT anything.
+repo snapshot, so tests and bench never JIT anything.  Every translation unit is compiled to an
+object file of its own (in parallel, re-using objects that are newer than their sources and every
+header), then linked.
 """
 from __future__ import annotations
 
@@ -9,17 +11,21 @@ import glob
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libtcrnet_b200.so")
+OBJ_DIR = os.path.join(HERE, "build")
 SRCS = sorted(glob.glob(os.path.join(HERE, "csrc", "*.cu")))
-DEPS = SRCS + glob.glob(os.path.join(HERE, "csrc", "*.h")) + [os.path.join(ROOT, "include", "tcrnet.h")]
+HDRS = (glob.glob(os.path.join(HERE, "csrc", "*.h")) + glob.glob(os.path.join(HERE, "csrc", "*.cuh"))
+        + [os.path.join(ROOT, "include", "tcrnet.h")])
+DEPS = SRCS + HDRS
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-lineinfo", "-std=c++17",
-    "-shared", "-Xcompiler", "-fPIC",
+    "-Xcompiler", "-fPIC",
     "-Xcompiler", "-fvisibility=hidden",
     "-I", os.path.join(ROOT, "include"),
     "-I", os.path.join(HERE, "csrc"),
@@ -33,21 +39,42 @@ def up_to_date() -> bool:
     return all(os.path.getmtime(d) <= t for d in DEPS)
 
 
+def _obj(src: str) -> str:
+    return os.path.join(OBJ_DIR, os.path.basename(src)[:-3] + ".o")
+
+
+def _compile(nvcc: str, src: str, verbose: bool):
+    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", _obj(src), src]
+    return src, subprocess.run(cmd, capture_output=True, text=True)
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and up_to_date():
+    if not force and not verbose and up_to_date():
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")
+    os.makedirs(OBJ_DIR, exist_ok=True)
+    hdr_time = max(os.path.getmtime(h) for h in HDRS)
+    stale = [s for s in SRCS
+             if force or verbose or not os.path.exists(_obj(s))
+             or os.path.getmtime(_obj(s)) < max(os.path.getmtime(s), hdr_time)]
+    with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as pool:
+        results = list(pool.map(lambda s: _compile(nvcc, s, verbose), stale))
+    failed = [(s, r) for s, r in results if r.returncode != 0]
+    for s, r in results:
+        if r.returncode != 0 or verbose:
+            sys.stderr.write(r.stdout + r.stderr)
+    if failed:
+        raise RuntimeError("nvcc failed on " + ", ".join(os.path.basename(s) for s, _ in failed))
     tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SRCS
-    res = subprocess.run(cmd, capture_output=True, text=True)
+    link = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-Xcompiler", "-fPIC", "-o", tmp] + \
+        [_obj(s) for s in SRCS]
+    res = subprocess.run(link, capture_output=True, text=True)
     if res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)
-        raise RuntimeError("nvcc failed building libtcrnet_b200.so")
-    if verbose:
-        sys.stderr.write(res.stdout + res.stderr)
+        raise RuntimeError("nvcc failed linking libtcrnet_b200.so")
     os.replace(tmp, LIB)
     return LIB
 
 
 if __name__ == "__main__":
-    print(build(force=True, verbose="-v" in sys.argv))
+    print(build(force="-f" in sys.argv, verbose="-v" in sys.argv))

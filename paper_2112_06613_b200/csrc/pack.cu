@@ -72,6 +72,7 @@ __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residu
                                              const int32_t* __restrict__ perm, int64_t n,
                                              const __grid_constant__ LengthTable lt, int pat_stride,
                                              uint8_t* __restrict__ pat, uint32_t* __restrict__ txt,
+                                             uint32_t* __restrict__ seq5, int s5_words,
                                              uint32_t* __restrict__ flags) {
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;  // sorted position
     bool bad = false;
@@ -111,6 +112,26 @@ __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residu
                 }
             }
         }
+        // seq5: the same codes as one little-endian bit string, residue j in bits [5j, 5j + 5), zero beyond
+        // the sequence; s5_words 32-bit words per row (a multiple of 4: rows are read with 128-bit loads)
+        uint32_t* srow = seq5 + (size_t)s * s5_words;
+        unsigned long long acc = 0ull;
+        int filled = 0, w = 0;
+        for (int i = 0; i < len; ++i) {
+            uint32_t c = (uint32_t)src[i] - (uint32_t)'A';
+            if (c >= (uint32_t)kNumCodes) c = 0;
+            acc |= (unsigned long long)c << filled;
+            filled += 5;
+            if (filled >= 32) {
+                srow[w++] = (uint32_t)acc;
+                acc >>= 32;
+                filled -= 32;
+            }
+        }
+        for (; w < s5_words; ++w) {
+            srow[w] = (uint32_t)acc;
+            acc = 0ull;
+        }
     }
     if (__syncthreads_or(bad) && threadIdx.x == 0) atomicOr(flags, kFlagBadResidue);
 }
@@ -136,9 +157,10 @@ cudaError_t launch_seq_keys(const uint8_t* residues, const int64_t* offsets, con
 
 cudaError_t launch_pack(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths,
                         const int32_t* perm, int64_t n, const LengthTable& lt, int pat_stride, uint8_t* pat,
-                        uint32_t* txt, uint32_t* flags, cudaStream_t s, int* launches) {
+                        uint32_t* txt, uint32_t* seq5, int s5_words, uint32_t* flags, cudaStream_t s, int* launches) {
     const int64_t blocks = (n + 255) / 256;
-    k_pack<<<(unsigned)blocks, 256, 0, s>>>(residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, flags);
+    k_pack<<<(unsigned)blocks, 256, 0, s>>>(residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, seq5, s5_words,
+                                            flags);
     *launches += 1;
     return cudaGetLastError();
 }

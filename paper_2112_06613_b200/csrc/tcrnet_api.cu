@@ -63,6 +63,7 @@ void drop_load(tcrnet_ctx* ctx) {
     ctx->loaded = false;
     ctx->all.loaded = ctx->query.loaded = false;
     ctx->n = 0;
+    ctx->join_l_max = -1;  // the segment index belongs to a load
 }
 
 // Step A1: everything after the raw arrays are in device memory.  Packs rows 0..n-1 into `set`.
@@ -112,6 +113,7 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
     lt.start[kNumLen] = (int32_t)pos;
     lt.txt_base[kNumLen] = words;
     set.pat_stride = (max_len + 15) & ~15;
+    set.s5_words = seq5_words(max_len);
 
     // offsets, stable sort by (length, first residues, row), re-layout
     DevBuf& offsets = ctx->offsets;
@@ -124,6 +126,7 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
     if (rc == TCRNET_OK) rc = dev_reserve(ctx, set.perm, sizeof(int32_t) * (size_t)n);
     if (rc == TCRNET_OK) rc = dev_reserve(ctx, set.pat, (size_t)n * set.pat_stride);
     if (rc == TCRNET_OK) rc = dev_reserve(ctx, set.txt, sizeof(uint32_t) * (size_t)(words + 4));
+    if (rc == TCRNET_OK) rc = dev_reserve(ctx, set.seq5, sizeof(uint32_t) * ((size_t)n * set.s5_words + 16));  // + slack: row_bits reads one word ahead
     if (rc != TCRNET_OK) return rc;
     // Sort key: (length, first kSortPrefix residues, row): one composite 64-bit key per row, stable LSD
     // radix sort with the row as payload.  The sub-order inside a length bucket is free (results are mapped
@@ -154,7 +157,8 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
     }
     if (e == cudaSuccess)
         e = launch_pack(d_res, d_off, d_len, (const int32_t*)set.perm.p, n, lt, set.pat_stride,
-                        (uint8_t*)set.pat.p, (uint32_t*)set.txt.p, &dc->flags, s, launches);
+                        (uint8_t*)set.pat.p, (uint32_t*)set.txt.p, (uint32_t*)set.seq5.p, set.s5_words, &dc->flags, s,
+                        launches);
     // prefix trie over the sorted texts (trie.cu); scratch: lcp8 + per-tile counts
     DevBuf& trie_scratch = ctx->trie_scratch;
     if (e == cudaSuccess) {
@@ -299,14 +303,54 @@ struct Schedule {
         const SeqSet* tset = nullptr;
         int mode = kPairsSelf;
         Part part[2][2];  // [trie][wide]
+        std::vector<JoinRow> join_rows[2];  // [wide]: pattern buckets served by the segment join (segjoin.cu)
+        int64_t join_items[2] = {0, 0};
     };
     std::vector<Pass> passes;
     size_t n_rows = 0;
+    size_t n_join_rows = 0;
+    bool use_join = false, fast_l1 = false;
 };
+
+// Segment join: where a text of length n is cut (k = l_max + 1 segments) and which (segment, shift) probes a
+// pattern shorter by delta has to make (segjoin.cu has the derivation: max(|d|, i) + |d + delta| <= l_max).
+// n = q k + r: every segment gets q residues and r of them one more - the two outer ones first, then inwards,
+// because CDR3 sequences are least diverse at their ends (conserved first / last residues), so the outer segments
+// need the extra residue most.  Any cut is exact; this one only keeps the candidate lists short.
+void make_join_tables(int l_max, JoinTables& tab) {
+    std::memset(&tab, 0, sizeof(tab));
+    const int k = l_max + 1;
+    tab.n_seg = (int8_t)k;
+    for (int n = 0; n < kNumLen; ++n) {
+        const int q = n / k, r = n % k;
+        int extra[kJoinMaxSeg] = {};
+        for (int x = 0, lo = 0, hi = k - 1; x < r; ++x) {
+            if (x % 2 == 0) extra[lo++] = 1; else extra[hi--] = 1;
+        }
+        int pos = 0;
+        for (int i = 0; i < k; ++i) {
+            tab.seg_start[n][i] = (uint8_t)pos;
+            pos += q + extra[i];
+        }
+        for (int i = k; i <= kJoinMaxSeg; ++i) tab.seg_start[n][i] = (uint8_t)n;
+    }
+    for (int delta = 0; delta <= l_max; ++delta) {
+        int np = 0;
+        for (int i = 0; i < k; ++i)
+            for (int d = -l_max; d <= l_max; ++d)
+                if (std::max(std::abs(d), i) + std::abs(d + delta) <= l_max && np < kJoinMaxProbes) {
+                    tab.probe_seg[delta][np] = (int8_t)i;
+                    tab.probe_shift[delta][np] = (int8_t)d;
+                    ++np;
+                }
+        tab.n_probes[delta] = (int8_t)np;
+    }
+}
 
 // Step A2, host side: the (pattern bucket, text bucket) pairs with len_t - len_p in 0..l_max
 // (kPairsAllQuery: 1..l_max; the equal-length pairs belong to the kPairsQueryAll pass).
-void schedule_pass(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule::Pass& pass, tcrnet_stats& st) {
+void schedule_pass(const tcrnet_ctx* ctx, int l_max, int first_check, bool use_join, Schedule::Pass& pass,
+                   tcrnet_stats& st) {
     const SeqSet& ps = *pass.pset;
     const SeqSet& ts = *pass.tset;
     // The trie kernel serves the rows whose early exit can act inside the trie (l_max <= kTrieMaxL, the
@@ -324,6 +368,19 @@ void schedule_pass(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule::
             st.cells_kept += pairs * m * n;
             st.columns_kept += pairs * n;
             if (pairs == 0) continue;
+            if (use_join && n >= l_max + 1) {  // the text can be cut into l_max + 1 non-empty segments
+                std::vector<JoinRow>& jr = pass.join_rows[m <= 32 ? 0 : 1];
+                if (jr.empty() || jr.back().m != m) {
+                    JoinRow r{};
+                    r.m = m;
+                    r.p_start = ps.lt.start[m];
+                    r.p_count = (int32_t)pc;
+                    jr.push_back(r);
+                }
+                jr.back().t_start[n - m] = ts.lt.start[n];
+                jr.back().t_count[n - m] = (int32_t)tc;
+                continue;
+            }
             const bool trie = use_trie && n > kTrieDepth;
             WorkRow r{};
             r.txt_base = ts.lt.txt_base[n];
@@ -357,6 +414,20 @@ void schedule_pass(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule::
                 part.max_rw = std::max(part.max_rw, (int)r.row_words);
             }
         }
+    for (int wide = 0; wide < 2; ++wide) {
+        std::vector<JoinRow>& jr = pass.join_rows[wide];
+        auto weight = [](const JoinRow& r) {
+            long double t = 0;
+            for (int d = 0; d < kJoinMaxSeg; ++d) t += r.t_count[d];
+            return t * r.p_count;
+        };
+        std::stable_sort(jr.begin(), jr.end(), [&](const JoinRow& a, const JoinRow& b) { return weight(a) > weight(b); });
+        pass.join_items[wide] = 0;
+        for (JoinRow& r : jr) {
+            r.item_begin = pass.join_items[wide];
+            pass.join_items[wide] += (r.p_count + 31) / 32;
+        }
+    }
 }
 
 void make_schedule(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule& sch, tcrnet_stats& st) {
@@ -385,17 +456,29 @@ void make_schedule(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule& 
         sch.passes[0].pset = sch.passes[0].tset = &ctx->all;
         sch.passes[0].mode = kPairsSelf;
     }
-    st.work_items = st.work_items_trie = 0;
-    sch.n_rows = 0;
+    st.work_items = st.work_items_trie = st.work_items_join = 0;
+    sch.n_rows = sch.n_join_rows = 0;
+    // The join serves the all-pairs mode with the early exit on (its verification always votes); the rectangular
+    // mode and l_max beyond the specialised range stay with the trie / text-chunk kernels.
+    const bool can_join = !ctx->query.loaded && ctx->early_exit && l_max <= kTrieMaxL;
+    sch.fast_l1 = can_join && ctx->fast_l1 && l_max <= 1;
+    sch.use_join = sch.fast_l1 || (can_join && (ctx->segment_join == 1 ||
+                                                (ctx->segment_join < 0 && l_max >= 2 && ctx->prefix_trie)));
     for (Schedule::Pass& pass : sch.passes) {
-        schedule_pass(ctx, l_max, first_check, pass, st);
+        schedule_pass(ctx, l_max, first_check, sch.use_join, pass, st);
         for (int trie = 0; trie < 2; ++trie)
             for (int wide = 0; wide < 2; ++wide) {
                 st.work_items += pass.part[trie][wide].items;
                 if (trie) st.work_items_trie += pass.part[trie][wide].items;
                 sch.n_rows += pass.part[trie][wide].rows.size();
             }
+        for (int wide = 0; wide < 2; ++wide) {
+            st.work_items += pass.join_items[wide];
+            st.work_items_join += pass.join_items[wide];
+            sch.n_join_rows += pass.join_rows[wide].size();
+        }
     }
+    st.join_mode = sch.n_join_rows == 0 ? 0 : (sch.fast_l1 ? 2 : 1);
 }
 
 int upload_schedule(tcrnet_ctx* ctx, const Schedule& sch) {
@@ -410,6 +493,47 @@ int upload_schedule(tcrnet_ctx* ctx, const Schedule& sch) {
                                              ctx->stream));
                 dst += rows.size();
             }
+    if (sch.n_join_rows) {
+        TRY(dev_reserve(ctx, ctx->join_rows, sizeof(JoinRow) * sch.n_join_rows));
+        JoinRow* jdst = (JoinRow*)ctx->join_rows.p;
+        for (const Schedule::Pass& pass : sch.passes)
+            for (int wide = 0; wide < 2; ++wide) {
+                const std::vector<JoinRow>& rows = pass.join_rows[wide];
+                if (!rows.empty())
+                    TRY_CUDA(cudaMemcpyAsync(jdst, rows.data(), sizeof(JoinRow) * rows.size(), cudaMemcpyHostToDevice, ctx->stream));
+                jdst += rows.size();
+            }
+    }
+    return TCRNET_OK;
+}
+
+// Segment index of the texts of ctx->all for threshold l_max (kept until the next load / another threshold).
+int ensure_join_index(tcrnet_ctx* ctx, int l_max, int* launches) {
+    tcrnet_stats& st = ctx->stats;
+    st.ms_index = 0.f;
+    const SeqSet& set = ctx->all;
+    const int k = l_max + 1;
+    int64_t n_idx = 0;
+    for (int l = k; l < kNumLen; ++l) n_idx += set.hist[l] * k;
+    st.join_index_entries = n_idx;
+    if (ctx->join_l_max == l_max) return TCRNET_OK;
+    cudaStream_t s = ctx->stream;
+    make_join_tables(l_max, ctx->join_tab);
+    uint32_t slots = 1024;
+    while ((int64_t)slots < 2 * n_idx && slots < (1u << 30)) slots <<= 1;
+    TRY(dev_reserve(ctx, ctx->join_cnt, sizeof(uint32_t) * (size_t)slots));
+    TRY(dev_reserve(ctx, ctx->join_dir, sizeof(uint32_t) * ((size_t)slots + 1)));
+    TRY(dev_reserve(ctx, ctx->join_entries, sizeof(uint2) * (size_t)std::max<int64_t>(n_idx, 1)));
+    TRY(dev_reserve(ctx, ctx->scan_scratch, scan_scratch_bytes((int64_t)slots)));
+    TRY_CUDA(cudaEventRecord(ctx->ev[6], s));
+    TRY_CUDA(cudaMemsetAsync(ctx->join_cnt.p, 0, sizeof(uint32_t) * (size_t)slots, s));
+    TRY_CUDA(launch_join_index((const uint32_t*)set.seq5.p, set.s5_words, set.lt, set.n, ctx->join_tab,
+                               (uint32_t*)ctx->join_cnt.p, (uint32_t*)ctx->join_dir.p, (uint2*)ctx->join_entries.p, slots,
+                               ctx->scan_scratch.p, s, launches));
+    TRY_CUDA(cudaEventRecord(ctx->ev[7], s));
+    ctx->join_slots = slots;
+    ctx->join_l_max = l_max;
+    st.ms_index = -1.f;  // measured once the events have completed (distance_phase)
     return TCRNET_OK;
 }
 
@@ -420,14 +544,15 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
                  int n_shards, bool expand_only, int* launches) {
     cudaStream_t s = ctx->stream;
     HostCtrl* dc = d_ctrl(ctx);
-    static_assert(offsetof(HostCtrl, queue) == offsetof(HostCtrl, edge_count) + 5 * sizeof(unsigned long long), "one memset");
+    static_assert(offsetof(HostCtrl, queue) == offsetof(HostCtrl, edge_count) + 9 * sizeof(unsigned long long), "one memset");
     static_assert(offsetof(HostCtrl, edge_total) == offsetof(HostCtrl, queue) + kTrieQueues * sizeof(unsigned long long), "one memset");
     if (expand_only) TRY_CUDA(cudaMemsetAsync(&dc->edge_total, 0, sizeof(unsigned long long), s));
-    else TRY_CUDA(cudaMemsetAsync(&dc->edge_count, 0, sizeof(unsigned long long) * (6 + kTrieQueues), s));  // edge_count, work[4], queue[], edge_total
+    else TRY_CUDA(cudaMemsetAsync(&dc->edge_count, 0, sizeof(unsigned long long) * (10 + kTrieQueues), s));  // edge_count, work[8], queue[], edge_total
     TRY_CUDA(cudaMemsetAsync(ctx->row_count.p, 0, sizeof(int32_t) * (size_t)ctx->n, s));
     TRY_CUDA(cudaMemsetAsync(ctx->deg.p, 0, sizeof(int32_t) * (size_t)ctx->n, s));
     int n_queues = 0;
     const WorkRow* d_rows = (const WorkRow*)ctx->rows.p;
+    const JoinRow* d_join_rows = (const JoinRow*)ctx->join_rows.p;
     if (!expand_only) TRY_CUDA(cudaEventRecord(ctx->ev[4], s));
     for (const Schedule::Pass& pass : sch.passes) {
         if (expand_only) break;
@@ -468,6 +593,19 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
                 }
                 d_rows += part.rows.size();
             }
+        for (int wide = 0; wide < 2; ++wide) {
+            const std::vector<JoinRow>& jr = pass.join_rows[wide];
+            if (!jr.empty()) {
+                if (n_queues >= kTrieQueues) return TCRNET_ERR_STATE;
+                p.queue = dc->queue + n_queues++;
+                p.n_items = pass.join_items[wide];
+                JoinIndex index{(const uint32_t*)ctx->join_dir.p, (const uint2*)ctx->join_entries.p, ctx->join_slots - 1u};
+                TRY_CUDA(launch_join(p, d_join_rows, (int)jr.size(), (const uint32_t*)pass.pset->seq5.p, pass.pset->s5_words,
+                                     index, ctx->join_tab, wide != 0, sch.fast_l1, ctx->count_work != 0, ctx->n_sm, s,
+                                     launches));
+            }
+            d_join_rows += jr.size();
+        }
     }
     if (!expand_only) TRY_CUDA(cudaEventRecord(ctx->ev[5], s));
     if (ctx->all.grouped) {
@@ -483,7 +621,7 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
                                        (int32_t*)ctx->deg.p, ctx->n_sm, s, launches));
         TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->edge_total, &dc->edge_total, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
     }
-    TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->edge_count, &dc->edge_count, sizeof(unsigned long long) * 5,
+    TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->edge_count, &dc->edge_count, sizeof(unsigned long long) * 9,
                              cudaMemcpyDeviceToHost, s));
     TRY_CUDA(cudaStreamSynchronize(s));
     return TCRNET_OK;
@@ -505,6 +643,9 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
     make_schedule(ctx, l_max, first_check, sch, st);
     TRY_CUDA(cudaEventRecord(ctx->ev[0], s));
     TRY(upload_schedule(ctx, sch));
+    st.ms_index = 0.f;
+    st.join_index_entries = 0;
+    if (sch.n_join_rows) TRY(ensure_join_index(ctx, l_max, launches));
 
     // distances + emission (second pass only if the edge buffer was too small)
     int64_t cap = ctx->edge_capacity_opt > 0 ? ctx->edge_capacity_opt : std::max<int64_t>((int64_t)1 << 20, 16 * n);
@@ -547,6 +688,11 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
     st.lane_tests_exec = (int64_t)ctx->h_ctrl->work[1];
     st.lane_pairs_exec = (int64_t)ctx->h_ctrl->work[2];
     st.lane_prefix_tests_exec = (int64_t)ctx->h_ctrl->work[3];
+    st.lane_columns_live = (int64_t)ctx->h_ctrl->work[4];
+    st.join_probes = (int64_t)ctx->h_ctrl->work[5];
+    st.join_entries = (int64_t)ctx->h_ctrl->work[6];
+    st.join_candidates = (int64_t)ctx->h_ctrl->work[7];
+    if (st.ms_index < 0.f) TRY_CUDA(cudaEventElapsedTime(&st.ms_index, ctx->ev[6], ctx->ev[7]));
     TRY_CUDA(cudaEventRecord(ctx->ev[1], s));
     ctx->n_keys = n_keys;
     return TCRNET_OK;
@@ -650,7 +796,7 @@ int tcrnet_create(tcrnet_ctx** out, int device, void* cuda_stream, const tcrnet_
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, device);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->h_ctrl, sizeof(HostCtrl));
-    for (int i = 0; e == cudaSuccess && i < 6; ++i) e = cudaEventCreate(&ctx->ev[i]);
+    for (int i = 0; e == cudaSuccess && i < 8; ++i) e = cudaEventCreate(&ctx->ev[i]);
     if (e != cudaSuccess) {
         (void)cudaGetLastError();
         tcrnet_destroy(ctx);
@@ -669,7 +815,8 @@ void tcrnet_destroy(tcrnet_ctx* ctx) {
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     DevBuf* bufs[] = {&ctx->all.perm, &ctx->all.pat, &ctx->all.txt, &ctx->all.trie, &ctx->query.perm, &ctx->query.pat,
-                      &ctx->query.txt, &ctx->query.trie, &ctx->inv_perm, &ctx->edge_dist, &ctx->edge_dist_b, &ctx->flags,
+                      &ctx->query.txt, &ctx->query.trie, &ctx->all.seq5, &ctx->query.seq5, &ctx->join_cnt, &ctx->join_dir,
+                      &ctx->join_entries, &ctx->join_rows, &ctx->inv_perm, &ctx->edge_dist, &ctx->edge_dist_b, &ctx->flags,
                       &ctx->flag_pos, &ctx->in_res, &ctx->in_len, &ctx->offsets,
                       &ctx->perm_tmp, &ctx->trie_scratch, &ctx->keys_a, &ctx->keys_b, &ctx->radix_scratch,
                       &ctx->scan_scratch, &ctx->rows, &ctx->row_ptr, &ctx->col, &ctx->row_count, &ctx->long_rows, &ctx->all.group_start, &ctx->all.members, &ctx->all.uid_of,
@@ -962,6 +1109,14 @@ int tcrnet_set_option(tcrnet_ctx* ctx, int option, int64_t value) {
         case TCRNET_OPT_DEDUP:
             if (value != 0 && value != 1) return TCRNET_ERR_ARG;
             ctx->dedup = (int)value;
+            return TCRNET_OK;
+        case TCRNET_OPT_SEGMENT_JOIN:
+            if (value < -1 || value > 1) return TCRNET_ERR_ARG;
+            ctx->segment_join = (int)value;
+            return TCRNET_OK;
+        case TCRNET_OPT_FAST_L1:
+            if (value != 0 && value != 1) return TCRNET_ERR_ARG;
+            ctx->fast_l1 = (int)value;
             return TCRNET_OK;
         case TCRNET_OPT_TRIE_CHUNK:
             if (value < kTQ || value % kTQ != 0 || value > (1 << 24)) return TCRNET_ERR_ARG;

@@ -15,7 +15,7 @@ struct DevBuf {
 struct HostCtrl {  // pinned mirror of the small device control block
     unsigned long long hist[kNumLen];
     unsigned long long edge_count;
-    unsigned long long work[4];
+    unsigned long long work[8];
     unsigned long long queue[kTrieQueues];  // dynamic work queues of the trie launches (zeroed with edge_count)
     unsigned long long edge_total;    // dedup: edges between rows after the expansion of the recorded pairs
     unsigned long long probe[3];
@@ -37,7 +37,8 @@ struct SeqSet {
     int min_len = 0, max_len = 0;
     LengthTable lt{};
     int pat_stride = 0;
-    DevBuf perm, pat, txt, trie;
+    DevBuf perm, pat, txt, trie, seq5;
+    int s5_words = 0;  // 32-bit words per row of seq5
     TrieLevels trie_levels{};
     uint32_t trie_root[kNumLen + 1] = {};  // level-1 node range of bucket L: [trie_root[L], trie_root[L+1])
     int64_t trie_nodes = 0;
@@ -66,6 +67,8 @@ struct tcrnet_ctx {
     int trie_chunk = 1 << 20;  // in practice the whole text bucket: the top of the trie is walked once per pattern tile
 
     int dedup = 1;        // collapse identical sequences at load (TCRNET_OPT_DEDUP)
+    int segment_join = -1;  // TCRNET_OPT_SEGMENT_JOIN: -1 automatic (l_max >= 2), 0 never, 1 whenever possible
+    int fast_l1 = 0;        // TCRNET_OPT_FAST_L1: l_max <= 1 builds through the join with the XOR / popcount check
     int64_t n_query = 0;  // > 0: rectangular mode (TCRNET_OPT_N_QUERY)
 
     // load state
@@ -85,6 +88,11 @@ struct tcrnet_ctx {
     int64_t n_edges = 0, n_keys = 0;
     DevBuf keys_a, keys_b, radix_scratch, scan_scratch, rows, row_ptr, col, deg, row_count, long_rows;
     DevBuf inv_perm, edge_dist, edge_dist_b, flags, flag_pos;
+    // segment join (segjoin.cu): directory + entries of the current load for join_l_max, work rows
+    DevBuf join_cnt, join_dir, join_entries, join_rows;
+    int join_l_max = -1;  // threshold the index in join_dir / join_entries was built for (-1: none)
+    uint32_t join_slots = 0;
+    JoinTables join_tab{};
 
     // observables state (observables_api.cu); valid for the current CSR only
     bool have_hist = false, have_nn = false, have_cc = false;
@@ -95,7 +103,7 @@ struct tcrnet_ctx {
 
     DevBuf ctrl;               // device HostCtrl
     HostCtrl* h_ctrl = nullptr;  // pinned
-    cudaEvent_t ev[6] = {};
+    cudaEvent_t ev[8] = {};
     tcrnet_stats stats{};
 };
 

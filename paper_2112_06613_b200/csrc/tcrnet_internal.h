@@ -95,11 +95,42 @@ struct DistanceParams {
     const int32_t* members;
     unsigned long long* edge_count;  // device counter (keeps counting beyond capacity)
     unsigned long long edge_cap;
-    unsigned long long* work;        // [4]: lane-columns, lane-tests (exit votes), lane-first-columns,
-                                     //      lane-V-sets (guided expansions); COUNT only
+    unsigned long long* work;        // [8], COUNT only: [0] lane-columns, [1] lane-tests (exit votes), [2] lane-first-columns,
+                                     //      [3] lane-V-sets (guided expansions), [4] lane-columns of lanes still alive,
+                                     //      join kernels: [5] probes, [6] directory entries read, [7] candidates checked
     const TrieNode* trie[kTrieDepth + 1];  // trie kernel: nodes of level 1..kTrieDepth ([0] unused)
     unsigned long long* queue;       // trie kernel: next unclaimed work item of this launch (zeroed before the launch)
     int64_t n_items;                 // trie kernel: work items of all shards of this launch
+};
+
+// ---- segment join (segjoin.cu): an exact candidate filter in front of the distance step ----
+// If lev(r, s) <= l_max and s is cut into l_max + 1 segments, at least one segment of s occurs unchanged in r
+// (l_max edits touch at most l_max segments), shifted by no more than the edits allow.  The segments of every
+// text are indexed in a hash directory; every pattern probes it with the substrings that could be such a
+// segment, and only the pairs found this way are handed to the column recurrence.
+constexpr int kJoinMaxSeg = kTrieMaxL + 1;  // segments per text: l_max + 1 <= 5
+constexpr int kJoinMaxProbes = 28;          // (segment, shift) probes per length difference
+struct JoinTables {
+    uint8_t seg_start[kNumLen][kJoinMaxSeg + 1];  // [n][i] = first residue of segment i of a text of length n; [n][k] = n
+    int8_t n_probes[kJoinMaxSeg];                 // [delta]: probes of a pattern against the texts longer by delta
+    int8_t probe_seg[kJoinMaxSeg][kJoinMaxProbes];
+    int8_t probe_shift[kJoinMaxSeg][kJoinMaxProbes];  // the segment starting at p in the text is looked for at p + shift
+    int8_t n_seg;                                 // l_max + 1
+    int8_t pad_[6];
+};
+// One pattern bucket of the join kernels: its 32-pattern tiles are the work items; texts = the buckets of
+// length m .. m + l_max that are indexed (t_count 0: none).
+struct JoinRow {
+    int64_t item_begin;
+    int32_t p_start, p_count;
+    int32_t m, pad_;
+    int32_t t_start[kJoinMaxSeg];
+    int32_t t_count[kJoinMaxSeg];
+};
+struct JoinIndex {
+    const uint32_t* dir;  // [slots + 1]: entries of hash bucket b are [dir[b], dir[b+1])
+    const uint2* entries; // (tag = high half of the segment hash, sorted position of the text)
+    uint32_t mask;        // slots - 1 (a power of two)
 };
 
 // ---- launch wrappers (each returns cudaGetLastError(); *launches is incremented per kernel) ----
@@ -134,7 +165,11 @@ cudaError_t launch_seq_keys(const uint8_t* residues, const int64_t* offsets, con
                             unsigned long long* keys, int32_t* vals, cudaStream_t s, int* launches);
 cudaError_t launch_pack(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths,
                         const int32_t* perm, int64_t n, const LengthTable& lt, int pat_stride,
-                        uint8_t* pat, uint32_t* txt, uint32_t* flags, cudaStream_t s, int* launches);
+                        uint8_t* pat, uint32_t* txt, uint32_t* seq5, int s5_words, uint32_t* flags, cudaStream_t s,
+                        int* launches);
+// seq5 row: 32-bit words per sequence of the 5-bit packed table (residue j in bits [5j, 5j+5) of the row's
+// little-endian bit string): 4 words up to 25 residues, 8 up to 51, 12 up to 64
+inline int seq5_words(int max_len) { return 4 * ((5 * max_len + 127) / 128); }
 
 // trie.cu: prefix trie over the sorted texts (levels 1..kTrieDepth, all length buckets).
 //   lcp8        : scratch, uint8[round_up(n,16) + 16]
@@ -185,6 +220,19 @@ cudaError_t launch_distance(const DistanceParams& p, int64_t n_items, bool wide,
 size_t distance_trie_smem_bytes(bool wide);
 cudaError_t launch_distance_trie(const DistanceParams& p, int64_t n_items, bool wide, bool count_work, int n_sm,
                                  cudaStream_t s, int* launches);
+
+// segjoin.cu
+// Index of the segments of the texts at sorted positions [0, n) with length >= tab.n_seg: cnt (uint32[slots], zeroed
+// by the caller) is consumed, dir gets slots + 1 offsets, entries n_entries pairs.
+cudaError_t launch_join_index(const uint32_t* seq5, int s5_words, const LengthTable& lt, int64_t n, const JoinTables& tab,
+                              uint32_t* cnt, uint32_t* dir, uint2* entries, uint32_t slots, void* scan_scratch,
+                              cudaStream_t s, int* launches);
+size_t join_smem_bytes(bool wide);
+// general kernel (verification by the column recurrence) and the l_max <= 1 fast path (XOR / popcount on the packed
+// codes); p carries the emission fields, the queue, n_items and the shard of the launch
+cudaError_t launch_join(const DistanceParams& p, const JoinRow* rows, int n_rows, const uint32_t* seq5, int s5_words,
+                        const JoinIndex& index, const JoinTables& tab, bool wide, bool fast_l1, bool count_work, int n_sm,
+                        cudaStream_t s, int* launches);
 
 // labels.cu: distance labels of the final edges, threshold restriction, key validation
 cudaError_t launch_inverse_perm(const int32_t* perm, int64_t n, int32_t* inv, cudaStream_t s, int* launches);
