@@ -188,6 +188,10 @@ def main() -> None:
     ap.add_argument("--text-chunk", type=int, default=0)
     ap.add_argument("--trie-chunk", type=int, default=0)
     ap.add_argument("--no-trie", action="store_true", help="text-chunk kernel only (every kept pair visited)")
+    ap.add_argument("--segment-join", type=int, default=None, choices=[-1, 0, 1],
+                    help="TCRNET_OPT_SEGMENT_JOIN (default: the library's)")
+    ap.add_argument("--fast-l1", action="store_true", help="TCRNET_OPT_FAST_L1 = 1 (l_max <= 1 without the recurrence)")
+    ap.add_argument("--no-dedup", action="store_true", help="TCRNET_OPT_DEDUP = 0 (identical rows are not collapsed)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -234,6 +238,12 @@ def main() -> None:
         net.set_option(pkg.OPT_TRIE_CHUNK, args.trie_chunk)
     if args.no_trie:
         net.set_option(pkg.OPT_PREFIX_TRIE, 0)
+    if args.segment_join is not None:
+        net.set_option(pkg.OPT_SEGMENT_JOIN, args.segment_join)
+    if args.fast_l1:
+        net.set_option(pkg.OPT_FAST_L1, 1)
+    if args.no_dedup:
+        net.set_option(pkg.OPT_DEDUP, 0)
 
     def step_device():
         net.load(d_res, d_len)
@@ -354,6 +364,10 @@ def main() -> None:
                 "trie_nodes": work["trie_nodes"], "lane_columns_exec": work["lane_columns_exec"],
                 "lane_prefix_tests_exec": work["lane_prefix_tests_exec"], "lane_tests_exec": work["lane_tests_exec"],
                 "ms_steps": ms_steps,
+                "join_mode": work["join_mode"], "ms_index": float(np.mean([s["ms_index"] for s in stats])),
+                "work_items_join": work["work_items_join"], "join_probes": work["join_probes"],
+                "join_entries": work["join_entries"], "join_candidates": work["join_candidates"],
+                "join_index_entries": work["join_index_entries"], "lane_columns_live": work["lane_columns_live"],
             },
         }
         # the emission / CSR passes against the HBM peak (algorithmic bytes of DESIGN.md section 7:

@@ -36,6 +36,8 @@ def _load():
         lib.oracle_edges.restype = C.c_int
         lib.oracle_edges.argtypes = [u8p, i64p, i32p, C.c_int64, C.c_int32, i64p, C.c_int64, C.c_int,
                                      C.c_int, C.c_int, C.POINTER(i64p), i64p, i32p]
+        lib.oracle_lev_pairs.restype = C.c_int
+        lib.oracle_lev_pairs.argtypes = [u8p, i64p, i32p, C.c_int64, i64p, C.c_int64, i32p, C.c_int]
         lib.oracle_free.restype = None
         lib.oracle_free.argtypes = [C.c_void_p]
         lib.oracle_csr.restype = C.c_int
@@ -118,6 +120,22 @@ def edges(residues, lengths, l_max: int, *, rows: Optional[Sequence[int]] = None
     pairs = np.ctypeslib.as_array(out, shape=(max(e, 1) * 2,))[: 2 * e].copy().reshape(e, 2)
     _load().oracle_free(out)
     return pairs, int(used.value)
+
+
+def lev_pairs(residues, lengths, pairs, *, threads: int = 0) -> np.ndarray:
+    """lev(s_i, s_j) (full table) for every (i, j) of ``pairs`` (int64[E, 2]): int32[E]."""
+    residues = _u8(residues)
+    lengths = np.ascontiguousarray(lengths, dtype=np.int32)
+    off = _offsets(lengths)
+    assert off[-1] == residues.size, "residues / lengths mismatch"
+    pairs = np.ascontiguousarray(pairs, dtype=np.int64).reshape(-1, 2)
+    out = np.zeros(pairs.shape[0], dtype=np.int32)
+    rc = _load().oracle_lev_pairs(_ptr(residues, C.c_uint8), _ptr(off, C.c_int64), _ptr(lengths, C.c_int32),
+                                  lengths.size, _ptr(pairs, C.c_int64), pairs.shape[0], _ptr(out, C.c_int32),
+                                  int(threads))
+    if rc != 0:
+        raise ValueError("oracle_lev_pairs: index out of range or out of memory")
+    return out
 
 
 def csr(pairs: np.ndarray, n: int) -> Tuple[np.ndarray, np.ndarray, np.ndarray]:

@@ -223,6 +223,44 @@ int oracle_edges(const uint8_t* residues, const int64_t* offsets, const int32_t*
 void oracle_free(void* p) { free(p); }
 
 /*
+ * Public: the distances of a caller-supplied list of pairs, out[k] = lev(s_i, s_j) for
+ * (i, j) = pairs[2k], pairs[2k+1] (the same full table as oracle_lev,
+ * one pair after the other; OpenMP over the list).  Used by the parity tests to check
+ * EVERY edge a large network holds (lev <= l_max) where the whole network is
+ * beyond the oracle's reach.  Returns 0, or -1 on allocation failure / an index out of range.
+ */
+int oracle_lev_pairs(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths, int64_t n,
+                     const int64_t* pairs, int64_t n_pairs, int32_t* out, int threads) {
+    int32_t max_len = 0;
+    for (int64_t r = 0; r < n; ++r)
+        if (lengths[r] > max_len) max_len = lengths[r];
+    int failed = 0;
+#ifdef _OPENMP
+    if (threads > 0) omp_set_num_threads(threads);
+#endif
+#pragma omp parallel
+    {
+        int32_t* D = (int32_t*)malloc(sizeof(int32_t) * (size_t)(max_len + 1) * (size_t)(max_len + 1));
+        if (!D) {
+#pragma omp atomic write
+            failed = 1;
+        }
+#pragma omp for schedule(static)
+        for (int64_t k = 0; k < n_pairs; ++k) {
+            const int64_t i = pairs[2 * k], j = pairs[2 * k + 1];
+            if (!D || i < 0 || j < 0 || i >= n || j >= n) {
+#pragma omp atomic write
+                failed = 1;
+                continue;
+            }
+            out[k] = lev_table(residues + offsets[i], lengths[i], residues + offsets[j], lengths[j], D);
+        }
+        free(D);
+    }
+    return failed ? -1 : 0;
+}
+
+/*
  * Public: edge list -> CSR of the strict upper triangle + degrees
  * (PAPER.md:301-318 adjacency, PAPER.md:224 degree).  `pairs` is (i,j) with
  * i < j in lexicographic order (as oracle_edges with all_partners = 0 yields).

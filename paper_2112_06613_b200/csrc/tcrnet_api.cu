@@ -249,10 +249,15 @@ int dedup_rows(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t
                                (int32_t*)set.members.p, s, launches));
     TRY_CUDA(cudaStreamSynchronize(s));
     if (ctx->h_ctrl->flags & kFlagBadLength) return TCRNET_ERR_LENGTH;
+    int64_t sum_len = 0;
     for (int l = 0; l < kNumLen; ++l) {
         ctx->row_hist[l] = (int64_t)ctx->h_ctrl->hist[l];
         ctx->hist_u_host[l] = ctx->h_ctrl->hist_u[l];  // (the pack clears the control block)
+        sum_len += ctx->row_hist[l] * l;
     }
+    // the header's contract: total_len = sum of the lengths (a shorter buffer would be read past its end by the
+    // pack; the insert / lookup kernels above never touch a row that does not fit)
+    if (sum_len != total_len) return TCRNET_ERR_ARG;
     *n_u = (int64_t)ctx->h_ctrl->n_distinct;
     if (*n_u < 1 || *n_u > n) return TCRNET_ERR_CUDA;
     return TCRNET_OK;
@@ -463,7 +468,7 @@ void make_schedule(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule& 
     const bool can_join = !ctx->query.loaded && ctx->early_exit && l_max <= kTrieMaxL;
     sch.fast_l1 = can_join && ctx->fast_l1 && l_max <= 1;
     sch.use_join = sch.fast_l1 || (can_join && (ctx->segment_join == 1 ||
-                                                (ctx->segment_join < 0 && l_max >= 2 && ctx->prefix_trie)));
+                                                (ctx->segment_join < 0 && ctx->prefix_trie)));
     for (Schedule::Pass& pass : sch.passes) {
         schedule_pass(ctx, l_max, first_check, sch.use_join, pass, st);
         for (int trie = 0; trie < 2; ++trie)

@@ -347,3 +347,56 @@ def test_thread_count_does_not_change_result():
     p1, t1 = oracle.edges(d.residues, d.lengths, 1, threads=1)
     p3, t3 = oracle.edges(d.residues, d.lengths, 1, threads=3)
     assert t1 == 1 and t3 == 3 and np.array_equal(p1, p3)
+
+
+def test_lev_pairs_is_the_same_table_pair_by_pair():
+    """oracle.lev_pairs (the batched driver the large-config parity tests use) against the breadth-first search over
+    edit scripts (all pairs of binary strings of length <= 4, laid out as rows) and against construction: a string
+    and the same string after k substitutions at distinct positions of a disjoint alphabet has distance exactly k."""
+    universe = [""] + ["".join(p) for k in range(1, 5) for p in itertools.product("AB", repeat=k)]
+    dist = _bfs_distances(universe, "AB", 4)
+    rows = [s for s in universe if s]
+    res, ln = from_strings(rows)
+    pairs = np.array([(i, j) for i in range(len(rows)) for j in range(len(rows))], dtype=np.int64)
+    got = oracle.lev_pairs(res, ln, pairs, threads=2)
+    want = np.array([dist[rows[i]][rows[j]] for i, j in pairs], dtype=np.int32)
+    assert np.array_equal(got, want)
+    base = [rand_str(int(RNG.integers(6, 30)), "ACDEF") for _ in range(200)]
+    ks = [int(RNG.integers(0, len(s) + 1)) for s in base]
+    changed = []
+    for s, k in zip(base, ks):
+        t = list(s)
+        for q in RNG.choice(len(s), k, replace=False):
+            t[q] = "W"
+        changed.append("".join(t))
+    res, ln = from_strings(base + changed)
+    pairs = np.array([(i, i + len(base)) for i in range(len(base))], dtype=np.int64)
+    assert oracle.lev_pairs(res, ln, pairs).tolist() == ks
+    with pytest.raises(ValueError):
+        oracle.lev_pairs(res, ln, np.array([[0, 2 * len(base)]], dtype=np.int64))
+
+
+@pytest.mark.skipif(os.environ.get("TCRNET_ORACLE_SANITIZE") == "1", reason="already inside the sanitizer run")
+def test_pins_under_address_and_ub_sanitizers():
+    """the oracle under -fsanitize=address,undefined.  A subprocess builds
+    oracle/libtcrnet_oracle_asan.so and runs the quick pins (tables, edge lists, CSR, threads) against it; any
+    out-of-bounds access, use after free, signed overflow or misaligned access in the C sources aborts it."""
+    import subprocess
+    import sys
+    from oracle import build as ob
+    runtime = ob.sanitizer_runtime()
+    if not os.path.isabs(runtime) or not os.path.exists(runtime):
+        pytest.skip("gcc has no libasan.so here")
+    env = dict(os.environ)
+    env.update({ob.SANITIZE_ENV: "1", "LD_PRELOAD": runtime, "ASAN_OPTIONS": "detect_leaks=0",
+                "UBSAN_OPTIONS": "halt_on_error=1:print_stacktrace=1", "OMP_NUM_THREADS": "4"})
+    sel = ("golden_examples or identity_empty or closed_forms or threshold_is_less or duplicates_form or "
+           "lmax_zero or five_node or csr_rejects or csr_invariants or rows_and_all_partners or thread_count or "
+           "lev_pairs or abort_variant")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-m", "pytest", "-x", "-q", "-p", "no:cacheprovider",
+                        os.path.join(root, "tests", "test_oracle_pins.py"),
+                        os.path.join(root, "tests", "test_observables_pins.py"), "-k", sel + " or observables or closed or paper"],
+                       cwd=root, env=env, capture_output=True, text=True, timeout=1500)
+    assert r.returncode == 0, r.stdout[-3000:] + r.stderr[-3000:]
+    assert "passed" in r.stdout

@@ -87,25 +87,59 @@ def test_early_exit_and_schedule_do_not_change_the_result(pkg):
 
 
 def test_prefix_trie_does_not_change_the_result(pkg, oracle):
-    """The prefix-trie kernel (default) against the text-chunk kernel and the oracle: every first
+    """The prefix-trie kernel (TCRNET_OPT_SEGMENT_JOIN = 0) against the text-chunk kernel and the oracle: every first
     test level, tiny trie chunks (chunk borders inside trie nodes), work counters on."""
     d = generate("cfg2", n=20000)
+    trie = {pkg.OPT_SEGMENT_JOIN: 0}
     for l_max in (0, 1, 2, 3, 4):
-        ref, st0 = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_PREFIX_TRIE: 0})
-        assert st0["work_items_trie"] == 0
-        got, st = gpu_network(pkg, d.residues, d.lengths, l_max)
-        assert st["work_items_trie"] > 0 and st["trie_nodes"] > d.n
+        ref, st0 = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_PREFIX_TRIE: 0, **trie})
+        assert st0["work_items_trie"] == 0 and st0["join_mode"] == 0
+        got, st = gpu_network(pkg, d.residues, d.lengths, l_max, trie)
+        assert st["work_items_trie"] > 0 and st["trie_nodes"] > d.n and st["join_mode"] == 0
         assert_same_network(got, ref)
         for ft in range(3, 7):
             got, st = gpu_network(pkg, d.residues, d.lengths, l_max,
-                                  {pkg.OPT_FIRST_CHECK: ft, pkg.OPT_TRIE_CHUNK: 256 * ft, pkg.OPT_COUNT_WORK: ft & 1})
+                                  {pkg.OPT_FIRST_CHECK: ft, pkg.OPT_TRIE_CHUNK: 256 * ft, pkg.OPT_COUNT_WORK: ft & 1, **trie})
             assert st["first_check"] == ft and st["work_items_trie"] > 0
             assert_same_network(got, ref)
             if ft & 1:
                 assert st["lane_prefix_tests_exec"] > 0 and st["lane_columns_exec"] > 0
     want = oracle.network(d.residues, d.lengths, 2, tier=1)[:3]
-    got, _ = gpu_network(pkg, d.residues, d.lengths, 2)
+    got, _ = gpu_network(pkg, d.residues, d.lengths, 2, trie)
     assert_same_network(got, want)
+
+
+def test_segment_join_does_not_change_the_result(pkg, oracle):
+    """The segment join (pigeonhole candidate filter, the default for l_max <= 4) against the oracle and against the
+    paths that visit every length-compatible pair: every threshold it serves, collapse on / off, counters on, a tiny
+    edge buffer (second pass), and the l_max <= 1 option."""
+    d = generate("cfg2", n=20000)
+    for l_max in (0, 1, 2, 3, 4):
+        want = oracle.network(d.residues, d.lengths, l_max, tier=1)[:3]
+        got, st = gpu_network(pkg, d.residues, d.lengths, l_max)
+        assert st["join_mode"] >= 1 and st["work_items_join"] > 0 and st["work_items_trie"] == 0
+        assert_same_network(got, want)
+        for opts in ({pkg.OPT_SEGMENT_JOIN: 1, pkg.OPT_DEDUP: 0}, {pkg.OPT_SEGMENT_JOIN: 1, pkg.OPT_COUNT_WORK: 1},
+                     {pkg.OPT_SEGMENT_JOIN: 1, pkg.OPT_EDGE_CAPACITY: 64}, {pkg.OPT_SEGMENT_JOIN: 1, pkg.OPT_DEDUP: 0, pkg.OPT_EDGE_CAPACITY: 64}):
+            got, st = gpu_network(pkg, d.residues, d.lengths, l_max, opts)
+            assert st["join_mode"] >= 1
+            if opts.get(pkg.OPT_COUNT_WORK):
+                assert st["join_probes"] > 0 and st["join_entries"] > 0 and (st["join_candidates"] > 0 or l_max == 0)
+            if opts.get(pkg.OPT_EDGE_CAPACITY) and opts.get(pkg.OPT_DEDUP) == 0 and l_max > 0:
+                assert st["distance_passes"] == 2  # (the record buffer of a collapsed load starts at n_distinct entries)
+            assert_same_network(got, want)
+        if l_max <= 1:
+            got, st = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_FAST_L1: 1})
+            assert st["join_mode"] == 2
+            assert_same_network(got, want)
+        got, st = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_SEGMENT_JOIN: 0})
+        assert st["join_mode"] == 0
+        assert_same_network(got, want)
+    # beyond the thresholds the join serves, the rectangular mode and early exit off: the other kernels
+    got, st = gpu_network(pkg, d.residues, d.lengths, 5)
+    assert st["join_mode"] == 0
+    got, st = gpu_network(pkg, d.residues, d.lengths, 2, {pkg.OPT_EARLY_EXIT: 0})
+    assert st["join_mode"] == 0
 
 
 def test_prefix_trie_shared_prefixes_and_short_buckets(pkg, oracle):
@@ -136,9 +170,17 @@ def test_prefix_trie_shared_prefixes_and_short_buckets(pkg, oracle):
     for l_max, opts in ((0, {}), (1, {}), (2, {}), (3, {pkg.OPT_TRIE_CHUNK: 256}), (4, {}), (4, {pkg.OPT_TRIE_CHUNK: 512}),
                         (6, {pkg.OPT_FIRST_CHECK: 3})):
         want = oracle.network(res, ln, l_max, tier=0)[:3]
-        got, st = gpu_network(pkg, res, ln, l_max, opts)
-        assert (st["work_items_trie"] > 0) == (l_max <= 4)
+        got, st = gpu_network(pkg, res, ln, l_max, {pkg.OPT_SEGMENT_JOIN: 0, **opts})
+        assert (st["work_items_trie"] > 0) == (l_max <= 4) and st["join_mode"] == 0
         assert_same_network(got, want)
+        # the default path: the segment join for the buckets long enough to be cut into l_max + 1 segments, the
+        # text-chunk kernel for the shorter ones (lengths 3..19 here: both occur for l_max >= 3)
+        got, st = gpu_network(pkg, res, ln, l_max, opts)
+        assert (st["join_mode"] >= 1) == (l_max <= 4)
+        assert_same_network(got, want)
+        if l_max <= 1:
+            got, st = gpu_network(pkg, res, ln, l_max, {pkg.OPT_FAST_L1: 1})
+            assert_same_network(got, want)
 
 
 def test_device_load_equals_host_load(pkg):
@@ -350,32 +392,59 @@ def test_device_side_validation(pkg):
         with pytest.raises(pkg.TcrNetError) as e:
             net.load(res, torch.tensor([10, 10], dtype=torch.int32, device="cuda"))
         assert e.value.status == pkg.ERR_RESIDUE
+        # total_len must equal sum(lengths), with or without repeated rows, collapse on or off (a residue buffer one
+        # byte too short / too long; the binding passes residues.numel() as total_len)
+        for dedup in (1, 0):
+            net.set_option(pkg.OPT_DEDUP, dedup)
+            for rows in (["CASSLF", "CASSF", "CASSLF", "CASSLF", "CAF"], ["CASSLF", "CASSF", "CAWF"]):
+                r, ln = from_strings(rows)
+                r_d, ln_d = torch.from_numpy(r).cuda(), torch.from_numpy(ln).cuda()
+                net.load(r_d, ln_d)
+                for bad in (r_d[:-1], torch.cat([r_d, r_d[:1]])):
+                    with pytest.raises(pkg.TcrNetError) as e:
+                        net.load(bad, ln_d)
+                    assert e.value.status == pkg.ERR_ARG
 
 
 # ------------------------------------------------------------------ BASELINE.json's large configs
-def _sampled_parity(pkg, oracle, name, l_max, n_sample, seed):
+def _sampled_parity(pkg, oracle, name, l_max, n_sample, seed, opts=None):
+    """What the oracle cannot compute in full: (i) the FULL neighbourhoods of n_sample uniformly drawn nodes (drawn from
+    the generator's row count alone, never from the GPU's output) against the tier-1 oracle, every partner visited;
+    (ii) EVERY edge the GPU emitted has oracle distance <= l_max (no spurious edge anywhere in the network);
+    (iii) CSR invariants; (iv) the generator-linked lower bound over all family pairs."""
     d = generate(name)
-    (rp, cl, dg), st = gpu_network(pkg, d.residues, d.lengths, l_max)
+    (rp, cl, dg), st = gpu_network(pkg, d.residues, d.lengths, l_max, opts)
     check_csr_invariants(rp, cl, dg, d.n)
     rng = np.random.default_rng(seed)
-    # half uniformly random nodes, half nodes the GPU says have neighbours (so the test sees edges)
-    nodes = np.unique(np.concatenate([rng.choice(d.n, n_sample // 2, replace=False),
-                                      rng.choice(np.nonzero(dg > 0)[0], n_sample // 2, replace=False)]))
-    pairs, _ = oracle.edges(d.residues, d.lengths, l_max, rows=nodes, all_partners=True, tier=0)
-    want = neighbours_from_pairs(pairs, nodes)
-    got = neighbours_from_csr(rp, cl, nodes)
+    nodes = np.sort(rng.choice(d.n, n_sample, replace=False))
+    pairs, _ = oracle.edges(d.residues, d.lengths, l_max, rows=nodes, all_partners=True, tier=1)
+    order = np.argsort(pairs[:, 0], kind="stable")
+    pairs = pairs[order]
+    cuts = np.searchsorted(pairs[:, 0], nodes, side="left"), np.searchsorted(pairs[:, 0], nodes, side="right")
+    # the GPU's neighbourhoods of the sampled nodes: upper part from the node's own row, lower part from the rows
+    # that list the node as a column
+    rows_of = np.repeat(np.arange(d.n, dtype=np.int64), np.diff(rp))
+    hit = np.nonzero(np.isin(cl, nodes))[0]
+    lower_of = {}
+    for e in hit:
+        lower_of.setdefault(int(cl[e]), []).append(int(rows_of[e]))
     n_edges_seen = 0
-    for u in nodes:
-        assert np.array_equal(got[int(u)], want[int(u)]), f"node {u}"
-        assert dg[u] == want[int(u)].size
-        n_edges_seen += want[int(u)].size
+    for k, u in enumerate(nodes):
+        want = np.sort(pairs[cuts[0][k]:cuts[1][k], 1])
+        got = np.sort(np.concatenate([np.array(lower_of.get(int(u), []), dtype=np.int64),
+                                      cl[rp[u]:rp[u + 1]].astype(np.int64)]))
+        assert np.array_equal(got, want), f"node {u}"
+        assert dg[u] == want.size
+        n_edges_seen += want.size
     assert n_edges_seen > 0
-    # generator-linked lower bound over ALL family pairs: edits sum <= l_max  =>  edge
+    # (ii) no spurious edge: the oracle's distance of every emitted pair
+    all_pairs = np.stack([rows_of, cl.astype(np.int64)], axis=1)
+    dist = oracle.lev_pairs(d.residues, d.lengths, all_pairs)
+    assert int(dist.max(initial=0)) <= l_max, f"{int((dist > l_max).sum())} emitted edges are farther apart than l_max"
+    # (iv) generator-linked lower bound over ALL family pairs: edits sum <= l_max  =>  edge
     order = np.argsort(d.family, kind="stable")
     fam = d.family[order]
     starts = np.nonzero(np.diff(fam, prepend=-2))[0]
-    keys = set()
-    rows_of = np.repeat(np.arange(d.n, dtype=np.int64), np.diff(rp))
     edge_keys = rows_of * d.n + cl
     must = []
     for a, b in zip(starts, list(starts[1:]) + [fam.size]):
@@ -390,16 +459,58 @@ def _sampled_parity(pkg, oracle, name, l_max, n_sample, seed):
             break
     must = np.array(must, dtype=np.int64)
     assert must.size > 0 and np.isin(must, edge_keys).all()
-    return st
+    return st, (rp, cl, dg)
+
+
+def _golden_digests(name, l_max):
+    """tests/golden/<name>_l<l_max>_network.sha256, written by tests/golden/make_config_hashes.py from the oracle alone."""
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", f"{name}_l{l_max}_network.sha256")
+    if not os.path.exists(path):
+        return None
+    out = {}
+    for line in open(path):
+        if line.startswith("#") or not line.strip():
+            continue
+        k, v = line.split()
+        out[k] = v
+    return out
+
+
+@pytest.mark.parametrize("name,l_max", [("cfg1", 1), ("cfg3", 2), ("cfg4", 1)])
+def test_whole_network_equals_the_oracles_digest(pkg, name, l_max):
+    """The WHOLE network of the config (default launch configuration, what bench.py times) against the tier-1 oracle's
+    network: SHA-256 of the exact bytes tcrnet_copy_csr hands back (row_ptr, col, deg) equal the stored digests the
+    oracle-only script wrote.  PAPER.md:297 (edge rule), 301-318 (adjacency), 224 (degrees)."""
+    import hashlib
+    want = _golden_digests(name, l_max)
+    assert want is not None, "run tests/golden/make_config_hashes.py"
+    d = generate(name)
+    assert hashlib.sha256(d.residues.tobytes() + d.lengths.astype("<i4").tobytes()).hexdigest() == want["sha256_input"]
+    (rp, cl, dg), st = gpu_network(pkg, d.residues, d.lengths, l_max)
+    assert int(rp[-1]) == int(want["n_edges"]) and int(dg.max()) == int(want["max_degree"])
+    assert int((dg == 0).sum()) == int(want["n_isolated"])
+    b_rp, b_cl, b_dg = (np.ascontiguousarray(rp, dtype="<i8").tobytes(), np.ascontiguousarray(cl, dtype="<i4").tobytes(),
+                        np.ascontiguousarray(dg, dtype="<i4").tobytes())
+    assert hashlib.sha256(b_rp).hexdigest() == want["sha256_row_ptr"]
+    assert hashlib.sha256(b_cl).hexdigest() == want["sha256_col"]
+    assert hashlib.sha256(b_dg).hexdigest() == want["sha256_deg"]
+    assert hashlib.sha256(b_rp + b_cl + b_dg).hexdigest() == want["sha256_all"]
+    if name == "cfg4":
+        assert st["pairs_all"] == 800000 * 799999 // 2 and st["distance_passes"] == 1
+    # the prefix-trie path gives the same bytes
+    (rp2, cl2, dg2), st2 = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_SEGMENT_JOIN: 0})
+    assert st2["join_mode"] == 0
+    assert_same_network((rp2, cl2, dg2), (rp, cl, dg))
 
 
 def test_cfg3_sampled(pkg, oracle):
-    _sampled_parity(pkg, oracle, "cfg3", 2, 64, 3)
+    _sampled_parity(pkg, oracle, "cfg3", 2, 2000, 3)
 
 
 def test_cfg4_sampled_headline_config(pkg, oracle):
     """N = 800,000, l_max = 1: the configuration bench.py times, default launch configuration."""
-    st = _sampled_parity(pkg, oracle, "cfg4", 1, 48, 4)
+    st, _ = _sampled_parity(pkg, oracle, "cfg4", 1, 2000, 4)
     assert st["pairs_all"] == 800000 * 799999 // 2
     assert st["distance_passes"] == 1
 
@@ -417,8 +528,17 @@ def test_cfg4_whole_network_is_the_same_row_by_row(pkg):
 
 
 def test_cfg5_sampled(pkg, oracle):
-    """N = 2,000,000, l_max = 3, lengths 5..40 (patterns > 32 use 64-bit words)."""
-    _sampled_parity(pkg, oracle, "cfg5", 3, 24, 5)
+    """N = 2,000,000, l_max = 3, length law N(16,3) clipped to [5,40] (the longest row drawn is 30).  The whole network is beyond the oracle
+    (about 125 core-hours): 2,000 uniformly drawn nodes' full neighbourhoods, every one of the ~2e7 emitted edges checked
+    against the oracle's distance, and the default path byte-equal to the prefix-trie path on a 300,000-row prefix."""
+    st, net = _sampled_parity(pkg, oracle, "cfg5", 3, 2000, 5)
+    d = generate("cfg5")
+    n = 300000
+    off = int(d.lengths[:n].astype(np.int64).sum())
+    a, _ = gpu_network(pkg, d.residues[:off], d.lengths[:n], 3)
+    b, stb = gpu_network(pkg, d.residues[:off], d.lengths[:n], 3, {pkg.OPT_SEGMENT_JOIN: 0})
+    assert stb["join_mode"] == 0
+    assert_same_network(a, b)
 
 
 # ------------------------------------------------------------------ 8(e): shards; 8(f): labels, sweep, query mode
