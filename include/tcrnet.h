@@ -176,8 +176,10 @@ typedef struct tcrnet_stats {
     int64_t join_candidates;   /* ... pairs handed to the recurrence / the l_max <= 1 check        */
     int64_t work_items_join;   /* work items (32 patterns) of the join kernels                    */
     int64_t join_index_entries;/* (text, segment) entries of the index                            */
-    int32_t join_mode;         /* 0: not used, 1: join + recurrence, 2: join + l_max <= 1 fast path */
+    int32_t join_mode;         /* 0: not used, 1: join + banded verification (l_max >= 2), 2: join at l_max <= 1,
+                                  where the verification is the XOR / prefix-suffix check                */
     int32_t pad2_;
+    int64_t join_survivors;    /* segment join: candidates that passed the filters and were verified (COUNT_WORK) */
 } tcrnet_stats;
 
 /*

@@ -1,5 +1,5 @@
-// Step A1 (pack): validation, length histogram and the re-layout of the sequences into the two
-// tables the distance kernel reads (residues "saved as a number ... BYTE";
+// Step A1 (pack): validation, length histogram and the re-layout of the sequences into the
+// tables the distance kernels read (residues "saved as a number ... BYTE";
 // north_star subsystem (1): 5-bit residue codes, sorted by length, bucketed by length).
 //
 //   pat : one row per sorted position, one residue code (0..25) per byte, row stride
@@ -10,6 +10,10 @@
 //         and read with one broadcast 128-bit load per four columns.  The code sits in a
 //         32-bit word so that the per-column Peq address is a single IMAD (code * row_bytes
 //         + lane offset) on the FMA pipe, leaving the ALU pipe to the bit-vector recurrence.
+//         Written on demand (k_txt_from_pat): only the prefix-trie / text-chunk kernels read it.
+//   planes : one row of 8 words per sorted position: plane k = bit k of the 5-bit code of every residue
+//         (north_star (1): 5-bit codes, here one bit of the code per word so that a residue-wise comparison of two
+//         sequences under any shift is five XORs) + the length - what the segment join reads (segjoin.cu).
 #include "tcrnet_internal.h"
 
 namespace tcrnet {
@@ -65,15 +69,16 @@ __global__ void __launch_bounds__(256) k_seq_keys(const uint8_t* __restrict__ re
 }
 
 // One thread per sorted position: the pattern row is written with 128-bit stores (pat_stride is a
-// multiple of 16), the text row with one 128-bit store per four columns.
+// multiple of 16), the text row (TXT: only when the trie / text-chunk kernels will run) with one 128-bit store per
+// four columns, the bit-plane row (segjoin.cu) as 8 words of W.
+template <typename W, bool TXT>
 __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residues,
                                              const int64_t* __restrict__ offsets,
                                              const int32_t* __restrict__ lengths,
                                              const int32_t* __restrict__ perm, int64_t n,
                                              const __grid_constant__ LengthTable lt, int pat_stride,
                                              uint8_t* __restrict__ pat, uint32_t* __restrict__ txt,
-                                             uint32_t* __restrict__ seq5, int s5_words,
-                                             uint32_t* __restrict__ flags) {
+                                             W* __restrict__ planes, uint32_t* __restrict__ flags) {
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;  // sorted position
     bool bad = false;
     if (s < n) {
@@ -82,7 +87,8 @@ __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residu
         const uint8_t* src = residues + offsets[o];
         uint4* prow = reinterpret_cast<uint4*>(pat + (size_t)s * pat_stride);
         const int rw = lt.row_words[len];
-        uint4* trow = reinterpret_cast<uint4*>(txt + lt.txt_base[len] + (int64_t)(s - lt.start[len]) * rw);
+        uint4* trow = TXT ? reinterpret_cast<uint4*>(txt + lt.txt_base[len] + (int64_t)(s - lt.start[len]) * rw) : nullptr;
+        W pl[5] = {W(0), W(0), W(0), W(0), W(0)};
         for (int i0 = 0; i0 < pat_stride; i0 += 16) {
             uint32_t c[16];
 #pragma unroll
@@ -95,45 +101,69 @@ __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residu
                         bad = true;
                         c[k] = 0;
                     }
+#pragma unroll
+                    for (int b = 0; b < 5; ++b) pl[b] |= (W)((c[k] >> b) & 1u) << i;
                 }
             }
             uint32_t w4[4];
 #pragma unroll
             for (int k = 0; k < 4; ++k) w4[k] = c[4 * k] | (c[4 * k + 1] << 8) | (c[4 * k + 2] << 16) | (c[4 * k + 3] << 24);
             prow[i0 >> 4] = make_uint4(w4[0], w4[1], w4[2], w4[3]);
+            if (TXT) {
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const int i = i0 + 4 * k;  // text columns i .. i+3
-                if (i < rw) {
-                    uint32_t t[4];
+                for (int k = 0; k < 4; ++k) {
+                    const int i = i0 + 4 * k;  // text columns i .. i+3
+                    if (i < rw) {
+                        uint32_t t[4];
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) t[q] = i + q < len ? c[4 * k + q] : (uint32_t)kPadCode;
-                    trow[i >> 2] = make_uint4(t[0], t[1], t[2], t[3]);
+                        for (int q = 0; q < 4; ++q) t[q] = i + q < len ? c[4 * k + q] : (uint32_t)kPadCode;
+                        trow[i >> 2] = make_uint4(t[0], t[1], t[2], t[3]);
+                    }
                 }
             }
         }
-        // seq5: the same codes as one little-endian bit string, residue j in bits [5j, 5j + 5), zero beyond
-        // the sequence; s5_words 32-bit words per row (a multiple of 4: rows are read with 128-bit loads)
-        uint32_t* srow = seq5 + (size_t)s * s5_words;
-        unsigned long long acc = 0ull;
-        int filled = 0, w = 0;
-        for (int i = 0; i < len; ++i) {
-            uint32_t c = (uint32_t)src[i] - (uint32_t)'A';
-            if (c >= (uint32_t)kNumCodes) c = 0;
-            acc |= (unsigned long long)c << filled;
-            filled += 5;
-            if (filled >= 32) {
-                srow[w++] = (uint32_t)acc;
-                acc >>= 32;
-                filled -= 32;
-            }
-        }
-        for (; w < s5_words; ++w) {
-            srow[w] = (uint32_t)acc;
-            acc = 0ull;
+        // bit-plane row: planes 0..4, the length, two zero words
+        W* row = planes + (size_t)s * kPlaneWords;
+        if (sizeof(W) == 4) {
+            uint4* r4 = reinterpret_cast<uint4*>(row);
+            r4[0] = make_uint4((uint32_t)pl[0], (uint32_t)pl[1], (uint32_t)pl[2], (uint32_t)pl[3]);
+            r4[1] = make_uint4((uint32_t)pl[4], (uint32_t)len, 0u, 0u);
+        } else {
+            ulonglong2* r2 = reinterpret_cast<ulonglong2*>(row);
+            r2[0] = make_ulonglong2((unsigned long long)pl[0], (unsigned long long)pl[1]);
+            r2[1] = make_ulonglong2((unsigned long long)pl[2], (unsigned long long)pl[3]);
+            r2[2] = make_ulonglong2((unsigned long long)pl[4], (unsigned long long)len);
+            r2[3] = make_ulonglong2(0ull, 0ull);
         }
     }
     if (__syncthreads_or(bad) && threadIdx.x == 0) atomicOr(flags, kFlagBadResidue);
+}
+
+// The text rows of the trie / text-chunk kernels from the pattern rows (same codes, one 32-bit word per column,
+// padded with kPadCode): written only when a build needs those kernels (tcrnet_api.cu: ensure_text_tables).
+__global__ void __launch_bounds__(256) k_txt_from_pat(const uint8_t* __restrict__ pat, int pat_stride, int64_t n,
+                                                     const __grid_constant__ LengthTable lt, uint32_t* __restrict__ txt) {
+    const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    int len = 0;
+    {
+        int lo = 0, hi = kNumLen;  // start[lo] <= s < start[hi]
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if ((int64_t)lt.start[mid] <= s) lo = mid; else hi = mid;
+        }
+        len = lo;
+    }
+    const int rw = lt.row_words[len];
+    uint4* trow = reinterpret_cast<uint4*>(txt + lt.txt_base[len] + (int64_t)(s - lt.start[len]) * rw);
+    const uint32_t* prow = reinterpret_cast<const uint32_t*>(pat + (size_t)s * pat_stride);
+    for (int i = 0; i < rw; i += 4) {
+        const uint32_t w = prow[i >> 2];
+        uint32_t t[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) t[q] = i + q < len ? ((w >> (8 * q)) & 0xffu) : (uint32_t)kPadCode;
+        trow[i >> 2] = make_uint4(t[0], t[1], t[2], t[3]);
+    }
 }
 
 }  // namespace
@@ -157,10 +187,23 @@ cudaError_t launch_seq_keys(const uint8_t* residues, const int64_t* offsets, con
 
 cudaError_t launch_pack(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths,
                         const int32_t* perm, int64_t n, const LengthTable& lt, int pat_stride, uint8_t* pat,
-                        uint32_t* txt, uint32_t* seq5, int s5_words, uint32_t* flags, cudaStream_t s, int* launches) {
-    const int64_t blocks = (n + 255) / 256;
-    k_pack<<<(unsigned)blocks, 256, 0, s>>>(residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, seq5, s5_words,
-                                            flags);
+                        uint32_t* txt, void* planes, bool wide_planes, uint32_t* flags, cudaStream_t s, int* launches) {
+    const unsigned blocks = (unsigned)((n + 255) / 256);
+    if (wide_planes) {
+        if (txt) k_pack<uint64_t, true><<<blocks, 256, 0, s>>>(residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint64_t*)planes, flags);
+        else k_pack<uint64_t, false><<<blocks, 256, 0, s>>>(residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint64_t*)planes, flags);
+    } else {
+        if (txt) k_pack<uint32_t, true><<<blocks, 256, 0, s>>>(residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint32_t*)planes, flags);
+        else k_pack<uint32_t, false><<<blocks, 256, 0, s>>>(residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint32_t*)planes, flags);
+    }
+    *launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_txt_from_pat(const uint8_t* pat, int pat_stride, int64_t n, const LengthTable& lt, uint32_t* txt,
+                                cudaStream_t s, int* launches) {
+    if (n <= 0) return cudaSuccess;
+    k_txt_from_pat<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(pat, pat_stride, n, lt, txt);
     *launches += 1;
     return cudaGetLastError();
 }

@@ -113,7 +113,9 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
     lt.start[kNumLen] = (int32_t)pos;
     lt.txt_base[kNumLen] = words;
     set.pat_stride = (max_len + 15) & ~15;
-    set.s5_words = seq5_words(max_len);
+    set.wide_planes = max_len > 32;
+    set.text_tables = false;
+    set.trie_nodes = 0;
 
     // offsets, stable sort by (length, first residues, row), re-layout
     DevBuf& offsets = ctx->offsets;
@@ -125,8 +127,7 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
     if (rc == TCRNET_OK) rc = dev_reserve(ctx, ctx->perm_tmp, sizeof(int32_t) * (size_t)n);
     if (rc == TCRNET_OK) rc = dev_reserve(ctx, set.perm, sizeof(int32_t) * (size_t)n);
     if (rc == TCRNET_OK) rc = dev_reserve(ctx, set.pat, (size_t)n * set.pat_stride);
-    if (rc == TCRNET_OK) rc = dev_reserve(ctx, set.txt, sizeof(uint32_t) * (size_t)(words + 4));
-    if (rc == TCRNET_OK) rc = dev_reserve(ctx, set.seq5, sizeof(uint32_t) * ((size_t)n * set.s5_words + 16));  // + slack: row_bits reads one word ahead
+    if (rc == TCRNET_OK) rc = dev_reserve(ctx, set.planes, (size_t)n * kPlaneWords * (set.wide_planes ? 8 : 4));
     if (rc != TCRNET_OK) return rc;
     // Sort key: (length, first kSortPrefix residues, row): one composite 64-bit key per row, stable LSD
     // radix sort with the row as payload.  The sub-order inside a length bucket is free (results are mapped
@@ -157,27 +158,8 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
     }
     if (e == cudaSuccess)
         e = launch_pack(d_res, d_off, d_len, (const int32_t*)set.perm.p, n, lt, set.pat_stride,
-                        (uint8_t*)set.pat.p, (uint32_t*)set.txt.p, (uint32_t*)set.seq5.p, set.s5_words, &dc->flags, s,
-                        launches);
-    // prefix trie over the sorted texts (trie.cu); scratch: lcp8 + per-tile counts
-    DevBuf& trie_scratch = ctx->trie_scratch;
-    if (e == cudaSuccess) {
-        size_t node_total = 0, level_off[kTrieDepth + 1] = {};
-        for (int k = 1; k <= kTrieDepth; ++k) {
-            level_off[k] = node_total;
-            node_total += (size_t)trie_level_capacity(n, k);
-        }
-        const size_t lcp_bytes = (((size_t)n + 15) & ~(size_t)15) + 256;  // keeps the tile counts aligned
-        rc = dev_reserve(ctx, set.trie, node_total * sizeof(TrieNode));
-        if (rc == TCRNET_OK) rc = dev_reserve(ctx, trie_scratch, lcp_bytes + (size_t)trie_tiles(n) * 8 * sizeof(uint32_t));
-        if (rc == TCRNET_OK) {
-            for (int k = 1; k <= kTrieDepth; ++k) set.trie_levels.p[k] = (TrieNode*)set.trie.p + level_off[k];
-            set.trie_levels.p[0] = nullptr;
-            e = launch_trie_build((const uint32_t*)set.txt.p, lt, n, (uint8_t*)trie_scratch.p,
-                                  (uint32_t*)((uint8_t*)trie_scratch.p + (lcp_bytes & ~(size_t)255)), set.trie_levels,
-                                  dc->trie_counts, dc->trie_root, s, launches);
-        }
-    }
+                        (uint8_t*)set.pat.p, nullptr, set.planes.p, set.wide_planes, &dc->flags, s, launches);
+    // (the text rows and the prefix trie are built by ensure_text_tables when a build needs them)
     // collapsed load: the rows were the distinct sequences; perm (position -> uid) has served the pack and now
     // becomes position -> row, or kGroupFlag | uid of a shared sequence
     if (rc == TCRNET_OK && e == cudaSuccess && code_groups)
@@ -190,17 +172,51 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
     if (rc != TCRNET_OK) return rc;
     TRY_CUDA(e);
     if (ctx->h_ctrl->flags & kFlagBadResidue) return TCRNET_ERR_RESIDUE;
+    set.n = n;
+    set.total_len = total_len;
+    set.min_len = min_len;
+    set.max_len = max_len;
+    set.loaded = true;
+    return TCRNET_OK;
+}
+
+// The tables only the prefix-trie / text-chunk kernels read: text rows (one 32-bit word per column) expanded from the
+// pattern rows and the prefix trie over them (trie.cu).  Built when a build first schedules one of those kernels (the
+// segment join, the default for l_max <= 4, needs neither).
+int ensure_text_tables(tcrnet_ctx* ctx, SeqSet& set, int* launches) {
+    if (set.text_tables) return TCRNET_OK;
+    cudaStream_t s = ctx->stream;
+    HostCtrl* dc = d_ctrl(ctx);
+    const int64_t n = set.n;
+    const LengthTable& lt = set.lt;
+    TRY(dev_reserve(ctx, set.txt, sizeof(uint32_t) * (size_t)(lt.txt_base[kNumLen] + 4)));
+    TRY_CUDA(launch_txt_from_pat((const uint8_t*)set.pat.p, set.pat_stride, n, lt, (uint32_t*)set.txt.p, s, launches));
+    size_t node_total = 0, level_off[kTrieDepth + 1] = {};
+    for (int k = 1; k <= kTrieDepth; ++k) {
+        level_off[k] = node_total;
+        node_total += (size_t)trie_level_capacity(n, k);
+    }
+    const size_t lcp_bytes = (((size_t)n + 15) & ~(size_t)15) + 256;  // keeps the tile counts aligned
+    DevBuf& trie_scratch = ctx->trie_scratch;
+    TRY(dev_reserve(ctx, set.trie, node_total * sizeof(TrieNode)));
+    TRY(dev_reserve(ctx, trie_scratch, lcp_bytes + (size_t)trie_tiles(n) * 8 * sizeof(uint32_t)));
+    for (int k = 1; k <= kTrieDepth; ++k) set.trie_levels.p[k] = (TrieNode*)set.trie.p + level_off[k];
+    set.trie_levels.p[0] = nullptr;
+    TRY_CUDA(cudaMemsetAsync(dc->trie_counts, 0, sizeof(dc->trie_counts) + sizeof(dc->trie_root), s));
+    static_assert(offsetof(HostCtrl, trie_root) == offsetof(HostCtrl, trie_counts) + sizeof(uint32_t) * 8, "one memset");
+    TRY_CUDA(launch_trie_build((const uint32_t*)set.txt.p, lt, n, (uint8_t*)trie_scratch.p,
+                               (uint32_t*)((uint8_t*)trie_scratch.p + (lcp_bytes & ~(size_t)255)), set.trie_levels,
+                               dc->trie_counts, dc->trie_root, s, launches));
+    TRY_CUDA(cudaMemcpyAsync(ctx->h_ctrl->trie_counts, dc->trie_counts, sizeof(dc->trie_counts) + sizeof(dc->trie_root),
+                             cudaMemcpyDeviceToHost, s));
+    TRY_CUDA(cudaStreamSynchronize(s));
     // level-1 node range of every bucket (empty buckets get an empty range)
     set.trie_root[kNumLen] = ctx->h_ctrl->trie_counts[1];
     for (int l = kNumLen - 1; l >= 0; --l)
         set.trie_root[l] = set.hist[l] ? ctx->h_ctrl->trie_root[l] : set.trie_root[l + 1];
     set.trie_nodes = 0;
     for (int k = 1; k <= kTrieDepth; ++k) set.trie_nodes += ctx->h_ctrl->trie_counts[k];
-    set.n = n;
-    set.total_len = total_len;
-    set.min_len = min_len;
-    set.max_len = max_len;
-    set.loaded = true;
+    set.text_tables = true;
     return TCRNET_OK;
 }
 
@@ -289,7 +305,7 @@ int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len
     ctx->stats.total_len = total_len;
     ctx->stats.min_len = ctx->all.min_len;
     ctx->stats.max_len = ctx->all.max_len;
-    ctx->stats.trie_nodes = ctx->all.trie_nodes;
+    ctx->stats.trie_nodes = 0;  // (built on demand: ensure_text_tables)
     ctx->loaded = true;
     return TCRNET_OK;
 }
@@ -354,8 +370,8 @@ void make_join_tables(int l_max, JoinTables& tab) {
 
 // Step A2, host side: the (pattern bucket, text bucket) pairs with len_t - len_p in 0..l_max
 // (kPairsAllQuery: 1..l_max; the equal-length pairs belong to the kPairsQueryAll pass).
-void schedule_pass(const tcrnet_ctx* ctx, int l_max, int first_check, bool use_join, Schedule::Pass& pass,
-                   tcrnet_stats& st) {
+void schedule_pass(const tcrnet_ctx* ctx, int l_max, int first_check, bool use_join, const JoinTables& tab,
+                   Schedule::Pass& pass, tcrnet_stats& st) {
     const SeqSet& ps = *pass.pset;
     const SeqSet& ts = *pass.tset;
     // The trie kernel serves the rows whose early exit can act inside the trie (l_max <= kTrieMaxL, the
@@ -374,7 +390,7 @@ void schedule_pass(const tcrnet_ctx* ctx, int l_max, int first_check, bool use_j
             st.columns_kept += pairs * n;
             if (pairs == 0) continue;
             if (use_join && n >= l_max + 1) {  // the text can be cut into l_max + 1 non-empty segments
-                std::vector<JoinRow>& jr = pass.join_rows[m <= 32 ? 0 : 1];
+                std::vector<JoinRow>& jr = pass.join_rows[0];  // (one launch: the word size belongs to the set's plane rows)
                 if (jr.empty() || jr.back().m != m) {
                     JoinRow r{};
                     r.m = m;
@@ -421,16 +437,14 @@ void schedule_pass(const tcrnet_ctx* ctx, int l_max, int first_check, bool use_j
         }
     for (int wide = 0; wide < 2; ++wide) {
         std::vector<JoinRow>& jr = pass.join_rows[wide];
-        auto weight = [](const JoinRow& r) {
-            long double t = 0;
-            for (int d = 0; d < kJoinMaxSeg; ++d) t += r.t_count[d];
-            return t * r.p_count;
-        };
-        std::stable_sort(jr.begin(), jr.end(), [&](const JoinRow& a, const JoinRow& b) { return weight(a) > weight(b); });
         pass.join_items[wide] = 0;
         for (JoinRow& r : jr) {
+            // a work item = 32 patterns x one probe of one length difference that has texts
+            r.probe_cum[0] = 0;
+            for (int d = 0; d < kJoinMaxSeg; ++d)
+                r.probe_cum[d + 1] = r.probe_cum[d] + (d <= l_max && r.t_count[d] > 0 ? tab.n_probes[d] : 0);
             r.item_begin = pass.join_items[wide];
-            pass.join_items[wide] += (r.p_count + 31) / 32;
+            pass.join_items[wide] += (int64_t)((r.p_count + 31) / 32) * r.probe_cum[kJoinMaxSeg];
         }
     }
 }
@@ -466,11 +480,14 @@ void make_schedule(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule& 
     // The join serves the all-pairs mode with the early exit on (its verification always votes); the rectangular
     // mode and l_max beyond the specialised range stay with the trie / text-chunk kernels.
     const bool can_join = !ctx->query.loaded && ctx->early_exit && l_max <= kTrieMaxL;
+    // (TCRNET_OPT_FAST_L1 forces the join for l_max <= 1: its verification IS the XOR / prefix-suffix check there)
     sch.fast_l1 = can_join && ctx->fast_l1 && l_max <= 1;
     sch.use_join = sch.fast_l1 || (can_join && (ctx->segment_join == 1 ||
                                                 (ctx->segment_join < 0 && ctx->prefix_trie)));
+    JoinTables tab;
+    make_join_tables(std::min(l_max, kTrieMaxL), tab);
     for (Schedule::Pass& pass : sch.passes) {
-        schedule_pass(ctx, l_max, first_check, sch.use_join, pass, st);
+        schedule_pass(ctx, l_max, first_check, sch.use_join, tab, pass, st);
         for (int trie = 0; trie < 2; ++trie)
             for (int wide = 0; wide < 2; ++wide) {
                 st.work_items += pass.part[trie][wide].items;
@@ -483,7 +500,7 @@ void make_schedule(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule& 
             sch.n_join_rows += pass.join_rows[wide].size();
         }
     }
-    st.join_mode = sch.n_join_rows == 0 ? 0 : (sch.fast_l1 ? 2 : 1);
+    st.join_mode = sch.n_join_rows == 0 ? 0 : (l_max <= 1 ? 2 : 1);
 }
 
 int upload_schedule(tcrnet_ctx* ctx, const Schedule& sch) {
@@ -532,7 +549,7 @@ int ensure_join_index(tcrnet_ctx* ctx, int l_max, int* launches) {
     TRY(dev_reserve(ctx, ctx->scan_scratch, scan_scratch_bytes((int64_t)slots)));
     TRY_CUDA(cudaEventRecord(ctx->ev[6], s));
     TRY_CUDA(cudaMemsetAsync(ctx->join_cnt.p, 0, sizeof(uint32_t) * (size_t)slots, s));
-    TRY_CUDA(launch_join_index((const uint32_t*)set.seq5.p, set.s5_words, set.lt, set.n, ctx->join_tab,
+    TRY_CUDA(launch_join_index(set.planes.p, set.wide_planes, set.lt, set.n, ctx->join_tab,
                                (uint32_t*)ctx->join_cnt.p, (uint32_t*)ctx->join_dir.p, (uint2*)ctx->join_entries.p, slots,
                                ctx->scan_scratch.p, s, launches));
     TRY_CUDA(cudaEventRecord(ctx->ev[7], s));
@@ -551,8 +568,9 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
     HostCtrl* dc = d_ctrl(ctx);
     static_assert(offsetof(HostCtrl, queue) == offsetof(HostCtrl, edge_count) + 9 * sizeof(unsigned long long), "one memset");
     static_assert(offsetof(HostCtrl, edge_total) == offsetof(HostCtrl, queue) + kTrieQueues * sizeof(unsigned long long), "one memset");
+    static_assert(offsetof(HostCtrl, cand_count) == offsetof(HostCtrl, edge_total) + sizeof(unsigned long long), "one memset");
     if (expand_only) TRY_CUDA(cudaMemsetAsync(&dc->edge_total, 0, sizeof(unsigned long long), s));
-    else TRY_CUDA(cudaMemsetAsync(&dc->edge_count, 0, sizeof(unsigned long long) * (10 + kTrieQueues), s));  // edge_count, work[8], queue[], edge_total
+    else TRY_CUDA(cudaMemsetAsync(&dc->edge_count, 0, sizeof(unsigned long long) * (11 + kTrieQueues), s));  // edge_count, work[8], queue[], edge_total, cand_count
     TRY_CUDA(cudaMemsetAsync(ctx->row_count.p, 0, sizeof(int32_t) * (size_t)ctx->n, s));
     TRY_CUDA(cudaMemsetAsync(ctx->deg.p, 0, sizeof(int32_t) * (size_t)ctx->n, s));
     int n_queues = 0;
@@ -601,13 +619,12 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
         for (int wide = 0; wide < 2; ++wide) {
             const std::vector<JoinRow>& jr = pass.join_rows[wide];
             if (!jr.empty()) {
-                if (n_queues >= kTrieQueues) return TCRNET_ERR_STATE;
-                p.queue = dc->queue + n_queues++;
                 p.n_items = pass.join_items[wide];
                 JoinIndex index{(const uint32_t*)ctx->join_dir.p, (const uint2*)ctx->join_entries.p, ctx->join_slots - 1u};
-                TRY_CUDA(launch_join(p, d_join_rows, (int)jr.size(), (const uint32_t*)pass.pset->seq5.p, pass.pset->s5_words,
-                                     index, ctx->join_tab, wide != 0, sch.fast_l1, ctx->count_work != 0, ctx->n_sm, s,
-                                     launches));
+                TRY_CUDA(launch_join(p, d_join_rows, (int)jr.size(), pass.pset->planes.p, pass.pset->wide_planes, index,
+                                     ctx->join_tab, (uint2*)ctx->join_cand.p, &dc->cand_count,
+                                     (unsigned long long)(ctx->join_cand.bytes / sizeof(uint2)), ctx->count_work != 0,
+                                     ctx->n_sm, s, launches));
             }
             d_join_rows += jr.size();
         }
@@ -628,6 +645,7 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
     }
     TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->edge_count, &dc->edge_count, sizeof(unsigned long long) * 9,
                              cudaMemcpyDeviceToHost, s));
+    TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->cand_count, &dc->cand_count, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
     TRY_CUDA(cudaStreamSynchronize(s));
     return TCRNET_OK;
 }
@@ -650,7 +668,22 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
     TRY(upload_schedule(ctx, sch));
     st.ms_index = 0.f;
     st.join_index_entries = 0;
-    if (sch.n_join_rows) TRY(ensure_join_index(ctx, l_max, launches));
+    if (sch.n_join_rows) {
+        TRY(ensure_join_index(ctx, l_max, launches));
+        if (l_max >= 2)  // queue of the pairs that pass the filters (grown to the exact count if it proves too small)
+            TRY(dev_reserve(ctx, ctx->join_cand, sizeof(uint2) * (size_t)std::max<int64_t>((int64_t)1 << 20, 8 * ctx->all.n)));
+    }
+    if (sch.n_rows) {  // the prefix-trie / text-chunk kernels run: they read txt (and the trie)
+        for (Schedule::Pass& pass : sch.passes) {
+            TRY(ensure_text_tables(ctx, const_cast<SeqSet&>(*pass.pset), launches));
+            TRY(ensure_text_tables(ctx, const_cast<SeqSet&>(*pass.tset), launches));
+        }
+        // the rows were laid out before the trie roots were known
+        sch = Schedule();
+        make_schedule(ctx, l_max, first_check, sch, st);
+        TRY(upload_schedule(ctx, sch));
+    }
+    st.trie_nodes = ctx->all.trie_nodes;
 
     // distances + emission (second pass only if the edge buffer was too small)
     int64_t cap = ctx->edge_capacity_opt > 0 ? ctx->edge_capacity_opt : std::max<int64_t>((int64_t)1 << 20, 16 * n);
@@ -673,10 +706,17 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
         if (!expand_only) ++st.distance_passes;
         TRY(run_distance(ctx, sch, l_max, first_check, (uint64_t)cap, (uint64_t)cap_b, shard, n_shards, expand_only, launches));
         const int64_t n_rec = (int64_t)ctx->h_ctrl->edge_count;  // pairs recorded by the distance kernels
+        const int64_t n_cand = (int64_t)ctx->h_ctrl->cand_count;
+        if (!expand_only && n_cand > (int64_t)(ctx->join_cand.bytes / sizeof(uint2))) {
+            // the verification queue of the join was too small: grow it to the exact count and run again
+            if (st.distance_passes >= 3) return TCRNET_ERR_CUDA;  // cannot happen: same input
+            TRY(dev_reserve(ctx, ctx->join_cand, sizeof(uint2) * (size_t)n_cand));
+            continue;
+        }
         n_keys = grouped ? (int64_t)ctx->h_ctrl->edge_total : n_rec;
         if (n_rec > ctx->edge_limit || (n_rec <= cap && n_keys > ctx->edge_limit)) return TCRNET_ERR_EDGE_OVERFLOW;
         if (n_rec > cap) {  // the record buffer was too small: grow it to the exact count and run again
-            if (st.distance_passes >= 2) return TCRNET_ERR_CUDA;  // cannot happen: same input
+            if (st.distance_passes >= 3) return TCRNET_ERR_CUDA;  // cannot happen: same input
             cap = n_rec;
             TRY(dev_reserve(ctx, ctx->keys_a, sizeof(unsigned long long) * (size_t)cap));
             continue;
@@ -697,6 +737,8 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
     st.join_probes = (int64_t)ctx->h_ctrl->work[5];
     st.join_entries = (int64_t)ctx->h_ctrl->work[6];
     st.join_candidates = (int64_t)ctx->h_ctrl->work[7];
+    st.join_survivors = st.join_mode ? (int64_t)ctx->h_ctrl->work[4] : 0;
+    if (st.join_mode) st.lane_columns_live = 0;
     if (st.ms_index < 0.f) TRY_CUDA(cudaEventElapsedTime(&st.ms_index, ctx->ev[6], ctx->ev[7]));
     TRY_CUDA(cudaEventRecord(ctx->ev[1], s));
     ctx->n_keys = n_keys;
@@ -820,7 +862,7 @@ void tcrnet_destroy(tcrnet_ctx* ctx) {
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     DevBuf* bufs[] = {&ctx->all.perm, &ctx->all.pat, &ctx->all.txt, &ctx->all.trie, &ctx->query.perm, &ctx->query.pat,
-                      &ctx->query.txt, &ctx->query.trie, &ctx->all.seq5, &ctx->query.seq5, &ctx->join_cnt, &ctx->join_dir,
+                      &ctx->query.txt, &ctx->query.trie, &ctx->all.planes, &ctx->query.planes, &ctx->join_cand, &ctx->join_cnt, &ctx->join_dir,
                       &ctx->join_entries, &ctx->join_rows, &ctx->inv_perm, &ctx->edge_dist, &ctx->edge_dist_b, &ctx->flags,
                       &ctx->flag_pos, &ctx->in_res, &ctx->in_len, &ctx->offsets,
                       &ctx->perm_tmp, &ctx->trie_scratch, &ctx->keys_a, &ctx->keys_b, &ctx->radix_scratch,

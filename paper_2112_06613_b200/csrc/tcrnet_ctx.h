@@ -18,6 +18,7 @@ struct HostCtrl {  // pinned mirror of the small device control block
     unsigned long long work[8];
     unsigned long long queue[kTrieQueues];  // dynamic work queues of the trie launches (zeroed with edge_count)
     unsigned long long edge_total;    // dedup: edges between rows after the expansion of the recorded pairs
+    unsigned long long cand_count;    // segment join, l_max >= 2: pairs queued for verification (zeroed with edge_count)
     unsigned long long probe[3];
     uint32_t flags;
     uint32_t n_long;                  // rows queued for k_sort_long_rows
@@ -37,8 +38,9 @@ struct SeqSet {
     int min_len = 0, max_len = 0;
     LengthTable lt{};
     int pat_stride = 0;
-    DevBuf perm, pat, txt, trie, seq5;
-    int s5_words = 0;  // 32-bit words per row of seq5
+    DevBuf perm, pat, txt, trie, planes;
+    bool wide_planes = false;  // bit-plane rows of 64-bit words (the longest sequence has more than 32 residues)
+    bool text_tables = false;  // txt + trie are built (on demand: only the prefix-trie / text-chunk kernels read them)
     TrieLevels trie_levels{};
     uint32_t trie_root[kNumLen + 1] = {};  // level-1 node range of bucket L: [trie_root[L], trie_root[L+1])
     int64_t trie_nodes = 0;
@@ -89,7 +91,7 @@ struct tcrnet_ctx {
     DevBuf keys_a, keys_b, radix_scratch, scan_scratch, rows, row_ptr, col, deg, row_count, long_rows;
     DevBuf inv_perm, edge_dist, edge_dist_b, flags, flag_pos;
     // segment join (segjoin.cu): directory + entries of the current load for join_l_max, work rows
-    DevBuf join_cnt, join_dir, join_entries, join_rows;
+    DevBuf join_cnt, join_dir, join_entries, join_rows, join_cand;
     int join_l_max = -1;  // threshold the index in join_dir / join_entries was built for (-1: none)
     uint32_t join_slots = 0;
     JoinTables join_tab{};

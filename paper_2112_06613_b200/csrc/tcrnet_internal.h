@@ -107,7 +107,7 @@ struct DistanceParams {
 // If lev(r, s) <= l_max and s is cut into l_max + 1 segments, at least one segment of s occurs unchanged in r
 // (l_max edits touch at most l_max segments), shifted by no more than the edits allow.  The segments of every
 // text are indexed in a hash directory; every pattern probes it with the substrings that could be such a
-// segment, and only the pairs found this way are handed to the column recurrence.
+// segment, and only the pairs found this way are verified.
 constexpr int kJoinMaxSeg = kTrieMaxL + 1;  // segments per text: l_max + 1 <= 5
 constexpr int kJoinMaxProbes = 28;          // (segment, shift) probes per length difference
 struct JoinTables {
@@ -118,20 +118,25 @@ struct JoinTables {
     int8_t n_seg;                                 // l_max + 1
     int8_t pad_[6];
 };
-// One pattern bucket of the join kernels: its 32-pattern tiles are the work items; texts = the buckets of
-// length m .. m + l_max that are indexed (t_count 0: none).
+// One pattern bucket of the join: a work item (one warp) is a tile of 32 patterns x ONE probe (delta, segment,
+// shift) against the indexed text bucket of length m + delta (t_count 0: none).
 struct JoinRow {
-    int64_t item_begin;
+    int64_t item_begin;   // first work item of this row; the row has ceil(p_count / 32) * probe_cum[n_seg] of them
     int32_t p_start, p_count;
     int32_t m, pad_;
     int32_t t_start[kJoinMaxSeg];
     int32_t t_count[kJoinMaxSeg];
+    int32_t probe_cum[kJoinMaxSeg + 1];  // [delta] = probes of the smaller deltas that have texts
 };
 struct JoinIndex {
     const uint32_t* dir;  // [slots + 1]: entries of hash bucket b are [dir[b], dir[b+1])
     const uint2* entries; // (tag = high half of the segment hash, sorted position of the text)
     uint32_t mask;        // slots - 1 (a power of two)
 };
+// Bit-plane rows (pack.cu, read by segjoin.cu): sequence at sorted position s = 8 words of W (uint32_t when the set's
+// longest sequence has <= 32 residues: one 32-byte sector per row; else uint64_t): words 0..4 = planes, bit j of
+// plane k = bit k of the 5-bit code of residue j (zero beyond the sequence); word 5 = length; 6, 7 = 0.
+constexpr int kPlaneWords = 8;
 
 // ---- launch wrappers (each returns cudaGetLastError(); *launches is incremented per kernel) ----
 
@@ -165,11 +170,11 @@ cudaError_t launch_seq_keys(const uint8_t* residues, const int64_t* offsets, con
                             unsigned long long* keys, int32_t* vals, cudaStream_t s, int* launches);
 cudaError_t launch_pack(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths,
                         const int32_t* perm, int64_t n, const LengthTable& lt, int pat_stride,
-                        uint8_t* pat, uint32_t* txt, uint32_t* seq5, int s5_words, uint32_t* flags, cudaStream_t s,
-                        int* launches);
-// seq5 row: 32-bit words per sequence of the 5-bit packed table (residue j in bits [5j, 5j+5) of the row's
-// little-endian bit string): 4 words up to 25 residues, 8 up to 51, 12 up to 64
-inline int seq5_words(int max_len) { return 4 * ((5 * max_len + 127) / 128); }
+                        uint8_t* pat, uint32_t* txt /*NULL: not written*/, void* planes, bool wide_planes, uint32_t* flags,
+                        cudaStream_t s, int* launches);
+// txt rows (trie / text-chunk kernels) from the pattern rows, on demand
+cudaError_t launch_txt_from_pat(const uint8_t* pat, int pat_stride, int64_t n, const LengthTable& lt, uint32_t* txt,
+                                cudaStream_t s, int* launches);
 
 // trie.cu: prefix trie over the sorted texts (levels 1..kTrieDepth, all length buckets).
 //   lcp8        : scratch, uint8[round_up(n,16) + 16]
@@ -224,15 +229,15 @@ cudaError_t launch_distance_trie(const DistanceParams& p, int64_t n_items, bool 
 // segjoin.cu
 // Index of the segments of the texts at sorted positions [0, n) with length >= tab.n_seg: cnt (uint32[slots], zeroed
 // by the caller) is consumed, dir gets slots + 1 offsets, entries n_entries pairs.
-cudaError_t launch_join_index(const uint32_t* seq5, int s5_words, const LengthTable& lt, int64_t n, const JoinTables& tab,
+cudaError_t launch_join_index(const void* planes, bool wide, const LengthTable& lt, int64_t n, const JoinTables& tab,
                               uint32_t* cnt, uint32_t* dir, uint2* entries, uint32_t slots, void* scan_scratch,
                               cudaStream_t s, int* launches);
-size_t join_smem_bytes(bool wide);
-// general kernel (verification by the column recurrence) and the l_max <= 1 fast path (XOR / popcount on the packed
-// codes); p carries the emission fields, the queue, n_items and the shard of the launch
-cudaError_t launch_join(const DistanceParams& p, const JoinRow* rows, int n_rows, const uint32_t* seq5, int s5_words,
-                        const JoinIndex& index, const JoinTables& tab, bool wide, bool fast_l1, bool count_work, int n_sm,
-                        cudaStream_t s, int* launches);
+// Probe + filter (+ verification and emission for l_max <= 1); for l_max >= 2 the surviving pairs go to `cand`
+// (at most cand_cap of the *cand_count counted) and a second kernel verifies them (Landau-Vishkin on the mismatch
+// masks of the band's diagonals) and emits.  p carries the emission fields, n_items and the shard of the launch.
+cudaError_t launch_join(const DistanceParams& p, const JoinRow* rows, int n_rows, const void* planes, bool wide,
+                        const JoinIndex& index, const JoinTables& tab, uint2* cand, unsigned long long* cand_count,
+                        unsigned long long cand_cap, bool count_work, int n_sm, cudaStream_t s, int* launches);
 
 // labels.cu: distance labels of the final edges, threshold restriction, key validation
 cudaError_t launch_inverse_perm(const int32_t* perm, int64_t n, int32_t* inv, cudaStream_t s, int* launches);
