@@ -17,9 +17,10 @@
 //
 //   index   k_join_index: one entry (tag, text) per (text, segment), bucketed by a hash of (n, i, segment bits) in a
 //           power-of-two directory (count -> prefix sum -> fill).
-//   probe   k_join_probe: one lane = one (pattern, probe): hash the pattern's substring, walk the directory bucket,
-//           and for every text whose tag matches (same length bucket: only texts after the pattern in sorted order,
-//           so every unordered pair is seen once) build the masks of the band's diagonals
+//   probe   k_join_probe: one warp = 32 patterns of one length x one length difference delta; for every probe each lane
+//           hashes its pattern's substring and walks the directory bucket; the texts whose tag matches (same length
+//           bucket: only texts after the pattern in sorted order, so every unordered pair is seen once) are queued in
+//           shared memory and checked 32 at a time, one per lane: build the masks of the band's diagonals
 //           s = -floor((l_max - delta) / 2) .. delta + floor((l_max - delta) / 2)  (no alignment with <= l_max edits
 //           leaves the band) and apply
 //             - the probe's own segment really matches (M restricted to it is zero: hash collisions die here),
@@ -250,9 +251,11 @@ struct JoinParams {
     const JoinRow* rows;
     int32_t n_rows;
     int32_t pad_;
+    int64_t n_local;                // work items of this shard
     const void* planes;
     JoinIndex index;
-    uint2* cand;                    // l_max >= 2: (pattern, text) pairs that passed the filters
+    uint2* cand;                    // l_max >= 2: (pattern, text) pairs that passed the filters ...
+    uint8_t* cand_probe;            // ... and the probe that found each
     unsigned long long* cand_count; // keeps counting beyond cand_cap
     unsigned long long cand_cap;
     JoinTables tab;
@@ -267,93 +270,170 @@ __device__ __forceinline__ const JoinRow& find_join_row(const JoinParams& S, int
     return S.rows[lo];
 }
 
+// Per-warp staging in shared memory: the texts found by the bucket walks wait in `queue` until 32 of them can be
+// checked at once, one per lane (the walks themselves keep few lanes busy: buckets differ in length and most lanes
+// find nothing in a given step); what passes waits in `out` until 32 results leave with ONE atomic on the global
+// cursor (edge list for l_max <= 1, verification queue beyond).
+struct WarpBuf {
+    uint2 queue[64];     // ring: (owner lane | probe << 5, text)
+    uint2 out[64];       // (pattern, text), sorted positions
+    uint8_t out_probe[64];
+};
+
+template <typename W, int L, bool COUNT>
+struct ProbeWarp {
+    WarpBuf* wb;
+    PlaneRow<W> A;  // this lane's pattern
+    int lane, p0;   // sorted position of lane 0's pattern
+    int m, n, delta, smin, nb;
+    int qhead = 0, qn = 0, on = 0;
+    unsigned long long n_pass = 0;
+};
+
+// the first 32 staged results leave
+template <typename W, int L, bool COUNT>
+__device__ __forceinline__ void flush_out(ProbeWarp<W, L, COUNT>& w, const JoinParams& S, int cnt) {
+    const bool act = w.lane < cnt;
+    const uint2 pt = act ? w.wb->out[w.lane] : make_uint2(0u, 0u);
+    const uint32_t pr = act ? w.wb->out_probe[w.lane] : 0u;
+    uint2 rest = make_uint2(0u, 0u);
+    uint32_t rest_pr = 0u;
+    const bool mv = cnt + w.lane < w.on;  // what stays moves to the front
+    if (mv) rest = w.wb->out[cnt + w.lane], rest_pr = w.wb->out_probe[cnt + w.lane];
+    __syncwarp();
+    if (mv) w.wb->out[w.lane] = rest, w.wb->out_probe[w.lane] = (uint8_t)rest_pr;
+    w.on -= cnt;
+    __syncwarp();
+    if (L <= 1) {
+        emit_edges(S.d, act, w.lane, (int)pt.x, (int)pt.y, w.m, w.n);
+    } else {
+        unsigned long long base = 0;
+        if (w.lane == 0) base = atomicAdd(S.cand_count, (unsigned long long)cnt);
+        base = __shfl_sync(kFullMask, base, 0);
+        if (act && base + w.lane < S.cand_cap) {
+            S.cand[base + w.lane] = pt;
+            S.cand_probe[base + w.lane] = (uint8_t)pr;
+        }
+    }
+}
+
+// the first cnt queued texts are checked, one per lane
+template <typename W, int L, bool COUNT>
+__device__ __forceinline__ void drain_round(ProbeWarp<W, L, COUNT>& w, const JoinParams& S, int cnt) {
+    const bool act = w.lane < cnt;
+    const uint2 q = act ? w.wb->queue[(w.qhead + w.lane) & 63] : make_uint2(0u, 0u);
+    w.qhead = (w.qhead + cnt) & 63;
+    w.qn -= cnt;
+    const int ow = (int)(q.x & 31u), pi = (int)(q.x >> 5), t = (int)q.y;
+    PlaneRow<W> Ao;  // the owner's pattern
+#pragma unroll
+    for (int k = 0; k < 5; ++k) Ao.p[k] = __shfl_sync(kFullMask, w.A.p[k], ow);
+    bool keep = false;
+    if (act) {
+        const PlaneRow<W> B = load_planes<W>(S.planes, t);
+        if (B.len == w.n) {  // (a tag collision across length buckets cannot pass the segment test below either)
+            W M[L + 1];
+            band_masks<W, L>(Ao, B, w.m, w.n, w.smin, w.nb, M);
+            const int i = S.tab.probe_seg[w.delta][pi], d = S.tab.probe_shift[w.delta][pi];
+            const int sq = S.tab.seg_start[w.n][i], len = S.tab.seg_start[w.n][i + 1] - sq;
+            keep = shd_pass<W, L>(M, w.m) && segment_matches<W, L>(M, w.smin, w.nb, sq, len, d, w.m);
+            if (COUNT && keep) ++w.n_pass;
+            if (L <= 1 && keep)
+                keep = first_matching_probe<W, L>(S.tab, M, w.smin, w.nb, w.m, w.n, w.delta, pi) &&
+                       lv_within<W, L>(M, w.m, w.n, w.delta, w.smin, w.nb);
+        }
+    }
+    const uint32_t bal = __ballot_sync(kFullMask, keep);
+    if (keep) {
+        const int pos = w.on + __popc(bal & ((1u << w.lane) - 1u));
+        w.wb->out[pos] = make_uint2((uint32_t)(w.p0 + ow), (uint32_t)t);
+        w.wb->out_probe[pos] = (uint8_t)pi;
+    }
+    w.on += __popc(bal);
+    __syncwarp();
+    if (w.on >= 32) flush_out<W, L, COUNT>(w, S, 32);
+}
+
+// One warp = 32 consecutive patterns of one length x the texts longer by delta: every probe of that delta in turn.
 template <typename W, int L, bool COUNT>
 __global__ void __launch_bounds__(kJoinThreads) k_join_probe(const __grid_constant__ JoinParams S) {
+    __shared__ WarpBuf bufs[kJoinWarps];
     const DistanceParams& P = S.d;
-    const int lane = threadIdx.x & 31;
-    const int64_t local = (int64_t)blockIdx.x * kJoinWarps + (threadIdx.x >> 5);
-    const int64_t n_local = (P.n_items - P.shard + P.n_shards - 1) / P.n_shards;
-    if (local >= n_local) return;  // the whole warp
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t local = (int64_t)blockIdx.x * kJoinWarps + warp;
+    if (local >= S.n_local) return;  // the whole warp
     const int64_t item = local * P.n_shards + P.shard;
     const JoinRow& Rw = find_join_row(S, item);
-    const int m = Rw.m;
-    const int n_pr = Rw.probe_cum[L + 1];
     const int rel = (int)(item - Rw.item_begin);
-    const int tile = rel / n_pr, pr = rel - tile * n_pr;
-    int delta = 0;
-    while (delta < L && pr >= Rw.probe_cum[delta + 1]) ++delta;
-    const int pi = pr - Rw.probe_cum[delta];
-    const int n = m + delta;
-    const int i = S.tab.probe_seg[delta][pi], d = S.tab.probe_shift[delta][pi];
-    const int sq = S.tab.seg_start[n][i], len = S.tab.seg_start[n][i + 1] - sq, rq = sq + d;
-    if (rq < 0 || rq + len > m) return;  // the segment does not fit at this shift (warp-uniform)
-    const int p_rel = tile * 32 + lane;
-    const bool p_valid = p_rel < Rw.p_count;
-    const int p = Rw.p_start + (p_valid ? p_rel : 0);
-    const PlaneRow<W> A = load_planes<W>(S.planes, p);
-    int smin, nb;
-    band_of(L, delta, smin, nb);
+    const int tile = rel / (L + 1), delta = rel - tile * (L + 1);
+    if (Rw.t_count[delta] == 0) return;  // no texts of that length
+    ProbeWarp<W, L, COUNT> w;
+    w.wb = &bufs[warp];
+    w.lane = lane;
+    w.m = Rw.m;
+    w.n = w.m + delta;
+    w.delta = delta;
+    band_of(L, delta, w.smin, w.nb);
+    w.p0 = Rw.p_start + tile * 32;
+    const bool p_valid = tile * 32 + lane < Rw.p_count;
+    const int p = p_valid ? w.p0 + lane : w.p0;
+    w.A = load_planes<W>(S.planes, p);
+    const int m = w.m, n = w.n;
+    unsigned long long n_entries = 0, n_cand = 0, n_probes = 0;
 
-    uint32_t e = 0, e_end = 0, tag = 0;
-    if (p_valid) {
-        const unsigned long long h = seg_hash<W>(A, rq, len, n, i);
-        const uint32_t b = (uint32_t)h & S.index.mask;
-        e = __ldg(S.index.dir + b);
-        e_end = __ldg(S.index.dir + b + 1);
-        tag = (uint32_t)(h >> 32);
-    }
-    unsigned long long n_entries = 0, n_cand = 0, n_pass = 0;
-    uint2 ent = make_uint2(0u, 0u);
-    if (e < e_end) ent = __ldg(S.index.entries + e);
-    while (__any_sync(kFullMask, e < e_end)) {
-        bool keep = false;
-        int t = p;
-        if (e < e_end) {
-            const uint2 cur = ent;
-            ++e;
-            if (e < e_end) ent = __ldg(S.index.entries + e);  // the next entry is on its way while this one is checked
-            if (COUNT) ++n_entries;
-            // same bucket: only the texts after the pattern (every unordered pair once)
-            if (cur.x == tag && (delta > 0 || (int)cur.y > p)) {
-                t = (int)cur.y;
-                const PlaneRow<W> B = load_planes<W>(S.planes, t);
-                if (COUNT) ++n_cand;
-                if (B.len == n) {  // (a tag collision across length buckets cannot pass the segment test below either)
-                    W M[L + 1];
-                    band_masks<W, L>(A, B, m, n, smin, nb, M);
-                    keep = shd_pass<W, L>(M, m) && segment_matches<W, L>(M, smin, nb, sq, len, d, m) &&
-                           first_matching_probe<W, L>(S.tab, M, smin, nb, m, n, delta, pi);
-                    if (COUNT && keep) ++n_pass;
-                    if (L <= 1 && keep) keep = lv_within<W, L>(M, m, n, delta, smin, nb);
-                }
-            }
+    const int np = S.tab.n_probes[delta];
+    for (int pi = 0; pi < np; ++pi) {
+        const int i = S.tab.probe_seg[delta][pi], d = S.tab.probe_shift[delta][pi];
+        const int sq = S.tab.seg_start[n][i], len = S.tab.seg_start[n][i + 1] - sq, rq = sq + d;
+        if (rq < 0 || rq + len > m) continue;  // the segment does not fit at this shift (warp-uniform)
+        uint32_t e = 0, e_end = 0, tag = 0;
+        if (p_valid) {
+            const unsigned long long h = seg_hash<W>(w.A, rq, len, n, i);
+            const uint32_t b = (uint32_t)h & S.index.mask;
+            e = __ldg(S.index.dir + b);
+            e_end = __ldg(S.index.dir + b + 1);
+            tag = (uint32_t)(h >> 32);
         }
-        if (L <= 1) {
-            emit_edges(P, keep, lane, p, t, m, n);
-        } else {
-            const uint32_t bal = __ballot_sync(kFullMask, keep);
+        if (COUNT) n_probes += (unsigned long long)__popc(__ballot_sync(kFullMask, p_valid));
+        uint2 ent = make_uint2(0u, 0u);
+        if (e < e_end) ent = __ldg(S.index.entries + e);
+        while (__any_sync(kFullMask, e < e_end)) {
+            bool has = false;
+            uint32_t t = 0;
+            if (e < e_end) {
+                const uint2 cur = ent;
+                ++e;
+                if (e < e_end) ent = __ldg(S.index.entries + e);  // the next entry is on its way
+                if (COUNT) ++n_entries;
+                // same bucket: only the texts after the pattern (every unordered pair once)
+                has = cur.x == tag && (delta > 0 || (int)cur.y > p);
+                t = cur.y;
+            }
+            const uint32_t bal = __ballot_sync(kFullMask, has);
             if (bal) {
-                unsigned long long base = 0;
-                if (lane == 0) base = atomicAdd(S.cand_count, (unsigned long long)__popc(bal));
-                base = __shfl_sync(kFullMask, base, 0);
-                const unsigned long long pos = base + __popc(bal & ((1u << lane) - 1u));
-                if (keep && pos < S.cand_cap) S.cand[pos] = make_uint2((uint32_t)p, (uint32_t)t);
+                if (has) w.wb->queue[(w.qhead + w.qn + __popc(bal & ((1u << lane) - 1u))) & 63] =
+                             make_uint2((uint32_t)lane | ((uint32_t)pi << 5), t);
+                const int c = __popc(bal);
+                w.qn += c;
+                if (COUNT) n_cand += (unsigned long long)c;
+                __syncwarp();
+                if (w.qn >= 32) drain_round<W, L, COUNT>(w, S, 32);
             }
         }
     }
+    if (w.qn > 0) drain_round<W, L, COUNT>(w, S, w.qn);
+    if (w.on > 0) flush_out<W, L, COUNT>(w, S, w.on);
     if (COUNT) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             n_entries += __shfl_xor_sync(kFullMask, n_entries, o);
-            n_cand += __shfl_xor_sync(kFullMask, n_cand, o);
-            n_pass += __shfl_xor_sync(kFullMask, n_pass, o);
+            w.n_pass += __shfl_xor_sync(kFullMask, w.n_pass, o);
         }
-        const unsigned long long n_probes = (unsigned long long)__popc(__ballot_sync(kFullMask, p_valid));
         if (lane == 0) {
             atomicAdd(P.work + 5, n_probes);
             atomicAdd(P.work + 6, n_entries);
             atomicAdd(P.work + 7, n_cand);
-            atomicAdd(P.work + 4, n_pass);
+            atomicAdd(P.work + 4, w.n_pass);
         }
     }
 }
@@ -372,6 +452,7 @@ __global__ void __launch_bounds__(kJoinThreads) k_join_verify(const __grid_const
         int p = 0, t = 0, m = 0, n = 0;
         if (c < total) {
             const uint2 pt = S.cand[c];
+            const int pi = (int)S.cand_probe[c];
             p = (int)pt.x, t = (int)pt.y;
             const PlaneRow<W> A = load_planes<W>(S.planes, p);
             const PlaneRow<W> B = load_planes<W>(S.planes, t);
@@ -381,7 +462,9 @@ __global__ void __launch_bounds__(kJoinThreads) k_join_verify(const __grid_const
             band_of(L, delta, smin, nb);
             W M[L + 1];
             band_masks<W, L>(A, B, m, n, smin, nb, M);
-            edge = lv_within<W, L>(M, m, n, delta, smin, nb);
+            // once: only the first probe whose segment matches keeps the pair
+            edge = first_matching_probe<W, L>(S.tab, M, smin, nb, m, n, delta, pi) &&
+                   lv_within<W, L>(M, m, n, delta, smin, nb);
             if (COUNT && edge) ++n_edges;
         }
         emit_edges(P, edge, lane, p, t, m, n);
@@ -395,8 +478,7 @@ __global__ void __launch_bounds__(kJoinThreads) k_join_verify(const __grid_const
 
 template <typename W, int L>
 cudaError_t launch_join_l(const JoinParams& S, bool count_work, int n_sm, cudaStream_t s, int* launches) {
-    const int64_t n_local = (S.d.n_items - S.d.shard + S.d.n_shards - 1) / S.d.n_shards;
-    const unsigned blocks = (unsigned)((n_local + kJoinWarps - 1) / kJoinWarps);
+    const unsigned blocks = (unsigned)((S.n_local + kJoinWarps - 1) / kJoinWarps);
     if (count_work) k_join_probe<W, L, true><<<blocks, kJoinThreads, 0, s>>>(S);
     else k_join_probe<W, L, false><<<blocks, kJoinThreads, 0, s>>>(S);
     *launches += 1;
@@ -444,8 +526,9 @@ cudaError_t launch_join_index(const void* planes, bool wide, const LengthTable& 
 }
 
 cudaError_t launch_join(const DistanceParams& p, const JoinRow* rows, int n_rows, const void* planes, bool wide,
-                        const JoinIndex& index, const JoinTables& tab, uint2* cand, unsigned long long* cand_count,
-                        unsigned long long cand_cap, bool count_work, int n_sm, cudaStream_t s, int* launches) {
+                        const JoinIndex& index, const JoinTables& tab, uint2* cand, uint8_t* cand_probe,
+                        unsigned long long* cand_count, unsigned long long cand_cap, bool count_work, int n_sm,
+                        cudaStream_t s, int* launches) {
     if (p.n_items <= p.shard || n_rows <= 0) return cudaSuccess;
     JoinParams S{};
     S.d = p;
@@ -454,6 +537,8 @@ cudaError_t launch_join(const DistanceParams& p, const JoinRow* rows, int n_rows
     S.planes = planes;
     S.index = index;
     S.cand = cand;
+    S.cand_probe = cand_probe;
+    S.n_local = (p.n_items - p.shard + p.n_shards - 1) / p.n_shards;
     S.cand_count = cand_count;
     S.cand_cap = cand_cap;
     S.tab = tab;

@@ -370,8 +370,8 @@ void make_join_tables(int l_max, JoinTables& tab) {
 
 // Step A2, host side: the (pattern bucket, text bucket) pairs with len_t - len_p in 0..l_max
 // (kPairsAllQuery: 1..l_max; the equal-length pairs belong to the kPairsQueryAll pass).
-void schedule_pass(const tcrnet_ctx* ctx, int l_max, int first_check, bool use_join, const JoinTables& tab,
-                   Schedule::Pass& pass, tcrnet_stats& st) {
+void schedule_pass(const tcrnet_ctx* ctx, int l_max, int first_check, bool use_join, Schedule::Pass& pass,
+                   tcrnet_stats& st) {
     const SeqSet& ps = *pass.pset;
     const SeqSet& ts = *pass.tset;
     // The trie kernel serves the rows whose early exit can act inside the trie (l_max <= kTrieMaxL, the
@@ -439,12 +439,9 @@ void schedule_pass(const tcrnet_ctx* ctx, int l_max, int first_check, bool use_j
         std::vector<JoinRow>& jr = pass.join_rows[wide];
         pass.join_items[wide] = 0;
         for (JoinRow& r : jr) {
-            // a work item = 32 patterns x one probe of one length difference that has texts
-            r.probe_cum[0] = 0;
-            for (int d = 0; d < kJoinMaxSeg; ++d)
-                r.probe_cum[d + 1] = r.probe_cum[d] + (d <= l_max && r.t_count[d] > 0 ? tab.n_probes[d] : 0);
+            // a work item = 32 patterns x one length difference (0..l_max; empty text buckets return at once)
             r.item_begin = pass.join_items[wide];
-            pass.join_items[wide] += (int64_t)((r.p_count + 31) / 32) * r.probe_cum[kJoinMaxSeg];
+            pass.join_items[wide] += (int64_t)((r.p_count + 31) / 32) * (l_max + 1);
         }
     }
 }
@@ -484,10 +481,8 @@ void make_schedule(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule& 
     sch.fast_l1 = can_join && ctx->fast_l1 && l_max <= 1;
     sch.use_join = sch.fast_l1 || (can_join && (ctx->segment_join == 1 ||
                                                 (ctx->segment_join < 0 && ctx->prefix_trie)));
-    JoinTables tab;
-    make_join_tables(std::min(l_max, kTrieMaxL), tab);
     for (Schedule::Pass& pass : sch.passes) {
-        schedule_pass(ctx, l_max, first_check, sch.use_join, tab, pass, st);
+        schedule_pass(ctx, l_max, first_check, sch.use_join, pass, st);
         for (int trie = 0; trie < 2; ++trie)
             for (int wide = 0; wide < 2; ++wide) {
                 st.work_items += pass.part[trie][wide].items;
@@ -622,9 +617,9 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
                 p.n_items = pass.join_items[wide];
                 JoinIndex index{(const uint32_t*)ctx->join_dir.p, (const uint2*)ctx->join_entries.p, ctx->join_slots - 1u};
                 TRY_CUDA(launch_join(p, d_join_rows, (int)jr.size(), pass.pset->planes.p, pass.pset->wide_planes, index,
-                                     ctx->join_tab, (uint2*)ctx->join_cand.p, &dc->cand_count,
-                                     (unsigned long long)(ctx->join_cand.bytes / sizeof(uint2)), ctx->count_work != 0,
-                                     ctx->n_sm, s, launches));
+                                     ctx->join_tab, (uint2*)ctx->join_cand.p,
+                                     (uint8_t*)ctx->join_cand.p + sizeof(uint2) * (size_t)ctx->join_cand_cap, &dc->cand_count,
+                                     (unsigned long long)ctx->join_cand_cap, ctx->count_work != 0, ctx->n_sm, s, launches));
             }
             d_join_rows += jr.size();
         }
@@ -670,8 +665,11 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
     st.join_index_entries = 0;
     if (sch.n_join_rows) {
         TRY(ensure_join_index(ctx, l_max, launches));
-        if (l_max >= 2)  // queue of the pairs that pass the filters (grown to the exact count if it proves too small)
-            TRY(dev_reserve(ctx, ctx->join_cand, sizeof(uint2) * (size_t)std::max<int64_t>((int64_t)1 << 20, 8 * ctx->all.n)));
+        if (l_max >= 2 && ctx->join_cand_cap == 0) {
+            // queue of the pairs that pass the filters: 8 + 1 bytes each (grown to the exact count if too small)
+            ctx->join_cand_cap = std::max<int64_t>((int64_t)1 << 20, 8 * ctx->all.n);
+            TRY(dev_reserve(ctx, ctx->join_cand, 9 * (size_t)ctx->join_cand_cap));
+        }
     }
     if (sch.n_rows) {  // the prefix-trie / text-chunk kernels run: they read txt (and the trie)
         for (Schedule::Pass& pass : sch.passes) {
@@ -707,10 +705,11 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
         TRY(run_distance(ctx, sch, l_max, first_check, (uint64_t)cap, (uint64_t)cap_b, shard, n_shards, expand_only, launches));
         const int64_t n_rec = (int64_t)ctx->h_ctrl->edge_count;  // pairs recorded by the distance kernels
         const int64_t n_cand = (int64_t)ctx->h_ctrl->cand_count;
-        if (!expand_only && n_cand > (int64_t)(ctx->join_cand.bytes / sizeof(uint2))) {
+        if (!expand_only && n_cand > ctx->join_cand_cap) {
             // the verification queue of the join was too small: grow it to the exact count and run again
             if (st.distance_passes >= 3) return TCRNET_ERR_CUDA;  // cannot happen: same input
-            TRY(dev_reserve(ctx, ctx->join_cand, sizeof(uint2) * (size_t)n_cand));
+            ctx->join_cand_cap = n_cand;
+            TRY(dev_reserve(ctx, ctx->join_cand, 9 * (size_t)n_cand));
             continue;
         }
         n_keys = grouped ? (int64_t)ctx->h_ctrl->edge_total : n_rec;

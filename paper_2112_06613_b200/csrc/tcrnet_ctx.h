@@ -92,6 +92,7 @@ struct tcrnet_ctx {
     DevBuf inv_perm, edge_dist, edge_dist_b, flags, flag_pos;
     // segment join (segjoin.cu): directory + entries of the current load for join_l_max, work rows
     DevBuf join_cnt, join_dir, join_entries, join_rows, join_cand;
+    int64_t join_cand_cap = 0;  // pairs the verification queue join_cand holds (uint2[cap] followed by uint8[cap])
     int join_l_max = -1;  // threshold the index in join_dir / join_entries was built for (-1: none)
     uint32_t join_slots = 0;
     JoinTables join_tab{};

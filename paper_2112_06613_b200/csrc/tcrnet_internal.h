@@ -118,15 +118,14 @@ struct JoinTables {
     int8_t n_seg;                                 // l_max + 1
     int8_t pad_[6];
 };
-// One pattern bucket of the join: a work item (one warp) is a tile of 32 patterns x ONE probe (delta, segment,
-// shift) against the indexed text bucket of length m + delta (t_count 0: none).
+// One pattern bucket of the join: a work item (one warp) is a tile of 32 patterns x ONE length difference delta
+// (all its probes) against the indexed text bucket of length m + delta (t_count 0: none).
 struct JoinRow {
-    int64_t item_begin;   // first work item of this row; the row has ceil(p_count / 32) * probe_cum[n_seg] of them
+    int64_t item_begin;   // first work item of this row; the row has ceil(p_count / 32) * (l_max + 1) of them
     int32_t p_start, p_count;
     int32_t m, pad_;
     int32_t t_start[kJoinMaxSeg];
     int32_t t_count[kJoinMaxSeg];
-    int32_t probe_cum[kJoinMaxSeg + 1];  // [delta] = probes of the smaller deltas that have texts
 };
 struct JoinIndex {
     const uint32_t* dir;  // [slots + 1]: entries of hash bucket b are [dir[b], dir[b+1])
@@ -236,8 +235,9 @@ cudaError_t launch_join_index(const void* planes, bool wide, const LengthTable& 
 // (at most cand_cap of the *cand_count counted) and a second kernel verifies them (Landau-Vishkin on the mismatch
 // masks of the band's diagonals) and emits.  p carries the emission fields, n_items and the shard of the launch.
 cudaError_t launch_join(const DistanceParams& p, const JoinRow* rows, int n_rows, const void* planes, bool wide,
-                        const JoinIndex& index, const JoinTables& tab, uint2* cand, unsigned long long* cand_count,
-                        unsigned long long cand_cap, bool count_work, int n_sm, cudaStream_t s, int* launches);
+                        const JoinIndex& index, const JoinTables& tab, uint2* cand, uint8_t* cand_probe,
+                        unsigned long long* cand_count, unsigned long long cand_cap, bool count_work, int n_sm,
+                        cudaStream_t s, int* launches);
 
 // labels.cu: distance labels of the final edges, threshold restriction, key validation
 cudaError_t launch_inverse_perm(const int32_t* perm, int64_t n, int32_t* inv, cudaStream_t s, int* launches);
