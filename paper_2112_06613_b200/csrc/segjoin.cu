@@ -117,11 +117,46 @@ __device__ __forceinline__ void band_of(int L, int delta, int& smin, int& nb) {
     nb = delta + 2 * h + 1;
 }
 
+// bits of M_s that are set whatever the residues are: j >= m, or j + s outside the text
+template <typename W>
+__device__ __forceinline__ W invalid_mask(int s, int m, int n) {
+    return ~(diag_shift<W>(low_mask<W>(n), s) & low_mask<W>(m));
+}
+
 template <typename W, int L>
 __device__ __forceinline__ void band_masks(const PlaneRow<W>& A, const PlaneRow<W>& B, int m, int n, int smin, int nb,
                                            W (&M)[L + 1]) {
 #pragma unroll
     for (int x = 0; x <= L; ++x) M[x] = x < nb ? mismatch_mask<W>(A, B, smin + x, m, n) : ~W(0);
+}
+
+// The same with the pair-independent parts hoisted (probe kernel: the band is the same for all pairs of a warp):
+// NV[x] = invalid_mask of diagonal x (all ones beyond the band).  32-bit planes: every plane of B is widened once
+// (b << 8 as a 64-bit pair), after which any diagonal s in -8..23 is ONE funnel shift.
+template <int L>
+__device__ __forceinline__ void band_masks_hoisted(const PlaneRow<uint32_t>& A, const PlaneRow<uint32_t>& B, int smin,
+                                                   const uint32_t (&NV)[L + 1], uint32_t (&M)[L + 1]) {
+    uint32_t lo[5], hi[5];
+#pragma unroll
+    for (int k = 0; k < 5; ++k) lo[k] = B.p[k] << 8, hi[k] = B.p[k] >> 24;
+#pragma unroll
+    for (int x = 0; x <= L; ++x) {
+        uint32_t v = NV[x];
+#pragma unroll
+        for (int k = 0; k < 5; ++k) v |= A.p[k] ^ __funnelshift_r(lo[k], hi[k], (uint32_t)(8 + smin + x));
+        M[x] = v;
+    }
+}
+template <int L>
+__device__ __forceinline__ void band_masks_hoisted(const PlaneRow<uint64_t>& A, const PlaneRow<uint64_t>& B, int smin,
+                                                   const uint64_t (&NV)[L + 1], uint64_t (&M)[L + 1]) {
+#pragma unroll
+    for (int x = 0; x <= L; ++x) {
+        uint64_t v = NV[x];
+#pragma unroll
+        for (int k = 0; k < 5; ++k) v |= A.p[k] ^ diag_shift<uint64_t>(B.p[k], smin + x);
+        M[x] = v;
+    }
 }
 
 // shifted-Hamming bound: pattern residues without a partner on any diagonal of the band
@@ -286,6 +321,7 @@ struct ProbeWarp {
     PlaneRow<W> A;  // this lane's pattern
     int lane, p0;   // sorted position of lane 0's pattern
     int m, n, delta, smin, nb;
+    W NV[L + 1];    // invalid_mask of every diagonal of the band (the same for all pairs of the warp)
     int qhead = 0, qn = 0, on = 0;
     unsigned long long n_pass = 0;
 };
@@ -333,7 +369,7 @@ __device__ __forceinline__ void drain_round(ProbeWarp<W, L, COUNT>& w, const Joi
         const PlaneRow<W> B = load_planes<W>(S.planes, t);
         if (B.len == w.n) {  // (a tag collision across length buckets cannot pass the segment test below either)
             W M[L + 1];
-            band_masks<W, L>(Ao, B, w.m, w.n, w.smin, w.nb, M);
+            band_masks_hoisted<L>(Ao, B, w.smin, w.NV, M);
             const int i = S.tab.probe_seg[w.delta][pi], d = S.tab.probe_shift[w.delta][pi];
             const int sq = S.tab.seg_start[w.n][i], len = S.tab.seg_start[w.n][i + 1] - sq;
             keep = shd_pass<W, L>(M, w.m) && segment_matches<W, L>(M, w.smin, w.nb, sq, len, d, w.m);
@@ -374,6 +410,8 @@ __global__ void __launch_bounds__(kJoinThreads) k_join_probe(const __grid_consta
     w.n = w.m + delta;
     w.delta = delta;
     band_of(L, delta, w.smin, w.nb);
+#pragma unroll
+    for (int x = 0; x <= L; ++x) w.NV[x] = x < w.nb ? invalid_mask<W>(w.smin + x, w.m, w.n) : ~W(0);
     w.p0 = Rw.p_start + tile * 32;
     const bool p_valid = tile * 32 + lane < Rw.p_count;
     const int p = p_valid ? w.p0 + lane : w.p0;
@@ -395,27 +433,44 @@ __global__ void __launch_bounds__(kJoinThreads) k_join_probe(const __grid_consta
             tag = (uint32_t)(h >> 32);
         }
         if (COUNT) n_probes += (unsigned long long)__popc(__ballot_sync(kFullMask, p_valid));
-        uint2 ent = make_uint2(0u, 0u);
-        if (e < e_end) ent = __ldg(S.index.entries + e);
-        while (__any_sync(kFullMask, e < e_end)) {
+        // The 32 buckets are walked as ONE list, 32 entries per step whatever their lengths: prefix sums of the bucket
+        // sizes, then every lane finds the bucket (owner lane) of its position by binary search over them.
+        const int c = (int)(e_end - e);
+        int incl = c;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(kFullMask, incl, o);
+            if (lane >= o) incl += v;
+        }
+        const int first = incl - c;  // position of this lane's first entry in the list
+        const int total = __shfl_sync(kFullMask, incl, 31);
+        if (COUNT) n_entries += (unsigned long long)total;
+        for (int f0 = 0; f0 < total; f0 += 32) {
+            const int f = f0 + lane;
+            int ow = 0;  // the last lane whose bucket starts at or before f (empty buckets share their start with the next)
+#pragma unroll
+            for (int step = 16; step > 0; step >>= 1) {
+                const int fc = __shfl_sync(kFullMask, first, ow + step);
+                if (fc <= f) ow += step;
+            }
+            const uint32_t e_o = __shfl_sync(kFullMask, e, ow);
+            const int first_o = __shfl_sync(kFullMask, first, ow);
+            const uint32_t tag_o = __shfl_sync(kFullMask, tag, ow);
             bool has = false;
             uint32_t t = 0;
-            if (e < e_end) {
-                const uint2 cur = ent;
-                ++e;
-                if (e < e_end) ent = __ldg(S.index.entries + e);  // the next entry is on its way
-                if (COUNT) ++n_entries;
+            if (f < total) {
+                const uint2 cur = __ldg(S.index.entries + e_o + (uint32_t)(f - first_o));
                 // same bucket: only the texts after the pattern (every unordered pair once)
-                has = cur.x == tag && (delta > 0 || (int)cur.y > p);
+                has = cur.x == tag_o && (delta > 0 || (int)cur.y > w.p0 + ow);
                 t = cur.y;
             }
             const uint32_t bal = __ballot_sync(kFullMask, has);
             if (bal) {
                 if (has) w.wb->queue[(w.qhead + w.qn + __popc(bal & ((1u << lane) - 1u))) & 63] =
-                             make_uint2((uint32_t)lane | ((uint32_t)pi << 5), t);
-                const int c = __popc(bal);
-                w.qn += c;
-                if (COUNT) n_cand += (unsigned long long)c;
+                             make_uint2((uint32_t)ow | ((uint32_t)pi << 5), t);
+                const int cq = __popc(bal);
+                w.qn += cq;
+                if (COUNT) n_cand += (unsigned long long)cq;
                 __syncwarp();
                 if (w.qn >= 32) drain_round<W, L, COUNT>(w, S, 32);
             }
@@ -425,10 +480,7 @@ __global__ void __launch_bounds__(kJoinThreads) k_join_probe(const __grid_consta
     if (w.on > 0) flush_out<W, L, COUNT>(w, S, w.on);
     if (COUNT) {
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            n_entries += __shfl_xor_sync(kFullMask, n_entries, o);
-            w.n_pass += __shfl_xor_sync(kFullMask, w.n_pass, o);
-        }
+        for (int o = 16; o > 0; o >>= 1) w.n_pass += __shfl_xor_sync(kFullMask, w.n_pass, o);
         if (lane == 0) {
             atomicAdd(P.work + 5, n_probes);
             atomicAdd(P.work + 6, n_entries);
