@@ -6,7 +6,8 @@ Recipe (BASELINE.json `configs`; restated in DESIGN.md):
    comes from it, in the order written here.
 2. ``n_dup = round(dup * N)`` rows will be copies; ``n_base = N - n_dup``.
 3. Seeds: ``n_seeds`` sequences.  Length ``clip(rint(Normal(mu, sigma)), lo,
-   hi)``.  First residue 'C', last residue 'F', the rest i.i.d. from the
+   hi)``.  First residue 'C', last residue 'F' (the stress input ``cfg4_cass``:
+   first residues 'CASS', last 'EQYF'), the rest i.i.d. from the
    residue law of that seed (uniform over the 20 standard amino acids of
    PAPER.md:211, or — config 5 — with probability ``zipf_frac`` a Zipf(s=1.1)
    law over the same 20 letters in ``AA20`` order).
@@ -51,6 +52,8 @@ class SynthConfig:
     hi: int
     dup: float
     zipf_frac: float = 0.0
+    prefix: bytes = b"C"   # conserved first residues of every seed / independent sequence
+    suffix: bytes = b"F"   # conserved last residues
 
     @property
     def seed(self) -> int:
@@ -65,6 +68,10 @@ CONFIGS: Dict[str, SynthConfig] = {
         SynthConfig("cfg3", 3, 200_000, (2,), 8_000, 24.0, 15.0, 2.5, 6, 30, 0.05),
         SynthConfig("cfg4", 4, 800_000, (1,), 30_000, 24.0, 15.0, 2.0, 8, 25, 0.03),
         SynthConfig("cfg5", 5, 2_000_000, (3,), 60_000, 24.0, 16.0, 3.0, 5, 40, 0.05, 0.10),
+        # Stress input, NOT a BASELINE.json config: config 4 with the conserved ends real CDR3-beta rows have (V gene:
+        # "CASS...", J gene: "...EQYF"), so that prefixes / suffixes carry no information (bench.py `detail`, DESIGN.md
+        # section 6).  lo >= len(prefix) + len(suffix).
+        SynthConfig("cfg4_cass", 14, 800_000, (1,), 30_000, 24.0, 15.0, 2.0, 8, 25, 0.03, 0.0, b"CASS", b"EQYF"),
     )
 }
 
@@ -127,8 +134,10 @@ def _random_sequences(rng, k, cfg):
     ln = _lengths(rng, k, cfg)
     zipf = rng.random(k) < cfg.zipf_frac if cfg.zipf_frac > 0 else np.zeros(k, dtype=bool)
     mat = _draw_residues(rng, zipf, (k, cfg.hi))
-    mat[:, 0] = ord("C")
-    mat[np.arange(k), ln - 1] = ord("F")
+    for q, ch in enumerate(cfg.prefix):
+        mat[:, q] = ch
+    for q, ch in enumerate(reversed(cfg.suffix)):
+        mat[np.arange(k), ln - 1 - q] = ch
     col = np.arange(cfg.hi)[None, :]
     mat[col >= ln[:, None]] = 0
     return mat, ln, zipf
@@ -176,7 +185,7 @@ def generate(cfg: SynthConfig | str, n: int | None = None, seed: int | None = No
     if n is not None and n != cfg.n:
         scale = n / cfg.n
         cfg = SynthConfig(cfg.name, cfg.index, n, cfg.l_max, max(1, int(round(cfg.n_seeds * scale))),
-                          cfg.lam, cfg.mu, cfg.sigma, cfg.lo, cfg.hi, cfg.dup, cfg.zipf_frac)
+                          cfg.lam, cfg.mu, cfg.sigma, cfg.lo, cfg.hi, cfg.dup, cfg.zipf_frac, cfg.prefix, cfg.suffix)
     rng = np.random.Generator(np.random.PCG64(cfg.seed if seed is None else seed))
     N = cfg.n
     n_dup = int(round(cfg.dup * N))

@@ -180,6 +180,9 @@ typedef struct tcrnet_stats {
                                   where the verification is the XOR / prefix-suffix check                */
     int32_t pad2_;
     int64_t join_survivors;    /* segment join: candidates that passed the filters and were verified (COUNT_WORK) */
+    int64_t join_diagonals;    /* ... per-diagonal mismatch masks built, probe + verify kernels (COUNT_WORK; 0 when
+                                  other distance kernels ran in the same build)                               */
+    int64_t join_verified_edges; /* ... pairs of distinct sequences the verify kernel (l_max >= 2) accepted     */
 } tcrnet_stats;
 
 /*

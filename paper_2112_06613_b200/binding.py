@@ -51,7 +51,8 @@ class tcrnet_stats(C.Structure):
         ("n_distinct", C.c_int64), ("ms_kernel", C.c_float), ("ms_index", C.c_float),
         ("lane_columns_live", C.c_int64), ("join_probes", C.c_int64), ("join_entries", C.c_int64),
         ("join_candidates", C.c_int64), ("work_items_join", C.c_int64), ("join_index_entries", C.c_int64),
-        ("join_mode", C.c_int32), ("pad2_", C.c_int32), ("join_survivors", C.c_int64),
+        ("join_mode", C.c_int32), ("pad2_", C.c_int32), ("join_survivors", C.c_int64), ("join_diagonals", C.c_int64),
+        ("join_verified_edges", C.c_int64),
     ]
 
 

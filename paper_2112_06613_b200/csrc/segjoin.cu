@@ -323,7 +323,7 @@ struct ProbeWarp {
     int m, n, delta, smin, nb;
     W NV[L + 1];    // invalid_mask of every diagonal of the band (the same for all pairs of the warp)
     int qhead = 0, qn = 0, on = 0;
-    unsigned long long n_pass = 0;
+    unsigned long long n_pass = 0, n_diag = 0;
 };
 
 // the first 32 staged results leave
@@ -360,6 +360,7 @@ __device__ __forceinline__ void drain_round(ProbeWarp<W, L, COUNT>& w, const Joi
     const uint2 q = act ? w.wb->queue[(w.qhead + w.lane) & 63] : make_uint2(0u, 0u);
     w.qhead = (w.qhead + cnt) & 63;
     w.qn -= cnt;
+    if (COUNT) w.n_diag += (unsigned long long)(cnt * w.nb);  // mismatch masks built (warp-level count)
     const int ow = (int)(q.x & 31u), pi = (int)(q.x >> 5), t = (int)q.y;
     PlaneRow<W> Ao;  // the owner's pattern
 #pragma unroll
@@ -486,6 +487,7 @@ __global__ void __launch_bounds__(kJoinThreads) k_join_probe(const __grid_consta
             atomicAdd(P.work + 6, n_entries);
             atomicAdd(P.work + 7, n_cand);
             atomicAdd(P.work + 4, w.n_pass);
+            atomicAdd(P.work + 0, w.n_diag);
         }
     }
 }
@@ -496,7 +498,7 @@ __global__ void __launch_bounds__(kJoinThreads) k_join_verify(const __grid_const
     const DistanceParams& P = S.d;
     const int lane = threadIdx.x & 31;
     const unsigned long long total = min(*S.cand_count, S.cand_cap);
-    unsigned long long n_edges = 0;
+    unsigned long long n_edges = 0, n_diag = 0;
     for (unsigned long long base = (unsigned long long)blockIdx.x * kJoinThreads; base < total;
          base += (unsigned long long)gridDim.x * kJoinThreads) {
         const unsigned long long c = base + threadIdx.x;
@@ -514,6 +516,7 @@ __global__ void __launch_bounds__(kJoinThreads) k_join_verify(const __grid_const
             band_of(L, delta, smin, nb);
             W M[L + 1];
             band_masks<W, L>(A, B, m, n, smin, nb, M);
+            if (COUNT) n_diag += (unsigned long long)nb;
             // once: only the first probe whose segment matches keeps the pair
             edge = first_matching_probe<W, L>(S.tab, M, smin, nb, m, n, delta, pi) &&
                    lv_within<W, L>(M, m, n, delta, smin, nb);
@@ -523,8 +526,14 @@ __global__ void __launch_bounds__(kJoinThreads) k_join_verify(const __grid_const
     }
     if (COUNT) {
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) n_edges += __shfl_xor_sync(kFullMask, n_edges, o);
-        if (lane == 0 && n_edges) atomicAdd(P.work + 3, n_edges);
+        for (int o = 16; o > 0; o >>= 1) {
+            n_edges += __shfl_xor_sync(kFullMask, n_edges, o);
+            n_diag += __shfl_xor_sync(kFullMask, n_diag, o);
+        }
+        if (lane == 0 && n_diag) {
+            atomicAdd(P.work + 3, n_edges);
+            atomicAdd(P.work + 0, n_diag);
+        }
     }
 }
 

@@ -737,7 +737,12 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
     st.join_entries = (int64_t)ctx->h_ctrl->work[6];
     st.join_candidates = (int64_t)ctx->h_ctrl->work[7];
     st.join_survivors = st.join_mode ? (int64_t)ctx->h_ctrl->work[4] : 0;
-    if (st.join_mode) st.lane_columns_live = 0;
+    st.join_diagonals = st.join_verified_edges = 0;
+    if (st.join_mode && st.work_items == st.work_items_join) {  // (the counters are shared with the other kernels)
+        st.join_diagonals = (int64_t)ctx->h_ctrl->work[0];
+        st.join_verified_edges = (int64_t)ctx->h_ctrl->work[3];
+        st.lane_columns_exec = st.lane_prefix_tests_exec = st.lane_columns_live = 0;
+    }
     if (st.ms_index < 0.f) TRY_CUDA(cudaEventElapsedTime(&st.ms_index, ctx->ev[6], ctx->ev[7]));
     TRY_CUDA(cudaEventRecord(ctx->ev[1], s));
     ctx->n_keys = n_keys;

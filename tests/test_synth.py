@@ -49,3 +49,21 @@ def test_stream_is_pinned():
     d = generate("cfg1")
     h = hashlib.sha256(d.residues.tobytes() + d.lengths.tobytes()).hexdigest()
     assert h == open(__file__.replace("test_synth.py", "golden/cfg1_input.sha256")).read().split()[0]
+
+
+def test_stored_network_digests_belong_to_the_generated_inputs():
+    """tests/golden/<cfg>_l<l_max>_network.sha256 (written by tests/golden/make_config_hashes.py from the oracle alone)
+    exist for config 1, 3 and 4 and were computed on exactly the rows the generator produces today."""
+    import hashlib
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    for name, l_max in (("cfg1", 1), ("cfg3", 2), ("cfg4", 1)):
+        path = os.path.join(here, f"{name}_l{l_max}_network.sha256")
+        assert os.path.exists(path), path
+        kv = dict(line.split() for line in open(path) if line.strip() and not line.startswith("#"))
+        d = generate(name)
+        assert int(kv["n"]) == d.n and int(kv["l_max"]) == l_max
+        assert kv["sha256_input"] == hashlib.sha256(d.residues.tobytes() + d.lengths.astype("<i4").tobytes()).hexdigest()
+        assert int(kv["sum_degree"]) == 2 * int(kv["n_edges"])
+        for k in ("sha256_row_ptr", "sha256_col", "sha256_deg", "sha256_all"):
+            assert len(kv[k]) == 64
