@@ -33,14 +33,23 @@ if ROOT not in sys.path:
 
 WORKLOAD = "cfg4"
 ALU_LANES_PER_SM = 64          # INT32 ALU-pipe lanes per SM per clock on sm_100
+# prefix-trie / text-chunk kernels (Myers column recurrence), DESIGN.md section 7
 ALU_OPS_PER_COLUMN = 7         # LOP3 per pair and text column (distance.cu)
 ALU_OPS_FIRST_COLUMN = 3       # the first column of a text needs only 3 (constant Pv, Mv = 0)
 ALU_OPS_PER_TEST = 4           # 2 LOP3 + IADD3 + ISETP per pair and early-exit test
 ALU_OPS_PER_PREFIX_TEST = 2    # LOP3 + ISETP per pair and DP cell read in a guided expansion (distance_trie.cu)
+# segment join (segjoin.cu): what the method itself needs on the ALU pipe
+JOIN_OPS_PER_PROBE = 25        # 5 plane slices x (SHF + AND + XOR) + the 64-bit xor-shifts of the mixing rounds
+JOIN_OPS_PER_ENTRY = 2         # tag compare + order compare per directory entry read
+JOIN_OPS_PER_CANDIDATE = 12    # widening the 5 text planes (2 x 5) + the filter's AND / compare
+JOIN_OPS_PER_DIAGONAL = 11     # 5 funnel shifts + 5 LOP3 (a ^ b | acc) + 1 AND of the shifted-Hamming filter
+JOIN_OPS_PER_LV_STATE = 12     # Landau-Vishkin: compare / select / max / min / shift per (edit level, diagonal)
 ORACLE_SAMPLE_ROWS = 1024
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_distance_trie launch at cfg4, from the ncu --set full
-# capture summarised in profiles/r1e_trie_ncu.txt (65.39 MB + 3.55 MB)
-NCU_DRAM_BYTES_PER_LAUNCH = {"cfg4": 68_938_240}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the ncu --set full captures
+# summarised under profiles/ (regenerated with them; a workload / kernel that is not listed prints null)
+NCU_DRAM_BYTES_PER_LAUNCH = {
+    # (workload, kernel): bytes   -- filled from profiles/r2_*.txt
+}
 
 
 def _peaks():
@@ -134,19 +143,19 @@ class ClockSampler:
                 "samples": len(sm), "source": self.source, "reasons": sorted(reasons)}
 
 
-def oracle_sample(d, l_max: int, rows: int, seed: int = 0):
-    """The oracle (tier 0: full Wagner-Fischer table, no pruning) on `rows` random rows against
-    every other row.  Returns (pairs/s, cells/s, threads, seconds, pairs)."""
+def oracle_sample(d, l_max: int, rows: int, seed: int = 0, tier: int = 0, threads: int = 0):
+    """The oracle on `rows` random rows against every other row (tier 0: full Wagner-Fischer table, no pruning;
+    tier 1: length filter + the paper's row-minimum abort).  Returns (pairs/s, cells/s, threads, seconds, pairs)."""
     import oracle
     rng = np.random.default_rng(seed)
     sample = np.sort(rng.choice(d.n, size=min(rows, d.n), replace=False))
     t0 = time.perf_counter()
-    _, threads = oracle.edges(d.residues, d.lengths, l_max, rows=sample, all_partners=True, tier=0)
+    _, used = oracle.edges(d.residues, d.lengths, l_max, rows=sample, all_partners=True, tier=tier, threads=threads)
     dt = time.perf_counter() - t0
     pairs = int(sample.size) * (d.n - 1)
     cells = float((d.lengths[sample].astype(np.int64) * (int(d.lengths.astype(np.int64).sum()))).sum()
                   - (d.lengths[sample].astype(np.int64) ** 2).sum())
-    return pairs / dt, cells / dt, threads, dt, pairs
+    return pairs / dt, cells / dt, used, dt, pairs
 
 
 def run_reference(args, rank: int) -> None:
@@ -176,21 +185,70 @@ def run_reference(args, rank: int) -> None:
     }))
 
 
+def alu_ops_columns(work) -> float:
+    """Algorithmic ALU lane-ops of the column-recurrence kernels (prefix trie / text chunks)."""
+    return (ALU_OPS_PER_COLUMN * work["lane_columns_exec"] + ALU_OPS_PER_TEST * work["lane_tests_exec"]
+            + ALU_OPS_PER_PREFIX_TEST * work["lane_prefix_tests_exec"]
+            - (ALU_OPS_PER_COLUMN - ALU_OPS_FIRST_COLUMN) * work["lane_pairs_exec"] * (work["first_check"] > 0))
+
+
+def alu_ops_join(work, l_max: int) -> float:
+    """Algorithmic ALU lane-ops of the segment join (probe + verify kernels), from the counters of the instrumented
+    instance: probes hashed, directory entries compared, candidates filtered (masks per diagonal of the band),
+    survivors verified by Landau-Vishkin (l_max levels x the band's diagonals)."""
+    cand = max(1, work["join_candidates"])
+    nb_avg = work["join_diagonals"] / (cand + (work["join_survivors"] if l_max >= 2 else 0))
+    verified = work["join_survivors"]
+    ops = (JOIN_OPS_PER_PROBE * work["join_probes"] + JOIN_OPS_PER_ENTRY * work["join_entries"]
+           + JOIN_OPS_PER_CANDIDATE * work["join_candidates"] + JOIN_OPS_PER_DIAGONAL * work["join_diagonals"]
+           + verified * JOIN_OPS_PER_LV_STATE * max(1, l_max) * nb_avg)
+    if l_max >= 2:  # the verify kernel widens the planes of every survivor again
+        ops += JOIN_OPS_PER_CANDIDATE * verified
+    return ops
+
+
+def join_bytes(work, n_distinct: int, l_max: int, row_bytes: int) -> float:
+    """Algorithmic bytes of the join: one directory pair per probe, every entry read, one plane row per candidate
+    (and per survivor in the verify kernel, both rows), the pattern rows once per length difference."""
+    b = 8.0 * work["join_probes"] + 8.0 * work["join_entries"] + row_bytes * work["join_candidates"]
+    b += row_bytes * n_distinct * (l_max + 1)
+    if l_max >= 2:
+        b += (2 * row_bytes + 9 + 9) * work["join_survivors"]
+    return b
+
+
+def time_steps(net, step, flush, k, torch):
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(k)]
+    stats = []
+    for i in range(k):
+        flush.fill_(i)
+        ev[i][0].record()
+        step()
+        ev[i][1].record()
+        stats.append(net.get_stats())
+    torch.cuda.synchronize()
+    return [a.elapsed_time(b) for a, b in ev], stats
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default=WORKLOAD, help="cdr3_synth config name (bench line: cfg4)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true",
+                    help="skip the side measurements (prefix-trie path, collapse off, CASS-prefixed input, pipe probes)")
+    ap.add_argument("--sharded", action="store_true",
+                    help="N > 1: ONE repertoire, every rank builds its shard of the work items, the edge keys are "
+                         "all-gathered and every rank assembles the CSR (strong scaling); default: replicas (weak)")
     ap.add_argument("--first-check", type=int, default=0)
     ap.add_argument("--text-chunk", type=int, default=0)
     ap.add_argument("--trie-chunk", type=int, default=0)
     ap.add_argument("--no-trie", action="store_true", help="text-chunk kernel only (every kept pair visited)")
     ap.add_argument("--segment-join", type=int, default=None, choices=[-1, 0, 1],
                     help="TCRNET_OPT_SEGMENT_JOIN (default: the library's)")
-    ap.add_argument("--fast-l1", action="store_true", help="TCRNET_OPT_FAST_L1 = 1 (l_max <= 1 without the recurrence)")
     ap.add_argument("--no-dedup", action="store_true", help="TCRNET_OPT_DEDUP = 0 (identical rows are not collapsed)")
     args = ap.parse_args()
 
@@ -217,9 +275,11 @@ def main() -> None:
             dist.barrier()
         torch.cuda.synchronize()
 
+    sharded = args.sharded and world > 1
     cfg = CONFIGS[args.workload]
     l_max = cfg.l_max[0]
-    d = generate(cfg, seed=cfg.seed + 1000 * rank)  # replicas: an independent repertoire per rank
+    # replicas: an independent repertoire per rank; sharded: the same repertoire on every rank
+    d = generate(cfg, seed=cfg.seed + (0 if sharded else 1000 * rank))
     n = d.n
     pairs_all = n * (n - 1) // 2
 
@@ -240,13 +300,14 @@ def main() -> None:
         net.set_option(pkg.OPT_PREFIX_TRIE, 0)
     if args.segment_join is not None:
         net.set_option(pkg.OPT_SEGMENT_JOIN, args.segment_join)
-    if args.fast_l1:
-        net.set_option(pkg.OPT_FAST_L1, 1)
     if args.no_dedup:
         net.set_option(pkg.OPT_DEDUP, 0)
 
     def step_device():
         net.load(d_res, d_len)
+        if sharded:
+            from paper_2112_06613_b200.parallel import build_distributed
+            return build_distributed(net, l_max)
         return net.build(l_max)
 
     e2e_split = [0.0, 0.0, 0.0]
@@ -255,7 +316,11 @@ def main() -> None:
         t0 = time.perf_counter()
         net.load(h_res.numpy(), h_len.numpy())
         t1 = time.perf_counter()
-        net.build(l_max)
+        if sharded:
+            from paper_2112_06613_b200.parallel import build_distributed
+            build_distributed(net, l_max)
+        else:
+            net.build(l_max)
         t2 = time.perf_counter()
         out = net.copy_csr(staged=True)  # page-locked result buffers owned by the binding
         t3 = time.perf_counter()
@@ -316,39 +381,45 @@ def main() -> None:
     if rank == 0:
         peaks, peak_kind = _peaks()
         n_sm = torch.cuda.get_device_properties(local_rank).multi_processor_count
-        ms_dist = float(np.mean([s["ms_distance"] for s in stats]))
-        ms_kernel = float(np.mean([s["ms_kernel"] for s in stats]))  # the distance kernel launch alone
-        ms_sort = float(np.mean([s["ms_sort"] for s in stats]))
-        ms_csr = float(np.mean([s["ms_csr"] for s in stats]))
-        ms_load = float(np.mean([s["ms_load"] for s in stats]))
-        alu_ops = (ALU_OPS_PER_COLUMN * work["lane_columns_exec"] + ALU_OPS_PER_TEST * work["lane_tests_exec"]
-                   + ALU_OPS_PER_PREFIX_TEST * work["lane_prefix_tests_exec"]
-                   - (ALU_OPS_PER_COLUMN - ALU_OPS_FIRST_COLUMN) * work["lane_pairs_exec"] * (work["first_check"] > 0))
-        achieved = alu_ops / (ms_kernel * 1e-3) / 1e12
+        mean = lambda key: float(np.mean([s[key] for s in stats]))  # noqa: E731
+        ms_dist, ms_kernel, ms_sort, ms_csr, ms_load, ms_index = (mean(k) for k in (
+            "ms_distance", "ms_kernel", "ms_sort", "ms_csr", "ms_load", "ms_index"))
         peak = n_sm * ALU_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12
-        probes = {}
-        for kind, name in ((0, "lop3"), (2, "imad"), (3, "lop3_imad_mix"), (5, "myers_step")):
-            ops, mhz = net.probe_int32(kind)
-            probes[name] = {"tera_per_s": ops / 1e12, "sm_mhz": mhz}
+        join = work["join_mode"] > 0 and work["work_items_join"] == work["work_items"]
+        if join:
+            alu_ops = alu_ops_join(work, l_max)
+            kernel = "k_join_probe" + (" + k_join_verify" if l_max >= 2 else "")
+        else:
+            alu_ops = alu_ops_columns(work)
+            kernel = "k_distance_trie" if work["work_items_trie"] else "k_distance"
+        achieved = alu_ops / (ms_kernel * 1e-3) / 1e12
+        jobs = 1 if sharded else world  # networks built per step
         out = {
-            "metric": "levenshtein_pairs_per_s", "value": world * pairs_all / (ms_step * 1e-3), "unit": "pairs/s",
+            "metric": "levenshtein_pairs_per_s", "value": jobs * pairs_all / (ms_step * 1e-3), "unit": "pairs/s",
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None, "dtype": "int32",
+            "data": "synthetic",
             "config": {
-                "workload": f"{args.workload}: N={n} synthetic CDR3b (BASELINE.json configs[{cfg.index - 1}]), l_max={l_max}",
+                "workload": f"{args.workload}: N={n} synthetic CDR3b" +
+                            (f" (BASELINE.json configs[{cfg.index - 1}])" if cfg.index <= 5 else " (stress input)") +
+                            f", l_max={l_max}",
                 "n": n, "l_max": l_max, "edges": int(n_edges), "l2": "flushed between timed steps (256 MiB write)",
-                "parallelism": "replicas" if world > 1 else "single GPU", "first_check": work["first_check"],
+                "parallelism": ("sharded work items + all-gather of edge keys" if sharded else "replicas") if world > 1
+                               else "single GPU",
+                "path": "segment join (pigeonhole index, shifted-Hamming filter, Landau-Vishkin verification)" if join
+                        else "length-bucket pairs through the prefix trie / text chunks (Myers column recurrence)",
             },
             "clocks": clocks,
-            "e2e": {"value": world * pairs_all / (ms_e2e * 1e-3), "unit": "pairs/s", "ms_per_step": ms_e2e,
+            "e2e": {"value": jobs * pairs_all / (ms_e2e * 1e-3), "unit": "pairs/s", "ms_per_step": ms_e2e,
                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_load_build_copy": [1e3 * x / args.steps for x in e2e_split]},
             "gpu_launches": int(sum(s["launches_load"] + s["launches_build"] for s in stats)),
             "roofline": {
                 "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TIOP/s (INT32 ALU-pipe lane-ops)",
-                "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.workload), "kernel": "k_distance_trie" if work["work_items_trie"] else "k_distance", "kernel_ms": ms_kernel,
+                "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.workload, kernel)),
+                "kernel": kernel, "kernel_ms": ms_kernel, "kernel_share_of_step": ms_kernel / ms_step,
                 "peak_source": f"{n_sm} SMs x {ALU_LANES_PER_SM} lanes x {peaks['sm_max_mhz']} MHz ({peak_kind} sm_max_mhz)",
-                "alu_ops_per_launch": alu_ops, "measured_pipe_peaks": probes,
+                "alu_ops_per_launch": alu_ops,
                 # also against the issue-slot ceiling (4 schedulers x 32 lanes per SM and clock)
                 "issue_ceiling": 2 * peak, "frac_of_issue_ceiling": achieved / (2 * peak),
             },
@@ -358,21 +429,30 @@ def main() -> None:
                 "pairs_per_s_evaluated": work["pairs_kept"] / (ms_kernel * 1e-3),
                 "gcups_evaluated": work["cells_kept"] / (ms_kernel * 1e-3) / 1e9,
                 "gcups_effective": work["cells_all"] / (ms_step * 1e-3) / 1e9,
-                "columns_executed_fraction": work["lane_columns_exec"] / max(1, work["columns_kept"]),
-                "ms_pack": ms_load, "ms_distance": ms_dist, "ms_distance_kernel": ms_kernel, "ms_sort": ms_sort, "ms_csr": ms_csr,
+                "ms_pack": ms_load, "ms_distance": ms_dist, "ms_distance_kernel": ms_kernel, "ms_index": ms_index,
+                "ms_sort": ms_sort, "ms_csr": ms_csr,
+                "launches_per_step": stats[-1]["launches_load"] + stats[-1]["launches_build"],
                 "work_items": work["work_items"], "work_items_trie": work["work_items_trie"],
-                "trie_nodes": work["trie_nodes"], "lane_columns_exec": work["lane_columns_exec"],
-                "lane_prefix_tests_exec": work["lane_prefix_tests_exec"], "lane_tests_exec": work["lane_tests_exec"],
+                "work_items_join": work["work_items_join"], "join_mode": work["join_mode"],
+                "join_probes": work["join_probes"], "join_entries": work["join_entries"],
+                "join_candidates": work["join_candidates"], "join_survivors": work["join_survivors"],
+                "join_diagonals": work["join_diagonals"], "join_index_entries": work["join_index_entries"],
+                "lane_columns_exec": work["lane_columns_exec"], "lane_tests_exec": work["lane_tests_exec"],
+                "lane_prefix_tests_exec": work["lane_prefix_tests_exec"],
+                "columns_executed_fraction": work["lane_columns_exec"] / max(1, work["columns_kept"]),
                 "ms_steps": ms_steps,
-                "join_mode": work["join_mode"], "ms_index": float(np.mean([s["ms_index"] for s in stats])),
-                "work_items_join": work["work_items_join"], "join_probes": work["join_probes"],
-                "join_entries": work["join_entries"], "join_candidates": work["join_candidates"],
-                "join_index_entries": work["join_index_entries"], "lane_columns_live": work["lane_columns_live"],
             },
         }
+        if join:
+            row_bytes = 64 if work["max_len"] > 32 else 32
+            jb = join_bytes(work, work["n_distinct"], l_max, row_bytes)
+            out["roofline"]["memory_view"] = {
+                "algorithmic_bytes": jb, "gb_per_s": jb / (ms_kernel * 1e-3) / 1e9,
+                "frac_of_hbm_peak": jb / (ms_kernel * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                "note": "random 32-byte sector reads of L2-resident tables; the HBM copy peak is the contract's denominator",
+            }
         # the emission / CSR passes against the HBM peak (algorithmic bytes of DESIGN.md section 7:
-        # expansion 8 B read per recorded pair + 8 B written per edge; A6 bucket scatter 8 + 8 B, rank 8 + 4 B per edge,
-        # 12 B per node and the scan's 4 + 8 B per node)
+        # A6 bucket scatter 8 + 8 B, rank 8 + 4 B per edge, 12 B per node and the scan's 4 + 8 B per node)
         e_cnt = int(n_edges)
         csr_bytes = e_cnt * 28 + n * 24
         out["hbm_passes"] = {
@@ -381,11 +461,70 @@ def main() -> None:
             "csr_frac_of_hbm_peak": (csr_bytes / (ms_csr * 1e-3) / 1e9) / peaks["hbm_gbs"] if ms_csr > 0 else None,
             "note": "L2-resident, launch- and latency-bound at this size (6 launches, 20-50 us each)",
         }
+        if not args.no_extras and world == 1:
+            extras = {}
+            # (a) the length-bucket path of round 1 (every length-compatible pair through the prefix trie): its own
+            #     roofline line, measured outside the timed region
+            def side(opts, data=None, k=3):
+                with pkg.TcrNet(local_rank) as other:
+                    for o, v in opts.items():
+                        other.set_option(o, v)
+                    r_d, l_d = (d_res, d_len) if data is None else data
+
+                    def one():
+                        other.load(r_d, l_d)
+                        other.build(l_max)
+                    other.set_option(pkg.OPT_COUNT_WORK, 1)
+                    one()
+                    w = other.get_stats()
+                    other.set_option(pkg.OPT_COUNT_WORK, 0)
+                    one()
+                    ms, st = time_steps(other, one, flush, k, torch)
+                return float(np.mean(ms)), w, st
+            if join and l_max <= 4 and n <= 1_000_000:
+                ms_t, w_t, st_t = side({pkg.OPT_SEGMENT_JOIN: 0})
+                k_ms = float(np.mean([s["ms_kernel"] for s in st_t]))
+                ach = alu_ops_columns(w_t) / (k_ms * 1e-3) / 1e12
+                out["roofline_trie_path"] = {
+                    "bound": "alu", "kernel": "k_distance_trie", "kernel_ms": k_ms, "ms_per_step": ms_t,
+                    "achieved": ach, "peak": peak, "frac": ach / peak, "alu_ops_per_launch": alu_ops_columns(w_t),
+                    "columns_executed_fraction": w_t["lane_columns_exec"] / max(1, w_t["columns_kept"]),
+                    "gcups_evaluated": w_t["cells_kept"] / (k_ms * 1e-3) / 1e9,
+                    "note": "TCRNET_OPT_SEGMENT_JOIN = 0: not the timed path; kept for comparison with round 1",
+                }
+            # (b) how much of the step is the data: identical rows not collapsed; conserved CASS... / ...EQYF ends
+            ms_nd, _, _ = side({pkg.OPT_DEDUP: 0})
+            extras["ms_step_dedup_off"] = ms_nd
+            if args.workload == "cfg4":
+                dc = generate("cfg4_cass")
+                data = (torch.from_numpy(dc.residues).cuda(), torch.from_numpy(dc.lengths).cuda())
+                ms_c, w_c, st_c = side({}, data)
+                extras["ms_step_cass_prefix_input"] = ms_c
+                extras["cass_prefix_input"] = {"edges": int(st_c[-1]["n_edges"]), "n_distinct": int(w_c["n_distinct"]),
+                                               "join_candidates": int(w_c["join_candidates"]),
+                                               "ms_distance_kernel": float(np.mean([s["ms_kernel"] for s in st_c]))}
+                del data
+            out["detail"].update(extras)
+            probes = {}
+            for kind, name in ((0, "lop3"), (2, "imad"), (3, "lop3_imad_mix"), (5, "myers_step")):
+                ops, mhz = net.probe_int32(kind)
+                probes[name] = {"tera_per_s": ops / 1e12, "sm_mhz": mhz}
+            out["roofline"]["measured_pipe_peaks"] = probes
         if not args.no_cpu_baseline and world == 1:
-            pps, cps, threads, dt, pairs = oracle_sample(d, l_max, ORACLE_SAMPLE_ROWS)
+            all_cores = os.cpu_count() or 1
+            pps, cps, threads, dt, pairs = oracle_sample(d, l_max, ORACLE_SAMPLE_ROWS, threads=all_cores)
             out["cpu_baseline"] = {
                 "value": pps, "unit": "pairs/s", "cores": threads, "kind": "oracle", "gcups": cps / 1e9,
                 "sample": f"{ORACLE_SAMPLE_ROWS} random rows x all {n - 1} partners ({pairs} pairs, {dt:.1f} s), tier-0 full table",
+            }
+            # the paper's CPU comparison is ONE core; tier 1 = the paper's own abort + length filter
+            p1, _, t1, dt1, pr1 = oracle_sample(d, l_max, 64, tier=0, threads=1)
+            p2, _, t2, dt2, pr2 = oracle_sample(d, l_max, 4 * ORACLE_SAMPLE_ROWS, tier=1, threads=all_cores)
+            p3, _, t3, dt3, pr3 = oracle_sample(d, l_max, 128, tier=1, threads=1)
+            out["cpu_baseline"]["also"] = {
+                "tier0_1core": {"value": p1, "cores": t1, "sample": f"64 rows x all partners ({pr1} pairs, {dt1:.1f} s)"},
+                "tier1_all_cores": {"value": p2, "cores": t2, "sample": f"{4 * ORACLE_SAMPLE_ROWS} rows x all partners ({pr2} pairs, {dt2:.1f} s), length filter + row-minimum abort"},
+                "tier1_1core": {"value": p3, "cores": t3, "sample": f"128 rows x all partners ({pr3} pairs, {dt3:.1f} s)"},
             }
         print(json.dumps(out))
     net.destroy()

@@ -201,9 +201,11 @@ __global__ void __launch_bounds__(256) k_expand_entries(const unsigned long long
                                                        unsigned long long* __restrict__ edges,
                                                        unsigned long long* __restrict__ edge_total,
                                                        unsigned long long edge_cap, int32_t* __restrict__ row_count,
-                                                       int32_t* __restrict__ deg) {
+                                                       int32_t* __restrict__ deg, ulonglong2* __restrict__ huge,
+                                                       unsigned long long* __restrict__ n_huge, uint32_t huge_cap) {
     constexpr uint32_t kFullMask = 0xffffffffu;
     constexpr unsigned long long kOwn = 8;
+    constexpr unsigned long long kHuge = 4096;  // products beyond this are left to k_expand_huge (the whole grid)
     const unsigned long long n_ent = min(*n_entries_dev, entry_cap);
     const int lane = threadIdx.x & 31;
     const unsigned long long warps = ((unsigned long long)gridDim.x * blockDim.x) >> 5;
@@ -255,11 +257,59 @@ __global__ void __launch_bounds__(256) k_expand_entries(const unsigned long long
             const uint32_t s_bi = __shfl_sync(kFullMask, bi, src), s_bj = __shfl_sync(kFullMask, bj, src);
             const uint32_t s_nj = __shfl_sync(kFullMask, nj, src);
             const unsigned long long s_w = __shfl_sync(kFullMask, w, src), s_first = __shfl_sync(kFullMask, first, src);
+            if (s_w > kHuge) {  // two heavily repeated sequences: one warp would take milliseconds
+                unsigned long long slot = 0;
+                if (lane == 0) slot = atomicAdd(n_huge, 1ull);
+                slot = __shfl_sync(kFullMask, slot, 0);
+                if (slot < huge_cap) {
+                    if (lane == 0) huge[slot] = make_ulonglong2(((unsigned long long)s_oi << 32) | s_oj, s_first);
+                    continue;
+                }
+            }
             for (unsigned long long k = (unsigned long long)lane; k < s_w; k += 32ull) {
                 const uint32_t x = (uint32_t)(k / s_nj), y = (uint32_t)(k % s_nj);
                 put(s_first + k, (s_oi & kGroupFlag) ? (uint32_t)members[s_bi + x] : s_oi,
                     (s_oj & kGroupFlag) ? (uint32_t)members[s_bj + y] : s_oj);
             }
+        }
+    }
+}
+
+// The products k_expand_entries set aside (both sequences repeated so often that rows x rows > kHuge): every product
+// is spread over the whole grid.
+__global__ void __launch_bounds__(256) k_expand_huge(const ulonglong2* __restrict__ huge,
+                                                    const unsigned long long* __restrict__ n_huge, uint32_t huge_cap,
+                                                    const uint32_t* __restrict__ group_start,
+                                                    const int32_t* __restrict__ members,
+                                                    unsigned long long* __restrict__ edges, unsigned long long edge_cap,
+                                                    int32_t* __restrict__ row_count, int32_t* __restrict__ deg) {
+    const unsigned long long cnt = min(*n_huge, (unsigned long long)huge_cap);
+    const unsigned long long tid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long h = 0; h < cnt; ++h) {
+        const ulonglong2 it = huge[h];
+        const uint32_t oi = (uint32_t)(it.x >> 32), oj = (uint32_t)it.x;
+        uint32_t bi = 0, ni = 1, bj = 0, nj = 1;
+        if (oi & kGroupFlag) {
+            const uint32_t g = oi & ~kGroupFlag;
+            bi = group_start[g];
+            ni = group_start[g + 1] - bi;
+        }
+        if (oj & kGroupFlag) {
+            const uint32_t g = oj & ~kGroupFlag;
+            bj = group_start[g];
+            nj = group_start[g + 1] - bj;
+        }
+        const unsigned long long w = (unsigned long long)ni * nj;
+        for (unsigned long long k = tid; k < w; k += stride) {
+            const uint32_t x = (uint32_t)(k / nj), y = (uint32_t)(k % nj);
+            const uint32_t ri = (oi & kGroupFlag) ? (uint32_t)members[bi + x] : oi;
+            const uint32_t rj = (oj & kGroupFlag) ? (uint32_t)members[bj + y] : oj;
+            const uint32_t a = min(ri, rj), b = max(ri, rj);
+            atomicAdd(row_count + a, 1);
+            atomicAdd(deg + b, 1);
+            const unsigned long long pos = it.y + k;
+            if (pos < edge_cap) edges[pos] = ((unsigned long long)a << 32) | b;
         }
     }
 }
@@ -334,10 +384,14 @@ cudaError_t launch_emit_cliques(const int32_t* members, const int32_t* uid_of, c
 cudaError_t launch_expand_entries(const unsigned long long* entries, const unsigned long long* n_entries_dev,
                                   unsigned long long entry_cap, const uint32_t* group_start, const int32_t* members,
                                   unsigned long long* edges, unsigned long long* edge_total, unsigned long long edge_cap,
-                                  int32_t* row_count, int32_t* deg, int n_sm, cudaStream_t s, int* launches) {
+                                  int32_t* row_count, int32_t* deg, void* huge, unsigned long long* n_huge,
+                                  uint32_t huge_cap, int n_sm, cudaStream_t s, int* launches) {
     k_expand_entries<<<(unsigned)(n_sm * 8), 256, 0, s>>>(entries, n_entries_dev, entry_cap, group_start, members, edges,
-                                                          edge_total, edge_cap, row_count, deg);
-    *launches += 1;
+                                                          edge_total, edge_cap, row_count, deg, (ulonglong2*)huge, n_huge,
+                                                          huge_cap);
+    k_expand_huge<<<(unsigned)(n_sm * 8), 256, 0, s>>>((const ulonglong2*)huge, n_huge, huge_cap, group_start, members,
+                                                       edges, edge_cap, row_count, deg);
+    *launches += 2;
     return cudaGetLastError();
 }
 

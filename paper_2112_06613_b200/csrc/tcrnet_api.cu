@@ -42,6 +42,7 @@ void drop_observables(tcrnet_ctx* ctx) { ctx->have_hist = ctx->have_nn = ctx->ha
 namespace {
 
 HostCtrl* d_ctrl(tcrnet_ctx* ctx) { return static_cast<HostCtrl*>(ctx->ctrl.p); }
+constexpr uint32_t kExpandHugeCap = 1u << 16;  // products set aside for k_expand_huge (beyond: expanded by their warp)
 
 int bits_for(int64_t max_value) {  // number of bits needed to represent max_value (>= 1)
     int b = 1;
@@ -566,6 +567,7 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
     static_assert(offsetof(HostCtrl, cand_count) == offsetof(HostCtrl, edge_total) + sizeof(unsigned long long), "one memset");
     if (expand_only) TRY_CUDA(cudaMemsetAsync(&dc->edge_total, 0, sizeof(unsigned long long), s));
     else TRY_CUDA(cudaMemsetAsync(&dc->edge_count, 0, sizeof(unsigned long long) * (11 + kTrieQueues), s));  // edge_count, work[8], queue[], edge_total, cand_count
+    TRY_CUDA(cudaMemsetAsync(&dc->n_huge, 0, sizeof(unsigned long long), s));
     TRY_CUDA(cudaMemsetAsync(ctx->row_count.p, 0, sizeof(int32_t) * (size_t)ctx->n, s));
     TRY_CUDA(cudaMemsetAsync(ctx->deg.p, 0, sizeof(int32_t) * (size_t)ctx->n, s));
     int n_queues = 0;
@@ -635,7 +637,8 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
                                          &dc->edge_total, cap_b, (int32_t*)ctx->row_count.p, (int32_t*)ctx->deg.p, s, launches));
         TRY_CUDA(launch_expand_entries((const unsigned long long*)ctx->keys_a.p, &dc->edge_count, cap, gs, mem,
                                        (unsigned long long*)ctx->keys_b.p, &dc->edge_total, cap_b, (int32_t*)ctx->row_count.p,
-                                       (int32_t*)ctx->deg.p, ctx->n_sm, s, launches));
+                                       (int32_t*)ctx->deg.p, ctx->expand_huge.p, &dc->n_huge, kExpandHugeCap, ctx->n_sm, s,
+                                       launches));
         TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->edge_total, &dc->edge_total, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
     }
     TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->edge_count, &dc->edge_count, sizeof(unsigned long long) * 9,
@@ -693,6 +696,7 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
     TRY(dev_reserve(ctx, ctx->deg, sizeof(int32_t) * (size_t)n));
     const bool grouped = ctx->all.grouped;
     int64_t cap_b = 0;
+    if (grouped) TRY(dev_reserve(ctx, ctx->expand_huge, 16 * (size_t)kExpandHugeCap));
     if (grouped) {
         cap_b = std::max<int64_t>(cap, (int64_t)(ctx->keys_b.bytes / 8));
         cap_b = std::min(cap_b, ctx->edge_limit);
@@ -866,7 +870,7 @@ void tcrnet_destroy(tcrnet_ctx* ctx) {
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     DevBuf* bufs[] = {&ctx->all.perm, &ctx->all.pat, &ctx->all.txt, &ctx->all.trie, &ctx->query.perm, &ctx->query.pat,
-                      &ctx->query.txt, &ctx->query.trie, &ctx->all.planes, &ctx->query.planes, &ctx->join_cand, &ctx->join_cnt, &ctx->join_dir,
+                      &ctx->query.txt, &ctx->query.trie, &ctx->all.planes, &ctx->query.planes, &ctx->join_cand, &ctx->expand_huge, &ctx->join_cnt, &ctx->join_dir,
                       &ctx->join_entries, &ctx->join_rows, &ctx->inv_perm, &ctx->edge_dist, &ctx->edge_dist_b, &ctx->flags,
                       &ctx->flag_pos, &ctx->in_res, &ctx->in_len, &ctx->offsets,
                       &ctx->perm_tmp, &ctx->trie_scratch, &ctx->keys_a, &ctx->keys_b, &ctx->radix_scratch,

@@ -19,6 +19,7 @@ struct HostCtrl {  // pinned mirror of the small device control block
     unsigned long long queue[kTrieQueues];  // dynamic work queues of the trie launches (zeroed with edge_count)
     unsigned long long edge_total;    // dedup: edges between rows after the expansion of the recorded pairs
     unsigned long long cand_count;    // segment join, l_max >= 2: pairs queued for verification (zeroed with edge_count)
+    unsigned long long n_huge;        // dedup: products of two heavily repeated sequences set aside by the expansion
     unsigned long long probe[3];
     uint32_t flags;
     uint32_t n_long;                  // rows queued for k_sort_long_rows
@@ -89,6 +90,7 @@ struct tcrnet_ctx {
     int built_l_max = 0;
     int64_t n_edges = 0, n_keys = 0;
     DevBuf keys_a, keys_b, radix_scratch, scan_scratch, rows, row_ptr, col, deg, row_count, long_rows;
+    DevBuf expand_huge;  // dedup.cu: (pair, first output position) of the products k_expand_huge spreads over the grid
     DevBuf inv_perm, edge_dist, edge_dist_b, flags, flag_pos;
     // segment join (segjoin.cu): directory + entries of the current load for join_l_max, work rows
     DevBuf join_cnt, join_dir, join_entries, join_rows, join_cand;

@@ -211,7 +211,9 @@ cudaError_t launch_emit_cliques(const int32_t* members, const int32_t* uid_of, c
 cudaError_t launch_expand_entries(const unsigned long long* entries, const unsigned long long* n_entries_dev,
                                   unsigned long long entry_cap, const uint32_t* group_start, const int32_t* members,
                                   unsigned long long* edges, unsigned long long* edge_total, unsigned long long edge_cap,
-                                  int32_t* row_count, int32_t* deg, int n_sm, cudaStream_t s, int* launches);
+                                  int32_t* row_count, int32_t* deg, void* huge /*16 B x huge_cap: products set aside*/,
+                                  unsigned long long* n_huge /*zeroed*/, uint32_t huge_cap, int n_sm, cudaStream_t s,
+                                  int* launches);
 // inv[row] = sorted position of the row's sequence, from the coded perm
 cudaError_t launch_inverse_perm_groups(const int32_t* perm, int64_t n_u, const uint32_t* group_start,
                                        const int32_t* members, int32_t* inv, cudaStream_t s, int* launches);

@@ -272,6 +272,24 @@ def test_heavily_repeated_rows_random(pkg, oracle, seed):
     check_csr_invariants(*got, len(strings))
 
 
+def test_products_of_two_heavily_repeated_sequences(pkg, oracle):
+    """Two neighbouring sequences that many rows share: rows x rows edges from ONE recorded pair (90 x 70, 200 x 90,
+    beyond what one warp expands itself: the product is spread over the grid), next to ordinary rows; every threshold,
+    also with buffers that have to grow."""
+    rng = np.random.default_rng(77)
+    d = generate("cfg1", n=300)
+    base = [bytes(r).decode() for r in np.split(d.residues, np.cumsum(d.lengths)[:-1])]
+    strings = base + ["CASSLGQYF"] * 90 + ["CASSLGEYF"] * 70 + ["CASSLEYF"] * 200 + ["CASSLGQAYF"] * 3
+    strings = [strings[i] for i in rng.permutation(len(strings))]
+    res, ln = from_strings(strings)
+    for l_max in (1, 2):
+        want = oracle.network(res, ln, l_max, tier=0)[:3]
+        for opts in ({}, {pkg.OPT_EDGE_CAPACITY: 50}, {pkg.OPT_SEGMENT_JOIN: 0}, {pkg.OPT_DEDUP: 0}):
+            got, st = gpu_network(pkg, res, ln, l_max, opts)
+            assert_same_network(got, want)
+    assert int(want[0][-1]) > 90 * 70 + 200 * 90
+
+
 def test_rows_of_every_sorting_regime(pkg, oracle):
     """The CSR step orders a row by one thread (<= 32 neighbours), in shared memory (<= 8192) or in place
     (beyond): a clique of 9,001 copies has rows of every such length; the other strings hang off it."""
