@@ -115,21 +115,24 @@ typedef enum tcrnet_option {
                                      for every l_max >= 0).  0: every row is its own pattern /
                                      text.  Never changes the result.  Ignored (off) in the
                                      rectangular mode.  Takes effect at the next load.          */
-    TCRNET_OPT_SEGMENT_JOIN = 11, /* exact candidate filter in front of the distance kernel: a text cut
-                                     into l_max + 1 segments shares at least one of them, unchanged and
-                                     shifted by at most the edits allow, with every sequence within
-                                     l_max of it; only pairs found through a hash index of the segments
-                                     are handed to the column recurrence.  -1 (default): used for
-                                     2 <= l_max <= 4 (all-pairs mode, early exit on); 1: also for
-                                     l_max <= 1; 0: never (every length-compatible pair is visited
-                                     through the prefix trie / text-chunk kernels).  Never changes the
-                                     result.                                                      */
-    TCRNET_OPT_FAST_L1 = 12       /* 1: builds with l_max <= 1 go through the segment
-                                     join and decide each candidate WITHOUT the recurrence - equal
-                                     lengths: XOR of the 5-bit packed codes confined to one residue;
-                                     lengths differing by one: common prefix + common suffix cover the
-                                     shorter sequence.  0 (default).  Never changes the result; its
-                                     time is reported beside, not inside, the cell-update metrics.  */
+    TCRNET_OPT_SEGMENT_JOIN = 11, /* exact candidate filter in front of the verification: a text cut into
+                                     l_max + 1 segments shares at least one of them, unchanged and shifted by
+                                     at most the edits allow, with every sequence within l_max of it; only
+                                     pairs found through a hash index of the segments are verified (banded,
+                                     Landau-Vishkin on per-diagonal mismatch masks).  -1 (default): used for
+                                     l_max <= 4 (all-pairs mode, early exit on, TCRNET_OPT_PREFIX_TRIE on); 1: the
+                                     same regardless of TCRNET_OPT_PREFIX_TRIE; 0: never (every length-compatible
+                                     pair is visited through the prefix trie / text-chunk kernels).  Never changes
+                                     the result.  Set it BEFORE tcrnet_load: a load made with 0 sorts the
+                                     sequences lexicographically inside their length buckets (the trie needs
+                                     that), any other load sorts by length only; a build that needs the trie on
+                                     a load sorted by length only falls back to the text-chunk kernel.        */
+    TCRNET_OPT_FAST_L1 = 12       /* 1: builds with l_max <= 1 go through the segment join
+                                     whatever TCRNET_OPT_SEGMENT_JOIN / TCRNET_OPT_PREFIX_TRIE say.  There the
+                                     verification IS the textbook check - equal lengths: at most one mismatching
+                                     residue (XOR of the packed codes); lengths differing by one: common prefix +
+                                     common suffix cover the shorter sequence.  0 (default): no effect (the
+                                     default path already takes the join).  Never changes the result.         */
 } tcrnet_option;
 
 /* Work and timing of the last tcrnet_load / tcrnet_build (tcrnet_get_stats). */

@@ -73,7 +73,8 @@ void drop_load(tcrnet_ctx* ctx) {
 // concatenated in order.
 // pre_hist != NULL: the (validated) length histogram of the rows is already on the host.
 int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* d_len, int64_t n, int64_t total_len,
-             const int64_t* ext_offsets, const unsigned long long* pre_hist, bool code_groups, int* launches) {
+             const int64_t* ext_offsets, const unsigned long long* pre_hist, bool code_groups, bool lexicographic,
+             int* launches) {
     set.loaded = false;
     set.grouped = false;
     set.n_rows = n;
@@ -141,21 +142,26 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
         d_off = (const int64_t*)offsets.p;
     }
     {
-        constexpr int kPasses = (kSeqKeyBits + kRadixBits - 1) / kRadixBits;
-        int shifts[kPasses];
-        for (int p = 0; p < kPasses; ++p) shifts[p] = kRadixBits * p;
+        // lexicographic: all 36 key bits (4 passes of 9-bit digits); else only the digit that holds the length (the
+        // segment join needs length buckets, nothing more: 1 pass)
+        constexpr int kAllPasses = (kSeqKeyBits + kRadixBits - 1) / kRadixBits;
+        static_assert(kRadixBits * (kAllPasses - 1) <= 5 * kSortPrefix, "the last digit holds the whole length field");
+        const int n_passes = lexicographic ? kAllPasses : 1;
+        int shifts[kAllPasses];
+        for (int p = 0; p < n_passes; ++p) shifts[p] = lexicographic ? kRadixBits * p : kRadixBits * (kAllPasses - 1);
         // an odd number of passes ends in the b buffers: make those set.perm
-        int32_t* va = (int32_t*)(kPasses & 1 ? ctx->perm_tmp.p : set.perm.p);
-        int32_t* vb = (int32_t*)(kPasses & 1 ? set.perm.p : ctx->perm_tmp.p);
+        int32_t* va = (int32_t*)(n_passes & 1 ? ctx->perm_tmp.p : set.perm.p);
+        int32_t* vb = (int32_t*)(n_passes & 1 ? set.perm.p : ctx->perm_tmp.p);
         if (e == cudaSuccess)
             e = launch_seq_keys(d_res, d_off, d_len, n, (unsigned long long*)ctx->keys_a.p, va, s, launches);
         bool in_b = false;
         if (e == cudaSuccess)
             e = radix_sort_u64((unsigned long long*)ctx->keys_a.p, (unsigned long long*)ctx->keys_b.p, va, vb, n, shifts,
-                               kPasses, ctx->radix_scratch.p, s, launches, &in_b);
+                               n_passes, ctx->radix_scratch.p, s, launches, &in_b);
         if (e == cudaSuccess && n > 1 && (in_b ? vb : va) != (int32_t*)set.perm.p) e = cudaErrorUnknown;
         if (e == cudaSuccess && n == 1)  // nothing was sorted: the payload sits in va
             e = cudaMemcpyAsync(set.perm.p, va, sizeof(int32_t), cudaMemcpyDeviceToDevice, s);
+        set.lexicographic = lexicographic;
     }
     if (e == cudaSuccess)
         e = launch_pack(d_res, d_off, d_len, (const int32_t*)set.perm.p, n, lt, set.pat_stride,
@@ -283,21 +289,24 @@ int dedup_rows(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t
 int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len, int64_t n, int64_t total_len,
                      int* launches) {
     const bool rect = ctx->n_query > 0 && ctx->n_query < n;
+    // Sub-order inside a length bucket: lexicographic by the first residues when the prefix-trie kernel will serve
+    // the builds of this load (it walks a trie over the sorted texts); the segment join only needs the buckets.
+    const bool lex = rect || !ctx->early_exit || ctx->segment_join == 0;
     int64_t n_u = n;
     if (ctx->dedup && !rect && n >= 2) {
         TRY(dedup_rows(ctx, ctx->all, d_res, d_len, n, total_len, &n_u, launches));
         if (n_u < n) {
             TRY(pack_set(ctx, ctx->all, d_res, (const int32_t*)ctx->dd_len.p, n_u, -1, (const int64_t*)ctx->dd_off.p,
-                         ctx->hist_u_host, true, launches));
+                         ctx->hist_u_host, true, lex, launches));
             ctx->all.grouped = true;
             ctx->all.n_rows = n;
         }
     }
     if (!ctx->all.loaded || !ctx->all.grouped) {
         n_u = n;
-        TRY(pack_set(ctx, ctx->all, d_res, d_len, n, total_len, nullptr, nullptr, false, launches));
+        TRY(pack_set(ctx, ctx->all, d_res, d_len, n, total_len, nullptr, nullptr, false, lex, launches));
     }
-    if (rect) TRY(pack_set(ctx, ctx->query, d_res, d_len, ctx->n_query, -1, nullptr, nullptr, false, launches));
+    if (rect) TRY(pack_set(ctx, ctx->query, d_res, d_len, ctx->n_query, -1, nullptr, nullptr, false, lex, launches));
     if (!ctx->all.grouped)
         for (int l = 0; l < kNumLen; ++l) ctx->row_hist[l] = ctx->all.hist[l];
     ctx->stats.n_distinct = n_u;
@@ -377,7 +386,8 @@ void schedule_pass(const tcrnet_ctx* ctx, int l_max, int first_check, bool use_j
     const SeqSet& ts = *pass.tset;
     // The trie kernel serves the rows whose early exit can act inside the trie (l_max <= kTrieMaxL, the
     // values it is specialised on) and that have at least one text column beyond the trie.
-    const bool use_trie = ctx->prefix_trie && first_check > 0 && l_max <= kTrieMaxL;
+    // (a set loaded for the segment join is bucketed by length only: no trie can be laid over it)
+    const bool use_trie = ctx->prefix_trie && first_check > 0 && l_max <= kTrieMaxL && ts.lexicographic;
     for (int m = 1; m < kNumLen; ++m) {
         if (!ps.hist[m]) continue;
         const int n0 = pass.mode == kPairsAllQuery ? m + 1 : m;

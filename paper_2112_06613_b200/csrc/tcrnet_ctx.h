@@ -41,6 +41,7 @@ struct SeqSet {
     int pat_stride = 0;
     DevBuf perm, pat, txt, trie, planes;
     bool wide_planes = false;  // bit-plane rows of 64-bit words (the longest sequence has more than 32 residues)
+    bool lexicographic = false;  // sorted by (length, first residues): the prefix trie can be built; else by length only
     bool text_tables = false;  // txt + trie are built (on demand: only the prefix-trie / text-chunk kernels read them)
     TrieLevels trie_levels{};
     uint32_t trie_root[kNumLen + 1] = {};  // level-1 node range of bucket L: [trie_root[L], trie_root[L+1])
