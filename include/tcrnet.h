@@ -357,11 +357,26 @@ TCRNET_API int tcrnet_degrees(tcrnet_ctx* ctx, const int32_t** deg_dev);
  */
 TCRNET_API int tcrnet_copy_csr(tcrnet_ctx* ctx, int64_t* row_ptr_host, int32_t* col_host, int32_t* deg_host);
 
-/* Set a tcrnet_option.  Takes effect at the next tcrnet_build.  Errors: ARG. */
+/* Set a tcrnet_option.  Takes effect at the next tcrnet_build unless the option says "next tcrnet_load".
+   Errors: ARG. */
 TCRNET_API int tcrnet_set_option(tcrnet_ctx* ctx, int option, int64_t value);
 
 /* Fill *out (host) with the work / timing record described above.  Errors: ARG. */
 TCRNET_API int tcrnet_get_stats(tcrnet_ctx* ctx, tcrnet_stats* out);
+
+/* Last cudaError_t seen by this context (0 if none), for diagnostics. */
+TCRNET_API int tcrnet_last_cuda_error(tcrnet_ctx* ctx);
+
+/* Static string for a tcrnet_status. */
+TCRNET_API const char* tcrnet_strerror(int status);
+
+/* TCRNET_VERSION the library was built with. */
+TCRNET_API int tcrnet_version(void);
+
+/* ---------------------------------------------------------------------------------------------
+ * Diagnostics - NOT part of the method: nothing above calls it and no result depends on it.
+ * bench.py uses it to print the measured pipe ceilings beside the roofline it reports.
+ * ------------------------------------------------------------------------------------------- */
 
 /*
  * Measurement aid for the roofline denominator: run a dependent-chain-
@@ -372,15 +387,6 @@ TCRNET_API int tcrnet_get_stats(tcrnet_ctx* ctx, tcrnet_stats* out);
  * clock64 / event time) are host pointers.  Errors: ARG, CUDA.
  */
 TCRNET_API int tcrnet_probe_int32(tcrnet_ctx* ctx, int kind, double* ops_per_s, double* sm_clock_mhz);
-
-/* Last cudaError_t seen by this context (0 if none), for diagnostics. */
-TCRNET_API int tcrnet_last_cuda_error(tcrnet_ctx* ctx);
-
-/* Static string for a tcrnet_status. */
-TCRNET_API const char* tcrnet_strerror(int status);
-
-/* TCRNET_VERSION the library was built with. */
-TCRNET_API int tcrnet_version(void);
 
 #ifdef __cplusplus
 }

@@ -152,7 +152,7 @@ __global__ void __launch_bounds__(256) k_sort_long_rows(const int64_t* __restric
 cudaError_t launch_count_rows(const unsigned long long* keys, int64_t n_keys, int32_t* row_count, int32_t* deg,
                               cudaStream_t s, int* launches) {
     if (n_keys <= 0) return cudaSuccess;
-    const int64_t blocks = std::min<int64_t>((n_keys + 255) / 256, kGridSMs * 16);
+    const int64_t blocks = std::min<int64_t>((n_keys + 255) / 256, device_sm_count() * 16);
     k_count_rows<<<(unsigned)blocks, 256, 0, s>>>(keys, n_keys, row_count, deg);
     *launches += 1;
     return cudaGetLastError();
@@ -166,9 +166,9 @@ cudaError_t launch_csr_unsorted(const unsigned long long* keys, int64_t n_keys, 
     if (e == cudaSuccess) e = cudaMemsetAsync(n_long, 0, sizeof(uint32_t), s);
     if (e != cudaSuccess || n_keys <= 0) return e;
     const int64_t blocks = (n_keys + 255) / 256;
-    k_scatter_keys<<<(unsigned)std::min<int64_t>(blocks, kGridSMs * 32), 256, 0, s>>>(keys, n_keys, row_ptr, row_count, bucket);
+    k_scatter_keys<<<(unsigned)std::min<int64_t>(blocks, device_sm_count() * 32), 256, 0, s>>>(keys, n_keys, row_ptr, row_count, bucket);
     k_rank_rows<<<(unsigned)blocks, 256, 0, s>>>(bucket, n_keys, row_ptr, col, deg, long_rows, n_long);
-    k_sort_long_rows<<<(unsigned)std::min<int64_t>(n, kGridSMs * 4), 256, 0, s>>>(row_ptr, bucket, col, long_rows, n_long);
+    k_sort_long_rows<<<(unsigned)std::min<int64_t>(n, device_sm_count() * 4), 256, 0, s>>>(row_ptr, bucket, col, long_rows, n_long);
     *launches += 3;
     return cudaGetLastError();
 }
@@ -180,7 +180,7 @@ cudaError_t launch_csr(const unsigned long long* sorted_keys, int64_t n_edges, i
     *launches += 2;
     if (n_edges > 0) {
         int64_t blocks = (n_edges + 255) / 256;
-        if (blocks > kGridSMs * 16) blocks = kGridSMs * 16;
+        if (blocks > device_sm_count() * 16) blocks = device_sm_count() * 16;
         k_col_deg_lower<<<(unsigned)blocks, 256, 0, s>>>(sorted_keys, n_edges, col, deg);
         *launches += 1;
     }

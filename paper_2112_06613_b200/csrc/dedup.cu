@@ -36,6 +36,14 @@ __device__ __forceinline__ unsigned long long hash_row(const uint8_t* src, int l
     return h;
 }
 
+// The probe path of a row starts at a slot derived from its FINGERPRINT alone, so all rows with one fingerprint walk
+// the same path and meet in one slot whatever the order of the inserts: which rows collapse does not depend on timing
+// (two different sequences with one fingerprint: the rows of the one that owns the smallest row collapse, the rows of
+// the other stay sequences of their own - on every rank of a sharded build alike).
+__device__ __forceinline__ uint32_t start_slot(unsigned long long fp, uint32_t mask) {
+    return (uint32_t)(((fp >> 32) * 0x9E3779B97F4A7C15ull) >> 32) & mask;
+}
+
 __global__ void __launch_bounds__(256) k_dedup_insert(const uint8_t* __restrict__ residues,
                                                      const int64_t* __restrict__ offsets,
                                                      const int32_t* __restrict__ lengths, int64_t n, int64_t total_len,
@@ -54,7 +62,7 @@ __global__ void __launch_bounds__(256) k_dedup_insert(const uint8_t* __restrict_
     hash[i] = h;
     const unsigned long long fp = h & 0xffffffff00000000ull;
     const unsigned long long mine = fp | (unsigned long long)i;
-    uint32_t s = (uint32_t)h & mask;
+    uint32_t s = start_slot(fp, mask);
     for (;;) {
         unsigned long long cur = table[s];
         if (cur == kEmptySlot) {
@@ -81,7 +89,7 @@ __global__ void __launch_bounds__(256) k_dedup_lookup(const uint8_t* __restrict_
     int64_t rep = i;
     if (h != kEmptySlot) {
         const unsigned long long fp = h & 0xffffffff00000000ull;
-        uint32_t s = (uint32_t)h & mask;
+        uint32_t s = start_slot(fp, mask);
         for (;;) {
             const unsigned long long cur = table[s];
             if ((cur & 0xffffffff00000000ull) == fp && cur != kEmptySlot) {
@@ -154,7 +162,7 @@ __global__ void __launch_bounds__(256) k_emit_cliques(const int32_t* __restrict_
                                                      unsigned long long* __restrict__ edges,
                                                      unsigned long long* __restrict__ edge_count,
                                                      unsigned long long edge_cap, int32_t* __restrict__ row_count,
-                                                     int32_t* __restrict__ deg) {
+                                                     int32_t* __restrict__ deg, uint32_t shard, uint32_t n_shards) {
     constexpr uint32_t kFullMask = 0xffffffffu;
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
@@ -162,9 +170,11 @@ __global__ void __launch_bounds__(256) k_emit_cliques(const int32_t* __restrict_
     if (s < n) {
         r = (uint32_t)members[s];
         const uint32_t uid = (uint32_t)uid_of[r];
-        begin = group_start[uid];
-        end = group_start[uid + 1u];
-        rest = end - 1u - (uint32_t)s;  // slots after this one
+        if (uid % n_shards == shard) {  // step 8(e): the shared sequences are dealt out to the shards by uid
+            begin = group_start[uid];
+            end = group_start[uid + 1u];
+            rest = end - 1u - (uint32_t)s;  // slots after this one
+        }
     }
     if (end - begin > 1u) {
         uint32_t larger = 0;
@@ -375,8 +385,9 @@ cudaError_t launch_dedup_codes(int32_t* perm, int64_t n_u, const uint32_t* group
 
 cudaError_t launch_emit_cliques(const int32_t* members, const int32_t* uid_of, const uint32_t* group_start, int64_t n,
                                 unsigned long long* edges, unsigned long long* edge_count, unsigned long long edge_cap,
-                                int32_t* row_count, int32_t* deg, cudaStream_t s, int* launches) {
-    k_emit_cliques<<<grid_for(n), 256, 0, s>>>(members, uid_of, group_start, n, edges, edge_count, edge_cap, row_count, deg);
+                                int32_t* row_count, int32_t* deg, int shard, int n_shards, cudaStream_t s, int* launches) {
+    k_emit_cliques<<<grid_for(n), 256, 0, s>>>(members, uid_of, group_start, n, edges, edge_count, edge_cap, row_count, deg,
+                                               (uint32_t)shard, (uint32_t)n_shards);
     *launches += 1;
     return cudaGetLastError();
 }

@@ -211,7 +211,7 @@ __global__ void __launch_bounds__(256) k_check_permutation(const int32_t* __rest
 unsigned grid_for(int64_t n) { return (unsigned)((n + 255) / 256); }
 unsigned grid_capped(int64_t n) {
     int64_t b = (n + 255) / 256;
-    if (b > kGridSMs * 8) b = kGridSMs * 8;
+    if (b > device_sm_count() * 8) b = device_sm_count() * 8;
     return (unsigned)(b > 0 ? b : 1);
 }
 

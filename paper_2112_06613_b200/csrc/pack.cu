@@ -168,10 +168,25 @@ __global__ void __launch_bounds__(256) k_txt_from_pat(const uint8_t* __restrict_
 
 }  // namespace
 
+int device_sm_count() {
+    static int cached[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
+    if (cached[dev] == 0) {
+        int v = 0;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0) {
+            (void)cudaGetLastError();
+            return 148;
+        }
+        cached[dev] = v;
+    }
+    return cached[dev];
+}
+
 cudaError_t launch_length_hist(const int32_t* lengths, int64_t n, const uint32_t* n_dev, unsigned long long* hist,
                                uint32_t* flags, cudaStream_t s, int* launches) {
     int64_t blocks = (n + 255) / 256;
-    if (blocks > kGridSMs * 8) blocks = kGridSMs * 8;
+    if (blocks > device_sm_count() * 8) blocks = device_sm_count() * 8;
     k_length_hist<<<(unsigned)blocks, 256, 0, s>>>(lengths, n, n_dev, hist, flags);
     *launches += 1;
     return cudaGetLastError();

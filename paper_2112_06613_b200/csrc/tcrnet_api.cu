@@ -639,12 +639,12 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
     if (!expand_only) TRY_CUDA(cudaEventRecord(ctx->ev[5], s));
     if (ctx->all.grouped) {
         // the recorded pairs of distinct sequences -> edges between rows (keys_b), counted for the CSR step; the rows
-        // of every shared sequence are joined to each other (d = 0) by the first shard
+        // of every shared sequence are joined to each other (d = 0), each sequence by the shard uid mod n_shards
         const uint32_t* gs = (const uint32_t*)ctx->all.group_start.p;
         const int32_t* mem = (const int32_t*)ctx->all.members.p;
-        if (shard == 0)
-            TRY_CUDA(launch_emit_cliques(mem, (const int32_t*)ctx->all.uid_of.p, gs, ctx->n, (unsigned long long*)ctx->keys_b.p,
-                                         &dc->edge_total, cap_b, (int32_t*)ctx->row_count.p, (int32_t*)ctx->deg.p, s, launches));
+        TRY_CUDA(launch_emit_cliques(mem, (const int32_t*)ctx->all.uid_of.p, gs, ctx->n, (unsigned long long*)ctx->keys_b.p,
+                                     &dc->edge_total, cap_b, (int32_t*)ctx->row_count.p, (int32_t*)ctx->deg.p, shard, n_shards,
+                                     s, launches));
         TRY_CUDA(launch_expand_entries((const unsigned long long*)ctx->keys_a.p, &dc->edge_count, cap, gs, mem,
                                        (unsigned long long*)ctx->keys_b.p, &dc->edge_total, cap_b, (int32_t*)ctx->row_count.p,
                                        (int32_t*)ctx->deg.p, ctx->expand_huge.p, &dc->n_huge, kExpandHugeCap, ctx->n_sm, s,

@@ -20,7 +20,6 @@ constexpr int kSortPrefix = 6;           // residues of the lexicographic sub-or
 constexpr int kTrieDepth = kSortPrefix;  // levels 1..kTrieDepth of the prefix trie over each text bucket
 constexpr int kTrieFan = 27;             // staging slots per trie level, indexed by residue code (0..26)
 constexpr int kTrieMaxL = 4;             // the trie kernel is specialised on l_max = 0..kTrieMaxL
-constexpr int kGridSMs = 148;            // B200: grid-stride kernels are sized in multiples of the SM count
 constexpr int kTrieTile = 32;            // patterns per work item of the trie kernel: one warp
 constexpr int kTrieQueues = 8;           // dynamic work queues (one per trie launch of a distance pass)
 constexpr uint32_t kGroupFlag = 0x80000000u;  // perm entry = kGroupFlag | uid: a sequence shared by several rows (dedup.cu)
@@ -137,6 +136,9 @@ struct JoinIndex {
 // plane k = bit k of the 5-bit code of residue j (zero beyond the sequence); word 5 = length; 6, 7 = 0.
 constexpr int kPlaneWords = 8;
 
+// SM count of the current device (148 on B200; cached per device): grid-stride kernels are sized in multiples of it
+int device_sm_count();
+
 // ---- launch wrappers (each returns cudaGetLastError(); *launches is incremented per kernel) ----
 
 // scan.cu: out[i] = sum_{k<i} in[k] for i in 0..n (n+1 outputs when write_total).
@@ -203,10 +205,10 @@ cudaError_t launch_dedup_fill(const int32_t* uid_of, int64_t n, const uint32_t* 
 // perm[s] = uid -> the row itself (a sequence of one row) or kGroupFlag | uid
 cudaError_t launch_dedup_codes(int32_t* perm, int64_t n_u, const uint32_t* group_start, const int32_t* members,
                                cudaStream_t s, int* launches);
-// the edges among the rows of every shared sequence (distance 0)
+// the edges among the rows of every shared sequence (distance 0); sequences uid = shard (mod n_shards) only
 cudaError_t launch_emit_cliques(const int32_t* members, const int32_t* uid_of, const uint32_t* group_start, int64_t n,
                                 unsigned long long* edges, unsigned long long* edge_count, unsigned long long edge_cap,
-                                int32_t* row_count, int32_t* deg, cudaStream_t s, int* launches);
+                                int32_t* row_count, int32_t* deg, int shard, int n_shards, cudaStream_t s, int* launches);
 // the recorded pairs of distinct sequences (at most entry_cap of the *n_entries_dev counted) -> edges between rows
 cudaError_t launch_expand_entries(const unsigned long long* entries, const unsigned long long* n_entries_dev,
                                   unsigned long long entry_cap, const uint32_t* group_start, const int32_t* members,

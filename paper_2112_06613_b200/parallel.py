@@ -19,21 +19,23 @@ import torch.distributed as dist
 
 def all_gather_v(t: torch.Tensor, group: Optional["dist.ProcessGroup"] = None) -> torch.Tensor:
     """Concatenation, in rank order, of every rank's 1-D tensor `t` (lengths may differ, 0 allowed).
-    Works for CUDA tensors over NCCL and CPU tensors over gloo."""
+    Works for CUDA tensors over NCCL and CPU tensors over gloo.  Two collectives, one host synchronisation: the
+    counts (one all_gather_into_tensor, read back once), then the keys padded to the longest shard (one
+    all_gather_into_tensor into a single buffer; shards of interleaved work items differ by a few percent)."""
     assert t.dim() == 1
     world = dist.get_world_size(group)
     if world == 1:
         return t
-    count = torch.tensor([t.numel()], dtype=torch.int64, device=t.device)
-    counts: List[torch.Tensor] = [torch.zeros_like(count) for _ in range(world)]
-    dist.all_gather(counts, count, group=group)
-    sizes = [int(c.item()) for c in counts]
+    counts = torch.empty(world, dtype=torch.int64, device=t.device)
+    dist.all_gather_into_tensor(counts, torch.tensor([t.numel()], dtype=torch.int64, device=t.device), group=group)
+    sizes = counts.tolist()  # the one host synchronisation
     width = max(max(sizes), 1)
-    padded = torch.zeros(width, dtype=t.dtype, device=t.device)
-    padded[: t.numel()] = t
-    parts = [torch.empty(width, dtype=t.dtype, device=t.device) for _ in range(world)]
-    dist.all_gather(parts, padded, group=group)
-    return torch.cat([p[:s] for p, s in zip(parts, sizes)])
+    padded = t if t.numel() == width else torch.cat([t, t.new_zeros(width - t.numel())])
+    parts = torch.empty(world * width, dtype=t.dtype, device=t.device)
+    dist.all_gather_into_tensor(parts, padded, group=group)
+    if all(s == width for s in sizes):
+        return parts
+    return torch.cat([parts[r * width: r * width + s] for r, s in enumerate(sizes)])
 
 
 def build_distributed(net, l_max: int, group: Optional["dist.ProcessGroup"] = None) -> int:

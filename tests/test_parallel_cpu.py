@@ -35,6 +35,26 @@ def _worker(rank: int, world: int, port: int, keys_by_rank, n: int, out_dir: str
         # ragged edge case: one rank contributes nothing
         empty = parallel.all_gather_v(mine[:0] if rank == 0 else mine[:5])
         assert empty.numel() == 5 and torch.equal(empty, torch.from_numpy(keys_by_rank[1][:5]))
+
+        # parallel.build_distributed itself, end to end, on a stand-in for the context: build_shard hands out this
+        # rank's share of the oracle's keys (what tcrnet_build_shard does with the work items), assemble collects
+        class Net:
+            def __init__(self):
+                self.calls = []
+
+            def build_shard(self, l_max, shard, n_shards):
+                self.calls.append((l_max, shard, n_shards))
+                return torch.from_numpy(keys_by_rank[shard])
+
+            def assemble(self, keys):
+                self.keys = keys
+                return int(keys.numel())
+
+        net = Net()
+        n_edges = parallel.build_distributed(net, 2)
+        assert net.calls == [(2, rank, world)]
+        assert n_edges == sum(k.size for k in keys_by_rank)
+        np.save(os.path.join(out_dir, f"built{rank}.npy"), net.keys.numpy())
     finally:
         dist.destroy_process_group()
 
@@ -56,6 +76,7 @@ def test_two_rank_key_exchange_matches_oracle(tmp_path):
         assert np.array_equal(got, np.concatenate(keys_by_rank))          # rank order, nothing lost
         assert np.array_equal(np.sort(got), keys)                          # the union is the edge set
         assert np.array_equal(np.load(tmp_path / f"deg{r}.npy"), deg.astype(np.int64))
+        assert np.array_equal(np.sort(np.load(tmp_path / f"built{r}.npy")), keys)  # build_distributed: every rank, all edges
 
 
 def test_single_process_is_identity():

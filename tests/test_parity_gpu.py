@@ -559,6 +559,33 @@ def test_cfg5_sampled(pkg, oracle):
     assert_same_network(a, b)
 
 
+def test_large_n_sort_and_scan_paths(pkg):
+    """N = 4,500,000 short rows: beyond the thresholds where the sequence sort switches to 4096-key tiles
+    (n >= 4,194,304) and the prefix sums to their three-launch form (n > 2,097,152).  l_max = 0, where the network is
+    known without any distance: rows are joined iff their bytes are equal (exact-match join by sorting, the oracle's
+    own pin for l_max = 0), so degrees and the edge count follow from the multiplicities.  Both load orders (by length
+    only / lexicographic) and both kernels."""
+    rng = np.random.default_rng(4500)
+    n = 4_500_000
+    ln = rng.integers(6, 11, n).astype(np.int32)
+    mat = np.frombuffer(b"ACDEFGHIKLMNPQRSTVWY", dtype=np.uint8)[rng.integers(0, 20, (n, 10))]
+    mat[np.arange(10)[None, :] >= ln[:, None]] = 0
+    res = np.ascontiguousarray(mat[mat != 0])
+    _, inv, cnt = np.unique(np.ascontiguousarray(mat).view("V10").ravel(), return_inverse=True, return_counts=True)
+    want_deg = (cnt[inv] - 1).astype(np.int32)
+    want_edges = int((cnt.astype(np.int64) * (cnt - 1) // 2).sum())
+    assert want_edges > 1000
+    for opts in ({}, {pkg.OPT_SEGMENT_JOIN: 0}):
+        (rp, cl, dg), st = gpu_network(pkg, res, ln, 0, opts)
+        # (two different sequences may share a 32-bit fingerprint: the repeated rows of one of them then stay sequences
+        # of their own - a few more "distinct" sequences than there are, never a different network)
+        assert cnt.size <= st["n_distinct"] <= cnt.size + 100 and int(rp[-1]) == want_edges
+        assert np.array_equal(dg, want_deg)
+        check_csr_invariants(rp, cl, dg, n)
+        rows_of = np.repeat(np.arange(n, dtype=np.int64), np.diff(rp))
+        assert np.array_equal(inv[rows_of], inv[cl])  # every edge joins two rows with the same bytes
+
+
 # ------------------------------------------------------------------ 8(e): shards; 8(f): labels, sweep, query mode
 def test_shards_partition_the_edge_set(pkg, oracle):
     """tcrnet_build_shard: the work items are dealt out to the shards interleaved; the shards' key
