@@ -48,7 +48,10 @@ ORACLE_SAMPLE_ROWS = 1024
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the ncu --set full captures
 # summarised under profiles/ (regenerated with them; a workload / kernel that is not listed prints null)
 NCU_DRAM_BYTES_PER_LAUNCH = {
-    # (workload, kernel): bytes   -- filled from profiles/r2_*.txt
+    # (workload, kernel): bytes per step of that kernel / kernel pair - profiles/r2_join_ncu.txt
+    ("cfg4", "k_join_probe"): 35_105_536 + 1_792,
+    ("cfg3", "k_join_probe + k_join_verify"): 11_109_632 + 12_340_224,
+    ("cfg5", "k_join_probe + k_join_verify"): 2_381_505_000 + 378_921_216 + 533_883_000 + 49_555_968,
 }
 
 

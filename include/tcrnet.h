@@ -202,10 +202,12 @@ TCRNET_API void tcrnet_destroy(tcrnet_ctx* ctx);
 
 /*
  * Step A1 (pack): take N sequences, validate them, copy them to the device and lay them out
- * for the distance kernels (rows collapsed to distinct sequences, stable sort by (length, first six
- * residues, row), length buckets, permutation; per sorted position one row of 8-bit residue codes for
- * the match masks and one row of 5-bit packed codes, 16 bytes up to 25 residues; prefix trie over the
- * sorted texts).  PAPER.md:326 ("each a.a. is saved as a number ... BYTE"), north_star (1).
+ * for the distance kernels: rows collapsed to distinct sequences; stable sort into length buckets (by
+ * length and row; by length, first six residues and row when TCRNET_OPT_SEGMENT_JOIN = 0, the rectangular
+ * mode or TCRNET_OPT_EARLY_EXIT = 0 announce the prefix-trie kernel); permutation; per sorted position one
+ * bit-plane row (5-bit residue codes, one bit of the code per word, 32 bytes up to 32 residues) and one row
+ * of 8-bit residue codes.  The text rows and the prefix trie of the trie / text-chunk kernels are built by
+ * the first build that needs them.  PAPER.md:326 ("each a.a. is saved as a number ... BYTE"), north_star (1).
  *
  *   residues  host, uint8[sum(lengths)]: the rows concatenated, ASCII 'A'..'Z' (any of the 26
  *             letters is a legal residue; only equality matters - DESIGN.md reading Q8)
@@ -229,10 +231,13 @@ TCRNET_API int tcrnet_load_device(tcrnet_ctx* ctx, const uint8_t* residues_dev, 
                        int64_t total_len);
 
 /*
- * Steps A2-A6: enumerate the length-compatible pairs (|len_i - len_j| <= l_max, each unordered
- * pair once), compute every such pair's Levenshtein distance (bit-parallel, exact), keep the
- * pairs with distance <= l_max, and assemble CSR + degrees on the device
- * (PAPER.md:301-318, 224).  l_max in 0..TCRNET_MAX_LEN.  May be called repeatedly on one load.
+ * Steps A2-A6: decide, for every unordered pair of rows, whether its Levenshtein distance
+ * is <= l_max, and assemble CSR + degrees on the device.  Pairs with
+ * |len_i - len_j| > l_max are never touched; for l_max <= 4 (default path) only pairs that share one of the
+ * l_max + 1 segments of the longer sequence are looked at (every pair within l_max does: pigeonhole) and decided
+ * exactly by a banded bit-parallel verification; otherwise every length-compatible pair goes through the
+ * bit-parallel column recurrence with an exact early exit (TCRNET_OPT_SEGMENT_JOIN).  The result is the same on
+ * every path.  l_max in 0..TCRNET_MAX_LEN.  May be called repeatedly on one load.
  * *n_edges_out (host, may be NULL) receives |E|.  Synchronises the stream.
  * Errors: STATE (no load), LMAX, NOMEM, EDGE_OVERFLOW, CUDA.
  */
