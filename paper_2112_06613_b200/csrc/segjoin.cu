@@ -15,10 +15,10 @@
 //      M_s[j] = (a_j != b_(j+s))  =  OR_k (A_k ^ (B_k >> s))[j],
 // costs five shifts and five LOP3 for ALL residues at once.  Everything below works on these masks:
 //
-//   index   k_join_index: one entry (tag, text) per (text, segment), bucketed by a hash of (n, i, segment bits) in a
-//           power-of-two directory (count -> prefix sum -> fill).
+//   index   k_join_index: one entry (composition signature, text) per (text, segment), bucketed by a hash of
+//           (n, i, segment bits) in a power-of-two directory (count -> prefix sum -> fill).
 //   probe   k_join_probe: one warp = 32 patterns of one length x one length difference delta; for every probe each lane
-//           hashes its pattern's substring and walks the directory bucket; the texts whose tag matches (same length
+//           hashes its pattern's substring and walks the directory bucket; the texts whose composition can be within l_max (same length
 //           bucket: only texts after the pattern in sorted order, so every unordered pair is seen once) are queued in
 //           shared memory and checked 32 at a time, one per lane: build the masks of the band's diagonals
 //           s = -floor((l_max - delta) / 2) .. delta + floor((l_max - delta) / 2)  (no alignment with <= l_max edits
@@ -232,6 +232,44 @@ __device__ __forceinline__ bool lv_within(const W (&M)[L + 1], int m, int n, int
     return end >= m;
 }
 
+// Composition signature of a sequence: the residue codes fall into 8 classes (code & 7); nibble g = the number of
+// residues of class g, saturated at 7.  One edit moves at most one residue out of a class and one into a class, so
+//     sum_g |count_r(g) - count_s(g)|  <=  2 * substitutions + insertions + deletions  <=  2 * l_max - delta
+// for every pair within l_max whose lengths differ by delta (at least delta of the edits are insertions); saturation
+// only shrinks the left side.  The index stores the signature of the text in every entry, so most texts that merely
+// share a (short, low-entropy) segment with the pattern are dropped before their row is fetched.
+template <typename W>
+__device__ __forceinline__ uint32_t class_counts(const PlaneRow<W>& R) {
+    const W valid = low_mask<W>(R.len);
+    uint32_t sig = 0u;
+#pragma unroll
+    for (int g = 0; g < 8; ++g) {
+        W mk = valid;
+        mk &= (g & 1) ? R.p[0] : ~R.p[0];
+        mk &= (g & 2) ? R.p[1] : ~R.p[1];
+        mk &= (g & 4) ? R.p[2] : ~R.p[2];
+        sig |= (uint32_t)min(WordOps<W>::popc(mk), 7) << (4 * g);
+    }
+    return sig;
+}
+// The top bit of every nibble is free: an index entry keeps its segment number there (bits 3, 7, 11), so that a probe
+// for segment i only ever takes entries OF segment i.  Together with the residue-wise test of the probe's segment this
+// makes a text appear at most once per probe: an entry of segment i that passes that test has the probe's key, and a
+// text has one entry per segment (a foreign key that merely shares the hash bucket would otherwise let a text in twice).
+__device__ __forceinline__ uint32_t segment_code(int i) {
+    return (((uint32_t)i & 1u) << 3) | (((uint32_t)i & 2u) << 6) | (((uint32_t)i & 4u) << 9);
+}
+constexpr uint32_t kSegmentCodeMask = 0x888u;
+// sum over the 8 nibbles of |a_g - b_g| (each 0..7; top bits of b ignored), SWAR
+__device__ __forceinline__ int class_distance(uint32_t a, uint32_t b) {
+    b &= 0x77777777u;
+    const uint32_t x = (a | 0x88888888u) - b;                 // nibble g = 8 + a_g - b_g: no borrow leaves a nibble
+    const uint32_t neg = (~x >> 3) & 0x11111111u;             // 1 where a_g < b_g
+    uint32_t v = (x ^ (neg * 7u)) & 0x77777777u;              // |a_g - b_g| - [a_g < b_g]
+    v = (v & 0x0F0F0F0Fu) + ((v >> 4) & 0x0F0F0F0Fu);
+    return (int)((v * 0x01010101u) >> 24) + __popc(neg);
+}
+
 // hash of (text length n, segment i, residues [q, q + len) of the row)
 template <typename W>
 __device__ __forceinline__ unsigned long long seg_hash(const PlaneRow<W>& R, int q, int len, int n, int i) {
@@ -276,7 +314,7 @@ __global__ void __launch_bounds__(256) k_join_index(const void* __restrict__ pla
         atomicAdd(cnt + b, 1u);
     } else {
         const uint32_t slot = atomicSub(cnt + b, 1u) - 1u;
-        entries[dir[b] + slot] = make_uint2((uint32_t)(h >> 32), (uint32_t)t);
+        entries[dir[b] + slot] = make_uint2(class_counts<W>(R) | segment_code(i), (uint32_t)t);
     }
 }
 
@@ -417,6 +455,8 @@ __global__ void __launch_bounds__(kJoinThreads) k_join_probe(const __grid_consta
     const bool p_valid = tile * 32 + lane < Rw.p_count;
     const int p = p_valid ? w.p0 + lane : w.p0;
     w.A = load_planes<W>(S.planes, p);
+    const uint32_t sig = class_counts<W>(w.A);
+    const int sig_max = 2 * L - delta;  // composition bound of a pair within L
     const int m = w.m, n = w.n;
     unsigned long long n_entries = 0, n_cand = 0, n_probes = 0;
 
@@ -425,13 +465,13 @@ __global__ void __launch_bounds__(kJoinThreads) k_join_probe(const __grid_consta
         const int i = S.tab.probe_seg[delta][pi], d = S.tab.probe_shift[delta][pi];
         const int sq = S.tab.seg_start[n][i], len = S.tab.seg_start[n][i + 1] - sq, rq = sq + d;
         if (rq < 0 || rq + len > m) continue;  // the segment does not fit at this shift (warp-uniform)
-        uint32_t e = 0, e_end = 0, tag = 0;
+        const uint32_t seg_code = segment_code(i);
+        uint32_t e = 0, e_end = 0;
         if (p_valid) {
             const unsigned long long h = seg_hash<W>(w.A, rq, len, n, i);
             const uint32_t b = (uint32_t)h & S.index.mask;
             e = __ldg(S.index.dir + b);
             e_end = __ldg(S.index.dir + b + 1);
-            tag = (uint32_t)(h >> 32);
         }
         if (COUNT) n_probes += (unsigned long long)__popc(__ballot_sync(kFullMask, p_valid));
         // The 32 buckets are walked as ONE list, 32 entries per step whatever their lengths: prefix sums of the bucket
@@ -456,13 +496,15 @@ __global__ void __launch_bounds__(kJoinThreads) k_join_probe(const __grid_consta
             }
             const uint32_t e_o = __shfl_sync(kFullMask, e, ow);
             const int first_o = __shfl_sync(kFullMask, first, ow);
-            const uint32_t tag_o = __shfl_sync(kFullMask, tag, ow);
+            const uint32_t sig_o = __shfl_sync(kFullMask, sig, ow);
             bool has = false;
             uint32_t t = 0;
             if (f < total) {
                 const uint2 cur = __ldg(S.index.entries + e_o + (uint32_t)(f - first_o));
-                // same bucket: only the texts after the pattern (every unordered pair once)
-                has = cur.x == tag_o && (delta > 0 || (int)cur.y > w.p0 + ow);
+                // composition bound (drops foreign keys of the bucket too: whatever passes is checked against the
+                // probe's segment later); same bucket: only the texts after the pattern (every unordered pair once)
+                has = (cur.x & kSegmentCodeMask) == seg_code && class_distance(sig_o, cur.x) <= sig_max &&
+                      (delta > 0 || (int)cur.y > w.p0 + ow);
                 t = cur.y;
             }
             const uint32_t bal = __ballot_sync(kFullMask, has);

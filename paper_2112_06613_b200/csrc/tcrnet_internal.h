@@ -128,7 +128,7 @@ struct JoinRow {
 };
 struct JoinIndex {
     const uint32_t* dir;  // [slots + 1]: entries of hash bucket b are [dir[b], dir[b+1])
-    const uint2* entries; // (tag = high half of the segment hash, sorted position of the text)
+    const uint2* entries; // (composition signature of the text, its sorted position)
     uint32_t mask;        // slots - 1 (a power of two)
 };
 // Bit-plane rows (pack.cu, read by segjoin.cu): sequence at sorted position s = 8 words of W (uint32_t when the set's
