@@ -341,6 +341,43 @@ def test_all_lengths_1_to_64_incl_wide_words(pkg, oracle):
         assert_same_network(got, want)
 
 
+@pytest.mark.parametrize("alphabet,lo,hi", [("AC", 4, 22), ("AIQY", 6, 40), ("ABCDEFGHIJKLMNOPQRSTUVWXYZ", 30, 64), ("A", 1, 64)])
+def test_low_complexity_sequences(pkg, oracle, alphabet, lo, hi):
+    """Repetitive strings over tiny alphabets (many diagonals match at once, the composition counts saturate, residues
+    of one class - A, I, Q, Y share code & 7 - and segments repeat inside a string), random strings over all 26 letters
+    up to 64 residues (64-bit planes), and runs of one letter: every threshold the join serves + one beyond it, against
+    the tier-0 oracle."""
+    rng = np.random.default_rng(len(alphabet) * 1000 + hi)
+    strings = []
+    for _ in range(500):
+        n = int(rng.integers(lo, hi + 1))
+        s = "".join(alphabet[i] for i in rng.integers(0, len(alphabet), n))
+        strings.append(s)
+        for _ in range(int(rng.integers(0, 4))):  # a few neighbours: up to 3 random edits
+            t = list(s)
+            for _ in range(int(rng.integers(1, 4))):
+                k = int(rng.integers(0, 3))
+                q = int(rng.integers(0, len(t)))
+                c = alphabet[int(rng.integers(0, len(alphabet)))]
+                if k == 0:
+                    t[q] = c
+                elif k == 1 and len(t) < 64:
+                    t.insert(q, c)
+                elif k == 2 and len(t) > 1:
+                    del t[q]
+            strings.append("".join(t))
+    strings = [strings[i] for i in rng.permutation(len(strings))]
+    res, ln = from_strings(strings)
+    for l_max in (0, 1, 2, 3, 4, 5):
+        want = oracle.network(res, ln, l_max, tier=0)[:3]
+        got, st = gpu_network(pkg, res, ln, l_max)
+        assert st["join_mode"] == 0 if l_max > 4 else (st["join_mode"] >= 1 or st["pairs_kept"] == 0)
+        assert_same_network(got, want)
+        if l_max in (1, 3):
+            got, _ = gpu_network(pkg, res, ln, l_max, {pkg.OPT_DEDUP: 0})
+            assert_same_network(got, want)
+
+
 def test_length_64_and_all_26_letters(pkg, oracle):
     rng = np.random.default_rng(5)
     letters = "ABCDEFGHIJKLMNOPQRSTUVWXYZ"
