@@ -8,6 +8,7 @@
 // HBM-bound: 8 B read + 4 B write per edge, 12 B written per node, plus one L2 atomic per edge.
 #include <algorithm>
 
+#include "launch.cuh"
 #include "tcrnet_internal.h"
 
 namespace tcrnet {
@@ -15,6 +16,7 @@ namespace {
 
 __global__ void __launch_bounds__(256) k_row_ptr(const unsigned long long* __restrict__ keys, int64_t n_edges,
                                                 int64_t n, int64_t* __restrict__ row_ptr) {
+    grid_dependency_wait();
     const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (r > n) return;
     const unsigned long long want = (unsigned long long)r << 32;
@@ -28,12 +30,14 @@ __global__ void __launch_bounds__(256) k_row_ptr(const unsigned long long* __res
 
 __global__ void __launch_bounds__(256) k_deg_upper(const int64_t* __restrict__ row_ptr, int64_t n,
                                                   int32_t* __restrict__ deg) {
+    grid_dependency_wait();
     const int64_t u = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (u < n) deg[u] = (int32_t)(row_ptr[u + 1] - row_ptr[u]);
 }
 
 __global__ void __launch_bounds__(256) k_col_deg_lower(const unsigned long long* __restrict__ keys, int64_t n_edges,
                                                       int32_t* __restrict__ col, int32_t* __restrict__ deg) {
+    grid_dependency_wait();
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_edges;
          e += (int64_t)gridDim.x * blockDim.x) {
         const uint32_t v = (uint32_t)keys[e];
@@ -61,6 +65,7 @@ constexpr int kSmemRow = 8192;   // longer rows up to this many: bitonic network
 
 __global__ void __launch_bounds__(256) k_count_rows(const unsigned long long* __restrict__ keys, int64_t n_keys,
                                                    int32_t* __restrict__ row_count, int32_t* __restrict__ deg) {
+    grid_dependency_wait();
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_keys; e += (int64_t)gridDim.x * blockDim.x) {
         const unsigned long long k = keys[e];
         atomicAdd(&row_count[k >> 32], 1);
@@ -72,6 +77,7 @@ __global__ void __launch_bounds__(256) k_count_rows(const unsigned long long* __
 __global__ void __launch_bounds__(256) k_scatter_keys(const unsigned long long* __restrict__ keys, int64_t n_keys,
                                                      const int64_t* __restrict__ row_ptr, int32_t* __restrict__ row_count,
                                                      unsigned long long* __restrict__ bucket) {
+    grid_dependency_wait();
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_keys; e += (int64_t)gridDim.x * blockDim.x) {
         const unsigned long long k = keys[e];
         const uint32_t u = (uint32_t)(k >> 32);
@@ -84,6 +90,7 @@ __global__ void __launch_bounds__(256) k_rank_rows(const unsigned long long* __r
                                                   const int64_t* __restrict__ row_ptr, int32_t* __restrict__ col,
                                                   int32_t* __restrict__ deg, int32_t* __restrict__ long_rows,
                                                   uint32_t* __restrict__ n_long) {
+    grid_dependency_wait();
     const int64_t pos = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (pos >= n_keys) return;
     const unsigned long long k = bucket[pos];
@@ -111,6 +118,7 @@ __global__ void __launch_bounds__(256) k_sort_long_rows(const int64_t* __restric
                                                        const unsigned long long* __restrict__ bucket,
                                                        int32_t* __restrict__ col, const int32_t* __restrict__ long_rows,
                                                        const uint32_t* __restrict__ n_long) {
+    grid_dependency_wait();
     __shared__ int32_t buf[kSmemRow];
     const uint32_t rows = *n_long;
     for (uint32_t r = blockIdx.x; r < rows; r += gridDim.x) {
@@ -153,7 +161,7 @@ cudaError_t launch_count_rows(const unsigned long long* keys, int64_t n_keys, in
                               cudaStream_t s, int* launches) {
     if (n_keys <= 0) return cudaSuccess;
     const int64_t blocks = std::min<int64_t>((n_keys + 255) / 256, device_sm_count() * 16);
-    k_count_rows<<<(unsigned)blocks, 256, 0, s>>>(keys, n_keys, row_count, deg);
+    launch_dep(k_count_rows, (unsigned)blocks, 256, 0, s, keys, n_keys, row_count, deg);
     *launches += 1;
     return cudaGetLastError();
 }
@@ -166,22 +174,22 @@ cudaError_t launch_csr_unsorted(const unsigned long long* keys, int64_t n_keys, 
     if (e == cudaSuccess) e = cudaMemsetAsync(n_long, 0, sizeof(uint32_t), s);
     if (e != cudaSuccess || n_keys <= 0) return e;
     const int64_t blocks = (n_keys + 255) / 256;
-    k_scatter_keys<<<(unsigned)std::min<int64_t>(blocks, device_sm_count() * 32), 256, 0, s>>>(keys, n_keys, row_ptr, row_count, bucket);
-    k_rank_rows<<<(unsigned)blocks, 256, 0, s>>>(bucket, n_keys, row_ptr, col, deg, long_rows, n_long);
-    k_sort_long_rows<<<(unsigned)std::min<int64_t>(n, device_sm_count() * 4), 256, 0, s>>>(row_ptr, bucket, col, long_rows, n_long);
+    launch_dep(k_scatter_keys, (unsigned)std::min<int64_t>(blocks, device_sm_count() * 32), 256, 0, s, keys, n_keys, row_ptr, row_count, bucket);
+    launch_dep(k_rank_rows, (unsigned)blocks, 256, 0, s, bucket, n_keys, row_ptr, col, deg, long_rows, n_long);
+    launch_dep(k_sort_long_rows, (unsigned)std::min<int64_t>(n, device_sm_count() * 4), 256, 0, s, row_ptr, bucket, col, long_rows, n_long);
     *launches += 3;
     return cudaGetLastError();
 }
 
 cudaError_t launch_csr(const unsigned long long* sorted_keys, int64_t n_edges, int64_t n, int64_t* row_ptr,
                        int32_t* col, int32_t* deg, cudaStream_t s, int* launches) {
-    k_row_ptr<<<(unsigned)((n + 1 + 255) / 256), 256, 0, s>>>(sorted_keys, n_edges, n, row_ptr);
-    k_deg_upper<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(row_ptr, n, deg);
+    launch_dep(k_row_ptr, (unsigned)((n + 1 + 255) / 256), 256, 0, s, sorted_keys, n_edges, n, row_ptr);
+    launch_dep(k_deg_upper, (unsigned)((n + 255) / 256), 256, 0, s, row_ptr, n, deg);
     *launches += 2;
     if (n_edges > 0) {
         int64_t blocks = (n_edges + 255) / 256;
         if (blocks > device_sm_count() * 16) blocks = device_sm_count() * 16;
-        k_col_deg_lower<<<(unsigned)blocks, 256, 0, s>>>(sorted_keys, n_edges, col, deg);
+        launch_dep(k_col_deg_lower, (unsigned)blocks, 256, 0, s, sorted_keys, n_edges, col, deg);
         *launches += 1;
     }
     return cudaGetLastError();

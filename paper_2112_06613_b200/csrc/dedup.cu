@@ -16,6 +16,7 @@
 //   scan + k_dedup_fill   the rows of every uid, contiguous (order inside a group is irrelevant)
 // Rows with an invalid length or out-of-range offset are never read and never merged; the pack step
 // reports them.  HBM/L2-bound: ~100 B per row over all kernels.
+#include "launch.cuh"
 #include "tcrnet_internal.h"
 
 namespace tcrnet {
@@ -49,6 +50,7 @@ __global__ void __launch_bounds__(256) k_dedup_insert(const uint8_t* __restrict_
                                                      const int32_t* __restrict__ lengths, int64_t n, int64_t total_len,
                                                      unsigned long long* __restrict__ table, uint32_t mask,
                                                      unsigned long long* __restrict__ hash) {
+    grid_dependency_wait();
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const int64_t off = offsets[i];
@@ -83,6 +85,7 @@ __global__ void __launch_bounds__(256) k_dedup_lookup(const uint8_t* __restrict_
                                                      const unsigned long long* __restrict__ table, uint32_t mask,
                                                      const unsigned long long* __restrict__ hash,
                                                      int32_t* __restrict__ rep_of, uint32_t* __restrict__ is_first) {
+    grid_dependency_wait();
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const unsigned long long h = hash[i];
@@ -119,6 +122,7 @@ __global__ void __launch_bounds__(256) k_dedup_groups(const int32_t* __restrict_
                                                      const int32_t* __restrict__ lengths, int64_t n,
                                                      int32_t* __restrict__ uid_of, uint32_t* __restrict__ group_count,
                                                      int32_t* __restrict__ len_u, int64_t* __restrict__ off_u) {
+    grid_dependency_wait();
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const int32_t rep = rep_of[i];
@@ -135,6 +139,7 @@ __global__ void __launch_bounds__(256) k_dedup_groups(const int32_t* __restrict_
 __global__ void __launch_bounds__(256) k_dedup_fill(const int32_t* __restrict__ uid_of, int64_t n,
                                                    const uint32_t* __restrict__ group_start,
                                                    uint32_t* __restrict__ group_count, int32_t* __restrict__ members) {
+    grid_dependency_wait();
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const uint32_t uid = (uint32_t)uid_of[i];
@@ -146,6 +151,7 @@ __global__ void __launch_bounds__(256) k_dedup_fill(const int32_t* __restrict__ 
 __global__ void __launch_bounds__(256) k_dedup_codes(int32_t* __restrict__ perm, int64_t n_u,
                                                     const uint32_t* __restrict__ group_start,
                                                     const int32_t* __restrict__ members) {
+    grid_dependency_wait();
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n_u) return;
     const uint32_t uid = (uint32_t)perm[s];
@@ -163,6 +169,7 @@ __global__ void __launch_bounds__(256) k_emit_cliques(const int32_t* __restrict_
                                                      unsigned long long* __restrict__ edge_count,
                                                      unsigned long long edge_cap, int32_t* __restrict__ row_count,
                                                      int32_t* __restrict__ deg, uint32_t shard, uint32_t n_shards) {
+    grid_dependency_wait();
     constexpr uint32_t kFullMask = 0xffffffffu;
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
@@ -213,6 +220,7 @@ __global__ void __launch_bounds__(256) k_expand_entries(const unsigned long long
                                                        unsigned long long edge_cap, int32_t* __restrict__ row_count,
                                                        int32_t* __restrict__ deg, ulonglong2* __restrict__ huge,
                                                        unsigned long long* __restrict__ n_huge, uint32_t huge_cap) {
+    grid_dependency_wait();
     constexpr uint32_t kFullMask = 0xffffffffu;
     constexpr unsigned long long kOwn = 8;
     constexpr unsigned long long kHuge = 4096;  // products beyond this are left to k_expand_huge (the whole grid)
@@ -293,6 +301,7 @@ __global__ void __launch_bounds__(256) k_expand_huge(const ulonglong2* __restric
                                                     const int32_t* __restrict__ members,
                                                     unsigned long long* __restrict__ edges, unsigned long long edge_cap,
                                                     int32_t* __restrict__ row_count, int32_t* __restrict__ deg) {
+    grid_dependency_wait();
     const unsigned long long cnt = min(*n_huge, (unsigned long long)huge_cap);
     const unsigned long long tid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
     const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
@@ -329,6 +338,7 @@ __global__ void __launch_bounds__(256) k_inverse_perm_groups(const int32_t* __re
                                                             const uint32_t* __restrict__ group_start,
                                                             const int32_t* __restrict__ members,
                                                             int32_t* __restrict__ inv) {
+    grid_dependency_wait();
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n_u) return;
     const uint32_t code = (uint32_t)perm[s];
@@ -355,8 +365,8 @@ cudaError_t launch_dedup_find(const uint8_t* residues, const int64_t* offsets, c
                               int32_t* rep_of, uint32_t* is_first, cudaStream_t s, int* launches) {
     cudaError_t e = cudaMemsetAsync(table, 0xff, sizeof(unsigned long long) * (size_t)slots, s);
     if (e != cudaSuccess) return e;
-    k_dedup_insert<<<grid_for(n), 256, 0, s>>>(residues, offsets, lengths, n, total_len, table, slots - 1u, hash);
-    k_dedup_lookup<<<grid_for(n), 256, 0, s>>>(residues, offsets, lengths, n, table, slots - 1u, hash, rep_of, is_first);
+    launch_dep(k_dedup_insert, grid_for(n), 256, 0, s, residues, offsets, lengths, n, total_len, table, slots - 1u, hash);
+    launch_dep(k_dedup_lookup, grid_for(n), 256, 0, s, residues, offsets, lengths, n, table, slots - 1u, hash, rep_of, is_first);
     *launches += 2;
     return cudaGetLastError();
 }
@@ -364,21 +374,21 @@ cudaError_t launch_dedup_find(const uint8_t* residues, const int64_t* offsets, c
 cudaError_t launch_dedup_groups(const int32_t* rep_of, const uint32_t* first_rank, const int64_t* offsets,
                                 const int32_t* lengths, int64_t n, int32_t* uid_of, uint32_t* group_count,
                                 int32_t* len_u, int64_t* off_u, cudaStream_t s, int* launches) {
-    k_dedup_groups<<<grid_for(n), 256, 0, s>>>(rep_of, first_rank, offsets, lengths, n, uid_of, group_count, len_u, off_u);
+    launch_dep(k_dedup_groups, grid_for(n), 256, 0, s, rep_of, first_rank, offsets, lengths, n, uid_of, group_count, len_u, off_u);
     *launches += 1;
     return cudaGetLastError();
 }
 
 cudaError_t launch_dedup_fill(const int32_t* uid_of, int64_t n, const uint32_t* group_start, uint32_t* group_count,
                               int32_t* members, cudaStream_t s, int* launches) {
-    k_dedup_fill<<<grid_for(n), 256, 0, s>>>(uid_of, n, group_start, group_count, members);
+    launch_dep(k_dedup_fill, grid_for(n), 256, 0, s, uid_of, n, group_start, group_count, members);
     *launches += 1;
     return cudaGetLastError();
 }
 
 cudaError_t launch_dedup_codes(int32_t* perm, int64_t n_u, const uint32_t* group_start, const int32_t* members,
                                cudaStream_t s, int* launches) {
-    k_dedup_codes<<<grid_for(n_u), 256, 0, s>>>(perm, n_u, group_start, members);
+    launch_dep(k_dedup_codes, grid_for(n_u), 256, 0, s, perm, n_u, group_start, members);
     *launches += 1;
     return cudaGetLastError();
 }
@@ -386,7 +396,7 @@ cudaError_t launch_dedup_codes(int32_t* perm, int64_t n_u, const uint32_t* group
 cudaError_t launch_emit_cliques(const int32_t* members, const int32_t* uid_of, const uint32_t* group_start, int64_t n,
                                 unsigned long long* edges, unsigned long long* edge_count, unsigned long long edge_cap,
                                 int32_t* row_count, int32_t* deg, int shard, int n_shards, cudaStream_t s, int* launches) {
-    k_emit_cliques<<<grid_for(n), 256, 0, s>>>(members, uid_of, group_start, n, edges, edge_count, edge_cap, row_count, deg,
+    launch_dep(k_emit_cliques, grid_for(n), 256, 0, s, members, uid_of, group_start, n, edges, edge_count, edge_cap, row_count, deg,
                                                (uint32_t)shard, (uint32_t)n_shards);
     *launches += 1;
     return cudaGetLastError();
@@ -397,10 +407,10 @@ cudaError_t launch_expand_entries(const unsigned long long* entries, const unsig
                                   unsigned long long* edges, unsigned long long* edge_total, unsigned long long edge_cap,
                                   int32_t* row_count, int32_t* deg, void* huge, unsigned long long* n_huge,
                                   uint32_t huge_cap, int n_sm, cudaStream_t s, int* launches) {
-    k_expand_entries<<<(unsigned)(n_sm * 8), 256, 0, s>>>(entries, n_entries_dev, entry_cap, group_start, members, edges,
+    launch_dep(k_expand_entries, (unsigned)(n_sm * 8), 256, 0, s, entries, n_entries_dev, entry_cap, group_start, members, edges,
                                                           edge_total, edge_cap, row_count, deg, (ulonglong2*)huge, n_huge,
                                                           huge_cap);
-    k_expand_huge<<<(unsigned)(n_sm * 8), 256, 0, s>>>((const ulonglong2*)huge, n_huge, huge_cap, group_start, members,
+    launch_dep(k_expand_huge, (unsigned)(n_sm * 8), 256, 0, s, (const ulonglong2*)huge, n_huge, huge_cap, group_start, members,
                                                        edges, edge_cap, row_count, deg);
     *launches += 2;
     return cudaGetLastError();
@@ -408,7 +418,7 @@ cudaError_t launch_expand_entries(const unsigned long long* entries, const unsig
 
 cudaError_t launch_inverse_perm_groups(const int32_t* perm, int64_t n_u, const uint32_t* group_start,
                                        const int32_t* members, int32_t* inv, cudaStream_t s, int* launches) {
-    k_inverse_perm_groups<<<grid_for(n_u), 256, 0, s>>>(perm, n_u, group_start, members, inv);
+    launch_dep(k_inverse_perm_groups, grid_for(n_u), 256, 0, s, perm, n_u, group_start, members, inv);
     *launches += 1;
     return cudaGetLastError();
 }

@@ -14,6 +14,7 @@
 //   planes : one row of 8 words per sorted position: plane k = bit k of the 5-bit code of every residue
 //         (north_star (1): 5-bit codes, here one bit of the code per word so that a residue-wise comparison of two
 //         sequences under any shift is five XORs) + the length - what the segment join reads (segjoin.cu).
+#include "launch.cuh"
 #include "tcrnet_internal.h"
 
 namespace tcrnet {
@@ -24,6 +25,7 @@ __global__ void __launch_bounds__(256) k_length_hist(const int32_t* __restrict__
                                                     const uint32_t* __restrict__ n_dev,
                                                     unsigned long long* __restrict__ hist,
                                                     uint32_t* __restrict__ flags) {
+    grid_dependency_wait();
     __shared__ uint32_t h[kNumLen];
     if (n_dev) n = min(n, (int64_t)*n_dev);
     for (int i = threadIdx.x; i < kNumLen; i += blockDim.x) h[i] = 0;
@@ -49,6 +51,7 @@ __global__ void __launch_bounds__(256) k_seq_keys(const uint8_t* __restrict__ re
                                                  const int64_t* __restrict__ offsets,
                                                  const int32_t* __restrict__ lengths, int64_t n,
                                                  unsigned long long* __restrict__ keys, int32_t* __restrict__ vals) {
+    grid_dependency_wait();
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     int32_t l = lengths[i];
@@ -79,6 +82,7 @@ __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residu
                                              const __grid_constant__ LengthTable lt, int pat_stride,
                                              uint8_t* __restrict__ pat, uint32_t* __restrict__ txt,
                                              W* __restrict__ planes, uint32_t* __restrict__ flags) {
+    grid_dependency_wait();
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;  // sorted position
     bool bad = false;
     if (s < n) {
@@ -143,6 +147,7 @@ __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residu
 // padded with kPadCode): written only when a build needs those kernels (tcrnet_api.cu: ensure_text_tables).
 __global__ void __launch_bounds__(256) k_txt_from_pat(const uint8_t* __restrict__ pat, int pat_stride, int64_t n,
                                                      const __grid_constant__ LengthTable lt, uint32_t* __restrict__ txt) {
+    grid_dependency_wait();
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
     int len = 0;
@@ -187,7 +192,7 @@ cudaError_t launch_length_hist(const int32_t* lengths, int64_t n, const uint32_t
                                uint32_t* flags, cudaStream_t s, int* launches) {
     int64_t blocks = (n + 255) / 256;
     if (blocks > device_sm_count() * 8) blocks = device_sm_count() * 8;
-    k_length_hist<<<(unsigned)blocks, 256, 0, s>>>(lengths, n, n_dev, hist, flags);
+    launch_dep(k_length_hist, (unsigned)blocks, 256, 0, s, lengths, n, n_dev, hist, flags);
     *launches += 1;
     return cudaGetLastError();
 }
@@ -195,7 +200,7 @@ cudaError_t launch_length_hist(const int32_t* lengths, int64_t n, const uint32_t
 cudaError_t launch_seq_keys(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths, int64_t n,
                             unsigned long long* keys, int32_t* vals, cudaStream_t s, int* launches) {
     if (n <= 0) return cudaSuccess;
-    k_seq_keys<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(residues, offsets, lengths, n, keys, vals);
+    launch_dep(k_seq_keys, (unsigned)((n + 255) / 256), 256, 0, s, residues, offsets, lengths, n, keys, vals);
     *launches += 1;
     return cudaGetLastError();
 }
@@ -205,11 +210,11 @@ cudaError_t launch_pack(const uint8_t* residues, const int64_t* offsets, const i
                         uint32_t* txt, void* planes, bool wide_planes, uint32_t* flags, cudaStream_t s, int* launches) {
     const unsigned blocks = (unsigned)((n + 255) / 256);
     if (wide_planes) {
-        if (txt) k_pack<uint64_t, true><<<blocks, 256, 0, s>>>(residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint64_t*)planes, flags);
-        else k_pack<uint64_t, false><<<blocks, 256, 0, s>>>(residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint64_t*)planes, flags);
+        if (txt) launch_dep(k_pack<uint64_t, true>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint64_t*)planes, flags);
+        else launch_dep(k_pack<uint64_t, false>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint64_t*)planes, flags);
     } else {
-        if (txt) k_pack<uint32_t, true><<<blocks, 256, 0, s>>>(residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint32_t*)planes, flags);
-        else k_pack<uint32_t, false><<<blocks, 256, 0, s>>>(residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint32_t*)planes, flags);
+        if (txt) launch_dep(k_pack<uint32_t, true>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint32_t*)planes, flags);
+        else launch_dep(k_pack<uint32_t, false>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint32_t*)planes, flags);
     }
     *launches += 1;
     return cudaGetLastError();
@@ -218,7 +223,7 @@ cudaError_t launch_pack(const uint8_t* residues, const int64_t* offsets, const i
 cudaError_t launch_txt_from_pat(const uint8_t* pat, int pat_stride, int64_t n, const LengthTable& lt, uint32_t* txt,
                                 cudaStream_t s, int* launches) {
     if (n <= 0) return cudaSuccess;
-    k_txt_from_pat<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(pat, pat_stride, n, lt, txt);
+    launch_dep(k_txt_from_pat, (unsigned)((n + 255) / 256), 256, 0, s, pat, pat_stride, n, lt, txt);
     *launches += 1;
     return cudaGetLastError();
 }

@@ -12,6 +12,7 @@
 //                    final slot.  Order inside a digit = input order, so every pass is stable.
 #include <utility>
 
+#include "launch.cuh"
 #include "tcrnet_internal.h"
 
 namespace tcrnet {
@@ -31,6 +32,7 @@ template <int kRounds>
 __global__ void __launch_bounds__(kThreads) k_radix_hist(const unsigned long long* __restrict__ keys, int64_t n,
                                                         int shift, uint32_t* __restrict__ hist,
                                                         uint32_t* __restrict__ totals, uint32_t tiles) {
+    grid_dependency_wait();
     constexpr int kTile = kThreads * kRounds;
     __shared__ uint32_t h[kDigits];
     for (int d = threadIdx.x; d < kDigits; d += kThreads) h[d] = 0;
@@ -52,6 +54,7 @@ __global__ void __launch_bounds__(kThreads) k_radix_hist(const unsigned long lon
 // Row d of hist (tiles entries) -> first output slot of (digit d, tile t), in place.
 __global__ void __launch_bounds__(kThreads) k_radix_scan(uint32_t* __restrict__ hist,
                                                         const uint32_t* __restrict__ totals, uint32_t tiles) {
+    grid_dependency_wait();
     __shared__ uint32_t wsum[kWarps];
     const uint32_t d = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // total of the smaller digits
@@ -94,6 +97,7 @@ __global__ void __launch_bounds__(kThreads) k_radix_scatter(const unsigned long 
                                                            const int32_t* __restrict__ vals_in,
                                                            int32_t* __restrict__ vals_out, int64_t n, int shift,
                                                            const uint32_t* __restrict__ scanned, uint32_t tiles) {
+    grid_dependency_wait();
     constexpr int kTile = kThreads * kRounds, kWarpItems = 32 * kRounds;
     __shared__ uint32_t wh[kWarps][kDigits];  // per warp: running digit counts, then first output slots
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -169,17 +173,17 @@ cudaError_t radix_sort_u64(unsigned long long* keys_a, unsigned long long* keys_
     const bool has_val = vals_a != nullptr;
     const bool small = rounds_for(n) == 4;
     for (int p = 0; p < n_passes; ++p) {
-        if (small) k_radix_hist<4><<<tiles, kThreads, 0, s>>>(keys_a, n, shifts[p], hist, totals + p * kDigits, tiles);
-        else k_radix_hist<16><<<tiles, kThreads, 0, s>>>(keys_a, n, shifts[p], hist, totals + p * kDigits, tiles);
-        k_radix_scan<<<kDigits, kThreads, 0, s>>>(hist, totals + p * kDigits, tiles);
+        if (small) launch_dep(k_radix_hist<4>, tiles, kThreads, 0, s, keys_a, n, shifts[p], hist, totals + p * kDigits, tiles);
+        else launch_dep(k_radix_hist<16>, tiles, kThreads, 0, s, keys_a, n, shifts[p], hist, totals + p * kDigits, tiles);
+        launch_dep(k_radix_scan, kDigits, kThreads, 0, s, hist, totals + p * kDigits, tiles);
         if (has_val && small)
-            k_radix_scatter<true, 4><<<tiles, kThreads, 0, s>>>(keys_a, keys_b, vals_a, vals_b, n, shifts[p], hist, tiles);
+            launch_dep(k_radix_scatter<true, 4>, tiles, kThreads, 0, s, keys_a, keys_b, vals_a, vals_b, n, shifts[p], hist, tiles);
         else if (has_val)
-            k_radix_scatter<true, 16><<<tiles, kThreads, 0, s>>>(keys_a, keys_b, vals_a, vals_b, n, shifts[p], hist, tiles);
+            launch_dep(k_radix_scatter<true, 16>, tiles, kThreads, 0, s, keys_a, keys_b, vals_a, vals_b, n, shifts[p], hist, tiles);
         else if (small)
-            k_radix_scatter<false, 4><<<tiles, kThreads, 0, s>>>(keys_a, keys_b, nullptr, nullptr, n, shifts[p], hist, tiles);
+            launch_dep(k_radix_scatter<false, 4>, tiles, kThreads, 0, s, keys_a, keys_b, nullptr, nullptr, n, shifts[p], hist, tiles);
         else
-            k_radix_scatter<false, 16><<<tiles, kThreads, 0, s>>>(keys_a, keys_b, nullptr, nullptr, n, shifts[p], hist, tiles);
+            launch_dep(k_radix_scatter<false, 16>, tiles, kThreads, 0, s, keys_a, keys_b, nullptr, nullptr, n, shifts[p], hist, tiles);
         *launches += 3;
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;

@@ -4,6 +4,7 @@
 // CTA adding up the sums of the tiles before it itself (<= 8 loads per thread): these scans are latency-bound,
 // so a launch less and four times as many CTAs matter more than the re-read sums.
 // HBM-bound streaming passes: 2 reads + 1 write of the array.
+#include "launch.cuh"
 #include "tcrnet_internal.h"
 
 namespace tcrnet {
@@ -46,6 +47,7 @@ __device__ __forceinline__ T block_exclusive(T v, T* warp_sums /*[32]*/, T* tota
 template <typename TIn, typename TOut, bool FUSED>
 __global__ void __launch_bounds__(kScanThreads) k_tile_sums(const TIn* __restrict__ in, int64_t n,
                                                            TOut* __restrict__ tile_sums) {
+    grid_dependency_wait();
     constexpr int kScanItems = scan_items(FUSED), kScanTile = kScanThreads * kScanItems;
     __shared__ TOut ws[32];
     __shared__ TOut tot;
@@ -63,6 +65,7 @@ __global__ void __launch_bounds__(kScanThreads) k_tile_sums(const TIn* __restric
 // One CTA scans the tile sums in place (exclusive), chunk by chunk with a carry.
 template <typename TOut>
 __global__ void __launch_bounds__(1024) k_scan_tile_sums(TOut* __restrict__ tile_sums, int64_t n_tiles) {
+    grid_dependency_wait();
     __shared__ TOut ws[32];
     __shared__ TOut tot;
     TOut carry = 0;
@@ -81,6 +84,7 @@ template <typename TIn, typename TOut, bool FUSED>
 __global__ void __launch_bounds__(kScanThreads) k_tile_scan(const TIn* __restrict__ in, TOut* __restrict__ out,
                                                            int64_t n, const TOut* __restrict__ tile_sums,
                                                            int write_total) {
+    grid_dependency_wait();
     constexpr int kScanItems = scan_items(FUSED), kScanTile = kScanThreads * kScanItems;
     __shared__ TOut ws[32];
     __shared__ TOut tot;
@@ -135,15 +139,15 @@ cudaError_t scan_impl(const TIn* in, TOut* out, int64_t n, bool write_total, voi
     const int64_t small_tile = kScanThreads * scan_items(true), big_tile = kScanThreads * scan_items(false);
     if ((n + small_tile - 1) / small_tile <= kFusedTiles) {
         const int64_t tiles = (n + small_tile - 1) / small_tile;
-        k_tile_sums<TIn, TOut, true><<<(unsigned)tiles, kScanThreads, 0, s>>>(in, n, sums);
-        k_tile_scan<TIn, TOut, true><<<(unsigned)tiles, kScanThreads, 0, s>>>(in, out, n, sums, write_total ? 1 : 0);
+        launch_dep(k_tile_sums<TIn, TOut, true>, (unsigned)tiles, kScanThreads, 0, s, in, n, sums);
+        launch_dep(k_tile_scan<TIn, TOut, true>, (unsigned)tiles, kScanThreads, 0, s, in, out, n, sums, write_total ? 1 : 0);
         *launches += 2;
         return cudaGetLastError();
     }
     const int64_t tiles = (n + big_tile - 1) / big_tile;
-    k_tile_sums<TIn, TOut, false><<<(unsigned)tiles, kScanThreads, 0, s>>>(in, n, sums);
-    k_scan_tile_sums<TOut><<<1, 1024, 0, s>>>(sums, tiles);
-    k_tile_scan<TIn, TOut, false><<<(unsigned)tiles, kScanThreads, 0, s>>>(in, out, n, sums, write_total ? 1 : 0);
+    launch_dep(k_tile_sums<TIn, TOut, false>, (unsigned)tiles, kScanThreads, 0, s, in, n, sums);
+    launch_dep(k_scan_tile_sums<TOut>, 1, 1024, 0, s, sums, tiles);
+    launch_dep(k_tile_scan<TIn, TOut, false>, (unsigned)tiles, kScanThreads, 0, s, in, out, n, sums, write_total ? 1 : 0);
     *launches += 3;
     return cudaGetLastError();
 }

@@ -39,6 +39,7 @@
 //           lane per survivor.
 #include <algorithm>
 
+#include "launch.cuh"
 #include "myers.cuh"
 
 namespace tcrnet {
@@ -300,6 +301,7 @@ __global__ void __launch_bounds__(256) k_join_index(const void* __restrict__ pla
                                                    const __grid_constant__ JoinTables tab, uint32_t* __restrict__ cnt,
                                                    const uint32_t* __restrict__ dir, uint2* __restrict__ entries,
                                                    uint32_t mask) {
+    grid_dependency_wait();
     const int k = tab.n_seg;
     const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t t = idx / k;
@@ -432,6 +434,7 @@ __device__ __forceinline__ void drain_round(ProbeWarp<W, L, COUNT>& w, const Joi
 // One warp = 32 consecutive patterns of one length x the texts longer by delta: every probe of that delta in turn.
 template <typename W, int L, bool COUNT>
 __global__ void __launch_bounds__(kJoinThreads) k_join_probe(const __grid_constant__ JoinParams S) {
+    grid_dependency_wait();
     __shared__ WarpBuf bufs[kJoinWarps];
     const DistanceParams& P = S.d;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -537,6 +540,7 @@ __global__ void __launch_bounds__(kJoinThreads) k_join_probe(const __grid_consta
 // ---- verify (l_max >= 2): one lane per surviving pair ----
 template <typename W, int L, bool COUNT>
 __global__ void __launch_bounds__(kJoinThreads) k_join_verify(const __grid_constant__ JoinParams S) {
+    grid_dependency_wait();
     const DistanceParams& P = S.d;
     const int lane = threadIdx.x & 31;
     const unsigned long long total = min(*S.cand_count, S.cand_cap);
@@ -582,14 +586,14 @@ __global__ void __launch_bounds__(kJoinThreads) k_join_verify(const __grid_const
 template <typename W, int L>
 cudaError_t launch_join_l(const JoinParams& S, bool count_work, int n_sm, cudaStream_t s, int* launches) {
     const unsigned blocks = (unsigned)((S.n_local + kJoinWarps - 1) / kJoinWarps);
-    if (count_work) k_join_probe<W, L, true><<<blocks, kJoinThreads, 0, s>>>(S);
-    else k_join_probe<W, L, false><<<blocks, kJoinThreads, 0, s>>>(S);
+    if (count_work) launch_dep(k_join_probe<W, L, true>, blocks, kJoinThreads, 0, s, S);
+    else launch_dep(k_join_probe<W, L, false>, blocks, kJoinThreads, 0, s, S);
     *launches += 1;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess || L <= 1) return e;
     const unsigned vblocks = (unsigned)(n_sm * 8);
-    if (count_work) k_join_verify<W, (L >= 2 ? L : 2), true><<<vblocks, kJoinThreads, 0, s>>>(S);
-    else k_join_verify<W, (L >= 2 ? L : 2), false><<<vblocks, kJoinThreads, 0, s>>>(S);
+    if (count_work) launch_dep(k_join_verify<W, (L >= 2 ? L : 2), true>, vblocks, kJoinThreads, 0, s, S);
+    else launch_dep(k_join_verify<W, (L >= 2 ? L : 2), false>, vblocks, kJoinThreads, 0, s, S);
     *launches += 1;
     return cudaGetLastError();
 }
@@ -615,15 +619,15 @@ cudaError_t launch_join_index(const void* planes, bool wide, const LengthTable& 
     const int64_t threads = n * tab.n_seg;
     if (threads <= 0) return cudaSuccess;
     const unsigned blocks = (unsigned)((threads + 255) / 256);
-    if (wide) k_join_index<uint64_t, false><<<blocks, 256, 0, s>>>(planes, n, tab, cnt, nullptr, nullptr, slots - 1u);
-    else k_join_index<uint32_t, false><<<blocks, 256, 0, s>>>(planes, n, tab, cnt, nullptr, nullptr, slots - 1u);
+    if (wide) launch_dep(k_join_index<uint64_t, false>, blocks, 256, 0, s, planes, n, tab, cnt, nullptr, nullptr, slots - 1u);
+    else launch_dep(k_join_index<uint32_t, false>, blocks, 256, 0, s, planes, n, tab, cnt, nullptr, nullptr, slots - 1u);
     *launches += 1;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     e = exclusive_scan_u32_total(cnt, dir, (int64_t)slots, scan_scratch, s, launches);
     if (e != cudaSuccess) return e;
-    if (wide) k_join_index<uint64_t, true><<<blocks, 256, 0, s>>>(planes, n, tab, cnt, dir, entries, slots - 1u);
-    else k_join_index<uint32_t, true><<<blocks, 256, 0, s>>>(planes, n, tab, cnt, dir, entries, slots - 1u);
+    if (wide) launch_dep(k_join_index<uint64_t, true>, blocks, 256, 0, s, planes, n, tab, cnt, dir, entries, slots - 1u);
+    else launch_dep(k_join_index<uint32_t, true>, blocks, 256, 0, s, planes, n, tab, cnt, dir, entries, slots - 1u);
     *launches += 1;
     return cudaGetLastError();
 }
