@@ -127,12 +127,17 @@ typedef enum tcrnet_option {
                                      sequences lexicographically inside their length buckets (the trie needs
                                      that), any other load sorts by length only; a build that needs the trie on
                                      a load sorted by length only falls back to the text-chunk kernel.        */
-    TCRNET_OPT_FAST_L1 = 12       /* 1: builds with l_max <= 1 go through the segment join
+    TCRNET_OPT_FAST_L1 = 12,      /* 1: builds with l_max <= 1 go through the segment join
                                      whatever TCRNET_OPT_SEGMENT_JOIN / TCRNET_OPT_PREFIX_TRIE say.  There the
                                      verification IS the textbook check - equal lengths: at most one mismatching
                                      residue (XOR of the packed codes); lengths differing by one: common prefix +
                                      common suffix cover the shorter sequence.  0 (default): no effect (the
                                      default path already takes the join).  Never changes the result.         */
+    TCRNET_OPT_TIMING = 13        /* CUDA events the library records on its stream for tcrnet_stats: 0 none; 1 (default)
+                                     around the distance kernels only (ms_kernel); 2 around every phase (ms_load,
+                                     ms_index, ms_distance, ms_csr, ms_build too; the fields not measured read 0).
+                                     An event between two short kernels costs 2-4 us and ends the programmatic
+                                     launch overlap there, so level 2 makes a config-4 step about 5 % slower.     */
 } tcrnet_option;
 
 /* Work and timing of the last tcrnet_load / tcrnet_build (tcrnet_get_stats). */

@@ -21,7 +21,7 @@ LIB_PATH = os.path.join(_HERE, "libtcrnet_b200.so")
 OK, ERR_ARG, ERR_LENGTH, ERR_RESIDUE, ERR_LMAX, ERR_STATE, ERR_NOMEM, ERR_EDGE_OVERFLOW, ERR_CUDA = (
     0, -1, -2, -3, -4, -5, -6, -7, -8)
 OPT_EARLY_EXIT, OPT_FIRST_CHECK, OPT_EDGE_CAPACITY, OPT_EDGE_LIMIT, OPT_COUNT_WORK, OPT_TEXT_CHUNK = 1, 2, 3, 4, 5, 6
-OPT_PREFIX_TRIE, OPT_TRIE_CHUNK, OPT_N_QUERY, OPT_DEDUP, OPT_SEGMENT_JOIN, OPT_FAST_L1 = 7, 8, 9, 10, 11, 12
+OPT_PREFIX_TRIE, OPT_TRIE_CHUNK, OPT_N_QUERY, OPT_DEDUP, OPT_SEGMENT_JOIN, OPT_FAST_L1, OPT_TIMING = 7, 8, 9, 10, 11, 12, 13
 
 EXPORTS = (
     "tcrnet_create", "tcrnet_destroy", "tcrnet_load", "tcrnet_load_device", "tcrnet_build", "tcrnet_csr",

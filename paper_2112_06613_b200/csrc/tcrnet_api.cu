@@ -42,6 +42,11 @@ void drop_observables(tcrnet_ctx* ctx) { ctx->have_hist = ctx->have_nn = ctx->ha
 namespace {
 
 HostCtrl* d_ctrl(tcrnet_ctx* ctx) { return static_cast<HostCtrl*>(ctx->ctrl.p); }
+// Timing events cost 2-4 us each between two short kernels (and end the programmatic launch chain there), so they are
+// recorded only at the level TCRNET_OPT_TIMING asks for: 1 = around the distance kernels, 2 = every phase.
+cudaError_t rec(tcrnet_ctx* ctx, int i, int level) {
+    return ctx->timing >= level ? cudaEventRecord(ctx->ev[i], ctx->stream) : cudaSuccess;
+}
 constexpr uint32_t kExpandHugeCap = 1u << 16;  // products set aside for k_expand_huge (beyond: expanded by their warp)
 
 int bits_for(int64_t max_value) {  // number of bits needed to represent max_value (>= 1)
@@ -553,15 +558,15 @@ int ensure_join_index(tcrnet_ctx* ctx, int l_max, int* launches) {
     TRY(dev_reserve(ctx, ctx->join_dir, sizeof(uint32_t) * ((size_t)slots + 1)));
     TRY(dev_reserve(ctx, ctx->join_entries, sizeof(uint2) * (size_t)std::max<int64_t>(n_idx, 1)));
     TRY(dev_reserve(ctx, ctx->scan_scratch, scan_scratch_bytes((int64_t)slots)));
-    TRY_CUDA(cudaEventRecord(ctx->ev[6], s));
+    TRY_CUDA(rec(ctx, 6, 2));
     TRY_CUDA(cudaMemsetAsync(ctx->join_cnt.p, 0, sizeof(uint32_t) * (size_t)slots, s));
     TRY_CUDA(launch_join_index(set.planes.p, set.wide_planes, set.lt, set.n, ctx->join_tab,
                                (uint32_t*)ctx->join_cnt.p, (uint32_t*)ctx->join_dir.p, (uint2*)ctx->join_entries.p, slots,
                                ctx->scan_scratch.p, s, launches));
-    TRY_CUDA(cudaEventRecord(ctx->ev[7], s));
+    TRY_CUDA(rec(ctx, 7, 2));
     ctx->join_slots = slots;
     ctx->join_l_max = l_max;
-    st.ms_index = -1.f;  // measured once the events have completed (distance_phase)
+    if (ctx->timing >= 2) st.ms_index = -1.f;  // measured once the events have completed (distance_phase)
     return TCRNET_OK;
 }
 
@@ -583,7 +588,7 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
     int n_queues = 0;
     const WorkRow* d_rows = (const WorkRow*)ctx->rows.p;
     const JoinRow* d_join_rows = (const JoinRow*)ctx->join_rows.p;
-    if (!expand_only) TRY_CUDA(cudaEventRecord(ctx->ev[4], s));
+    if (!expand_only) TRY_CUDA(rec(ctx, 4, 1));
     for (const Schedule::Pass& pass : sch.passes) {
         if (expand_only) break;
         DistanceParams p{};
@@ -636,7 +641,7 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
             d_join_rows += jr.size();
         }
     }
-    if (!expand_only) TRY_CUDA(cudaEventRecord(ctx->ev[5], s));
+    if (!expand_only) TRY_CUDA(rec(ctx, 5, 1));
     if (ctx->all.grouped) {
         // the recorded pairs of distinct sequences -> edges between rows (keys_b), counted for the CSR step; the rows
         // of every shared sequence are joined to each other (d = 0), each sequence by the shard uid mod n_shards
@@ -672,7 +677,7 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
     st.l_max = l_max;
     Schedule sch;
     make_schedule(ctx, l_max, first_check, sch, st);
-    TRY_CUDA(cudaEventRecord(ctx->ev[0], s));
+    TRY_CUDA(rec(ctx, 0, 2));
     TRY(upload_schedule(ctx, sch));
     st.ms_index = 0.f;
     st.join_index_entries = 0;
@@ -741,7 +746,8 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
         expand_only = true;
     }
     if (grouped) std::swap(ctx->keys_a, ctx->keys_b);  // the edges between rows are what the CSR step takes
-    TRY_CUDA(cudaEventElapsedTime(&st.ms_kernel, ctx->ev[4], ctx->ev[5]));  // of the last pass (both complete: synced)
+    st.ms_kernel = 0.f;
+    if (ctx->timing >= 1) TRY_CUDA(cudaEventElapsedTime(&st.ms_kernel, ctx->ev[4], ctx->ev[5]));  // of the last pass (both complete: synced)
     st.lane_columns_exec = (int64_t)ctx->h_ctrl->work[0];
     st.lane_tests_exec = (int64_t)ctx->h_ctrl->work[1];
     st.lane_pairs_exec = (int64_t)ctx->h_ctrl->work[2];
@@ -758,7 +764,7 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
         st.lane_columns_exec = st.lane_prefix_tests_exec = st.lane_columns_live = 0;
     }
     if (st.ms_index < 0.f) TRY_CUDA(cudaEventElapsedTime(&st.ms_index, ctx->ev[6], ctx->ev[7]));
-    TRY_CUDA(cudaEventRecord(ctx->ev[1], s));
+    TRY_CUDA(rec(ctx, 1, 2));
     ctx->n_keys = n_keys;
     return TCRNET_OK;
 }
@@ -783,15 +789,18 @@ int assemble_phase(tcrnet_ctx* ctx, int64_t n_keys, bool counts_ready, int* laun
         TRY_CUDA(launch_count_rows((const unsigned long long*)ctx->keys_a.p, n_keys, (int32_t*)ctx->row_count.p,
                                    (int32_t*)ctx->deg.p, s, launches));
     }
-    TRY_CUDA(cudaEventRecord(ctx->ev[2], s));
+    TRY_CUDA(rec(ctx, 2, 2));
     TRY_CUDA(launch_csr_unsorted((const unsigned long long*)ctx->keys_a.p, n_keys, n, (int32_t*)ctx->row_count.p,
                                  (int64_t*)ctx->row_ptr.p, (unsigned long long*)ctx->keys_b.p, (int32_t*)ctx->col.p,
                                  (int32_t*)ctx->deg.p, (int32_t*)ctx->long_rows.p, &dc->n_long, ctx->scan_scratch.p, s,
                                  launches));
-    TRY_CUDA(cudaEventRecord(ctx->ev[3], s));
-    TRY_CUDA(cudaEventSynchronize(ctx->ev[3]));
-    TRY_CUDA(cudaEventElapsedTime(&st.ms_sort, ctx->ev[1], ctx->ev[2]));
-    TRY_CUDA(cudaEventElapsedTime(&st.ms_csr, ctx->ev[2], ctx->ev[3]));
+    TRY_CUDA(rec(ctx, 3, 2));
+    TRY_CUDA(cudaStreamSynchronize(s));
+    st.ms_sort = st.ms_csr = 0.f;
+    if (ctx->timing >= 2) {
+        TRY_CUDA(cudaEventElapsedTime(&st.ms_sort, ctx->ev[1], ctx->ev[2]));
+        TRY_CUDA(cudaEventElapsedTime(&st.ms_csr, ctx->ev[2], ctx->ev[3]));
+    }
     st.n_edges = n_keys;
     ctx->n_edges = n_keys;
     ctx->have_keys = false;
@@ -904,11 +913,14 @@ int tcrnet_load_device(tcrnet_ctx* ctx, const uint8_t* residues_dev, const int32
     TRY_CUDA(cudaSetDevice(ctx->device));
     drop_load(ctx);
     int launches = 0;
-    TRY_CUDA(cudaEventRecord(ctx->ev[0], ctx->stream));
-    TRY(load_from_device(ctx, residues_dev, lengths_dev, n, total_len, &launches));
-    TRY_CUDA(cudaEventRecord(ctx->ev[1], ctx->stream));
-    TRY_CUDA(cudaEventSynchronize(ctx->ev[1]));
-    TRY_CUDA(cudaEventElapsedTime(&ctx->stats.ms_load, ctx->ev[0], ctx->ev[1]));
+    TRY_CUDA(rec(ctx, 0, 2));
+    TRY(load_from_device(ctx, residues_dev, lengths_dev, n, total_len, &launches));  // (ends synchronised)
+    ctx->stats.ms_load = 0.f;
+    if (ctx->timing >= 2) {
+        TRY_CUDA(cudaEventRecord(ctx->ev[1], ctx->stream));
+        TRY_CUDA(cudaEventSynchronize(ctx->ev[1]));
+        TRY_CUDA(cudaEventElapsedTime(&ctx->stats.ms_load, ctx->ev[0], ctx->ev[1]));
+    }
     ctx->stats.launches_load = launches;
     return TCRNET_OK;
 }
@@ -924,7 +936,7 @@ int tcrnet_load(tcrnet_ctx* ctx, const uint8_t* residues, const int32_t* lengths
     cudaStream_t s = ctx->stream;
     int rc = dev_reserve(ctx, d_len, sizeof(int32_t) * (size_t)n);
     if (rc != TCRNET_OK) return rc;
-    TRY_CUDA(cudaEventRecord(ctx->ev[0], s));
+    TRY_CUDA(rec(ctx, 0, 2));
     TRY_CUDA(cudaMemcpyAsync(d_len.p, lengths, sizeof(int32_t) * (size_t)n, cudaMemcpyHostToDevice, s));
     int64_t total_len = 0;
     uint32_t bad = 0;
@@ -950,9 +962,13 @@ int tcrnet_load(tcrnet_ctx* ctx, const uint8_t* residues, const int32_t* lengths
     if (rc == TCRNET_OK)
         rc = load_from_device(ctx, (const uint8_t*)d_res.p, (const int32_t*)d_len.p, n, total_len, &launches);
     if (rc == TCRNET_OK) {
-        cudaError_t e = cudaEventRecord(ctx->ev[1], ctx->stream);
-        if (e == cudaSuccess) e = cudaEventSynchronize(ctx->ev[1]);
-        if (e == cudaSuccess) e = cudaEventElapsedTime(&ctx->stats.ms_load, ctx->ev[0], ctx->ev[1]);
+        cudaError_t e = cudaSuccess;
+        ctx->stats.ms_load = 0.f;
+        if (ctx->timing >= 2) {
+            e = cudaEventRecord(ctx->ev[1], ctx->stream);
+            if (e == cudaSuccess) e = cudaEventSynchronize(ctx->ev[1]);
+            if (e == cudaSuccess) e = cudaEventElapsedTime(&ctx->stats.ms_load, ctx->ev[0], ctx->ev[1]);
+        }
         if (e != cudaSuccess) {
             ctx->last_cuda = (int)e;
             (void)cudaGetLastError();
@@ -975,8 +991,11 @@ int tcrnet_build(tcrnet_ctx* ctx, int l_max, int64_t* n_edges_out) {
     TRY(distance_phase(ctx, l_max, 0, 1, &launches));
     TRY(assemble_phase(ctx, ctx->n_keys, true, &launches));
     tcrnet_stats& st = ctx->stats;
-    TRY_CUDA(cudaEventElapsedTime(&st.ms_distance, ctx->ev[0], ctx->ev[1]));
-    TRY_CUDA(cudaEventElapsedTime(&st.ms_build, ctx->ev[0], ctx->ev[3]));
+    st.ms_distance = st.ms_build = 0.f;
+    if (ctx->timing >= 2) {
+        TRY_CUDA(cudaEventElapsedTime(&st.ms_distance, ctx->ev[0], ctx->ev[1]));
+        TRY_CUDA(cudaEventElapsedTime(&st.ms_build, ctx->ev[0], ctx->ev[3]));
+    }
     st.launches_build = launches;
     ctx->built_l_max = l_max;
     if (n_edges_out) *n_edges_out = ctx->n_edges;
@@ -993,8 +1012,11 @@ int tcrnet_build_shard(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, cons
     int launches = 0;
     TRY(distance_phase(ctx, l_max, shard, n_shards, &launches));
     tcrnet_stats& st = ctx->stats;
-    TRY_CUDA(cudaEventSynchronize(ctx->ev[1]));
-    TRY_CUDA(cudaEventElapsedTime(&st.ms_distance, ctx->ev[0], ctx->ev[1]));
+    st.ms_distance = 0.f;
+    if (ctx->timing >= 2) {
+        TRY_CUDA(cudaEventSynchronize(ctx->ev[1]));
+        TRY_CUDA(cudaEventElapsedTime(&st.ms_distance, ctx->ev[0], ctx->ev[1]));
+    }
     st.ms_sort = st.ms_csr = 0.f;
     st.ms_build = st.ms_distance;
     st.launches_build = launches;
@@ -1030,12 +1052,13 @@ int tcrnet_assemble(tcrnet_ctx* ctx, const uint64_t* keys_dev, int64_t n_keys, i
     TRY_CUDA(cudaMemsetAsync(&dc->flags, 0, sizeof(uint32_t), s));
     TRY_CUDA(launch_validate_keys((const unsigned long long*)ctx->keys_a.p, n_keys, ctx->n, &dc->flags, s, &launches));
     TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->flags, &dc->flags, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
-    TRY_CUDA(cudaEventRecord(ctx->ev[1], s));
+    TRY_CUDA(rec(ctx, 1, 2));
     TRY_CUDA(cudaStreamSynchronize(s));
     if (ctx->h_ctrl->flags) return TCRNET_ERR_ARG;
     TRY(assemble_phase(ctx, n_keys, false, &launches));
     ctx->stats.launches_build = launches;
-    TRY_CUDA(cudaEventElapsedTime(&ctx->stats.ms_build, ctx->ev[1], ctx->ev[3]));
+    ctx->stats.ms_build = 0.f;
+    if (ctx->timing >= 2) TRY_CUDA(cudaEventElapsedTime(&ctx->stats.ms_build, ctx->ev[1], ctx->ev[3]));
     if (n_edges_out) *n_edges_out = ctx->n_edges;
     return TCRNET_OK;
 }
@@ -1182,6 +1205,10 @@ int tcrnet_set_option(tcrnet_ctx* ctx, int option, int64_t value) {
         case TCRNET_OPT_FAST_L1:
             if (value != 0 && value != 1) return TCRNET_ERR_ARG;
             ctx->fast_l1 = (int)value;
+            return TCRNET_OK;
+        case TCRNET_OPT_TIMING:
+            if (value < 0 || value > 2) return TCRNET_ERR_ARG;
+            ctx->timing = (int)value;
             return TCRNET_OK;
         case TCRNET_OPT_TRIE_CHUNK:
             if (value < kTQ || value % kTQ != 0 || value > (1 << 24)) return TCRNET_ERR_ARG;
