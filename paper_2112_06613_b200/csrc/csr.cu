@@ -170,8 +170,8 @@ cudaError_t launch_csr_unsorted(const unsigned long long* keys, int64_t n_keys, 
                                 int64_t* row_ptr, unsigned long long* bucket, int32_t* col, int32_t* deg,
                                 int32_t* long_rows, uint32_t* n_long, void* scan_scratch, cudaStream_t s,
                                 int* launches) {
-    cudaError_t e = exclusive_scan_i32_to_i64(row_count, row_ptr, n, true, scan_scratch, s, launches);
-    if (e == cudaSuccess) e = cudaMemsetAsync(n_long, 0, sizeof(uint32_t), s);
+    cudaError_t e = cudaMemsetAsync(n_long, 0, sizeof(uint32_t), s);  // (ahead of the kernels: none sits between two)
+    if (e == cudaSuccess) e = exclusive_scan_i32_to_i64(row_count, row_ptr, n, true, scan_scratch, s, launches);
     if (e != cudaSuccess || n_keys <= 0) return e;
     const int64_t blocks = (n_keys + 255) / 256;
     launch_dep(k_scatter_keys, (unsigned)std::min<int64_t>(blocks, device_sm_count() * 32), 256, 0, s, keys, n_keys, row_ptr, row_count, bucket);

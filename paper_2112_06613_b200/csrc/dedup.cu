@@ -363,8 +363,7 @@ uint32_t dedup_table_slots(int64_t n) {
 cudaError_t launch_dedup_find(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths, int64_t n,
                               int64_t total_len, unsigned long long* table, uint32_t slots, unsigned long long* hash,
                               int32_t* rep_of, uint32_t* is_first, cudaStream_t s, int* launches) {
-    cudaError_t e = cudaMemsetAsync(table, 0xff, sizeof(unsigned long long) * (size_t)slots, s);
-    if (e != cudaSuccess) return e;
+    // (table is all ones: cleared by the caller, ahead of the kernels that precede this one)
     launch_dep(k_dedup_insert, grid_for(n), 256, 0, s, residues, offsets, lengths, n, total_len, table, slots - 1u, hash);
     launch_dep(k_dedup_lookup, grid_for(n), 256, 0, s, residues, offsets, lengths, n, table, slots - 1u, hash, rep_of, is_first);
     *launches += 2;

@@ -159,16 +159,20 @@ size_t radix_scratch_bytes(int64_t n) {
     return ((size_t)radix_tiles(n) * kDigits + (size_t)kRadixMaxPasses * kDigits) * sizeof(uint32_t);
 }
 
+cudaError_t radix_clear_totals(void* scratch, cudaStream_t s) {
+    return cudaMemsetAsync(scratch, 0, sizeof(uint32_t) * kRadixMaxPasses * kDigits, s);
+}
+
 cudaError_t radix_sort_u64(unsigned long long* keys_a, unsigned long long* keys_b, int32_t* vals_a, int32_t* vals_b,
                            int64_t n, const int* shifts, int n_passes, void* scratch, cudaStream_t s, int* launches,
-                           bool* result_in_b) {
+                           bool* result_in_b, bool totals_cleared) {
     *result_in_b = false;
     if (n <= 1 || n_passes <= 0) return cudaSuccess;
     if (n_passes > kRadixMaxPasses || n > 0x7fffffffLL) return cudaErrorInvalidValue;
     const uint32_t tiles = (uint32_t)radix_tiles(n);
     uint32_t* totals = (uint32_t*)scratch;                     // [kRadixMaxPasses][kDigits]
     uint32_t* hist = totals + kRadixMaxPasses * kDigits;       // [kDigits][tiles]
-    cudaError_t e = cudaMemsetAsync(totals, 0, sizeof(uint32_t) * kRadixMaxPasses * kDigits, s);
+    cudaError_t e = totals_cleared ? cudaSuccess : radix_clear_totals(scratch, s);
     if (e != cudaSuccess) return e;
     const bool has_val = vals_a != nullptr;
     const bool small = rounds_for(n) == 4;

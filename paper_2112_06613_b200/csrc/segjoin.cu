@@ -323,7 +323,7 @@ __global__ void __launch_bounds__(256) k_join_index(const void* __restrict__ pla
 // ---- probe ----
 struct JoinParams {
     DistanceParams d;  // emission, n_items, shard
-    const JoinRow* rows;
+    JoinRowDev rows[kJoinMaxRows];  // (in the parameter block: no upload, no global loads in the row search)
     int32_t n_rows;
     int32_t pad_;
     int64_t n_local;                // work items of this shard
@@ -336,11 +336,11 @@ struct JoinParams {
     JoinTables tab;
 };
 
-__device__ __forceinline__ const JoinRow& find_join_row(const JoinParams& S, int64_t item) {
+__device__ __forceinline__ const JoinRowDev& find_join_row(const JoinParams& S, int64_t item) {
     int lo = 0, hi = S.n_rows;
     while (hi - lo > 1) {
         const int mid = (lo + hi) >> 1;
-        if (S.rows[mid].item_begin <= item) lo = mid; else hi = mid;
+        if ((int64_t)S.rows[mid].item_begin <= item) lo = mid; else hi = mid;
     }
     return S.rows[lo];
 }
@@ -441,10 +441,10 @@ __global__ void __launch_bounds__(kJoinThreads) k_join_probe(const __grid_consta
     const int64_t local = (int64_t)blockIdx.x * kJoinWarps + warp;
     if (local >= S.n_local) return;  // the whole warp
     const int64_t item = local * P.n_shards + P.shard;
-    const JoinRow& Rw = find_join_row(S, item);
-    const int rel = (int)(item - Rw.item_begin);
+    const JoinRowDev& Rw = find_join_row(S, item);
+    const int rel = (int)(item - (int64_t)Rw.item_begin);
     const int tile = rel / (L + 1), delta = rel - tile * (L + 1);
-    if (Rw.t_count[delta] == 0) return;  // no texts of that length
+    if (!((Rw.t_mask >> delta) & 1u)) return;  // no texts of that length
     ProbeWarp<W, L, COUNT> w;
     w.wb = &bufs[warp];
     w.lane = lane;
@@ -639,7 +639,17 @@ cudaError_t launch_join(const DistanceParams& p, const JoinRow* rows, int n_rows
     if (p.n_items <= p.shard || n_rows <= 0) return cudaSuccess;
     JoinParams S{};
     S.d = p;
-    S.rows = rows;
+    if (n_rows > kJoinMaxRows || p.n_items > 0xffffffffLL) return cudaErrorInvalidValue;
+    for (int r = 0; r < n_rows; ++r) {  // rows: host memory
+        JoinRowDev& d = S.rows[r];
+        d.item_begin = (uint32_t)rows[r].item_begin;
+        d.p_start = rows[r].p_start;
+        d.p_count = rows[r].p_count;
+        d.m = (uint8_t)rows[r].m;
+        d.t_mask = 0;
+        for (int q = 0; q < kJoinMaxSeg; ++q)
+            if (rows[r].t_count[q] > 0) d.t_mask |= (uint8_t)(1u << q);
+    }
     S.n_rows = n_rows;
     S.planes = planes;
     S.index = index;

@@ -85,7 +85,8 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
     set.n_rows = n;
     cudaStream_t s = ctx->stream;
     HostCtrl* dc = d_ctrl(ctx);
-    TRY_CUDA(cudaMemsetAsync(dc, 0, sizeof(HostCtrl), s));
+    // (a collapsed load arrives with the histogram and a clean control block: dedup_rows returned on any flag)
+    if (!pre_hist) TRY_CUDA(cudaMemsetAsync(dc, 0, sizeof(HostCtrl), s));
     if (!pre_hist) {
         TRY_CUDA(launch_length_hist(d_len, n, nullptr, dc->hist, &dc->flags, s, launches));
         TRY_CUDA(cudaMemcpyAsync(ctx->h_ctrl, dc, sizeof(HostCtrl), cudaMemcpyDeviceToHost, s));
@@ -157,12 +158,13 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
         // an odd number of passes ends in the b buffers: make those set.perm
         int32_t* va = (int32_t*)(n_passes & 1 ? ctx->perm_tmp.p : set.perm.p);
         int32_t* vb = (int32_t*)(n_passes & 1 ? set.perm.p : ctx->perm_tmp.p);
+        if (e == cudaSuccess) e = radix_clear_totals(ctx->radix_scratch.p, s);
         if (e == cudaSuccess)
             e = launch_seq_keys(d_res, d_off, d_len, n, (unsigned long long*)ctx->keys_a.p, va, s, launches);
         bool in_b = false;
         if (e == cudaSuccess)
             e = radix_sort_u64((unsigned long long*)ctx->keys_a.p, (unsigned long long*)ctx->keys_b.p, va, vb, n, shifts,
-                               n_passes, ctx->radix_scratch.p, s, launches, &in_b);
+                               n_passes, ctx->radix_scratch.p, s, launches, &in_b, true);
         if (e == cudaSuccess && n > 1 && (in_b ? vb : va) != (int32_t*)set.perm.p) e = cudaErrorUnknown;
         if (e == cudaSuccess && n == 1)  // nothing was sorted: the payload sits in va
             e = cudaMemcpyAsync(set.perm.p, va, sizeof(int32_t), cudaMemcpyDeviceToDevice, s);
@@ -255,26 +257,27 @@ int dedup_rows(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t
     const int64_t* off = (const int64_t*)ctx->dd_offsets.p;
     uint32_t* rank = (uint32_t*)ctx->dd_rank.p;
     uint32_t* count = (uint32_t*)ctx->dd_count.p;
+    // every reset first and every read-back last: nothing but kernels in between, so that each of them is scheduled
+    // while its predecessor drains (launch.cuh)
     TRY_CUDA(cudaMemsetAsync(dc, 0, sizeof(HostCtrl), s));
+    TRY_CUDA(cudaMemsetAsync(ctx->dd_table.p, 0xff, sizeof(unsigned long long) * (size_t)slots, s));
+    TRY_CUDA(cudaMemsetAsync(count, 0, sizeof(uint32_t) * (size_t)(n + 1), s));
     TRY_CUDA(launch_length_hist(d_len, n, nullptr, dc->hist, &dc->flags, s, launches));  // of the ROWS (nominal work, validation)
     TRY_CUDA(exclusive_scan_i32_to_i64(d_len, (int64_t*)ctx->dd_offsets.p, n, true, ctx->scan_scratch.p, s, launches));
     TRY_CUDA(launch_dedup_find(d_res, off, d_len, n, total_len, (unsigned long long*)ctx->dd_table.p, slots,
                                (unsigned long long*)ctx->dd_hash.p, (int32_t*)ctx->dd_rep.p, (uint32_t*)ctx->dd_first.p, s,
                                launches));
     TRY_CUDA(exclusive_scan_u32_total((const uint32_t*)ctx->dd_first.p, rank, n, ctx->scan_scratch.p, s, launches));
-    TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->n_distinct, rank + n, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
-    TRY_CUDA(cudaMemsetAsync(count, 0, sizeof(uint32_t) * (size_t)(n + 1), s));
     TRY_CUDA(launch_dedup_groups((const int32_t*)ctx->dd_rep.p, rank, off, d_len, n, (int32_t*)set.uid_of.p, count,
                                  (int32_t*)ctx->dd_len.p, (int64_t*)ctx->dd_off.p, s, launches));
     // the length histogram of the distinct sequences, so that the pack needs no round trip of its own
     TRY_CUDA(launch_length_hist((const int32_t*)ctx->dd_len.p, n, rank + n, dc->hist_u, &dc->flags, s, launches));
-    TRY_CUDA(cudaMemcpyAsync(ctx->h_ctrl->hist, dc->hist, sizeof(dc->hist), cudaMemcpyDeviceToHost, s));
-    TRY_CUDA(cudaMemcpyAsync(ctx->h_ctrl->hist_u, dc->hist_u, sizeof(dc->hist_u), cudaMemcpyDeviceToHost, s));
-    TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->flags, &dc->flags, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
     // group_start over n + 1 counts (the tail is zero): entry n_u is the total = n
     TRY_CUDA(exclusive_scan_u32_total(count, (uint32_t*)set.group_start.p, n + 1, ctx->scan_scratch.p, s, launches));
     TRY_CUDA(launch_dedup_fill((const int32_t*)set.uid_of.p, n, (const uint32_t*)set.group_start.p, count,
                                (int32_t*)set.members.p, s, launches));
+    TRY_CUDA(cudaMemcpyAsync(ctx->h_ctrl, dc, sizeof(HostCtrl), cudaMemcpyDeviceToHost, s));  // hist, hist_u, flags
+    TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->n_distinct, rank + n, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
     TRY_CUDA(cudaStreamSynchronize(s));
     if (ctx->h_ctrl->flags & kFlagBadLength) return TCRNET_ERR_LENGTH;
     int64_t sum_len = 0;
@@ -526,17 +529,6 @@ int upload_schedule(tcrnet_ctx* ctx, const Schedule& sch) {
                                              ctx->stream));
                 dst += rows.size();
             }
-    if (sch.n_join_rows) {
-        TRY(dev_reserve(ctx, ctx->join_rows, sizeof(JoinRow) * sch.n_join_rows));
-        JoinRow* jdst = (JoinRow*)ctx->join_rows.p;
-        for (const Schedule::Pass& pass : sch.passes)
-            for (int wide = 0; wide < 2; ++wide) {
-                const std::vector<JoinRow>& rows = pass.join_rows[wide];
-                if (!rows.empty())
-                    TRY_CUDA(cudaMemcpyAsync(jdst, rows.data(), sizeof(JoinRow) * rows.size(), cudaMemcpyHostToDevice, ctx->stream));
-                jdst += rows.size();
-            }
-    }
     return TCRNET_OK;
 }
 
@@ -573,21 +565,36 @@ int ensure_join_index(tcrnet_ctx* ctx, int l_max, int* launches) {
 // cap: capacity of keys_a (the pairs the distance kernels record); cap_b: of keys_b (grouped loads only: the edges
 // between rows after the expansion).
 // expand_only: the recorded pairs in keys_a are complete, only keys_b was too small - redo the expansion alone.
-int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_check, uint64_t cap, uint64_t cap_b, int shard,
-                 int n_shards, bool expand_only, int* launches) {
+// The counters and per-row counts a distance pass starts from (issued ahead of the index kernels for the first pass,
+// so that no memset sits between two kernels of the chain index -> join -> cliques -> expansion).
+int reset_build_counters(tcrnet_ctx* ctx, bool expand_only) {
     cudaStream_t s = ctx->stream;
     HostCtrl* dc = d_ctrl(ctx);
     static_assert(offsetof(HostCtrl, queue) == offsetof(HostCtrl, edge_count) + 9 * sizeof(unsigned long long), "one memset");
     static_assert(offsetof(HostCtrl, edge_total) == offsetof(HostCtrl, queue) + kTrieQueues * sizeof(unsigned long long), "one memset");
     static_assert(offsetof(HostCtrl, cand_count) == offsetof(HostCtrl, edge_total) + sizeof(unsigned long long), "one memset");
-    if (expand_only) TRY_CUDA(cudaMemsetAsync(&dc->edge_total, 0, sizeof(unsigned long long), s));
-    else TRY_CUDA(cudaMemsetAsync(&dc->edge_count, 0, sizeof(unsigned long long) * (11 + kTrieQueues), s));  // edge_count, work[8], queue[], edge_total, cand_count
-    TRY_CUDA(cudaMemsetAsync(&dc->n_huge, 0, sizeof(unsigned long long), s));
+    static_assert(offsetof(HostCtrl, n_huge) == offsetof(HostCtrl, cand_count) + sizeof(unsigned long long), "one memset");
+    if (expand_only) {
+        TRY_CUDA(cudaMemsetAsync(&dc->edge_total, 0, sizeof(unsigned long long), s));
+        TRY_CUDA(cudaMemsetAsync(&dc->n_huge, 0, sizeof(unsigned long long), s));
+    } else {  // edge_count, work[8], queue[], edge_total, cand_count, n_huge
+        TRY_CUDA(cudaMemsetAsync(&dc->edge_count, 0, sizeof(unsigned long long) * (12 + kTrieQueues), s));
+    }
     TRY_CUDA(cudaMemsetAsync(ctx->row_count.p, 0, sizeof(int32_t) * (size_t)ctx->n, s));
     TRY_CUDA(cudaMemsetAsync(ctx->deg.p, 0, sizeof(int32_t) * (size_t)ctx->n, s));
+    return TCRNET_OK;
+}
+
+int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_check, uint64_t cap, uint64_t cap_b, int shard,
+                 int n_shards, bool expand_only, bool counters_cleared, int* launches) {
+    cudaStream_t s = ctx->stream;
+    HostCtrl* dc = d_ctrl(ctx);
+    static_assert(offsetof(HostCtrl, queue) == offsetof(HostCtrl, edge_count) + 9 * sizeof(unsigned long long), "one memset");
+    static_assert(offsetof(HostCtrl, edge_total) == offsetof(HostCtrl, queue) + kTrieQueues * sizeof(unsigned long long), "one memset");
+    static_assert(offsetof(HostCtrl, cand_count) == offsetof(HostCtrl, edge_total) + sizeof(unsigned long long), "one memset");
+    if (!counters_cleared) TRY(reset_build_counters(ctx, expand_only));
     int n_queues = 0;
     const WorkRow* d_rows = (const WorkRow*)ctx->rows.p;
-    const JoinRow* d_join_rows = (const JoinRow*)ctx->join_rows.p;
     if (!expand_only) TRY_CUDA(rec(ctx, 4, 1));
     for (const Schedule::Pass& pass : sch.passes) {
         if (expand_only) break;
@@ -633,12 +640,11 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
             if (!jr.empty()) {
                 p.n_items = pass.join_items[wide];
                 JoinIndex index{(const uint32_t*)ctx->join_dir.p, (const uint2*)ctx->join_entries.p, ctx->join_slots - 1u};
-                TRY_CUDA(launch_join(p, d_join_rows, (int)jr.size(), pass.pset->planes.p, pass.pset->wide_planes, index,
+                TRY_CUDA(launch_join(p, jr.data(), (int)jr.size(), pass.pset->planes.p, pass.pset->wide_planes, index,
                                      ctx->join_tab, (uint2*)ctx->join_cand.p,
                                      (uint8_t*)ctx->join_cand.p + sizeof(uint2) * (size_t)ctx->join_cand_cap, &dc->cand_count,
                                      (unsigned long long)ctx->join_cand_cap, ctx->count_work != 0, ctx->n_sm, s, launches));
             }
-            d_join_rows += jr.size();
         }
     }
     if (!expand_only) TRY_CUDA(rec(ctx, 5, 1));
@@ -679,6 +685,25 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
     make_schedule(ctx, l_max, first_check, sch, st);
     TRY_CUDA(rec(ctx, 0, 2));
     TRY(upload_schedule(ctx, sch));
+    // distances + emission (second pass only if the edge buffer was too small)
+    int64_t cap = ctx->edge_capacity_opt > 0 ? ctx->edge_capacity_opt : std::max<int64_t>((int64_t)1 << 20, 16 * n);
+    cap = std::min(cap, ctx->edge_limit);
+    cap = std::max<int64_t>(cap, 1);
+    if (ctx->keys_a.p && (int64_t)(ctx->keys_a.bytes / 8) > cap) cap = std::min<int64_t>(ctx->keys_a.bytes / 8, ctx->edge_limit);
+    TRY(dev_reserve(ctx, ctx->keys_a, sizeof(unsigned long long) * (size_t)cap));
+    TRY(dev_reserve(ctx, ctx->row_count, sizeof(int32_t) * (size_t)n));
+    TRY(dev_reserve(ctx, ctx->deg, sizeof(int32_t) * (size_t)n));
+    const bool grouped = ctx->all.grouped;
+    int64_t cap_b = 0;
+    if (grouped) TRY(dev_reserve(ctx, ctx->expand_huge, 16 * (size_t)kExpandHugeCap));
+    if (grouped) {
+        cap_b = std::max<int64_t>(cap, (int64_t)(ctx->keys_b.bytes / 8));
+        cap_b = std::min(cap_b, ctx->edge_limit);
+        TRY(dev_reserve(ctx, ctx->keys_b, sizeof(unsigned long long) * (size_t)cap_b));
+    }
+    // the first pass's resets go ahead of the index kernels: index -> join -> cliques -> expansion is one chain of kernels
+    TRY(reset_build_counters(ctx, false));
+    bool counters_cleared = true;
     st.ms_index = 0.f;
     st.join_index_entries = 0;
     if (sch.n_join_rows) {
@@ -701,27 +726,13 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
     }
     st.trie_nodes = ctx->all.trie_nodes;
 
-    // distances + emission (second pass only if the edge buffer was too small)
-    int64_t cap = ctx->edge_capacity_opt > 0 ? ctx->edge_capacity_opt : std::max<int64_t>((int64_t)1 << 20, 16 * n);
-    cap = std::min(cap, ctx->edge_limit);
-    cap = std::max<int64_t>(cap, 1);
-    if (ctx->keys_a.p && (int64_t)(ctx->keys_a.bytes / 8) > cap) cap = std::min<int64_t>(ctx->keys_a.bytes / 8, ctx->edge_limit);
-    TRY(dev_reserve(ctx, ctx->keys_a, sizeof(unsigned long long) * (size_t)cap));
-    TRY(dev_reserve(ctx, ctx->row_count, sizeof(int32_t) * (size_t)n));
-    TRY(dev_reserve(ctx, ctx->deg, sizeof(int32_t) * (size_t)n));
-    const bool grouped = ctx->all.grouped;
-    int64_t cap_b = 0;
-    if (grouped) TRY(dev_reserve(ctx, ctx->expand_huge, 16 * (size_t)kExpandHugeCap));
-    if (grouped) {
-        cap_b = std::max<int64_t>(cap, (int64_t)(ctx->keys_b.bytes / 8));
-        cap_b = std::min(cap_b, ctx->edge_limit);
-        TRY(dev_reserve(ctx, ctx->keys_b, sizeof(unsigned long long) * (size_t)cap_b));
-    }
     int64_t n_keys = 0;
     st.distance_passes = 0;
     for (bool expand_only = false;;) {
         if (!expand_only) ++st.distance_passes;
-        TRY(run_distance(ctx, sch, l_max, first_check, (uint64_t)cap, (uint64_t)cap_b, shard, n_shards, expand_only, launches));
+        TRY(run_distance(ctx, sch, l_max, first_check, (uint64_t)cap, (uint64_t)cap_b, shard, n_shards, expand_only,
+                         counters_cleared, launches));
+        counters_cleared = false;
         const int64_t n_rec = (int64_t)ctx->h_ctrl->edge_count;  // pairs recorded by the distance kernels
         const int64_t n_cand = (int64_t)ctx->h_ctrl->cand_count;
         if (!expand_only && n_cand > ctx->join_cand_cap) {

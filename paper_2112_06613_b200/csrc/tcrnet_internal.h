@@ -126,6 +126,14 @@ struct JoinRow {
     int32_t t_start[kJoinMaxSeg];
     int32_t t_count[kJoinMaxSeg];
 };
+// ... as the kernel sees it (passed in the parameter block)
+constexpr int kJoinMaxRows = kMaxLen;
+struct JoinRowDev {
+    uint32_t item_begin;
+    int32_t p_start, p_count;
+    uint8_t m, t_mask;  // t_mask bit delta: texts of length m + delta exist
+    uint16_t pad_;
+};
 struct JoinIndex {
     const uint32_t* dir;  // [slots + 1]: entries of hash bucket b are [dir[b], dir[b+1])
     const uint2* entries; // (composition signature of the text, its sorted position)
@@ -159,7 +167,10 @@ constexpr int kRadixBits = 9;
 size_t radix_scratch_bytes(int64_t n);
 cudaError_t radix_sort_u64(unsigned long long* keys_a, unsigned long long* keys_b, int32_t* vals_a, int32_t* vals_b,
                            int64_t n, const int* shifts, int n_passes, void* scratch, cudaStream_t s, int* launches,
-                           bool* result_in_b);
+                           bool* result_in_b, bool totals_cleared = false);
+// the digit totals at the head of `scratch` have to be zero when the sort starts: radix_sort_u64 clears them itself
+// unless the caller did (ahead of the kernels that produce the keys, so that no memset sits between two kernels)
+cudaError_t radix_clear_totals(void* scratch, cudaStream_t s);
 
 // pack.cu
 // n_dev (may be NULL): device count of rows, at most n
@@ -236,7 +247,7 @@ cudaError_t launch_join_index(const void* planes, bool wide, const LengthTable& 
                               uint32_t* cnt, uint32_t* dir, uint2* entries, uint32_t slots, void* scan_scratch,
                               cudaStream_t s, int* launches);
 // Probe + filter (+ verification and emission for l_max <= 1); for l_max >= 2 the surviving pairs go to `cand`
-// (at most cand_cap of the *cand_count counted) and a second kernel verifies them (Landau-Vishkin on the mismatch
+// (at most cand_cap of the *cand_count counted; `rows` is HOST memory) and a second kernel verifies them (Landau-Vishkin on the mismatch
 // masks of the band's diagonals) and emits.  p carries the emission fields, n_items and the shard of the launch.
 cudaError_t launch_join(const DistanceParams& p, const JoinRow* rows, int n_rows, const void* planes, bool wide,
                         const JoinIndex& index, const JoinTables& tab, uint2* cand, uint8_t* cand_probe,
