@@ -45,38 +45,51 @@ __device__ __forceinline__ uint32_t start_slot(unsigned long long fp, uint32_t m
     return (uint32_t)(((fp >> 32) * 0x9E3779B97F4A7C15ull) >> 32) & mask;
 }
 
+// Also the length histogram of the ROWS and their validation (what k_length_hist does for a load without collapse):
+// the lengths are read here anyway.
 __global__ void __launch_bounds__(256) k_dedup_insert(const uint8_t* __restrict__ residues,
                                                      const int64_t* __restrict__ offsets,
                                                      const int32_t* __restrict__ lengths, int64_t n, int64_t total_len,
                                                      unsigned long long* __restrict__ table, uint32_t mask,
-                                                     unsigned long long* __restrict__ hash) {
+                                                     unsigned long long* __restrict__ hash,
+                                                     unsigned long long* __restrict__ hist, uint32_t* __restrict__ flags) {
     grid_dependency_wait();
+    __shared__ uint32_t h[kNumLen];
+    for (int k = threadIdx.x; k < kNumLen; k += blockDim.x) h[k] = 0;
+    __syncthreads();
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const int64_t off = offsets[i];
-    const int32_t len = lengths[i];
-    if (!row_ok(off, len, total_len)) {
-        hash[i] = kEmptySlot;  // never merged
-        return;
-    }
-    unsigned long long h = hash_row(residues + off, len);
-    if (h == kEmptySlot) h = 0;
-    hash[i] = h;
-    const unsigned long long fp = h & 0xffffffff00000000ull;
-    const unsigned long long mine = fp | (unsigned long long)i;
-    uint32_t s = start_slot(fp, mask);
-    for (;;) {
-        unsigned long long cur = table[s];
-        if (cur == kEmptySlot) {
-            cur = atomicCAS(&table[s], kEmptySlot, mine);
-            if (cur == kEmptySlot) return;
+    bool bad = false;
+    if (i < n) {
+        const int64_t off = offsets[i];
+        const int32_t len = lengths[i];
+        bad = len < 1 || len > kMaxLen;
+        atomicAdd(&h[bad ? 0 : len], 1u);
+        if (!row_ok(off, len, total_len)) {
+            hash[i] = kEmptySlot;  // never merged
+        } else {
+            unsigned long long hv = hash_row(residues + off, len);
+            if (hv == kEmptySlot) hv = 0;
+            hash[i] = hv;
+            const unsigned long long fp = hv & 0xffffffff00000000ull;
+            const unsigned long long mine = fp | (unsigned long long)i;
+            uint32_t s = start_slot(fp, mask);
+            for (;;) {
+                unsigned long long cur = table[s];
+                if (cur == kEmptySlot) {
+                    cur = atomicCAS(&table[s], kEmptySlot, mine);
+                    if (cur == kEmptySlot) break;
+                }
+                if ((cur & 0xffffffff00000000ull) == fp) {
+                    atomicMin(&table[s], mine);
+                    break;
+                }
+                s = (s + 1u) & mask;
+            }
         }
-        if ((cur & 0xffffffff00000000ull) == fp) {
-            atomicMin(&table[s], mine);
-            return;
-        }
-        s = (s + 1u) & mask;
     }
+    if (__syncthreads_or(bad) && threadIdx.x == 0) atomicOr(flags, kFlagBadLength);
+    for (int k = threadIdx.x; k < kNumLen; k += blockDim.x)
+        if (h[k]) atomicAdd(&hist[k], (unsigned long long)h[k]);
 }
 
 __global__ void __launch_bounds__(256) k_dedup_lookup(const uint8_t* __restrict__ residues,
@@ -121,18 +134,28 @@ __global__ void __launch_bounds__(256) k_dedup_groups(const int32_t* __restrict_
                                                      const int64_t* __restrict__ offsets,
                                                      const int32_t* __restrict__ lengths, int64_t n,
                                                      int32_t* __restrict__ uid_of, uint32_t* __restrict__ group_count,
-                                                     int32_t* __restrict__ len_u, int64_t* __restrict__ off_u) {
+                                                     int32_t* __restrict__ len_u, int64_t* __restrict__ off_u,
+                                                     unsigned long long* __restrict__ hist_u) {
     grid_dependency_wait();
+    __shared__ uint32_t h[kNumLen];  // length histogram of the distinct sequences (their first rows)
+    for (int k = threadIdx.x; k < kNumLen; k += blockDim.x) h[k] = 0;
+    __syncthreads();
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const int32_t rep = rep_of[i];
-    const uint32_t uid = first_rank[rep];
-    uid_of[i] = (int32_t)uid;
-    atomicAdd(&group_count[uid], 1u);
-    if (rep == i) {
-        len_u[uid] = lengths[i];
-        off_u[uid] = offsets[i];
+    if (i < n) {
+        const int32_t rep = rep_of[i];
+        const uint32_t uid = first_rank[rep];
+        uid_of[i] = (int32_t)uid;
+        atomicAdd(&group_count[uid], 1u);
+        if (rep == i) {
+            const int32_t len = lengths[i];
+            len_u[uid] = len;
+            off_u[uid] = offsets[i];
+            atomicAdd(&h[(len < 1 || len > kMaxLen) ? 0 : len], 1u);
+        }
     }
+    __syncthreads();
+    for (int k = threadIdx.x; k < kNumLen; k += blockDim.x)
+        if (h[k]) atomicAdd(&hist_u[k], (unsigned long long)h[k]);
 }
 
 // group_count[uid] counts down to 0 while the rows take their places
@@ -362,9 +385,10 @@ uint32_t dedup_table_slots(int64_t n) {
 
 cudaError_t launch_dedup_find(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths, int64_t n,
                               int64_t total_len, unsigned long long* table, uint32_t slots, unsigned long long* hash,
-                              int32_t* rep_of, uint32_t* is_first, cudaStream_t s, int* launches) {
+                              int32_t* rep_of, uint32_t* is_first, unsigned long long* hist, uint32_t* flags,
+                              cudaStream_t s, int* launches) {
     // (table is all ones: cleared by the caller, ahead of the kernels that precede this one)
-    launch_dep(k_dedup_insert, grid_for(n), 256, 0, s, residues, offsets, lengths, n, total_len, table, slots - 1u, hash);
+    launch_dep(k_dedup_insert, grid_for(n), 256, 0, s, residues, offsets, lengths, n, total_len, table, slots - 1u, hash, hist, flags);
     launch_dep(k_dedup_lookup, grid_for(n), 256, 0, s, residues, offsets, lengths, n, table, slots - 1u, hash, rep_of, is_first);
     *launches += 2;
     return cudaGetLastError();
@@ -372,8 +396,9 @@ cudaError_t launch_dedup_find(const uint8_t* residues, const int64_t* offsets, c
 
 cudaError_t launch_dedup_groups(const int32_t* rep_of, const uint32_t* first_rank, const int64_t* offsets,
                                 const int32_t* lengths, int64_t n, int32_t* uid_of, uint32_t* group_count,
-                                int32_t* len_u, int64_t* off_u, cudaStream_t s, int* launches) {
-    launch_dep(k_dedup_groups, grid_for(n), 256, 0, s, rep_of, first_rank, offsets, lengths, n, uid_of, group_count, len_u, off_u);
+                                int32_t* len_u, int64_t* off_u, unsigned long long* hist_u, cudaStream_t s,
+                                int* launches) {
+    launch_dep(k_dedup_groups, grid_for(n), 256, 0, s, rep_of, first_rank, offsets, lengths, n, uid_of, group_count, len_u, off_u, hist_u);
     *launches += 1;
     return cudaGetLastError();
 }

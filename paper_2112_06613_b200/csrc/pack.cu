@@ -78,10 +78,12 @@ template <typename W, bool TXT>
 __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residues,
                                              const int64_t* __restrict__ offsets,
                                              const int32_t* __restrict__ lengths,
-                                             const int32_t* __restrict__ perm, int64_t n,
+                                             int32_t* __restrict__ perm, int64_t n,
                                              const __grid_constant__ LengthTable lt, int pat_stride,
                                              uint8_t* __restrict__ pat, uint32_t* __restrict__ txt,
-                                             W* __restrict__ planes, uint32_t* __restrict__ flags) {
+                                             W* __restrict__ planes, uint32_t* __restrict__ flags,
+                                             const uint32_t* __restrict__ group_start,
+                                             const int32_t* __restrict__ members) {
     grid_dependency_wait();
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;  // sorted position
     bool bad = false;
@@ -138,6 +140,12 @@ __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residu
             r2[1] = make_ulonglong2((unsigned long long)pl[2], (unsigned long long)pl[3]);
             r2[2] = make_ulonglong2((unsigned long long)pl[4], (unsigned long long)len);
             r2[3] = make_ulonglong2(0ull, 0ull);
+        }
+        // collapsed load (dedup.cu): the rows were the distinct sequences and perm[s] their uid; it now becomes the row
+        // itself for a sequence that one row has, kGroupFlag | uid for a shared one
+        if (group_start) {
+            const uint32_t b = group_start[o];
+            perm[s] = group_start[o + 1] - b == 1u ? members[b] : (int32_t)(kGroupFlag | (uint32_t)o);
         }
     }
     if (__syncthreads_or(bad) && threadIdx.x == 0) atomicOr(flags, kFlagBadResidue);
@@ -206,15 +214,16 @@ cudaError_t launch_seq_keys(const uint8_t* residues, const int64_t* offsets, con
 }
 
 cudaError_t launch_pack(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths,
-                        const int32_t* perm, int64_t n, const LengthTable& lt, int pat_stride, uint8_t* pat,
-                        uint32_t* txt, void* planes, bool wide_planes, uint32_t* flags, cudaStream_t s, int* launches) {
+                        int32_t* perm, int64_t n, const LengthTable& lt, int pat_stride, uint8_t* pat,
+                        uint32_t* txt, void* planes, bool wide_planes, uint32_t* flags, const uint32_t* group_start,
+                        const int32_t* members, cudaStream_t s, int* launches) {
     const unsigned blocks = (unsigned)((n + 255) / 256);
     if (wide_planes) {
-        if (txt) launch_dep(k_pack<uint64_t, true>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint64_t*)planes, flags);
-        else launch_dep(k_pack<uint64_t, false>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint64_t*)planes, flags);
+        if (txt) launch_dep(k_pack<uint64_t, true>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint64_t*)planes, flags, group_start, members);
+        else launch_dep(k_pack<uint64_t, false>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint64_t*)planes, flags, group_start, members);
     } else {
-        if (txt) launch_dep(k_pack<uint32_t, true>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint32_t*)planes, flags);
-        else launch_dep(k_pack<uint32_t, false>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint32_t*)planes, flags);
+        if (txt) launch_dep(k_pack<uint32_t, true>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint32_t*)planes, flags, group_start, members);
+        else launch_dep(k_pack<uint32_t, false>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint32_t*)planes, flags, group_start, members);
     }
     *launches += 1;
     return cudaGetLastError();

@@ -171,14 +171,12 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
         set.lexicographic = lexicographic;
     }
     if (e == cudaSuccess)
-        e = launch_pack(d_res, d_off, d_len, (const int32_t*)set.perm.p, n, lt, set.pat_stride,
-                        (uint8_t*)set.pat.p, nullptr, set.planes.p, set.wide_planes, &dc->flags, s, launches);
+        e = launch_pack(d_res, d_off, d_len, (int32_t*)set.perm.p, n, lt, set.pat_stride,
+                        (uint8_t*)set.pat.p, nullptr, set.planes.p, set.wide_planes, &dc->flags,
+                        code_groups ? (const uint32_t*)set.group_start.p : nullptr,
+                        code_groups ? (const int32_t*)set.members.p : nullptr, s, launches);
     // (the text rows and the prefix trie are built by ensure_text_tables when a build needs them)
-    // collapsed load: the rows were the distinct sequences; perm (position -> uid) has served the pack and now
-    // becomes position -> row, or kGroupFlag | uid of a shared sequence
-    if (rc == TCRNET_OK && e == cudaSuccess && code_groups)
-        e = launch_dedup_codes((int32_t*)set.perm.p, n, (const uint32_t*)set.group_start.p, (const int32_t*)set.members.p, s,
-                               launches);
+    // (collapsed load: the pack kernel has re-coded perm from uids to rows / kGroupFlag | uid)
     if (rc == TCRNET_OK && e == cudaSuccess)
         e = cudaMemcpyAsync(&ctx->h_ctrl->flags, &dc->flags,
                             sizeof(HostCtrl) - offsetof(HostCtrl, flags), cudaMemcpyDeviceToHost, s);
@@ -262,16 +260,15 @@ int dedup_rows(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t
     TRY_CUDA(cudaMemsetAsync(dc, 0, sizeof(HostCtrl), s));
     TRY_CUDA(cudaMemsetAsync(ctx->dd_table.p, 0xff, sizeof(unsigned long long) * (size_t)slots, s));
     TRY_CUDA(cudaMemsetAsync(count, 0, sizeof(uint32_t) * (size_t)(n + 1), s));
-    TRY_CUDA(launch_length_hist(d_len, n, nullptr, dc->hist, &dc->flags, s, launches));  // of the ROWS (nominal work, validation)
     TRY_CUDA(exclusive_scan_i32_to_i64(d_len, (int64_t*)ctx->dd_offsets.p, n, true, ctx->scan_scratch.p, s, launches));
+    // (the insert kernel also takes the length histogram of the ROWS - nominal work - and validates the lengths)
     TRY_CUDA(launch_dedup_find(d_res, off, d_len, n, total_len, (unsigned long long*)ctx->dd_table.p, slots,
-                               (unsigned long long*)ctx->dd_hash.p, (int32_t*)ctx->dd_rep.p, (uint32_t*)ctx->dd_first.p, s,
-                               launches));
+                               (unsigned long long*)ctx->dd_hash.p, (int32_t*)ctx->dd_rep.p, (uint32_t*)ctx->dd_first.p,
+                               dc->hist, &dc->flags, s, launches));
     TRY_CUDA(exclusive_scan_u32_total((const uint32_t*)ctx->dd_first.p, rank, n, ctx->scan_scratch.p, s, launches));
     TRY_CUDA(launch_dedup_groups((const int32_t*)ctx->dd_rep.p, rank, off, d_len, n, (int32_t*)set.uid_of.p, count,
-                                 (int32_t*)ctx->dd_len.p, (int64_t*)ctx->dd_off.p, s, launches));
-    // the length histogram of the distinct sequences, so that the pack needs no round trip of its own
-    TRY_CUDA(launch_length_hist((const int32_t*)ctx->dd_len.p, n, rank + n, dc->hist_u, &dc->flags, s, launches));
+                                 (int32_t*)ctx->dd_len.p, (int64_t*)ctx->dd_off.p, dc->hist_u, s, launches));
+    // (... and the groups kernel the length histogram of the distinct sequences: the pack needs no round trip of its own)
     // group_start over n + 1 counts (the tail is zero): entry n_u is the total = n
     TRY_CUDA(exclusive_scan_u32_total(count, (uint32_t*)set.group_start.p, n + 1, ctx->scan_scratch.p, s, launches));
     TRY_CUDA(launch_dedup_fill((const int32_t*)set.uid_of.p, n, (const uint32_t*)set.group_start.p, count,

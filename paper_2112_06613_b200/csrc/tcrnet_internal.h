@@ -180,10 +180,12 @@ cudaError_t launch_length_hist(const int32_t* lengths, int64_t n, const uint32_t
 constexpr int kSeqKeyBits = 6 + 5 * kSortPrefix;  // length - 1 (0..63) takes 6 bits
 cudaError_t launch_seq_keys(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths, int64_t n,
                             unsigned long long* keys, int32_t* vals, cudaStream_t s, int* launches);
+// group_start != NULL (collapsed load): perm holds uids on entry and is re-coded in place (the row of an unshared
+// sequence, or kGroupFlag | uid)
 cudaError_t launch_pack(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths,
-                        const int32_t* perm, int64_t n, const LengthTable& lt, int pat_stride,
+                        int32_t* perm, int64_t n, const LengthTable& lt, int pat_stride,
                         uint8_t* pat, uint32_t* txt /*NULL: not written*/, void* planes, bool wide_planes, uint32_t* flags,
-                        cudaStream_t s, int* launches);
+                        const uint32_t* group_start, const int32_t* members, cudaStream_t s, int* launches);
 // txt rows (trie / text-chunk kernels) from the pattern rows, on demand
 cudaError_t launch_txt_from_pat(const uint8_t* pat, int pat_stride, int64_t n, const LengthTable& lt, uint32_t* txt,
                                 cudaStream_t s, int* launches);
@@ -204,12 +206,15 @@ cudaError_t launch_trie_build(const uint32_t* txt, const LengthTable& lt, int64_
 // dedup.cu: identical sequences collapse before the pack (see the file header for the steps)
 uint32_t dedup_table_slots(int64_t n);
 cudaError_t launch_dedup_find(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths, int64_t n,
-                              int64_t total_len, unsigned long long* table, uint32_t slots, unsigned long long* hash,
-                              int32_t* rep_of, uint32_t* is_first, cudaStream_t s, int* launches);
+                              int64_t total_len, unsigned long long* table /*all ones*/, uint32_t slots,
+                              unsigned long long* hash, int32_t* rep_of, uint32_t* is_first,
+                              unsigned long long* hist /*[kNumLen], += lengths of the rows*/, uint32_t* flags,
+                              cudaStream_t s, int* launches);
 // first_rank = exclusive scan of is_first; group_count zeroed by the caller
 cudaError_t launch_dedup_groups(const int32_t* rep_of, const uint32_t* first_rank, const int64_t* offsets,
                                 const int32_t* lengths, int64_t n, int32_t* uid_of, uint32_t* group_count,
-                                int32_t* len_u, int64_t* off_u, cudaStream_t s, int* launches);
+                                int32_t* len_u, int64_t* off_u, unsigned long long* hist_u /*[kNumLen], += lengths of
+                                the distinct sequences*/, cudaStream_t s, int* launches);
 // group_start = exclusive scan of group_count (n_u + 1 entries); group_count is consumed
 cudaError_t launch_dedup_fill(const int32_t* uid_of, int64_t n, const uint32_t* group_start, uint32_t* group_count,
                               int32_t* members, cudaStream_t s, int* launches);
