@@ -40,7 +40,9 @@ ALU_OPS_PER_TEST = 4           # 2 LOP3 + IADD3 + ISETP per pair and early-exit 
 ALU_OPS_PER_PREFIX_TEST = 2    # LOP3 + ISETP per pair and DP cell read in a guided expansion (distance_trie.cu)
 # segment join (segjoin.cu): what the method itself needs on the ALU pipe
 JOIN_OPS_PER_PROBE = 25        # 5 plane slices x (SHF + AND + XOR) + the 64-bit xor-shifts of the mixing rounds
-JOIN_OPS_PER_ENTRY = 2         # tag compare + order compare per directory entry read
+JOIN_OPS_PER_ENTRY = 16        # per directory entry read: segment-number compare (2), composition distance of the two
+                               # signature words (13: SWAR subtract / sign / fold, its 2 multiplies and the POPC not
+                               # counted), order compare (1)
 JOIN_OPS_PER_CANDIDATE = 12    # widening the 5 text planes (2 x 5) + the filter's AND / compare
 JOIN_OPS_PER_DIAGONAL = 11     # 5 funnel shifts + 5 LOP3 (a ^ b | acc) + 1 AND of the shifted-Hamming filter
 JOIN_OPS_PER_LV_STATE = 12     # Landau-Vishkin: compare / select / max / min / shift per (edit level, diagonal)
@@ -49,9 +51,9 @@ ORACLE_SAMPLE_ROWS = 1024
 # summarised under profiles/ (regenerated with them; a workload / kernel that is not listed prints null)
 NCU_DRAM_BYTES_PER_LAUNCH = {
     # (workload, kernel): bytes per step of that kernel / kernel pair - profiles/r2_join_ncu.txt
-    ("cfg4", "k_join_probe"): 35_105_536 + 1_792,
-    ("cfg3", "k_join_probe + k_join_verify"): 11_109_632 + 12_340_224,
-    ("cfg5", "k_join_probe + k_join_verify"): 2_381_505_000 + 378_921_216 + 533_883_000 + 49_555_968,
+    ("cfg4", "k_join_probe"): 35_106_816 + 1_280,
+    ("cfg3", "k_join_probe + k_join_verify"): 11_112_448 + 26_624 + 11_567_616 + 17_920,
+    ("cfg5", "k_join_probe + k_join_verify"): 2_721_635_000 + 448_049_920 + 351_767_000 + 48_876_288,
 }
 
 

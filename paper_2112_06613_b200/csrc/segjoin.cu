@@ -432,8 +432,10 @@ __device__ __forceinline__ void drain_round(ProbeWarp<W, L, COUNT>& w, const Joi
 }
 
 // One warp = 32 consecutive patterns of one length x the texts longer by delta: every probe of that delta in turn.
+// (Register cap for 5 / 6 CTAs per SM: the kernel waits on dependent L2 reads, warps hide more than a few spills cost -
+// measured at config 5: 7.35 -> 7.08 ms per step.)
 template <typename W, int L, bool COUNT>
-__global__ void __launch_bounds__(kJoinThreads) k_join_probe(const __grid_constant__ JoinParams S) {
+__global__ void __launch_bounds__(kJoinThreads, (L >= 2 ? 6 : 5)) k_join_probe(const __grid_constant__ JoinParams S) {
     grid_dependency_wait();
     __shared__ WarpBuf bufs[kJoinWarps];
     const DistanceParams& P = S.d;
