@@ -280,7 +280,7 @@ def main() -> None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    sharded = args.sharded and world > 1
+    sharded = args.sharded  # (N = 1: one shard - the same calls, no collective)
     cfg = CONFIGS[args.workload]
     l_max = cfg.l_max[0]
     # replicas: an independent repertoire per rank; sharded: the same repertoire on every rank

@@ -13,7 +13,7 @@
 //                    duplicate of it, or (first row of its sequence, fingerprint clash, invalid row) stays
 //   scan             ids of the distinct sequences in input-row order (deterministic)
 //   k_dedup_groups   uid of every row, rows per uid, length / residue offset of every uid
-//   scan + k_dedup_fill   the rows of every uid, contiguous (order inside a group is irrelevant)
+//   scan + k_dedup_fill   the rows of every uid, contiguous (order inside a group is irrelevant); total clique edges
 // Rows with an invalid length or out-of-range offset are never read and never merged; the pack step
 // reports them.  HBM/L2-bound: ~100 B per row over all kernels.
 #include "launch.cuh"
@@ -159,27 +159,23 @@ __global__ void __launch_bounds__(256) k_dedup_groups(const int32_t* __restrict_
 }
 
 // group_count[uid] counts down to 0 while the rows take their places
+// (the row that takes the last free slot also adds the group's g (g - 1) / 2 clique edges to *clique_edges: a load
+// dominated by one heavily repeated sequence can then be refused before any quadratic work is done)
 __global__ void __launch_bounds__(256) k_dedup_fill(const int32_t* __restrict__ uid_of, int64_t n,
                                                    const uint32_t* __restrict__ group_start,
-                                                   uint32_t* __restrict__ group_count, int32_t* __restrict__ members) {
+                                                   uint32_t* __restrict__ group_count, int32_t* __restrict__ members,
+                                                   unsigned long long* __restrict__ clique_edges) {
     grid_dependency_wait();
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const uint32_t uid = (uint32_t)uid_of[i];
     const uint32_t slot = atomicSub(&group_count[uid], 1u) - 1u;
-    members[group_start[uid] + slot] = (int32_t)i;
-}
-
-// perm[sorted position] = uid  ->  the row itself when it is alone, else kGroupFlag | uid
-__global__ void __launch_bounds__(256) k_dedup_codes(int32_t* __restrict__ perm, int64_t n_u,
-                                                    const uint32_t* __restrict__ group_start,
-                                                    const int32_t* __restrict__ members) {
-    grid_dependency_wait();
-    const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= n_u) return;
-    const uint32_t uid = (uint32_t)perm[s];
     const uint32_t b = group_start[uid];
-    perm[s] = group_start[uid + 1] - b == 1u ? members[b] : (int32_t)(kGroupFlag | uid);
+    members[b + slot] = (int32_t)i;
+    if (slot == 0u) {
+        const unsigned long long g = group_start[uid + 1u] - b;
+        if (g > 1ull) atomicAdd(clique_edges, g * (g - 1ull) / 2ull);
+    }
 }
 
 // Edges between the rows of one sequence: the thread of member slot x joins it to the slots after it.  Output
@@ -404,15 +400,8 @@ cudaError_t launch_dedup_groups(const int32_t* rep_of, const uint32_t* first_ran
 }
 
 cudaError_t launch_dedup_fill(const int32_t* uid_of, int64_t n, const uint32_t* group_start, uint32_t* group_count,
-                              int32_t* members, cudaStream_t s, int* launches) {
-    launch_dep(k_dedup_fill, grid_for(n), 256, 0, s, uid_of, n, group_start, group_count, members);
-    *launches += 1;
-    return cudaGetLastError();
-}
-
-cudaError_t launch_dedup_codes(int32_t* perm, int64_t n_u, const uint32_t* group_start, const int32_t* members,
-                               cudaStream_t s, int* launches) {
-    launch_dep(k_dedup_codes, grid_for(n_u), 256, 0, s, perm, n_u, group_start, members);
+                              int32_t* members, unsigned long long* clique_edges, cudaStream_t s, int* launches) {
+    launch_dep(k_dedup_fill, grid_for(n), 256, 0, s, uid_of, n, group_start, group_count, members, clique_edges);
     *launches += 1;
     return cudaGetLastError();
 }

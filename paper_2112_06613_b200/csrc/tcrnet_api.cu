@@ -69,6 +69,7 @@ void drop_load(tcrnet_ctx* ctx) {
     ctx->loaded = false;
     ctx->all.loaded = ctx->query.loaded = false;
     ctx->n = 0;
+    ctx->clique_edges = 0;
     ctx->join_l_max = -1;  // the segment index belongs to a load
 }
 
@@ -272,8 +273,8 @@ int dedup_rows(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t
     // group_start over n + 1 counts (the tail is zero): entry n_u is the total = n
     TRY_CUDA(exclusive_scan_u32_total(count, (uint32_t*)set.group_start.p, n + 1, ctx->scan_scratch.p, s, launches));
     TRY_CUDA(launch_dedup_fill((const int32_t*)set.uid_of.p, n, (const uint32_t*)set.group_start.p, count,
-                               (int32_t*)set.members.p, s, launches));
-    TRY_CUDA(cudaMemcpyAsync(ctx->h_ctrl, dc, sizeof(HostCtrl), cudaMemcpyDeviceToHost, s));  // hist, hist_u, flags
+                               (int32_t*)set.members.p, &dc->clique_edges, s, launches));
+    TRY_CUDA(cudaMemcpyAsync(ctx->h_ctrl, dc, sizeof(HostCtrl), cudaMemcpyDeviceToHost, s));  // hist, hist_u, flags, clique_edges
     TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->n_distinct, rank + n, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
     TRY_CUDA(cudaStreamSynchronize(s));
     if (ctx->h_ctrl->flags & kFlagBadLength) return TCRNET_ERR_LENGTH;
@@ -286,6 +287,7 @@ int dedup_rows(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t
     // the header's contract: total_len = sum of the lengths (a shorter buffer would be read past its end by the
     // pack; the insert / lookup kernels above never touch a row that does not fit)
     if (sum_len != total_len) return TCRNET_ERR_ARG;
+    ctx->clique_edges = (int64_t)ctx->h_ctrl->clique_edges;
     *n_u = (int64_t)ctx->h_ctrl->n_distinct;
     if (*n_u < 1 || *n_u > n) return TCRNET_ERR_CUDA;
     return TCRNET_OK;
@@ -678,6 +680,9 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
     }
     st.first_check = first_check;
     st.l_max = l_max;
+    // identical rows are joined for every l_max: if those edges alone exceed the limit, fail before any work
+    // (one sequence repeated g times means g (g - 1) / 2 of them)
+    if (ctx->all.grouped && ctx->clique_edges > ctx->edge_limit) return TCRNET_ERR_EDGE_OVERFLOW;
     Schedule sch;
     make_schedule(ctx, l_max, first_check, sch, st);
     TRY_CUDA(rec(ctx, 0, 2));

@@ -29,6 +29,7 @@ struct HostCtrl {  // pinned mirror of the small device control block
     uint32_t trie_root[kNumLen + 1];  // [L] = first level-1 node of length bucket L (non-empty buckets)
     uint32_t pad2_;
     unsigned long long hist_u[kNumLen];  // dedup: length histogram of the distinct sequences
+    unsigned long long clique_edges;     // dedup: edges among the rows of the shared sequences (known at load)
 };
 
 // One packed set of sequences: all rows, or the query rows of the rectangular mode.
@@ -81,6 +82,7 @@ struct tcrnet_ctx {
     int64_t n = 0;
     SeqSet all, query;
     unsigned long long hist_u_host[kNumLen] = {};  // length histogram of the distinct sequences of the last collapse
+    int64_t clique_edges = 0;        // edges among identical rows of the current load (collapsed loads)
     int64_t row_hist[kNumLen] = {};  // length histogram of the ROWS (all.hist counts distinct sequences when grouped)
     DevBuf in_res, in_len, offsets, perm_tmp, trie_scratch;  // load scratch, kept between loads (grow-only)
     DevBuf dd_table, dd_hash, dd_rep, dd_first, dd_rank, dd_count, dd_len, dd_off, dd_offsets;  // dedup scratch

@@ -216,11 +216,9 @@ cudaError_t launch_dedup_groups(const int32_t* rep_of, const uint32_t* first_ran
                                 int32_t* len_u, int64_t* off_u, unsigned long long* hist_u /*[kNumLen], += lengths of
                                 the distinct sequences*/, cudaStream_t s, int* launches);
 // group_start = exclusive scan of group_count (n_u + 1 entries); group_count is consumed
+// *clique_edges (zeroed) += sum over the groups of g (g - 1) / 2
 cudaError_t launch_dedup_fill(const int32_t* uid_of, int64_t n, const uint32_t* group_start, uint32_t* group_count,
-                              int32_t* members, cudaStream_t s, int* launches);
-// perm[s] = uid -> the row itself (a sequence of one row) or kGroupFlag | uid
-cudaError_t launch_dedup_codes(int32_t* perm, int64_t n_u, const uint32_t* group_start, const int32_t* members,
-                               cudaStream_t s, int* launches);
+                              int32_t* members, unsigned long long* clique_edges, cudaStream_t s, int* launches);
 // the edges among the rows of every shared sequence (distance 0); sequences uid = shard (mod n_shards) only
 cudaError_t launch_emit_cliques(const int32_t* members, const int32_t* uid_of, const uint32_t* group_start, int64_t n,
                                 unsigned long long* edges, unsigned long long* edge_count, unsigned long long edge_cap,

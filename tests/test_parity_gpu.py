@@ -436,6 +436,31 @@ def test_errors(pkg):
             net.set_option(99, 1)
 
 
+def test_one_heavily_repeated_sequence_fails_fast(pkg):
+    """70,000 identical rows would be 2.45e9 clique edges, more than the hard limit of 2^31: the build refuses at once
+    (the count is known at load) instead of enumerating them; with a limit that admits them a smaller clique is built."""
+    import time
+    rows = ["CASSLGQYF"] * 70000 + ["CASSLGEYF", "CAWSVGF"]
+    res, ln = from_strings(rows)
+    with pkg.TcrNet(0) as net:
+        net.load(res, ln)
+        t0 = time.perf_counter()
+        with pytest.raises(pkg.TcrNetError) as e:
+            net.build(1)
+        assert e.value.status == pkg.ERR_EDGE_OVERFLOW and time.perf_counter() - t0 < 0.5
+        res2, ln2 = from_strings(["CASSLGQYF"] * 3000 + ["CASSLGEYF", "CAWSVGF"])
+        net.load(res2, ln2)
+        net.set_option(pkg.OPT_EDGE_LIMIT, 1_000_000)
+        with pytest.raises(pkg.TcrNetError) as e:
+            net.build(0)
+        assert e.value.status == pkg.ERR_EDGE_OVERFLOW
+        net.set_option(pkg.OPT_EDGE_LIMIT, 1 << 31)
+        assert net.build(1) == 3000 * 2999 // 2 + 3000
+        rp, cl, dg = net.copy_csr()
+        check_csr_invariants(rp, cl, dg, 3002)
+        assert dg[:3000].tolist() == [3000] * 3000 and dg[3000] == 3000 and dg[3001] == 0
+
+
 def test_device_side_validation(pkg):
     import torch
     with pkg.TcrNet(0) as net:
