@@ -105,8 +105,10 @@ typedef enum tcrnet_option {
                                      antigen-cognate sequences and analyses only those nodes.
                                      n_q > 0: rows 0..n_q-1 of the next tcrnet_load are the query
                                      rows and builds keep only the edges with at least one query
-                                     endpoint (query-query and query-repertoire); pairs of two
-                                     non-query rows are never evaluated.  0 (default): all pairs.
+                                     endpoint (query-query and query-repertoire).  Through the segment
+                                     join (l_max <= 4) all candidate pairs are decided and the others
+                                     dropped at emission; the trie / text-chunk kernels never evaluate a
+                                     pair of two non-query rows.  0 (default): all pairs.
                                      Takes effect at the next tcrnet_load.                      */
     TCRNET_OPT_DEDUP = 10,        /* 1 (default): rows with identical sequences are collapsed at
                                      load; the distance step runs over the distinct sequences and

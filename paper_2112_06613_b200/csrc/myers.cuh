@@ -194,6 +194,7 @@ __device__ __forceinline__ void emit_edges(const DistanceParams& P, bool edge, i
         oj = (uint32_t)P.perm_t[t_sorted];
         if (P.mode == kPairsQueryAll) edge = oj >= (uint32_t)P.n_query || n > m || oi < oj;
         else if (P.mode == kPairsAllQuery) edge = oi >= (uint32_t)P.n_query;
+        else if (P.mode == kPairsSelfQuery) edge = min(oi, oj) < (uint32_t)P.n_query;
     }
     const uint32_t bal = __ballot_sync(0xffffffffu, edge);
     if (bal) {

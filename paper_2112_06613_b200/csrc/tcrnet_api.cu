@@ -401,7 +401,7 @@ void schedule_pass(const tcrnet_ctx* ctx, int l_max, int first_check, bool use_j
         for (int n = n0; n <= std::min(kMaxLen, m + l_max); ++n) {
             if (!ts.hist[n]) continue;
             const int64_t pc = ps.hist[m], tc = ts.hist[n];
-            const bool diag = pass.mode == kPairsSelf && m == n;
+            const bool diag = (pass.mode == kPairsSelf || pass.mode == kPairsSelfQuery) && m == n;
             const int64_t pairs = diag ? pc * (pc - 1) / 2 : pc * tc;
             st.pairs_kept += pairs;
             st.cells_kept += pairs * m * n;
@@ -475,16 +475,30 @@ void make_schedule(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule& 
         st.cells_all = (int64_t)((sum_len * sum_len - sum_sq) / 2);
     }
     st.pairs_all = ctx->n * (ctx->n - 1) / 2;
+    // The join serves the thresholds it is specialised on, with the early exit on (its verification is banded by
+    // construction); beyond them the trie / text-chunk kernels.
+    const bool can_join = ctx->early_exit && l_max <= kTrieMaxL;
+    sch.fast_l1 = can_join && ctx->fast_l1 && l_max <= 1;
+    sch.use_join = sch.fast_l1 || (can_join && (ctx->segment_join == 1 ||
+                                                (ctx->segment_join < 0 && ctx->prefix_trie)));
     if (ctx->query.loaded) {  // rectangular mode: the pairs with at least one endpoint among the query rows
         const int64_t rest = ctx->n - ctx->query.n;
         st.pairs_all = ctx->query.n * (ctx->query.n - 1) / 2 + ctx->query.n * rest;
-        sch.passes.resize(2);
-        sch.passes[0].pset = &ctx->query;
-        sch.passes[0].tset = &ctx->all;
-        sch.passes[0].mode = kPairsQueryAll;
-        sch.passes[1].pset = &ctx->all;
-        sch.passes[1].tset = &ctx->query;
-        sch.passes[1].mode = kPairsAllQuery;
+        if (sch.use_join) {
+            // through the join: ONE pass over all rows as in the all-pairs mode; the emission keeps the pairs that
+            // have a query row (kPairsSelfQuery)
+            sch.passes.resize(1);
+            sch.passes[0].pset = sch.passes[0].tset = &ctx->all;
+            sch.passes[0].mode = kPairsSelfQuery;
+        } else {
+            sch.passes.resize(2);
+            sch.passes[0].pset = &ctx->query;
+            sch.passes[0].tset = &ctx->all;
+            sch.passes[0].mode = kPairsQueryAll;
+            sch.passes[1].pset = &ctx->all;
+            sch.passes[1].tset = &ctx->query;
+            sch.passes[1].mode = kPairsAllQuery;
+        }
     } else {
         sch.passes.resize(1);
         sch.passes[0].pset = sch.passes[0].tset = &ctx->all;
@@ -492,13 +506,6 @@ void make_schedule(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule& 
     }
     st.work_items = st.work_items_trie = st.work_items_join = 0;
     sch.n_rows = sch.n_join_rows = 0;
-    // The join serves the all-pairs mode with the early exit on (its verification always votes); the rectangular
-    // mode and l_max beyond the specialised range stay with the trie / text-chunk kernels.
-    const bool can_join = !ctx->query.loaded && ctx->early_exit && l_max <= kTrieMaxL;
-    // (TCRNET_OPT_FAST_L1 forces the join for l_max <= 1: its verification IS the XOR / prefix-suffix check there)
-    sch.fast_l1 = can_join && ctx->fast_l1 && l_max <= 1;
-    sch.use_join = sch.fast_l1 || (can_join && (ctx->segment_join == 1 ||
-                                                (ctx->segment_join < 0 && ctx->prefix_trie)));
     for (Schedule::Pass& pass : sch.passes) {
         schedule_pass(ctx, l_max, first_check, sch.use_join, pass, st);
         for (int trie = 0; trie < 2; ++trie)

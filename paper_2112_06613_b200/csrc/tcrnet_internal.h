@@ -72,7 +72,10 @@ struct TrieLevels {
 //                   a query is kept only if it is longer, or of equal length with the larger row id
 //   kPairsAllQuery  patterns = all rows, texts = query set, len_t > len_p; patterns that are
 //                   queries themselves are dropped (the pair was found by the first pass)
-enum PairMode : int32_t { kPairsSelf = 0, kPairsQueryAll = 1, kPairsAllQuery = 2 };
+//   kPairsSelfQuery the rectangular mode through the segment join: patterns and texts are all rows as in kPairsSelf,
+//                   and a pair is kept iff one of its rows is a query row (the join looks at so few pairs that
+//                   deciding all of them and dropping the others costs less than two restricted passes)
+enum PairMode : int32_t { kPairsSelf = 0, kPairsQueryAll = 1, kPairsAllQuery = 2, kPairsSelfQuery = 3 };
 
 struct DistanceParams {
     const WorkRow* rows;

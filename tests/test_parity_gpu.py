@@ -724,7 +724,12 @@ def test_query_mode(pkg, oracle, n_query):
     """NEXT-2 (PAPER.md:109-115, antigen-specific networks): the first N_a rows are the queries;
     the build keeps exactly the edges with at least one query endpoint."""
     d = generate("cfg2", n=12000)
-    for l_max, opts in ((0, {}), (1, {}), (2, {}), (3, {pkg.OPT_PREFIX_TRIE: 0}), (4, {pkg.OPT_TRIE_CHUNK: 512})):
+    # default: through the segment join (one pass over all rows, the emission keeps the pairs with a query row);
+    # TCRNET_OPT_SEGMENT_JOIN = 0 / TCRNET_OPT_PREFIX_TRIE = 0 / l_max > 4: the two restricted passes of the trie /
+    # text-chunk kernels
+    for l_max, opts in ((0, {}), (1, {}), (2, {}), (3, {}), (4, {}), (5, {}), (0, {pkg.OPT_SEGMENT_JOIN: 0}),
+                        (1, {pkg.OPT_SEGMENT_JOIN: 0}), (2, {pkg.OPT_SEGMENT_JOIN: 0}), (3, {pkg.OPT_PREFIX_TRIE: 0}),
+                        (4, {pkg.OPT_SEGMENT_JOIN: 0, pkg.OPT_TRIE_CHUNK: 512})):
         want = _query_network(oracle, d, n_query, l_max)
         with pkg.TcrNet(0) as net:
             for k, v in opts.items():
@@ -734,6 +739,7 @@ def test_query_mode(pkg, oracle, n_query):
             net.build(l_max)
             got = net.copy_csr()
             st = net.get_stats()
+            assert (st["join_mode"] >= 1) == (not opts and l_max <= 4)
             assert_same_network(got, want)
             assert (np.diff(got[0])[n_query:] == 0).all()                 # no row without a query endpoint
             assert st["pairs_all"] == n_query * (n_query - 1) // 2 + n_query * (d.n - n_query)
