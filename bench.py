@@ -235,6 +235,71 @@ def time_steps(net, step, flush, k, torch):
     return [a.elapsed_time(b) for a, b in ev], stats
 
 
+def run_widenings(args) -> None:
+    """Wall-clock device timings (synchronised, best of 5) of the calls SURVEY 8(f) adds around the hot path."""
+    import torch
+
+    import paper_2112_06613_b200 as pkg
+    from cdr3_synth import CONFIGS, generate
+    cfg = CONFIGS[args.workload]
+    l_max = cfg.l_max[0]
+    d = generate(cfg)
+    d_res, d_len = torch.from_numpy(d.residues).cuda(), torch.from_numpy(d.lengths).cuda()
+
+    def best(f, k=5):
+        f()
+        ts = []
+        for _ in range(k):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            f()
+            torch.cuda.synchronize()
+            ts.append(time.perf_counter() - t0)
+        return 1e3 * min(ts)
+
+    out = {"workload": args.workload, "n": d.n, "l_max": l_max, "unit": "ms (wall clock between synchronisations, best of 5)"}
+    with pkg.TcrNet(0) as net:
+        net.load(d_res, d_len)
+        out["edges"] = net.build(l_max)
+        # NEXT-1: observables on the CSR in HBM
+        out["degree_histogram"] = best(lambda: (net.build(l_max), net.degree_histogram()))
+        out["build_alone"] = best(lambda: net.build(l_max))
+        out["degree_histogram"] -= out["build_alone"]
+        out["neighbor_degree"] = best(lambda: (net.build(l_max), net.neighbor_degree())) - out["build_alone"]
+        lab = {}
+        def comp():
+            net.build(l_max)
+            lab["c"] = net.components()
+        out["components"] = best(comp) - out["build_alone"]
+        out["n_components"], out["lcc"] = lab["c"][2], lab["c"][3]
+        rng = np.random.default_rng(0)
+        rank = rng.permutation(d.n).astype(np.int32)
+        steps = np.linspace(0, d.n, 21).astype(np.int64)
+        out["percolation_21_steps"] = best(lambda: net.percolation(rank, steps), 3)
+        # NEXT-3: labels of a build at l_max + 1, then the sweep down
+        def sweep():
+            net.build(l_max + 1)
+            net.edge_distances()
+            for t in range(l_max, -1, -1):
+                net.restrict(t)
+        out[f"build_l{l_max + 1}_labels_restrict_down_to_0"] = best(sweep, 3)
+        out[f"build_l{l_max + 1}_alone"] = best(lambda: net.build(l_max + 1), 3)
+        # 8(e): one shard through build_shard + assemble (what every rank of a sharded build does, world = 1)
+        out["build_shard_plus_assemble"] = best(lambda: net.assemble(net.build_shard(l_max, 0, 1)))
+    # NEXT-2: query x repertoire mode (first n_q rows are the queries), load + build
+    for n_q in (177, 16663):
+        if n_q >= d.n:
+            continue
+        with pkg.TcrNet(0) as net:
+            net.set_option(pkg.OPT_N_QUERY, n_q)
+            def step():
+                net.load(d_res, d_len)
+                return net.build(l_max)
+            out[f"query_mode_nq{n_q}_load_build"] = best(step)
+            out[f"query_mode_nq{n_q}_edges"] = step()
+    print(json.dumps(out))
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -248,6 +313,9 @@ def main() -> None:
     ap.add_argument("--sharded", action="store_true",
                     help="N > 1: ONE repertoire, every rank builds its shard of the work items, the edge keys are "
                          "all-gathered and every rank assembles the CSR (strong scaling); default: replicas (weak)")
+    ap.add_argument("--widenings", action="store_true",
+                    help="instead of the bench line: device timings of the SURVEY 8(f) rows on the workload (observables, "
+                         "distance labels + threshold sweep, query x repertoire mode, one shard + assemble), one JSON line")
     ap.add_argument("--first-check", type=int, default=0)
     ap.add_argument("--text-chunk", type=int, default=0)
     ap.add_argument("--trie-chunk", type=int, default=0)
@@ -262,6 +330,10 @@ def main() -> None:
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.impl == "reference":
         run_reference(args, rank)
+        return
+    if args.widenings:
+        if rank == 0:
+            run_widenings(args)
         return
 
     import torch
