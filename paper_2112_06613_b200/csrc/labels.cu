@@ -3,10 +3,13 @@
 // the key validation of tcrnet_assemble.
 //
 // The distance kernels decide "lev <= l_max" for ~10^11 pairs and keep ~10^6..10^7 of them; the
-// labels are computed afterwards for the kept edges only (one thread per edge, the same
-// Myers/Hyyro column recurrence on a 64-bit word with the match mask of each column derived on
-// the fly from the pattern bytes), which costs microseconds and needs no room in the edge keys.
-// HBM/L2-bound: 2 pattern rows (<= 128 B) read and 1 byte written per edge.
+// labels are computed afterwards for the kept edges only: one thread per edge, the Myers/Hyyro
+// column recurrence on one word, the match mask of each column derived from the two bit-plane rows
+// (Eq = AND over the five planes of "plane of a agrees with bit k of the text residue": five selects),
+// so an edge costs two 32-byte rows and ~25 instructions per column.  The first index of every edge
+// is written once per CSR by k_edge_rows (one thread per row) instead of a binary search per edge.
+// HBM/L2-bound: 2 plane rows read and 1 byte written per edge.
+#include "planes.cuh"
 #include "tcrnet_internal.h"
 
 namespace tcrnet {
@@ -18,54 +21,49 @@ __global__ void __launch_bounds__(256) k_inverse_perm(const int32_t* __restrict_
     if (s < n) inv[perm[s]] = (int32_t)s;
 }
 
-// first index of edge e = the row r with row_ptr[r] <= e < row_ptr[r+1]
-__device__ __forceinline__ int64_t row_of_edge(const int64_t* __restrict__ row_ptr, int64_t n, int64_t e) {
-    int64_t lo = 0, hi = n;  // invariant: row_ptr[lo] <= e < row_ptr[hi]
-    while (hi - lo > 1) {
-        const int64_t mid = (lo + hi) >> 1;
-        if (row_ptr[mid] <= e) lo = mid; else hi = mid;
-    }
-    return lo;
+// edge_row[e] = first index of edge e (the row r with row_ptr[r] <= e < row_ptr[r+1])
+__global__ void __launch_bounds__(256) k_edge_rows(const int64_t* __restrict__ row_ptr, int64_t n,
+                                                  int32_t* __restrict__ edge_row) {
+    const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n) return;
+    const int64_t b = row_ptr[r], e = row_ptr[r + 1];
+    for (int64_t k = b; k < e; ++k) edge_row[k] = (int32_t)r;
 }
 
-__device__ __forceinline__ int row_length(const uint8_t* row, int pat_stride) {
-    int len = 0;
-    while (len < pat_stride && row[len] != 0xffu) ++len;
-    return len;
-}
-
-// lev(a, b) for |a| = m <= 64: Pv / Mv are the +1 / -1 vertical deltas of the current DP column
-// (PAPER.md:277-293 computed column by column; the "| 1" is the boundary D[0][j] = j).
-__device__ int lev64(const uint8_t* a, int m, const uint8_t* b, int n) {
+// lev(a, b) column by column: Pv / Mv are the +1 / -1 vertical deltas of the current DP column,
+// the "| 1" is the boundary D[0][j] = j; |a| = m <= bits of W.
+template <typename W>
+__device__ __forceinline__ int lev_planes(const PlaneRow<W>& A, const PlaneRow<W>& B) {
+    const int m = A.len, n = B.len;
     if (m == 0) return n;
-    const unsigned long long low_m = m >= 64 ? ~0ull : ((1ull << m) - 1ull);
-    unsigned long long Pv = low_m, Mv = 0ull;
+    const W low_m = m >= (int)(8 * sizeof(W)) ? ~W(0) : ((W(1) << m) - W(1));
+    W Pv = low_m, Mv = W(0);
     for (int j = 0; j < n; ++j) {
-        const uint8_t c = b[j];
-        unsigned long long Eq = 0ull;
-        for (int i = 0; i < m; ++i) Eq |= (unsigned long long)(a[i] == c) << i;
-        const unsigned long long D0 = ((((Eq & Pv) + Pv) ^ Pv) | Eq) | Mv;
-        const unsigned long long Hp = Mv | ~(D0 | Pv);
-        const unsigned long long Hn = Pv & D0;
-        const unsigned long long Hp1 = (Hp << 1) | 1ull;
+        W Eq = low_m;
+#pragma unroll
+        for (int k = 0; k < 5; ++k) Eq &= ((B.p[k] >> j) & W(1)) ? A.p[k] : ~A.p[k];
+        const W D0 = ((((Eq & Pv) + Pv) ^ Pv) | Eq) | Mv;
+        const W Hp = Mv | ~(D0 | Pv);
+        const W Hn = Pv & D0;
+        const W Hp1 = (Hp << 1) | W(1);
         Pv = (Hn << 1) | ~(D0 | Hp1);
         Mv = D0 & Hp1;
     }
-    return n + __popcll(Pv & low_m) - __popcll(Mv & low_m);
+    const W pm = Pv & low_m, mm = Mv & low_m;
+    return n + (sizeof(W) == 8 ? __popcll((unsigned long long)pm) - __popcll((unsigned long long)mm)
+                               : __popc((uint32_t)pm) - __popc((uint32_t)mm));
 }
 
-__global__ void __launch_bounds__(256) k_edge_distances(const int64_t* __restrict__ row_ptr,
-                                                       const int32_t* __restrict__ col, int64_t n, int64_t n_edges,
+template <typename W>
+__global__ void __launch_bounds__(256) k_edge_distances(const int32_t* __restrict__ edge_row,
+                                                       const int32_t* __restrict__ col, int64_t n_edges,
                                                        const int32_t* __restrict__ inv_perm,
-                                                       const uint8_t* __restrict__ pat, int pat_stride,
-                                                       uint8_t* __restrict__ dist) {
+                                                       const void* __restrict__ planes, uint8_t* __restrict__ dist) {
     const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= n_edges) return;
-    const int64_t u = row_of_edge(row_ptr, n, e);
-    const int64_t v = col[e];
-    const uint8_t* a = pat + (size_t)inv_perm[u] * pat_stride;
-    const uint8_t* b = pat + (size_t)inv_perm[v] * pat_stride;
-    dist[e] = (uint8_t)lev64(a, row_length(a, pat_stride), b, row_length(b, pat_stride));
+    const PlaneRow<W> A = load_planes<W>(planes, inv_perm[edge_row[e]]);
+    const PlaneRow<W> B = load_planes<W>(planes, inv_perm[col[e]]);
+    dist[e] = (uint8_t)lev_planes<W>(A, B);
 }
 
 __global__ void __launch_bounds__(256) k_restrict_flags(const uint8_t* __restrict__ dist, int64_t n_edges, int l_max,
@@ -74,16 +72,16 @@ __global__ void __launch_bounds__(256) k_restrict_flags(const uint8_t* __restric
     if (e < n_edges) flags[e] = (int)dist[e] <= l_max ? 1u : 0u;
 }
 
-__global__ void __launch_bounds__(256) k_restrict_compact(const int64_t* __restrict__ row_ptr,
+__global__ void __launch_bounds__(256) k_restrict_compact(const int32_t* __restrict__ edge_row,
                                                          const int32_t* __restrict__ col,
-                                                         const uint8_t* __restrict__ dist, int64_t n, int64_t n_edges,
+                                                         const uint8_t* __restrict__ dist, int64_t n_edges,
                                                          const uint32_t* __restrict__ flags,
                                                          const uint32_t* __restrict__ pos,
                                                          unsigned long long* __restrict__ keys_out,
                                                          uint8_t* __restrict__ dist_out) {
     const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= n_edges || !flags[e]) return;
-    const unsigned long long u = (unsigned long long)row_of_edge(row_ptr, n, e);
+    const unsigned long long u = (unsigned long long)(uint32_t)edge_row[e];
     keys_out[pos[e]] = (u << 32) | (uint32_t)col[e];
     dist_out[pos[e]] = dist[e];
 }
@@ -110,11 +108,18 @@ cudaError_t launch_inverse_perm(const int32_t* perm, int64_t n, int32_t* inv, cu
     return cudaGetLastError();
 }
 
-cudaError_t launch_edge_distances(const int64_t* row_ptr, const int32_t* col, int64_t n, int64_t n_edges,
-                                  const int32_t* inv_perm, const uint8_t* pat, int pat_stride, uint8_t* dist,
-                                  cudaStream_t s, int* launches) {
+cudaError_t launch_edge_rows(const int64_t* row_ptr, int64_t n, int32_t* edge_row, cudaStream_t s, int* launches) {
+    if (n <= 0) return cudaSuccess;
+    k_edge_rows<<<grid_for(n), 256, 0, s>>>(row_ptr, n, edge_row);
+    *launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_edge_distances(const int32_t* edge_row, const int32_t* col, int64_t n_edges, const int32_t* inv_perm,
+                                  const void* planes, bool wide_planes, uint8_t* dist, cudaStream_t s, int* launches) {
     if (n_edges <= 0) return cudaSuccess;
-    k_edge_distances<<<grid_for(n_edges), 256, 0, s>>>(row_ptr, col, n, n_edges, inv_perm, pat, pat_stride, dist);
+    if (wide_planes) k_edge_distances<uint64_t><<<grid_for(n_edges), 256, 0, s>>>(edge_row, col, n_edges, inv_perm, planes, dist);
+    else k_edge_distances<uint32_t><<<grid_for(n_edges), 256, 0, s>>>(edge_row, col, n_edges, inv_perm, planes, dist);
     *launches += 1;
     return cudaGetLastError();
 }
@@ -127,12 +132,11 @@ cudaError_t launch_restrict_flags(const uint8_t* dist, int64_t n_edges, int l_ma
     return cudaGetLastError();
 }
 
-cudaError_t launch_restrict_compact(const int64_t* row_ptr, const int32_t* col, const uint8_t* dist, int64_t n,
+cudaError_t launch_restrict_compact(const int32_t* edge_row, const int32_t* col, const uint8_t* dist,
                                     int64_t n_edges, const uint32_t* flags, const uint32_t* pos,
                                     unsigned long long* keys_out, uint8_t* dist_out, cudaStream_t s, int* launches) {
     if (n_edges <= 0) return cudaSuccess;
-    k_restrict_compact<<<grid_for(n_edges), 256, 0, s>>>(row_ptr, col, dist, n, n_edges, flags, pos, keys_out,
-                                                         dist_out);
+    k_restrict_compact<<<grid_for(n_edges), 256, 0, s>>>(edge_row, col, dist, n_edges, flags, pos, keys_out, dist_out);
     *launches += 1;
     return cudaGetLastError();
 }

@@ -841,9 +841,11 @@ int ensure_edge_distances(tcrnet_ctx* ctx, int* launches) {
                                             (const int32_t*)ctx->all.members.p, (int32_t*)ctx->inv_perm.p, s, launches));
     else
         TRY_CUDA(launch_inverse_perm((const int32_t*)ctx->all.perm.p, ctx->n, (int32_t*)ctx->inv_perm.p, s, launches));
-    TRY_CUDA(launch_edge_distances((const int64_t*)ctx->row_ptr.p, (const int32_t*)ctx->col.p, ctx->n, ctx->n_edges,
-                                   (const int32_t*)ctx->inv_perm.p, (const uint8_t*)ctx->all.pat.p,
-                                   ctx->all.pat_stride, (uint8_t*)ctx->edge_dist.p, s, launches));
+    TRY(dev_reserve(ctx, ctx->edge_row, sizeof(int32_t) * (size_t)std::max<int64_t>(ctx->n_edges, 1)));
+    TRY_CUDA(launch_edge_rows((const int64_t*)ctx->row_ptr.p, ctx->n, (int32_t*)ctx->edge_row.p, s, launches));
+    TRY_CUDA(launch_edge_distances((const int32_t*)ctx->edge_row.p, (const int32_t*)ctx->col.p, ctx->n_edges,
+                                   (const int32_t*)ctx->inv_perm.p, ctx->all.planes.p, ctx->all.wide_planes,
+                                   (uint8_t*)ctx->edge_dist.p, s, launches));
     ctx->have_dist = true;
     return TCRNET_OK;
 }
@@ -910,7 +912,7 @@ void tcrnet_destroy(tcrnet_ctx* ctx) {
     cudaStreamSynchronize(ctx->stream);
     DevBuf* bufs[] = {&ctx->all.perm, &ctx->all.pat, &ctx->all.txt, &ctx->all.trie, &ctx->query.perm, &ctx->query.pat,
                       &ctx->query.txt, &ctx->query.trie, &ctx->all.planes, &ctx->query.planes, &ctx->join_cand, &ctx->expand_huge, &ctx->join_cnt, &ctx->join_dir,
-                      &ctx->join_entries, &ctx->join_rows, &ctx->inv_perm, &ctx->edge_dist, &ctx->edge_dist_b, &ctx->flags,
+                      &ctx->join_entries, &ctx->join_rows, &ctx->inv_perm, &ctx->edge_row, &ctx->edge_dist, &ctx->edge_dist_b, &ctx->flags,
                       &ctx->flag_pos, &ctx->in_res, &ctx->in_len, &ctx->offsets,
                       &ctx->perm_tmp, &ctx->trie_scratch, &ctx->keys_a, &ctx->keys_b, &ctx->radix_scratch,
                       &ctx->scan_scratch, &ctx->rows, &ctx->row_ptr, &ctx->col, &ctx->row_count, &ctx->long_rows, &ctx->all.group_start, &ctx->all.members, &ctx->all.uid_of,
@@ -1115,8 +1117,9 @@ int tcrnet_restrict(tcrnet_ctx* ctx, int l_max, int64_t* n_edges_out) {
         TRY_CUDA(launch_restrict_flags((const uint8_t*)ctx->edge_dist.p, e_old, l_max, (uint32_t*)ctx->flags.p, s, &launches));
         TRY_CUDA(exclusive_scan_u32_total((const uint32_t*)ctx->flags.p, (uint32_t*)ctx->flag_pos.p, e_old,
                                           ctx->scan_scratch.p, s, &launches));
-        TRY_CUDA(launch_restrict_compact((const int64_t*)ctx->row_ptr.p, (const int32_t*)ctx->col.p,
-                                         (const uint8_t*)ctx->edge_dist.p, ctx->n, e_old, (const uint32_t*)ctx->flags.p,
+        // (edge_row belongs to the CSR being restricted: ensure_edge_distances wrote it, or the restriction before)
+        TRY_CUDA(launch_restrict_compact((const int32_t*)ctx->edge_row.p, (const int32_t*)ctx->col.p,
+                                         (const uint8_t*)ctx->edge_dist.p, e_old, (const uint32_t*)ctx->flags.p,
                                          (const uint32_t*)ctx->flag_pos.p, (unsigned long long*)ctx->keys_a.p,
                                          (uint8_t*)ctx->edge_dist_b.p, s, &launches));
         uint32_t total = 0;
@@ -1131,6 +1134,8 @@ int tcrnet_restrict(tcrnet_ctx* ctx, int l_max, int64_t* n_edges_out) {
     TRY_CUDA(cudaEventRecord(ctx->ev[2], s));
     TRY_CUDA(launch_csr((const unsigned long long*)ctx->keys_a.p, e_new, ctx->n, (int64_t*)ctx->row_ptr.p,
                         (int32_t*)ctx->col.p, (int32_t*)ctx->deg.p, s, &launches));
+    // the labels stay valid for the restricted CSR (compacted above); so must the first indices of its edges
+    if (e_new > 0) TRY_CUDA(launch_edge_rows((const int64_t*)ctx->row_ptr.p, ctx->n, (int32_t*)ctx->edge_row.p, s, &launches));
     TRY_CUDA(cudaEventRecord(ctx->ev[3], s));
     TRY_CUDA(cudaEventSynchronize(ctx->ev[3]));
     tcrnet_stats& st = ctx->stats;

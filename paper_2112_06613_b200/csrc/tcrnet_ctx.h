@@ -95,6 +95,7 @@ struct tcrnet_ctx {
     int64_t n_edges = 0, n_keys = 0;
     DevBuf keys_a, keys_b, radix_scratch, scan_scratch, rows, row_ptr, col, deg, row_count, long_rows;
     DevBuf expand_huge;  // dedup.cu: (pair, first output position) of the products k_expand_huge spreads over the grid
+    DevBuf edge_row;  // first index of every edge of the current CSR (labels.cu; valid with edge_dist)
     DevBuf inv_perm, edge_dist, edge_dist_b, flags, flag_pos;
     // segment join (segjoin.cu): directory + entries of the current load for join_l_max, work rows
     DevBuf join_cnt, join_dir, join_entries, join_rows, join_cand;

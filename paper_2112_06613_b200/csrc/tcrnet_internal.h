@@ -262,14 +262,16 @@ cudaError_t launch_join(const DistanceParams& p, const JoinRow* rows, int n_rows
 
 // labels.cu: distance labels of the final edges, threshold restriction, key validation
 cudaError_t launch_inverse_perm(const int32_t* perm, int64_t n, int32_t* inv, cudaStream_t s, int* launches);
-cudaError_t launch_edge_distances(const int64_t* row_ptr, const int32_t* col, int64_t n, int64_t n_edges,
-                                  const int32_t* inv_perm, const uint8_t* pat, int pat_stride, uint8_t* dist,
-                                  cudaStream_t s, int* launches);
+// edge_row[e] = first index of edge e of the CSR
+cudaError_t launch_edge_rows(const int64_t* row_ptr, int64_t n, int32_t* edge_row, cudaStream_t s, int* launches);
+// dist[e] = lev(row edge_row[e], row col[e]) from the bit-plane rows (planes.cuh)
+cudaError_t launch_edge_distances(const int32_t* edge_row, const int32_t* col, int64_t n_edges, const int32_t* inv_perm,
+                                  const void* planes, bool wide_planes, uint8_t* dist, cudaStream_t s, int* launches);
 // flags[e] = dist[e] <= l_max (uint32 0/1)
 cudaError_t launch_restrict_flags(const uint8_t* dist, int64_t n_edges, int l_max, uint32_t* flags, cudaStream_t s,
                                   int* launches);
 // stable compaction of the kept edges into keys (row << 32 | col) and their labels
-cudaError_t launch_restrict_compact(const int64_t* row_ptr, const int32_t* col, const uint8_t* dist, int64_t n,
+cudaError_t launch_restrict_compact(const int32_t* edge_row, const int32_t* col, const uint8_t* dist,
                                     int64_t n_edges, const uint32_t* flags, const uint32_t* pos /*exclusive scan*/,
                                     unsigned long long* keys_out, uint8_t* dist_out, cudaStream_t s, int* launches);
 // *flag |= 1 if any key has u >= v or v >= n

@@ -710,6 +710,41 @@ def test_edge_distances_and_threshold_sweep(pkg, oracle):
         assert ei.value.status == pkg.ERR_LMAX
 
 
+def test_edge_distances_long_sequences_and_large_thresholds(pkg, oracle):
+    """Labels on 64-bit plane rows (sequences of up to 64 residues) and for a build beyond the thresholds the join
+    serves (l_max = 9: text-chunk kernel), against oracle.lev_pairs edge by edge; the sweep down to 0."""
+    rng = np.random.default_rng(64)
+    strings = []
+    for _ in range(300):
+        n = int(rng.integers(20, 65))
+        s = "".join("ACDEFGHIKLMNPQRSTVWY"[i] for i in rng.integers(0, 20, n))
+        strings.append(s)
+        for _ in range(3):
+            t = list(s)
+            for _ in range(int(rng.integers(1, 9))):
+                q = int(rng.integers(0, len(t)))
+                k = int(rng.integers(0, 3))
+                if k == 0:
+                    t[q] = "ACDEFGHIKLMNPQRSTVWY"[int(rng.integers(0, 20))]
+                elif k == 1 and len(t) < 64:
+                    t.insert(q, "W")
+                elif len(t) > 1:
+                    del t[q]
+            strings.append("".join(t))
+    res, ln = from_strings(strings)
+    with pkg.TcrNet(0) as net:
+        net.load(res, ln)
+        for top in (9, 3):
+            net.build(top)
+            rp, cl, dg = net.copy_csr()
+            rows = np.repeat(np.arange(len(strings), dtype=np.int64), np.diff(rp))
+            want_d = oracle.lev_pairs(res, ln, np.stack([rows, cl.astype(np.int64)], axis=1)).astype(np.uint8)
+            assert np.array_equal(net.edge_distances().cpu().numpy(), want_d) and want_d.max() == top
+            for l in range(top - 1, -1, -2):
+                assert net.restrict(l) == int((want_d <= l).sum())
+                assert_same_network(net.copy_csr(), oracle.network(res, ln, l, tier=1)[:3])
+
+
 def _query_network(oracle, d, n_query, l_max):
     """Oracle side of the rectangular mode: rows 0..n_query-1 against every other row."""
     pairs, _ = oracle.edges(d.residues, d.lengths, l_max, rows=np.arange(n_query), all_partners=True, tier=0)
