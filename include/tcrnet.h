@@ -212,9 +212,8 @@ TCRNET_API void tcrnet_destroy(tcrnet_ctx* ctx);
  * for the distance kernels: rows collapsed to distinct sequences; stable sort into length buckets (by
  * length and row; by length, first six residues and row when TCRNET_OPT_SEGMENT_JOIN = 0, the rectangular
  * mode or TCRNET_OPT_EARLY_EXIT = 0 announce the prefix-trie kernel); permutation; per sorted position one
- * bit-plane row (5-bit residue codes, one bit of the code per word, 32 bytes up to 32 residues) and one row
- * of 8-bit residue codes.  The text rows and the prefix trie of the trie / text-chunk kernels are built by
- * the first build that needs them.  PAPER.md:326 ("each a.a. is saved as a number ... BYTE"), north_star (1).
+ * bit-plane row (5-bit residue codes, one bit of the code per word, 32 bytes up to 32 residues).  The byte / word
+ * rows and the prefix trie of the trie / text-chunk kernels are built by the first build that needs them.  PAPER.md:326 ("each a.a. is saved as a number ... BYTE"), north_star (1).
  *
  *   residues  host, uint8[sum(lengths)]: the rows concatenated, ASCII 'A'..'Z' (any of the 26
  *             letters is a legal residue; only equality matters - DESIGN.md reading Q8)

@@ -4,13 +4,13 @@
 //
 //   pat : one row per sorted position, one residue code (0..25) per byte, row stride
 //         pat_stride bytes (multiple of 16), padded with 0xff - read once per work item to
-//         build the Peq match masks.
+//         build the Peq match masks.  Written on demand, like txt.
 //   txt : per length bucket, one row of round_up(len,4) 32-bit words per sequence holding the
 //         residue code of each column, padded with kPadCode - streamed into shared memory
 //         and read with one broadcast 128-bit load per four columns.  The code sits in a
 //         32-bit word so that the per-column Peq address is a single IMAD (code * row_bytes
 //         + lane offset) on the FMA pipe, leaving the ALU pipe to the bit-vector recurrence.
-//         Written on demand (k_txt_from_pat): only the prefix-trie / text-chunk kernels read it.
+//         Written on demand (k_rows_from_planes): only the prefix-trie / text-chunk kernels read it.
 //   planes : one row of 8 words per sorted position: plane k = bit k of the 5-bit code of every residue
 //         (north_star (1): 5-bit codes, here one bit of the code per word so that a residue-wise comparison of two
 //         sequences under any shift is five XORs) + the length - what the segment join reads (segjoin.cu).
@@ -71,16 +71,14 @@ __global__ void __launch_bounds__(256) k_seq_keys(const uint8_t* __restrict__ re
     vals[i] = (int32_t)i;
 }
 
-// One thread per sorted position: the pattern row is written with 128-bit stores (pat_stride is a
-// multiple of 16), the text row (TXT: only when the trie / text-chunk kernels will run) with one 128-bit store per
-// four columns, the bit-plane row (segjoin.cu) as 8 words of W.
-template <typename W, bool TXT>
+// One thread per sorted position: the residues of the row become its bit-plane row (8 words of W: planes 0..4, the
+// length, two zero words).  A collapsed load (dedup.cu) arrives with perm[s] = uid of the distinct sequence; perm[s] is
+// re-coded on the way out: the row itself for a sequence that one row has, kGroupFlag | uid for a shared one.
+template <typename W>
 __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residues,
                                              const int64_t* __restrict__ offsets,
                                              const int32_t* __restrict__ lengths,
                                              int32_t* __restrict__ perm, int64_t n,
-                                             const __grid_constant__ LengthTable lt, int pat_stride,
-                                             uint8_t* __restrict__ pat, uint32_t* __restrict__ txt,
                                              W* __restrict__ planes, uint32_t* __restrict__ flags,
                                              const uint32_t* __restrict__ group_start,
                                              const int32_t* __restrict__ members) {
@@ -91,44 +89,16 @@ __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residu
         const int32_t o = perm[s];
         const int32_t len = lengths[o];
         const uint8_t* src = residues + offsets[o];
-        uint4* prow = reinterpret_cast<uint4*>(pat + (size_t)s * pat_stride);
-        const int rw = lt.row_words[len];
-        uint4* trow = TXT ? reinterpret_cast<uint4*>(txt + lt.txt_base[len] + (int64_t)(s - lt.start[len]) * rw) : nullptr;
         W pl[5] = {W(0), W(0), W(0), W(0), W(0)};
-        for (int i0 = 0; i0 < pat_stride; i0 += 16) {
-            uint32_t c[16];
-#pragma unroll
-            for (int k = 0; k < 16; ++k) {
-                const int i = i0 + k;
-                c[k] = 0xffu;
-                if (i < len) {
-                    c[k] = (uint32_t)src[i] - (uint32_t)'A';
-                    if (c[k] >= (uint32_t)kNumCodes) {
-                        bad = true;
-                        c[k] = 0;
-                    }
-#pragma unroll
-                    for (int b = 0; b < 5; ++b) pl[b] |= (W)((c[k] >> b) & 1u) << i;
-                }
+        for (int i = 0; i < len; ++i) {
+            uint32_t c = (uint32_t)src[i] - (uint32_t)'A';
+            if (c >= (uint32_t)kNumCodes) {
+                bad = true;
+                c = 0;
             }
-            uint32_t w4[4];
 #pragma unroll
-            for (int k = 0; k < 4; ++k) w4[k] = c[4 * k] | (c[4 * k + 1] << 8) | (c[4 * k + 2] << 16) | (c[4 * k + 3] << 24);
-            prow[i0 >> 4] = make_uint4(w4[0], w4[1], w4[2], w4[3]);
-            if (TXT) {
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    const int i = i0 + 4 * k;  // text columns i .. i+3
-                    if (i < rw) {
-                        uint32_t t[4];
-#pragma unroll
-                        for (int q = 0; q < 4; ++q) t[q] = i + q < len ? c[4 * k + q] : (uint32_t)kPadCode;
-                        trow[i >> 2] = make_uint4(t[0], t[1], t[2], t[3]);
-                    }
-                }
-            }
+            for (int b = 0; b < 5; ++b) pl[b] |= (W)((c >> b) & 1u) << i;
         }
-        // bit-plane row: planes 0..4, the length, two zero words
         W* row = planes + (size_t)s * kPlaneWords;
         if (sizeof(W) == 4) {
             uint4* r4 = reinterpret_cast<uint4*>(row);
@@ -141,8 +111,6 @@ __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residu
             r2[2] = make_ulonglong2((unsigned long long)pl[4], (unsigned long long)len);
             r2[3] = make_ulonglong2(0ull, 0ull);
         }
-        // collapsed load (dedup.cu): the rows were the distinct sequences and perm[s] their uid; it now becomes the row
-        // itself for a sequence that one row has, kGroupFlag | uid for a shared one
         if (group_start) {
             const uint32_t b = group_start[o];
             perm[s] = group_start[o + 1] - b == 1u ? members[b] : (int32_t)(kGroupFlag | (uint32_t)o);
@@ -151,31 +119,49 @@ __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residu
     if (__syncthreads_or(bad) && threadIdx.x == 0) atomicOr(flags, kFlagBadResidue);
 }
 
-// The text rows of the trie / text-chunk kernels from the pattern rows (same codes, one 32-bit word per column,
-// padded with kPadCode): written only when a build needs those kernels (tcrnet_api.cu: ensure_text_tables).
-__global__ void __launch_bounds__(256) k_txt_from_pat(const uint8_t* __restrict__ pat, int pat_stride, int64_t n,
-                                                     const __grid_constant__ LengthTable lt, uint32_t* __restrict__ txt) {
-    grid_dependency_wait();
+// The rows of the prefix-trie / text-chunk kernels from the bit-plane rows, written only when a build needs those
+// kernels (tcrnet_api.cu: ensure_text_tables): pat = one residue code per byte, 0xff beyond the sequence, 128-bit
+// stores; txt = one 32-bit word per column, padded with kPadCode, one 128-bit store per four columns.
+template <typename W>
+__global__ void __launch_bounds__(256) k_rows_from_planes(const W* __restrict__ planes, int64_t n,
+                                                         const __grid_constant__ LengthTable lt, int pat_stride,
+                                                         uint8_t* __restrict__ pat, uint32_t* __restrict__ txt) {
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
-    int len = 0;
-    {
-        int lo = 0, hi = kNumLen;  // start[lo] <= s < start[hi]
-        while (hi - lo > 1) {
-            const int mid = (lo + hi) >> 1;
-            if ((int64_t)lt.start[mid] <= s) lo = mid; else hi = mid;
-        }
-        len = lo;
-    }
+    const W* row = planes + (size_t)s * kPlaneWords;
+    W pl[5];
+#pragma unroll
+    for (int b = 0; b < 5; ++b) pl[b] = row[b];
+    const int len = (int)row[5];
+    uint4* prow = reinterpret_cast<uint4*>(pat + (size_t)s * pat_stride);
     const int rw = lt.row_words[len];
     uint4* trow = reinterpret_cast<uint4*>(txt + lt.txt_base[len] + (int64_t)(s - lt.start[len]) * rw);
-    const uint32_t* prow = reinterpret_cast<const uint32_t*>(pat + (size_t)s * pat_stride);
-    for (int i = 0; i < rw; i += 4) {
-        const uint32_t w = prow[i >> 2];
-        uint32_t t[4];
+    for (int i0 = 0; i0 < pat_stride; i0 += 16) {
+        uint32_t c[16];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) t[q] = i + q < len ? ((w >> (8 * q)) & 0xffu) : (uint32_t)kPadCode;
-        trow[i >> 2] = make_uint4(t[0], t[1], t[2], t[3]);
+        for (int k = 0; k < 16; ++k) {
+            const int i = i0 + k;
+            c[k] = 0xffu;
+            if (i < len) {
+                c[k] = 0u;
+#pragma unroll
+                for (int b = 0; b < 5; ++b) c[k] |= (uint32_t)((pl[b] >> i) & W(1)) << b;
+            }
+        }
+        uint32_t w4[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) w4[k] = c[4 * k] | (c[4 * k + 1] << 8) | (c[4 * k + 2] << 16) | (c[4 * k + 3] << 24);
+        prow[i0 >> 4] = make_uint4(w4[0], w4[1], w4[2], w4[3]);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int i = i0 + 4 * k;  // text columns i .. i+3
+            if (i < rw) {
+                uint32_t t[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) t[q] = i + q < len ? c[4 * k + q] : (uint32_t)kPadCode;
+                trow[i >> 2] = make_uint4(t[0], t[1], t[2], t[3]);
+            }
+        }
     }
 }
 
@@ -213,26 +199,26 @@ cudaError_t launch_seq_keys(const uint8_t* residues, const int64_t* offsets, con
     return cudaGetLastError();
 }
 
-cudaError_t launch_pack(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths,
-                        int32_t* perm, int64_t n, const LengthTable& lt, int pat_stride, uint8_t* pat,
-                        uint32_t* txt, void* planes, bool wide_planes, uint32_t* flags, const uint32_t* group_start,
+cudaError_t launch_pack(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths, int32_t* perm, int64_t n,
+                        void* planes, bool wide_planes, uint32_t* flags, const uint32_t* group_start,
                         const int32_t* members, cudaStream_t s, int* launches) {
     const unsigned blocks = (unsigned)((n + 255) / 256);
-    if (wide_planes) {
-        if (txt) launch_dep(k_pack<uint64_t, true>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint64_t*)planes, flags, group_start, members);
-        else launch_dep(k_pack<uint64_t, false>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint64_t*)planes, flags, group_start, members);
-    } else {
-        if (txt) launch_dep(k_pack<uint32_t, true>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint32_t*)planes, flags, group_start, members);
-        else launch_dep(k_pack<uint32_t, false>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, lt, pat_stride, pat, txt, (uint32_t*)planes, flags, group_start, members);
-    }
+    if (wide_planes)
+        launch_dep(k_pack<uint64_t>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, (uint64_t*)planes, flags,
+                   group_start, members);
+    else
+        launch_dep(k_pack<uint32_t>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, (uint32_t*)planes, flags,
+                   group_start, members);
     *launches += 1;
     return cudaGetLastError();
 }
 
-cudaError_t launch_txt_from_pat(const uint8_t* pat, int pat_stride, int64_t n, const LengthTable& lt, uint32_t* txt,
-                                cudaStream_t s, int* launches) {
+cudaError_t launch_rows_from_planes(const void* planes, bool wide_planes, int64_t n, const LengthTable& lt, int pat_stride,
+                                    uint8_t* pat, uint32_t* txt, cudaStream_t s, int* launches) {
     if (n <= 0) return cudaSuccess;
-    launch_dep(k_txt_from_pat, (unsigned)((n + 255) / 256), 256, 0, s, pat, pat_stride, n, lt, txt);
+    const unsigned blocks = (unsigned)((n + 255) / 256);
+    if (wide_planes) k_rows_from_planes<uint64_t><<<blocks, 256, 0, s>>>((const uint64_t*)planes, n, lt, pat_stride, pat, txt);
+    else k_rows_from_planes<uint32_t><<<blocks, 256, 0, s>>>((const uint32_t*)planes, n, lt, pat_stride, pat, txt);
     *launches += 1;
     return cudaGetLastError();
 }

@@ -135,7 +135,6 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
     if (rc == TCRNET_OK) rc = dev_reserve(ctx, ctx->keys_b, sizeof(unsigned long long) * (size_t)n);
     if (rc == TCRNET_OK) rc = dev_reserve(ctx, ctx->perm_tmp, sizeof(int32_t) * (size_t)n);
     if (rc == TCRNET_OK) rc = dev_reserve(ctx, set.perm, sizeof(int32_t) * (size_t)n);
-    if (rc == TCRNET_OK) rc = dev_reserve(ctx, set.pat, (size_t)n * set.pat_stride);
     if (rc == TCRNET_OK) rc = dev_reserve(ctx, set.planes, (size_t)n * kPlaneWords * (set.wide_planes ? 8 : 4));
     if (rc != TCRNET_OK) return rc;
     // Sort key: (length, first kSortPrefix residues, row): one composite 64-bit key per row, stable LSD
@@ -172,8 +171,7 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
         set.lexicographic = lexicographic;
     }
     if (e == cudaSuccess)
-        e = launch_pack(d_res, d_off, d_len, (int32_t*)set.perm.p, n, lt, set.pat_stride,
-                        (uint8_t*)set.pat.p, nullptr, set.planes.p, set.wide_planes, &dc->flags,
+        e = launch_pack(d_res, d_off, d_len, (int32_t*)set.perm.p, n, set.planes.p, set.wide_planes, &dc->flags,
                         code_groups ? (const uint32_t*)set.group_start.p : nullptr,
                         code_groups ? (const int32_t*)set.members.p : nullptr, s, launches);
     // (the text rows and the prefix trie are built by ensure_text_tables when a build needs them)
@@ -193,8 +191,8 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
     return TCRNET_OK;
 }
 
-// The tables only the prefix-trie / text-chunk kernels read: text rows (one 32-bit word per column) expanded from the
-// pattern rows and the prefix trie over them (trie.cu).  Built when a build first schedules one of those kernels (the
+// The tables only the prefix-trie / text-chunk kernels read: pattern rows (one residue code per byte) and text rows (one
+// 32-bit word per column) expanded from the bit-plane rows, and the prefix trie over the text rows (trie.cu).  Built when a build first schedules one of those kernels (the
 // segment join, the default for l_max <= 4, needs neither).
 int ensure_text_tables(tcrnet_ctx* ctx, SeqSet& set, int* launches) {
     if (set.text_tables) return TCRNET_OK;
@@ -203,7 +201,9 @@ int ensure_text_tables(tcrnet_ctx* ctx, SeqSet& set, int* launches) {
     const int64_t n = set.n;
     const LengthTable& lt = set.lt;
     TRY(dev_reserve(ctx, set.txt, sizeof(uint32_t) * (size_t)(lt.txt_base[kNumLen] + 4)));
-    TRY_CUDA(launch_txt_from_pat((const uint8_t*)set.pat.p, set.pat_stride, n, lt, (uint32_t*)set.txt.p, s, launches));
+    TRY(dev_reserve(ctx, set.pat, (size_t)n * set.pat_stride));
+    TRY_CUDA(launch_rows_from_planes(set.planes.p, set.wide_planes, n, lt, set.pat_stride, (uint8_t*)set.pat.p,
+                                     (uint32_t*)set.txt.p, s, launches));
     size_t node_total = 0, level_off[kTrieDepth + 1] = {};
     for (int k = 1; k <= kTrieDepth; ++k) {
         level_off[k] = node_total;

@@ -183,15 +183,14 @@ cudaError_t launch_length_hist(const int32_t* lengths, int64_t n, const uint32_t
 constexpr int kSeqKeyBits = 6 + 5 * kSortPrefix;  // length - 1 (0..63) takes 6 bits
 cudaError_t launch_seq_keys(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths, int64_t n,
                             unsigned long long* keys, int32_t* vals, cudaStream_t s, int* launches);
-// group_start != NULL (collapsed load): perm holds uids on entry and is re-coded in place (the row of an unshared
-// sequence, or kGroupFlag | uid)
-cudaError_t launch_pack(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths,
-                        int32_t* perm, int64_t n, const LengthTable& lt, int pat_stride,
-                        uint8_t* pat, uint32_t* txt /*NULL: not written*/, void* planes, bool wide_planes, uint32_t* flags,
-                        const uint32_t* group_start, const int32_t* members, cudaStream_t s, int* launches);
-// txt rows (trie / text-chunk kernels) from the pattern rows, on demand
-cudaError_t launch_txt_from_pat(const uint8_t* pat, int pat_stride, int64_t n, const LengthTable& lt, uint32_t* txt,
-                                cudaStream_t s, int* launches);
+// bit-plane rows of the rows in sorted order.  group_start != NULL (collapsed load): perm holds uids on entry and is
+// re-coded in place (the row of an unshared sequence, or kGroupFlag | uid)
+cudaError_t launch_pack(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths, int32_t* perm, int64_t n,
+                        void* planes, bool wide_planes, uint32_t* flags, const uint32_t* group_start,
+                        const int32_t* members, cudaStream_t s, int* launches);
+// pat rows (match masks) and txt rows of the trie / text-chunk kernels from the bit-plane rows, on demand
+cudaError_t launch_rows_from_planes(const void* planes, bool wide_planes, int64_t n, const LengthTable& lt, int pat_stride,
+                                    uint8_t* pat, uint32_t* txt, cudaStream_t s, int* launches);
 
 // trie.cu: prefix trie over the sorted texts (levels 1..kTrieDepth, all length buckets).
 //   lcp8        : scratch, uint8[round_up(n,16) + 16]
