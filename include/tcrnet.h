@@ -165,26 +165,26 @@ typedef struct tcrnet_stats {
                                   CTA of 256 patterns; prefix-trie kernel: one warp of 32)     */
     int64_t work_items_trie;   /* ... of which prefix-trie kernel                             */
     int64_t trie_nodes;        /* nodes of the prefix trie built by the last load             */
-    int32_t distance_passes;   /* 1, or 2 if the edge buffer had to grow                      */
+    int32_t distance_passes;   /* 1; 2 or 3 if the edge buffer / the join's verification queue had to grow */
     int32_t launches_load;     /* kernels launched by the last tcrnet_load[_device]           */
     int32_t launches_build;    /* kernels launched by the last tcrnet_build                   */
-    float ms_load;             /* device time of the last load (H2D copy + pack), CUDA events */
-    float ms_distance;         /* distance kernel(s) incl. emission                           */
+    /* times in ms from CUDA events on the context's stream; a field TCRNET_OPT_TIMING did not ask for reads 0 */
+    float ms_load;             /* device time of the last load (H2D copy + pack) [TIMING 2]   */
+    float ms_distance;         /* index + distance kernel(s) + emission / expansion [TIMING 2] */
     float ms_sort;             /* counting of caller-supplied keys (tcrnet_assemble), else ~0  */
-    float ms_csr;              /* row_ptr / col / degrees                                     */
-    float ms_build;            /* whole tcrnet_build on the device                            */
+    float ms_csr;              /* row_ptr / col / degrees [TIMING 2]                          */
+    float ms_build;            /* whole tcrnet_build on the device [TIMING 2]                 */
     int64_t n_distinct;        /* distinct sequences among the rows (= n when TCRNET_OPT_DEDUP
                                   is off or in the rectangular mode)                         */
-    float ms_kernel;           /* the distance kernel launches alone (CUDA events right around
-                                  them; ms_distance adds the schedule upload, the counter
-                                  resets and the expansion of collapsed pairs)               */
-    float ms_index;            /* segment join: building the segment index (inside ms_distance)  */
-    int64_t lane_columns_live; /* column steps of lanes whose pair was still undecided (COUNT_WORK;
-                                  join kernel; the trie / chunk kernels report warp-level counts)   */
+    float ms_kernel;           /* the distance kernel launches alone (events right around them: the join's
+                                  probe + verify kernels, or the trie / text-chunk kernels) [TIMING 1]  */
+    float ms_index;            /* segment join: building the segment index (inside ms_distance) [TIMING 2] */
+    int64_t lane_columns_live; /* unused (0)                                                     */
     int64_t join_probes;       /* segment join: directory look-ups (COUNT_WORK)                  */
     int64_t join_entries;      /* ... directory entries read (COUNT_WORK)                        */
-    int64_t join_candidates;   /* ... pairs handed to the recurrence / the l_max <= 1 check        */
-    int64_t work_items_join;   /* work items (32 patterns) of the join kernels                    */
+    int64_t join_candidates;   /* ... entries that passed the composition test: their rows were fetched and
+                                  the mismatch masks built (COUNT_WORK)                              */
+    int64_t work_items_join;   /* work items (32 patterns x one length difference) of the join      */
     int64_t join_index_entries;/* (text, segment) entries of the index                            */
     int32_t join_mode;         /* 0: not used, 1: join + banded verification (l_max >= 2), 2: join at l_max <= 1,
                                   where the verification is the XOR / prefix-suffix check                */

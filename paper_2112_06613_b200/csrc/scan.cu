@@ -165,11 +165,6 @@ cudaError_t exclusive_scan_i32_to_i64(const int32_t* in, int64_t* out, int64_t n
     return scan_impl<int32_t, int64_t>(in, out, n, write_total, scratch, s, launches);
 }
 
-cudaError_t exclusive_scan_u32(const uint32_t* in, uint32_t* out, int64_t n, void* scratch, cudaStream_t s,
-                               int* launches) {
-    return scan_impl<uint32_t, uint32_t>(in, out, n, false, scratch, s, launches);
-}
-
 cudaError_t exclusive_scan_u32_total(const uint32_t* in, uint32_t* out, int64_t n, void* scratch, cudaStream_t s,
                                      int* launches) {
     return scan_impl<uint32_t, uint32_t>(in, out, n, true, scratch, s, launches);

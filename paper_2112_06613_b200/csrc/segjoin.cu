@@ -382,7 +382,7 @@ __device__ __forceinline__ void drain_round(ProbeWarp<W, L, COUNT>& w, const Joi
     bool keep = false;
     if (act) {
         const PlaneRow<W> B = load_planes<W>(S.planes, t);
-        if (B.len == w.n) {  // (a tag collision across length buckets cannot pass the segment test below either)
+        if (B.len == w.n) {  // (an entry of another length bucket that shares the hash bucket cannot pass the segment test below either)
             W M[L + 1];
             band_masks_hoisted<L>(Ao, B, w.smin, w.NV, M);
             const int i = S.tab.probe_seg[w.delta][pi], d = S.tab.probe_shift[w.delta][pi];

@@ -157,8 +157,6 @@ int device_sm_count();
 size_t scan_scratch_bytes(int64_t n);
 cudaError_t exclusive_scan_i32_to_i64(const int32_t* in, int64_t* out, int64_t n, bool write_total,
                                       void* scratch, cudaStream_t s, int* launches);
-cudaError_t exclusive_scan_u32(const uint32_t* in, uint32_t* out, int64_t n, void* scratch,
-                               cudaStream_t s, int* launches);
 cudaError_t exclusive_scan_u32_total(const uint32_t* in, uint32_t* out /*[n+1]*/, int64_t n, void* scratch,
                                      cudaStream_t s, int* launches);
 
