@@ -35,8 +35,8 @@
 //           reaches the end of the pattern.  This IS the banded early exit of step A4: cells outside the band are
 //           never touched.  For l_max <= 1 it degenerates to the textbook check (equal lengths: at most one mismatch;
 //           one longer: common prefix + common suffix cover the shorter sequence - SURVEY 8(f) NEXT-4) and runs
-//           inline in the probe kernel; for l_max >= 2 the survivors are queued and k_join_verify runs it densely, one
-//           lane per survivor.
+//           inline in the probe kernel; for l_max >= 2 the survivors are queued and k_join_verify applies the once
+//           rule and then runs Landau-Vishkin densely, one lane per pair that is still there.
 #include <algorithm>
 
 #include "launch.cuh"
@@ -514,38 +514,72 @@ __global__ void __launch_bounds__(kJoinThreads, (L >= 2 ? 6 : 5)) k_join_probe(c
 }
 
 // ---- verify (l_max >= 2): one lane per surviving pair ----
+// Two steps, each at full lane occupancy: (1) every lane takes a queued pair and applies the *once* rule (most of the
+// queue are pairs found through several probes: only the first matching probe keeps its find); what is kept waits in a
+// per-warp shared-memory queue until (2) 32 pairs can run Landau-Vishkin together.
+template <typename W, int L>
+__device__ __forceinline__ bool verify_pair(const JoinParams& S, uint2 pt, int& m, int& n) {
+    const PlaneRow<W> A = load_planes<W>(S.planes, pt.x);
+    const PlaneRow<W> B = load_planes<W>(S.planes, pt.y);
+    m = A.len, n = B.len;
+    const int delta = n - m;
+    int smin, nb;
+    band_of(L, delta, smin, nb);
+    W M[L + 1];
+    band_masks<W, L>(A, B, m, n, smin, nb, M);
+    return lv_within<W, L>(M, m, n, delta, smin, nb);
+}
+
 template <typename W, int L, bool COUNT>
 __global__ void __launch_bounds__(kJoinThreads) k_join_verify(const __grid_constant__ JoinParams S) {
     grid_dependency_wait();
+    __shared__ uint2 kept[kJoinWarps][64];
     const DistanceParams& P = S.d;
-    const int lane = threadIdx.x & 31;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint2* q = kept[warp];
+    int qn = 0;
     const unsigned long long total = min(*S.cand_count, S.cand_cap);
     unsigned long long n_edges = 0, n_diag = 0;
+    auto lv_round = [&](int cnt) {  // the first cnt kept pairs, one per lane; the rest moves to the front
+        const bool act = lane < cnt;
+        const uint2 pt = act ? q[lane] : make_uint2(0u, 0u);
+        const bool mv = cnt + lane < qn;
+        const uint2 rest = mv ? q[cnt + lane] : make_uint2(0u, 0u);
+        __syncwarp();
+        if (mv) q[lane] = rest;
+        qn -= cnt;
+        __syncwarp();
+        int m = 0, n = 0;
+        const bool edge = act && verify_pair<W, L>(S, pt, m, n);
+        if (COUNT && edge) ++n_edges;
+        emit_edges(P, edge, lane, (int)pt.x, (int)pt.y, m, n);
+    };
     for (unsigned long long base = (unsigned long long)blockIdx.x * kJoinThreads; base < total;
          base += (unsigned long long)gridDim.x * kJoinThreads) {
         const unsigned long long c = base + threadIdx.x;
-        bool edge = false;
-        int p = 0, t = 0, m = 0, n = 0;
+        bool keep = false;
+        uint2 pt = make_uint2(0u, 0u);
         if (c < total) {
-            const uint2 pt = S.cand[c];
+            pt = S.cand[c];
             const int pi = (int)S.cand_probe[c];
-            p = (int)pt.x, t = (int)pt.y;
-            const PlaneRow<W> A = load_planes<W>(S.planes, p);
-            const PlaneRow<W> B = load_planes<W>(S.planes, t);
-            m = A.len, n = B.len;
-            const int delta = n - m;
+            const PlaneRow<W> A = load_planes<W>(S.planes, pt.x);
+            const PlaneRow<W> B = load_planes<W>(S.planes, pt.y);
+            const int m = A.len, n = B.len, delta = n - m;
             int smin, nb;
             band_of(L, delta, smin, nb);
             W M[L + 1];
             band_masks<W, L>(A, B, m, n, smin, nb, M);
             if (COUNT) n_diag += (unsigned long long)nb;
             // once: only the first probe whose segment matches keeps the pair
-            edge = first_matching_probe<W, L>(S.tab, M, smin, nb, m, n, delta, pi) &&
-                   lv_within<W, L>(M, m, n, delta, smin, nb);
-            if (COUNT && edge) ++n_edges;
+            keep = first_matching_probe<W, L>(S.tab, M, smin, nb, m, n, delta, pi);
         }
-        emit_edges(P, edge, lane, p, t, m, n);
+        const uint32_t bal = __ballot_sync(kFullMask, keep);
+        if (keep) q[qn + __popc(bal & ((1u << lane) - 1u))] = pt;
+        qn += __popc(bal);
+        __syncwarp();
+        if (qn >= 32) lv_round(32);
     }
+    if (qn > 0) lv_round(qn);
     if (COUNT) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
