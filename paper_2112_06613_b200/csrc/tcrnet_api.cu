@@ -573,7 +573,9 @@ int ensure_join_index(tcrnet_ctx* ctx, int l_max, int* launches) {
 // expand_only: the recorded pairs in keys_a are complete, only keys_b was too small - redo the expansion alone.
 // The counters and per-row counts a distance pass starts from (issued ahead of the index kernels for the first pass,
 // so that no memset sits between two kernels of the chain index -> join -> cliques -> expansion).
-int reset_build_counters(tcrnet_ctx* ctx, bool expand_only) {
+// On a collapsed load the cliques of the shared sequences (k_emit_cliques: they depend on the load alone) are emitted
+// from here on a second stream, next to the index / join kernels, and joined before the counts are read back.
+int reset_build_counters(tcrnet_ctx* ctx, bool expand_only, uint64_t cap_b, int shard, int n_shards, int* launches) {
     cudaStream_t s = ctx->stream;
     HostCtrl* dc = d_ctrl(ctx);
     static_assert(offsetof(HostCtrl, queue) == offsetof(HostCtrl, edge_count) + 9 * sizeof(unsigned long long), "one memset");
@@ -588,6 +590,15 @@ int reset_build_counters(tcrnet_ctx* ctx, bool expand_only) {
     }
     TRY_CUDA(cudaMemsetAsync(ctx->row_count.p, 0, sizeof(int32_t) * (size_t)ctx->n, s));
     TRY_CUDA(cudaMemsetAsync(ctx->deg.p, 0, sizeof(int32_t) * (size_t)ctx->n, s));
+    if (ctx->all.grouped) {
+        TRY_CUDA(cudaEventRecord(ctx->ev_fork, s));
+        TRY_CUDA(cudaStreamWaitEvent(ctx->side_stream, ctx->ev_fork, 0));
+        TRY_CUDA(launch_emit_cliques((const int32_t*)ctx->all.members.p, (const int32_t*)ctx->all.uid_of.p,
+                                     (const uint32_t*)ctx->all.group_start.p, ctx->n, (unsigned long long*)ctx->keys_b.p,
+                                     &dc->edge_total, cap_b, (int32_t*)ctx->row_count.p, (int32_t*)ctx->deg.p, shard, n_shards,
+                                     ctx->side_stream, launches));
+        TRY_CUDA(cudaEventRecord(ctx->ev_join, ctx->side_stream));
+    }
     return TCRNET_OK;
 }
 
@@ -598,7 +609,7 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
     static_assert(offsetof(HostCtrl, queue) == offsetof(HostCtrl, edge_count) + 9 * sizeof(unsigned long long), "one memset");
     static_assert(offsetof(HostCtrl, edge_total) == offsetof(HostCtrl, queue) + kTrieQueues * sizeof(unsigned long long), "one memset");
     static_assert(offsetof(HostCtrl, cand_count) == offsetof(HostCtrl, edge_total) + sizeof(unsigned long long), "one memset");
-    if (!counters_cleared) TRY(reset_build_counters(ctx, expand_only));
+    if (!counters_cleared) TRY(reset_build_counters(ctx, expand_only, cap_b, shard, n_shards, launches));
     int n_queues = 0;
     const WorkRow* d_rows = (const WorkRow*)ctx->rows.p;
     if (!expand_only) TRY_CUDA(rec(ctx, 4, 1));
@@ -655,17 +666,15 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
     }
     if (!expand_only) TRY_CUDA(rec(ctx, 5, 1));
     if (ctx->all.grouped) {
-        // the recorded pairs of distinct sequences -> edges between rows (keys_b), counted for the CSR step; the rows
-        // of every shared sequence are joined to each other (d = 0), each sequence by the shard uid mod n_shards
+        // the recorded pairs of distinct sequences -> edges between rows (keys_b), counted for the CSR step (the rows of
+        // every shared sequence are being joined to each other on the side stream: reset_build_counters)
         const uint32_t* gs = (const uint32_t*)ctx->all.group_start.p;
         const int32_t* mem = (const int32_t*)ctx->all.members.p;
-        TRY_CUDA(launch_emit_cliques(mem, (const int32_t*)ctx->all.uid_of.p, gs, ctx->n, (unsigned long long*)ctx->keys_b.p,
-                                     &dc->edge_total, cap_b, (int32_t*)ctx->row_count.p, (int32_t*)ctx->deg.p, shard, n_shards,
-                                     s, launches));
         TRY_CUDA(launch_expand_entries((const unsigned long long*)ctx->keys_a.p, &dc->edge_count, cap, gs, mem,
                                        (unsigned long long*)ctx->keys_b.p, &dc->edge_total, cap_b, (int32_t*)ctx->row_count.p,
                                        (int32_t*)ctx->deg.p, ctx->expand_huge.p, &dc->n_huge, kExpandHugeCap, ctx->n_sm, s,
                                        launches));
+        TRY_CUDA(cudaStreamWaitEvent(s, ctx->ev_join, 0));  // the cliques are in
         TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->edge_total, &dc->edge_total, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
     }
     TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->edge_count, &dc->edge_count, sizeof(unsigned long long) * 9,
@@ -711,7 +720,7 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
         TRY(dev_reserve(ctx, ctx->keys_b, sizeof(unsigned long long) * (size_t)cap_b));
     }
     // the first pass's resets go ahead of the index kernels: index -> join -> cliques -> expansion is one chain of kernels
-    TRY(reset_build_counters(ctx, false));
+    TRY(reset_build_counters(ctx, false, (uint64_t)cap_b, shard, n_shards, launches));
     bool counters_cleared = true;
     st.ms_index = 0.f;
     st.join_index_entries = 0;
@@ -893,6 +902,9 @@ int tcrnet_create(tcrnet_ctx** out, int device, void* cuda_stream, const tcrnet_
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, device);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->h_ctrl, sizeof(HostCtrl));
     for (int i = 0; e == cudaSuccess && i < 8; ++i) e = cudaEventCreate(&ctx->ev[i]);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming);
     if (e != cudaSuccess) {
         (void)cudaGetLastError();
         tcrnet_destroy(ctx);
@@ -910,6 +922,12 @@ void tcrnet_destroy(tcrnet_ctx* ctx) {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
+    if (ctx->side_stream) {
+        cudaStreamSynchronize(ctx->side_stream);
+        cudaStreamDestroy(ctx->side_stream);
+    }
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+    if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
     DevBuf* bufs[] = {&ctx->all.perm, &ctx->all.pat, &ctx->all.txt, &ctx->all.trie, &ctx->query.perm, &ctx->query.pat,
                       &ctx->query.txt, &ctx->query.trie, &ctx->all.planes, &ctx->query.planes, &ctx->join_cand, &ctx->expand_huge, &ctx->join_cnt, &ctx->join_dir,
                       &ctx->join_entries, &ctx->join_rows, &ctx->inv_perm, &ctx->edge_row, &ctx->edge_dist, &ctx->edge_dist_b, &ctx->flags,

@@ -114,6 +114,8 @@ struct tcrnet_ctx {
     DevBuf ctrl;               // device HostCtrl
     HostCtrl* h_ctrl = nullptr;  // pinned
     cudaEvent_t ev[8] = {};
+    cudaStream_t side_stream = nullptr;           // work that does not depend on the distance kernels runs beside them
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;  // (no timing: cheap)
     tcrnet_stats stats{};
 };
 
