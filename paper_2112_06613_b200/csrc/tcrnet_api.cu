@@ -170,6 +170,10 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
             e = cudaMemcpyAsync(set.perm.p, va, sizeof(int32_t), cudaMemcpyDeviceToDevice, s);
         set.lexicographic = lexicographic;
     }
+    if (e == cudaSuccess && code_groups && ctx->side_pending) {  // the member lists (dedup_rows, second stream) are in
+        e = cudaStreamWaitEvent(s, ctx->ev_join, 0);
+        ctx->side_pending = false;
+    }
     if (e == cudaSuccess)
         e = launch_pack(d_res, d_off, d_len, (int32_t*)set.perm.p, n, set.planes.p, set.wide_planes, &dc->flags,
                         code_groups ? (const uint32_t*)set.group_start.p : nullptr,
@@ -233,6 +237,15 @@ int ensure_text_tables(tcrnet_ctx* ctx, SeqSet& set, int* launches) {
     return TCRNET_OK;
 }
 
+// Work left on the second stream (dedup_rows forks the member lists there) is waited for on the host: used on the
+// paths where no kernel of the main stream will.
+void join_side_stream(tcrnet_ctx* ctx) {
+    if (ctx->side_pending) {
+        cudaStreamSynchronize(ctx->side_stream);
+        ctx->side_pending = false;
+    }
+}
+
 // Step A0 (dedup.cu): the distinct sequences of the rows.  On success *n_u of them, their lengths / residue
 // offsets in dd_len / dd_off, and in `set` the rows behind every distinct sequence.
 int dedup_rows(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* d_len, int64_t n, int64_t total_len,
@@ -270,12 +283,19 @@ int dedup_rows(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t
     TRY_CUDA(launch_dedup_groups((const int32_t*)ctx->dd_rep.p, rank, off, d_len, n, (int32_t*)set.uid_of.p, count,
                                  (int32_t*)ctx->dd_len.p, (int64_t*)ctx->dd_off.p, dc->hist_u, s, launches));
     // (... and the groups kernel the length histogram of the distinct sequences: the pack needs no round trip of its own)
-    // group_start over n + 1 counts (the tail is zero): entry n_u is the total = n
-    TRY_CUDA(exclusive_scan_u32_total(count, (uint32_t*)set.group_start.p, n + 1, ctx->scan_scratch.p, s, launches));
-    TRY_CUDA(launch_dedup_fill((const int32_t*)set.uid_of.p, n, (const uint32_t*)set.group_start.p, count,
-                               (int32_t*)set.members.p, &dc->clique_edges, s, launches));
-    TRY_CUDA(cudaMemcpyAsync(ctx->h_ctrl, dc, sizeof(HostCtrl), cudaMemcpyDeviceToHost, s));  // hist, hist_u, flags, clique_edges
+    TRY_CUDA(cudaMemcpyAsync(ctx->h_ctrl, dc, sizeof(HostCtrl), cudaMemcpyDeviceToHost, s));  // hist, hist_u, flags
     TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->n_distinct, rank + n, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+    // The member lists are not needed before the pack: they are filled on the second stream while the host reads the
+    // counts back and the sort of the distinct sequences runs (pack_set waits for ev_join before its pack kernel).
+    // group_start over n + 1 counts (the tail is zero): entry n_u is the total = n
+    TRY_CUDA(cudaEventRecord(ctx->ev_fork, s));
+    TRY_CUDA(cudaStreamWaitEvent(ctx->side_stream, ctx->ev_fork, 0));
+    TRY_CUDA(exclusive_scan_u32_total(count, (uint32_t*)set.group_start.p, n + 1, ctx->scan_scratch.p, ctx->side_stream,
+                                      launches));
+    TRY_CUDA(launch_dedup_fill((const int32_t*)set.uid_of.p, n, (const uint32_t*)set.group_start.p, count,
+                               (int32_t*)set.members.p, &dc->clique_edges, ctx->side_stream, launches));
+    TRY_CUDA(cudaEventRecord(ctx->ev_join, ctx->side_stream));
+    ctx->side_pending = true;
     TRY_CUDA(cudaStreamSynchronize(s));
     if (ctx->h_ctrl->flags & kFlagBadLength) return TCRNET_ERR_LENGTH;
     int64_t sum_len = 0;
@@ -287,7 +307,6 @@ int dedup_rows(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t
     // the header's contract: total_len = sum of the lengths (a shorter buffer would be read past its end by the
     // pack; the insert / lookup kernels above never touch a row that does not fit)
     if (sum_len != total_len) return TCRNET_ERR_ARG;
-    ctx->clique_edges = (int64_t)ctx->h_ctrl->clique_edges;
     *n_u = (int64_t)ctx->h_ctrl->n_distinct;
     if (*n_u < 1 || *n_u > n) return TCRNET_ERR_CUDA;
     return TCRNET_OK;
@@ -301,10 +320,15 @@ int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len
     const bool lex = rect || !ctx->early_exit || ctx->segment_join == 0;
     int64_t n_u = n;
     if (ctx->dedup && !rect && n >= 2) {
-        TRY(dedup_rows(ctx, ctx->all, d_res, d_len, n, total_len, &n_u, launches));
+        const int rc_dedup = dedup_rows(ctx, ctx->all, d_res, d_len, n, total_len, &n_u, launches);
+        if (rc_dedup != TCRNET_OK || n_u >= n) join_side_stream(ctx);  // (nothing will wait for the member lists)
+        TRY(rc_dedup);
         if (n_u < n) {
-            TRY(pack_set(ctx, ctx->all, d_res, (const int32_t*)ctx->dd_len.p, n_u, -1, (const int64_t*)ctx->dd_off.p,
-                         ctx->hist_u_host, true, lex, launches));
+            const int rc_pack = pack_set(ctx, ctx->all, d_res, (const int32_t*)ctx->dd_len.p, n_u, -1,
+                                         (const int64_t*)ctx->dd_off.p, ctx->hist_u_host, true, lex, launches);
+            join_side_stream(ctx);
+            TRY(rc_pack);
+            ctx->clique_edges = (int64_t)ctx->h_ctrl->clique_edges;  // (read back with the pack's flags)
             ctx->all.grouped = true;
             ctx->all.n_rows = n;
         }

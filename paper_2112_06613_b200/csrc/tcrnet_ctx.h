@@ -116,6 +116,7 @@ struct tcrnet_ctx {
     cudaEvent_t ev[8] = {};
     cudaStream_t side_stream = nullptr;           // work that does not depend on the distance kernels runs beside them
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;  // (no timing: cheap)
+    bool side_pending = false;                    // the load left work on side_stream that nothing has waited for yet
     tcrnet_stats stats{};
 };
 
