@@ -52,8 +52,8 @@ ORACLE_SAMPLE_ROWS = 1024
 NCU_DRAM_BYTES_PER_LAUNCH = {
     # (workload, kernel): bytes per step of that kernel / kernel pair - profiles/r2_join_ncu.txt
     ("cfg4", "k_join_probe"): 35_106_816 + 1_280,
-    ("cfg3", "k_join_probe + k_join_verify"): 11_112_448 + 26_624 + 11_567_616 + 17_920,
-    ("cfg5", "k_join_probe + k_join_verify"): 2_721_635_000 + 448_049_920 + 351_767_000 + 48_876_288,
+    ("cfg3", "k_join_probe + k_join_verify"): 11_111_936 + 10_752 + 11_591_936 + 13_056,
+    ("cfg5", "k_join_probe + k_join_verify"): 2_734_769_000 + 447_397_120 + 369_453_000 + 54_436_608,
 }
 
 
