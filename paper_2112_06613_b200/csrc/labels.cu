@@ -9,6 +9,7 @@
 // so an edge costs two 32-byte rows and ~25 instructions per column.  The first index of every edge
 // is written once per CSR by k_edge_rows (one thread per row) instead of a binary search per edge.
 // HBM/L2-bound: 2 plane rows read and 1 byte written per edge.
+#include "launch.cuh"
 #include "planes.cuh"
 #include "tcrnet_internal.h"
 
@@ -17,6 +18,7 @@ namespace {
 
 __global__ void __launch_bounds__(256) k_inverse_perm(const int32_t* __restrict__ perm, int64_t n,
                                                      int32_t* __restrict__ inv) {
+    grid_dependency_wait();
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (s < n) inv[perm[s]] = (int32_t)s;
 }
@@ -24,6 +26,7 @@ __global__ void __launch_bounds__(256) k_inverse_perm(const int32_t* __restrict_
 // edge_row[e] = first index of edge e (the row r with row_ptr[r] <= e < row_ptr[r+1])
 __global__ void __launch_bounds__(256) k_edge_rows(const int64_t* __restrict__ row_ptr, int64_t n,
                                                   int32_t* __restrict__ edge_row) {
+    grid_dependency_wait();
     const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= n) return;
     const int64_t b = row_ptr[r], e = row_ptr[r + 1];
@@ -59,6 +62,7 @@ __global__ void __launch_bounds__(256) k_edge_distances(const int32_t* __restric
                                                        const int32_t* __restrict__ col, int64_t n_edges,
                                                        const int32_t* __restrict__ inv_perm,
                                                        const void* __restrict__ planes, uint8_t* __restrict__ dist) {
+    grid_dependency_wait();
     const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= n_edges) return;
     const PlaneRow<W> A = load_planes<W>(planes, inv_perm[edge_row[e]]);
@@ -68,6 +72,7 @@ __global__ void __launch_bounds__(256) k_edge_distances(const int32_t* __restric
 
 __global__ void __launch_bounds__(256) k_restrict_flags(const uint8_t* __restrict__ dist, int64_t n_edges, int l_max,
                                                        uint32_t* __restrict__ flags) {
+    grid_dependency_wait();
     const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (e < n_edges) flags[e] = (int)dist[e] <= l_max ? 1u : 0u;
 }
@@ -79,6 +84,7 @@ __global__ void __launch_bounds__(256) k_restrict_compact(const int32_t* __restr
                                                          const uint32_t* __restrict__ pos,
                                                          unsigned long long* __restrict__ keys_out,
                                                          uint8_t* __restrict__ dist_out) {
+    grid_dependency_wait();
     const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= n_edges || !flags[e]) return;
     const unsigned long long u = (unsigned long long)(uint32_t)edge_row[e];
@@ -88,6 +94,7 @@ __global__ void __launch_bounds__(256) k_restrict_compact(const int32_t* __restr
 
 __global__ void __launch_bounds__(256) k_validate_keys(const unsigned long long* __restrict__ keys, int64_t n_keys,
                                                       int64_t n, uint32_t* __restrict__ flag) {
+    grid_dependency_wait();
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     bool bad = false;
     if (i < n_keys) {
@@ -103,14 +110,14 @@ inline unsigned grid_for(int64_t n) { return (unsigned)((n + 255) / 256); }
 }  // namespace
 
 cudaError_t launch_inverse_perm(const int32_t* perm, int64_t n, int32_t* inv, cudaStream_t s, int* launches) {
-    k_inverse_perm<<<grid_for(n), 256, 0, s>>>(perm, n, inv);
+    launch_dep(k_inverse_perm, grid_for(n), 256, 0, s, perm, n, inv);
     *launches += 1;
     return cudaGetLastError();
 }
 
 cudaError_t launch_edge_rows(const int64_t* row_ptr, int64_t n, int32_t* edge_row, cudaStream_t s, int* launches) {
     if (n <= 0) return cudaSuccess;
-    k_edge_rows<<<grid_for(n), 256, 0, s>>>(row_ptr, n, edge_row);
+    launch_dep(k_edge_rows, grid_for(n), 256, 0, s, row_ptr, n, edge_row);
     *launches += 1;
     return cudaGetLastError();
 }
@@ -118,8 +125,8 @@ cudaError_t launch_edge_rows(const int64_t* row_ptr, int64_t n, int32_t* edge_ro
 cudaError_t launch_edge_distances(const int32_t* edge_row, const int32_t* col, int64_t n_edges, const int32_t* inv_perm,
                                   const void* planes, bool wide_planes, uint8_t* dist, cudaStream_t s, int* launches) {
     if (n_edges <= 0) return cudaSuccess;
-    if (wide_planes) k_edge_distances<uint64_t><<<grid_for(n_edges), 256, 0, s>>>(edge_row, col, n_edges, inv_perm, planes, dist);
-    else k_edge_distances<uint32_t><<<grid_for(n_edges), 256, 0, s>>>(edge_row, col, n_edges, inv_perm, planes, dist);
+    if (wide_planes) launch_dep(k_edge_distances<uint64_t>, grid_for(n_edges), 256, 0, s, edge_row, col, n_edges, inv_perm, planes, dist);
+    else launch_dep(k_edge_distances<uint32_t>, grid_for(n_edges), 256, 0, s, edge_row, col, n_edges, inv_perm, planes, dist);
     *launches += 1;
     return cudaGetLastError();
 }
@@ -127,7 +134,7 @@ cudaError_t launch_edge_distances(const int32_t* edge_row, const int32_t* col, i
 cudaError_t launch_restrict_flags(const uint8_t* dist, int64_t n_edges, int l_max, uint32_t* flags, cudaStream_t s,
                                   int* launches) {
     if (n_edges <= 0) return cudaSuccess;
-    k_restrict_flags<<<grid_for(n_edges), 256, 0, s>>>(dist, n_edges, l_max, flags);
+    launch_dep(k_restrict_flags, grid_for(n_edges), 256, 0, s, dist, n_edges, l_max, flags);
     *launches += 1;
     return cudaGetLastError();
 }
@@ -136,7 +143,7 @@ cudaError_t launch_restrict_compact(const int32_t* edge_row, const int32_t* col,
                                     int64_t n_edges, const uint32_t* flags, const uint32_t* pos,
                                     unsigned long long* keys_out, uint8_t* dist_out, cudaStream_t s, int* launches) {
     if (n_edges <= 0) return cudaSuccess;
-    k_restrict_compact<<<grid_for(n_edges), 256, 0, s>>>(edge_row, col, dist, n_edges, flags, pos, keys_out, dist_out);
+    launch_dep(k_restrict_compact, grid_for(n_edges), 256, 0, s, edge_row, col, dist, n_edges, flags, pos, keys_out, dist_out);
     *launches += 1;
     return cudaGetLastError();
 }
@@ -144,7 +151,7 @@ cudaError_t launch_restrict_compact(const int32_t* edge_row, const int32_t* col,
 cudaError_t launch_validate_keys(const unsigned long long* keys, int64_t n_keys, int64_t n, uint32_t* flag,
                                  cudaStream_t s, int* launches) {
     if (n_keys <= 0) return cudaSuccess;
-    k_validate_keys<<<grid_for(n_keys), 256, 0, s>>>(keys, n_keys, n, flag);
+    launch_dep(k_validate_keys, grid_for(n_keys), 256, 0, s, keys, n_keys, n, flag);
     *launches += 1;
     return cudaGetLastError();
 }

@@ -9,6 +9,7 @@
 // the oracle's breadth-first search yields.  find() uses path halving with plain stores (a stale
 // parent is still an ancestor in the same tree, so races only cost extra hops); parent reads bypass
 // L1 (ld.global.cg) so that a CAS loser sees the winner's update.
+#include "launch.cuh"
 #include "tcrnet_internal.h"
 
 namespace tcrnet {
@@ -23,6 +24,7 @@ __device__ __forceinline__ bool node_alive(const int32_t* __restrict__ rank, int
 // ---- degree distribution -------------------------------------------------------------------
 
 __global__ void __launch_bounds__(256) k_max_degree(const int32_t* __restrict__ deg, int64_t n, int32_t* out) {
+    grid_dependency_wait();
     int32_t m = 0;
     for (int64_t u = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; u < n; u += (int64_t)gridDim.x * blockDim.x)
         m = max(m, deg[u]);
@@ -35,6 +37,7 @@ __global__ void __launch_bounds__(256) k_max_degree(const int32_t* __restrict__ 
 __global__ void __launch_bounds__(256) k_degree_hist(const int32_t* __restrict__ deg, int64_t n,
                                                     const int32_t* __restrict__ rank, int32_t threshold,
                                                     unsigned long long* __restrict__ hist) {
+    grid_dependency_wait();
     __shared__ uint32_t sh[kHistSmem];
     for (int i = threadIdx.x; i < kHistSmem; i += blockDim.x) sh[i] = 0u;
     __syncthreads();
@@ -56,6 +59,7 @@ __global__ void __launch_bounds__(256) k_degree_hist(const int32_t* __restrict__
 __global__ void __launch_bounds__(256) k_nn_sum(const int64_t* __restrict__ row_ptr, const int32_t* __restrict__ col,
                                                const int32_t* __restrict__ deg, int64_t n,
                                                unsigned long long* __restrict__ nn_sum) {
+    grid_dependency_wait();
     const int64_t u = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (u >= n) return;
     const int64_t b = row_ptr[u], e = row_ptr[u + 1];
@@ -73,6 +77,7 @@ __global__ void __launch_bounds__(256) k_nn_sum(const int64_t* __restrict__ row_
 __global__ void __launch_bounds__(256) k_class_sum(const int32_t* __restrict__ deg,
                                                   const unsigned long long* __restrict__ nn_sum, int64_t n,
                                                   unsigned long long* __restrict__ class_sum) {
+    grid_dependency_wait();
     __shared__ unsigned long long sh[kHistSmem];
     for (int i = threadIdx.x; i < kHistSmem; i += blockDim.x) sh[i] = 0ull;
     __syncthreads();
@@ -92,6 +97,7 @@ __global__ void __launch_bounds__(256) k_class_sum(const int32_t* __restrict__ d
 __global__ void __launch_bounds__(256) k_knn(const unsigned long long* __restrict__ class_sum,
                                             const unsigned long long* __restrict__ hist, int32_t hist_len,
                                             double* __restrict__ knn) {
+    grid_dependency_wait();
     const int d = blockIdx.x * blockDim.x + threadIdx.x;
     if (d >= hist_len) return;
     double v = 0.0;
@@ -131,6 +137,7 @@ __device__ __forceinline__ void cc_unite(int32_t* parent, int32_t a, int32_t b) 
 // parent[u] = u, count[u] = 0 (dead nodes too: they are simply never hooked or counted)
 __global__ void __launch_bounds__(256) k_cc_init(int64_t n, int32_t* __restrict__ parent, int32_t* __restrict__ count,
                                                 int32_t* __restrict__ sub_deg) {
+    grid_dependency_wait();
     const int64_t u = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (u >= n) return;
     parent[u] = (int32_t)u;
@@ -143,6 +150,7 @@ __global__ void __launch_bounds__(256) k_cc_init(int64_t n, int32_t* __restrict_
 __global__ void __launch_bounds__(256) k_cc_hook(const int64_t* __restrict__ row_ptr, const int32_t* __restrict__ col,
                                                 int64_t n, const int32_t* __restrict__ rank, int32_t threshold,
                                                 int32_t* parent, int32_t* __restrict__ sub_deg) {
+    grid_dependency_wait();
     const int64_t u = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (u >= n || !node_alive(rank, threshold, u)) return;
     const int64_t b = row_ptr[u], e = row_ptr[u + 1];
@@ -165,6 +173,7 @@ __global__ void __launch_bounds__(256) k_cc_label(int64_t n, const int32_t* __re
                                                  int32_t* parent, int32_t* __restrict__ label,
                                                  int32_t* __restrict__ count, unsigned long long* lcc,
                                                  unsigned long long* n_comp) {
+    grid_dependency_wait();
     const int64_t u = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool alive = u < n && node_alive(rank, threshold, u);
     int32_t root = -1;
@@ -186,6 +195,7 @@ __global__ void __launch_bounds__(256) k_cc_label(int64_t n, const int32_t* __re
 
 __global__ void __launch_bounds__(256) k_cc_sizes(int64_t n, const int32_t* __restrict__ label,
                                                  const int32_t* __restrict__ count, int32_t* __restrict__ comp_size) {
+    grid_dependency_wait();
     const int64_t u = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (u >= n) return;
     const int32_t r = label[u];
@@ -197,6 +207,7 @@ __global__ void __launch_bounds__(256) k_cc_sizes(int64_t n, const int32_t* __re
 // *flag |= 1 unless rank is a permutation of 0..n-1 (seen must be zeroed)
 __global__ void __launch_bounds__(256) k_check_permutation(const int32_t* __restrict__ rank, int64_t n,
                                                           uint32_t* __restrict__ seen, uint32_t* flag) {
+    grid_dependency_wait();
     const int64_t u = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (u >= n) return;
     const int32_t r = rank[u];
@@ -218,14 +229,14 @@ unsigned grid_capped(int64_t n) {
 }  // namespace
 
 cudaError_t launch_max_degree(const int32_t* deg, int64_t n, int32_t* out, cudaStream_t s, int* launches) {
-    k_max_degree<<<grid_capped(n), 256, 0, s>>>(deg, n, out);
+    launch_dep(k_max_degree, grid_capped(n), 256, 0, s, deg, n, out);
     *launches += 1;
     return cudaGetLastError();
 }
 
 cudaError_t launch_degree_hist(const int32_t* deg, int64_t n, const int32_t* rank, int32_t threshold,
                                unsigned long long* hist, cudaStream_t s, int* launches) {
-    k_degree_hist<<<grid_capped(n), 256, 0, s>>>(deg, n, rank, threshold, hist);
+    launch_dep(k_degree_hist, grid_capped(n), 256, 0, s, deg, n, rank, threshold, hist);
     *launches += 1;
     return cudaGetLastError();
 }
@@ -233,9 +244,9 @@ cudaError_t launch_degree_hist(const int32_t* deg, int64_t n, const int32_t* ran
 cudaError_t launch_neighbor_degree(const int64_t* row_ptr, const int32_t* col, const int32_t* deg, int64_t n,
                                    const unsigned long long* hist, int32_t hist_len, unsigned long long* nn_sum,
                                    unsigned long long* class_sum, double* knn, cudaStream_t s, int* launches) {
-    k_nn_sum<<<grid_for(n), 256, 0, s>>>(row_ptr, col, deg, n, nn_sum);
-    k_class_sum<<<grid_capped(n), 256, 0, s>>>(deg, nn_sum, n, class_sum);
-    k_knn<<<grid_for(hist_len), 256, 0, s>>>(class_sum, hist, hist_len, knn);
+    launch_dep(k_nn_sum, grid_for(n), 256, 0, s, row_ptr, col, deg, n, nn_sum);
+    launch_dep(k_class_sum, grid_capped(n), 256, 0, s, deg, nn_sum, n, class_sum);
+    launch_dep(k_knn, grid_for(hist_len), 256, 0, s, class_sum, hist, hist_len, knn);
     *launches += 3;
     return cudaGetLastError();
 }
@@ -243,23 +254,23 @@ cudaError_t launch_neighbor_degree(const int64_t* row_ptr, const int32_t* col, c
 cudaError_t launch_components(const int64_t* row_ptr, const int32_t* col, int64_t n, const int32_t* rank,
                               int32_t threshold, int32_t* parent, int32_t* count, int32_t* label, int32_t* sub_deg,
                               unsigned long long* lcc, unsigned long long* n_comp, cudaStream_t s, int* launches) {
-    k_cc_init<<<grid_for(n), 256, 0, s>>>(n, parent, count, sub_deg);
-    k_cc_hook<<<grid_for(n), 256, 0, s>>>(row_ptr, col, n, rank, threshold, parent, sub_deg);
-    k_cc_label<<<grid_for(n), 256, 0, s>>>(n, rank, threshold, parent, label, count, lcc, n_comp);
+    launch_dep(k_cc_init, grid_for(n), 256, 0, s, n, parent, count, sub_deg);
+    launch_dep(k_cc_hook, grid_for(n), 256, 0, s, row_ptr, col, n, rank, threshold, parent, sub_deg);
+    launch_dep(k_cc_label, grid_for(n), 256, 0, s, n, rank, threshold, parent, label, count, lcc, n_comp);
     *launches += 3;
     return cudaGetLastError();
 }
 
 cudaError_t launch_component_sizes(int64_t n, const int32_t* label, const int32_t* count, int32_t* comp_size,
                                    cudaStream_t s, int* launches) {
-    k_cc_sizes<<<grid_for(n), 256, 0, s>>>(n, label, count, comp_size);
+    launch_dep(k_cc_sizes, grid_for(n), 256, 0, s, n, label, count, comp_size);
     *launches += 1;
     return cudaGetLastError();
 }
 
 cudaError_t launch_check_permutation(const int32_t* rank, int64_t n, uint32_t* seen, uint32_t* flag, cudaStream_t s,
                                      int* launches) {
-    k_check_permutation<<<grid_for(n), 256, 0, s>>>(rank, n, seen, flag);
+    launch_dep(k_check_permutation, grid_for(n), 256, 0, s, rank, n, seen, flag);
     *launches += 1;
     return cudaGetLastError();
 }
