@@ -379,6 +379,68 @@ def test_low_complexity_sequences(pkg, oracle, alphabet, lo, hi):
             assert_same_network(got, want)
 
 
+@pytest.mark.parametrize("seed", range(6))
+def test_many_small_random_instances(pkg, oracle, seed):
+    """Forty small random inputs per seed - short strings (1..14 residues: segments of one residue, texts barely long
+    enough to be cut into l_max + 1 segments, buckets that stay with the text-chunk kernel), alphabets of 2..6 letters
+    (dense networks, many pairs found through several probes), a third of the rows repeated - at every threshold 0..5,
+    collapse on and off, against the tier-0 oracle."""
+    rng = np.random.default_rng(9000 + seed)
+    letters = "ACDEFGHIKLMNPQRSTVWY"
+    with pkg.TcrNet(0) as net, pkg.TcrNet(0) as net_rows:
+        net_rows.set_option(pkg.OPT_DEDUP, 0)
+        for _ in range(40):
+            k = int(rng.integers(2, 7))
+            alpha = [letters[i] for i in rng.choice(20, k, replace=False)]
+            lo = int(rng.integers(1, 6))
+            hi = lo + int(rng.integers(0, 10))
+            n = int(rng.integers(2, 180))
+            strings = ["".join(alpha[i] for i in rng.integers(0, k, int(rng.integers(lo, hi + 1)))) for _ in range(n)]
+            strings += [strings[i] for i in rng.integers(0, n, n // 3)]
+            res, ln = from_strings(strings)
+            for l_max in range(6):
+                want = oracle.network(res, ln, l_max, tier=0)[:3]
+                for ctx in (net, net_rows):
+                    ctx.load(res, ln)
+                    ctx.build(l_max)
+                    assert_same_network(ctx.copy_csr(), want)
+
+
+@pytest.mark.parametrize("seed", range(3))
+def test_many_small_random_instances_long_rows(pkg, oracle, seed):
+    """The same with rows of 20..64 residues (64-bit planes as soon as one row exceeds 32; pairs whose text is longer
+    than 32 while the pattern is not) and planted neighbours (1..5 random edits of an earlier row)."""
+    rng = np.random.default_rng(9100 + seed)
+    letters = "ACDEFGHIKLMNPQRSTVWY"
+    with pkg.TcrNet(0) as net:
+        for _ in range(25):
+            k = int(rng.integers(3, 21))
+            lo = int(rng.integers(20, 40))
+            hi = min(64, lo + int(rng.integers(0, 30)))
+            strings = []
+            for _ in range(int(rng.integers(5, 60))):
+                s0 = [letters[i] for i in rng.integers(0, k, int(rng.integers(lo, hi + 1)))]
+                strings.append("".join(s0))
+                for _ in range(int(rng.integers(0, 4))):
+                    t = list(s0)
+                    for _ in range(int(rng.integers(1, 6))):
+                        q = int(rng.integers(0, len(t)))
+                        op = int(rng.integers(0, 3))
+                        if op == 0:
+                            t[q] = letters[int(rng.integers(0, k))]
+                        elif op == 1 and len(t) < 64:
+                            t.insert(q, letters[int(rng.integers(0, k))])
+                        elif op == 2 and len(t) > 1:
+                            del t[q]
+                    strings.append("".join(t))
+            res, ln = from_strings(strings)
+            for l_max in range(6):
+                want = oracle.network(res, ln, l_max, tier=0)[:3]
+                net.load(res, ln)
+                net.build(l_max)
+                assert_same_network(net.copy_csr(), want)
+
+
 def test_length_64_and_all_26_letters(pkg, oracle):
     rng = np.random.default_rng(5)
     letters = "ABCDEFGHIJKLMNOPQRSTUVWXYZ"
