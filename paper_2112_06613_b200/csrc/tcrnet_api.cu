@@ -312,6 +312,8 @@ int dedup_rows(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t
     return TCRNET_OK;
 }
 
+int build_join_index_ahead(tcrnet_ctx* ctx, int* launches);
+
 int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len, int64_t n, int64_t total_len,
                      int* launches) {
     const bool rect = ctx->n_query > 0 && ctx->n_query < n;
@@ -348,6 +350,7 @@ int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len
     ctx->stats.max_len = ctx->all.max_len;
     ctx->stats.trie_nodes = 0;  // (built on demand: ensure_text_tables)
     ctx->loaded = true;
+    TRY(build_join_index_ahead(ctx, launches));
     return TCRNET_OK;
 }
 
@@ -562,32 +565,71 @@ int upload_schedule(tcrnet_ctx* ctx, const Schedule& sch) {
     return TCRNET_OK;
 }
 
-// Segment index of the texts of ctx->all for threshold l_max (kept until the next load / another threshold).
-int ensure_join_index(tcrnet_ctx* ctx, int l_max, int* launches) {
-    tcrnet_stats& st = ctx->stats;
-    st.ms_index = 0.f;
-    const SeqSet& set = ctx->all;
+// (entries of the index of `set` for threshold l_max)
+int64_t join_index_entries(const SeqSet& set, int l_max) {
     const int k = l_max + 1;
     int64_t n_idx = 0;
     for (int l = k; l < kNumLen; ++l) n_idx += set.hist[l] * k;
-    st.join_index_entries = n_idx;
-    if (ctx->join_l_max == l_max) return TCRNET_OK;
-    cudaStream_t s = ctx->stream;
+    return n_idx;
+}
+
+// The index kernels on stream s (prefix sum in `scan_scratch`, which nothing else may use meanwhile).
+int build_join_index(tcrnet_ctx* ctx, int l_max, cudaStream_t s, DevBuf& scan_scratch, int* launches) {
+    const SeqSet& set = ctx->all;
+    const int64_t n_idx = join_index_entries(set, l_max);
     make_join_tables(l_max, ctx->join_tab);
     uint32_t slots = 1024;
     while ((int64_t)slots < 2 * n_idx && slots < (1u << 30)) slots <<= 1;
     TRY(dev_reserve(ctx, ctx->join_cnt, sizeof(uint32_t) * (size_t)slots));
     TRY(dev_reserve(ctx, ctx->join_dir, sizeof(uint32_t) * ((size_t)slots + 1)));
     TRY(dev_reserve(ctx, ctx->join_entries, sizeof(uint2) * (size_t)std::max<int64_t>(n_idx, 1)));
-    TRY(dev_reserve(ctx, ctx->scan_scratch, scan_scratch_bytes((int64_t)slots)));
-    TRY_CUDA(rec(ctx, 6, 2));
+    TRY(dev_reserve(ctx, scan_scratch, scan_scratch_bytes((int64_t)slots)));
     TRY_CUDA(cudaMemsetAsync(ctx->join_cnt.p, 0, sizeof(uint32_t) * (size_t)slots, s));
     TRY_CUDA(launch_join_index(set.planes.p, set.wide_planes, set.lt, set.n, ctx->join_tab,
                                (uint32_t*)ctx->join_cnt.p, (uint32_t*)ctx->join_dir.p, (uint2*)ctx->join_entries.p, slots,
-                               ctx->scan_scratch.p, s, launches));
-    TRY_CUDA(rec(ctx, 7, 2));
+                               scan_scratch.p, s, launches));
     ctx->join_slots = slots;
     ctx->join_l_max = l_max;
+    return TCRNET_OK;
+}
+
+// Whatever the load left running on the second stream (the index built ahead, below) is ordered before the main
+// stream's next operation.
+int settle_index(tcrnet_ctx* ctx) {
+    if (ctx->index_pending) {
+        TRY_CUDA(cudaStreamWaitEvent(ctx->stream, ctx->ev_index, 0));
+        ctx->index_pending = false;
+    }
+    return TCRNET_OK;
+}
+
+// Built AHEAD: a load ends with a host synchronisation and the build that follows starts with host work (schedule,
+// reservations); the index depends on the load and on l_max alone, so the load starts building it on the second stream
+// for the threshold of the previous build (the usual case: the same threshold again) and returns without waiting.
+// A build at another threshold waits for it and builds its own.
+int build_join_index_ahead(tcrnet_ctx* ctx, int* launches) {
+    const int l_max = ctx->ahead_l_max;
+    const bool join_on = ctx->early_exit && ctx->segment_join != 0;  // (ahead_l_max: a build did use the join)
+    // (timing level 2 measures the phases one after the other: nothing is built ahead there)
+    if (l_max < 0 || l_max > kTrieMaxL || !join_on || ctx->timing >= 2) return TCRNET_OK;
+    if (join_index_entries(ctx->all, l_max) == 0) return TCRNET_OK;
+    TRY(build_join_index(ctx, l_max, ctx->side_stream, ctx->join_scan_scratch, launches));
+    TRY_CUDA(cudaEventRecord(ctx->ev_index, ctx->side_stream));
+    ctx->index_pending = true;
+    return TCRNET_OK;
+}
+
+// Segment index of the texts of ctx->all for threshold l_max (kept until the next load / another threshold).
+int ensure_join_index(tcrnet_ctx* ctx, int l_max, int* launches) {
+    tcrnet_stats& st = ctx->stats;
+    st.ms_index = 0.f;
+    st.join_index_entries = join_index_entries(ctx->all, l_max);
+    TRY(settle_index(ctx));
+    ctx->ahead_l_max = l_max;
+    if (ctx->join_l_max == l_max) return TCRNET_OK;
+    TRY_CUDA(rec(ctx, 6, 2));
+    TRY(build_join_index(ctx, l_max, ctx->stream, ctx->scan_scratch, launches));
+    TRY_CUDA(rec(ctx, 7, 2));
     if (ctx->timing >= 2) st.ms_index = -1.f;  // measured once the events have completed (distance_phase)
     return TCRNET_OK;
 }
@@ -929,6 +971,7 @@ int tcrnet_create(tcrnet_ctx** out, int device, void* cuda_stream, const tcrnet_
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_index, cudaEventDisableTiming);
     if (e != cudaSuccess) {
         (void)cudaGetLastError();
         tcrnet_destroy(ctx);
@@ -952,8 +995,9 @@ void tcrnet_destroy(tcrnet_ctx* ctx) {
     }
     if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
     if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
+    if (ctx->ev_index) cudaEventDestroy(ctx->ev_index);
     DevBuf* bufs[] = {&ctx->all.perm, &ctx->all.pat, &ctx->all.txt, &ctx->all.trie, &ctx->query.perm, &ctx->query.pat,
-                      &ctx->query.txt, &ctx->query.trie, &ctx->all.planes, &ctx->query.planes, &ctx->join_cand, &ctx->expand_huge, &ctx->join_cnt, &ctx->join_dir,
+                      &ctx->query.txt, &ctx->query.trie, &ctx->all.planes, &ctx->query.planes, &ctx->join_cand, &ctx->expand_huge, &ctx->join_scan_scratch, &ctx->join_cnt, &ctx->join_dir,
                       &ctx->join_entries, &ctx->join_rows, &ctx->inv_perm, &ctx->edge_row, &ctx->edge_dist, &ctx->edge_dist_b, &ctx->flags,
                       &ctx->flag_pos, &ctx->in_res, &ctx->in_len, &ctx->offsets,
                       &ctx->perm_tmp, &ctx->trie_scratch, &ctx->keys_a, &ctx->keys_b, &ctx->radix_scratch,
@@ -975,6 +1019,7 @@ int tcrnet_load_device(tcrnet_ctx* ctx, const uint8_t* residues_dev, const int32
                        int64_t total_len) {
     if (!ctx || !residues_dev || !lengths_dev || n < 1 || n > 0x7ffffffeLL || total_len < n) return TCRNET_ERR_ARG;
     TRY_CUDA(cudaSetDevice(ctx->device));
+    TRY(settle_index(ctx));  // (an index still being built ahead reads the tables this load rewrites)
     drop_load(ctx);
     int launches = 0;
     TRY_CUDA(rec(ctx, 0, 2));
@@ -992,6 +1037,7 @@ int tcrnet_load_device(tcrnet_ctx* ctx, const uint8_t* residues_dev, const int32
 int tcrnet_load(tcrnet_ctx* ctx, const uint8_t* residues, const int32_t* lengths, int64_t n) {
     if (!ctx || !residues || !lengths || n < 1 || n > 0x7ffffffeLL) return TCRNET_ERR_ARG;
     TRY_CUDA(cudaSetDevice(ctx->device));
+    TRY(settle_index(ctx));
     drop_load(ctx);
     // The lengths go first: their copy runs while the host pass below sizes the residue copy (validation proper
     // happens on the device; this pass only keeps the sum meaningful).

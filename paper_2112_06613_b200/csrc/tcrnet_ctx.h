@@ -98,7 +98,7 @@ struct tcrnet_ctx {
     DevBuf edge_row;  // first index of every edge of the current CSR (labels.cu; valid with edge_dist)
     DevBuf inv_perm, edge_dist, edge_dist_b, flags, flag_pos;
     // segment join (segjoin.cu): directory + entries of the current load for join_l_max, work rows
-    DevBuf join_cnt, join_dir, join_entries, join_rows, join_cand;
+    DevBuf join_cnt, join_dir, join_entries, join_rows, join_cand, join_scan_scratch;
     int64_t join_cand_cap = 0;  // pairs the verification queue join_cand holds (uint2[cap] followed by uint8[cap])
     int join_l_max = -1;  // threshold the index in join_dir / join_entries was built for (-1: none)
     uint32_t join_slots = 0;
@@ -116,6 +116,9 @@ struct tcrnet_ctx {
     cudaEvent_t ev[8] = {};
     cudaStream_t side_stream = nullptr;           // work that does not depend on the distance kernels runs beside them
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;  // (no timing: cheap)
+    cudaEvent_t ev_index = nullptr;               // the index built ahead by the load (second stream) is complete
+    bool index_pending = false;                   // ... and nothing on the main stream has waited for it yet
+    int ahead_l_max = -1;                         // threshold of the last build that used the join (-1: none yet)
     bool side_pending = false;                    // the load left work on side_stream that nothing has waited for yet
     tcrnet_stats stats{};
 };
