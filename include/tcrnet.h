@@ -228,6 +228,14 @@ TCRNET_API void tcrnet_destroy(tcrnet_ctx* ctx);
 TCRNET_API int tcrnet_load(tcrnet_ctx* ctx, const uint8_t* residues, const int32_t* lengths, int64_t n);
 
 /*
+ * tcrnet_load for a caller that knows the size of its residue array but has not summed the lengths (a binding that
+ * was handed two arrays): residues_size >= sum(lengths) is checked block by block as the lengths are read, and no
+ * byte at or beyond residues_size is ever read - TCRNET_ERR_ARG instead.  Everything else as tcrnet_load.
+ */
+TCRNET_API int tcrnet_load_sized(tcrnet_ctx* ctx, const uint8_t* residues, int64_t residues_size,
+                                 const int32_t* lengths, int64_t n);
+
+/*
  * Same as tcrnet_load with both arrays already in device memory (ordered on the context's
  * stream).  total_len must equal sum(lengths); it sizes the residue array.
  * The arrays are borrowed for the duration of the call only (they are re-laid out into

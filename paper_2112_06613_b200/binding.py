@@ -24,7 +24,8 @@ OPT_EARLY_EXIT, OPT_FIRST_CHECK, OPT_EDGE_CAPACITY, OPT_EDGE_LIMIT, OPT_COUNT_WO
 OPT_PREFIX_TRIE, OPT_TRIE_CHUNK, OPT_N_QUERY, OPT_DEDUP, OPT_SEGMENT_JOIN, OPT_FAST_L1, OPT_TIMING = 7, 8, 9, 10, 11, 12, 13
 
 EXPORTS = (
-    "tcrnet_create", "tcrnet_destroy", "tcrnet_load", "tcrnet_load_device", "tcrnet_build", "tcrnet_csr",
+    "tcrnet_create", "tcrnet_destroy", "tcrnet_load", "tcrnet_load_sized", "tcrnet_load_device", "tcrnet_build",
+    "tcrnet_csr",
     "tcrnet_degrees", "tcrnet_copy_csr", "tcrnet_set_option", "tcrnet_get_stats", "tcrnet_probe_int32",
     "tcrnet_last_cuda_error", "tcrnet_strerror", "tcrnet_version", "tcrnet_build_shard", "tcrnet_assemble",
     "tcrnet_edge_distances", "tcrnet_restrict", "tcrnet_degree_histogram", "tcrnet_neighbor_degree",
@@ -82,6 +83,8 @@ def load_library() -> C.CDLL:
     lib.tcrnet_destroy.argtypes = [vp]
     lib.tcrnet_load.restype = C.c_int
     lib.tcrnet_load.argtypes = [vp, u8p, i32p, C.c_int64]
+    lib.tcrnet_load_sized.restype = C.c_int
+    lib.tcrnet_load_sized.argtypes = [vp, u8p, C.c_int64, i32p, C.c_int64]
     lib.tcrnet_load_device.restype = C.c_int
     lib.tcrnet_load_device.argtypes = [vp, vp, vp, C.c_int64, C.c_int64]
     lib.tcrnet_build.restype = C.c_int
@@ -197,7 +200,7 @@ class TcrNet:
 
     # -- the calls of tcrnet.h -------------------------------------------------------------
     def load(self, residues, lengths) -> None:
-        """tcrnet_load (host numpy arrays) or tcrnet_load_device (CUDA torch tensors)."""
+        """tcrnet_load_sized (host numpy arrays) or tcrnet_load_device (CUDA torch tensors)."""
         torch = self._torch
         if isinstance(residues, torch.Tensor):
             assert residues.is_cuda and lengths.is_cuda, "device load needs CUDA tensors"
@@ -211,13 +214,10 @@ class TcrNet:
             residues = np.ascontiguousarray(residues, dtype=np.uint8)
             lengths = np.ascontiguousarray(lengths, dtype=np.int32)
             n = int(lengths.size)
-            # Exact for valid lengths (1..64); invalid ones are rejected by the library before it reads a residue,
-            # so the 32-bit accumulator (vectorised: this sum is on the end-to-end path) may wrap for them.
-            total = int(np.add.reduce(lengths, dtype=np.int32)) if n <= (1 << 25) else int(lengths.sum(dtype=np.int64))
-            if n >= 1 and total > residues.size:
-                raise TcrNetError(ERR_ARG, "tcrnet_load (residues shorter than sum(lengths))")
-            _check(self._lib.tcrnet_load(self._ctx, residues.ctypes.data_as(C.POINTER(C.c_uint8)),
-                                         lengths.ctypes.data_as(C.POINTER(C.c_int32)), n), "tcrnet_load")
+            # (tcrnet_load_sized checks sum(lengths) <= residues.size as it reads the lengths: no pass over them here)
+            _check(self._lib.tcrnet_load_sized(self._ctx, residues.ctypes.data_as(C.POINTER(C.c_uint8)),
+                                               int(residues.size), lengths.ctypes.data_as(C.POINTER(C.c_int32)), n),
+                   "tcrnet_load")
         self.n = n
         self.n_edges = 0
 

@@ -1035,12 +1035,19 @@ int tcrnet_load_device(tcrnet_ctx* ctx, const uint8_t* residues_dev, const int32
 }
 
 int tcrnet_load(tcrnet_ctx* ctx, const uint8_t* residues, const int32_t* lengths, int64_t n) {
-    if (!ctx || !residues || !lengths || n < 1 || n > 0x7ffffffeLL) return TCRNET_ERR_ARG;
+    return tcrnet_load_sized(ctx, residues, INT64_MAX, lengths, n);
+}
+
+int tcrnet_load_sized(tcrnet_ctx* ctx, const uint8_t* residues, int64_t residues_size, const int32_t* lengths,
+                      int64_t n) {
+    if (!ctx || !residues || !lengths || n < 1 || n > 0x7ffffffeLL || residues_size < n) return TCRNET_ERR_ARG;
     TRY_CUDA(cudaSetDevice(ctx->device));
     TRY(settle_index(ctx));
     drop_load(ctx);
-    // The lengths go first: their copy runs while the host pass below sizes the residue copy (validation proper
-    // happens on the device; this pass only keeps the sum meaningful).
+    // The lengths go first.  The residue array is sized by their sum, which only a host pass over them gives: that pass
+    // runs in blocks of rows and, as long as the buffer of the previous load is large enough, the residues of every
+    // finished block are copied at once - the pass hides behind the copies instead of preceding them (config 4: 0.25 ms
+    // of a 0.9 ms load).  Validation proper happens on the device; this pass only keeps the sum meaningful.
     DevBuf& d_res = ctx->in_res;
     DevBuf& d_len = ctx->in_len;
     cudaStream_t s = ctx->stream;
@@ -1048,21 +1055,46 @@ int tcrnet_load(tcrnet_ctx* ctx, const uint8_t* residues, const int32_t* lengths
     if (rc != TCRNET_OK) return rc;
     TRY_CUDA(rec(ctx, 0, 2));
     TRY_CUDA(cudaMemcpyAsync(d_len.p, lengths, sizeof(int32_t) * (size_t)n, cudaMemcpyHostToDevice, s));
-    int64_t total_len = 0;
+    constexpr int64_t kBlockRows = 1 << 16, kInner = 4096;  // (4096 x kMaxLen fits 32 bits: the inner sums vectorise)
+    int64_t total_len = 0, copied = 0;
     uint32_t bad = 0;
-    for (int64_t i = 0; i < n; ++i) {
-        const int32_t l = lengths[i];
-        bad |= (uint32_t)(l - 1) >= (uint32_t)kMaxLen;
-        total_len += l;
+    bool too_short = false;
+    cudaError_t ce = cudaSuccess;
+    for (int64_t b0 = 0; b0 < n && !bad && !too_short && ce == cudaSuccess; b0 += kBlockRows) {
+        const int64_t b1 = std::min<int64_t>(n, b0 + kBlockRows);
+        for (int64_t i0 = b0; i0 < b1; i0 += kInner) {
+            const int64_t i1 = std::min<int64_t>(b1, i0 + kInner);
+            uint32_t sum = 0, any = 0;
+            for (int64_t i = i0; i < i1; ++i) {
+                const uint32_t l = (uint32_t)lengths[i];
+                sum += l;
+                any |= l - 1u;
+            }
+            bad |= any & ~(uint32_t)(kMaxLen - 1);  // some l - 1 >= kMaxLen (kMaxLen is a power of two)
+            total_len += sum;
+        }
+        too_short = !bad && total_len > residues_size;  // (checked before a byte of the block is read)
+        if (!bad && !too_short && d_res.p && (size_t)total_len <= d_res.bytes && total_len > copied) {
+            ce = cudaMemcpyAsync((uint8_t*)d_res.p + copied, residues + copied, (size_t)(total_len - copied),
+                                 cudaMemcpyHostToDevice, s);
+            copied = total_len;
+        }
     }
-    if (bad) {
-        cudaStreamSynchronize(s);  // the host array is borrowed for this call only
-        return TCRNET_ERR_LENGTH;
+    static_assert((kMaxLen & (kMaxLen - 1)) == 0, "length check above");
+    if (bad || too_short || ce != cudaSuccess) {
+        cudaStreamSynchronize(s);  // the host arrays are borrowed for this call only
+        if (ce != cudaSuccess) ctx->last_cuda = (int)ce, (void)cudaGetLastError();
+        return bad ? TCRNET_ERR_LENGTH : too_short ? TCRNET_ERR_ARG : TCRNET_ERR_CUDA;
+    }
+    if (copied < total_len && (!d_res.p || d_res.bytes < (size_t)total_len)) {
+        if (copied) cudaStreamSynchronize(s);  // (copies into the buffer that is replaced)
+        copied = 0;
     }
     rc = dev_reserve(ctx, d_res, (size_t)total_len);
     int launches = 0;
-    if (rc == TCRNET_OK) {
-        cudaError_t e = cudaMemcpyAsync(d_res.p, residues, (size_t)total_len, cudaMemcpyHostToDevice, s);
+    if (rc == TCRNET_OK && copied < total_len) {
+        cudaError_t e = cudaMemcpyAsync((uint8_t*)d_res.p + copied, residues + copied, (size_t)(total_len - copied),
+                                        cudaMemcpyHostToDevice, s);
         if (e != cudaSuccess) {
             ctx->last_cuda = (int)e;
             (void)cudaGetLastError();

@@ -549,6 +549,37 @@ def test_device_side_validation(pkg):
                     assert e.value.status == pkg.ERR_ARG
 
 
+def test_host_loads_reuse_the_buffers_of_the_previous_load(pkg):
+    """tcrnet_load[_sized] copies the residues block by block while it sums the lengths whenever the buffer left by the
+    previous load is large enough: a small load, a larger one (the buffer grows), the same again (copied in several
+    blocks: N > 65,536 rows), a smaller one - each equal to the network of a fresh context.  A residue array shorter
+    than sum(lengths) is refused without being read past its end; the four-argument tcrnet_load gives the same."""
+    import ctypes as C
+    small, large = generate("cfg1"), generate("cfg3")
+    want = {id(d): gpu_network(pkg, d.residues, d.lengths, 1)[0] for d in (small, large)}
+    with pkg.TcrNet(0) as net:
+        for d in (small, large, large, small, large):
+            net.load(d.residues, d.lengths)
+            net.build(1)
+            assert_same_network(net.copy_csr(), want[id(d)])
+            with pytest.raises(pkg.TcrNetError) as e:
+                net.load(d.residues[:-1], d.lengths)
+            assert e.value.status == pkg.ERR_ARG
+        r = np.ascontiguousarray(large.residues)
+        ln = np.ascontiguousarray(large.lengths)
+        rc = net._lib.tcrnet_load(net._ctx, r.ctypes.data_as(C.POINTER(C.c_uint8)),
+                                  ln.ctypes.data_as(C.POINTER(C.c_int32)), int(ln.size))
+        assert rc == pkg.OK
+        net.n = int(ln.size)
+        net.build(1)
+        assert_same_network(net.copy_csr(), want[id(large)])
+        bad = ln.copy()
+        bad[150_000] = 65
+        with pytest.raises(pkg.TcrNetError) as e:
+            net.load(r, bad)
+        assert e.value.status == pkg.ERR_LENGTH
+
+
 # ------------------------------------------------------------------ BASELINE.json's large configs
 def _sampled_parity(pkg, oracle, name, l_max, n_sample, seed, opts=None):
     """What the oracle cannot compute in full: (i) the FULL neighbourhoods of n_sample uniformly drawn nodes (drawn from
