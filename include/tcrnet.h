@@ -106,7 +106,7 @@ typedef enum tcrnet_option {
                                      n_q > 0: rows 0..n_q-1 of the next tcrnet_load are the query
                                      rows and builds keep only the edges with at least one query
                                      endpoint (query-query and query-repertoire).  Through the segment
-                                     join (l_max <= 4) all candidate pairs are decided and the others
+                                     join (l_max <= 6) all candidate pairs are decided and the others
                                      dropped at emission; the trie / text-chunk kernels never evaluate a
                                      pair of two non-query rows.  0 (default): all pairs.
                                      Takes effect at the next tcrnet_load.                      */
@@ -122,7 +122,7 @@ typedef enum tcrnet_option {
                                      at most the edits allow, with every sequence within l_max of it; only
                                      pairs found through a hash index of the segments are verified (banded,
                                      Landau-Vishkin on per-diagonal mismatch masks).  -1 (default): used for
-                                     l_max <= 4 (all-pairs mode, early exit on, TCRNET_OPT_PREFIX_TRIE on); 1: the
+                                     l_max <= 6 (all-pairs mode, early exit on, TCRNET_OPT_PREFIX_TRIE on); 1: the
                                      same regardless of TCRNET_OPT_PREFIX_TRIE; 0: never (every length-compatible
                                      pair is visited through the prefix trie / text-chunk kernels).  Never changes
                                      the result.  Set it BEFORE tcrnet_load: a load made with 0 sorts the
@@ -213,7 +213,8 @@ TCRNET_API void tcrnet_destroy(tcrnet_ctx* ctx);
  * length and row; by length, first six residues and row when TCRNET_OPT_SEGMENT_JOIN = 0, the rectangular
  * mode or TCRNET_OPT_EARLY_EXIT = 0 announce the prefix-trie kernel); permutation; per sorted position one
  * bit-plane row (5-bit residue codes, one bit of the code per word, 32 bytes up to 32 residues).  The byte / word
- * rows and the prefix trie of the trie / text-chunk kernels are built by the first build that needs them.  PAPER.md:326 ("each a.a. is saved as a number ... BYTE"), north_star (1).
+ * rows and the prefix trie of the trie / text-chunk kernels are built by the first build that needs them.
+ * PAPER.md:326 ("each a.a. is saved as a number ... BYTE"), north_star (1).
  *
  *   residues  host, uint8[sum(lengths)]: the rows concatenated, ASCII 'A'..'Z' (any of the 26
  *             letters is a legal residue; only equality matters - DESIGN.md reading Q8)
@@ -247,7 +248,7 @@ TCRNET_API int tcrnet_load_device(tcrnet_ctx* ctx, const uint8_t* residues_dev, 
 /*
  * Steps A2-A6: decide, for every unordered pair of rows, whether its Levenshtein distance
  * is <= l_max, and assemble CSR + degrees on the device.  Pairs with
- * |len_i - len_j| > l_max are never touched; for l_max <= 4 (default path) only pairs that share one of the
+ * |len_i - len_j| > l_max are never touched; for l_max <= 6 (default path) only pairs that share one of the
  * l_max + 1 segments of the longer sequence are looked at (every pair within l_max does: pigeonhole) and decided
  * exactly by a banded bit-parallel verification; otherwise every length-compatible pair goes through the
  * bit-parallel column recurrence with an exact early exit (TCRNET_OPT_SEGMENT_JOIN).  The result is the same on

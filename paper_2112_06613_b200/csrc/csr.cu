@@ -174,9 +174,11 @@ cudaError_t launch_csr_unsorted(const unsigned long long* keys, int64_t n_keys, 
     if (e == cudaSuccess) e = exclusive_scan_i32_to_i64(row_count, row_ptr, n, true, scan_scratch, s, launches);
     if (e != cudaSuccess || n_keys <= 0) return e;
     const int64_t blocks = (n_keys + 255) / 256;
-    launch_dep(k_scatter_keys, (unsigned)std::min<int64_t>(blocks, device_sm_count() * 32), 256, 0, s, keys, n_keys, row_ptr, row_count, bucket);
+    launch_dep(k_scatter_keys, (unsigned)std::min<int64_t>(blocks, device_sm_count() * 32), 256, 0, s, keys, n_keys,
+               row_ptr, row_count, bucket);
     launch_dep(k_rank_rows, (unsigned)blocks, 256, 0, s, bucket, n_keys, row_ptr, col, deg, long_rows, n_long);
-    launch_dep(k_sort_long_rows, (unsigned)std::min<int64_t>(n, device_sm_count() * 4), 256, 0, s, row_ptr, bucket, col, long_rows, n_long);
+    launch_dep(k_sort_long_rows, (unsigned)std::min<int64_t>(n, device_sm_count() * 4), 256, 0, s, row_ptr, bucket,
+               col, long_rows, n_long);
     *launches += 3;
     return cudaGetLastError();
 }

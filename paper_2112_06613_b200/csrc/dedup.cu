@@ -395,8 +395,10 @@ cudaError_t launch_dedup_find(const uint8_t* residues, const int64_t* offsets, c
                               int32_t* rep_of, uint32_t* is_first, unsigned long long* hist, uint32_t* flags,
                               cudaStream_t s, int* launches) {
     // (table is all ones: cleared by the caller, ahead of the kernels that precede this one)
-    launch_dep(k_dedup_insert, grid_for(n), 256, 0, s, residues, offsets, lengths, n, total_len, table, slots - 1u, hash, hist, flags);
-    launch_dep(k_dedup_lookup, grid_for(n), 256, 0, s, residues, offsets, lengths, n, table, slots - 1u, hash, rep_of, is_first);
+    launch_dep(k_dedup_insert, grid_for(n), 256, 0, s, residues, offsets, lengths, n, total_len, table, slots - 1u,
+               hash, hist, flags);
+    launch_dep(k_dedup_lookup, grid_for(n), 256, 0, s, residues, offsets, lengths, n, table, slots - 1u, hash, rep_of,
+               is_first);
     *launches += 2;
     return cudaGetLastError();
 }
@@ -405,7 +407,8 @@ cudaError_t launch_dedup_groups(const int32_t* rep_of, const uint32_t* first_ran
                                 const int32_t* lengths, int64_t n, int32_t* uid_of, uint32_t* group_count,
                                 int32_t* len_u, int64_t* off_u, unsigned long long* hist_u, cudaStream_t s,
                                 int* launches) {
-    launch_dep(k_dedup_groups, grid_for(n), 256, 0, s, rep_of, first_rank, offsets, lengths, n, uid_of, group_count, len_u, off_u, hist_u);
+    launch_dep(k_dedup_groups, grid_for(n), 256, 0, s, rep_of, first_rank, offsets, lengths, n, uid_of, group_count,
+               len_u, off_u, hist_u);
     *launches += 1;
     return cudaGetLastError();
 }

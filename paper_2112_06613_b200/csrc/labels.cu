@@ -125,8 +125,10 @@ cudaError_t launch_edge_rows(const int64_t* row_ptr, int64_t n, int32_t* edge_ro
 cudaError_t launch_edge_distances(const int32_t* edge_row, const int32_t* col, int64_t n_edges, const int32_t* inv_perm,
                                   const void* planes, bool wide_planes, uint8_t* dist, cudaStream_t s, int* launches) {
     if (n_edges <= 0) return cudaSuccess;
-    if (wide_planes) launch_dep(k_edge_distances<uint64_t>, grid_for(n_edges), 256, 0, s, edge_row, col, n_edges, inv_perm, planes, dist);
-    else launch_dep(k_edge_distances<uint32_t>, grid_for(n_edges), 256, 0, s, edge_row, col, n_edges, inv_perm, planes, dist);
+    if (wide_planes) launch_dep(k_edge_distances<uint64_t>, grid_for(n_edges), 256, 0, s, edge_row, col, n_edges,
+                                inv_perm, planes, dist);
+    else launch_dep(k_edge_distances<uint32_t>, grid_for(n_edges), 256, 0, s, edge_row, col, n_edges, inv_perm,
+                    planes, dist);
     *launches += 1;
     return cudaGetLastError();
 }
@@ -143,7 +145,8 @@ cudaError_t launch_restrict_compact(const int32_t* edge_row, const int32_t* col,
                                     int64_t n_edges, const uint32_t* flags, const uint32_t* pos,
                                     unsigned long long* keys_out, uint8_t* dist_out, cudaStream_t s, int* launches) {
     if (n_edges <= 0) return cudaSuccess;
-    launch_dep(k_restrict_compact, grid_for(n_edges), 256, 0, s, edge_row, col, dist, n_edges, flags, pos, keys_out, dist_out);
+    launch_dep(k_restrict_compact, grid_for(n_edges), 256, 0, s, edge_row, col, dist, n_edges, flags, pos, keys_out,
+               dist_out);
     *launches += 1;
     return cudaGetLastError();
 }

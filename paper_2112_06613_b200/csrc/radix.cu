@@ -115,7 +115,8 @@ __global__ void __launch_bounds__(kThreads) k_radix_scatter(const unsigned long 
         const int64_t i = first + r * 32;
         const bool valid = i < n;
         key[r] = valid ? keys_in[i] : 0ull;
-        const uint32_t d = valid ? (uint32_t)(key[r] >> shift) & (uint32_t)(kDigits - 1) : kDigits + lane;  // invalid lanes match nobody
+        // (invalid lanes match nobody)
+        const uint32_t d = valid ? (uint32_t)(key[r] >> shift) & (uint32_t)(kDigits - 1) : kDigits + lane;
         const uint32_t peers = __match_any_sync(kFull, d);
         const int leader = __ffs((int)peers) - 1;
         uint32_t old = 0;
@@ -177,17 +178,23 @@ cudaError_t radix_sort_u64(unsigned long long* keys_a, unsigned long long* keys_
     const bool has_val = vals_a != nullptr;
     const bool small = rounds_for(n) == 4;
     for (int p = 0; p < n_passes; ++p) {
-        if (small) launch_dep(k_radix_hist<4>, tiles, kThreads, 0, s, keys_a, n, shifts[p], hist, totals + p * kDigits, tiles);
-        else launch_dep(k_radix_hist<16>, tiles, kThreads, 0, s, keys_a, n, shifts[p], hist, totals + p * kDigits, tiles);
+        if (small) launch_dep(k_radix_hist<4>, tiles, kThreads, 0, s, keys_a, n, shifts[p], hist,
+                              totals + p * kDigits, tiles);
+        else launch_dep(k_radix_hist<16>, tiles, kThreads, 0, s, keys_a, n, shifts[p], hist, totals + p * kDigits,
+                        tiles);
         launch_dep(k_radix_scan, kDigits, kThreads, 0, s, hist, totals + p * kDigits, tiles);
         if (has_val && small)
-            launch_dep(k_radix_scatter<true, 4>, tiles, kThreads, 0, s, keys_a, keys_b, vals_a, vals_b, n, shifts[p], hist, tiles);
+            launch_dep(k_radix_scatter<true, 4>, tiles, kThreads, 0, s, keys_a, keys_b, vals_a, vals_b, n, shifts[p],
+                       hist, tiles);
         else if (has_val)
-            launch_dep(k_radix_scatter<true, 16>, tiles, kThreads, 0, s, keys_a, keys_b, vals_a, vals_b, n, shifts[p], hist, tiles);
+            launch_dep(k_radix_scatter<true, 16>, tiles, kThreads, 0, s, keys_a, keys_b, vals_a, vals_b, n, shifts[p],
+                       hist, tiles);
         else if (small)
-            launch_dep(k_radix_scatter<false, 4>, tiles, kThreads, 0, s, keys_a, keys_b, nullptr, nullptr, n, shifts[p], hist, tiles);
+            launch_dep(k_radix_scatter<false, 4>, tiles, kThreads, 0, s, keys_a, keys_b, nullptr, nullptr, n,
+                       shifts[p], hist, tiles);
         else
-            launch_dep(k_radix_scatter<false, 16>, tiles, kThreads, 0, s, keys_a, keys_b, nullptr, nullptr, n, shifts[p], hist, tiles);
+            launch_dep(k_radix_scatter<false, 16>, tiles, kThreads, 0, s, keys_a, keys_b, nullptr, nullptr, n,
+                       shifts[p], hist, tiles);
         *launches += 3;
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;

@@ -140,14 +140,16 @@ cudaError_t scan_impl(const TIn* in, TOut* out, int64_t n, bool write_total, voi
     if ((n + small_tile - 1) / small_tile <= kFusedTiles) {
         const int64_t tiles = (n + small_tile - 1) / small_tile;
         launch_dep(k_tile_sums<TIn, TOut, true>, (unsigned)tiles, kScanThreads, 0, s, in, n, sums);
-        launch_dep(k_tile_scan<TIn, TOut, true>, (unsigned)tiles, kScanThreads, 0, s, in, out, n, sums, write_total ? 1 : 0);
+        launch_dep(k_tile_scan<TIn, TOut, true>, (unsigned)tiles, kScanThreads, 0, s, in, out, n, sums,
+                   write_total ? 1 : 0);
         *launches += 2;
         return cudaGetLastError();
     }
     const int64_t tiles = (n + big_tile - 1) / big_tile;
     launch_dep(k_tile_sums<TIn, TOut, false>, (unsigned)tiles, kScanThreads, 0, s, in, n, sums);
     launch_dep(k_scan_tile_sums<TOut>, 1, 1024, 0, s, sums, tiles);
-    launch_dep(k_tile_scan<TIn, TOut, false>, (unsigned)tiles, kScanThreads, 0, s, in, out, n, sums, write_total ? 1 : 0);
+    launch_dep(k_tile_scan<TIn, TOut, false>, (unsigned)tiles, kScanThreads, 0, s, in, out, n, sums,
+               write_total ? 1 : 0);
     *launches += 3;
     return cudaGetLastError();
 }

@@ -382,7 +382,8 @@ __device__ __forceinline__ void drain_round(ProbeWarp<W, L, COUNT>& w, const Joi
     bool keep = false;
     if (act) {
         const PlaneRow<W> B = load_planes<W>(S.planes, t);
-        if (B.len == w.n) {  // (an entry of another length bucket that shares the hash bucket cannot pass the segment test below either)
+        // (an entry of another length bucket that shares the hash bucket could not pass the segment test below either)
+        if (B.len == w.n) {
             W M[L + 1];
             band_masks_hoisted<L>(Ao, B, w.smin, w.NV, M);
             const int i = S.tab.probe_seg[w.delta][pi], d = S.tab.probe_shift[w.delta][pi];
@@ -409,7 +410,7 @@ __device__ __forceinline__ void drain_round(ProbeWarp<W, L, COUNT>& w, const Joi
 // (Register cap for 5 / 6 CTAs per SM: the kernel waits on dependent L2 reads, warps hide more than a few spills cost -
 // measured at config 5: 7.35 -> 7.08 ms per step.)
 template <typename W, int L, bool COUNT>
-__global__ void __launch_bounds__(kJoinThreads, (L >= 2 ? 6 : 5)) k_join_probe(const __grid_constant__ JoinParams S) {
+__global__ void __launch_bounds__(kJoinThreads, (L >= 5 ? 4 : L >= 2 ? 6 : 5)) k_join_probe(const __grid_constant__ JoinParams S) {
     grid_dependency_wait();
     __shared__ WarpBuf bufs[kJoinWarps];
     const DistanceParams& P = S.d;
@@ -616,6 +617,8 @@ cudaError_t launch_join_w(const JoinParams& S, bool count_work, int n_sm, cudaSt
         case 2: return launch_join_l<W, 2>(S, count_work, n_sm, s, launches);
         case 3: return launch_join_l<W, 3>(S, count_work, n_sm, s, launches);
         case 4: return launch_join_l<W, 4>(S, count_work, n_sm, s, launches);
+        case 5: return launch_join_l<W, 5>(S, count_work, n_sm, s, launches);
+        case 6: return launch_join_l<W, 6>(S, count_work, n_sm, s, launches);
         default: return cudaErrorInvalidValue;
     }
 }
@@ -629,14 +632,17 @@ cudaError_t launch_join_index(const void* planes, bool wide, const LengthTable& 
     const int64_t threads = n * tab.n_seg;
     if (threads <= 0) return cudaSuccess;
     const unsigned blocks = (unsigned)((threads + 255) / 256);
-    if (wide) launch_dep(k_join_index<uint64_t, false>, blocks, 256, 0, s, planes, n, tab, cnt, nullptr, nullptr, slots - 1u);
-    else launch_dep(k_join_index<uint32_t, false>, blocks, 256, 0, s, planes, n, tab, cnt, nullptr, nullptr, slots - 1u);
+    if (wide) launch_dep(k_join_index<uint64_t, false>, blocks, 256, 0, s, planes, n, tab, cnt, nullptr, nullptr,
+                         slots - 1u);
+    else launch_dep(k_join_index<uint32_t, false>, blocks, 256, 0, s, planes, n, tab, cnt, nullptr, nullptr,
+                    slots - 1u);
     *launches += 1;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     e = exclusive_scan_u32_total(cnt, dir, (int64_t)slots, scan_scratch, s, launches);
     if (e != cudaSuccess) return e;
-    if (wide) launch_dep(k_join_index<uint64_t, true>, blocks, 256, 0, s, planes, n, tab, cnt, dir, entries, slots - 1u);
+    if (wide) launch_dep(k_join_index<uint64_t, true>, blocks, 256, 0, s, planes, n, tab, cnt, dir, entries,
+                         slots - 1u);
     else launch_dep(k_join_index<uint32_t, true>, blocks, 256, 0, s, planes, n, tab, cnt, dir, entries, slots - 1u);
     *launches += 1;
     return cudaGetLastError();

@@ -196,8 +196,8 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
 }
 
 // The tables only the prefix-trie / text-chunk kernels read: pattern rows (one residue code per byte) and text rows (one
-// 32-bit word per column) expanded from the bit-plane rows, and the prefix trie over the text rows (trie.cu).  Built when a build first schedules one of those kernels (the
-// segment join, the default for l_max <= 4, needs neither).
+// 32-bit word per column) expanded from the bit-plane rows, and the prefix trie over the text rows (trie.cu).  Built
+// when a build first schedules one of those kernels (the segment join, the default for l_max <= 6, needs neither).
 int ensure_text_tables(tcrnet_ctx* ctx, SeqSet& set, int* launches) {
     if (set.text_tables) return TCRNET_OK;
     cudaStream_t s = ctx->stream;
@@ -382,7 +382,7 @@ struct Schedule {
 // n = q k + r: every segment gets q residues and r of them one more - the two outer ones first, then inwards,
 // because CDR3 sequences are least diverse at their ends (conserved first / last residues), so the outer segments
 // need the extra residue most.  Any cut is exact; this one only keeps the candidate lists short.
-void make_join_tables(int l_max, JoinTables& tab) {
+bool make_join_tables(int l_max, JoinTables& tab) {
     std::memset(&tab, 0, sizeof(tab));
     const int k = l_max + 1;
     tab.n_seg = (int8_t)k;
@@ -403,13 +403,15 @@ void make_join_tables(int l_max, JoinTables& tab) {
         int np = 0;
         for (int i = 0; i < k; ++i)
             for (int d = -l_max; d <= l_max; ++d)
-                if (std::max(std::abs(d), i) + std::abs(d + delta) <= l_max && np < kJoinMaxProbes) {
+                if (std::max(std::abs(d), i) + std::abs(d + delta) <= l_max) {
+                    if (np >= kJoinMaxProbes) return false;  // (a dropped probe would lose edges)
                     tab.probe_seg[delta][np] = (int8_t)i;
                     tab.probe_shift[delta][np] = (int8_t)d;
                     ++np;
                 }
         tab.n_probes[delta] = (int8_t)np;
     }
+    return true;
 }
 
 // Step A2, host side: the (pattern bucket, text bucket) pairs with len_t - len_p in 0..l_max
@@ -504,7 +506,7 @@ void make_schedule(const tcrnet_ctx* ctx, int l_max, int first_check, Schedule& 
     st.pairs_all = ctx->n * (ctx->n - 1) / 2;
     // The join serves the thresholds it is specialised on, with the early exit on (its verification is banded by
     // construction); beyond them the trie / text-chunk kernels.
-    const bool can_join = ctx->early_exit && l_max <= kTrieMaxL;
+    const bool can_join = ctx->early_exit && l_max <= kJoinMaxL;
     sch.fast_l1 = can_join && ctx->fast_l1 && l_max <= 1;
     sch.use_join = sch.fast_l1 || (can_join && (ctx->segment_join == 1 ||
                                                 (ctx->segment_join < 0 && ctx->prefix_trie)));
@@ -577,7 +579,7 @@ int64_t join_index_entries(const SeqSet& set, int l_max) {
 int build_join_index(tcrnet_ctx* ctx, int l_max, cudaStream_t s, DevBuf& scan_scratch, int* launches) {
     const SeqSet& set = ctx->all;
     const int64_t n_idx = join_index_entries(set, l_max);
-    make_join_tables(l_max, ctx->join_tab);
+    if (l_max > kJoinMaxL || !make_join_tables(l_max, ctx->join_tab)) return TCRNET_ERR_LMAX;
     uint32_t slots = 1024;
     while ((int64_t)slots < 2 * n_idx && slots < (1u << 30)) slots <<= 1;
     TRY(dev_reserve(ctx, ctx->join_cnt, sizeof(uint32_t) * (size_t)slots));
@@ -611,7 +613,7 @@ int build_join_index_ahead(tcrnet_ctx* ctx, int* launches) {
     const int l_max = ctx->ahead_l_max;
     const bool join_on = ctx->early_exit && ctx->segment_join != 0;  // (ahead_l_max: a build did use the join)
     // (timing level 2 measures the phases one after the other: nothing is built ahead there)
-    if (l_max < 0 || l_max > kTrieMaxL || !join_on || ctx->timing >= 2) return TCRNET_OK;
+    if (l_max < 0 || l_max > kJoinMaxL || !join_on || ctx->timing >= 2) return TCRNET_OK;
     if (join_index_entries(ctx->all, l_max) == 0) return TCRNET_OK;
     TRY(build_join_index(ctx, l_max, ctx->side_stream, ctx->join_scan_scratch, launches));
     TRY_CUDA(cudaEventRecord(ctx->ev_index, ctx->side_stream));
@@ -842,7 +844,8 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
     }
     if (grouped) std::swap(ctx->keys_a, ctx->keys_b);  // the edges between rows are what the CSR step takes
     st.ms_kernel = 0.f;
-    if (ctx->timing >= 1) TRY_CUDA(cudaEventElapsedTime(&st.ms_kernel, ctx->ev[4], ctx->ev[5]));  // of the last pass (both complete: synced)
+    // (of the last pass; both events complete: synchronised above)
+    if (ctx->timing >= 1) TRY_CUDA(cudaEventElapsedTime(&st.ms_kernel, ctx->ev[4], ctx->ev[5]));
     st.lane_columns_exec = (int64_t)ctx->h_ctrl->work[0];
     st.lane_tests_exec = (int64_t)ctx->h_ctrl->work[1];
     st.lane_pairs_exec = (int64_t)ctx->h_ctrl->work[2];
@@ -996,17 +999,18 @@ void tcrnet_destroy(tcrnet_ctx* ctx) {
     if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
     if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
     if (ctx->ev_index) cudaEventDestroy(ctx->ev_index);
-    DevBuf* bufs[] = {&ctx->all.perm, &ctx->all.pat, &ctx->all.txt, &ctx->all.trie, &ctx->query.perm, &ctx->query.pat,
-                      &ctx->query.txt, &ctx->query.trie, &ctx->all.planes, &ctx->query.planes, &ctx->join_cand, &ctx->expand_huge, &ctx->join_scan_scratch, &ctx->join_cnt, &ctx->join_dir,
-                      &ctx->join_entries, &ctx->join_rows, &ctx->inv_perm, &ctx->edge_row, &ctx->edge_dist, &ctx->edge_dist_b, &ctx->flags,
-                      &ctx->flag_pos, &ctx->in_res, &ctx->in_len, &ctx->offsets,
-                      &ctx->perm_tmp, &ctx->trie_scratch, &ctx->keys_a, &ctx->keys_b, &ctx->radix_scratch,
-                      &ctx->scan_scratch, &ctx->rows, &ctx->row_ptr, &ctx->col, &ctx->row_count, &ctx->long_rows, &ctx->all.group_start, &ctx->all.members, &ctx->all.uid_of,
-                      &ctx->dd_table, &ctx->dd_hash, &ctx->dd_rep, &ctx->dd_first, &ctx->dd_rank, &ctx->dd_count, &ctx->dd_len,
-                      &ctx->dd_off, &ctx->dd_offsets,
-                      &ctx->deg, &ctx->ctrl, &ctx->obs_ctrl, &ctx->deg_hist, &ctx->nn_sum, &ctx->class_sum, &ctx->knn,
-                      &ctx->cc_parent, &ctx->cc_count, &ctx->cc_label, &ctx->cc_size, &ctx->perc_rank,
-                      &ctx->perc_seen, &ctx->perc_deg, &ctx->perc_hist, &ctx->perc_lcc};
+    DevBuf* bufs[] = {
+        &ctx->all.perm, &ctx->all.pat, &ctx->all.txt, &ctx->all.trie, &ctx->query.perm, &ctx->query.pat,
+        &ctx->query.txt, &ctx->query.trie, &ctx->all.planes, &ctx->query.planes, &ctx->join_cand, &ctx->expand_huge,
+        &ctx->join_scan_scratch, &ctx->join_cnt, &ctx->join_dir, &ctx->join_entries, &ctx->join_rows, &ctx->inv_perm,
+        &ctx->edge_row, &ctx->edge_dist, &ctx->edge_dist_b, &ctx->flags, &ctx->flag_pos, &ctx->in_res, &ctx->in_len,
+        &ctx->offsets, &ctx->perm_tmp, &ctx->trie_scratch, &ctx->keys_a, &ctx->keys_b, &ctx->radix_scratch,
+        &ctx->scan_scratch, &ctx->rows, &ctx->row_ptr, &ctx->col, &ctx->row_count, &ctx->long_rows,
+        &ctx->all.group_start, &ctx->all.members, &ctx->all.uid_of, &ctx->dd_table, &ctx->dd_hash, &ctx->dd_rep,
+        &ctx->dd_first, &ctx->dd_rank, &ctx->dd_count, &ctx->dd_len, &ctx->dd_off, &ctx->dd_offsets, &ctx->deg,
+        &ctx->ctrl, &ctx->obs_ctrl, &ctx->deg_hist, &ctx->nn_sum, &ctx->class_sum, &ctx->knn, &ctx->cc_parent,
+        &ctx->cc_count, &ctx->cc_label, &ctx->cc_size, &ctx->perc_rank, &ctx->perc_seen, &ctx->perc_deg,
+        &ctx->perc_hist, &ctx->perc_lcc};
     for (DevBuf* b : bufs) dev_free(ctx, *b);
     if (ctx->h_ctrl) cudaFreeHost(ctx->h_ctrl);
     for (cudaEvent_t ev : ctx->ev)

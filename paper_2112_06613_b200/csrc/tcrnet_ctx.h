@@ -72,7 +72,8 @@ struct tcrnet_ctx {
     int trie_chunk = 1 << 20;  // in practice the whole text bucket: the top of the trie is walked once per pattern tile
 
     int dedup = 1;        // collapse identical sequences at load (TCRNET_OPT_DEDUP)
-    int segment_join = -1;  // TCRNET_OPT_SEGMENT_JOIN: -1 automatic (l_max <= 4, unless TCRNET_OPT_PREFIX_TRIE = 0), 0 never, 1 whenever possible
+    // TCRNET_OPT_SEGMENT_JOIN: -1 automatic (l_max <= 6, unless TCRNET_OPT_PREFIX_TRIE = 0), 0 never, 1 whenever possible
+    int segment_join = -1;
     int fast_l1 = 0;        // TCRNET_OPT_FAST_L1: l_max <= 1 builds through the join with the XOR / popcount check
     int timing = 1;         // TCRNET_OPT_TIMING: 0 no events, 1 around the distance kernels (ms_kernel), 2 every phase
     int64_t n_query = 0;  // > 0: rectangular mode (TCRNET_OPT_N_QUERY)

@@ -110,15 +110,17 @@ struct DistanceParams {
 // (l_max edits touch at most l_max segments), shifted by no more than the edits allow.  The segments of every
 // text are indexed in a hash directory; every pattern probes it with the substrings that could be such a
 // segment, and only the pairs found this way are verified.
-constexpr int kJoinMaxSeg = kTrieMaxL + 1;  // segments per text: l_max + 1 <= 5
-constexpr int kJoinMaxProbes = 28;          // (segment, shift) probes per length difference
+constexpr int kJoinMaxL = 6;                // the join kernels are specialised on l_max = 0..kJoinMaxL
+constexpr int kJoinMaxSeg = kJoinMaxL + 1;  // segments per text: l_max + 1 <= 7
+constexpr int kJoinMaxProbes = 40;          // (segment, shift) probes per length difference: 1, 3, 7, 12, 19, 27, 37
+                                            // at most for l_max = 0..6 (make_join_tables checks)
 struct JoinTables {
     uint8_t seg_start[kNumLen][kJoinMaxSeg + 1];  // [n][i] = first residue of segment i of a text of length n; [n][k] = n
     int8_t n_probes[kJoinMaxSeg];                 // [delta]: probes of a pattern against the texts longer by delta
     int8_t probe_seg[kJoinMaxSeg][kJoinMaxProbes];
     int8_t probe_shift[kJoinMaxSeg][kJoinMaxProbes];  // the segment starting at p in the text is looked for at p + shift
     int8_t n_seg;                                 // l_max + 1
-    int8_t pad_[6];
+    int8_t pad_[8 - (1 + kJoinMaxSeg) % 8];
 };
 // One pattern bucket of the join: a work item (one warp) is a tile of 32 patterns x ONE length difference delta
 // (all its probes) against the indexed text bucket of length m + delta (t_count 0: none).
@@ -177,7 +179,8 @@ cudaError_t radix_clear_totals(void* scratch, cudaStream_t s);
 // n_dev (may be NULL): device count of rows, at most n
 cudaError_t launch_length_hist(const int32_t* lengths, int64_t n, const uint32_t* n_dev,
                                unsigned long long* hist /*[kNumLen]*/, uint32_t* flags, cudaStream_t s, int* launches);
-// sort key of row i: ((length - 1) << 30, invalid lengths: 0) | the first kSortPrefix residues, 5 bits each (0 = past the end); vals[i] = i
+// sort key of row i: ((length - 1) << 30, invalid lengths: 0) | the first kSortPrefix residues, 5 bits each (0 = past
+// the end); vals[i] = i
 constexpr int kSeqKeyBits = 6 + 5 * kSortPrefix;  // length - 1 (0..63) takes 6 bits
 cudaError_t launch_seq_keys(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths, int64_t n,
                             unsigned long long* keys, int32_t* vals, cudaStream_t s, int* launches);
@@ -250,8 +253,8 @@ cudaError_t launch_join_index(const void* planes, bool wide, const LengthTable& 
                               uint32_t* cnt, uint32_t* dir, uint2* entries, uint32_t slots, void* scan_scratch,
                               cudaStream_t s, int* launches);
 // Probe + filter (+ verification and emission for l_max <= 1); for l_max >= 2 the surviving pairs go to `cand`
-// (at most cand_cap of the *cand_count counted; `rows` is HOST memory) and a second kernel verifies them (Landau-Vishkin on the mismatch
-// masks of the band's diagonals) and emits.  p carries the emission fields, n_items and the shard of the launch.
+// (at most cand_cap of the *cand_count counted; `rows` is HOST memory) and a second kernel verifies them
+// (Landau-Vishkin on the mismatch masks of the band's diagonals) and emits.  p carries the emission fields, n_items and the shard of the launch.
 cudaError_t launch_join(const DistanceParams& p, const JoinRow* rows, int n_rows, const void* planes, bool wide,
                         const JoinIndex& index, const JoinTables& tab, uint2* cand, uint8_t* cand_probe,
                         unsigned long long* cand_count, unsigned long long cand_cap, bool count_work, int n_sm,

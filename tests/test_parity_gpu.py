@@ -111,11 +111,11 @@ def test_prefix_trie_does_not_change_the_result(pkg, oracle):
 
 
 def test_segment_join_does_not_change_the_result(pkg, oracle):
-    """The segment join (pigeonhole candidate filter, the default for l_max <= 4) against the oracle and against the
+    """The segment join (pigeonhole candidate filter, the default for l_max <= 6) against the oracle and against the
     paths that visit every length-compatible pair: every threshold it serves, collapse on / off, counters on, a tiny
     edge buffer (second pass), and the l_max <= 1 option."""
     d = generate("cfg2", n=20000)
-    for l_max in (0, 1, 2, 3, 4):
+    for l_max in (0, 1, 2, 3, 4, 5, 6):
         want = oracle.network(d.residues, d.lengths, l_max, tier=1)[:3]
         got, st = gpu_network(pkg, d.residues, d.lengths, l_max)
         assert st["join_mode"] >= 1 and st["work_items_join"] > 0 and st["work_items_trie"] == 0
@@ -127,7 +127,9 @@ def test_segment_join_does_not_change_the_result(pkg, oracle):
             if opts.get(pkg.OPT_COUNT_WORK):
                 assert st["join_probes"] > 0 and st["join_entries"] > 0 and (st["join_candidates"] > 0 or l_max == 0)
             if opts.get(pkg.OPT_EDGE_CAPACITY) and opts.get(pkg.OPT_DEDUP) == 0 and l_max > 0:
-                assert st["distance_passes"] == 2  # (the record buffer of a collapsed load starts at n_distinct entries)
+                # (the record buffer of a collapsed load starts at n_distinct entries; 3: the verification queue of
+                # the join grew as well)
+                assert st["distance_passes"] in (2, 3)
             assert_same_network(got, want)
         if l_max <= 1:
             got, st = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_FAST_L1: 1})
@@ -137,7 +139,7 @@ def test_segment_join_does_not_change_the_result(pkg, oracle):
         assert st["join_mode"] == 0
         assert_same_network(got, want)
     # beyond the thresholds the join serves, the rectangular mode and early exit off: the other kernels
-    got, st = gpu_network(pkg, d.residues, d.lengths, 5)
+    got, st = gpu_network(pkg, d.residues, d.lengths, 7)
     assert st["join_mode"] == 0
     got, st = gpu_network(pkg, d.residues, d.lengths, 2, {pkg.OPT_EARLY_EXIT: 0})
     assert st["join_mode"] == 0
@@ -169,7 +171,7 @@ def test_prefix_trie_shared_prefixes_and_short_buckets(pkg, oracle):
     order = rng.permutation(len(strings))
     res, ln = from_strings([strings[i] for i in order])
     for l_max, opts in ((0, {}), (1, {}), (2, {}), (3, {pkg.OPT_TRIE_CHUNK: 256}), (4, {}), (4, {pkg.OPT_TRIE_CHUNK: 512}),
-                        (6, {pkg.OPT_FIRST_CHECK: 3})):
+                        (6, {pkg.OPT_FIRST_CHECK: 3}), (7, {})):
         want = oracle.network(res, ln, l_max, tier=0)[:3]
         got, st = gpu_network(pkg, res, ln, l_max, {pkg.OPT_SEGMENT_JOIN: 0, **opts})
         assert (st["work_items_trie"] > 0) == (l_max <= 4) and st["join_mode"] == 0
@@ -177,7 +179,7 @@ def test_prefix_trie_shared_prefixes_and_short_buckets(pkg, oracle):
         # the default path: the segment join for the buckets long enough to be cut into l_max + 1 segments, the
         # text-chunk kernel for the shorter ones (lengths 3..19 here: both occur for l_max >= 3)
         got, st = gpu_network(pkg, res, ln, l_max, opts)
-        assert (st["join_mode"] >= 1) == (l_max <= 4)
+        assert (st["join_mode"] >= 1) == (l_max <= 6)
         assert_same_network(got, want)
         if l_max <= 1:
             got, st = gpu_network(pkg, res, ln, l_max, {pkg.OPT_FAST_L1: 1})
@@ -369,10 +371,10 @@ def test_low_complexity_sequences(pkg, oracle, alphabet, lo, hi):
             strings.append("".join(t))
     strings = [strings[i] for i in rng.permutation(len(strings))]
     res, ln = from_strings(strings)
-    for l_max in (0, 1, 2, 3, 4, 5):
+    for l_max in (0, 1, 2, 3, 4, 5, 6, 7):
         want = oracle.network(res, ln, l_max, tier=0)[:3]
         got, st = gpu_network(pkg, res, ln, l_max)
-        assert st["join_mode"] == 0 if l_max > 4 else (st["join_mode"] >= 1 or st["pairs_kept"] == 0)
+        assert st["join_mode"] == 0 if l_max > 6 else (st["join_mode"] >= 1 or st["pairs_kept"] == 0)
         assert_same_network(got, want)
         if l_max in (1, 3):
             got, _ = gpu_network(pkg, res, ln, l_max, {pkg.OPT_DEDUP: 0})
@@ -398,7 +400,7 @@ def test_many_small_random_instances(pkg, oracle, seed):
             strings = ["".join(alpha[i] for i in rng.integers(0, k, int(rng.integers(lo, hi + 1)))) for _ in range(n)]
             strings += [strings[i] for i in rng.integers(0, n, n // 3)]
             res, ln = from_strings(strings)
-            for l_max in range(6):
+            for l_max in range(8):
                 want = oracle.network(res, ln, l_max, tier=0)[:3]
                 for ctx in (net, net_rows):
                     ctx.load(res, ln)
@@ -434,7 +436,7 @@ def test_many_small_random_instances_long_rows(pkg, oracle, seed):
                             del t[q]
                     strings.append("".join(t))
             res, ln = from_strings(strings)
-            for l_max in range(6):
+            for l_max in range(8):
                 want = oracle.network(res, ln, l_max, tier=0)[:3]
                 net.load(res, ln)
                 net.build(l_max)
@@ -854,9 +856,10 @@ def test_query_mode(pkg, oracle, n_query):
     the build keeps exactly the edges with at least one query endpoint."""
     d = generate("cfg2", n=12000)
     # default: through the segment join (one pass over all rows, the emission keeps the pairs with a query row);
-    # TCRNET_OPT_SEGMENT_JOIN = 0 / TCRNET_OPT_PREFIX_TRIE = 0 / l_max > 4: the two restricted passes of the trie /
+    # TCRNET_OPT_SEGMENT_JOIN = 0 / TCRNET_OPT_PREFIX_TRIE = 0 / l_max > 6: the two restricted passes of the trie /
     # text-chunk kernels
-    for l_max, opts in ((0, {}), (1, {}), (2, {}), (3, {}), (4, {}), (5, {}), (0, {pkg.OPT_SEGMENT_JOIN: 0}),
+    for l_max, opts in ((0, {}), (1, {}), (2, {}), (3, {}), (4, {}), (5, {}), (6, {}), (7, {}),
+                        (0, {pkg.OPT_SEGMENT_JOIN: 0}),
                         (1, {pkg.OPT_SEGMENT_JOIN: 0}), (2, {pkg.OPT_SEGMENT_JOIN: 0}), (3, {pkg.OPT_PREFIX_TRIE: 0}),
                         (4, {pkg.OPT_SEGMENT_JOIN: 0, pkg.OPT_TRIE_CHUNK: 512})):
         want = _query_network(oracle, d, n_query, l_max)
@@ -868,7 +871,7 @@ def test_query_mode(pkg, oracle, n_query):
             net.build(l_max)
             got = net.copy_csr()
             st = net.get_stats()
-            assert (st["join_mode"] >= 1) == (not opts and l_max <= 4)
+            assert (st["join_mode"] >= 1) == (not opts and l_max <= 6)
             assert_same_network(got, want)
             assert (np.diff(got[0])[n_query:] == 0).all()                 # no row without a query endpoint
             assert st["pairs_all"] == n_query * (n_query - 1) // 2 + n_query * (d.n - n_query)
