@@ -323,19 +323,26 @@ __device__ __forceinline__ const JoinRowDev& find_join_row(const JoinParams& S, 
 // checked at once, one per lane (the walks themselves keep few lanes busy: buckets differ in length and most lanes
 // find nothing in a given step); what passes waits in `out` until 32 results leave with ONE atomic on the global
 // cursor (edge list for l_max <= 1, verification queue beyond).
+static_assert(kJoinMaxProbes <= 64, "queue entries keep the probe in 6 bits");
+constexpr int kWin = 2;              // windows of 32 list positions per step of the bucket walk (join kernels at
+                                     // config 5: 4.17 ms with 1, 3.83 with 2, 4.18 with 4 - registers)
+constexpr int kQueue = 64 * kWin;    // ring: < 32 waiting + kWin windows (a power of two)
+template <typename W>
 struct WarpBuf {
-    uint2 queue[64];     // ring: (owner lane | probe << 5, text)
+    W a[5][32];          // [plane][lane]: the 32 patterns of the warp (registers are scarcer than shared memory here)
+    W nv[8];             // invalid_mask of every diagonal of the band (the same for all pairs of the warp)
+    uint4 bucket[32];    // the non-empty buckets of the current probe: (first entry, entries, signature, pattern lane)
+                         // on the low slots; .x becomes first entry - start in the walked list
+    uint2 queue[kQueue]; // ring: (owner lane | probe << 5 | segment code of the entry << 12, text)
     uint2 out[64];       // (pattern, text), sorted positions
     uint8_t out_probe[64];
 };
 
 template <typename W, int L, bool COUNT>
 struct ProbeWarp {
-    WarpBuf* wb;
-    PlaneRow<W> A;  // this lane's pattern
+    WarpBuf<W>* wb;
     int lane, p0;   // sorted position of lane 0's pattern
     int m, n, delta, smin, nb;
-    W NV[L + 1];    // invalid_mask of every diagonal of the band (the same for all pairs of the warp)
     int qhead = 0, qn = 0, on = 0;
     unsigned long long n_pass = 0, n_diag = 0;
 };
@@ -371,24 +378,29 @@ __device__ __forceinline__ void flush_out(ProbeWarp<W, L, COUNT>& w, const JoinP
 template <typename W, int L, bool COUNT>
 __device__ __forceinline__ void drain_round(ProbeWarp<W, L, COUNT>& w, const JoinParams& S, int cnt) {
     const bool act = w.lane < cnt;
-    const uint2 q = act ? w.wb->queue[(w.qhead + w.lane) & 63] : make_uint2(0u, 0u);
-    w.qhead = (w.qhead + cnt) & 63;
+    const uint2 q = act ? w.wb->queue[(w.qhead + w.lane) & (kQueue - 1)] : make_uint2(0u, 0u);
+    w.qhead = (w.qhead + cnt) & (kQueue - 1);
     w.qn -= cnt;
     if (COUNT) w.n_diag += (unsigned long long)(cnt * w.nb);  // mismatch masks built (warp-level count)
-    const int ow = (int)(q.x & 31u), pi = (int)(q.x >> 5), t = (int)q.y;
+    const int ow = (int)(q.x & 31u), pi = (int)((q.x >> 5) & 63u), t = (int)q.y;
     PlaneRow<W> Ao;  // the owner's pattern
+    W NV[L + 1];
 #pragma unroll
-    for (int k = 0; k < 5; ++k) Ao.p[k] = __shfl_sync(kFullMask, w.A.p[k], ow);
+    for (int k = 0; k < 5; ++k) Ao.p[k] = w.wb->a[k][ow];
+#pragma unroll
+    for (int x = 0; x <= L; ++x) NV[x] = w.wb->nv[x];
     bool keep = false;
     if (act) {
         const PlaneRow<W> B = load_planes<W>(S.planes, t);
         // (an entry of another length bucket that shares the hash bucket could not pass the segment test below either)
         if (B.len == w.n) {
             W M[L + 1];
-            band_masks_hoisted<L>(Ao, B, w.smin, w.NV, M);
+            band_masks_hoisted<L>(Ao, B, w.smin, NV, M);
             const int i = S.tab.probe_seg[w.delta][pi], d = S.tab.probe_shift[w.delta][pi];
             const int sq = S.tab.seg_start[w.n][i], len = S.tab.seg_start[w.n][i + 1] - sq;
-            keep = shd_pass<W, L>(M, w.m) && segment_matches<W, L>(M, w.smin, w.nb, sq, len, d, w.m);
+            // (the entry belongs to the probe's segment - a foreign key that shares the hash bucket does not)
+            keep = ((q.x >> 12) & kSegmentCodeMask) == segment_code(i) && shd_pass<W, L>(M, w.m) &&
+                   segment_matches<W, L>(M, w.smin, w.nb, sq, len, d, w.m);
             if (COUNT && keep) ++w.n_pass;
             if (L <= 1 && keep)
                 keep = first_matching_probe<W, L>(S.tab, M, w.smin, w.nb, w.m, w.n, w.delta, pi) &&
@@ -412,7 +424,7 @@ __device__ __forceinline__ void drain_round(ProbeWarp<W, L, COUNT>& w, const Joi
 template <typename W, int L, bool COUNT>
 __global__ void __launch_bounds__(kJoinThreads, (L >= 5 ? 4 : L >= 2 ? 6 : 5)) k_join_probe(const __grid_constant__ JoinParams S) {
     grid_dependency_wait();
-    __shared__ WarpBuf bufs[kJoinWarps];
+    __shared__ WarpBuf<W> bufs[kJoinWarps];
     const DistanceParams& P = S.d;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t local = (int64_t)blockIdx.x * kJoinWarps + warp;
@@ -430,73 +442,97 @@ __global__ void __launch_bounds__(kJoinThreads, (L >= 5 ? 4 : L >= 2 ? 6 : 5)) k
     w.delta = delta;
     band_of(L, delta, w.smin, w.nb);
 #pragma unroll
-    for (int x = 0; x <= L; ++x) w.NV[x] = x < w.nb ? invalid_mask<W>(w.smin + x, w.m, w.n) : ~W(0);
+    for (int x = 0; x <= L; ++x)
+        if (lane == x) w.wb->nv[x] = x < w.nb ? invalid_mask<W>(w.smin + x, w.m, w.n) : ~W(0);
     w.p0 = Rw.p_start + tile * 32;
     const bool p_valid = tile * 32 + lane < Rw.p_count;
     const int p = p_valid ? w.p0 + lane : w.p0;
-    w.A = load_planes<W>(S.planes, p);
-    const uint32_t sig = class_counts<W>(w.A);
+    uint32_t sig;
+    {
+        const PlaneRow<W> A = load_planes<W>(S.planes, p);
+        sig = class_counts<W>(A);
+#pragma unroll
+        for (int k = 0; k < 5; ++k) w.wb->a[k][lane] = A.p[k];
+    }
+    __syncwarp();
     const int sig_max = 2 * L - delta;  // composition bound of a pair within L
     const int m = w.m, n = w.n;
     unsigned long long n_entries = 0, n_cand = 0, n_probes = 0;
+    const uint32_t lt_mask = (1u << lane) - 1u, le_mask = (2u << lane) - 1u;
 
     const int np = S.tab.n_probes[delta];
     for (int pi = 0; pi < np; ++pi) {
         const int i = S.tab.probe_seg[delta][pi], d = S.tab.probe_shift[delta][pi];
         const int sq = S.tab.seg_start[n][i], len = S.tab.seg_start[n][i + 1] - sq, rq = sq + d;
         if (rq < 0 || rq + len > m) continue;  // the segment does not fit at this shift (warp-uniform)
-        const uint32_t seg_code = segment_code(i);
         uint32_t e = 0, e_end = 0;
         if (p_valid) {
-            const unsigned long long h = seg_hash<W>(w.A, rq, len, n, i);
+            PlaneRow<W> A;
+#pragma unroll
+            for (int k = 0; k < 5; ++k) A.p[k] = w.wb->a[k][lane];
+            const unsigned long long h = seg_hash<W>(A, rq, len, n, i);
             const uint32_t b = (uint32_t)h & S.index.mask;
             e = __ldg(S.index.dir + b);
             e_end = __ldg(S.index.dir + b + 1);
         }
         if (COUNT) n_probes += (unsigned long long)__popc(__ballot_sync(kFullMask, p_valid));
-        // The 32 buckets are walked as ONE list, 32 entries per step whatever their lengths: prefix sums of the bucket
-        // sizes, then every lane finds the bucket (owner lane) of its position by binary search over them.
+        // The 32 buckets are walked as ONE list, 32 entries per step whatever their lengths.  The non-empty buckets are
+        // moved to the low lanes (their starts in the list are then strictly increasing); in every step the buckets that
+        // start inside the current window of 32 positions mark their start in one mask (one warp-wide OR), and a
+        // position's bucket is the number of starts at or before it.
         const int c = (int)(e_end - e);
-        int incl = c;
+        const uint32_t nz = __ballot_sync(kFullMask, c > 0);
+        if (!nz) continue;
+        if (c > 0) w.wb->bucket[__popc(nz & lt_mask)] = make_uint4(e, (uint32_t)c, sig, (uint32_t)lane);
+        __syncwarp();
+        const int c_k = lane < __popc(nz) ? (int)w.wb->bucket[lane].y : 0;  // entries of bucket `lane`
+        int incl = c_k;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             const int v = __shfl_up_sync(kFullMask, incl, o);
             if (lane >= o) incl += v;
         }
-        const int first = incl - c;  // position of this lane's first entry in the list
         const int total = __shfl_sync(kFullMask, incl, 31);
+        const int first = c_k ? incl - c_k : 0x7fffffff;  // position of this bucket's first entry in the list
+        if (c_k) w.wb->bucket[lane].x -= (uint32_t)first;  // list position f of this bucket = entry .x + f
+        __syncwarp();
         if (COUNT) n_entries += (unsigned long long)total;
-        for (int f0 = 0; f0 < total; f0 += 32) {
-            const int f = f0 + lane;
-            int ow = 0;  // the last lane whose bucket starts at or before f (empty buckets share their start with the next)
+        int before = 0;  // buckets that start before the window
+        // kWin windows per step: all their entry reads are in flight before the first is looked at
+        for (int f0 = 0; f0 < total; f0 += 32 * kWin) {
+            uint2 cur[kWin];
+            uint32_t sig_o[kWin];
+            int ow[kWin];  // the lane whose pattern probes the bucket
+            bool in[kWin];
 #pragma unroll
-            for (int step = 16; step > 0; step >>= 1) {
-                const int fc = __shfl_sync(kFullMask, first, ow + step);
-                if (fc <= f) ow += step;
+            for (int u = 0; u < kWin; ++u) {
+                const int f = f0 + 32 * u + lane;
+                const uint32_t rel = (uint32_t)(first - (f0 + 32 * u));
+                const uint32_t starts = __reduce_or_sync(kFullMask, rel < 32u ? 1u << rel : 0u);
+                const int src = before + __popc(starts & le_mask) - 1;  // (position 0 starts bucket 0: never negative)
+                before += __popc(starts);
+                const uint4 bo = w.wb->bucket[src];
+                sig_o[u] = bo.z;
+                ow[u] = (int)bo.w;
+                in[u] = f < total;
+                cur[u] = make_uint2(0u, 0u);
+                if (in[u]) cur[u] = __ldg(S.index.entries + (uint32_t)(bo.x + (uint32_t)f));  // (32-bit wrap intended)
             }
-            const uint32_t e_o = __shfl_sync(kFullMask, e, ow);
-            const int first_o = __shfl_sync(kFullMask, first, ow);
-            const uint32_t sig_o = __shfl_sync(kFullMask, sig, ow);
-            bool has = false;
-            uint32_t t = 0;
-            if (f < total) {
-                const uint2 cur = __ldg(S.index.entries + e_o + (uint32_t)(f - first_o));
-                // composition bound (drops foreign keys of the bucket too: whatever passes is checked against the
-                // probe's segment later); same bucket: only the texts after the pattern (every unordered pair once)
-                has = (cur.x & kSegmentCodeMask) == seg_code && class_distance(sig_o, cur.x) <= sig_max &&
-                      (delta > 0 || (int)cur.y > w.p0 + ow);
-                t = cur.y;
-            }
-            const uint32_t bal = __ballot_sync(kFullMask, has);
-            if (bal) {
-                if (has) w.wb->queue[(w.qhead + w.qn + __popc(bal & ((1u << lane) - 1u))) & 63] =
-                             make_uint2((uint32_t)ow | ((uint32_t)pi << 5), t);
+#pragma unroll
+            for (int u = 0; u < kWin; ++u) {
+                // composition bound; same length bucket: only the texts after the pattern (every unordered pair once).
+                // (An entry of ANOTHER segment that merely shares the hash bucket is dropped by drain_round.)
+                const bool has = in[u] && class_distance(sig_o[u], cur[u].x) <= sig_max &&
+                                 (delta > 0 || (int)cur[u].y > w.p0 + ow[u]);
+                const uint32_t bal = __ballot_sync(kFullMask, has);
+                if (has) w.wb->queue[(w.qhead + w.qn + __popc(bal & lt_mask)) & (kQueue - 1)] = make_uint2(
+                             (uint32_t)ow[u] | ((uint32_t)pi << 5) | ((cur[u].x & kSegmentCodeMask) << 12), cur[u].y);
                 const int cq = __popc(bal);
                 w.qn += cq;
                 if (COUNT) n_cand += (unsigned long long)cq;
-                __syncwarp();
-                if (w.qn >= 32) drain_round<W, L, COUNT>(w, S, 32);
             }
+            __syncwarp();
+            while (w.qn >= 32) drain_round<W, L, COUNT>(w, S, 32);
         }
     }
     if (w.qn > 0) drain_round<W, L, COUNT>(w, S, w.qn);
