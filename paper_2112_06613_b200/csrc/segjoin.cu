@@ -49,6 +49,8 @@ namespace {
 constexpr uint32_t kFullMask = 0xffffffffu;
 constexpr int kJoinWarps = 8;
 constexpr int kJoinThreads = 32 * kJoinWarps;
+constexpr int kProbeWarps = kJoinWarps;  // (CTAs of 4 warps, 12 per SM: no difference measured at configs 3-5)
+constexpr int kProbeThreads = 32 * kProbeWarps;
 constexpr int kUnreached = -1000;  // Landau-Vishkin: no alignment ends on this diagonal yet
 
 // b seen from diagonal s: bit j of the result = bit j + s of b (zero outside)
@@ -260,15 +262,6 @@ __device__ __forceinline__ unsigned long long seg_hash(const PlaneRow<W>& R, int
     return h;
 }
 
-__device__ __forceinline__ int length_of(const LengthTable& lt, int64_t t) {  // bucket of sorted position t
-    int lo = 0, hi = kNumLen;  // start[lo] <= t < start[hi]
-    while (hi - lo > 1) {
-        const int mid = (lo + hi) >> 1;
-        if ((int64_t)lt.start[mid] <= t) lo = mid; else hi = mid;
-    }
-    return lo;
-}
-
 // ---- index ----
 template <typename W, bool FILL>
 __global__ void __launch_bounds__(256) k_join_index(const void* __restrict__ planes, int64_t n,
@@ -422,12 +415,13 @@ __device__ __forceinline__ void drain_round(ProbeWarp<W, L, COUNT>& w, const Joi
 // (Register cap for 5 / 6 CTAs per SM: the kernel waits on dependent L2 reads, warps hide more than a few spills cost -
 // measured at config 5: 7.35 -> 7.08 ms per step.)
 template <typename W, int L, bool COUNT>
-__global__ void __launch_bounds__(kJoinThreads, (L >= 5 ? 4 : L >= 2 ? 6 : 5)) k_join_probe(const __grid_constant__ JoinParams S) {
+__global__ void __launch_bounds__(kProbeThreads, (L >= 5 ? 4 : L >= 2 ? 6 : 5))
+k_join_probe(const __grid_constant__ JoinParams S) {
     grid_dependency_wait();
-    __shared__ WarpBuf<W> bufs[kJoinWarps];
+    __shared__ WarpBuf<W> bufs[kProbeWarps];
     const DistanceParams& P = S.d;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t local = (int64_t)blockIdx.x * kJoinWarps + warp;
+    const int64_t local = (int64_t)blockIdx.x * kProbeWarps + warp;
     if (local >= S.n_local) return;  // the whole warp
     const int64_t item = local * P.n_shards + P.shard;
     const JoinRowDev& Rw = find_join_row(S, item);
@@ -458,7 +452,9 @@ __global__ void __launch_bounds__(kJoinThreads, (L >= 5 ? 4 : L >= 2 ? 6 : 5)) k
     const int sig_max = 2 * L - delta;  // composition bound of a pair within L
     const int m = w.m, n = w.n;
     unsigned long long n_entries = 0, n_cand = 0, n_probes = 0;
-    const uint32_t lt_mask = (1u << lane) - 1u, le_mask = (2u << lane) - 1u;
+    uint32_t lt_mask, le_mask;  // (special registers: one instruction wherever the compiler re-creates them)
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(lt_mask));
+    asm("mov.u32 %0, %%lanemask_le;" : "=r"(le_mask));
 
     const int np = S.tab.n_probes[delta];
     for (int pi = 0; pi < np; ++pi) {
@@ -632,9 +628,9 @@ __global__ void __launch_bounds__(kJoinThreads) k_join_verify(const __grid_const
 
 template <typename W, int L>
 cudaError_t launch_join_l(const JoinParams& S, bool count_work, int n_sm, cudaStream_t s, int* launches) {
-    const unsigned blocks = (unsigned)((S.n_local + kJoinWarps - 1) / kJoinWarps);
-    if (count_work) launch_dep(k_join_probe<W, L, true>, blocks, kJoinThreads, 0, s, S);
-    else launch_dep(k_join_probe<W, L, false>, blocks, kJoinThreads, 0, s, S);
+    const unsigned blocks = (unsigned)((S.n_local + kProbeWarps - 1) / kProbeWarps);
+    if (count_work) launch_dep(k_join_probe<W, L, true>, blocks, kProbeThreads, 0, s, S);
+    else launch_dep(k_join_probe<W, L, false>, blocks, kProbeThreads, 0, s, S);
     *launches += 1;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess || L <= 1) return e;

@@ -49,12 +49,6 @@ cudaError_t rec(tcrnet_ctx* ctx, int i, int level) {
 }
 constexpr uint32_t kExpandHugeCap = 1u << 16;  // products set aside for k_expand_huge (beyond: expanded by their warp)
 
-int bits_for(int64_t max_value) {  // number of bits needed to represent max_value (>= 1)
-    int b = 1;
-    while (b < 63 && (max_value >> b) != 0) ++b;
-    return b;
-}
-
 void drop_build(tcrnet_ctx* ctx) {
     drop_observables(ctx);
     ctx->built = false;
@@ -755,7 +749,6 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
 // Steps A2-A5 for the work items of one shard: unsorted keys in keys_a, ctx->n_keys of them.
 int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* launches) {
     tcrnet_stats& st = ctx->stats;
-    cudaStream_t s = ctx->stream;
     const int64_t n = ctx->n;
     int first_check = 0;
     if (ctx->early_exit) {
