@@ -59,17 +59,6 @@ __device__ __forceinline__ W diag_shift(W b, int s) {
     return s >= 0 ? (b >> s) : (b << (-s));
 }
 
-// M_s: bit j set iff pattern residue j has NO equal partner on diagonal s (a_j != b_(j+s), or j >= m, or j + s
-// outside the text)
-template <typename W>
-__device__ __forceinline__ W mismatch_mask(const PlaneRow<W>& A, const PlaneRow<W>& B, int s, int m, int n) {
-    W x = W(0);
-#pragma unroll
-    for (int k = 0; k < 5; ++k) x |= A.p[k] ^ diag_shift<W>(B.p[k], s);
-    const W valid = diag_shift<W>(low_mask<W>(n), s) & low_mask<W>(m);
-    return x | ~valid;
-}
-
 template <typename W>
 __device__ __forceinline__ int ctz_word(W x);
 template <>
@@ -100,15 +89,10 @@ __device__ __forceinline__ W invalid_mask(int s, int m, int n) {
     return ~(diag_shift<W>(low_mask<W>(n), s) & low_mask<W>(m));
 }
 
-template <typename W, int L>
-__device__ __forceinline__ void band_masks(const PlaneRow<W>& A, const PlaneRow<W>& B, int m, int n, int smin, int nb,
-                                           W (&M)[L + 1]) {
-#pragma unroll
-    for (int x = 0; x <= L; ++x) M[x] = x < nb ? mismatch_mask<W>(A, B, smin + x, m, n) : ~W(0);
-}
-
-// The same with the pair-independent parts hoisted (probe kernel: the band is the same for all pairs of a warp):
-// NV[x] = invalid_mask of diagonal x (all ones beyond the band).  32-bit planes: every plane of B is widened once
+// M_s: bit j set iff pattern residue j has NO equal partner on diagonal s (a_j != b_(j+s), or j >= m, or j + s
+// outside the text).
+// Mismatch masks of a band with the pair-independent parts given (probe kernel: the band is the same for all pairs of
+// a warp): NV[x] = invalid_mask of diagonal x (all ones beyond the band).  32-bit planes: every plane of B is widened once
 // (b << 8 as a 64-bit pair), after which any diagonal s in -8..23 is ONE funnel shift.
 template <int L>
 __device__ __forceinline__ void band_masks_hoisted(const PlaneRow<uint32_t>& A, const PlaneRow<uint32_t>& B, int smin,
@@ -134,6 +118,16 @@ __device__ __forceinline__ void band_masks_hoisted(const PlaneRow<uint64_t>& A, 
         for (int k = 0; k < 5; ++k) v |= A.p[k] ^ diag_shift<uint64_t>(B.p[k], smin + x);
         M[x] = v;
     }
+}
+
+// Mismatch masks of the band of ONE pair (verification kernel: every lane has its own m, n).
+template <typename W, int L>
+__device__ __forceinline__ void band_masks(const PlaneRow<W>& A, const PlaneRow<W>& B, int m, int n, int smin, int nb,
+                                           W (&M)[L + 1]) {
+    W NV[L + 1];
+#pragma unroll
+    for (int x = 0; x <= L; ++x) NV[x] = x < nb ? invalid_mask<W>(smin + x, m, n) : ~W(0);
+    band_masks_hoisted<L>(A, B, smin, NV, M);
 }
 
 // shifted-Hamming bound: pattern residues without a partner on any diagonal of the band
@@ -247,18 +241,21 @@ __device__ __forceinline__ int class_distance(uint32_t a, uint32_t b) {
     return (int)((v * 0x01010101u) >> 24) + __popc(neg);
 }
 
-// hash of (text length n, segment i, residues [q, q + len) of the row)
+// hash of (text length n, segment i, residues [q, q + len) of the row): 32-bit arithmetic throughout (the directory has
+// at most 2^30 slots; a collision only lets a foreign key into a bucket, where the residue-wise tests drop it)
+__device__ __forceinline__ uint32_t fold32(uint32_t x) { return x; }
+__device__ __forceinline__ uint32_t fold32(uint64_t x) { return (uint32_t)x ^ ((uint32_t)(x >> 32) * 0x9E3779B1u); }
 template <typename W>
-__device__ __forceinline__ unsigned long long seg_hash(const PlaneRow<W>& R, int q, int len, int n, int i) {
-    unsigned long long h = 0x9E3779B97F4A7C15ull ^ ((unsigned long long)(n * 8 + i) * 0xD6E8FEB86659FD93ull);
+__device__ __forceinline__ uint32_t seg_hash(const PlaneRow<W>& R, int q, int len, int n, int i) {
+    uint32_t h = (uint32_t)(n * 8 + i) * 0x9E3779B1u + 0x7F4A7C15u;
     const W mk = low_mask<W>(len);
 #pragma unroll
-    for (int k = 0; k < 5; ++k) {
-        h = (h ^ (unsigned long long)((R.p[k] >> q) & mk)) * 0xFF51AFD7ED558CCDull;
-        h ^= h >> 32;
-    }
-    h *= 0xC4CEB9FE1A85EC53ull;
-    h ^= h >> 29;
+    for (int k = 0; k < 5; ++k) h = (h ^ fold32((R.p[k] >> q) & mk)) * 0x85EBCA6Bu + 0xC2B2AE35u;
+    h ^= h >> 16;  // (murmur3's finaliser: the low bits select the slot)
+    h *= 0x85EBCA6Bu;
+    h ^= h >> 13;
+    h *= 0xC2B2AE35u;
+    h ^= h >> 16;
     return h;
 }
 
@@ -277,8 +274,7 @@ __global__ void __launch_bounds__(256) k_join_index(const void* __restrict__ pla
     const PlaneRow<W> R = load_planes<W>(planes, t);
     if (R.len < k) return;  // too short to be cut into k segments: such buckets stay with the other kernels
     const int q = tab.seg_start[R.len][i], len = tab.seg_start[R.len][i + 1] - q;
-    const unsigned long long h = seg_hash<W>(R, q, len, R.len, i);
-    const uint32_t b = (uint32_t)h & mask;
+    const uint32_t b = seg_hash<W>(R, q, len, R.len, i) & mask;
     if (!FILL) {
         atomicAdd(cnt + b, 1u);
     } else {
@@ -466,8 +462,7 @@ k_join_probe(const __grid_constant__ JoinParams S) {
             PlaneRow<W> A;
 #pragma unroll
             for (int k = 0; k < 5; ++k) A.p[k] = w.wb->a[k][lane];
-            const unsigned long long h = seg_hash<W>(A, rq, len, n, i);
-            const uint32_t b = (uint32_t)h & S.index.mask;
+            const uint32_t b = seg_hash<W>(A, rq, len, n, i) & S.index.mask;
             e = __ldg(S.index.dir + b);
             e_end = __ldg(S.index.dir + b + 1);
         }
@@ -547,67 +542,77 @@ k_join_probe(const __grid_constant__ JoinParams S) {
 }
 
 // ---- verify (l_max >= 2): one lane per surviving pair ----
-// Two steps, each at full lane occupancy: (1) every lane takes a queued pair and applies the *once* rule (most of the
-// queue are pairs found through several probes: only the first matching probe keeps its find); what is kept waits in a
-// per-warp shared-memory queue until (2) 32 pairs can run Landau-Vishkin together.
+// Two steps, each at full lane occupancy: (1) every lane takes a queued pair, builds the mismatch masks of its band and
+// applies the *once* rule (most of the queue are pairs found through several probes: only the first matching probe
+// keeps its find); what is kept waits - masks included - in a per-warp ring in shared memory until (2) 32 pairs can run
+// Landau-Vishkin together.
 template <typename W, int L>
-__device__ __forceinline__ bool verify_pair(const JoinParams& S, uint2 pt, int& m, int& n) {
-    const PlaneRow<W> A = load_planes<W>(S.planes, pt.x);
-    const PlaneRow<W> B = load_planes<W>(S.planes, pt.y);
-    m = A.len, n = B.len;
-    const int delta = n - m;
-    int smin, nb;
-    band_of(L, delta, smin, nb);
-    W M[L + 1];
-    band_masks<W, L>(A, B, m, n, smin, nb, M);
-    return lv_within<W, L>(M, m, n, delta, smin, nb);
-}
+struct VerifyRing {
+    uint2 pt[64];       // (pattern, text), sorted positions
+    W M[L + 1][64];     // mismatch masks of the band
+    uint16_t mn[64];    // m | n << 8
+};
 
 template <typename W, int L, bool COUNT>
 __global__ void __launch_bounds__(kJoinThreads) k_join_verify(const __grid_constant__ JoinParams S) {
     grid_dependency_wait();
-    __shared__ uint2 kept[kJoinWarps][64];
+    __shared__ VerifyRing<W, L> rings[kJoinWarps];
     const DistanceParams& P = S.d;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    uint2* q = kept[warp];
-    int qn = 0;
+    VerifyRing<W, L>& q = rings[warp];
+    int qhead = 0, qn = 0;
     const unsigned long long total = min(*S.cand_count, S.cand_cap);
     unsigned long long n_edges = 0, n_diag = 0;
-    auto lv_round = [&](int cnt) {  // the first cnt kept pairs, one per lane; the rest moves to the front
+    auto lv_round = [&](int cnt) {  // the first cnt kept pairs, one per lane
         const bool act = lane < cnt;
-        const uint2 pt = act ? q[lane] : make_uint2(0u, 0u);
-        const bool mv = cnt + lane < qn;
-        const uint2 rest = mv ? q[cnt + lane] : make_uint2(0u, 0u);
-        __syncwarp();
-        if (mv) q[lane] = rest;
+        const int slot = (qhead + lane) & 63;
+        qhead = (qhead + cnt) & 63;
         qn -= cnt;
-        __syncwarp();
+        uint2 pt = make_uint2(0u, 0u);
         int m = 0, n = 0;
-        const bool edge = act && verify_pair<W, L>(S, pt, m, n);
+        bool edge = false;
+        if (act) {
+            pt = q.pt[slot];
+            m = q.mn[slot] & 0xff, n = q.mn[slot] >> 8;
+            W M[L + 1];
+#pragma unroll
+            for (int x = 0; x <= L; ++x) M[x] = q.M[x][slot];
+            int smin, nb;
+            band_of(L, n - m, smin, nb);
+            edge = lv_within<W, L>(M, m, n, n - m, smin, nb);
+        }
         if (COUNT && edge) ++n_edges;
         emit_edges(P, edge, lane, (int)pt.x, (int)pt.y, m, n);
+        __syncwarp();  // (the slots are free again)
     };
     for (unsigned long long base = (unsigned long long)blockIdx.x * kJoinThreads; base < total;
          base += (unsigned long long)gridDim.x * kJoinThreads) {
         const unsigned long long c = base + threadIdx.x;
         bool keep = false;
         uint2 pt = make_uint2(0u, 0u);
+        W M[L + 1];
+        int m = 0, n = 0;
         if (c < total) {
             pt = S.cand[c];
             const int pi = (int)S.cand_probe[c];
             const PlaneRow<W> A = load_planes<W>(S.planes, pt.x);
             const PlaneRow<W> B = load_planes<W>(S.planes, pt.y);
-            const int m = A.len, n = B.len, delta = n - m;
+            m = A.len, n = B.len;
             int smin, nb;
-            band_of(L, delta, smin, nb);
-            W M[L + 1];
+            band_of(L, n - m, smin, nb);
             band_masks<W, L>(A, B, m, n, smin, nb, M);
             if (COUNT) n_diag += (unsigned long long)nb;
             // once: only the first probe whose segment matches keeps the pair
-            keep = first_matching_probe<W, L>(S.tab, M, smin, nb, m, n, delta, pi);
+            keep = first_matching_probe<W, L>(S.tab, M, smin, nb, m, n, n - m, pi);
         }
         const uint32_t bal = __ballot_sync(kFullMask, keep);
-        if (keep) q[qn + __popc(bal & ((1u << lane) - 1u))] = pt;
+        if (keep) {
+            const int slot = (qhead + qn + __popc(bal & ((1u << lane) - 1u))) & 63;
+            q.pt[slot] = pt;
+            q.mn[slot] = (uint16_t)(m | (n << 8));
+#pragma unroll
+            for (int x = 0; x <= L; ++x) q.M[x][slot] = M[x];
+        }
         qn += __popc(bal);
         __syncwarp();
         if (qn >= 32) lv_round(32);
