@@ -51,9 +51,9 @@ ORACLE_SAMPLE_ROWS = 1024
 # summarised under profiles/ (regenerated with them; a workload / kernel that is not listed prints null)
 NCU_DRAM_BYTES_PER_LAUNCH = {
     # (workload, kernel): bytes per step of that kernel / kernel pair - profiles/r2_join_ncu.txt
-    ("cfg4", "k_join_probe"): 35_106_816 + 1_280,
-    ("cfg3", "k_join_probe + k_join_verify"): 11_111_936 + 10_752 + 11_591_936 + 13_056,
-    ("cfg5", "k_join_probe + k_join_verify"): 2_734_769_000 + 447_397_120 + 369_453_000 + 54_436_608,
+    ("cfg4", "k_join_probe"): 35_106_816 + 46_592,
+    ("cfg3", "k_join_probe + k_join_verify"): 11_111_168 + 256 + 11_573_760 + 0,
+    ("cfg5", "k_join_probe + k_join_verify"): 2_324_235_000 + 300_706_816 + 367_888_000 + 52_318_208,
 }
 
 
@@ -508,6 +508,9 @@ def main() -> None:
                 "alu_ops_per_launch": alu_ops,
                 # also against the issue-slot ceiling (4 schedulers x 32 lanes per SM and clock)
                 "issue_ceiling": 2 * peak, "frac_of_issue_ceiling": achieved / (2 * peak),
+                **({"concurrent": "k_emit_cliques runs beside this kernel on the library's second stream and shares "
+                                  "the SMs (kernel_ms is the live duration; alone, under ncu: profiles/r2_launches_cfg4.md)"}
+                   if join and not args.no_dedup else {}),
             },
             "detail": {
                 "pairs_kept": work["pairs_kept"], "cells_kept": work["cells_kept"], "cells_all": work["cells_all"],
