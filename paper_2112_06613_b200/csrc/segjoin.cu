@@ -18,9 +18,10 @@
 //   index   k_join_index: one entry (composition signature, text) per (text, segment), bucketed by a hash of
 //           (n, i, segment bits) in a power-of-two directory (count -> prefix sum -> fill).
 //   probe   k_join_probe: one warp = 32 patterns of one length x one length difference delta; for every probe each lane
-//           hashes its pattern's substring and walks the directory bucket; the texts whose composition can be within l_max (same length
-//           bucket: only texts after the pattern in sorted order, so every unordered pair is seen once) are queued in
-//           shared memory and checked 32 at a time, one per lane: build the masks of the band's diagonals
+//           hashes its pattern's substring; the 32 directory buckets are walked as ONE list, 32 entries per step; the
+//           texts whose composition can be within l_max (same length bucket: only texts after the pattern in sorted
+//           order, so every unordered pair is seen once) are queued in shared memory and checked 32 at a time, one per
+//           lane: build the masks of the band's diagonals
 //           s = -floor((l_max - delta) / 2) .. delta + floor((l_max - delta) / 2)  (no alignment with <= l_max edits
 //           leaves the band) and apply
 //             - the probe's own segment really matches (M restricted to it is zero: hash collisions die here),
@@ -36,7 +37,8 @@
 //           never touched.  For l_max <= 1 it degenerates to the textbook check (equal lengths: at most one mismatch;
 //           one longer: common prefix + common suffix cover the shorter sequence - SURVEY 8(f) NEXT-4) and runs
 //           inline in the probe kernel; for l_max >= 2 the survivors are queued and k_join_verify applies the once
-//           rule and then runs Landau-Vishkin densely, one lane per pair that is still there.
+//           rule and then runs Landau-Vishkin densely, one lane per pair that is still there (the masks of a kept
+//           pair wait with it in a shared-memory ring).
 #include <algorithm>
 
 #include "launch.cuh"
