@@ -443,6 +443,42 @@ def test_many_small_random_instances_long_rows(pkg, oracle, seed):
                 assert_same_network(net.copy_csr(), want)
 
 
+@pytest.mark.parametrize("seed", range(3))
+def test_many_small_random_instances_cdr3_families(pkg, oracle, seed):
+    """The same with CDR3-shaped rows: conserved first / last residue, 8..25 residues, families of a seed and up to
+    seven copies with 0..4 random edits each, a third of all rows repeated, shuffled."""
+    rng = np.random.default_rng(9200 + seed)
+    letters = "ACDEFGHIKLMNPQRSTVWY"
+    with pkg.TcrNet(0) as net, pkg.TcrNet(0) as net_rows:
+        net_rows.set_option(pkg.OPT_DEDUP, 0)
+        for _ in range(30):
+            strings = []
+            for _ in range(int(rng.integers(5, 120))):
+                s0 = ["C"] + [letters[i] for i in rng.integers(0, 20, int(rng.integers(6, 24)))] + ["F"]
+                strings.append("".join(s0))
+                for _ in range(int(rng.integers(0, 8))):
+                    t = list(s0)
+                    for _ in range(int(rng.integers(0, 5))):
+                        q = int(rng.integers(0, len(t)))
+                        op = int(rng.integers(0, 3))
+                        if op == 0:
+                            t[q] = letters[int(rng.integers(0, 20))]
+                        elif op == 1:
+                            t.insert(q, letters[int(rng.integers(0, 20))])
+                        elif len(t) > 2:
+                            del t[q]
+                    strings.append("".join(t))
+            strings += [strings[i] for i in rng.integers(0, len(strings), len(strings) // 3)]
+            strings = [strings[i] for i in rng.permutation(len(strings))]
+            res, ln = from_strings(strings)
+            for l_max in range(8):
+                want = oracle.network(res, ln, l_max, tier=0)[:3]
+                for ctx in (net, net_rows):
+                    ctx.load(res, ln)
+                    ctx.build(l_max)
+                    assert_same_network(ctx.copy_csr(), want)
+
+
 def test_length_64_and_all_26_letters(pkg, oracle):
     rng = np.random.default_rng(5)
     letters = "ABCDEFGHIJKLMNOPQRSTUVWXYZ"
