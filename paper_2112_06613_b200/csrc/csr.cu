@@ -51,8 +51,9 @@ __global__ void __launch_bounds__(256) k_col_deg_lower(const unsigned long long*
 // The edges of a row are few (a handful at TCR scale), so the CSR is built the way a CSR is defined.  The
 // emission (or k_count_rows for caller-supplied keys) counts, for every edge (u, v), row_count[u]++ and
 // deg[v]++ (fire-and-forget L2 reductions); then
-//   row_ptr   = exclusive prefix sum of row_count                                   (scan.cu)
-//   k_scatter_keys   every key into a free slot of its row: bucket[row_ptr[u] + --row_count[u]] = key
+//   row_ptr   = INCLUSIVE prefix sum of row_count (the end of every row)                (scan.cu)
+//   k_scatter_keys   every key into a free slot of its row: bucket[--row_ptr[u]] = key; when all keys are placed
+//                    row_ptr[u] has counted down to the start of row u, i.e. it is the exclusive prefix sum
 //   k_rank_rows      one thread per slot: col[row_ptr[u] + #{w in row u : w < v}] = v for rows of <= kRankRow
 //                    neighbours (equal keys of a caller's list: ties broken by slot); coalesced, the row is
 //                    read from L1.  The thread of slot 0 adds the row length to deg[u] and queues longer rows
@@ -73,19 +74,32 @@ __global__ void __launch_bounds__(256) k_count_rows(const unsigned long long* __
     }
 }
 
-// row_count[u] = edges of row u not yet placed: counts down to 0
+// row_ptr[u] arrives as the END of row u (inclusive prefix sum of the counts) and counts down to its start: when the
+// kernel ends it IS the exclusive prefix sum.  Consecutive keys often share their row (the products of two repeated
+// sequences are emitted together), so the lanes of a warp that hold the same row take their slots with ONE returning
+// atomic (match.any; the returning atomics are what bounds this kernel).
 __global__ void __launch_bounds__(256) k_scatter_keys(const unsigned long long* __restrict__ keys, int64_t n_keys,
-                                                     const int64_t* __restrict__ row_ptr, int32_t* __restrict__ row_count,
+                                                     unsigned long long* __restrict__ row_ptr,
                                                      unsigned long long* __restrict__ bucket) {
     grid_dependency_wait();
-    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_keys; e += (int64_t)gridDim.x * blockDim.x) {
-        const unsigned long long k = keys[e];
-        const uint32_t u = (uint32_t)(k >> 32);
-        const int32_t slot = atomicSub(&row_count[u], 1) - 1;
-        bucket[row_ptr[u] + slot] = k;
+    const int lane = threadIdx.x & 31;
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    for (int64_t e0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) & ~(int64_t)31; e0 < n_keys;
+         e0 += (int64_t)gridDim.x * blockDim.x) {
+        const bool valid = e0 + lane < n_keys;
+        const unsigned long long k = valid ? keys[e0 + lane] : ~0ull;
+        const uint32_t u = (uint32_t)(k >> 32);  // (0xffffffff is no row: n <= 2^31 - 2)
+        const uint32_t same = __match_any_sync(0xffffffffu, u);
+        const int leader = __ffs((int)same) - 1;
+        unsigned long long end = 0;
+        if (valid && lane == leader) end = atomicAdd(&row_ptr[u], (unsigned long long)(-(long long)__popc(same)));
+        end = __shfl_sync(0xffffffffu, end, leader);
+        if (valid) bucket[end - 1ull - (unsigned long long)__popc(same & lt_mask)] = k;
     }
 }
 
+// TIES: the keys may repeat (a caller's list); the library's own edge lists hold every pair once.
+template <bool TIES>
 __global__ void __launch_bounds__(256) k_rank_rows(const unsigned long long* __restrict__ bucket, int64_t n_keys,
                                                   const int64_t* __restrict__ row_ptr, int32_t* __restrict__ col,
                                                   int32_t* __restrict__ deg, int32_t* __restrict__ long_rows,
@@ -103,11 +117,12 @@ __global__ void __launch_bounds__(256) k_rank_rows(const unsigned long long* __r
         if (len > kRankRow) long_rows[atomicAdd(n_long, 1u)] = (int32_t)u;
     }
     if (len > kRankRow) return;
-    const unsigned long long* a = bucket + b;
+    const uint32_t* a = reinterpret_cast<const uint32_t*>(bucket + b);  // the neighbour is the low word of a key
     int rank = 0;
+#pragma unroll 4
     for (int i = 0; i < len; ++i) {
-        const uint32_t x = (uint32_t)a[i];
-        rank += (x < v) || (x == v && i < my);
+        const uint32_t x = __ldg(a + 2 * i);
+        rank += TIES ? ((x < v) || (x == v && i < my)) : (x < v);
     }
     col[b + rank] = (int32_t)v;
 }
@@ -168,15 +183,17 @@ cudaError_t launch_count_rows(const unsigned long long* keys, int64_t n_keys, in
 
 cudaError_t launch_csr_unsorted(const unsigned long long* keys, int64_t n_keys, int64_t n, int32_t* row_count,
                                 int64_t* row_ptr, unsigned long long* bucket, int32_t* col, int32_t* deg,
-                                int32_t* long_rows, uint32_t* n_long, void* scan_scratch, cudaStream_t s,
-                                int* launches) {
+                                int32_t* long_rows, uint32_t* n_long, void* scan_scratch, bool distinct_keys,
+                                cudaStream_t s, int* launches) {
     cudaError_t e = cudaMemsetAsync(n_long, 0, sizeof(uint32_t), s);  // (ahead of the kernels: none sits between two)
-    if (e == cudaSuccess) e = exclusive_scan_i32_to_i64(row_count, row_ptr, n, true, scan_scratch, s, launches);
+    if (e == cudaSuccess) e = inclusive_scan_i32_to_i64(row_count, row_ptr, n, scan_scratch, s, launches);
     if (e != cudaSuccess || n_keys <= 0) return e;
     const int64_t blocks = (n_keys + 255) / 256;
     launch_dep(k_scatter_keys, (unsigned)std::min<int64_t>(blocks, device_sm_count() * 32), 256, 0, s, keys, n_keys,
-               row_ptr, row_count, bucket);
-    launch_dep(k_rank_rows, (unsigned)blocks, 256, 0, s, bucket, n_keys, row_ptr, col, deg, long_rows, n_long);
+               (unsigned long long*)row_ptr, bucket);
+    if (distinct_keys) launch_dep(k_rank_rows<false>, (unsigned)blocks, 256, 0, s, bucket, n_keys, row_ptr, col, deg,
+                                  long_rows, n_long);
+    else launch_dep(k_rank_rows<true>, (unsigned)blocks, 256, 0, s, bucket, n_keys, row_ptr, col, deg, long_rows, n_long);
     launch_dep(k_sort_long_rows, (unsigned)std::min<int64_t>(n, device_sm_count() * 4), 256, 0, s, row_ptr, bucket,
                col, long_rows, n_long);
     *launches += 3;

@@ -314,10 +314,16 @@ __global__ void __launch_bounds__(256) k_expand_entries(const unsigned long long
                     continue;
                 }
             }
+            // (x, y) = (k / nj, k % nj) kept incrementally: one 32-bit division per lane and product instead of a
+            // 64-bit one per edge
+            uint32_t x = (uint32_t)lane / s_nj, y = (uint32_t)lane % s_nj;
+            const uint32_t dx = 32u / s_nj, dy = 32u % s_nj;
             for (unsigned long long k = (unsigned long long)lane; k < s_w; k += 32ull) {
-                const uint32_t x = (uint32_t)(k / s_nj), y = (uint32_t)(k % s_nj);
                 put(s_first + k, (s_oi & kGroupFlag) ? (uint32_t)members[s_bi + x] : s_oi,
                     (s_oj & kGroupFlag) ? (uint32_t)members[s_bj + y] : s_oj);
+                x += dx;
+                y += dy;
+                if (y >= s_nj) y -= s_nj, ++x;
             }
         }
     }

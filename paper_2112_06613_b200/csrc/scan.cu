@@ -83,7 +83,7 @@ __global__ void __launch_bounds__(1024) k_scan_tile_sums(TOut* __restrict__ tile
 template <typename TIn, typename TOut, bool FUSED>
 __global__ void __launch_bounds__(kScanThreads) k_tile_scan(const TIn* __restrict__ in, TOut* __restrict__ out,
                                                            int64_t n, const TOut* __restrict__ tile_sums,
-                                                           int write_total) {
+                                                           int write_total, int inclusive) {
     grid_dependency_wait();
     constexpr int kScanItems = scan_items(FUSED), kScanTile = kScanThreads * kScanItems;
     __shared__ TOut ws[32];
@@ -123,14 +123,14 @@ __global__ void __launch_bounds__(kScanThreads) k_tile_scan(const TIn* __restric
     for (int k = 0; k < kScanItems; ++k) {
         int idx = k * kScanThreads + threadIdx.x;
         int64_t i = base + idx;
-        if (i < n) out[i] = stage[idx];
+        if (i < n) out[i] = stage[idx] + (inclusive ? (TOut)in[i] : TOut(0));
     }
     if (write_total && blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) out[n] = tile_base + tot;
 }
 
 template <typename TIn, typename TOut>
 cudaError_t scan_impl(const TIn* in, TOut* out, int64_t n, bool write_total, void* scratch, cudaStream_t s,
-                      int* launches) {
+                      int* launches, bool inclusive = false) {
     if (n <= 0) {
         if (write_total) return cudaMemsetAsync(out, 0, sizeof(TOut), s);
         return cudaSuccess;
@@ -141,7 +141,7 @@ cudaError_t scan_impl(const TIn* in, TOut* out, int64_t n, bool write_total, voi
         const int64_t tiles = (n + small_tile - 1) / small_tile;
         launch_dep(k_tile_sums<TIn, TOut, true>, (unsigned)tiles, kScanThreads, 0, s, in, n, sums);
         launch_dep(k_tile_scan<TIn, TOut, true>, (unsigned)tiles, kScanThreads, 0, s, in, out, n, sums,
-                   write_total ? 1 : 0);
+                   write_total ? 1 : 0, inclusive ? 1 : 0);
         *launches += 2;
         return cudaGetLastError();
     }
@@ -149,7 +149,7 @@ cudaError_t scan_impl(const TIn* in, TOut* out, int64_t n, bool write_total, voi
     launch_dep(k_tile_sums<TIn, TOut, false>, (unsigned)tiles, kScanThreads, 0, s, in, n, sums);
     launch_dep(k_scan_tile_sums<TOut>, 1, 1024, 0, s, sums, tiles);
     launch_dep(k_tile_scan<TIn, TOut, false>, (unsigned)tiles, kScanThreads, 0, s, in, out, n, sums,
-               write_total ? 1 : 0);
+               write_total ? 1 : 0, inclusive ? 1 : 0);
     *launches += 3;
     return cudaGetLastError();
 }
@@ -165,6 +165,12 @@ size_t scan_scratch_bytes(int64_t n) {
 cudaError_t exclusive_scan_i32_to_i64(const int32_t* in, int64_t* out, int64_t n, bool write_total, void* scratch,
                                       cudaStream_t s, int* launches) {
     return scan_impl<int32_t, int64_t>(in, out, n, write_total, scratch, s, launches);
+}
+
+// out[i] = in[0] + ... + in[i]; out[n] = the total
+cudaError_t inclusive_scan_i32_to_i64(const int32_t* in, int64_t* out, int64_t n, void* scratch, cudaStream_t s,
+                                      int* launches) {
+    return scan_impl<int32_t, int64_t>(in, out, n, true, scratch, s, launches, true);
 }
 
 cudaError_t exclusive_scan_u32_total(const uint32_t* in, uint32_t* out, int64_t n, void* scratch, cudaStream_t s,

@@ -883,8 +883,8 @@ int assemble_phase(tcrnet_ctx* ctx, int64_t n_keys, bool counts_ready, int* laun
     TRY_CUDA(rec(ctx, 2, 2));
     TRY_CUDA(launch_csr_unsorted((const unsigned long long*)ctx->keys_a.p, n_keys, n, (int32_t*)ctx->row_count.p,
                                  (int64_t*)ctx->row_ptr.p, (unsigned long long*)ctx->keys_b.p, (int32_t*)ctx->col.p,
-                                 (int32_t*)ctx->deg.p, (int32_t*)ctx->long_rows.p, &dc->n_long, ctx->scan_scratch.p, s,
-                                 launches));
+                                 (int32_t*)ctx->deg.p, (int32_t*)ctx->long_rows.p, &dc->n_long, ctx->scan_scratch.p,
+                                 /*distinct_keys=*/counts_ready, s, launches));
     TRY_CUDA(rec(ctx, 3, 2));
     TRY_CUDA(cudaStreamSynchronize(s));
     st.ms_sort = st.ms_csr = 0.f;

@@ -159,6 +159,8 @@ int device_sm_count();
 size_t scan_scratch_bytes(int64_t n);
 cudaError_t exclusive_scan_i32_to_i64(const int32_t* in, int64_t* out, int64_t n, bool write_total,
                                       void* scratch, cudaStream_t s, int* launches);
+cudaError_t inclusive_scan_i32_to_i64(const int32_t* in, int64_t* out, int64_t n, void* scratch, cudaStream_t s,
+                                      int* launches);  // out[i] = in[0] + ... + in[i], out[n] = the total
 cudaError_t exclusive_scan_u32_total(const uint32_t* in, uint32_t* out /*[n+1]*/, int64_t n, void* scratch,
                                      cudaStream_t s, int* launches);
 
@@ -282,13 +284,14 @@ cudaError_t launch_validate_keys(const unsigned long long* keys, int64_t n_keys,
 // counts of caller-supplied keys: row_count[u]++, deg[v]++ (both zeroed by the caller)
 cudaError_t launch_count_rows(const unsigned long long* keys, int64_t n_keys, int32_t* row_count, int32_t* deg,
                               cudaStream_t s, int* launches);
-// CSR + degrees from UNSORTED keys whose counts are in row_count[u] (edges of row u; consumed: all zero
-// afterwards) and deg[v] (edges whose larger endpoint is v).  bucket: uint64[n_keys] scratch,
-// long_rows: int32[n] scratch, n_long: device counter, scan_scratch: scan_scratch_bytes(n).
+// CSR + degrees from UNSORTED keys whose counts are in row_count[u] (edges of row u; left as they are) and
+// deg[v] (edges whose larger endpoint is v).  bucket: uint64[n_keys] scratch, long_rows: int32[n] scratch,
+// n_long: device counter, scan_scratch: scan_scratch_bytes(n).  distinct_keys: no key occurs twice (the
+// library's own edge lists; a caller's list may repeat keys).
 cudaError_t launch_csr_unsorted(const unsigned long long* keys, int64_t n_keys, int64_t n, int32_t* row_count,
                                 int64_t* row_ptr, unsigned long long* bucket, int32_t* col, int32_t* deg,
-                                int32_t* long_rows, uint32_t* n_long, void* scan_scratch, cudaStream_t s,
-                                int* launches);
+                                int32_t* long_rows, uint32_t* n_long, void* scan_scratch, bool distinct_keys,
+                                cudaStream_t s, int* launches);
 // the same from keys that are already sorted (tcrnet_restrict)
 cudaError_t launch_csr(const unsigned long long* sorted_keys, int64_t n_edges, int64_t n, int64_t* row_ptr,
                        int32_t* col, int32_t* deg, cudaStream_t s, int* launches);
