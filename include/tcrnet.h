@@ -58,7 +58,8 @@ typedef enum tcrnet_status {
     TCRNET_ERR_STATE = -5,         /* build before load, csr/degrees before build              */
     TCRNET_ERR_NOMEM = -6,         /* the allocator returned NULL / cudaMalloc failed          */
     TCRNET_ERR_EDGE_OVERFLOW = -7, /* more edges than the configured hard limit                */
-    TCRNET_ERR_CUDA = -8           /* any other CUDA runtime error (see tcrnet_last_cuda_error)*/
+    TCRNET_ERR_CUDA = -8,          /* any other CUDA runtime error (see tcrnet_last_cuda_error)*/
+    TCRNET_ERR_CAPACITY = -9       /* size beyond the fixed capacity of a no-allocation call   */
 } tcrnet_status;
 
 typedef struct tcrnet_ctx tcrnet_ctx; /* opaque */
@@ -392,6 +393,42 @@ TCRNET_API const char* tcrnet_strerror(int status);
 
 /* TCRNET_VERSION the library was built with. */
 TCRNET_API int tcrnet_version(void);
+
+/* ---------------------------------------------------------------------------------------------
+ * A call that allocates nothing - for callers that cannot call cudaMalloc: code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid allocation.  It needs no context.
+ * ------------------------------------------------------------------------------------------- */
+
+#define TCRNET_NOALLOC_MAX_ROWS 2097152 /* 2^21 */
+
+/*
+ * The prefix-sum step of A6 (the network as sorted adjacency lists; row u's list
+ * starts where the lists of the rows before it end):
+ *     row_ptr[0] = 0,  row_ptr[u + 1] = row_ptr[u] + counts[u]   for u = 0..n-1
+ * computed by the kernels tcrnet_build uses for it, with their scratch (one partial sum per tile of
+ * 1,024 counts) in a static device array of the library instead of allocated memory: 16 KB, held by
+ * every GPU that loads the library until the process exits.  No cudaMalloc, cudaFree or allocating
+ * library routine is called; inputs and outputs are the caller's.
+ *
+ *   counts_dev     device, int32[n], each >= 0 (edges of row u whose other endpoint is larger)
+ *   n              0 .. TCRNET_NOALLOC_MAX_ROWS; beyond: TCRNET_ERR_CAPACITY, and nothing is read,
+ *                  written or launched
+ *   row_ptr_dev    device, int64[n + 1], written
+ *   cuda_stream    a cudaStream_t (NULL: the default stream).  The two kernels are enqueued there;
+ *                  the call does not synchronise: row_ptr_dev is valid once the stream gets there.
+ *   cuda_error_out host, may be NULL: the cudaError_t behind a TCRNET_ERR_CUDA, else 0
+ *
+ * The device is the one current on the calling thread (the pointers and the stream belong to it).
+ * The first call on a device looks the array's address up (cudaGetSymbolAddress; the CUDA runtime
+ * may load the module then): make one call - n = 0 will do - before capturing a graph.
+ * ALL calls on a device share the one array: two calls whose kernels overlap on the GPU (different
+ * streams, no dependency between them) race and give wrong sums; calls on one stream, or ordered by
+ * events, are fine.  Nothing in the array has to start at zero: every partial sum a call reads it
+ * has written itself, whatever the previous call left.
+ * Errors: ARG (n < 0, NULL pointer), CAPACITY, CUDA.
+ */
+TCRNET_API int tcrnet_row_ptr_noalloc(const int32_t* counts_dev, int64_t n, int64_t* row_ptr_dev, void* cuda_stream,
+                                      int* cuda_error_out);
 
 /* ---------------------------------------------------------------------------------------------
  * Diagnostics - NOT part of the method: nothing above calls it and no result depends on it.

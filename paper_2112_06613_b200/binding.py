@@ -20,12 +20,14 @@ LIB_PATH = os.path.join(_HERE, "libtcrnet_b200.so")
 # status codes / options (mirrors of the enums in tcrnet.h)
 OK, ERR_ARG, ERR_LENGTH, ERR_RESIDUE, ERR_LMAX, ERR_STATE, ERR_NOMEM, ERR_EDGE_OVERFLOW, ERR_CUDA = (
     0, -1, -2, -3, -4, -5, -6, -7, -8)
+ERR_CAPACITY = -9
+NOALLOC_MAX_ROWS = 1 << 21  # TCRNET_NOALLOC_MAX_ROWS
 OPT_EARLY_EXIT, OPT_FIRST_CHECK, OPT_EDGE_CAPACITY, OPT_EDGE_LIMIT, OPT_COUNT_WORK, OPT_TEXT_CHUNK = 1, 2, 3, 4, 5, 6
 OPT_PREFIX_TRIE, OPT_TRIE_CHUNK, OPT_N_QUERY, OPT_DEDUP, OPT_SEGMENT_JOIN, OPT_FAST_L1, OPT_TIMING = 7, 8, 9, 10, 11, 12, 13
 
 EXPORTS = (
     "tcrnet_create", "tcrnet_destroy", "tcrnet_load", "tcrnet_load_sized", "tcrnet_load_device", "tcrnet_build",
-    "tcrnet_csr",
+    "tcrnet_csr", "tcrnet_row_ptr_noalloc",
     "tcrnet_degrees", "tcrnet_copy_csr", "tcrnet_set_option", "tcrnet_get_stats", "tcrnet_probe_int32",
     "tcrnet_last_cuda_error", "tcrnet_strerror", "tcrnet_version", "tcrnet_build_shard", "tcrnet_assemble",
     "tcrnet_edge_distances", "tcrnet_restrict", "tcrnet_degree_histogram", "tcrnet_neighbor_degree",
@@ -108,6 +110,8 @@ def load_library() -> C.CDLL:
                                        C.POINTER(C.c_double), i64p]
     lib.tcrnet_csr.restype = C.c_int
     lib.tcrnet_csr.argtypes = [vp, C.POINTER(vp), C.POINTER(vp)]
+    lib.tcrnet_row_ptr_noalloc.restype = C.c_int
+    lib.tcrnet_row_ptr_noalloc.argtypes = [vp, C.c_int64, vp, vp, C.POINTER(C.c_int)]
     lib.tcrnet_degrees.restype = C.c_int
     lib.tcrnet_degrees.argtypes = [vp, C.POINTER(vp)]
     lib.tcrnet_copy_csr.restype = C.c_int
@@ -370,6 +374,27 @@ class TcrNet:
 
     def last_cuda_error(self) -> int:
         return int(self._lib.tcrnet_last_cuda_error(self._ctx))
+
+
+def row_ptr_noalloc(counts, row_ptr, n: Optional[int] = None, stream=None) -> None:
+    """tcrnet_row_ptr_noalloc: row_ptr[0] = 0, row_ptr[u + 1] = row_ptr[u] + counts[u], enqueued on `stream` (default:
+    torch's current stream of the tensors' device) - no allocation here or in the library, no synchronisation.
+    counts: int32 CUDA tensor (>= n elements), row_ptr: int64 CUDA tensor (>= n + 1 elements), both the caller's."""
+    import torch
+    assert counts.is_cuda and row_ptr.is_cuda and counts.device == row_ptr.device
+    assert counts.dtype == torch.int32 and row_ptr.dtype == torch.int64
+    assert counts.is_contiguous() and row_ptr.is_contiguous()
+    n = int(counts.numel()) if n is None else int(n)
+    if 0 <= n <= NOALLOC_MAX_ROWS:  # (beyond the capacity the library refuses before it looks at a pointer)
+        assert counts.numel() >= n and row_ptr.numel() >= n + 1
+    lib = load_library()
+    err = C.c_int(0)
+    with torch.cuda.device(counts.device):
+        s = stream if stream is not None else torch.cuda.current_stream(counts.device)
+        status = lib.tcrnet_row_ptr_noalloc(C.c_void_p(counts.data_ptr()), n, C.c_void_p(row_ptr.data_ptr()),
+                                            C.c_void_p(s.cuda_stream), C.byref(err))
+    if status != OK:
+        raise TcrNetError(status, "tcrnet_row_ptr_noalloc" + (f" (cudaError {err.value})" if err.value else ""))
 
 
 def build_network(residues, lengths, l_max: int, device: int = 0):

@@ -4,6 +4,8 @@
 // CTA adding up the sums of the tiles before it itself (<= 8 loads per thread): these scans are latency-bound,
 // so a launch less and four times as many CTAs matter more than the re-read sums.
 // HBM-bound streaming passes: 2 reads + 1 write of the array.
+#include <mutex>
+
 #include "launch.cuh"
 #include "tcrnet_internal.h"
 
@@ -179,3 +181,62 @@ cudaError_t exclusive_scan_u32_total(const uint32_t* in, uint32_t* out, int64_t 
 }
 
 }  // namespace tcrnet
+
+// ---- tcrnet_row_ptr_noalloc (tcrnet.h): the prefix sum with its scratch in a static device array ----
+// For callers that cannot call cudaMalloc (CUDA graph capture, serving loops, harnesses that forbid it): the same two
+// kernels as exclusive_scan_i32_to_i64, their per-tile sums in a file-scope array instead of a buffer of the context.
+// Every GPU that loads the library holds the array (16 KB) until exit.
+namespace {
+
+constexpr int64_t kNoAllocTiles = tcrnet::kFusedTiles;  // tiles of 1024 counts: TCRNET_NOALLOC_MAX_ROWS counts
+static_assert(kNoAllocTiles * tcrnet::kScanThreads * tcrnet::scan_items(true) == TCRNET_NOALLOC_MAX_ROWS,
+              "the header states the limit");
+static __device__ __align__(256) unsigned long long g_noalloc_tile_sums[kNoAllocTiles];
+
+// In host code the array's name is a host-side stand-in, not a device address: the kernels get what
+// cudaGetSymbolAddress returns on the device that is current, looked up once per device.
+constexpr int kMaxDevices = 64;
+void* g_noalloc_addr[kMaxDevices];
+bool g_noalloc_have[kMaxDevices];
+std::mutex g_noalloc_mutex;
+
+cudaError_t noalloc_scratch(void** out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_have[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_noalloc_tile_sums);
+        if (e != cudaSuccess) return e;
+        if (!p) return cudaErrorInvalidSymbol;
+        g_noalloc_addr[dev] = p;
+        g_noalloc_have[dev] = true;
+    }
+    *out = g_noalloc_addr[dev];
+    return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" int tcrnet_row_ptr_noalloc(const int32_t* counts_dev, int64_t n, int64_t* row_ptr_dev, void* cuda_stream,
+                                      int* cuda_error_out) {
+    if (cuda_error_out) *cuda_error_out = 0;
+    if (n < 0 || !row_ptr_dev || (n > 0 && !counts_dev)) return TCRNET_ERR_ARG;
+    if (n > TCRNET_NOALLOC_MAX_ROWS) return TCRNET_ERR_CAPACITY;  // (before anything is read or launched)
+    void* scratch = nullptr;
+    cudaError_t e = noalloc_scratch(&scratch);
+    int launches = 0;
+    // (the sums of the tiles in use are written by the first kernel before the second reads them: nothing in the
+    // array has to start at zero, whatever the last call left there)
+    if (e == cudaSuccess)
+        e = tcrnet::scan_impl<int32_t, int64_t>(counts_dev, row_ptr_dev, n, true, scratch, (cudaStream_t)cuda_stream,
+                                                &launches);
+    if (e != cudaSuccess) {
+        if (cuda_error_out) *cuda_error_out = (int)e;
+        (void)cudaGetLastError();
+        return TCRNET_ERR_CUDA;
+    }
+    return TCRNET_OK;
+}

@@ -939,6 +939,7 @@ const char* tcrnet_strerror(int status) {
         case TCRNET_ERR_NOMEM: return "out of device memory";
         case TCRNET_ERR_EDGE_OVERFLOW: return "edge count exceeds the configured limit";
         case TCRNET_ERR_CUDA: return "CUDA runtime error";
+        case TCRNET_ERR_CAPACITY: return "size beyond the fixed capacity of a no-allocation call";
         default: return "unknown status";
     }
 }

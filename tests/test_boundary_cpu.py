@@ -39,7 +39,7 @@ def test_version_and_strerror(lib):
     import paper_2112_06613_b200 as pkg
     assert pkg.version() == 100
     assert pkg.strerror(0) == "ok"
-    for code in range(-8, 0):
+    for code in range(-9, 0):
         assert pkg.strerror(code) not in ("ok", "unknown status")
     assert pkg.strerror(-99) == "unknown status"
 
@@ -51,6 +51,11 @@ def test_argument_errors_without_a_device(lib):
     assert lib.tcrnet_build(None, 1, None) == pkg.ERR_ARG
     assert lib.tcrnet_get_stats(None, None) == pkg.ERR_ARG
     lib.tcrnet_destroy(None)  # NULL is allowed
+    # the no-allocation call refuses what does not fit its static scratch before it looks at a pointer or at CUDA
+    fake = ctypes.c_void_p(256)
+    assert lib.tcrnet_row_ptr_noalloc(fake, pkg.NOALLOC_MAX_ROWS + 1, fake, None, None) == pkg.ERR_CAPACITY
+    assert lib.tcrnet_row_ptr_noalloc(fake, -1, fake, None, None) == pkg.ERR_ARG
+    assert lib.tcrnet_row_ptr_noalloc(fake, 10, None, None, None) == pkg.ERR_ARG
 
 
 def test_product_fails_loudly_without_gpu():
