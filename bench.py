@@ -51,9 +51,9 @@ ORACLE_SAMPLE_ROWS = 1024
 # summarised under profiles/ (regenerated with them; a workload / kernel that is not listed prints null)
 NCU_DRAM_BYTES_PER_LAUNCH = {
     # (workload, kernel): bytes per step of that kernel / kernel pair - profiles/r2_join_ncu.txt
-    ("cfg4", "k_join_probe"): 35_106_816 + 46_592,
-    ("cfg3", "k_join_probe + k_join_verify"): 11_111_168 + 256 + 11_573_760 + 0,
-    ("cfg5", "k_join_probe + k_join_verify"): 2_324_235_000 + 300_706_816 + 367_888_000 + 52_318_208,
+    ("cfg4", "k_join_probe"): 30_911_744 + 0,
+    ("cfg3", "k_join_probe + k_join_verify"): 9_014_272 + 0 + 11_573_760 + 0,
+    ("cfg5", "k_join_probe + k_join_verify"): 1_270_505_000 + 286_985_472 + 368_325_000 + 53_345_792,
 }
 
 
