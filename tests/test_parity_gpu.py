@@ -294,8 +294,9 @@ def test_products_of_two_heavily_repeated_sequences(pkg, oracle):
 
 
 def test_rows_of_every_sorting_regime(pkg, oracle):
-    """The CSR step orders a row by one thread (<= 32 neighbours), in shared memory (<= 8192) or in place
-    (beyond): a clique of 9,001 copies has rows of every such length; the other strings hang off it."""
+    """The CSR step orders a row by ranking (<= 256 neighbours, one thread per edge), by a bitonic network in shared
+    memory (<= 8192) or in place (beyond): a clique of 9,001 copies has rows of every such length; the other strings
+    hang off it."""
     strings = ["CASSLGQF"] * 5000 + ["CASSLGQW", "CASRLGQF", "CWWWWWWW"] + ["CASSLGQF"] * 4001 + ["CASSLGF"] * 40
     res, ln = from_strings(strings)
     got, _ = gpu_network(pkg, res, ln, 1)
