@@ -130,21 +130,64 @@ __global__ void __launch_bounds__(256) k_rank_rows(const unsigned long long* __r
 }
 
 // Ascending bitonic network over the next power of two of len, the missing tail being virtual +infinity entries
-// (every exchange puts the smaller value at the smaller index, so they never move).  One CTA; jj is a power of two, so
-// the position of an exchange is shifts and masks.
+// (every exchange puts the smaller value at the smaller index, so they never move).  One CTA.  The partner of element
+// e at distance jj is e ^ jj, in the first stage of every k the mirror image e ^ (2 jj - 1).  Exchanges at distance
+// <= 32 stay inside aligned chunks of 64 elements: a warp takes a chunk through all of them in REGISTERS (two elements
+// per lane, partners by shuffle: 9 instructions per stage and lane instead of 35 through shared memory); only the
+// stages of distance >= 64 go through memory, with a block barrier each.
+__device__ __forceinline__ void warp_stage(int32_t& r0, int32_t& r1, int lane, int jj, bool mirror) {
+    constexpr uint32_t kFull = 0xffffffffu;
+    if (jj == 32) {
+        if (mirror) {  // e ^ 63: the other slot of lane ^ 31
+            const int32_t o0 = __shfl_xor_sync(kFull, r1, 31), o1 = __shfl_xor_sync(kFull, r0, 31);
+            r0 = min(r0, o0);
+            r1 = max(r1, o1);
+        } else {       // e ^ 32: the other slot of this lane
+            const int32_t lo = min(r0, r1);
+            r1 = max(r0, r1);
+            r0 = lo;
+        }
+    } else {
+        const int m = mirror ? 2 * jj - 1 : jj;
+        const int32_t o0 = __shfl_xor_sync(kFull, r0, m), o1 = __shfl_xor_sync(kFull, r1, m);
+        const bool lower = (lane & jj) == 0;
+        r0 = lower ? min(r0, o0) : max(r0, o0);
+        r1 = lower ? min(r1, o1) : max(r1, o1);
+    }
+}
+
 template <typename I>
 __device__ __forceinline__ void bitonic_row(int32_t* a, I len) {
-    I p2 = 1;
+    I p2 = 64;
     while (p2 < len) p2 <<= 1;
-    for (I k = 2; k <= p2; k <<= 1) {
-        int lg = 0;
+    const I half = p2 >> 1;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, n_warp = blockDim.x >> 5;
+    // a chunk of 64 through the stages jj_first .. 1 of one k (k_last = 0), or through all of k = 2 .. k_last
+    auto chunks = [&](int jj_first, int k_last) {
+        for (I c = (I)warp * 64; c < p2; c += (I)n_warp * 64) {
+            const I e0 = c + (I)lane, e1 = e0 + 32;
+            int32_t r0 = e0 < len ? a[e0] : INT32_MAX, r1 = e1 < len ? a[e1] : INT32_MAX;  // (row ids are < 2^31 - 2)
+            if (k_last) {
+                for (int k = 2; k <= k_last; k <<= 1)
+                    for (int jj = k >> 1; jj >= 1; jj >>= 1) warp_stage(r0, r1, lane, jj, jj == (k >> 1));
+            } else {
+                for (int jj = jj_first; jj >= 1; jj >>= 1) warp_stage(r0, r1, lane, jj, false);
+            }
+            if (e0 < len) a[e0] = r0;
+            if (e1 < len) a[e1] = r1;
+        }
+        __syncthreads();
+    };
+    chunks(0, 64);  // sorted runs of 64
+    for (I k = 128; k <= p2; k <<= 1) {
+        int lg = 6;
         while (((I)2 << lg) < k) ++lg;  // jj = 1 << lg starts at k / 2
-        for (I jj = k >> 1; jj >= 1; jj >>= 1, --lg) {
-            const bool flip = jj == (k >> 1);
-            for (I t = threadIdx.x; t < (p2 >> 1); t += blockDim.x) {
+        for (I jj = k >> 1; jj >= 64; jj >>= 1, --lg) {
+            const bool mirror = jj == (k >> 1);
+            for (I t = threadIdx.x; t < half; t += blockDim.x) {
                 const I off = t & (jj - 1);
                 const I i = ((t >> lg) << (lg + 1)) + off;
-                const I j = flip ? i + 2 * (jj - off) - 1 : i + jj;
+                const I j = mirror ? i + 2 * (jj - off) - 1 : i + jj;
                 if (j < len) {
                     const int32_t x = a[i], y = a[j];
                     if (x > y) {
@@ -155,6 +198,7 @@ __device__ __forceinline__ void bitonic_row(int32_t* a, I len) {
             }
             __syncthreads();
         }
+        chunks(32, 0);
     }
 }
 
@@ -209,8 +253,8 @@ cudaError_t launch_csr_unsorted(const unsigned long long* keys, int64_t n_keys, 
                                   long_rows, n_long, rank_row);
     else launch_dep(k_rank_rows<true>, (unsigned)blocks, 256, 0, s, bucket, n_keys, row_ptr, col, deg, long_rows, n_long,
                     rank_row);
-    launch_dep(k_sort_long_rows, (unsigned)std::min<int64_t>(n, device_sm_count() * 4), 256, 0, s, row_ptr, bucket,
-               col, long_rows, n_long);
+    launch_dep(k_sort_long_rows, (unsigned)std::min<int64_t>(n, device_sm_count() * 7), 256, 0, s, row_ptr, bucket,
+               col, long_rows, n_long);  // (7 CTAs of 32 KB shared memory per SM)
     *launches += 3;
     return cudaGetLastError();
 }
