@@ -194,6 +194,9 @@ typedef struct tcrnet_stats {
     int64_t join_diagonals;    /* ... per-diagonal mismatch masks built, probe + verify kernels (COUNT_WORK; 0 when
                                   other distance kernels ran in the same build)                               */
     int64_t join_verified_edges; /* ... pairs of distinct sequences the verify kernel (l_max >= 2) accepted     */
+    int32_t join_adapted_lengths;/* ... sequence lengths whose segment cut follows the residue statistics of the load
+                                    (conserved ends) instead of the even cut                                     */
+    int32_t pad3_;
 } tcrnet_stats;
 
 /*

@@ -56,6 +56,8 @@ class tcrnet_stats(C.Structure):
         ("join_candidates", C.c_int64), ("work_items_join", C.c_int64), ("join_index_entries", C.c_int64),
         ("join_mode", C.c_int32), ("pad2_", C.c_int32), ("join_survivors", C.c_int64), ("join_diagonals", C.c_int64),
         ("join_verified_edges", C.c_int64),
+        ("join_adapted_lengths", C.c_int32),
+        ("pad3_", C.c_int32),
     ]
 
 

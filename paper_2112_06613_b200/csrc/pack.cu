@@ -14,6 +14,8 @@
 //   planes : one row of 8 words per sorted position: plane k = bit k of the 5-bit code of every residue
 //         (north_star (1): 5-bit codes, here one bit of the code per word so that a residue-wise comparison of two
 //         sequences under any shift is five XORs) + the length - what the segment join reads (segjoin.cu).
+#include <algorithm>
+
 #include "launch.cuh"
 #include "tcrnet_internal.h"
 
@@ -74,6 +76,10 @@ __global__ void __launch_bounds__(256) k_seq_keys(const uint8_t* __restrict__ re
 // One thread per sorted position: the residues of the row become its bit-plane row (8 words of W: planes 0..4, the
 // length, two zero words).  A collapsed load (dedup.cu) arrives with perm[s] = uid of the distinct sequence; perm[s] is
 // re-coded on the way out: the row itself for a sequence that one row has, kGroupFlag | uid for a shared one.
+// Every sample_stride-th CTA also counts which residue stands at each of the first / last kPosStat positions of its
+// sequences (pos_hist[0][p][c]: residue c at position p; [1][p][c]: at position len - 1 - p): the segment join cuts
+// the texts where that makes its segments equally informative (tcrnet_api.cu: make_join_tables).  A sample is enough -
+// any cut is exact, the statistics only shorten the candidate lists.
 template <typename W>
 __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residues,
                                              const int64_t* __restrict__ offsets,
@@ -81,8 +87,15 @@ __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residu
                                              int32_t* __restrict__ perm, int64_t n,
                                              W* __restrict__ planes, uint32_t* __restrict__ flags,
                                              const uint32_t* __restrict__ group_start,
-                                             const int32_t* __restrict__ members) {
+                                             const int32_t* __restrict__ members, uint32_t* __restrict__ pos_hist,
+                                             uint32_t sample_stride) {
     grid_dependency_wait();
+    __shared__ uint32_t ph[2 * kPosStat * 32];
+    const bool sampled = pos_hist != nullptr && blockIdx.x % sample_stride == 0;
+    if (sampled) {
+        for (int i = threadIdx.x; i < 2 * kPosStat * 32; i += blockDim.x) ph[i] = 0u;
+        __syncthreads();
+    }
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;  // sorted position
     bool bad = false;
     if (s < n) {
@@ -99,6 +112,14 @@ __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residu
 #pragma unroll
             for (int b = 0; b < 5; ++b) pl[b] |= (W)((c >> b) & 1u) << i;
         }
+        // (a loop of its own: inside the loop above it doubled the kernel's duration for every CTA; every 8th row only:
+        // hot residues serialise the shared-memory atomics)
+        if (sampled && (threadIdx.x & 7) == 0 && !bad)
+            for (int i = 0; i < len; ++i) {
+                const uint32_t c = (uint32_t)src[i] - (uint32_t)'A';
+                if (i < kPosStat) atomicAdd(&ph[i * 32 + c], 1u);
+                if (len - 1 - i < kPosStat) atomicAdd(&ph[(kPosStat + len - 1 - i) * 32 + c], 1u);
+            }
         W* row = planes + (size_t)s * kPlaneWords;
         if (sizeof(W) == 4) {
             uint4* r4 = reinterpret_cast<uint4*>(row);
@@ -117,6 +138,9 @@ __global__ void __launch_bounds__(256) k_pack(const uint8_t* __restrict__ residu
         }
     }
     if (__syncthreads_or(bad) && threadIdx.x == 0) atomicOr(flags, kFlagBadResidue);
+    if (sampled)  // (the barrier above has made the counts of the CTA visible)
+        for (int i = threadIdx.x; i < 2 * kPosStat * 32; i += blockDim.x)
+            if (ph[i]) atomicAdd(pos_hist + i, ph[i]);
 }
 
 // The rows of the prefix-trie / text-chunk kernels from the bit-plane rows, written only when a build needs those
@@ -201,14 +225,15 @@ cudaError_t launch_seq_keys(const uint8_t* residues, const int64_t* offsets, con
 
 cudaError_t launch_pack(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths, int32_t* perm, int64_t n,
                         void* planes, bool wide_planes, uint32_t* flags, const uint32_t* group_start,
-                        const int32_t* members, cudaStream_t s, int* launches) {
+                        const int32_t* members, uint32_t* pos_hist, cudaStream_t s, int* launches) {
     const unsigned blocks = (unsigned)((n + 255) / 256);
+    const uint32_t stride = std::max(1u, blocks / 128u);  // about 128 CTAs x 32 rows = 4,096 sequences are sampled
     if (wide_planes)
         launch_dep(k_pack<uint64_t>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, (uint64_t*)planes, flags,
-                   group_start, members);
+                   group_start, members, pos_hist, stride);
     else
         launch_dep(k_pack<uint32_t>, blocks, 256, 0, s, residues, offsets, lengths, perm, n, (uint32_t*)planes, flags,
-                   group_start, members);
+                   group_start, members, pos_hist, stride);
     *launches += 1;
     return cudaGetLastError();
 }

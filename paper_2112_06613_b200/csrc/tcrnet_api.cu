@@ -2,6 +2,7 @@
 // scheduler (step A2) and the orchestration of steps A1-A6 on one CUDA stream.
 #include <algorithm>
 #include <cstddef>
+#include <cmath>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -171,7 +172,7 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
     if (e == cudaSuccess)
         e = launch_pack(d_res, d_off, d_len, (int32_t*)set.perm.p, n, set.planes.p, set.wide_planes, &dc->flags,
                         code_groups ? (const uint32_t*)set.group_start.p : nullptr,
-                        code_groups ? (const int32_t*)set.members.p : nullptr, s, launches);
+                        code_groups ? (const int32_t*)set.members.p : nullptr, &dc->pos_hist[0][0][0], s, launches);
     // (the text rows and the prefix trie are built by ensure_text_tables when a build needs them)
     // (collapsed load: the pack kernel has re-coded perm from uids to rows / kGroupFlag | uid)
     if (rc == TCRNET_OK && e == cudaSuccess)
@@ -181,6 +182,18 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
     if (rc != TCRNET_OK) return rc;
     TRY_CUDA(e);
     if (ctx->h_ctrl->flags & kFlagBadResidue) return TCRNET_ERR_RESIDUE;
+    // how informative the residue at each of the first / last positions is: -log2 of the probability that two sampled
+    // sequences agree there (0: too few samples to tell)
+    for (int d = 0; d < 2; ++d)
+        for (int p = 0; p < kPosStat; ++p) {
+            double tot = 0, sq = 0;
+            for (int c = 0; c < 32; ++c) {
+                const double v = (double)ctx->h_ctrl->pos_hist[d][p][c];
+                tot += v;
+                sq += v * v;
+            }
+            set.pos_bits[d][p] = tot >= 64 ? (float)std::max(0.01, -std::log2(sq / (tot * tot))) : 0.f;
+        }
     set.n = n;
     set.total_len = total_len;
     set.min_len = min_len;
@@ -376,21 +389,65 @@ struct Schedule {
 // n = q k + r: every segment gets q residues and r of them one more - the two outer ones first, then inwards,
 // because CDR3 sequences are least diverse at their ends (conserved first / last residues), so the outer segments
 // need the extra residue most.  Any cut is exact; this one only keeps the candidate lists short.
-bool make_join_tables(int l_max, JoinTables& tab) {
+// `set`: where its residue statistics (pack.cu) say that another cut makes the LEAST informative segment of a length
+// clearly more informative (real CDR3 start CASS.. and end ..EQYF: with l_max = 1 the halves of a 15-residue text then
+// hold 4 + 3 free residues, cutting one residue later gives 3.5 + 3.5), that cut is taken; *adapted counts such lengths.
+bool make_join_tables(int l_max, const SeqSet* set, JoinTables& tab, int* adapted) {
     std::memset(&tab, 0, sizeof(tab));
     const int k = l_max + 1;
     tab.n_seg = (int8_t)k;
+    if (adapted) *adapted = 0;
+    bool have_stats = false;
+    if (set)
+        for (int p = 0; p < kPosStat; ++p) have_stats = have_stats || set->pos_bits[0][p] > 0.f || set->pos_bits[1][p] > 0.f;
     for (int n = 0; n < kNumLen; ++n) {
         const int q = n / k, r = n % k;
         int extra[kJoinMaxSeg] = {};
         for (int x = 0, lo = 0, hi = k - 1; x < r; ++x) {
             if (x % 2 == 0) extra[lo++] = 1; else extra[hi--] = 1;
         }
-        int pos = 0;
-        for (int i = 0; i < k; ++i) {
-            tab.seg_start[n][i] = (uint8_t)pos;
-            pos += q + extra[i];
+        int cut[kJoinMaxSeg + 1];  // segment i = [cut[i], cut[i + 1])
+        cut[0] = 0;
+        for (int i = 0; i < k; ++i) cut[i + 1] = cut[i] + q + extra[i];
+        if (have_stats && n >= k && k >= 2 && set->hist[n] > 0) {
+            constexpr float kUnknown = 4.f;  // (bits; 20 equally likely residues would be 4.3)
+            float bits[kMaxLen + 1], pre[kMaxLen + 2];
+            pre[0] = 0.f;
+            for (int p = 0; p < n; ++p) {
+                const int back = n - 1 - p;
+                float b = p <= back ? (p < kPosStat ? set->pos_bits[0][p] : 0.f) : (back < kPosStat ? set->pos_bits[1][back] : 0.f);
+                bits[p] = b > 0.f ? b : kUnknown;
+                pre[p + 1] = pre[p] + bits[p];
+            }
+            auto seg_bits = [&](int b0, int e0) { return pre[e0] - pre[b0]; };
+            float def_min = 1e30f;
+            for (int i = 0; i < k; ++i) def_min = std::min(def_min, seg_bits(cut[i], cut[i + 1]));
+            // best[j][e]: the largest possible minimum over j segments that cover [0, e)
+            static thread_local float best[kJoinMaxSeg + 1][kMaxLen + 1];
+            static thread_local int8_t from[kJoinMaxSeg + 1][kMaxLen + 1];
+            for (int e0 = 1; e0 <= n; ++e0) best[1][e0] = seg_bits(0, e0), from[1][e0] = 0;
+            for (int j = 2; j <= k; ++j)
+                for (int e0 = j; e0 <= n; ++e0) {
+                    float bv = -1.f;
+                    int bs = j - 1;
+                    for (int s0 = j - 1; s0 < e0; ++s0) {
+                        const float v = std::min(best[j - 1][s0], seg_bits(s0, e0));
+                        if (v > bv) bv = v, bs = s0;
+                    }
+                    best[j][e0] = bv;
+                    from[j][e0] = (int8_t)bs;
+                }
+            if (best[k][n] > def_min + 0.75f) {
+                int e0 = n;
+                for (int j = k; j >= 1; --j) {
+                    cut[j] = e0;
+                    e0 = from[j][e0];
+                }
+                cut[0] = 0;
+                if (adapted) ++*adapted;
+            }
         }
+        for (int i = 0; i < k; ++i) tab.seg_start[n][i] = (uint8_t)cut[i];
         for (int i = k; i <= kJoinMaxSeg; ++i) tab.seg_start[n][i] = (uint8_t)n;
     }
     for (int delta = 0; delta <= l_max; ++delta) {
@@ -573,7 +630,7 @@ int64_t join_index_entries(const SeqSet& set, int l_max) {
 int build_join_index(tcrnet_ctx* ctx, int l_max, cudaStream_t s, DevBuf& scan_scratch, int* launches) {
     const SeqSet& set = ctx->all;
     const int64_t n_idx = join_index_entries(set, l_max);
-    if (l_max > kJoinMaxL || !make_join_tables(l_max, ctx->join_tab)) return TCRNET_ERR_LMAX;
+    if (l_max > kJoinMaxL || !make_join_tables(l_max, &set, ctx->join_tab, &ctx->join_adapted)) return TCRNET_ERR_LMAX;
     uint32_t slots = 1024;
     // (one slot per entry at least: a bucket then holds 0.5-1 foreign entries on average, which the walk drops by their
     // segment number / residues; twice the slots cost more in the index build - memset, prefix sum - and in cold
@@ -624,6 +681,10 @@ int ensure_join_index(tcrnet_ctx* ctx, int l_max, int* launches) {
     st.ms_index = 0.f;
     st.join_index_entries = join_index_entries(ctx->all, l_max);
     TRY(settle_index(ctx));
+    struct SetAdapted {  // (whichever path leaves the index in place: the count belongs to it)
+        tcrnet_ctx* c;
+        ~SetAdapted() { c->stats.join_adapted_lengths = c->join_adapted; }
+    } set_adapted{ctx};
     ctx->ahead_l_max = l_max;
     if (ctx->join_l_max == l_max) return TCRNET_OK;
     TRY_CUDA(rec(ctx, 6, 2));

@@ -30,6 +30,7 @@ struct HostCtrl {  // pinned mirror of the small device control block
     uint32_t pad2_;
     unsigned long long hist_u[kNumLen];  // dedup: length histogram of the distinct sequences
     unsigned long long clique_edges;     // dedup: edges among the rows of the shared sequences (known at load)
+    uint32_t pos_hist[2][kPosStat][32];  // pack: residue counts at the first / last positions of a sample of the rows
 };
 
 // One packed set of sequences: all rows, or the query rows of the rectangular mode.
@@ -42,6 +43,7 @@ struct SeqSet {
     int pat_stride = 0;
     DevBuf perm, pat, txt, trie, planes;
     bool wide_planes = false;  // bit-plane rows of 64-bit words (the longest sequence has more than 32 residues)
+    float pos_bits[2][kPosStat] = {};  // collision entropy (bits) of the residue at the first / last positions; 0: unknown
     bool lexicographic = false;  // sorted by (length, first residues): the prefix trie can be built; else by length only
     bool text_tables = false;  // txt + trie are built (on demand: only the prefix-trie / text-chunk kernels read them)
     TrieLevels trie_levels{};
@@ -101,6 +103,7 @@ struct tcrnet_ctx {
     // segment join (segjoin.cu): directory + entries of the current load for join_l_max, work rows
     DevBuf join_cnt, join_dir, join_entries, join_rows, join_cand, join_scan_scratch;
     int64_t join_cand_cap = 0;  // pairs the verification queue join_cand holds (uint2[cap] followed by uint8[cap])
+    int join_adapted = 0; // lengths whose segment cut was adapted to the residue statistics (make_join_tables)
     int join_l_max = -1;  // threshold the index in join_dir / join_entries was built for (-1: none)
     uint32_t join_slots = 0;
     JoinTables join_tab{};

@@ -110,6 +110,7 @@ struct DistanceParams {
 // (l_max edits touch at most l_max segments), shifted by no more than the edits allow.  The segments of every
 // text are indexed in a hash directory; every pattern probes it with the substrings that could be such a
 // segment, and only the pairs found this way are verified.
+constexpr int kPosStat = 32;                // residue statistics of the first / last kPosStat positions (pack.cu)
 constexpr int kJoinMaxL = 6;                // the join kernels are specialised on l_max = 0..kJoinMaxL
 constexpr int kJoinMaxSeg = kJoinMaxL + 1;  // segments per text: l_max + 1 <= 7
 constexpr int kJoinMaxProbes = 40;          // (segment, shift) probes per length difference: 1, 3, 7, 12, 19, 27, 37
@@ -190,7 +191,8 @@ cudaError_t launch_seq_keys(const uint8_t* residues, const int64_t* offsets, con
 // re-coded in place (the row of an unshared sequence, or kGroupFlag | uid)
 cudaError_t launch_pack(const uint8_t* residues, const int64_t* offsets, const int32_t* lengths, int32_t* perm, int64_t n,
                         void* planes, bool wide_planes, uint32_t* flags, const uint32_t* group_start,
-                        const int32_t* members, cudaStream_t s, int* launches);
+                        const int32_t* members, uint32_t* pos_hist /*[2][kPosStat][32], zeroed; may be NULL*/,
+                        cudaStream_t s, int* launches);
 // pat rows (match masks) and txt rows of the trie / text-chunk kernels from the bit-plane rows, on demand
 cudaError_t launch_rows_from_planes(const void* planes, bool wide_planes, int64_t n, const LengthTable& lt, int pat_stride,
                                     uint8_t* pat, uint32_t* txt, cudaStream_t s, int* launches);

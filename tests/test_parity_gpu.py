@@ -145,6 +145,49 @@ def test_segment_join_does_not_change_the_result(pkg, oracle):
     assert st["join_mode"] == 0
 
 
+def test_segment_cuts_follow_the_residue_statistics(pkg, oracle):
+    """Conserved ends (real CDR3-beta: CASS.. / ..EQYF) leave the outer segments of an even cut with one or two
+    informative residues; the load samples the residues per position and the index cuts where the least informative
+    segment gains most (make_join_tables).  Any cut is exact: the CASS-shaped stress input and an input whose first
+    six residues only are conserved (the cut moves at l_max = 1 too), every threshold of the join, against the oracle."""
+    d = generate("cfg4_cass", n=12000)
+    for l_max in (0, 1, 2, 3, 4):
+        want = oracle.network(d.residues, d.lengths, l_max, tier=1)[:3]
+        got, st = gpu_network(pkg, d.residues, d.lengths, l_max)
+        # (l_max <= 1: the two halves of a text with four conserved residues at either end are balanced as they are)
+        assert st["join_mode"] >= 1 and (st["join_adapted_lengths"] > 0 or l_max <= 1)
+        assert_same_network(got, want)
+        got, _ = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_DEDUP: 0})
+        assert_same_network(got, want)
+    rng = np.random.default_rng(77)
+    letters = "ACDEFGHIKLMNPQRSTVWY"
+    strings = []
+    for _ in range(1500):
+        s0 = list("CASSLG") + [letters[i] for i in rng.integers(0, 20, int(rng.integers(4, 14)))]
+        strings.append("".join(s0))
+        for _ in range(int(rng.integers(0, 4))):
+            t = list(s0)
+            for _ in range(int(rng.integers(1, 4))):
+                q = int(rng.integers(5, len(t)))
+                op = int(rng.integers(0, 3))
+                if op == 0:
+                    t[q] = letters[int(rng.integers(0, 20))]
+                elif op == 1:
+                    t.insert(q, letters[int(rng.integers(0, 20))])
+                elif len(t) > 8:
+                    del t[q]
+            strings.append("".join(t))
+    res, ln = from_strings([strings[i] for i in rng.permutation(len(strings))])
+    for l_max in (1, 2, 3, 5, 6):
+        want = oracle.network(res, ln, l_max, tier=0)[:3]
+        got, st = gpu_network(pkg, res, ln, l_max)
+        assert st["join_adapted_lengths"] > 0
+        assert_same_network(got, want)
+    # a load whose positions are all equally informative keeps the even cut
+    _, st = gpu_network(pkg, *[getattr(generate("cfg2", n=20000), k) for k in ("residues", "lengths")], 2)
+    assert st["join_adapted_lengths"] == 0
+
+
 def test_prefix_trie_shared_prefixes_and_short_buckets(pkg, oracle):
     """Real CDR3-beta rows mostly start CASS...: few distinct prefixes, deep shared runs, many
     duplicates; plus buckets shorter than the trie depth (they take the text-chunk kernel), every
@@ -620,12 +663,12 @@ def test_host_loads_reuse_the_buffers_of_the_previous_load(pkg):
 
 
 # ------------------------------------------------------------------ BASELINE.json's large configs
-def _sampled_parity(pkg, oracle, name, l_max, n_sample, seed, opts=None):
+def _sampled_parity(pkg, oracle, name, l_max, n_sample, seed, opts=None, n=None):
     """What the oracle cannot compute in full: (i) the FULL neighbourhoods of n_sample uniformly drawn nodes (drawn from
     the generator's row count alone, never from the GPU's output) against the tier-1 oracle, every partner visited;
     (ii) EVERY edge the GPU emitted has oracle distance <= l_max (no spurious edge anywhere in the network);
     (iii) CSR invariants; (iv) the generator-linked lower bound over all family pairs."""
-    d = generate(name)
+    d = generate(name) if n is None else generate(name, n=n)
     (rp, cl, dg), st = gpu_network(pkg, d.residues, d.lengths, l_max, opts)
     check_csr_invariants(rp, cl, dg, d.n)
     rng = np.random.default_rng(seed)
@@ -738,6 +781,14 @@ def test_cfg4_whole_network_is_the_same_row_by_row(pkg):
     assert st_on["n_distinct"] < st_off["n_distinct"] == d.n
     assert_same_network(on, off)
     check_csr_invariants(*on, d.n)
+
+
+def test_cass_shaped_input_sampled_at_large_size(pkg, oracle):
+    """The stress input of DESIGN.md section 6 (every row CASS...EQYF; here N = 400,000) at l_max = 2, where the segment
+    cuts follow the residue statistics: 1,000 uniformly drawn nodes' full neighbourhoods and every one of the 1.9e7
+    emitted edges against the oracle."""
+    st, _ = _sampled_parity(pkg, oracle, "cfg4_cass", 2, 1000, 6, n=400000)
+    assert st["join_mode"] == 1 and st["join_adapted_lengths"] >= 10
 
 
 def test_cfg5_sampled(pkg, oracle):
