@@ -51,9 +51,9 @@ ORACLE_SAMPLE_ROWS = 1024
 # summarised under profiles/ (regenerated with them; a workload / kernel that is not listed prints null)
 NCU_DRAM_BYTES_PER_LAUNCH = {
     # (workload, kernel): bytes per step of that kernel / kernel pair - profiles/r2_join_ncu.txt
-    ("cfg4", "k_join_probe"): 30_911_744 + 0,
-    ("cfg3", "k_join_probe + k_join_verify"): 9_014_272 + 0 + 11_573_760 + 0,
-    ("cfg5", "k_join_probe + k_join_verify"): 1_270_505_000 + 286_985_472 + 368_325_000 + 53_345_792,
+    ("cfg4", "k_join_probe"): 30_912_000 + 0,
+    ("cfg3", "k_join_probe + k_join_verify"): 9_014_016 + 512 + 11_573_504 + 0,
+    ("cfg5", "k_join_probe + k_join_verify"): 1_270_800_000 + 287_637_504 + 367_959_000 + 53_251_328,
 }
 
 
@@ -554,7 +554,7 @@ def main() -> None:
             extras = {}
             # (a) the length-bucket path of round 1 (every length-compatible pair through the prefix trie): its own
             #     roofline line, measured outside the timed region
-            def side(opts, data=None, k=3):
+            def side(opts, data=None, k=3, lm=None):
                 with pkg.TcrNet(local_rank) as other:
                     for o, v in opts.items():
                         other.set_option(o, v)
@@ -562,7 +562,7 @@ def main() -> None:
 
                     def one():
                         other.load(r_d, l_d)
-                        other.build(l_max)
+                        other.build(l_max if lm is None else lm)
                     other.set_option(pkg.OPT_COUNT_WORK, 1)
                     one()
                     w = other.get_stats()
@@ -592,6 +592,13 @@ def main() -> None:
                 extras["cass_prefix_input"] = {"edges": int(st_c[-1]["n_edges"]), "n_distinct": int(w_c["n_distinct"]),
                                                "join_candidates": int(w_c["join_candidates"]),
                                                "ms_distance_kernel": float(np.mean([s["ms_kernel"] for s in st_c]))}
+                # ... and at l_max = 2, where the segment cuts follow the residue statistics of the load
+                ms_c2, w_c2, st_c2 = side({}, data, lm=2)
+                extras["cass_prefix_input_l_max_2"] = {
+                    "ms_step": ms_c2, "edges": int(st_c2[-1]["n_edges"]),
+                    "join_entries": int(w_c2["join_entries"]), "join_candidates": int(w_c2["join_candidates"]),
+                    "join_adapted_lengths": int(w_c2["join_adapted_lengths"]),
+                    "ms_distance_kernel": float(np.mean([s["ms_kernel"] for s in st_c2]))}
                 del data
             out["detail"].update(extras)
             probes = {}
