@@ -253,9 +253,18 @@ cudaError_t launch_csr_unsorted(const unsigned long long* keys, int64_t n_keys, 
                                   long_rows, n_long, rank_row);
     else launch_dep(k_rank_rows<true>, (unsigned)blocks, 256, 0, s, bucket, n_keys, row_ptr, col, deg, long_rows, n_long,
                     rank_row);
+    *launches += 2;
+    return cudaGetLastError();
+}
+
+// The rows k_rank_rows queued (more than kRankRow neighbours).  Launched by the caller once it has read *n_long back
+// with the build's final synchronisation and found it non-zero: repertoires without conserved ends have no such row,
+// and a launch that finds nothing to do still costs 3 us.
+cudaError_t launch_sort_long_rows(int64_t n, const int64_t* row_ptr, const unsigned long long* bucket, int32_t* col,
+                                  const int32_t* long_rows, const uint32_t* n_long, cudaStream_t s, int* launches) {
     launch_dep(k_sort_long_rows, (unsigned)std::min<int64_t>(n, device_sm_count() * 7), 256, 0, s, row_ptr, bucket,
                col, long_rows, n_long);  // (7 CTAs of 32 KB shared memory per SM)
-    *launches += 3;
+    *launches += 1;
     return cudaGetLastError();
 }
 

@@ -164,13 +164,16 @@ __global__ void __launch_bounds__(256) k_dedup_groups(const int32_t* __restrict_
 __global__ void __launch_bounds__(256) k_dedup_fill(const int32_t* __restrict__ uid_of, int64_t n,
                                                    const uint32_t* __restrict__ group_start,
                                                    uint32_t* __restrict__ group_count, int32_t* __restrict__ members,
-                                                   unsigned long long* __restrict__ clique_edges) {
+                                                   unsigned long long* __restrict__ clique_edges,
+                                                   uint32_t* __restrict__ max_group) {
     grid_dependency_wait();
     __shared__ unsigned long long block_sum;
-    if (threadIdx.x == 0) block_sum = 0ull;
+    __shared__ uint32_t block_max;
+    if (threadIdx.x == 0) block_sum = 0ull, block_max = 0u;
     __syncthreads();
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     unsigned long long mine = 0ull;
+    uint32_t g_mine = 0u;
     if (i < n) {
         const uint32_t uid = (uint32_t)uid_of[i];
         const uint32_t slot = atomicSub(&group_count[uid], 1u) - 1u;
@@ -179,14 +182,20 @@ __global__ void __launch_bounds__(256) k_dedup_fill(const int32_t* __restrict__ 
         if (slot == 0u) {
             const unsigned long long g = group_start[uid + 1u] - b;
             mine = g * (g - 1ull) / 2ull;
+            g_mine = (uint32_t)g;
         }
     }
+    // ... and the largest group: the expansion of the recorded pairs needs its second kernel only if two groups can
+    // have more than kHuge pairs of rows between them
+    g_mine = __reduce_max_sync(0xffffffffu, g_mine);
+    if ((threadIdx.x & 31) == 0 && g_mine > 1u) atomicMax(&block_max, g_mine);
     // one atomic per CTA on the global sum (one per shared sequence on a single address cost 40 us at config 4)
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) mine += __shfl_xor_sync(0xffffffffu, mine, o);
     if ((threadIdx.x & 31) == 0 && mine) atomicAdd(&block_sum, mine);
     __syncthreads();
     if (threadIdx.x == 0 && block_sum) atomicAdd(clique_edges, block_sum);
+    if (threadIdx.x == 0 && block_max) atomicMax(max_group, block_max);
 }
 
 // Edges between the rows of one sequence: the thread of member slot x joins it to the slots after it.  Output
@@ -420,8 +429,10 @@ cudaError_t launch_dedup_groups(const int32_t* rep_of, const uint32_t* first_ran
 }
 
 cudaError_t launch_dedup_fill(const int32_t* uid_of, int64_t n, const uint32_t* group_start, uint32_t* group_count,
-                              int32_t* members, unsigned long long* clique_edges, cudaStream_t s, int* launches) {
-    launch_dep(k_dedup_fill, grid_for(n), 256, 0, s, uid_of, n, group_start, group_count, members, clique_edges);
+                              int32_t* members, unsigned long long* clique_edges, uint32_t* max_group, cudaStream_t s,
+                              int* launches) {
+    launch_dep(k_dedup_fill, grid_for(n), 256, 0, s, uid_of, n, group_start, group_count, members, clique_edges,
+               max_group);
     *launches += 1;
     return cudaGetLastError();
 }
@@ -439,13 +450,15 @@ cudaError_t launch_expand_entries(const unsigned long long* entries, const unsig
                                   unsigned long long entry_cap, const uint32_t* group_start, const int32_t* members,
                                   unsigned long long* edges, unsigned long long* edge_total, unsigned long long edge_cap,
                                   int32_t* row_count, int32_t* deg, void* huge, unsigned long long* n_huge,
-                                  uint32_t huge_cap, int n_sm, cudaStream_t s, int* launches) {
+                                  uint32_t huge_cap, bool huge_possible, int n_sm, cudaStream_t s, int* launches) {
     launch_dep(k_expand_entries, (unsigned)(n_sm * 8), 256, 0, s, entries, n_entries_dev, entry_cap, group_start, members, edges,
                                                           edge_total, edge_cap, row_count, deg, (ulonglong2*)huge, n_huge,
-                                                          huge_cap);
+                                                          huge_possible ? huge_cap : 0u);  // (0: nothing is set aside)
+    *launches += 1;
+    if (!huge_possible) return cudaGetLastError();  // (no two groups of the load have more than kHuge pairs of rows)
     launch_dep(k_expand_huge, (unsigned)(n_sm * 8), 256, 0, s, (const ulonglong2*)huge, n_huge, huge_cap, group_start, members,
                                                        edges, edge_cap, row_count, deg);
-    *launches += 2;
+    *launches += 1;
     return cudaGetLastError();
 }
 

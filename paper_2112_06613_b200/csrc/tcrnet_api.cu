@@ -65,6 +65,7 @@ void drop_load(tcrnet_ctx* ctx) {
     ctx->all.loaded = ctx->query.loaded = false;
     ctx->n = 0;
     ctx->clique_edges = 0;
+    ctx->max_group = 0;
     ctx->join_l_max = -1;  // the segment index belongs to a load
 }
 
@@ -300,7 +301,7 @@ int dedup_rows(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t
     TRY_CUDA(exclusive_scan_u32_total(count, (uint32_t*)set.group_start.p, n + 1, ctx->scan_scratch.p, ctx->side_stream,
                                       launches));
     TRY_CUDA(launch_dedup_fill((const int32_t*)set.uid_of.p, n, (const uint32_t*)set.group_start.p, count,
-                               (int32_t*)set.members.p, &dc->clique_edges, ctx->side_stream, launches));
+                               (int32_t*)set.members.p, &dc->clique_edges, &dc->max_group, ctx->side_stream, launches));
     TRY_CUDA(cudaEventRecord(ctx->ev_join, ctx->side_stream));
     ctx->side_pending = true;
     TRY_CUDA(cudaStreamSynchronize(s));
@@ -338,6 +339,7 @@ int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len
             join_side_stream(ctx);
             TRY(rc_pack);
             ctx->clique_edges = (int64_t)ctx->h_ctrl->clique_edges;  // (read back with the pack's flags)
+            ctx->max_group = ctx->h_ctrl->max_group;
             ctx->all.grouped = true;
             ctx->all.n_rows = n;
         }
@@ -798,8 +800,8 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
         const int32_t* mem = (const int32_t*)ctx->all.members.p;
         TRY_CUDA(launch_expand_entries((const unsigned long long*)ctx->keys_a.p, &dc->edge_count, cap, gs, mem,
                                        (unsigned long long*)ctx->keys_b.p, &dc->edge_total, cap_b, (int32_t*)ctx->row_count.p,
-                                       (int32_t*)ctx->deg.p, ctx->expand_huge.p, &dc->n_huge, kExpandHugeCap, ctx->n_sm, s,
-                                       launches));
+                                       (int32_t*)ctx->deg.p, ctx->expand_huge.p, &dc->n_huge, kExpandHugeCap,
+                                       /*huge_possible=*/ctx->max_group > 64u, ctx->n_sm, s, launches));
         TRY_CUDA(cudaStreamWaitEvent(s, ctx->ev_join, 0));  // the cliques are in
         TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->edge_total, &dc->edge_total, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
     }
@@ -949,8 +951,21 @@ int assemble_phase(tcrnet_ctx* ctx, int64_t n_keys, bool counts_ready, int* laun
                                  (int64_t*)ctx->row_ptr.p, (unsigned long long*)ctx->keys_b.p, (int32_t*)ctx->col.p,
                                  (int32_t*)ctx->deg.p, (int32_t*)ctx->long_rows.p, &dc->n_long, ctx->scan_scratch.p,
                                  /*distinct_keys=*/counts_ready, s, launches));
-    TRY_CUDA(rec(ctx, 3, 2));
-    TRY_CUDA(cudaStreamSynchronize(s));
+    TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->n_long, &dc->n_long, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+    if (ctx->timing >= 2) {  // (the phase events bracket the whole step: no read-back in between)
+        if (n_keys > 0)
+            TRY_CUDA(launch_sort_long_rows(n, (const int64_t*)ctx->row_ptr.p, (const unsigned long long*)ctx->keys_b.p,
+                                           (int32_t*)ctx->col.p, (const int32_t*)ctx->long_rows.p, &dc->n_long, s, launches));
+        TRY_CUDA(rec(ctx, 3, 2));
+        TRY_CUDA(cudaStreamSynchronize(s));
+    } else {
+        TRY_CUDA(cudaStreamSynchronize(s));
+        if (n_keys > 0 && ctx->h_ctrl->n_long > 0) {  // rows of more than 256 neighbours: ordered by their own kernel
+            TRY_CUDA(launch_sort_long_rows(n, (const int64_t*)ctx->row_ptr.p, (const unsigned long long*)ctx->keys_b.p,
+                                           (int32_t*)ctx->col.p, (const int32_t*)ctx->long_rows.p, &dc->n_long, s, launches));
+            TRY_CUDA(cudaStreamSynchronize(s));
+        }
+    }
     st.ms_sort = st.ms_csr = 0.f;
     if (ctx->timing >= 2) {
         TRY_CUDA(cudaEventElapsedTime(&st.ms_sort, ctx->ev[1], ctx->ev[2]));

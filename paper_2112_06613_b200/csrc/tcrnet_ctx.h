@@ -24,7 +24,7 @@ struct HostCtrl {  // pinned mirror of the small device control block
     uint32_t flags;
     uint32_t n_long;                  // rows queued for k_sort_long_rows
     uint32_t n_distinct;              // dedup: distinct sequences of the load
-    uint32_t pad_;
+    uint32_t max_group;               // dedup: rows of the most repeated sequence
     uint32_t trie_counts[8];          // [k] = nodes of trie level k
     uint32_t trie_root[kNumLen + 1];  // [L] = first level-1 node of length bucket L (non-empty buckets)
     uint32_t pad2_;
@@ -85,6 +85,7 @@ struct tcrnet_ctx {
     int64_t n = 0;
     SeqSet all, query;
     unsigned long long hist_u_host[kNumLen] = {};  // length histogram of the distinct sequences of the last collapse
+    uint32_t max_group = 0;          // rows of the most repeated sequence of the current load (collapsed loads)
     int64_t clique_edges = 0;        // edges among identical rows of the current load (collapsed loads)
     int64_t row_hist[kNumLen] = {};  // length histogram of the ROWS (all.hist counts distinct sequences when grouped)
     DevBuf in_res, in_len, offsets, perm_tmp, trie_scratch;  // load scratch, kept between loads (grow-only)

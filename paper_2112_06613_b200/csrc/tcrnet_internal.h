@@ -225,7 +225,8 @@ cudaError_t launch_dedup_groups(const int32_t* rep_of, const uint32_t* first_ran
 // group_start = exclusive scan of group_count (n_u + 1 entries); group_count is consumed
 // *clique_edges (zeroed) += sum over the groups of g (g - 1) / 2
 cudaError_t launch_dedup_fill(const int32_t* uid_of, int64_t n, const uint32_t* group_start, uint32_t* group_count,
-                              int32_t* members, unsigned long long* clique_edges, cudaStream_t s, int* launches);
+                              int32_t* members, unsigned long long* clique_edges, uint32_t* max_group /*zeroed: largest
+                              group*/, cudaStream_t s, int* launches);
 // the edges among the rows of every shared sequence (distance 0); sequences uid = shard (mod n_shards) only
 cudaError_t launch_emit_cliques(const int32_t* members, const int32_t* uid_of, const uint32_t* group_start, int64_t n,
                                 unsigned long long* edges, unsigned long long* edge_count, unsigned long long edge_cap,
@@ -235,8 +236,9 @@ cudaError_t launch_expand_entries(const unsigned long long* entries, const unsig
                                   unsigned long long entry_cap, const uint32_t* group_start, const int32_t* members,
                                   unsigned long long* edges, unsigned long long* edge_total, unsigned long long edge_cap,
                                   int32_t* row_count, int32_t* deg, void* huge /*16 B x huge_cap: products set aside*/,
-                                  unsigned long long* n_huge /*zeroed*/, uint32_t huge_cap, int n_sm, cudaStream_t s,
-                                  int* launches);
+                                  unsigned long long* n_huge /*zeroed*/, uint32_t huge_cap,
+                                  bool huge_possible /*two groups may have more than 4096 pairs of rows between them*/,
+                                  int n_sm, cudaStream_t s, int* launches);
 // inv[row] = sorted position of the row's sequence, from the coded perm
 cudaError_t launch_inverse_perm_groups(const int32_t* perm, int64_t n_u, const uint32_t* group_start,
                                        const int32_t* members, int32_t* inv, cudaStream_t s, int* launches);
@@ -294,6 +296,10 @@ cudaError_t launch_csr_unsorted(const unsigned long long* keys, int64_t n_keys, 
                                 int64_t* row_ptr, unsigned long long* bucket, int32_t* col, int32_t* deg,
                                 int32_t* long_rows, uint32_t* n_long, void* scan_scratch, bool distinct_keys,
                                 cudaStream_t s, int* launches);
+// ... its last step, for the caller to launch when *n_long (rows of more than 256 neighbours, queued in long_rows) is
+// not zero: until then col holds no entries for those rows
+cudaError_t launch_sort_long_rows(int64_t n, const int64_t* row_ptr, const unsigned long long* bucket, int32_t* col,
+                                  const int32_t* long_rows, const uint32_t* n_long, cudaStream_t s, int* launches);
 // the same from keys that are already sorted (tcrnet_restrict)
 cudaError_t launch_csr(const unsigned long long* sorted_keys, int64_t n_edges, int64_t n, int64_t* row_ptr,
                        int32_t* col, int32_t* deg, cudaStream_t s, int* launches);
