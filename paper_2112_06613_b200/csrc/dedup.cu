@@ -135,7 +135,9 @@ __global__ void __launch_bounds__(256) k_dedup_groups(const int32_t* __restrict_
                                                      const int32_t* __restrict__ lengths, int64_t n,
                                                      int32_t* __restrict__ uid_of, uint32_t* __restrict__ group_count,
                                                      int32_t* __restrict__ len_u, int64_t* __restrict__ off_u,
-                                                     unsigned long long* __restrict__ hist_u) {
+                                                     unsigned long long* __restrict__ hist_u,
+                                                     unsigned long long* __restrict__ sort_key,
+                                                     int32_t* __restrict__ sort_val) {
     grid_dependency_wait();
     __shared__ uint32_t h[kNumLen];  // length histogram of the distinct sequences (their first rows)
     for (int k = threadIdx.x; k < kNumLen; k += blockDim.x) h[k] = 0;
@@ -150,7 +152,10 @@ __global__ void __launch_bounds__(256) k_dedup_groups(const int32_t* __restrict_
             const int32_t len = lengths[i];
             len_u[uid] = len;
             off_u[uid] = offsets[i];
-            atomicAdd(&h[(len < 1 || len > kMaxLen) ? 0 : len], 1u);
+            const int l = (len < 1 || len > kMaxLen) ? 0 : len;
+            atomicAdd(&h[l], 1u);
+            // (a load that is bucketed by length only: the key k_seq_keys would write, without its residue digits)
+            if (sort_key) sort_key[uid] = (unsigned long long)(uint32_t)(l > 0 ? l - 1 : 0) << (5 * kSortPrefix), sort_val[uid] = (int32_t)uid;
         }
     }
     __syncthreads();
@@ -420,10 +425,10 @@ cudaError_t launch_dedup_find(const uint8_t* residues, const int64_t* offsets, c
 
 cudaError_t launch_dedup_groups(const int32_t* rep_of, const uint32_t* first_rank, const int64_t* offsets,
                                 const int32_t* lengths, int64_t n, int32_t* uid_of, uint32_t* group_count,
-                                int32_t* len_u, int64_t* off_u, unsigned long long* hist_u, cudaStream_t s,
-                                int* launches) {
+                                int32_t* len_u, int64_t* off_u, unsigned long long* hist_u,
+                                unsigned long long* sort_key, int32_t* sort_val, cudaStream_t s, int* launches) {
     launch_dep(k_dedup_groups, grid_for(n), 256, 0, s, rep_of, first_rank, offsets, lengths, n, uid_of, group_count,
-               len_u, off_u, hist_u);
+               len_u, off_u, hist_u, sort_key, sort_val);
     *launches += 1;
     return cudaGetLastError();
 }

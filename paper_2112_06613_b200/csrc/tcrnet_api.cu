@@ -76,7 +76,7 @@ void drop_load(tcrnet_ctx* ctx) {
 // pre_hist != NULL: the (validated) length histogram of the rows is already on the host.
 int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* d_len, int64_t n, int64_t total_len,
              const int64_t* ext_offsets, const unsigned long long* pre_hist, bool code_groups, bool lexicographic,
-             int* launches) {
+             int* launches, bool keys_ready = false /*keys_a / perm_tmp hold the keys of the by-length sort*/) {
     set.loaded = false;
     set.grouped = false;
     set.n_rows = n;
@@ -155,7 +155,8 @@ int pack_set(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* 
         int32_t* va = (int32_t*)(n_passes & 1 ? ctx->perm_tmp.p : set.perm.p);
         int32_t* vb = (int32_t*)(n_passes & 1 ? set.perm.p : ctx->perm_tmp.p);
         if (e == cudaSuccess) e = radix_clear_totals(ctx->radix_scratch.p, s);
-        if (e == cudaSuccess)
+        if (keys_ready && (lexicographic || va != (int32_t*)ctx->perm_tmp.p)) e = cudaErrorUnknown;
+        if (e == cudaSuccess && !keys_ready)
             e = launch_seq_keys(d_res, d_off, d_len, n, (unsigned long long*)ctx->keys_a.p, va, s, launches);
         bool in_b = false;
         if (e == cudaSuccess)
@@ -257,7 +258,7 @@ void join_side_stream(tcrnet_ctx* ctx) {
 // Step A0 (dedup.cu): the distinct sequences of the rows.  On success *n_u of them, their lengths / residue
 // offsets in dd_len / dd_off, and in `set` the rows behind every distinct sequence.
 int dedup_rows(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t* d_len, int64_t n, int64_t total_len,
-               int64_t* n_u, int* launches) {
+               bool by_length_keys, int64_t* n_u, int* launches) {
     cudaStream_t s = ctx->stream;
     HostCtrl* dc = d_ctrl(ctx);
     const uint32_t slots = dedup_table_slots(n);
@@ -274,6 +275,10 @@ int dedup_rows(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t
     TRY(dev_reserve(ctx, set.uid_of, sizeof(int32_t) * (size_t)n));
     TRY(dev_reserve(ctx, set.group_start, sizeof(uint32_t) * (size_t)(n + 2)));
     TRY(dev_reserve(ctx, set.members, sizeof(int32_t) * (size_t)n));
+    if (by_length_keys) {  // the groups kernel writes the keys of the by-length sort of pack_set (no k_seq_keys launch)
+        TRY(dev_reserve(ctx, ctx->keys_a, sizeof(unsigned long long) * (size_t)n));
+        TRY(dev_reserve(ctx, ctx->perm_tmp, sizeof(int32_t) * (size_t)n));
+    }
     const int64_t* off = (const int64_t*)ctx->dd_offsets.p;
     uint32_t* rank = (uint32_t*)ctx->dd_rank.p;
     uint32_t* count = (uint32_t*)ctx->dd_count.p;
@@ -289,7 +294,9 @@ int dedup_rows(tcrnet_ctx* ctx, SeqSet& set, const uint8_t* d_res, const int32_t
                                dc->hist, &dc->flags, s, launches));
     TRY_CUDA(exclusive_scan_u32_total((const uint32_t*)ctx->dd_first.p, rank, n, ctx->scan_scratch.p, s, launches));
     TRY_CUDA(launch_dedup_groups((const int32_t*)ctx->dd_rep.p, rank, off, d_len, n, (int32_t*)set.uid_of.p, count,
-                                 (int32_t*)ctx->dd_len.p, (int64_t*)ctx->dd_off.p, dc->hist_u, s, launches));
+                                 (int32_t*)ctx->dd_len.p, (int64_t*)ctx->dd_off.p, dc->hist_u,
+                                 by_length_keys ? (unsigned long long*)ctx->keys_a.p : nullptr,
+                                 by_length_keys ? (int32_t*)ctx->perm_tmp.p : nullptr, s, launches));
     // (... and the groups kernel the length histogram of the distinct sequences: the pack needs no round trip of its own)
     TRY_CUDA(cudaMemcpyAsync(ctx->h_ctrl, dc, sizeof(HostCtrl), cudaMemcpyDeviceToHost, s));  // hist, hist_u, flags
     TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->n_distinct, rank + n, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
@@ -330,12 +337,13 @@ int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len
     const bool lex = rect || !ctx->early_exit || ctx->segment_join == 0;
     int64_t n_u = n;
     if (ctx->dedup && !rect && n >= 2) {
-        const int rc_dedup = dedup_rows(ctx, ctx->all, d_res, d_len, n, total_len, &n_u, launches);
+        const int rc_dedup = dedup_rows(ctx, ctx->all, d_res, d_len, n, total_len, /*by_length_keys=*/!lex, &n_u, launches);
         if (rc_dedup != TCRNET_OK || n_u >= n) join_side_stream(ctx);  // (nothing will wait for the member lists)
         TRY(rc_dedup);
         if (n_u < n) {
             const int rc_pack = pack_set(ctx, ctx->all, d_res, (const int32_t*)ctx->dd_len.p, n_u, -1,
-                                         (const int64_t*)ctx->dd_off.p, ctx->hist_u_host, true, lex, launches);
+                                         (const int64_t*)ctx->dd_off.p, ctx->hist_u_host, true, lex, launches,
+                                         /*keys_ready=*/!lex);
             join_side_stream(ctx);
             TRY(rc_pack);
             ctx->clique_edges = (int64_t)ctx->h_ctrl->clique_edges;  // (read back with the pack's flags)

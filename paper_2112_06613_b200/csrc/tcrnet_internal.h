@@ -221,7 +221,9 @@ cudaError_t launch_dedup_find(const uint8_t* residues, const int64_t* offsets, c
 cudaError_t launch_dedup_groups(const int32_t* rep_of, const uint32_t* first_rank, const int64_t* offsets,
                                 const int32_t* lengths, int64_t n, int32_t* uid_of, uint32_t* group_count,
                                 int32_t* len_u, int64_t* off_u, unsigned long long* hist_u /*[kNumLen], += lengths of
-                                the distinct sequences*/, cudaStream_t s, int* launches);
+                                the distinct sequences*/,
+                                unsigned long long* sort_key /*may be NULL: [uid] = key of the by-length sort*/,
+                                int32_t* sort_val /*[uid] = uid*/, cudaStream_t s, int* launches);
 // group_start = exclusive scan of group_count (n_u + 1 entries); group_count is consumed
 // *clique_edges (zeroed) += sum over the groups of g (g - 1) / 2
 cudaError_t launch_dedup_fill(const int32_t* uid_of, int64_t n, const uint32_t* group_start, uint32_t* group_count,
