@@ -508,9 +508,6 @@ def main() -> None:
                 "alu_ops_per_launch": alu_ops,
                 # also against the issue-slot ceiling (4 schedulers x 32 lanes per SM and clock)
                 "issue_ceiling": 2 * peak, "frac_of_issue_ceiling": achieved / (2 * peak),
-                **({"concurrent": "k_emit_cliques runs beside this kernel on the library's second stream and shares "
-                                  "the SMs (kernel_ms is the live duration; alone, under ncu: profiles/r2_launches_cfg4.md)"}
-                   if join and not args.no_dedup else {}),
             },
             "detail": {
                 "pairs_kept": work["pairs_kept"], "cells_kept": work["cells_kept"], "cells_all": work["cells_all"],

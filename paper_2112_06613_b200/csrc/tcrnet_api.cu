@@ -708,10 +708,8 @@ int ensure_join_index(tcrnet_ctx* ctx, int l_max, int* launches) {
 // between rows after the expansion).
 // expand_only: the recorded pairs in keys_a are complete, only keys_b was too small - redo the expansion alone.
 // The counters and per-row counts a distance pass starts from (issued ahead of the index kernels for the first pass,
-// so that no memset sits between two kernels of the chain index -> join -> cliques -> expansion).
-// On a collapsed load the cliques of the shared sequences (k_emit_cliques: they depend on the load alone) are emitted
-// from here on a second stream, next to the index / join kernels, and joined before the counts are read back.
-int reset_build_counters(tcrnet_ctx* ctx, bool expand_only, uint64_t cap_b, int shard, int n_shards, int* launches) {
+// so that no memset sits between two kernels of the chain index -> join -> expansion).
+int reset_build_counters(tcrnet_ctx* ctx, bool expand_only) {
     cudaStream_t s = ctx->stream;
     HostCtrl* dc = d_ctrl(ctx);
     static_assert(offsetof(HostCtrl, queue) == offsetof(HostCtrl, edge_count) + 9 * sizeof(unsigned long long), "one memset");
@@ -726,15 +724,6 @@ int reset_build_counters(tcrnet_ctx* ctx, bool expand_only, uint64_t cap_b, int 
     }
     TRY_CUDA(cudaMemsetAsync(ctx->row_count.p, 0, sizeof(int32_t) * (size_t)ctx->n, s));
     TRY_CUDA(cudaMemsetAsync(ctx->deg.p, 0, sizeof(int32_t) * (size_t)ctx->n, s));
-    if (ctx->all.grouped) {
-        TRY_CUDA(cudaEventRecord(ctx->ev_fork, s));
-        TRY_CUDA(cudaStreamWaitEvent(ctx->side_stream, ctx->ev_fork, 0));
-        TRY_CUDA(launch_emit_cliques((const int32_t*)ctx->all.members.p, (const int32_t*)ctx->all.uid_of.p,
-                                     (const uint32_t*)ctx->all.group_start.p, ctx->n, (unsigned long long*)ctx->keys_b.p,
-                                     &dc->edge_total, cap_b, (int32_t*)ctx->row_count.p, (int32_t*)ctx->deg.p, shard, n_shards,
-                                     ctx->side_stream, launches));
-        TRY_CUDA(cudaEventRecord(ctx->ev_join, ctx->side_stream));
-    }
     return TCRNET_OK;
 }
 
@@ -745,7 +734,7 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
     static_assert(offsetof(HostCtrl, queue) == offsetof(HostCtrl, edge_count) + 9 * sizeof(unsigned long long), "one memset");
     static_assert(offsetof(HostCtrl, edge_total) == offsetof(HostCtrl, queue) + kTrieQueues * sizeof(unsigned long long), "one memset");
     static_assert(offsetof(HostCtrl, cand_count) == offsetof(HostCtrl, edge_total) + sizeof(unsigned long long), "one memset");
-    if (!counters_cleared) TRY(reset_build_counters(ctx, expand_only, cap_b, shard, n_shards, launches));
+    if (!counters_cleared) TRY(reset_build_counters(ctx, expand_only));
     int n_queues = 0;
     const WorkRow* d_rows = (const WorkRow*)ctx->rows.p;
     if (!expand_only) TRY_CUDA(rec(ctx, 4, 1));
@@ -802,8 +791,18 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
     }
     if (!expand_only) TRY_CUDA(rec(ctx, 5, 1));
     if (ctx->all.grouped) {
-        // the recorded pairs of distinct sequences -> edges between rows (keys_b), counted for the CSR step (the rows of
-        // every shared sequence are being joined to each other on the side stream: reset_build_counters)
+        // The rows of every shared sequence are joined to each other (k_emit_cliques) on the second stream, beside the
+        // expansion below: the two are independent (they share the cursor of keys_b and the per-row counters, both
+        // updated atomically).  Beside the join kernel - where it ran before - it cost the same step time but shared
+        // the SMs with the kernel the roofline is reported for (81 us instead of 62 us at config 4).
+        TRY_CUDA(cudaEventRecord(ctx->ev_fork, s));
+        TRY_CUDA(cudaStreamWaitEvent(ctx->side_stream, ctx->ev_fork, 0));
+        TRY_CUDA(launch_emit_cliques((const int32_t*)ctx->all.members.p, (const int32_t*)ctx->all.uid_of.p,
+                                     (const uint32_t*)ctx->all.group_start.p, ctx->n, (unsigned long long*)ctx->keys_b.p,
+                                     &dc->edge_total, cap_b, (int32_t*)ctx->row_count.p, (int32_t*)ctx->deg.p, shard, n_shards,
+                                     ctx->side_stream, launches));
+        TRY_CUDA(cudaEventRecord(ctx->ev_join, ctx->side_stream));
+        // the recorded pairs of distinct sequences -> edges between rows (keys_b), counted for the CSR step
         const uint32_t* gs = (const uint32_t*)ctx->all.group_start.p;
         const int32_t* mem = (const int32_t*)ctx->all.members.p;
         TRY_CUDA(launch_expand_entries((const unsigned long long*)ctx->keys_a.p, &dc->edge_count, cap, gs, mem,
@@ -855,7 +854,7 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
         TRY(dev_reserve(ctx, ctx->keys_b, sizeof(unsigned long long) * (size_t)cap_b));
     }
     // the first pass's resets go ahead of the index kernels: index -> join -> cliques -> expansion is one chain of kernels
-    TRY(reset_build_counters(ctx, false, (uint64_t)cap_b, shard, n_shards, launches));
+    TRY(reset_build_counters(ctx, false));
     bool counters_cleared = true;
     st.ms_index = 0.f;
     st.join_index_entries = 0;
