@@ -51,9 +51,9 @@ ORACLE_SAMPLE_ROWS = 1024
 # summarised under profiles/ (regenerated with them; a workload / kernel that is not listed prints null)
 NCU_DRAM_BYTES_PER_LAUNCH = {
     # (workload, kernel): bytes per step of that kernel / kernel pair - profiles/r2_join_ncu.txt
-    ("cfg4", "k_join_probe"): 30_912_000 + 0,
-    ("cfg3", "k_join_probe + k_join_verify"): 9_014_016 + 512 + 11_573_504 + 0,
-    ("cfg5", "k_join_probe + k_join_verify"): 1_270_800_000 + 287_637_504 + 367_959_000 + 53_251_328,
+    ("cfg4", "k_join_probe"): 30_912_000 + 1_024,
+    ("cfg3", "k_join_probe + k_join_verify"): 9_014_016 + 0 + 11_577_088 + 0,
+    ("cfg5", "k_join_probe + k_join_verify"): 1_280_987_000 + 287_489_024 + 367_860_000 + 52_898_304,
 }
 
 
