@@ -80,10 +80,22 @@ __global__ void __launch_bounds__(256) k_count_rows(const unsigned long long* __
 // kernel ends it IS the exclusive prefix sum.  Consecutive keys often share their row (the products of two repeated
 // sequences are emitted together), so the lanes of a warp that hold the same row take their slots with ONE returning
 // atomic (match.any; the returning atomics are what bounds this kernel).
-__global__ void __launch_bounds__(256) k_scatter_keys(const unsigned long long* __restrict__ keys, int64_t n_keys,
+//
+// The number of keys is n_bound, or - a build that assembles before the host has read the edge count back - *n_dev,
+// of which at most n_bound fit the buffers: beyond that nothing is written (the host will find the count too large and
+// repeat the step with larger buffers).
+__device__ __forceinline__ int64_t key_count(const unsigned long long* n_dev, int64_t n_bound) {
+    if (!n_dev) return n_bound;
+    const unsigned long long v = *n_dev;
+    return v > (unsigned long long)n_bound ? -1 : (int64_t)v;  // (-1: the per-row counts describe more keys than fit)
+}
+
+__global__ void __launch_bounds__(256) k_scatter_keys(const unsigned long long* __restrict__ keys,
+                                                     const unsigned long long* __restrict__ n_dev, int64_t n_bound,
                                                      unsigned long long* __restrict__ row_ptr,
                                                      unsigned long long* __restrict__ bucket) {
     grid_dependency_wait();
+    const int64_t n_keys = key_count(n_dev, n_bound);
     const int lane = threadIdx.x & 31;
     const uint32_t lt_mask = (1u << lane) - 1u;
     for (int64_t e0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) & ~(int64_t)31; e0 < n_keys;
@@ -102,13 +114,10 @@ __global__ void __launch_bounds__(256) k_scatter_keys(const unsigned long long* 
 
 // TIES: the keys may repeat (a caller's list); the library's own edge lists hold every pair once.
 template <bool TIES>
-__global__ void __launch_bounds__(256) k_rank_rows(const unsigned long long* __restrict__ bucket, int64_t n_keys,
-                                                  const int64_t* __restrict__ row_ptr, int32_t* __restrict__ col,
-                                                  int32_t* __restrict__ deg, int32_t* __restrict__ long_rows,
-                                                  uint32_t* __restrict__ n_long, int rank_row) {
-    grid_dependency_wait();
-    const int64_t pos = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (pos >= n_keys) return;
+__device__ __forceinline__ void rank_slot(const unsigned long long* __restrict__ bucket, int64_t pos,
+                                          const int64_t* __restrict__ row_ptr, int32_t* __restrict__ col,
+                                          int32_t* __restrict__ deg, int32_t* __restrict__ long_rows,
+                                          uint32_t* __restrict__ n_long, int rank_row) {
     const unsigned long long k = bucket[pos];
     const uint32_t u = (uint32_t)(k >> 32), v = (uint32_t)k;
     const int64_t b = row_ptr[u];
@@ -128,6 +137,20 @@ __global__ void __launch_bounds__(256) k_rank_rows(const unsigned long long* __r
     }
     col[b + rank] = (int32_t)v;
 }
+
+template <bool TIES>
+__global__ void __launch_bounds__(256) k_rank_rows(const unsigned long long* __restrict__ bucket,
+                                                  const unsigned long long* __restrict__ n_dev, int64_t n_bound,
+                                                  const int64_t* __restrict__ row_ptr, int32_t* __restrict__ col,
+                                                  int32_t* __restrict__ deg, int32_t* __restrict__ long_rows,
+                                                  uint32_t* __restrict__ n_long, int rank_row) {
+    grid_dependency_wait();
+    const int64_t n_keys = key_count(n_dev, n_bound);
+    for (int64_t pos = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; pos < n_keys;
+         pos += (int64_t)gridDim.x * blockDim.x)
+        rank_slot<TIES>(bucket, pos, row_ptr, col, deg, long_rows, n_long, rank_row);
+}
+
 
 // Ascending bitonic network over the next power of two of len, the missing tail being virtual +infinity entries
 // (every exchange puts the smaller value at the smaller index, so they never move).  One CTA.  The partner of element
@@ -238,21 +261,24 @@ cudaError_t launch_count_rows(const unsigned long long* keys, int64_t n_keys, in
     return cudaGetLastError();
 }
 
-cudaError_t launch_csr_unsorted(const unsigned long long* keys, int64_t n_keys, int64_t n, int32_t* row_count,
-                                int64_t* row_ptr, unsigned long long* bucket, int32_t* col, int32_t* deg,
-                                int32_t* long_rows, uint32_t* n_long, void* scan_scratch, bool distinct_keys,
-                                cudaStream_t s, int* launches) {
+cudaError_t launch_csr_unsorted(const unsigned long long* keys, const unsigned long long* n_dev, int64_t n_bound,
+                                int64_t n, int32_t* row_count, int64_t* row_ptr, unsigned long long* bucket,
+                                int32_t* col, int32_t* deg, int32_t* long_rows, uint32_t* n_long, void* scan_scratch,
+                                bool distinct_keys, cudaStream_t s, int* launches) {
     cudaError_t e = cudaMemsetAsync(n_long, 0, sizeof(uint32_t), s);  // (ahead of the kernels: none sits between two)
     if (e == cudaSuccess) e = inclusive_scan_i32_to_i64(row_count, row_ptr, n, scan_scratch, s, launches);
-    if (e != cudaSuccess || n_keys <= 0) return e;
-    const int64_t blocks = (n_keys + 255) / 256;
-    launch_dep(k_scatter_keys, (unsigned)std::min<int64_t>(blocks, device_sm_count() * 32), 256, 0, s, keys, n_keys,
+    if (e != cudaSuccess || n_bound <= 0) return e;
+    // (grids: by the number of keys when the host knows it, else a fixed one - the kernels stride)
+    const int64_t blocks = (n_bound + 255) / 256;
+    const int64_t cap_blocks = (int64_t)device_sm_count() * (n_dev ? 16 : 32);
+    launch_dep(k_scatter_keys, (unsigned)std::min<int64_t>(blocks, cap_blocks), 256, 0, s, keys, n_dev, n_bound,
                (unsigned long long*)row_ptr, bucket);
     const int rank_row = kRankRow;
-    if (distinct_keys) launch_dep(k_rank_rows<false>, (unsigned)blocks, 256, 0, s, bucket, n_keys, row_ptr, col, deg,
+    const unsigned rank_blocks = (unsigned)(n_dev ? std::min<int64_t>(blocks, (int64_t)device_sm_count() * 64) : blocks);
+    if (distinct_keys) launch_dep(k_rank_rows<false>, rank_blocks, 256, 0, s, bucket, n_dev, n_bound, row_ptr, col, deg,
                                   long_rows, n_long, rank_row);
-    else launch_dep(k_rank_rows<true>, (unsigned)blocks, 256, 0, s, bucket, n_keys, row_ptr, col, deg, long_rows, n_long,
-                    rank_row);
+    else launch_dep(k_rank_rows<true>, rank_blocks, 256, 0, s, bucket, n_dev, n_bound, row_ptr, col, deg, long_rows,
+                    n_long, rank_row);
     *launches += 2;
     return cudaGetLastError();
 }

@@ -727,8 +727,15 @@ int reset_build_counters(tcrnet_ctx* ctx, bool expand_only) {
     return TCRNET_OK;
 }
 
+int assemble_reserve(tcrnet_ctx* ctx, int64_t bound);
+int assemble_launch(tcrnet_ctx* ctx, const unsigned long long* edges, unsigned long long* bucket,
+                    const unsigned long long* n_dev, int64_t bound, bool distinct_keys, int* launches);
+int assemble_finish(tcrnet_ctx* ctx, int64_t n_keys, const unsigned long long* bucket, int* launches);
+
+// assemble_too: step A6 is launched right behind the distance kernels, on the edge count as the device holds it, and
+// the ONE synchronisation at the end serves both (the host then finds out whether the buffers were large enough).
 int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_check, uint64_t cap, uint64_t cap_b, int shard,
-                 int n_shards, bool expand_only, bool counters_cleared, int* launches) {
+                 int n_shards, bool expand_only, bool counters_cleared, int* launches, bool assemble_too = false) {
     cudaStream_t s = ctx->stream;
     HostCtrl* dc = d_ctrl(ctx);
     static_assert(offsetof(HostCtrl, queue) == offsetof(HostCtrl, edge_count) + 9 * sizeof(unsigned long long), "one memset");
@@ -815,12 +822,20 @@ int run_distance(tcrnet_ctx* ctx, const Schedule& sch, int l_max, int first_chec
     TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->edge_count, &dc->edge_count, sizeof(unsigned long long) * 9,
                              cudaMemcpyDeviceToHost, s));
     TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->cand_count, &dc->cand_count, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
+    if (assemble_too) {
+        const bool grouped = ctx->all.grouped;  // (grouped: the edges are in keys_b and keys_a is free again)
+        TRY(assemble_launch(ctx, (const unsigned long long*)(grouped ? ctx->keys_b.p : ctx->keys_a.p),
+                            (unsigned long long*)(grouped ? ctx->keys_a.p : ctx->keys_b.p),
+                            grouped ? &dc->edge_total : &dc->edge_count, (int64_t)(grouped ? cap_b : cap), true, launches));
+    }
     TRY_CUDA(cudaStreamSynchronize(s));
     return TCRNET_OK;
 }
 
 // Steps A2-A5 for the work items of one shard: unsorted keys in keys_a, ctx->n_keys of them.
-int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* launches) {
+int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* launches, bool assemble_too = false) {
+    ctx->assembled = false;
+    assemble_too = assemble_too && ctx->timing < 2;  // (level 2 times the phases one after the other)
     tcrnet_stats& st = ctx->stats;
     const int64_t n = ctx->n;
     int first_check = 0;
@@ -853,6 +868,16 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
         cap_b = std::min(cap_b, ctx->edge_limit);
         TRY(dev_reserve(ctx, ctx->keys_b, sizeof(unsigned long long) * (size_t)cap_b));
     }
+    if (assemble_too) {
+        // every buffer of step A6 by its upper bound, before anything is launched; the scratch of the scatter is the
+        // other key buffer (grouped: keys_a, free once the expansion has read the recorded pairs)
+        if (grouped && cap_b > cap) {
+            cap = cap_b;
+            TRY(dev_reserve(ctx, ctx->keys_a, sizeof(unsigned long long) * (size_t)cap));
+        }
+        if (!grouped) TRY(dev_reserve(ctx, ctx->keys_b, sizeof(unsigned long long) * (size_t)cap));
+        TRY(assemble_reserve(ctx, grouped ? cap_b : cap));
+    }
     // the first pass's resets go ahead of the index kernels: index -> join -> cliques -> expansion is one chain of kernels
     TRY(reset_build_counters(ctx, false));
     bool counters_cleared = true;
@@ -882,8 +907,9 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
     st.distance_passes = 0;
     for (bool expand_only = false;;) {
         if (!expand_only) ++st.distance_passes;
+        const bool with_a6 = assemble_too && st.distance_passes == 1 && !expand_only;  // (the first pass only)
         TRY(run_distance(ctx, sch, l_max, first_check, (uint64_t)cap, (uint64_t)cap_b, shard, n_shards, expand_only,
-                         counters_cleared, launches));
+                         counters_cleared, launches, with_a6));
         counters_cleared = false;
         const int64_t n_rec = (int64_t)ctx->h_ctrl->edge_count;  // pairs recorded by the distance kernels
         const int64_t n_cand = (int64_t)ctx->h_ctrl->cand_count;
@@ -902,13 +928,17 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
             TRY(dev_reserve(ctx, ctx->keys_a, sizeof(unsigned long long) * (size_t)cap));
             continue;
         }
-        if (!grouped || n_keys <= cap_b) break;
+        if (!grouped || n_keys <= cap_b) {
+            ctx->assembled = with_a6;  // (every count fits: what step A6 was launched on is the whole edge list)
+            break;
+        }
         if (expand_only) return TCRNET_ERR_CUDA;  // cannot happen: exact size
         cap_b = n_keys;
         TRY(dev_reserve(ctx, ctx->keys_b, sizeof(unsigned long long) * (size_t)cap_b));
         expand_only = true;
     }
     if (grouped) std::swap(ctx->keys_a, ctx->keys_b);  // the edges between rows are what the CSR step takes
+    // (... and has taken already if it was launched with the first pass: its scratch is then in keys_b)
     st.ms_kernel = 0.f;
     // (of the last pass; both events complete: synchronised above)
     if (ctx->timing >= 1) TRY_CUDA(cudaEventElapsedTime(&st.ms_kernel, ctx->ev[4], ctx->ev[5]));
@@ -933,45 +963,46 @@ int distance_phase(tcrnet_ctx* ctx, int l_max, int shard, int n_shards, int* lau
     return TCRNET_OK;
 }
 
-// Step A6 on the n_keys unsorted keys (u << 32) | v in keys_a: per-row counts (left in row_count by the emission
-// when counts_ready), prefix sum -> row_ptr, every edge into a slot of its row, rows ordered; degrees.
-int assemble_phase(tcrnet_ctx* ctx, int64_t n_keys, bool counts_ready, int* launches) {
-    tcrnet_stats& st = ctx->stats;
-    cudaStream_t s = ctx->stream;
+// Buffers of step A6 for n rows and up to `bound` keys (no-ops when they are large enough).
+int assemble_reserve(tcrnet_ctx* ctx, int64_t bound) {
     const int64_t n = ctx->n;
-    HostCtrl* dc = d_ctrl(ctx);
     TRY(dev_reserve(ctx, ctx->row_count, sizeof(int32_t) * (size_t)n));
     TRY(dev_reserve(ctx, ctx->long_rows, sizeof(int32_t) * (size_t)n));
     TRY(dev_reserve(ctx, ctx->scan_scratch, scan_scratch_bytes(n)));
     TRY(dev_reserve(ctx, ctx->row_ptr, sizeof(int64_t) * (size_t)(n + 1)));
-    TRY(dev_reserve(ctx, ctx->col, sizeof(int32_t) * (size_t)std::max<int64_t>(n_keys, 1)));
+    TRY(dev_reserve(ctx, ctx->col, sizeof(int32_t) * (size_t)std::max<int64_t>(bound, 1)));
     TRY(dev_reserve(ctx, ctx->deg, sizeof(int32_t) * (size_t)n));
-    TRY(dev_reserve(ctx, ctx->keys_b, sizeof(unsigned long long) * (size_t)std::max<int64_t>(n_keys, 1)));
-    if (!counts_ready) {
-        TRY_CUDA(cudaMemsetAsync(ctx->row_count.p, 0, sizeof(int32_t) * (size_t)n, s));
-        TRY_CUDA(cudaMemsetAsync(ctx->deg.p, 0, sizeof(int32_t) * (size_t)n, s));
-        TRY_CUDA(launch_count_rows((const unsigned long long*)ctx->keys_a.p, n_keys, (int32_t*)ctx->row_count.p,
-                                   (int32_t*)ctx->deg.p, s, launches));
-    }
+    return TCRNET_OK;
+}
+
+// The kernels of step A6 on the keys in `edges` (their number: `bound`, or *n_dev with `bound` the capacity of edges,
+// bucket and col - launch_csr_unsorted), per-row counts in row_count / deg; the count of the long rows is on its way to
+// the host.  Nothing is synchronised.
+int assemble_launch(tcrnet_ctx* ctx, const unsigned long long* edges, unsigned long long* bucket,
+                    const unsigned long long* n_dev, int64_t bound, bool distinct_keys, int* launches) {
+    cudaStream_t s = ctx->stream;
+    HostCtrl* dc = d_ctrl(ctx);
     TRY_CUDA(rec(ctx, 2, 2));
-    TRY_CUDA(launch_csr_unsorted((const unsigned long long*)ctx->keys_a.p, n_keys, n, (int32_t*)ctx->row_count.p,
-                                 (int64_t*)ctx->row_ptr.p, (unsigned long long*)ctx->keys_b.p, (int32_t*)ctx->col.p,
-                                 (int32_t*)ctx->deg.p, (int32_t*)ctx->long_rows.p, &dc->n_long, ctx->scan_scratch.p,
-                                 /*distinct_keys=*/counts_ready, s, launches));
+    TRY_CUDA(launch_csr_unsorted(edges, n_dev, bound, ctx->n, (int32_t*)ctx->row_count.p, (int64_t*)ctx->row_ptr.p, bucket,
+                                 (int32_t*)ctx->col.p, (int32_t*)ctx->deg.p, (int32_t*)ctx->long_rows.p, &dc->n_long,
+                                 ctx->scan_scratch.p, distinct_keys, s, launches));
     TRY_CUDA(cudaMemcpyAsync(&ctx->h_ctrl->n_long, &dc->n_long, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
-    if (ctx->timing >= 2) {  // (the phase events bracket the whole step: no read-back in between)
-        if (n_keys > 0)
-            TRY_CUDA(launch_sort_long_rows(n, (const int64_t*)ctx->row_ptr.p, (const unsigned long long*)ctx->keys_b.p,
-                                           (int32_t*)ctx->col.p, (const int32_t*)ctx->long_rows.p, &dc->n_long, s, launches));
-        TRY_CUDA(rec(ctx, 3, 2));
-        TRY_CUDA(cudaStreamSynchronize(s));
-    } else {
-        TRY_CUDA(cudaStreamSynchronize(s));
-        if (n_keys > 0 && ctx->h_ctrl->n_long > 0) {  // rows of more than 256 neighbours: ordered by their own kernel
-            TRY_CUDA(launch_sort_long_rows(n, (const int64_t*)ctx->row_ptr.p, (const unsigned long long*)ctx->keys_b.p,
-                                           (int32_t*)ctx->col.p, (const int32_t*)ctx->long_rows.p, &dc->n_long, s, launches));
-            TRY_CUDA(cudaStreamSynchronize(s));
-        }
+    return TCRNET_OK;
+}
+
+int assemble_sort_long(tcrnet_ctx* ctx, const unsigned long long* bucket, int* launches) {
+    return launch_sort_long_rows(ctx->n, (const int64_t*)ctx->row_ptr.p, bucket, (int32_t*)ctx->col.p,
+                                 (const int32_t*)ctx->long_rows.p, &d_ctrl(ctx)->n_long, ctx->stream, launches) == cudaSuccess
+               ? TCRNET_OK : TCRNET_ERR_CUDA;
+}
+
+// ... once the stream has been synchronised behind assemble_launch: the rows of more than 256 neighbours (if any: they
+// are ordered by a kernel of their own), bookkeeping.
+int assemble_finish(tcrnet_ctx* ctx, int64_t n_keys, const unsigned long long* bucket, int* launches) {
+    tcrnet_stats& st = ctx->stats;
+    if (ctx->timing < 2 && n_keys > 0 && ctx->h_ctrl->n_long > 0) {
+        TRY(assemble_sort_long(ctx, bucket, launches));
+        TRY_CUDA(cudaStreamSynchronize(ctx->stream));
     }
     st.ms_sort = st.ms_csr = 0.f;
     if (ctx->timing >= 2) {
@@ -985,6 +1016,29 @@ int assemble_phase(tcrnet_ctx* ctx, int64_t n_keys, bool counts_ready, int* laun
     drop_observables(ctx);
     ctx->built = true;
     return TCRNET_OK;
+}
+
+// Step A6 on the n_keys unsorted keys (u << 32) | v in keys_a: per-row counts (left in row_count by the emission
+// when counts_ready), prefix sum -> row_ptr, every edge into a slot of its row, rows ordered; degrees.
+int assemble_phase(tcrnet_ctx* ctx, int64_t n_keys, bool counts_ready, int* launches) {
+    cudaStream_t s = ctx->stream;
+    const int64_t n = ctx->n;
+    TRY(assemble_reserve(ctx, n_keys));
+    TRY(dev_reserve(ctx, ctx->keys_b, sizeof(unsigned long long) * (size_t)std::max<int64_t>(n_keys, 1)));
+    if (!counts_ready) {
+        TRY_CUDA(cudaMemsetAsync(ctx->row_count.p, 0, sizeof(int32_t) * (size_t)n, s));
+        TRY_CUDA(cudaMemsetAsync(ctx->deg.p, 0, sizeof(int32_t) * (size_t)n, s));
+        TRY_CUDA(launch_count_rows((const unsigned long long*)ctx->keys_a.p, n_keys, (int32_t*)ctx->row_count.p,
+                                   (int32_t*)ctx->deg.p, s, launches));
+    }
+    unsigned long long* bucket = (unsigned long long*)ctx->keys_b.p;
+    TRY(assemble_launch(ctx, (const unsigned long long*)ctx->keys_a.p, bucket, nullptr, n_keys, counts_ready, launches));
+    if (ctx->timing >= 2) {  // (the phase events bracket the whole step: no read-back in between)
+        if (n_keys > 0) TRY(assemble_sort_long(ctx, bucket, launches));
+        TRY_CUDA(rec(ctx, 3, 2));
+    }
+    TRY_CUDA(cudaStreamSynchronize(s));
+    return assemble_finish(ctx, n_keys, bucket, launches);
 }
 
 // Distance labels of the current CSR's edges (labels.cu), computed on first use.
@@ -1214,8 +1268,9 @@ int tcrnet_build(tcrnet_ctx* ctx, int l_max, int64_t* n_edges_out) {
     TRY_CUDA(cudaSetDevice(ctx->device));
     drop_build(ctx);
     int launches = 0;
-    TRY(distance_phase(ctx, l_max, 0, 1, &launches));
-    TRY(assemble_phase(ctx, ctx->n_keys, true, &launches));
+    TRY(distance_phase(ctx, l_max, 0, 1, &launches, /*assemble_too=*/true));
+    if (ctx->assembled) TRY(assemble_finish(ctx, ctx->n_keys, (const unsigned long long*)ctx->keys_b.p, &launches));
+    else TRY(assemble_phase(ctx, ctx->n_keys, true, &launches));
     tcrnet_stats& st = ctx->stats;
     st.ms_distance = st.ms_build = 0.f;
     if (ctx->timing >= 2) {

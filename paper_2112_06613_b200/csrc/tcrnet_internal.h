@@ -293,11 +293,13 @@ cudaError_t launch_count_rows(const unsigned long long* keys, int64_t n_keys, in
 // CSR + degrees from UNSORTED keys whose counts are in row_count[u] (edges of row u; left as they are) and
 // deg[v] (edges whose larger endpoint is v).  bucket: uint64[n_keys] scratch, long_rows: int32[n] scratch,
 // n_long: device counter, scan_scratch: scan_scratch_bytes(n).  distinct_keys: no key occurs twice (the
-// library's own edge lists; a caller's list may repeat keys).
-cudaError_t launch_csr_unsorted(const unsigned long long* keys, int64_t n_keys, int64_t n, int32_t* row_count,
-                                int64_t* row_ptr, unsigned long long* bucket, int32_t* col, int32_t* deg,
-                                int32_t* long_rows, uint32_t* n_long, void* scan_scratch, bool distinct_keys,
-                                cudaStream_t s, int* launches);
+// library's own edge lists; a caller's list may repeat keys).  The number of keys is n_bound (n_dev = NULL) or
+// *n_dev (device; a build that assembles before the host has read the count back): if that exceeds n_bound - the
+// capacity of keys, bucket and col - nothing is written and the caller repeats the step with larger buffers.
+cudaError_t launch_csr_unsorted(const unsigned long long* keys, const unsigned long long* n_dev, int64_t n_bound,
+                                int64_t n, int32_t* row_count, int64_t* row_ptr, unsigned long long* bucket,
+                                int32_t* col, int32_t* deg, int32_t* long_rows, uint32_t* n_long, void* scan_scratch,
+                                bool distinct_keys, cudaStream_t s, int* launches);
 // ... its last step, for the caller to launch when *n_long (rows of more than 256 neighbours, queued in long_rows) is
 // not zero: until then col holds no entries for those rows
 cudaError_t launch_sort_long_rows(int64_t n, const int64_t* row_ptr, const unsigned long long* bucket, int32_t* col,
