@@ -51,6 +51,12 @@ def test_cfg1_full(pkg, oracle, l_max):
     assert_same_network(got, want)
     check_csr_invariants(*got, d.n)
     assert st["pairs_all"] == d.n * (d.n - 1) // 2 and st["launches_build"] > 0
+    # TCRNET_OPT_TIMING: 2 = an event around every phase (the build then runs its phases one after the other, each behind
+    # its own read-back), 0 = none; the default 1 launches step A6 behind the distance kernels on the device's edge count
+    for level in (2, 0):
+        got2, st2 = gpu_network(pkg, d.residues, d.lengths, l_max, {pkg.OPT_TIMING: level})
+        assert_same_network(got2, want)
+        assert (st2["ms_build"] > 0) == (level == 2) and (st2["ms_kernel"] > 0) == (level == 2)
 
 
 @pytest.mark.parametrize("l_max,tier", [(1, 1), (2, 0)])
