@@ -117,7 +117,11 @@ typedef enum tcrnet_option {
                                      behind it (reading Q3: one node per row, duplicates joined
                                      for every l_max >= 0).  0: every row is its own pattern /
                                      text.  Never changes the result.  Ignored (off) in the
-                                     rectangular mode.  Takes effect at the next load.          */
+                                     rectangular mode.  Takes effect at the next load.  A load that
+                                     finds no repeated sequence makes the next seven loads of the
+                                     context skip the attempt (tables of distinct clonotypes come in
+                                     series; tcrnet_stats.n_distinct then reads n); setting the option
+                                     again re-arms it.                                          */
     TCRNET_OPT_SEGMENT_JOIN = 11, /* exact candidate filter in front of the verification: a text cut into
                                      l_max + 1 segments shares at least one of them, unchanged and shifted by
                                      at most the edits allow, with every sequence within l_max of it; only
@@ -176,7 +180,7 @@ typedef struct tcrnet_stats {
     float ms_csr;              /* row_ptr / col / degrees [TIMING 2]                          */
     float ms_build;            /* whole tcrnet_build on the device [TIMING 2]                 */
     int64_t n_distinct;        /* distinct sequences among the rows (= n when TCRNET_OPT_DEDUP
-                                  is off or in the rectangular mode)                         */
+                                  is off or paused, or in the rectangular mode)              */
     float ms_kernel;           /* the distance kernel launches alone (events right around them: the join's
                                   probe + verify kernels, or the trie / text-chunk kernels) [TIMING 1]  */
     float ms_index;            /* segment join: building the segment index (inside ms_distance) [TIMING 2] */

@@ -336,7 +336,13 @@ int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len
     // the builds of this load (it walks a trie over the sorted texts); the segment join only needs the buckets.
     const bool lex = rect || !ctx->early_exit || ctx->segment_join == 0;
     int64_t n_u = n;
-    if (ctx->dedup && !rect && n >= 2) {
+    // A load that found no repeated sequence makes the next kDedupPause loads of the context skip the attempt (tables
+    // of distinct clonotypes come in series; the attempt costs 0.1 ms at N = 5e5 and finds nothing there).
+    constexpr int kDedupPause = 7;
+    const bool attempt = ctx->dedup && !rect && n >= 2 && ctx->dedup_pause == 0;
+    if (ctx->dedup_pause > 0) --ctx->dedup_pause;
+    bool rows_known = false;  // the collapse found nothing, but left the offsets, the histogram and the sort keys of the rows
+    if (attempt) {
         const int rc_dedup = dedup_rows(ctx, ctx->all, d_res, d_len, n, total_len, /*by_length_keys=*/!lex, &n_u, launches);
         if (rc_dedup != TCRNET_OK || n_u >= n) join_side_stream(ctx);  // (nothing will wait for the member lists)
         TRY(rc_dedup);
@@ -350,11 +356,20 @@ int load_from_device(tcrnet_ctx* ctx, const uint8_t* d_res, const int32_t* d_len
             ctx->max_group = ctx->h_ctrl->max_group;
             ctx->all.grouped = true;
             ctx->all.n_rows = n;
+        } else {
+            ctx->dedup_pause = kDedupPause;
+            rows_known = true;
         }
     }
     if (!ctx->all.loaded || !ctx->all.grouped) {
         n_u = n;
-        TRY(pack_set(ctx, ctx->all, d_res, d_len, n, total_len, nullptr, nullptr, false, lex, launches));
+        if (rows_known) {  // (uid = row: what dedup_rows computed per distinct sequence is per row)
+            for (int l = 0; l < kNumLen; ++l) ctx->hist_u_host[l] = ctx->h_ctrl->hist[l];
+            TRY(pack_set(ctx, ctx->all, d_res, d_len, n, total_len, (const int64_t*)ctx->dd_offsets.p, ctx->hist_u_host,
+                         false, lex, launches, /*keys_ready=*/!lex));
+        } else {
+            TRY(pack_set(ctx, ctx->all, d_res, d_len, n, total_len, nullptr, nullptr, false, lex, launches));
+        }
     }
     if (rect) TRY(pack_set(ctx, ctx->query, d_res, d_len, ctx->n_query, -1, nullptr, nullptr, false, lex, launches));
     if (!ctx->all.grouped)
@@ -1481,6 +1496,7 @@ int tcrnet_set_option(tcrnet_ctx* ctx, int option, int64_t value) {
         case TCRNET_OPT_DEDUP:
             if (value != 0 && value != 1) return TCRNET_ERR_ARG;
             ctx->dedup = (int)value;
+            ctx->dedup_pause = 0;
             return TCRNET_OK;
         case TCRNET_OPT_SEGMENT_JOIN:
             if (value < -1 || value > 1) return TCRNET_ERR_ARG;

@@ -104,6 +104,7 @@ struct tcrnet_ctx {
     // segment join (segjoin.cu): directory + entries of the current load for join_l_max, work rows
     DevBuf join_cnt, join_dir, join_entries, join_rows, join_cand, join_scan_scratch;
     int64_t join_cand_cap = 0;  // pairs the verification queue join_cand holds (uint2[cap] followed by uint8[cap])
+    int dedup_pause = 0;     // loads that will not try to collapse identical rows (the last attempt found none)
     bool assembled = false;  // distance_phase has run step A6 behind its first pass (tcrnet_build) and all counts fit
     int join_adapted = 0; // lengths whose segment cut was adapted to the residue statistics (make_join_tables)
     int join_l_max = -1;  // threshold the index in join_dir / join_entries was built for (-1: none)

@@ -612,6 +612,39 @@ def test_one_heavily_repeated_sequence_fails_fast(pkg):
         assert dg[:3000].tolist() == [3000] * 3000 and dg[3000] == 3000 and dg[3001] == 0
 
 
+def test_collapse_pauses_after_a_load_without_repeats(pkg, oracle):
+    """A load that finds no repeated sequence hands the offsets / histogram / sort keys it computed on to the pack, and
+    the next seven loads of the context do not try to collapse (TCRNET_OPT_DEDUP re-arms it).  None of it changes a
+    result: a series of loads with and without repeated rows on ONE context, each against the oracle."""
+    d = generate("cfg2", n=20000)
+    off = np.concatenate([[0], np.cumsum(d.lengths.astype(np.int64))])
+    first = {}
+    for i in range(d.n):
+        first.setdefault(d.residues[off[i]:off[i + 1]].tobytes(), i)
+    keep = np.array(sorted(first.values()))
+    assert keep.size < d.n
+    u_res = np.concatenate([d.residues[off[i]:off[i + 1]] for i in keep])
+    u_len = np.ascontiguousarray(d.lengths[keep])
+    want_u = {l_max: oracle.network(u_res, u_len, l_max, tier=1)[:3] for l_max in (1, 2)}
+    want_d = {l_max: oracle.network(d.residues, d.lengths, l_max, tier=1)[:3] for l_max in (1, 2)}
+    with pkg.TcrNet(0) as net:
+        seen = []
+        for k in range(11):
+            dup = k in (0, 3, 10)
+            if k == 10:
+                net.set_option(pkg.OPT_DEDUP, 1)  # re-armed
+            net.load(*((d.residues, d.lengths) if dup else (u_res, u_len)))
+            for l_max in (1, 2):
+                net.build(l_max)
+                assert_same_network(net.copy_csr(), (want_d if dup else want_u)[l_max])
+            seen.append(int(net.get_stats()["n_distinct"]))
+        n_d, n_u = d.n, int(keep.size)
+        # 0: collapsed; 1: attempt, nothing found; 2..8: paused (3: repeated rows go uncollapsed); 9: attempt again;
+        # 10: re-armed by the option, collapsed
+        assert seen[0] == n_u and seen[1] == n_u and seen[3] == n_d and seen[10] == n_u
+        assert all(x == n_u for k, x in enumerate(seen) if k not in (3,))
+
+
 def test_device_side_validation(pkg):
     import torch
     with pkg.TcrNet(0) as net:
