@@ -51,9 +51,9 @@ ORACLE_SAMPLE_ROWS = 1024
 # summarised under profiles/ (regenerated with them; a workload / kernel that is not listed prints null)
 NCU_DRAM_BYTES_PER_LAUNCH = {
     # (workload, kernel): bytes per step of that kernel / kernel pair - profiles/r2_join_ncu.txt
-    ("cfg4", "k_join_probe"): 30_912_000 + 1_024,
-    ("cfg3", "k_join_probe + k_join_verify"): 9_014_016 + 0 + 11_577_088 + 0,
-    ("cfg5", "k_join_probe + k_join_verify"): 1_280_987_000 + 287_489_024 + 367_860_000 + 52_898_304,
+    ("cfg4", "k_join_probe"): 30_912_000 + 5_376,
+    ("cfg3", "k_join_probe + k_join_verify"): 9_013_760 + 0 + 11_579_648 + 0,
+    ("cfg5", "k_join_probe + k_join_verify"): 1_270_189_000 + 288_741_376 + 368_049_000 + 52_908_544,
 }
 
 
@@ -596,6 +596,19 @@ def main() -> None:
                     "join_entries": int(w_c2["join_entries"]), "join_candidates": int(w_c2["join_candidates"]),
                     "join_adapted_lengths": int(w_c2["join_adapted_lengths"]),
                     "ms_distance_kernel": float(np.mean([s["ms_kernel"] for s in st_c2]))}
+                del data
+                # ... and the same repertoire as a table of DISTINCT sequences (the usual form of real data): nothing
+                # to collapse; after the first such load the library pauses the attempt (TCRNET_OPT_DEDUP)
+                off = np.concatenate([[0], np.cumsum(d.lengths.astype(np.int64))])
+                first = {}
+                for i in range(n):
+                    first.setdefault(d.residues[off[i]:off[i + 1]].tobytes(), i)
+                keep = np.fromiter(sorted(first.values()), dtype=np.int64)
+                u_res = np.concatenate([d.residues[off[i]:off[i + 1]] for i in keep])
+                data = (torch.from_numpy(u_res).cuda(), torch.from_numpy(np.ascontiguousarray(d.lengths[keep])).cuda())
+                ms_u, w_u, st_u = side({}, data)
+                extras["distinct_rows_input"] = {"n": int(keep.size), "ms_step": ms_u, "edges": int(st_u[-1]["n_edges"]),
+                                                 "pairs_per_s": keep.size * (keep.size - 1) / 2 / (ms_u * 1e-3)}
                 del data
             out["detail"].update(extras)
             probes = {}
