@@ -261,7 +261,9 @@ TCRNET_API int tcrnet_load_device(tcrnet_ctx* ctx, const uint8_t* residues_dev, 
  * exactly by a banded bit-parallel verification; otherwise every length-compatible pair goes through the
  * bit-parallel column recurrence with an exact early exit (TCRNET_OPT_SEGMENT_JOIN).  The result is the same on
  * every path.  l_max in 0..TCRNET_MAX_LEN.  May be called repeatedly on one load.
- * *n_edges_out (host, may be NULL) receives |E|.  Synchronises the stream.
+ * *n_edges_out (host, may be NULL) receives |E|.  Synchronises the stream (once: the CSR step is launched behind the
+ * distance kernels on the edge count as the device holds it, into buffers reserved for TCRNET_OPT_EDGE_CAPACITY edges -
+ * default max(2^20, 16 n): 28 bytes per edge of capacity; more edges than that: the buffers grow and the step repeats).
  * Errors: STATE (no load), LMAX, NOMEM, EDGE_OVERFLOW, CUDA.
  */
 TCRNET_API int tcrnet_build(tcrnet_ctx* ctx, int l_max, int64_t* n_edges_out);
